@@ -1,0 +1,197 @@
+/*
+ * hines.h -- C ABI of the B200-native batched Hines solver (libhines_b200.so).
+ *
+ * The operation: every implicit-Euler time step of a compartmental neuron simulation solves, for
+ * each cell, the symmetric strictly diagonally dominant system A x = b with
+ *     A[i,i] = d[i],   A[i,p[i]] = A[p[i],i] = u[i]   (i >= 1),   p[i] < i,  p[root] = -1
+ * (arXiv 1810.12742: PAPER.md:34-38 the discretisation, :44-50 the numbering and the statement of
+ * the algorithm's inputs d, u, b, p, :78-100 Listing 2).  The solve is one backward elimination
+ * from the leaves to the root and one forward substitution from the root to the leaves
+ * (PAPER.md:50), for many independent cells at once.  The work distribution is
+ * computed once at setup and reused every step.
+ *
+ * Conventions
+ *   - "HOST" / "DEVICE" says where a pointer must live.  Device pointers must be 16-byte aligned.
+ *   - Cells are concatenated; cell c owns compartments [cell_offsets[c], cell_offsets[c+1]).
+ *     parent[] holds CELL-LOCAL indices (so identical morphologies have identical parent arrays).
+ *   - The plan copies what it needs: parent / cell_offsets may be freed after hines_plan_create.
+ *   - d, u, b are never written.  x may be exactly b (in place) or must not overlap d, u, b.
+ *   - u[root] is never read in a way that can reach the result.
+ *   - hines_solve only enqueues work on `stream` and never synchronises; it returns launch
+ *     errors only.  One solve in flight per plan (the plan owns one workspace).
+ *   - No C++ exception crosses this boundary.  Every function returns a status; details of the
+ *     last failure on the calling thread are available from hines_last_error().
+ *   - There is no CPU fallback: without a CUDA device the solve entry points return
+ *     HINES_ERR_CUDA.  (hines_plan_create itself is host-only work and succeeds without a
+ *     device, so the scheduler tables can be inspected anywhere; device tables are uploaded by
+ *     the first solve or by hines_plan_upload.)
+ */
+#ifndef HINES_B200_H
+#define HINES_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hines_plan hines_plan_t;          /* opaque, owned by the library            */
+typedef struct CUstream_st* hines_stream_t;      /* == cudaStream_t; NULL = default stream  */
+
+typedef enum {
+    HINES_OK = 0,
+    HINES_ERR_INVALID_ARG = 1,     /* null pointer, bad size, misaligned device pointer, bad option      */
+    HINES_ERR_BAD_TOPOLOGY = 2,    /* parent / cell_offsets do not describe a forest of rooted trees      */
+    HINES_ERR_ALLOC = 3,           /* host or device allocation failed                                    */
+    HINES_ERR_CUDA = 4,            /* no device, or a CUDA call / kernel launch failed                    */
+    HINES_ERR_UNSUPPORTED = 5      /* valid request this build cannot serve                               */
+} hines_status_t;
+
+typedef enum { HINES_F64 = 0, HINES_F32 = 1 } hines_dtype_t;
+
+/* policy_flags */
+enum {
+    HINES_POLICY_DEFAULT      = 0,
+    HINES_POLICY_FORCE_STREAM = 1,   /* every cell through the streaming (global-memory) path           */
+    HINES_POLICY_NO_GROUPING  = 2,   /* one cell per shared-memory work item (paper: >= 1 cell per block) */
+    HINES_POLICY_INPUT_ORDER  = 4    /* launch work items in input order, not heaviest first (PAPER.md:128
+                                        "greedy": cells are taken in the order given)                     */
+};
+
+typedef struct {
+    int32_t struct_size;            /* = sizeof(hines_options_t); lets the struct grow                     */
+    int32_t threads_per_block;      /* 0 = default (256); multiple of 32, <= 1024                          */
+    int32_t smem_bytes_per_block;   /* 0 = default (227 KiB: sm_100 opt-in maximum); upper bound for the
+                                       shared memory one resident work item may use                       */
+    int32_t policy_flags;           /* HINES_POLICY_*                                                      */
+    int32_t stream_threads;         /* 0 = default (128): block size of the streaming-path kernels         */
+    int32_t group_smem_bytes;       /* 0 = default (56 KiB): small cells are grouped into work items up to
+                                       this much shared memory ("fit as many matrices into one
+                                       block as possible")                                                 */
+} hines_options_t;
+
+typedef struct {
+    int64_t n;                  /* unknowns of the whole batch                                             */
+    int64_t ncells;
+    int64_t nbranches;          /* under the canonical branch rule (reading S4)                  */
+    int32_t max_levels;         /* deepest dependency tree in the batch                                    */
+    int32_t dtype;              /* hines_dtype_t                                                           */
+    int64_t n_resident_items;   /* shared-memory work items (cell groups)                                  */
+    int64_t n_resident_cells;
+    int64_t n_resident_unknowns;
+    int64_t n_stream_cells;     /* cells too large for shared memory -> streaming path                     */
+    int64_t n_stream_unknowns;
+    int64_t n_stream_branches;
+    int64_t padded_lane_steps;  /* sum over 32-lane tiles of (longest branch in the tile * 32)             */
+    int64_t useful_lane_steps;  /* = n minus nothing: sum of branch lengths; ratio = lane efficiency       */
+    int64_t workspace_bytes;    /* device memory the plan owns (tables + streaming workspace)              */
+    int64_t bytes_min;          /* n*4*w + 4*nbranches: d,u,b read, x written, one parent per branch
+                                   (PAPER.md:138); the roofline numerator                                  */
+    int64_t bytes_literal;      /* n*(4*w + 4): one parent per compartment (Listing 2 as printed)          */
+    int32_t breadth_first;      /* 1 if every cell's branches are numbered level by level    */
+    int32_t n_classes;          /* shared-memory size classes in use                                       */
+} hines_plan_info_t;
+
+/* Canonical, policy-free tables (bit-exact against the table oracle); all indices cell-local.
+ * Branch ids are in order of start compartment (readings S4, S5, S7). */
+typedef enum {
+    HINES_TABLE_CELL_BRANCH_OFFSETS  = 0,   /* int64[ncells+1]                                              */
+    HINES_TABLE_BRANCH_START         = 1,   /* int32[nbranches]  first compartment  */
+    HINES_TABLE_BRANCH_LEN           = 2,   /* int32[nbranches]  compartments in the branch  */
+    HINES_TABLE_BRANCH_PARENT_COMP   = 3,   /* int32[nbranches]  p[start], -1 for the root branch (:138)    */
+    HINES_TABLE_BRANCH_PARENT_BRANCH = 4,   /* int32[nbranches]  -1 for the root branch                     */
+    HINES_TABLE_BRANCH_LEVEL         = 5,   /* int32[nbranches]  depth from the root branch  */
+    HINES_TABLE_CELL_NLEVELS         = 6,   /* int32[ncells]                                                */
+    HINES_TABLE_CELL_LEVEL_OFFSETS   = 7,   /* int64[ncells+1]   into LEVEL_COUNT                           */
+    HINES_TABLE_LEVEL_COUNT          = 8,   /* int32[sum nlevels] branches per (cell, level) */
+    HINES_TABLE_LEVEL_LIST           = 9,   /* int32[nbranches]  per cell: ids by (level, length desc, id)  */
+    HINES_TABLE_CHILD_OFFSETS        = 10,  /* int64[nbranches+1] CSR over global branch index              */
+    HINES_TABLE_CHILD_IDS            = 11,  /* int32[nbranches-ncells] ascending                            */
+    /* Policy tables (depend on options; validity-checked in tests) */
+    HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  resident work item of the cell, -1 = streaming path     */
+    HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
+    HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  shared-memory size class                                */
+    HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
+    HINES_TABLE_ITEM_DESC_OFFSETS    = 36,  /* int64[nitems+1] into ITEM_DESC (in units of descriptors)               */
+    HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
+    HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] descriptor index (item-local) where each
+                                               level's lane list begins                                               */
+    HINES_TABLE_ITEM_DESC            = 39,  /* int32[3*ndesc] {start (item-local compartment), len, parent compartment
+                                               (item-local, -1 = root branch)}; len = 0 marks a padding lane           */
+    HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
+    HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment
+                                               (-1 root), workspace start, child_begin, nchild}                       */
+    HINES_TABLE_STREAM_CHILD         = 42,  /* int32[2*nstream_children] {global start, workspace start} of each child */
+    HINES_TABLE_CLASS_SMEM_BYTES     = 43   /* int32[n_classes] dynamic shared memory per block of each class          */
+} hines_table_id_t;
+
+/*
+ * Setup ("only once during the setup phase"): validates the topology, finds the
+ * branches and the branch dependency tree, the per-level branch lists (:110, :128),
+ * packs cells into work items (:128), sorts each level's branches by length and assigns them to
+ * lanes (:130), and lays out the per-item tables.  HOST pointers; O(N) time and memory.
+ *   parent        HOST int32[N], N = cell_offsets[ncells]; cell-local; parent[first of cell] = -1,
+ *                 0 <= parent[i] < i otherwise.  Any such array is accepted; breadth-first branch
+ *                 numbering is what makes branches long and is reported in info.
+ *   cell_offsets  HOST int64[ncells+1]; [0] == 0, strictly increasing (no empty cell); N < 2^31.
+ *   opt           NULL = defaults.
+ * Errors: INVALID_ARG (null, ncells <= 0, bad dtype/options, N >= 2^31), BAD_TOPOLOGY (offsets
+ * not increasing, parent out of range; hines_last_error names the first offending index), ALLOC.
+ */
+hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offsets, int64_t ncells,
+                                 hines_dtype_t dtype, const hines_options_t* opt,
+                                 hines_plan_t** out_plan);
+
+/* Upload the plan's tables to the current CUDA device and allocate its workspace (done implicitly by
+ * the first solve).  Synchronous.  Errors: CUDA (no device / API failure), ALLOC. */
+hines_status_t hines_plan_upload(hines_plan_t* plan);
+
+/*
+ * The per-step call ("solved in every time step"): x = A^-1 b for every cell.
+ *   d, u, b   DEVICE, N elements of the plan's dtype, natural (input) order, 16-byte aligned, read only.
+ *   x         DEVICE, N elements; may be == b.
+ * Steps run, all inside the library's kernels: load / permute-in,
+ * backward elimination level by level, branch-end hand-off (:50),
+ * root solve (:91), forward substitution (:97), store / permute-out (:173).
+ */
+hines_status_t hines_solve(hines_plan_t* plan, const void* d, const void* u, const void* b, void* x,
+                           hines_stream_t stream);
+
+/*
+ * Same solve with HOST buffers (pageable or pinned): copies d, u, b to plan-owned device buffers,
+ * solves, copies x back and synchronises `stream`.  This is the end-to-end entry that bench.py times
+ * as "e2e".  Bytes moved: 3*N*w host->device, N*w device->host.
+ */
+hines_status_t hines_solve_host(hines_plan_t* plan, const void* d, const void* u, const void* b, void* x,
+                                hines_stream_t stream);
+
+hines_status_t hines_plan_destroy(hines_plan_t* plan);
+
+/* Introspection: needed for the bit-exact table parity tests and for reporting. */
+hines_status_t hines_plan_get_info(const hines_plan_t* plan, hines_plan_info_t* out);
+
+/* Copies table `table_id` to host_dst if capacity_bytes suffices; always writes the size needed to
+ * *needed_bytes (host_dst may be NULL to query).  Errors: INVALID_ARG (unknown id, null needed_bytes,
+ * capacity too small). */
+hines_status_t hines_plan_get_table(const hines_plan_t* plan, int32_t table_id, void* host_dst,
+                                    int64_t capacity_bytes, int64_t* needed_bytes);
+
+/* Device-side timing of the two paths, for the roofline report.  With timing enabled every
+ * hines_solve records three CUDA events on its stream (before the shared-memory kernels, between the
+ * two paths, after the streaming kernels).  hines_plan_get_timing waits for the last solve and returns
+ * the milliseconds the resident (shared-memory) launches and the streaming launches took.
+ * Errors: INVALID_ARG (null, timing not enabled, no solve yet), CUDA. */
+hines_status_t hines_plan_enable_timing(hines_plan_t* plan, int32_t enable);
+hines_status_t hines_plan_get_timing(hines_plan_t* plan, float* resident_ms, float* stream_ms);
+
+/* Number of kernel launches one hines_solve enqueues with this plan (bench.py's gpu_launches). */
+hines_status_t hines_plan_launches_per_solve(const hines_plan_t* plan, int32_t* out);
+
+const char* hines_status_string(hines_status_t s);
+const char* hines_last_error(void);      /* thread-local, never NULL */
+const char* hines_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HINES_B200_H */

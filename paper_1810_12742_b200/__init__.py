@@ -1,0 +1,197 @@
+"""paper_1810_12742_b200 -- thin Python binding of libhines_b200.so (include/hines.h).
+
+Argument marshalling only: every step of the solve runs in the library's CUDA kernels.
+PyTorch is used by callers for device memory and streams; this module passes raw pointers.
+There is no CPU fallback: if the extension is missing or there is no GPU, calls fail loudly.
+
+Names mirror the C ABI: hines_plan_create -> Plan(...), hines_solve -> Plan.solve,
+hines_solve_host -> Plan.solve_host, hines_plan_get_info -> Plan.info,
+hines_plan_get_table -> Plan.table, hines_plan_destroy -> Plan.close.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from ._build import LIB as _LIB_PATH, build as build_library
+
+F64, F32 = 0, 1
+POLICY_DEFAULT, POLICY_FORCE_STREAM, POLICY_NO_GROUPING, POLICY_INPUT_ORDER = 0, 1, 2, 4
+
+STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",
+          4: "HINES_ERR_CUDA", 5: "HINES_ERR_UNSUPPORTED"}
+
+# table id -> (name, numpy dtype)
+TABLES = {
+    "cell_branch_offsets": (0, np.int64), "branch_start": (1, np.int32), "branch_len": (2, np.int32),
+    "branch_parent_comp": (3, np.int32), "branch_parent_branch": (4, np.int32), "branch_level": (5, np.int32),
+    "cell_nlevels": (6, np.int32), "cell_level_offsets": (7, np.int64), "level_count": (8, np.int32),
+    "level_list": (9, np.int32), "child_offsets": (10, np.int64), "child_ids": (11, np.int32),
+    "cell_item": (32, np.int32), "item_cell_range": (33, np.int64), "item_class": (34, np.int32),
+    "item_launch_order": (35, np.int32), "item_desc_offsets": (36, np.int64),
+    "item_level_offsets": (37, np.int64), "item_level_begin": (38, np.int32), "item_desc": (39, np.int32),
+    "stream_level_begin": (40, np.int64), "stream_desc": (41, np.int32), "stream_child": (42, np.int32),
+    "class_smem_bytes": (43, np.int32),
+}
+
+# every symbol include/hines.h declares
+ABI_SYMBOLS = ["hines_plan_create", "hines_plan_upload", "hines_solve", "hines_solve_host",
+               "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
+               "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
+               "hines_status_string", "hines_last_error", "hines_version"]
+
+
+class Options(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("threads_per_block", C.c_int32),
+                ("smem_bytes_per_block", C.c_int32), ("policy_flags", C.c_int32),
+                ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32)]
+
+
+class PlanInfo(C.Structure):
+    _fields_ = [("n", C.c_int64), ("ncells", C.c_int64), ("nbranches", C.c_int64),
+                ("max_levels", C.c_int32), ("dtype", C.c_int32),
+                ("n_resident_items", C.c_int64), ("n_resident_cells", C.c_int64),
+                ("n_resident_unknowns", C.c_int64), ("n_stream_cells", C.c_int64),
+                ("n_stream_unknowns", C.c_int64), ("n_stream_branches", C.c_int64),
+                ("padded_lane_steps", C.c_int64), ("useful_lane_steps", C.c_int64),
+                ("workspace_bytes", C.c_int64), ("bytes_min", C.c_int64), ("bytes_literal", C.c_int64),
+                ("breadth_first", C.c_int32), ("n_classes", C.c_int32)]
+
+
+class HinesError(RuntimeError):
+    def __init__(self, status, detail):
+        super().__init__(f"{STATUS.get(status, status)}: {detail}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libhines_b200.so (built in-tree).  Raises if it cannot be found or built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        if not build_if_missing:
+            raise ImportError(f"{_LIB_PATH} missing: run `python -c 'import __graft_entry__ as g; g.build()'`")
+        build_library()
+    lib = C.CDLL(_LIB_PATH)
+    vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
+    lib.hines_plan_create.argtypes = [vp, vp, i64, i32, C.POINTER(Options), C.POINTER(vp)]
+    lib.hines_plan_upload.argtypes = [vp]
+    lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hines_plan_destroy.argtypes = [vp]
+    lib.hines_plan_get_info.argtypes = [vp, C.POINTER(PlanInfo)]
+    lib.hines_plan_get_table.argtypes = [vp, i32, vp, i64, C.POINTER(i64)]
+    lib.hines_plan_launches_per_solve.argtypes = [vp, C.POINTER(i32)]
+    lib.hines_plan_enable_timing.argtypes = [vp, i32]
+    lib.hines_plan_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    for f in ("hines_status_string", "hines_last_error", "hines_version"):
+        getattr(lib, f).restype = C.c_char_p
+    lib.hines_status_string.argtypes = [i32]
+    _lib = lib
+    return lib
+
+
+def _check(status):
+    if status != 0:
+        raise HinesError(status, load_library().hines_last_error().decode())
+
+
+def _ptr(t):
+    """Raw address of a torch tensor / numpy array / int."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    assert t.is_contiguous()
+    return t.data_ptr()
+
+
+class Plan:
+    """hines_plan_create(parent arrays, cell offsets) -- setup-time scheduler."""
+
+    def __init__(self, parent, cell_offsets, dtype=F64, threads_per_block=0, smem_bytes_per_block=0,
+                 policy_flags=0, stream_threads=0, group_smem_bytes=0):
+        lib = load_library()
+        parent = np.ascontiguousarray(parent, dtype=np.int32)
+        offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
+        opt = Options(C.sizeof(Options), threads_per_block, smem_bytes_per_block, policy_flags,
+                      stream_threads, group_smem_bytes)
+        h = C.c_void_p()
+        self._h = None
+        _check(lib.hines_plan_create(parent.ctypes.data, offs.ctypes.data, len(offs) - 1, int(dtype),
+                                     C.byref(opt), C.byref(h)))
+        self._h = h
+        self.dtype = int(dtype)
+        self.np_dtype = np.float64 if self.dtype == F64 else np.float32
+
+    # hines_plan_get_info
+    @property
+    def info(self) -> PlanInfo:
+        out = PlanInfo()
+        _check(load_library().hines_plan_get_info(self._h, C.byref(out)))
+        return out
+
+    # hines_plan_get_table
+    def table(self, name: str) -> np.ndarray:
+        tid, dt = TABLES[name]
+        need = C.c_int64()
+        _check(load_library().hines_plan_get_table(self._h, tid, None, 0, C.byref(need)))
+        out = np.empty(need.value // np.dtype(dt).itemsize, dtype=dt)
+        _check(load_library().hines_plan_get_table(self._h, tid, out.ctypes.data, need.value, C.byref(need)))
+        return out
+
+    @property
+    def launches_per_solve(self) -> int:
+        out = C.c_int32()
+        _check(load_library().hines_plan_launches_per_solve(self._h, C.byref(out)))
+        return out.value
+
+    # hines_plan_enable_timing / hines_plan_get_timing
+    def enable_timing(self, enable=True):
+        _check(load_library().hines_plan_enable_timing(self._h, int(bool(enable))))
+
+    def timing(self):
+        """(resident_ms, stream_ms) of the last solve; waits for it."""
+        a, b = C.c_float(), C.c_float()
+        _check(load_library().hines_plan_get_timing(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
+    def upload(self):
+        _check(load_library().hines_plan_upload(self._h))
+
+    # hines_solve: device pointers (torch CUDA tensors or raw addresses); enqueues on `stream`
+    def solve(self, d, u, b, x, stream=None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        _check(load_library().hines_solve(self._h, _ptr(d), _ptr(u), _ptr(b), _ptr(x), stream))
+        return x
+
+    # hines_solve_host: host buffers (numpy arrays or pinned torch CPU tensors); synchronous
+    def solve_host(self, d, u, b, x, stream=None):
+        _check(load_library().hines_solve_host(self._h, _ptr(d), _ptr(u), _ptr(b), _ptr(x), stream or 0))
+        return x
+
+    def close(self):
+        if self._h is not None:
+            load_library().hines_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def version() -> str:
+    return load_library().hines_version().decode()

@@ -1,0 +1,531 @@
+// hines_plan_create: the setup-time scheduler (host only, O(N)).
+//
+// What it builds, with the passage of arXiv 1810.12742 each table comes from:
+//   T1-T4  branches, their parent compartment / parent branch and level: the branch dependency
+//          tree ("form a dependency tree. Each node in this tree represents a
+//          submatrix"; :138 "it is sufficient to store only one parent compartment for each branch").
+//   T5-T6  per-level branch counts and per-level lists sorted by size.
+//   T7     child lists (the edges of the dependency tree, used by the streaming path's pull hand-off).
+//   P1-P2  cells -> work items: greedy in input order while the item fits the block's shared memory
+//          ("we assign matrices to a Cuda block as long as ... When a matrix doesn't fit
+//          into a Cuda block any longer, we start a new Cuda block"); the fit test here is bytes of
+//          shared memory instead of "branches per level <= threads", because a B200 block loops over
+//          a level's lane list and is limited by its 227 KB of shared memory, not its thread count.
+//          Cells that do not fit any block go to the streaming path (the paper has no such path:
+//          PAPER.md:114 requires one matrix per block).
+//   P3     per (item, level): lane list.  Sibling branches (same parent compartment) are kept in one
+//          32-lane tile so the hand-off at the branch point is a warp shuffle; sibling
+//          groups are sorted by their longest member, descending (Fig 4.1).
+// Written policy: DESIGN.md "Scheduler policy".
+#include <algorithm>
+#include <cstring>
+#include <new>
+#include <numeric>
+#include <string>
+
+#include "plan_internal.h"
+
+namespace hines {
+
+static thread_local std::string g_last_error;
+void set_error(const std::string& msg) { g_last_error = msg; }
+
+static const int64_t kSmemPerSM = 233472;       // 228 KiB
+static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
+static const int32_t kAtomicFlag = 1 << 30;     // descriptor len bit: sibling group spans tiles
+static const int kClassK[] = {1, 2, 3, 4, 6, 8};
+static const int kNumClassK = 6;
+
+static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
+
+static int64_t class_cap(int k, int64_t max_smem)
+{
+    int64_t cap = (kSmemPerSM / k - 1024) / 128 * 128;
+    return std::min(cap, max_smem);
+}
+
+struct Entry { int32_t start, len, pc, ord; int64_t key; };
+
+// Lane lists of one work item (cells [c0,c1)), policy P3.  Returns the shared-memory need in bytes.
+struct ItemBuild {
+    int64_t comp_begin = 0, n = 0;
+    int32_t nlev = 0;
+    std::vector<int32_t> level_begin;   // nlev+1
+    std::vector<int32_t> desc;          // 3 per descriptor
+    int64_t padded_steps = 0;
+    int64_t smem_need = 0;
+};
+
+static void build_item(const hines_plan& P, int64_t c0, int64_t c1, ItemBuild& out)
+{
+    out.comp_begin = P.cell_offsets[c0];
+    out.n = P.cell_offsets[c1] - out.comp_begin;
+    out.nlev = 0;
+    for (int64_t c = c0; c < c1; ++c) out.nlev = std::max(out.nlev, P.cell_nlevels[c]);
+    std::vector<std::vector<Entry>> lv(out.nlev);
+    int32_t ord = 0;
+    for (int64_t c = c0; c < c1; ++c) {
+        const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
+        const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
+        for (int64_t j = b0; j < b1; ++j, ++ord) {
+            Entry e;
+            e.start = P.branch_start[j] + shift;
+            e.len = P.branch_len[j];
+            e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
+            e.ord = ord;                                    // (cell, branch id) order
+            e.key = e.pc >= 0 ? (int64_t)e.pc : -(int64_t)ord - 1;   // roots are singletons
+            lv[P.branch_level[j]].push_back(e);
+        }
+    }
+    out.level_begin.assign(out.nlev + 1, 0);
+    out.desc.clear();
+    out.padded_steps = 0;
+    struct Group { int32_t first, count, maxlen, minord; };
+    std::vector<Group> groups;
+    for (int32_t l = 0; l < out.nlev; ++l) {
+        auto& v = lv[l];
+        // siblings contiguous; inside a group: length descending, then (cell, id)
+        std::sort(v.begin(), v.end(), [](const Entry& a, const Entry& b) {
+            if (a.key != b.key) return a.key < b.key;
+            if (a.len != b.len) return a.len > b.len;
+            return a.ord < b.ord;
+        });
+        groups.clear();
+        for (int32_t i = 0; i < (int32_t)v.size();) {
+            int32_t j = i, mo = v[i].ord;
+            while (j < (int32_t)v.size() && v[j].key == v[i].key) { mo = std::min(mo, v[j].ord); ++j; }
+            groups.push_back({i, j - i, v[i].len, mo});
+            i = j;
+        }
+        // groups by longest member descending, ties by first (cell, id)
+        std::sort(groups.begin(), groups.end(), [](const Group& a, const Group& b) {
+            if (a.maxlen != b.maxlen) return a.maxlen > b.maxlen;
+            return a.minord < b.minord;
+        });
+        out.level_begin[l] = (int32_t)(out.desc.size() / 3);
+        int32_t pos = 0;
+        for (const Group& g : groups) {
+            const bool spans = g.count > 32;
+            if (!spans && (pos % 32) + g.count > 32) {          // keep the sibling group in one tile
+                while (pos % 32) { out.desc.insert(out.desc.end(), {0, 0, -1}); ++pos; }
+            }
+            for (int32_t i = 0; i < g.count; ++i) {
+                const Entry& e = v[g.first + i];
+                out.desc.push_back(e.start);
+                out.desc.push_back(spans ? (e.len | kAtomicFlag) : e.len);
+                out.desc.push_back(e.pc);
+                ++pos;
+            }
+        }
+        // lane-step accounting: 32 lanes x longest branch of each tile
+        const int32_t lb = out.level_begin[l], le = (int32_t)(out.desc.size() / 3);
+        for (int32_t t = lb; t < le; t += 32) {
+            int32_t mx = 0;
+            for (int32_t i = t; i < std::min(le, t + 32); ++i) mx = std::max(mx, out.desc[3 * i + 1] & ~kAtomicFlag);
+            out.padded_steps += 32 * (int64_t)mx;
+        }
+    }
+    out.level_begin[out.nlev] = (int32_t)(out.desc.size() / 3);
+    const int E = 16 / P.width;
+    const int64_t L = round_up(out.comp_begin % E + out.n, E);
+    const int64_t meta = round_up(out.nlev + 1, 4) + round_up((int64_t)out.desc.size(), 4);
+    out.smem_need = 16 + 3 * L * P.width + meta * 4;
+}
+
+static hines_status_t canonical_tables(hines_plan& P, const int32_t* parent)
+{
+    const int64_t nc = P.ncells;
+    P.cell_branch_offsets.assign(nc + 1, 0);
+    P.cell_level_offsets.assign(nc + 1, 0);
+    P.cell_nlevels.assign(nc, 0);
+    std::vector<int32_t> nchild, branch_of, lens;
+    std::vector<int32_t> order;
+    P.max_levels = 0;
+    P.breadth_first = 1;
+    for (int64_t c = 0; c < nc; ++c) {
+        const int64_t o = P.cell_offsets[c];
+        const int32_t n = (int32_t)(P.cell_offsets[c + 1] - o);
+        const int32_t* p = parent + o;
+        if (p[0] != -1) {
+            set_error("cell " + std::to_string(c) + ": parent of the first compartment is " +
+                      std::to_string(p[0]) + ", expected -1 (global index " + std::to_string(o) + ")");
+            return HINES_ERR_BAD_TOPOLOGY;
+        }
+        nchild.assign(n, 0);
+        for (int32_t i = 1; i < n; ++i) {
+            if (p[i] < 0 || p[i] >= i) {
+                set_error("cell " + std::to_string(c) + ": parent[" + std::to_string(i) + "] = " +
+                          std::to_string(p[i]) + " not in [0, " + std::to_string(i) + ") (global index " +
+                          std::to_string(o + i) + ")");
+                return HINES_ERR_BAD_TOPOLOGY;
+            }
+            nchild[p[i]]++;
+        }
+        // T1 (reading S4): a compartment continues its parent's branch only if it is the parent's
+        // only child and is numbered right after it.
+        branch_of.resize(n);
+        const int64_t b0 = (int64_t)P.branch_start.size();
+        for (int32_t i = 0; i < n; ++i) {
+            const bool continues = i > 0 && p[i] == i - 1 && nchild[i - 1] == 1;
+            if (!continues) { P.branch_start.push_back(i); P.branch_len.push_back(0); }
+            branch_of[i] = (int32_t)(P.branch_start.size() - b0) - 1;
+            P.branch_len.back()++;
+        }
+        const int32_t nbc = (int32_t)(P.branch_start.size() - b0);
+        // T2-T4
+        int32_t deepest = 0;
+        for (int32_t j = 0; j < nbc; ++j) {
+            const int32_t s = P.branch_start[b0 + j];
+            int32_t pc = -1, pb = -1, lev = 0;
+            if (s > 0) { pc = p[s]; pb = branch_of[pc]; lev = P.branch_level[b0 + pb] + 1; }
+            P.branch_parent_comp.push_back(pc);
+            P.branch_parent_branch.push_back(pb);
+            if (j > 0 && lev < P.branch_level.back()) P.breadth_first = 0;
+            P.branch_level.push_back(lev);
+            deepest = std::max(deepest, lev);
+        }
+        // T5
+        const int32_t nlev = deepest + 1;
+        P.cell_nlevels[c] = nlev;
+        P.max_levels = std::max(P.max_levels, nlev);
+        const int64_t l0 = (int64_t)P.level_count.size();
+        P.level_count.resize(l0 + nlev, 0);
+        for (int32_t j = 0; j < nbc; ++j) P.level_count[l0 + P.branch_level[b0 + j]]++;
+        P.cell_level_offsets[c + 1] = l0 + nlev;
+        // T6 (reading S7): level ascending, length descending, id ascending
+        order.resize(nbc);
+        std::iota(order.begin(), order.end(), 0);
+        const int32_t* lev = P.branch_level.data() + b0;
+        const int32_t* len = P.branch_len.data() + b0;
+        std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) {
+            if (lev[a] != lev[b]) return lev[a] < lev[b];
+            return len[a] > len[b];
+        });
+        P.level_list.insert(P.level_list.end(), order.begin(), order.end());
+        P.cell_branch_offsets[c + 1] = b0 + nbc;
+    }
+    P.nbranches = (int64_t)P.branch_start.size();
+    // T7
+    P.child_offsets.assign(P.nbranches + 1, 0);
+    P.child_ids.assign(P.nbranches - nc, 0);
+    for (int64_t c = 0; c < nc; ++c) {
+        const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
+        for (int64_t j = b0 + 1; j < b1; ++j) P.child_offsets[b0 + P.branch_parent_branch[j] + 1]++;
+    }
+    for (int64_t j = 0; j < P.nbranches; ++j) P.child_offsets[j + 1] += P.child_offsets[j];
+    {
+        std::vector<int64_t> fill(P.child_offsets.begin(), P.child_offsets.end() - 1);
+        for (int64_t c = 0; c < nc; ++c) {
+            const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
+            for (int64_t j = b0 + 1; j < b1; ++j)
+                P.child_ids[fill[b0 + P.branch_parent_branch[j]]++] = (int32_t)(j - b0);
+        }
+    }
+    return HINES_OK;
+}
+
+static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib)
+{
+    const int32_t item = (int32_t)P.item_class.size();
+    for (int64_t c = c0; c < c1; ++c) P.cell_item[c] = item;
+    P.item_cell_range.push_back(c0);
+    P.item_cell_range.push_back(c1);
+    P.item_class.push_back(0);                     // filled by assign_classes
+    P.item_level_begin.insert(P.item_level_begin.end(), ib.level_begin.begin(), ib.level_begin.end());
+    P.item_level_offsets.push_back((int64_t)P.item_level_begin.size());
+    P.item_desc.insert(P.item_desc.end(), ib.desc.begin(), ib.desc.end());
+    P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 3);
+    // device blob: [level_begin | pad4 | desc | pad4]
+    hines::ItemHeader h;
+    h.comp_begin = ib.comp_begin;
+    h.n = (int32_t)ib.n;
+    h.nlev = ib.nlev;
+    h.meta_off = (int64_t)P.item_meta.size();
+    P.item_meta.insert(P.item_meta.end(), ib.level_begin.begin(), ib.level_begin.end());
+    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
+    h.desc_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    P.item_meta.insert(P.item_meta.end(), ib.desc.begin(), ib.desc.end());
+    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
+    h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    P.item_headers.push_back(h);
+    P.padded_lane_steps += ib.padded_steps;
+    P.n_resident_cells += c1 - c0;
+    P.n_resident_unknowns += ib.n;
+    // remember the need in item_class temporarily through a side vector
+}
+
+static void pack_items(hines_plan& P, std::vector<int64_t>& item_need, std::vector<char>& is_stream)
+{
+    const int64_t nc = P.ncells;
+    const int64_t max_smem = P.opt.smem_bytes_per_block;
+    const int64_t group_cap = std::min<int64_t>(P.opt.group_smem_bytes, max_smem);
+    const bool force_stream = P.opt.policy_flags & HINES_POLICY_FORCE_STREAM;
+    const bool no_group = P.opt.policy_flags & HINES_POLICY_NO_GROUPING;
+    P.cell_item.assign(nc, -1);
+    P.item_level_offsets.assign(1, 0);
+    P.item_desc_offsets.assign(1, 0);
+    is_stream.assign(nc, 0);
+    ItemBuild cur, cand;
+    int64_t g0 = -1;                                   // first cell of the open group
+    auto flush = [&](int64_t c_end) {
+        if (g0 >= 0) { emit_item(P, g0, c_end, cur); item_need.push_back(cur.smem_need); g0 = -1; }
+    };
+    for (int64_t c = 0; c < nc; ++c) {
+        const int64_t ncomp = P.cell_offsets[c + 1] - P.cell_offsets[c];
+        // quick reject before building lists: the three arrays alone
+        bool fits_alone = !force_stream && 16 + 3 * ncomp * P.width <= max_smem;
+        ItemBuild alone;
+        if (fits_alone) { build_item(P, c, c + 1, alone); fits_alone = alone.smem_need <= max_smem; }
+        if (!fits_alone) { flush(c); is_stream[c] = 1; continue; }
+        if (no_group || alone.smem_need > group_cap) {            // its own item
+            flush(c);
+            emit_item(P, c, c + 1, alone); item_need.push_back(alone.smem_need);
+            continue;
+        }
+        if (g0 < 0) { g0 = c; cur = std::move(alone); continue; }
+        build_item(P, g0, c + 1, cand);                           // greedy: does the next cell still fit?
+        if (cand.smem_need <= group_cap) { std::swap(cur, cand); continue; }
+        flush(c);
+        g0 = c; cur = std::move(alone);
+    }
+    flush(nc);
+}
+
+static void assign_classes(hines_plan& P, const std::vector<int64_t>& item_need)
+{
+    const int64_t nitems = (int64_t)item_need.size();
+    const int64_t max_smem = P.opt.smem_bytes_per_block;
+    std::vector<int> item_k(nitems, 1);
+    int64_t need_max[kNumClassK] = {0};
+    int64_t count[kNumClassK] = {0};
+    for (int64_t i = 0; i < nitems; ++i) {
+        int best = 0;
+        for (int q = 0; q < kNumClassK; ++q)
+            if (item_need[i] <= class_cap(kClassK[q], max_smem)) best = q;
+        item_k[i] = best;
+        need_max[best] = std::max(need_max[best], item_need[i]);
+        count[best]++;
+    }
+    // classes in launch order: biggest blocks first
+    int cls_of_q[kNumClassK];
+    for (int q = 0; q < kNumClassK; ++q) {
+        cls_of_q[q] = -1;
+        if (!count[q]) continue;
+        cls_of_q[q] = (int)P.class_smem_bytes.size();
+        P.class_smem_bytes.push_back((int32_t)round_up(need_max[q], 128));
+        P.class_blocks_per_sm.push_back(kClassK[q]);
+    }
+    for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[item_k[i]];
+    const int ncls = (int)P.class_smem_bytes.size();
+    P.class_first.assign(ncls, 0);
+    P.class_count.assign(ncls, 0);
+    P.item_launch_order.resize(nitems);
+    std::iota(P.item_launch_order.begin(), P.item_launch_order.end(), 0);
+    const bool input_order = P.opt.policy_flags & HINES_POLICY_INPUT_ORDER;
+    std::stable_sort(P.item_launch_order.begin(), P.item_launch_order.end(), [&](int32_t a, int32_t b) {
+        if (P.item_class[a] != P.item_class[b]) return P.item_class[a] < P.item_class[b];
+        if (input_order) return false;
+        return P.item_headers[a].n > P.item_headers[b].n;          // heaviest first
+    });
+    for (int64_t i = 0; i < nitems; ++i) P.class_count[P.item_class[P.item_launch_order[i]]]++;
+    for (int q = 1; q < ncls; ++q) P.class_first[q] = P.class_first[q - 1] + P.class_count[q - 1];
+}
+
+static void build_stream(hines_plan& P, const std::vector<char>& is_stream)
+{
+    // workspace offsets of the streaming cells, in input order
+    std::vector<int64_t> ws_off(P.ncells, -1);
+    int64_t ws = 0; int32_t maxlev = 0;
+    for (int64_t c = 0; c < P.ncells; ++c) {
+        if (!is_stream[c]) continue;
+        ws_off[c] = ws; ws += P.cell_offsets[c + 1] - P.cell_offsets[c];
+        maxlev = std::max(maxlev, P.cell_nlevels[c]);
+        P.n_stream_cells++;
+    }
+    P.n_stream_unknowns = ws;
+    if (!P.n_stream_cells) { P.stream_level_begin.assign(1, 0); return; }
+    struct SE { int64_t gbranch; int32_t len; };
+    std::vector<std::vector<SE>> lv(maxlev);
+    for (int64_t c = 0; c < P.ncells; ++c) {
+        if (!is_stream[c]) continue;
+        for (int64_t j = P.cell_branch_offsets[c]; j < P.cell_branch_offsets[c + 1]; ++j)
+            lv[P.branch_level[j]].push_back({j, P.branch_len[j]});
+    }
+    // cell of a global branch id: walk cells alongside (branches are in cell order)
+    std::vector<int32_t> cell_of_branch;   // only needed for stream branches; build lazily via search
+    auto cell_of = [&](int64_t gb) {
+        return (int64_t)(std::upper_bound(P.cell_branch_offsets.begin(), P.cell_branch_offsets.end(), gb) -
+                         P.cell_branch_offsets.begin()) - 1;
+    };
+    P.stream_level_begin.assign(maxlev + 1, 0);
+    for (int32_t l = 0; l < maxlev; ++l) {
+        auto& v = lv[l];
+        // whole-level order (reading S7 applied across the streaming cells): length descending, then id
+        std::stable_sort(v.begin(), v.end(), [](const SE& a, const SE& b) { return a.len > b.len; });
+        P.stream_level_begin[l] = (int64_t)P.stream_desc.size();
+        for (size_t t = 0; t < v.size(); t += 32) P.padded_lane_steps += 32 * (int64_t)v[t].len;
+        for (const SE& e : v) {
+            const int64_t c = cell_of(e.gbranch);
+            const int64_t o = P.cell_offsets[c], b0 = P.cell_branch_offsets[c];
+            hines::StreamDesc s;
+            s.gstart = (int32_t)(o + P.branch_start[e.gbranch]);
+            s.len = e.len;
+            s.gparent = P.branch_parent_comp[e.gbranch] < 0 ? -1 : (int32_t)(o + P.branch_parent_comp[e.gbranch]);
+            s.ws = (int32_t)(ws_off[c] + P.branch_start[e.gbranch]);
+            s.child_begin = (int32_t)(P.stream_child.size() / 2);
+            s.nchild = (int32_t)(P.child_offsets[e.gbranch + 1] - P.child_offsets[e.gbranch]);
+            for (int64_t k = P.child_offsets[e.gbranch]; k < P.child_offsets[e.gbranch + 1]; ++k) {
+                const int64_t ch = b0 + P.child_ids[k];
+                P.stream_child.push_back((int32_t)(o + P.branch_start[ch]));
+                P.stream_child.push_back((int32_t)(ws_off[c] + P.branch_start[ch]));
+            }
+            P.stream_desc.push_back(s);
+        }
+    }
+    P.stream_level_begin[maxlev] = (int64_t)P.stream_desc.size();
+}
+
+}  // namespace hines
+
+using namespace hines;
+
+extern "C" {
+
+hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offsets, int64_t ncells,
+                                 hines_dtype_t dtype, const hines_options_t* opt, hines_plan_t** out_plan)
+{
+    if (out_plan) *out_plan = nullptr;
+    if (!parent || !cell_offsets || !out_plan) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    if (ncells <= 0) { set_error("ncells must be positive"); return HINES_ERR_INVALID_ARG; }
+    if (dtype != HINES_F64 && dtype != HINES_F32) { set_error("unknown dtype"); return HINES_ERR_INVALID_ARG; }
+    hines_options_t o{};
+    o.struct_size = (int32_t)sizeof(hines_options_t);
+    if (opt) {
+        if (opt->struct_size <= 0 || opt->struct_size > (int32_t)sizeof(hines_options_t)) {
+            set_error("options: bad struct_size"); return HINES_ERR_INVALID_ARG;
+        }
+        std::memcpy(&o, opt, (size_t)opt->struct_size);
+    }
+    if (o.threads_per_block == 0) o.threads_per_block = 256;
+    if (o.smem_bytes_per_block == 0) o.smem_bytes_per_block = (int32_t)kSmemMaxOptin;
+    if (o.stream_threads == 0) o.stream_threads = 128;
+    if (o.group_smem_bytes == 0) o.group_smem_bytes = 57344;
+    if (o.threads_per_block < 32 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
+        o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
+        o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
+        (o.policy_flags & ~7)) {
+        set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
+    }
+    if (cell_offsets[0] != 0) { set_error("cell_offsets[0] must be 0"); return HINES_ERR_BAD_TOPOLOGY; }
+    for (int64_t c = 0; c < ncells; ++c)
+        if (cell_offsets[c + 1] <= cell_offsets[c]) {
+            set_error("cell_offsets not strictly increasing at cell " + std::to_string(c) + " (empty cells are rejected)");
+            return HINES_ERR_BAD_TOPOLOGY;
+        }
+    if (cell_offsets[ncells] >= (int64_t)1 << 31) { set_error("N >= 2^31 is not supported"); return HINES_ERR_INVALID_ARG; }
+    try {
+        hines_plan* P = new hines_plan();
+        P->n = cell_offsets[ncells]; P->ncells = ncells; P->dtype = dtype; P->width = dtype == HINES_F64 ? 8 : 4;
+        P->opt = o;
+        P->cell_offsets.assign(cell_offsets, cell_offsets + ncells + 1);
+        hines_status_t st = canonical_tables(*P, parent);
+        if (st != HINES_OK) { delete P; return st; }
+        std::vector<int64_t> item_need;
+        std::vector<char> is_stream;
+        pack_items(*P, item_need, is_stream);
+        assign_classes(*P, item_need);
+        build_stream(*P, is_stream);
+        *out_plan = P;
+        return HINES_OK;
+    } catch (const std::bad_alloc&) {
+        set_error("host allocation failed while building the plan"); return HINES_ERR_ALLOC;
+    } catch (const std::exception& e) {
+        set_error(std::string("internal error: ") + e.what()); return HINES_ERR_ALLOC;
+    }
+}
+
+hines_status_t hines_plan_get_info(const hines_plan_t* P, hines_plan_info_t* out)
+{
+    if (!P || !out) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    std::memset(out, 0, sizeof(*out));
+    out->n = P->n; out->ncells = P->ncells; out->nbranches = P->nbranches;
+    out->max_levels = P->max_levels; out->dtype = P->dtype;
+    out->n_resident_items = (int64_t)P->item_class.size();
+    out->n_resident_cells = P->n_resident_cells; out->n_resident_unknowns = P->n_resident_unknowns;
+    out->n_stream_cells = P->n_stream_cells; out->n_stream_unknowns = P->n_stream_unknowns;
+    out->n_stream_branches = (int64_t)P->stream_desc.size();
+    out->padded_lane_steps = P->padded_lane_steps; out->useful_lane_steps = P->n;
+    out->workspace_bytes = (int64_t)(P->item_meta.size() * 4 + P->item_headers.size() * sizeof(ItemHeader) +
+                                     P->item_launch_order.size() * 4 + P->stream_desc.size() * sizeof(StreamDesc) +
+                                     P->stream_child.size() * 4 + 2 * P->n_stream_unknowns * P->width);
+    out->bytes_min = P->n * 4 * P->width + 4 * P->nbranches;
+    out->bytes_literal = P->n * (4 * P->width + 4);
+    out->breadth_first = P->breadth_first;
+    out->n_classes = (int32_t)P->class_smem_bytes.size();
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst, int64_t cap, int64_t* needed)
+{
+    if (!P || !needed) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    const void* src = nullptr; int64_t bytes = 0;
+#define TBL(ID, V) case ID: src = (V).data(); bytes = (int64_t)((V).size() * sizeof((V)[0])); break;
+    switch (id) {
+        TBL(HINES_TABLE_CELL_BRANCH_OFFSETS, P->cell_branch_offsets)
+        TBL(HINES_TABLE_BRANCH_START, P->branch_start)
+        TBL(HINES_TABLE_BRANCH_LEN, P->branch_len)
+        TBL(HINES_TABLE_BRANCH_PARENT_COMP, P->branch_parent_comp)
+        TBL(HINES_TABLE_BRANCH_PARENT_BRANCH, P->branch_parent_branch)
+        TBL(HINES_TABLE_BRANCH_LEVEL, P->branch_level)
+        TBL(HINES_TABLE_CELL_NLEVELS, P->cell_nlevels)
+        TBL(HINES_TABLE_CELL_LEVEL_OFFSETS, P->cell_level_offsets)
+        TBL(HINES_TABLE_LEVEL_COUNT, P->level_count)
+        TBL(HINES_TABLE_LEVEL_LIST, P->level_list)
+        TBL(HINES_TABLE_CHILD_OFFSETS, P->child_offsets)
+        TBL(HINES_TABLE_CHILD_IDS, P->child_ids)
+        TBL(HINES_TABLE_CELL_ITEM, P->cell_item)
+        TBL(HINES_TABLE_ITEM_CELL_RANGE, P->item_cell_range)
+        TBL(HINES_TABLE_ITEM_CLASS, P->item_class)
+        TBL(HINES_TABLE_ITEM_LAUNCH_ORDER, P->item_launch_order)
+        TBL(HINES_TABLE_ITEM_DESC_OFFSETS, P->item_desc_offsets)
+        TBL(HINES_TABLE_ITEM_LEVEL_OFFSETS, P->item_level_offsets)
+        TBL(HINES_TABLE_ITEM_LEVEL_BEGIN, P->item_level_begin)
+        TBL(HINES_TABLE_ITEM_DESC, P->item_desc)
+        TBL(HINES_TABLE_STREAM_LEVEL_BEGIN, P->stream_level_begin)
+        TBL(HINES_TABLE_STREAM_DESC, P->stream_desc)
+        TBL(HINES_TABLE_STREAM_CHILD, P->stream_child)
+        TBL(HINES_TABLE_CLASS_SMEM_BYTES, P->class_smem_bytes)
+        default: set_error("unknown table id " + std::to_string(id)); return HINES_ERR_INVALID_ARG;
+    }
+#undef TBL
+    *needed = bytes;
+    if (!dst) return HINES_OK;
+    if (cap < bytes) { set_error("table buffer too small"); return HINES_ERR_INVALID_ARG; }
+    if (bytes) std::memcpy(dst, src, (size_t)bytes);
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_launches_per_solve(const hines_plan_t* P, int32_t* out)
+{
+    if (!P || !out) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    *out = (int32_t)P->class_smem_bytes.size() + 2 * (int32_t)(P->stream_level_begin.size() - 1);
+    return HINES_OK;
+}
+
+const char* hines_status_string(hines_status_t s)
+{
+    switch (s) {
+        case HINES_OK: return "ok";
+        case HINES_ERR_INVALID_ARG: return "invalid argument";
+        case HINES_ERR_BAD_TOPOLOGY: return "bad topology";
+        case HINES_ERR_ALLOC: return "allocation failed";
+        case HINES_ERR_CUDA: return "CUDA error";
+        case HINES_ERR_UNSUPPORTED: return "unsupported";
+    }
+    return "unknown status";
+}
+
+const char* hines_last_error(void) { return g_last_error.c_str(); }
+const char* hines_version(void) { return "hines-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

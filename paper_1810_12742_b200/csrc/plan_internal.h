@@ -1,0 +1,67 @@
+// Internal layout of hines_plan (library-private; the public surface is include/hines.h).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "hines.h"
+
+namespace hines {
+
+// One shared-memory work item = a contiguous run of cells (cells are packed into a
+// block in the order given).  32 bytes, read by one thread per block.
+struct ItemHeader {
+    int64_t comp_begin;   // global index of the item's first compartment
+    int32_t n;            // unknowns in the item
+    int32_t nlev;         // levels of the deepest cell in the item
+    int64_t meta_off;     // offset (int32 units, multiple of 4) of the item's metadata blob
+    int32_t meta_len;     // int32 count (multiple of 4): [level_begin (nlev+1) | pad | desc 3*ndesc | pad]
+    int32_t desc_off;     // offset (int32 units, multiple of 4) of the descriptors inside the blob
+};
+
+// Streaming-path branch descriptor (24 bytes).
+struct StreamDesc {
+    int32_t gstart;       // global compartment index of the branch's first compartment
+    int32_t len;
+    int32_t gparent;      // global index of the parent compartment, -1 for a root branch
+    int32_t ws;           // workspace index of the branch's first compartment
+    int32_t child_begin;  // into stream_child
+    int32_t nchild;
+};
+
+struct DeviceTables;      // solve.cu
+
+void set_error(const std::string& msg);
+
+}  // namespace hines
+
+struct hines_plan {
+    int64_t n = 0, ncells = 0, nbranches = 0;
+    int32_t dtype = 0, width = 8;
+    hines_options_t opt{};
+    int32_t max_levels = 0;
+    int32_t breadth_first = 1;
+
+    std::vector<int64_t> cell_offsets;
+    // canonical tables T1-T7
+    std::vector<int64_t> cell_branch_offsets, cell_level_offsets, child_offsets;
+    std::vector<int32_t> branch_start, branch_len, branch_parent_comp, branch_parent_branch,
+        branch_level, cell_nlevels, level_count, level_list, child_ids;
+    // policy tables
+    std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc;
+    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets;
+    std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
+    std::vector<int32_t> class_blocks_per_sm;
+    std::vector<int64_t> class_first, class_count;     // ranges in item_launch_order
+    std::vector<hines::ItemHeader> item_headers;       // indexed by item id
+    std::vector<int32_t> item_meta;                    // device blob
+    // streaming path
+    std::vector<int64_t> stream_level_begin;           // [nstream_levels+1]
+    std::vector<hines::StreamDesc> stream_desc;
+    std::vector<int32_t> stream_child;                 // pairs {gstart, ws}
+    int64_t n_stream_cells = 0, n_stream_unknowns = 0;
+    int64_t n_resident_cells = 0, n_resident_unknowns = 0;
+    int64_t padded_lane_steps = 0;
+
+    hines::DeviceTables* dev = nullptr;                // null until uploaded
+};

@@ -1,0 +1,489 @@
+// hines_solve: the per-step kernels (sm_100a) and their host launcher.
+//
+// Two paths, chosen per cell by the plan:
+//   resident  whole cells / cell groups staged into shared memory by TMA bulk copies
+//             (cp.async.bulk + mbarrier), level-synchronous sweeps with one lane per branch
+//             (PAPER.md:110-114), block barrier per level, sibling hand-off by warp shuffle,
+//             x written back by a bulk store.  d,u,b are read from and x written to the caller's
+//             natural-order arrays directly: the paper's separate permute kernels
+//             do not exist here.
+//   stream    cells too large for one block's shared memory: one launch per level over all such
+//             cells (global synchronisation = kernel boundary, which PAPER.md:114 avoids by
+//             requiring one matrix per block), intermediates in a plan-owned global workspace.
+//
+// Arithmetic per compartment i with parent/previous compartment q (Listing 2 read
+// with u[i], reading G1), written with the reciprocal r = 1/d'[i] (reading S12):
+//   backward:  f = u[i] r;  c = b'[i] r;  d'[q] -= f u[i];  b'[q] -= f b'[i]
+//   root:      x[0] = b'[0] r
+//   forward:   x[i] = (b'[i] - u[i] x[q]) / d'[i] = c - f x[q]
+// f overwrites d and c, then x, overwrite b in the on-chip copy; the caller's d,u,b are not written.
+#include <cuda_runtime.h>
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "plan_internal.h"
+
+namespace hines {
+
+struct DeviceTables {
+    int device = -1;
+    ItemHeader* items = nullptr;
+    int32_t* launch_order = nullptr;
+    int32_t* item_meta = nullptr;
+    StreamDesc* stream_desc = nullptr;
+    int32_t* stream_child = nullptr;
+    void* ws_f = nullptr;           // streaming workspace: f (n_stream_unknowns elements)
+    void* ws_c = nullptr;           // streaming workspace: c
+    void* host_stage[4] = {nullptr, nullptr, nullptr, nullptr};   // hines_solve_host device buffers d,u,b,x
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};              // timing hook
+    bool timing = false, timed_once = false;
+    int64_t bytes = 0;
+};
+
+#define CUDA_TRY(expr)                                                                         \
+    do {                                                                                       \
+        cudaError_t e_ = (expr);                                                               \
+        if (e_ != cudaSuccess) {                                                               \
+            set_error(std::string(#expr) + ": " + cudaGetErrorString(e_));                     \
+            return e_ == cudaErrorMemoryAllocation ? HINES_ERR_ALLOC : HINES_ERR_CUDA;         \
+        }                                                                                      \
+    } while (0)
+
+static const int32_t kAtomicFlag = 1 << 30;
+
+// ------------------------------------------------------------------------------------------------
+// PTX helpers: mbarrier + 1-D TMA bulk copies (SASS: UBLKCP, SYNCS)
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// global -> shared bulk copy, completion counted in bytes on the mbarrier
+__device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// shared -> global bulk copy (bulk async-group completion)
+__device__ __forceinline__ void tma_store_1d(void* dst_gmem, const void* src_smem, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                 ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit_wait()
+{
+    asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+}
+__device__ __forceinline__ void fence_proxy_async()
+{
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+template <typename T> __device__ __forceinline__ T rcp(T v);
+template <> __device__ __forceinline__ double rcp<double>(double v) { return 1.0 / v; }
+template <> __device__ __forceinline__ float rcp<float>(float v) { return 1.0f / v; }
+
+template <typename T> __device__ __forceinline__ T fnma(T a, T b, T c);   // c - a*b
+template <> __device__ __forceinline__ double fnma<double>(double a, double b, double c) { return fma(-a, b, c); }
+template <> __device__ __forceinline__ float fnma<float>(float a, float b, float c) { return fmaf(-a, b, c); }
+
+// ------------------------------------------------------------------------------------------------
+// Resident kernel: one block per work item (a contiguous run of cells held in shared memory).
+// Shared-memory image (bytes): [0,16) mbarrier | sd[L] | su[L] | sb[L] | meta[meta_len]
+//   L = landed elements = item range widened to 16-byte boundaries; compartment j of the item sits
+//   at index j + off, off = comp_begin mod (16 / sizeof(T)).
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, const int32_t* __restrict__ order,
+                                      const int32_t* __restrict__ meta_g, const T* __restrict__ d,
+                                      const T* __restrict__ u, const T* __restrict__ b, T* x, int64_t n_total)
+{
+    extern __shared__ __align__(128) unsigned char smem[];
+    constexpr int E = 16 / (int)sizeof(T);
+    const ItemHeader it = items[order[blockIdx.x]];
+    const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
+    const int off = (int)(it.comp_begin % E);
+    const int64_t g0 = it.comp_begin - off;                 // 16-byte aligned global element index
+    const int L = (off + it.n + E - 1) / E * E;             // landed elements
+    // the last item may end beyond a 16-byte boundary of the arrays: copy that remainder by hand
+    const int64_t avail = n_total - g0;
+    const int Lb = (int)(avail >= L ? L : (avail / E * E)); // elements brought by the bulk copies
+
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
+    T* sd = reinterpret_cast<T*>(smem + 16);
+    T* su = sd + L;
+    T* sb = su + L;
+    int32_t* smeta = reinterpret_cast<int32_t*>(sb + L);
+
+    if (tid == 0) mbar_init(bar, 1);
+    __syncthreads();
+    if (tid == 0) {
+        const uint32_t bytes = (uint32_t)Lb * sizeof(T);
+        mbar_expect_tx(bar, 3u * bytes + (uint32_t)it.meta_len * 4u);
+        tma_load_1d(smeta, meta_g + it.meta_off, (uint32_t)it.meta_len * 4u, bar);
+        if (bytes) {
+            tma_load_1d(sb, b + g0, bytes, bar);
+            tma_load_1d(sd, d + g0, bytes, bar);
+            tma_load_1d(su, u + g0, bytes, bar);
+        }
+    }
+    // remainder of the very last item (fewer than E elements), plain loads
+    for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
+    mbar_wait(bar, 0);
+    __syncthreads();
+
+    const int32_t* lvl = smeta;
+    const int32_t* desc = smeta + it.desc_off;
+    const unsigned FULL = 0xffffffffu;
+
+    // ---- backward elimination, deepest level first ----
+    for (int lev = it.nlev - 1; lev >= 0; --lev) {
+        const int eb = lvl[lev], ee = lvl[lev + 1];
+        for (int base = eb + (tid & ~31); base < ee; base += nthreads) {
+            const int e = base + lane;
+            int start = 0, len = 0, pc = -1; bool atomic_handoff = false;
+            if (e < ee) {
+                start = desc[3 * e]; len = desc[3 * e + 1]; pc = desc[3 * e + 2];
+                atomic_handoff = len & kAtomicFlag; len &= ~kAtomicFlag;
+            }
+            const int maxlen = __reduce_max_sync(FULL, len);
+            int i = start + off + len - 1;                  // last compartment of the branch
+            T D = T(1), B = T(0), dd = T(0), db = T(0);
+            if (len > 0) { D = sd[i]; B = sb[i]; }
+            for (int s = 0; s < maxlen; ++s) {              // lanes walk their branches in lock-step
+                if (s < len) {
+                    const T r = rcp<T>(D);
+                    const T c = B * r;
+                    if (s < len - 1) {                      // inside the branch: parent is i-1
+                        const T uk = su[i];
+                        const T f = uk * r;
+                        sd[i] = f; sb[i] = c;
+                        D = fnma<T>(f, uk, sd[i - 1]);
+                        B = fnma<T>(f, B, sb[i - 1]);
+                        --i;
+                    } else if (pc >= 0) {                   // first compartment: hand off to the parent branch
+                        const T uk = su[i];
+                        const T f = uk * r;
+                        sd[i] = f; sb[i] = c;
+                        dd = f * uk; db = f * B;
+                    } else {                                // root compartment: x0 = b'/d'; u[root] unread
+                        sd[i] = T(0); sb[i] = c;
+                    }
+                }
+            }
+            // hand-off at the branch point: siblings sit in one tile; the lowest lane of
+            // each sibling group gathers the others' contributions by shuffle and updates the parent.
+            const int key = (len > 0 && pc >= 0) ? pc : -2 - lane;
+            const unsigned peers = __match_any_sync(FULL, key);
+            const int leader = __ffs(peers) - 1;
+            const int maxcnt = __reduce_max_sync(FULL, __popc(peers));
+            unsigned rest = (lane == leader) ? (peers & ~(1u << lane)) : 0u;
+            for (int t = 1; t < maxcnt; ++t) {
+                const int src = rest ? (__ffs(rest) - 1) : lane;
+                const T vd = __shfl_sync(FULL, dd, src);
+                const T vb = __shfl_sync(FULL, db, src);
+                if (rest) { dd += vd; db += vb; rest &= rest - 1; }
+            }
+            if (lane == leader && key >= 0) {
+                if (!atomic_handoff) { sd[pc + off] -= dd; sb[pc + off] -= db; }
+                else { atomicAdd(&sd[pc + off], -dd); atomicAdd(&sb[pc + off], -db); }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- forward substitution, root level first ----
+    for (int lev = 0; lev < it.nlev; ++lev) {
+        const int eb = lvl[lev], ee = lvl[lev + 1];
+        for (int base = eb + (tid & ~31); base < ee; base += nthreads) {
+            const int e = base + lane;
+            int start = 0, len = 0, pc = -1;
+            if (e < ee) { start = desc[3 * e]; len = desc[3 * e + 1] & ~kAtomicFlag; pc = desc[3 * e + 2]; }
+            const int maxlen = __reduce_max_sync(FULL, len);
+            T xp = (len > 0 && pc >= 0) ? sb[pc + off] : T(0);
+            int i = start + off;
+            for (int s = 0; s < maxlen; ++s) {
+                if (s < len) {
+                    xp = fnma<T>(sd[i], xp, sb[i]);
+                    sb[i] = xp;
+                    ++i;
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    // ---- store x (natural order): bulk store of the 16-byte aligned interior, edges by hand ----
+    const int head_end = min(it.n, (E - off) % E);                     // item-local [0, head_end)
+    const int tail_begin = max(head_end, (int)(((off + it.n) / E) * E) - off);   // item-local [tail_begin, n)
+    fence_proxy_async();
+    __syncthreads();
+    if (tid == 0 && tail_begin > head_end) {
+        tma_store_1d(x + it.comp_begin + head_end, sb + off + head_end, (uint32_t)(tail_begin - head_end) * sizeof(T));
+        tma_store_commit_wait();
+    }
+    for (int j = tid; j < head_end; j += nthreads) x[it.comp_begin + j] = sb[off + j];
+    for (int j = tail_begin + tid; j < it.n; j += nthreads) x[it.comp_begin + j] = sb[off + j];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Streaming path: one launch per level, one thread per branch, lanes of a warp = 32 branches of
+// similar length (sorted at setup).  f and c go to the plan's workspace.
+// ------------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void hines_stream_backward(const StreamDesc* __restrict__ desc, int64_t begin, int64_t end,
+                                      const int2* __restrict__ child, const T* __restrict__ d,
+                                      const T* __restrict__ u, const T* __restrict__ b,
+                                      T* __restrict__ wf, T* __restrict__ wc)
+{
+    const int64_t e = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= end) return;
+    const StreamDesc s = desc[e];
+    const T* dp = d + s.gstart; const T* up = u + s.gstart; const T* bp = b + s.gstart;
+    T* fp = wf + s.ws; T* cp = wc + s.ws;
+    T D = dp[s.len - 1], B = bp[s.len - 1];
+    // pull the children's contributions (ascending child id): d' -= f_c u_c, b' -= u_c c_c (= f_c b'_c)
+    for (int k = 0; k < s.nchild; ++k) {
+        const int2 ch = child[s.child_begin + k];
+        const T uc = u[ch.x];
+        D = fnma<T>(wf[ch.y], uc, D);
+        B = fnma<T>(uc, wc[ch.y], B);
+    }
+    for (int k = s.len - 1; k >= 1; --k) {
+        const T r = rcp<T>(D);
+        const T uk = up[k];
+        const T f = uk * r;
+        fp[k] = f; cp[k] = B * r;
+        D = fnma<T>(f, uk, dp[k - 1]);
+        B = fnma<T>(f, B, bp[k - 1]);
+    }
+    const T r = rcp<T>(D);
+    fp[0] = s.gparent >= 0 ? up[0] * r : T(0);
+    cp[0] = B * r;
+}
+
+template <typename T>
+__global__ void hines_stream_forward(const StreamDesc* __restrict__ desc, int64_t begin, int64_t end,
+                                     const T* __restrict__ wf, const T* __restrict__ wc, T* x)
+{
+    const int64_t e = begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= end) return;
+    const StreamDesc s = desc[e];
+    const T* fp = wf + s.ws; const T* cp = wc + s.ws;
+    T* xo = x + s.gstart;
+    T xp = s.gparent >= 0 ? x[s.gparent] : T(0);
+    for (int k = 0; k < s.len; ++k) { xp = fnma<T>(fp[k], xp, cp[k]); xo[k] = xp; }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host side
+// ------------------------------------------------------------------------------------------------
+template <typename V>
+static hines_status_t upload_vec(const V& v, void** dst, int64_t& total)
+{
+    *dst = nullptr;
+    const size_t bytes = v.size() * sizeof(v[0]);
+    if (!bytes) return HINES_OK;
+    CUDA_TRY(cudaMalloc(dst, bytes));
+    CUDA_TRY(cudaMemcpy(*dst, v.data(), bytes, cudaMemcpyHostToDevice));
+    total += (int64_t)bytes;
+    return HINES_OK;
+}
+
+static void free_device(DeviceTables* D)
+{
+    if (!D) return;
+    cudaFree(D->items); cudaFree(D->launch_order); cudaFree(D->item_meta); cudaFree(D->stream_desc);
+    cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c);
+    for (void* p : D->host_stage) cudaFree(p);
+    for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
+    delete D;
+}
+
+static hines_status_t upload(hines_plan* P)
+{
+    if (P->dev) return HINES_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        set_error("no CUDA device: this library has no CPU fallback");
+        return HINES_ERR_CUDA;
+    }
+    DeviceTables* D = new (std::nothrow) DeviceTables();
+    if (!D) { set_error("host allocation failed"); return HINES_ERR_ALLOC; }
+    hines_status_t st = HINES_OK;
+    auto run = [&]() -> hines_status_t {
+        CUDA_TRY(cudaGetDevice(&D->device));
+        int max_optin = 0;
+        CUDA_TRY(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, D->device));
+        for (int32_t s : P->class_smem_bytes)
+            if (s > max_optin) {
+                set_error("device offers " + std::to_string(max_optin) + " bytes of shared memory per block, plan needs " + std::to_string(s));
+                return HINES_ERR_UNSUPPORTED;
+            }
+        if ((st = upload_vec(P->item_headers, (void**)&D->items, D->bytes))) return st;
+        if ((st = upload_vec(P->item_launch_order, (void**)&D->launch_order, D->bytes))) return st;
+        if ((st = upload_vec(P->item_meta, (void**)&D->item_meta, D->bytes))) return st;
+        if ((st = upload_vec(P->stream_desc, (void**)&D->stream_desc, D->bytes))) return st;
+        if ((st = upload_vec(P->stream_child, (void**)&D->stream_child, D->bytes))) return st;
+        if (P->n_stream_unknowns) {
+            const size_t wb = (size_t)P->n_stream_unknowns * P->width;
+            CUDA_TRY(cudaMalloc(&D->ws_f, wb));
+            CUDA_TRY(cudaMalloc(&D->ws_c, wb));
+            D->bytes += 2 * (int64_t)wb;
+        }
+        int32_t max_smem = 0;
+        for (int32_t s : P->class_smem_bytes) max_smem = s > max_smem ? s : max_smem;
+        if (max_smem) {
+            if (P->dtype == HINES_F64)
+                CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+            else
+                CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        }
+        return HINES_OK;
+    };
+    st = run();
+    if (st != HINES_OK) { free_device(D); return st; }
+    P->dev = D;
+    return HINES_OK;
+}
+
+template <typename T>
+static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T* b, T* x, cudaStream_t stream)
+{
+    DeviceTables* D = P->dev;
+    const int nthreads = P->opt.threads_per_block;
+    if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
+    for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
+        const int64_t cnt = P->class_count[q];
+        if (!cnt) continue;
+        hines_resident_kernel<T><<<(unsigned)cnt, nthreads, P->class_smem_bytes[q], stream>>>(
+            D->items, D->launch_order + P->class_first[q], D->item_meta, d, u, b, x, P->n);
+    }
+    if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
+    const int nlev = (int)P->stream_level_begin.size() - 1;
+    const int st = P->opt.stream_threads;
+    T* wf = static_cast<T*>(D->ws_f); T* wc = static_cast<T*>(D->ws_c);
+    for (int l = nlev - 1; l >= 0; --l) {
+        const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
+        hines_stream_backward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, stream>>>(
+            D->stream_desc, b0, b1, reinterpret_cast<const int2*>(D->stream_child), d, u, b, wf, wc);
+    }
+    for (int l = 0; l < nlev; ++l) {
+        const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
+        hines_stream_forward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, stream>>>(
+            D->stream_desc, b0, b1, wf, wc, x);
+    }
+    if (D->timing) { CUDA_TRY(cudaEventRecord(D->ev[2], stream)); D->timed_once = true; }
+    CUDA_TRY(cudaGetLastError());
+    return HINES_OK;
+}
+
+static hines_status_t check_ptrs(const hines_plan* P, const void* d, const void* u, const void* b, const void* x)
+{
+    if (!P || !d || !u || !b || !x) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    return HINES_OK;
+}
+
+}  // namespace hines
+
+using namespace hines;
+
+extern "C" {
+
+hines_status_t hines_plan_upload(hines_plan_t* P)
+{
+    if (!P) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    return upload(P);
+}
+
+hines_status_t hines_solve(hines_plan_t* P, const void* d, const void* u, const void* b, void* x, hines_stream_t stream)
+{
+    hines_status_t st = check_ptrs(P, d, u, b, x);
+    if (st != HINES_OK) return st;
+    if (((uintptr_t)d | (uintptr_t)u | (uintptr_t)b | (uintptr_t)x) & 15) {
+        set_error("device pointers must be 16-byte aligned"); return HINES_ERR_INVALID_ARG;
+    }
+    if (d == x || u == x) { set_error("x may alias b only"); return HINES_ERR_INVALID_ARG; }
+    if ((st = upload(P)) != HINES_OK) return st;
+    if (P->dtype == HINES_F64)
+        return launch_all<double>(P, (const double*)d, (const double*)u, (const double*)b, (double*)x, (cudaStream_t)stream);
+    return launch_all<float>(P, (const float*)d, (const float*)u, (const float*)b, (float*)x, (cudaStream_t)stream);
+}
+
+hines_status_t hines_solve_host(hines_plan_t* P, const void* d, const void* u, const void* b, void* x, hines_stream_t stream)
+{
+    hines_status_t st = check_ptrs(P, d, u, b, x);
+    if (st != HINES_OK) return st;
+    if ((st = upload(P)) != HINES_OK) return st;
+    DeviceTables* D = P->dev;
+    const size_t bytes = (size_t)P->n * P->width;
+    for (int k = 0; k < 4; ++k)
+        if (!D->host_stage[k]) { CUDA_TRY(cudaMalloc(&D->host_stage[k], bytes)); D->bytes += (int64_t)bytes; }
+    cudaStream_t s = (cudaStream_t)stream;
+    CUDA_TRY(cudaMemcpyAsync(D->host_stage[0], d, bytes, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaMemcpyAsync(D->host_stage[1], u, bytes, cudaMemcpyHostToDevice, s));
+    CUDA_TRY(cudaMemcpyAsync(D->host_stage[2], b, bytes, cudaMemcpyHostToDevice, s));
+    st = hines_solve(P, D->host_stage[0], D->host_stage[1], D->host_stage[2], D->host_stage[3], stream);
+    if (st != HINES_OK) return st;
+    CUDA_TRY(cudaMemcpyAsync(x, D->host_stage[3], bytes, cudaMemcpyDeviceToHost, s));
+    CUDA_TRY(cudaStreamSynchronize(s));
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_enable_timing(hines_plan_t* P, int32_t enable)
+{
+    if (!P) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    hines_status_t st = upload(P);
+    if (st != HINES_OK) return st;
+    DeviceTables* D = P->dev;
+    if (enable)
+        for (auto& e : D->ev) if (!e) CUDA_TRY(cudaEventCreate(&e));
+    D->timing = enable != 0;
+    D->timed_once = false;
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_get_timing(hines_plan_t* P, float* resident_ms, float* stream_ms)
+{
+    if (!P || !resident_ms || !stream_ms) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    if (!P->dev || !P->dev->timing || !P->dev->timed_once) { set_error("timing not enabled or no solve yet"); return HINES_ERR_INVALID_ARG; }
+    DeviceTables* D = P->dev;
+    CUDA_TRY(cudaEventSynchronize(D->ev[2]));
+    CUDA_TRY(cudaEventElapsedTime(resident_ms, D->ev[0], D->ev[1]));
+    CUDA_TRY(cudaEventElapsedTime(stream_ms, D->ev[1], D->ev[2]));
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_destroy(hines_plan_t* P)
+{
+    if (!P) return HINES_OK;
+    free_device(P->dev);
+    delete P;
+    return HINES_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,160 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Bar (BASELINE.json north_star): per-cell relative max-norm error
+<= 1e-10 in fp64; <= 1e-4 in fp32 against the fp64 oracle run on the fp32-rounded inputs
+(reading S15)."""
+import numpy as np
+import pytest
+
+import morphgen as mg
+import oracle
+from helpers import random_parent
+
+pytestmark = pytest.mark.gpu
+
+TOL = {np.float64: 1e-10, np.float32: 1e-4}
+
+
+def _gpu_solve(m, d, u, b, dtype=np.float64, inplace=False, **kw):
+    import torch
+    import paper_1810_12742_b200 as hb
+    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == np.float64 else hb.F32, **kw)
+    dd, du, db = (torch.from_numpy(np.ascontiguousarray(a, dtype)).cuda() for a in (d, u, b))
+    x = db if inplace else torch.full_like(db, float("nan"))
+    plan.solve(dd, du, db, x)
+    torch.cuda.synchronize()
+    out = x.cpu().numpy()
+    if not inplace:      # inputs are never written
+        assert torch.equal(dd.cpu(), torch.from_numpy(np.ascontiguousarray(d, dtype)))
+        assert torch.equal(db.cpu(), torch.from_numpy(np.ascontiguousarray(b, dtype)))
+    info = plan.info
+    plan.close()
+    return out, info
+
+
+def _check(m, d, u, b, dtype=np.float64, **kw):
+    x, info = _gpu_solve(m, d, u, b, dtype, **kw)
+    dr, ur, br = (np.ascontiguousarray(a, dtype).astype(np.float64) for a in (d, u, b))
+    xr = oracle.hines_solve(m.parent, m.cell_offsets, dr, ur, br)
+    err = oracle.rel_err(m.cell_offsets, x.astype(np.float64), xr)
+    assert np.isfinite(x).all()
+    assert err.max() <= TOL[dtype], (err.max(), int(err.argmax()))
+    return err.max(), info
+
+
+SMALL = [(0, 1.0), (1, 0.01), (2, 0.01), (3, 0.003)]
+
+
+@pytest.mark.parametrize("cfg,scale", SMALL)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_small_configs_default_policy(cfg, scale, dtype):
+    m = mg.make_config(cfg, scale)
+    d, u, b = mg.system(m)
+    _check(m, d, u, b, dtype)
+
+
+@pytest.mark.parametrize("cfg,scale", SMALL)
+def test_small_configs_streaming_path(cfg, scale):
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(cfg, scale)
+    d, u, b = mg.system(m)
+    _, info = _check(m, d, u, b, policy_flags=hb.POLICY_FORCE_STREAM)
+    assert info.n_resident_items == 0 and info.n_stream_cells == m.ncells
+
+
+@pytest.mark.parametrize("kw", [dict(policy_flags=2), dict(policy_flags=4), dict(smem_bytes_per_block=48 * 1024),
+                                dict(threads_per_block=64), dict(threads_per_block=1024, group_smem_bytes=200 * 1024),
+                                dict(group_smem_bytes=8 * 1024, stream_threads=32)])
+def test_policy_variants_mixed_paths(kw):
+    """Several size classes, resident + streaming in one solve, different block sizes."""
+    m = mg.make_config(2, 0.006)
+    d, u, b = mg.system(m)
+    _, info = _check(m, d, u, b, **kw)
+    if kw.get("smem_bytes_per_block"):
+        assert info.n_stream_cells > 0 and info.n_resident_items > 0
+
+
+def _edge_morphology():
+    star = np.array([-1] + [0] * 70, np.int32)            # 70 siblings: hand-off spans tiles (atomic path)
+    ps = [np.array([-1], np.int32), star, random_parent(33, 1), np.array([-1], np.int32),
+          random_parent(201, 2, .7), star[:40], np.arange(-1, 6, dtype=np.int32),
+          random_parent(1001, 3, .97), np.array([-1, 0], np.int32), random_parent(77, 5, .2)]
+    if sum(len(p) for p in ps) % 2 == 0:
+        ps.append(np.array([-1, 0, 0], np.int32))           # make N odd: the last item ends off a 16-byte boundary
+    offs = np.concatenate([[0], np.cumsum([len(p) for p in ps])])
+    return mg.Morphology(np.concatenate(ps), offs)          # odd offsets, odd N, non-BFS numbering
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("kw", [{}, dict(policy_flags=1), dict(policy_flags=2), dict(smem_bytes_per_block=8 * 1024)])
+def test_edge_cases(dtype, kw):
+    m = _edge_morphology()
+    assert m.n % 2 == 1
+    d, u, b = mg.system(m, seed=11)
+    _check(m, d, u, b, dtype, **kw)
+
+
+def test_in_place_and_nan_poisoned_root_u():
+    m = _edge_morphology()
+    d, u, b = mg.system(m, seed=12)
+    x0, _ = _gpu_solve(m, d, u, b)
+    u2 = u.copy(); u2[m.cell_offsets[:-1]] = np.nan         # reading S2: u[root] is never used
+    for kw in ({}, dict(policy_flags=1)):
+        x1, _ = _gpu_solve(m, d, u2, b, inplace=True, **kw)
+        xr = oracle.hines_solve(m.parent, m.cell_offsets, d, u, b)
+        assert oracle.rel_err(m.cell_offsets, x1, xr).max() < 1e-10
+    assert np.array_equal(x0, _gpu_solve(m, d, u, b)[0])     # run-to-run deterministic
+
+
+def test_row_sums_give_ones_on_gpu():
+    m = mg.make_config(2, 0.005)
+    d, u, _ = mg.system(m)
+    b1 = oracle.matvec(m.parent, m.cell_offsets, d, u, np.ones(m.n))
+    x, _ = _gpu_solve(m, d, u, b1)
+    assert np.abs(x - 1).max() < 1e-13
+
+
+def test_bad_pointers_rejected():
+    import torch
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(0)
+    plan = hb.Plan(m.parent, m.cell_offsets)
+    t = torch.zeros(m.n + 1, dtype=torch.float64, device="cuda")
+    with pytest.raises(hb.HinesError) as e:
+        plan.solve(t[1:], t[1:], t[1:], t[1:])               # 8-byte aligned only
+    assert e.value.status == 1
+    with pytest.raises(hb.HinesError):
+        plan.solve(t, t, t, t)                               # x aliases d
+
+
+# ---- full BASELINE.json sizes, in the launch configuration bench.py times ----------------------
+@pytest.mark.parametrize("cfg,dtype", [(1, np.float64), (2, np.float64), (2, np.float32), (4, np.float64)])
+def test_full_size(cfg, dtype):
+    m = mg.make_config(cfg, 1.0)
+    d, u, b = mg.system(m)
+    err, info = _check(m, d, u, b, dtype)
+    print(f"cfg{cfg} {np.dtype(dtype).name}: n={m.n} max rel err {err:.3e} resident_items={info.n_resident_items} "
+          f"stream_cells={info.n_stream_cells}")
+
+
+def test_full_size_config3():
+    m = mg.make_config(3, 1.0)
+    d, u, b = mg.system(m)
+    err, info = _check(m, d, u, b)
+    print(f"cfg3: n={m.n} max rel err {err:.3e} resident_items={info.n_resident_items} stream_cells={info.n_stream_cells}")
+
+
+def test_config4_fresh_rhs_steps():
+    """Config 4: one very large cell solved for several time steps with a fresh b each step."""
+    import torch
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(4)
+    d, u, _ = mg.system(m)
+    plan = hb.Plan(m.parent, m.cell_offsets)
+    dd, du = torch.from_numpy(d).cuda(), torch.from_numpy(u).cuda()
+    x = torch.empty_like(dd)
+    for step in (0, 1, 2, 999):
+        b = mg.rhs(m, step=step)
+        plan.solve(dd, du, torch.from_numpy(b).cuda(), x)
+        xr = oracle.hines_solve(m.parent, m.cell_offsets, d, u, b)
+        assert oracle.rel_err(m.cell_offsets, x.cpu().numpy(), xr).max() < 1e-10
+    plan.close()
