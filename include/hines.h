@@ -68,6 +68,8 @@ typedef struct {
     int32_t group_smem_bytes;       /* 0 = default (56 KiB): small cells are grouped into work items up to
                                        this much shared memory ("fit as many matrices into one
                                        block as possible")                                                 */
+    int32_t max_segment;            /* 0 = default (64), 2..2047: branches longer than this are cut into
+                                       chained segments ("we split branches that are too long") */
 } hines_options_t;
 
 typedef struct {
@@ -82,8 +84,10 @@ typedef struct {
     int64_t n_stream_cells;     /* cells too large for shared memory -> streaming path                     */
     int64_t n_stream_unknowns;
     int64_t n_stream_branches;
-    int64_t padded_lane_steps;  /* sum over 32-lane tiles of (longest branch in the tile * 32)             */
-    int64_t useful_lane_steps;  /* = n minus nothing: sum of branch lengths; ratio = lane efficiency       */
+    int64_t padded_lane_steps;  /* sum over 32-lane tiles of (longest lane of the tile * 32) in the segment
+                                   sweeps (resident path) and the branch sweeps (streaming path)           */
+    int64_t useful_lane_steps;  /* the same without idle lanes: interior compartments of all segments +
+                                   compartments of streamed branches; ratio = lane efficiency              */
     int64_t workspace_bytes;    /* device memory the plan owns (tables + streaming workspace)              */
     int64_t bytes_min;          /* n*4*w + 4*nbranches: d,u,b read, x written, one parent per branch
                                    (PAPER.md:138); the roofline numerator                                  */
@@ -116,8 +120,14 @@ typedef enum {
     HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
     HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] descriptor index (item-local) where each
                                                level's lane list begins                                               */
-    HINES_TABLE_ITEM_DESC            = 39,  /* int32[3*ndesc] {start (item-local compartment), len, parent compartment
-                                               (item-local, -1 = root branch)}; len = 0 marks a padding lane           */
+    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*ndesc] per branch {end = last compartment (item-local),
+                                               nseg | Sj<<20 | spans-tiles flag<<31, parent compartment (item-local,
+                                               -1 = root branch), first separator id}; nseg = 0 marks a padding lane   */
+    HINES_TABLE_ITEM_SEG_OFFSETS     = 44,  /* int64[nitems+1] into ITEM_SEG (in units of descriptors)                */
+    HINES_TABLE_ITEM_SEG             = 45,  /* int32[4*nseglanes] per segment with a non-empty interior {a = first
+                                               interior compartment, m = interior length, t = separator above (-1 = none),
+                                               separator id}; m = 0 marks a padding lane                               */
+    HINES_TABLE_ITEM_NSEP            = 46,  /* int32[nitems] separators (= segments) per item                          */
     HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
     HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment
                                                (-1 root), workspace start, child_begin, nchild}                       */

@@ -33,7 +33,8 @@ TABLES = {
     "item_launch_order": (35, np.int32), "item_desc_offsets": (36, np.int64),
     "item_level_offsets": (37, np.int64), "item_level_begin": (38, np.int32), "item_desc": (39, np.int32),
     "stream_level_begin": (40, np.int64), "stream_desc": (41, np.int32), "stream_child": (42, np.int32),
-    "class_smem_bytes": (43, np.int32),
+    "class_smem_bytes": (43, np.int32), "item_seg_offsets": (44, np.int64), "item_seg": (45, np.int32),
+    "item_nsep": (46, np.int32),
 }
 
 # every symbol include/hines.h declares
@@ -46,7 +47,7 @@ ABI_SYMBOLS = ["hines_plan_create", "hines_plan_upload", "hines_solve", "hines_s
 class Options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("threads_per_block", C.c_int32),
                 ("smem_bytes_per_block", C.c_int32), ("policy_flags", C.c_int32),
-                ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32)]
+                ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32), ("max_segment", C.c_int32)]
 
 
 class PlanInfo(C.Structure):
@@ -119,12 +120,12 @@ class Plan:
     """hines_plan_create(parent arrays, cell offsets) -- setup-time scheduler."""
 
     def __init__(self, parent, cell_offsets, dtype=F64, threads_per_block=0, smem_bytes_per_block=0,
-                 policy_flags=0, stream_threads=0, group_smem_bytes=0):
+                 policy_flags=0, stream_threads=0, group_smem_bytes=0, max_segment=0):
         lib = load_library()
         parent = np.ascontiguousarray(parent, dtype=np.int32)
         offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
         opt = Options(C.sizeof(Options), threads_per_block, smem_bytes_per_block, policy_flags,
-                      stream_threads, group_smem_bytes)
+                      stream_threads, group_smem_bytes, max_segment)
         h = C.c_void_p()
         self._h = None
         _check(lib.hines_plan_create(parent.ctypes.data, offs.ctypes.data, len(offs) - 1, int(dtype),

@@ -13,9 +13,18 @@
 //          a level's lane list and is limited by its 227 KB of shared memory, not its thread count.
 //          Cells that do not fit any block go to the streaming path (the paper has no such path:
 //          PAPER.md:114 requires one matrix per block).
-//   P3     per (item, level): lane list.  Sibling branches (same parent compartment) are kept in one
-//          32-lane tile so the hand-off at the branch point is a warp shuffle; sibling
-//          groups are sorted by their longest member, descending (Fig 4.1).
+//   P3     per (item, level): lane list of the level-synchronous part.  Sibling branches (same parent
+//          compartment) are kept in one 32-lane tile so the hand-off at the branch point
+//           is a warp shuffle; sibling groups are sorted by their longest member,
+//          descending (Fig 4.1).
+//   P4     segments.  Every branch is cut, from its end, into nseg = ceil(len / max_segment) segments
+//          of Sj = ceil(len / nseg) compartments (the paper's branch splitting, with a
+//          fixed bound instead of the level average).  The last compartment of a segment is its
+//          separator; the compartments above it are its interior.  Interiors are eliminated
+//          independently of the tree level (one lane per segment, all segments of the item at once),
+//          which leaves the level-synchronous sweeps with one node per segment.  The segment lane list
+//          is ordered so that the 16 (fp64) / 32 (fp32) lanes that access shared memory together start
+//          at different bank residues and have similar lengths.
 // Written policy: DESIGN.md "Scheduler policy".
 #include <algorithm>
 #include <cstring>
@@ -32,7 +41,7 @@ void set_error(const std::string& msg) { g_last_error = msg; }
 
 static const int64_t kSmemPerSM = 233472;       // 228 KiB
 static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
-static const int32_t kAtomicFlag = 1 << 30;     // descriptor len bit: sibling group spans tiles
+static const int32_t kAtomicFlag = (int32_t)0x80000000u;   // descriptor bit 31: sibling group spans tiles
 static const int kClassK[] = {1, 2, 3, 4, 6, 8};
 static const int kNumClassK = 6;
 
@@ -44,26 +53,30 @@ static int64_t class_cap(int k, int64_t max_smem)
     return std::min(cap, max_smem);
 }
 
-struct Entry { int32_t start, len, pc, ord; int64_t key; };
+struct Entry { int32_t start, len, pc, ord; int64_t key; int32_t nseg, sj, sep_base; };
 
-// Lane lists of one work item (cells [c0,c1)), policy P3.  Returns the shared-memory need in bytes.
+// Lane lists of one work item (cells [c0,c1)), policies P3 + P4.
 struct ItemBuild {
     int64_t comp_begin = 0, n = 0;
-    int32_t nlev = 0;
-    std::vector<int32_t> level_begin;   // nlev+1
-    std::vector<int32_t> desc;          // 3 per descriptor
-    int64_t padded_steps = 0;
+    int32_t nlev = 0, nsep = 0;
+    std::vector<int32_t> level_begin;   // nlev+1, in branch descriptors
+    std::vector<int32_t> desc;          // 4 per branch descriptor: {end, nseg | sj<<20 | flag, pc, sep_base}
+    std::vector<int32_t> seg;           // 4 per segment descriptor: {a, m, t, sep_id}; m = 0 is a padding lane
+    int64_t padded_steps = 0;           // lane-steps of the segment sweeps incl. idle lanes
     int64_t smem_need = 0;
 };
 
 static void build_item(const hines_plan& P, int64_t c0, int64_t c1, ItemBuild& out)
 {
+    const int32_t smax = P.opt.max_segment;
     out.comp_begin = P.cell_offsets[c0];
     out.n = P.cell_offsets[c1] - out.comp_begin;
     out.nlev = 0;
     for (int64_t c = c0; c < c1; ++c) out.nlev = std::max(out.nlev, P.cell_nlevels[c]);
     std::vector<std::vector<Entry>> lv(out.nlev);
-    int32_t ord = 0;
+    int32_t ord = 0, nsep = 0;
+    struct Seg { int32_t a, m, t, sid; };
+    std::vector<Seg> segs;
     for (int64_t c = c0; c < c1; ++c) {
         const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
         const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
@@ -74,62 +87,111 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, ItemBuild& o
             e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
             e.ord = ord;                                    // (cell, branch id) order
             e.key = e.pc >= 0 ? (int64_t)e.pc : -(int64_t)ord - 1;   // roots are singletons
+            e.nseg = (e.len + smax - 1) / smax;
+            e.sj = (e.len + e.nseg - 1) / e.nseg;
+            e.sep_base = nsep;
+            const int32_t end = e.start + e.len - 1;
+            for (int32_t k = 0; k < e.nseg; ++k) {          // segments counted from the branch's end
+                const int32_t b = end - k * e.sj;
+                const int32_t a = std::max(e.start, b - e.sj + 1);
+                const int32_t t = k < e.nseg - 1 ? b - e.sj : e.pc;
+                if (b - a > 0) segs.push_back({a, b - a, t, nsep + k});
+            }
+            nsep += e.nseg;
             lv[P.branch_level[j]].push_back(e);
         }
     }
+    out.nsep = nsep;
     out.level_begin.assign(out.nlev + 1, 0);
     out.desc.clear();
-    out.padded_steps = 0;
-    struct Group { int32_t first, count, maxlen, minord; };
+    struct Group { int32_t first, count, maxseg, minord; };
     std::vector<Group> groups;
     for (int32_t l = 0; l < out.nlev; ++l) {
         auto& v = lv[l];
-        // siblings contiguous; inside a group: length descending, then (cell, id)
+        // siblings contiguous; inside a group: segment count descending, then (cell, id)
         std::sort(v.begin(), v.end(), [](const Entry& a, const Entry& b) {
             if (a.key != b.key) return a.key < b.key;
-            if (a.len != b.len) return a.len > b.len;
+            if (a.nseg != b.nseg) return a.nseg > b.nseg;
             return a.ord < b.ord;
         });
         groups.clear();
         for (int32_t i = 0; i < (int32_t)v.size();) {
             int32_t j = i, mo = v[i].ord;
             while (j < (int32_t)v.size() && v[j].key == v[i].key) { mo = std::min(mo, v[j].ord); ++j; }
-            groups.push_back({i, j - i, v[i].len, mo});
+            groups.push_back({i, j - i, v[i].nseg, mo});
             i = j;
         }
-        // groups by longest member descending, ties by first (cell, id)
+        // groups by their longest member (in level-synchronous steps) descending
         std::sort(groups.begin(), groups.end(), [](const Group& a, const Group& b) {
-            if (a.maxlen != b.maxlen) return a.maxlen > b.maxlen;
+            if (a.maxseg != b.maxseg) return a.maxseg > b.maxseg;
             return a.minord < b.minord;
         });
-        out.level_begin[l] = (int32_t)(out.desc.size() / 3);
+        out.level_begin[l] = (int32_t)(out.desc.size() / 4);
         int32_t pos = 0;
         for (const Group& g : groups) {
             const bool spans = g.count > 32;
             if (!spans && (pos % 32) + g.count > 32) {          // keep the sibling group in one tile
-                while (pos % 32) { out.desc.insert(out.desc.end(), {0, 0, -1}); ++pos; }
+                while (pos % 32) { out.desc.insert(out.desc.end(), {0, 0, -1, 0}); ++pos; }
             }
             for (int32_t i = 0; i < g.count; ++i) {
                 const Entry& e = v[g.first + i];
-                out.desc.push_back(e.start);
-                out.desc.push_back(spans ? (e.len | kAtomicFlag) : e.len);
+                out.desc.push_back(e.start + e.len - 1);
+                out.desc.push_back(e.nseg | (e.sj << 20) | (spans ? kAtomicFlag : 0));
                 out.desc.push_back(e.pc);
+                out.desc.push_back(e.sep_base);
                 ++pos;
             }
         }
-        // lane-step accounting: 32 lanes x longest branch of each tile
-        const int32_t lb = out.level_begin[l], le = (int32_t)(out.desc.size() / 3);
-        for (int32_t t = lb; t < le; t += 32) {
-            int32_t mx = 0;
-            for (int32_t i = t; i < std::min(le, t + 32); ++i) mx = std::max(mx, out.desc[3 * i + 1] & ~kAtomicFlag);
-            out.padded_steps += 32 * (int64_t)mx;
-        }
     }
-    out.level_begin[out.nlev] = (int32_t)(out.desc.size() / 3);
+    out.level_begin[out.nlev] = (int32_t)(out.desc.size() / 4);
+
+    // P4: segment lane list.  R lanes access shared memory in one wavefront (16 x 8 B or 32 x 4 B);
+    // give them distinct start residues mod R (then they stay distinct while all lanes advance in
+    // lock-step) and similar lengths: bucket by residue, each bucket longest first, one round = the
+    // heads of all buckets, topped up from the fullest buckets when some are exhausted.
+    const int R = 128 / P.width;
+    std::vector<std::vector<Seg>> bucket(R);
+    for (const Seg& sg : segs) bucket[sg.a % R].push_back(sg);
+    for (auto& bk : bucket)
+        std::stable_sort(bk.begin(), bk.end(), [](const Seg& x, const Seg& y) { return x.m > y.m; });
+    std::vector<size_t> head(R, 0);
+    size_t remaining = segs.size();
+    out.seg.clear();
+    std::vector<int> pick;
+    while (remaining) {
+        pick.clear();
+        for (int r = 0; r < R; ++r) if (head[r] < bucket[r].size()) pick.push_back(r);
+        size_t taken = pick.size();
+        // top up: second helpings from the buckets with most left (conflicts only in these tail rounds)
+        while (taken < (size_t)R && taken < remaining) {
+            int best = -1; size_t left = 0;
+            for (int r = 0; r < R; ++r) {
+                size_t used = 0;
+                for (int q : pick) used += (q == r);
+                const size_t l = bucket[r].size() - head[r] > used ? bucket[r].size() - head[r] - used : 0;
+                if (l > left) { left = l; best = r; }
+            }
+            if (best < 0) break;
+            pick.push_back(best); ++taken;
+        }
+        for (int r : pick) {
+            const Seg& sg = bucket[r][head[r]++];
+            out.seg.insert(out.seg.end(), {sg.a, sg.m, sg.t, sg.sid});
+            --remaining;
+        }
+        if (remaining) while ((out.seg.size() / 4) % R) out.seg.insert(out.seg.end(), {0, 0, -1, 0});
+    }
+    out.padded_steps = 0;
+    const int32_t ns = (int32_t)(out.seg.size() / 4);
+    for (int32_t t = 0; t < ns; t += 32) {
+        int32_t mx = 0;
+        for (int32_t i = t; i < std::min(ns, t + 32); ++i) mx = std::max(mx, out.seg[4 * i + 1]);
+        out.padded_steps += 32 * (int64_t)mx;
+    }
     const int E = 16 / P.width;
     const int64_t L = round_up(out.comp_begin % E + out.n, E);
-    const int64_t meta = round_up(out.nlev + 1, 4) + round_up((int64_t)out.desc.size(), 4);
-    out.smem_need = 16 + 3 * L * P.width + meta * 4;
+    const int64_t meta = round_up(out.nlev + 1, 4) + (int64_t)out.desc.size() + (int64_t)out.seg.size();
+    out.smem_need = 16 + 3 * L * P.width + 2 * round_up(out.nsep, E) * P.width + meta * 4;
 }
 
 static hines_status_t canonical_tables(hines_plan& P, const int32_t* parent)
@@ -234,8 +296,11 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_level_begin.insert(P.item_level_begin.end(), ib.level_begin.begin(), ib.level_begin.end());
     P.item_level_offsets.push_back((int64_t)P.item_level_begin.size());
     P.item_desc.insert(P.item_desc.end(), ib.desc.begin(), ib.desc.end());
-    P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 3);
-    // device blob: [level_begin | pad4 | desc | pad4]
+    P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 4);
+    P.item_seg.insert(P.item_seg.end(), ib.seg.begin(), ib.seg.end());
+    P.item_seg_offsets.push_back((int64_t)P.item_seg.size() / 4);
+    P.item_nsep.push_back(ib.nsep);
+    // device blob: [level_begin | pad4 | branch desc | segment desc]
     hines::ItemHeader h;
     h.comp_begin = ib.comp_begin;
     h.n = (int32_t)ib.n;
@@ -245,13 +310,16 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
     h.desc_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
     P.item_meta.insert(P.item_meta.end(), ib.desc.begin(), ib.desc.end());
-    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
+    h.seg_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    P.item_meta.insert(P.item_meta.end(), ib.seg.begin(), ib.seg.end());
     h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    h.nseg_lanes = (int32_t)(ib.seg.size() / 4);
+    h.nsep = ib.nsep;
     P.item_headers.push_back(h);
     P.padded_lane_steps += ib.padded_steps;
+    for (size_t q = 1; q < ib.seg.size(); q += 4) P.useful_lane_steps += ib.seg[q];
     P.n_resident_cells += c1 - c0;
     P.n_resident_unknowns += ib.n;
-    // remember the need in item_class temporarily through a side vector
 }
 
 static void pack_items(hines_plan& P, std::vector<int64_t>& item_need, std::vector<char>& is_stream)
@@ -264,6 +332,7 @@ static void pack_items(hines_plan& P, std::vector<int64_t>& item_need, std::vect
     P.cell_item.assign(nc, -1);
     P.item_level_offsets.assign(1, 0);
     P.item_desc_offsets.assign(1, 0);
+    P.item_seg_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
     ItemBuild cur, cand;
     int64_t g0 = -1;                                   // first cell of the open group
@@ -380,6 +449,7 @@ static void build_stream(hines_plan& P, const std::vector<char>& is_stream)
                 P.stream_child.push_back((int32_t)(ws_off[c] + P.branch_start[ch]));
             }
             P.stream_desc.push_back(s);
+            P.useful_lane_steps += e.len;
         }
     }
     P.stream_level_begin[maxlev] = (int64_t)P.stream_desc.size();
@@ -410,10 +480,11 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.smem_bytes_per_block == 0) o.smem_bytes_per_block = (int32_t)kSmemMaxOptin;
     if (o.stream_threads == 0) o.stream_threads = 128;
     if (o.group_smem_bytes == 0) o.group_smem_bytes = 57344;
+    if (o.max_segment == 0) o.max_segment = 64;
     if (o.threads_per_block < 32 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        (o.policy_flags & ~7)) {
+        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~7)) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }
     if (cell_offsets[0] != 0) { set_error("cell_offsets[0] must be 0"); return HINES_ERR_BAD_TOPOLOGY; }
@@ -454,7 +525,7 @@ hines_status_t hines_plan_get_info(const hines_plan_t* P, hines_plan_info_t* out
     out->n_resident_cells = P->n_resident_cells; out->n_resident_unknowns = P->n_resident_unknowns;
     out->n_stream_cells = P->n_stream_cells; out->n_stream_unknowns = P->n_stream_unknowns;
     out->n_stream_branches = (int64_t)P->stream_desc.size();
-    out->padded_lane_steps = P->padded_lane_steps; out->useful_lane_steps = P->n;
+    out->padded_lane_steps = P->padded_lane_steps; out->useful_lane_steps = P->useful_lane_steps;
     out->workspace_bytes = (int64_t)(P->item_meta.size() * 4 + P->item_headers.size() * sizeof(ItemHeader) +
                                      P->item_launch_order.size() * 4 + P->stream_desc.size() * sizeof(StreamDesc) +
                                      P->stream_child.size() * 4 + 2 * P->n_stream_unknowns * P->width);
@@ -491,6 +562,9 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_LEVEL_OFFSETS, P->item_level_offsets)
         TBL(HINES_TABLE_ITEM_LEVEL_BEGIN, P->item_level_begin)
         TBL(HINES_TABLE_ITEM_DESC, P->item_desc)
+        TBL(HINES_TABLE_ITEM_SEG_OFFSETS, P->item_seg_offsets)
+        TBL(HINES_TABLE_ITEM_SEG, P->item_seg)
+        TBL(HINES_TABLE_ITEM_NSEP, P->item_nsep)
         TBL(HINES_TABLE_STREAM_LEVEL_BEGIN, P->stream_level_begin)
         TBL(HINES_TABLE_STREAM_DESC, P->stream_desc)
         TBL(HINES_TABLE_STREAM_CHILD, P->stream_child)

@@ -15,8 +15,12 @@ struct ItemHeader {
     int32_t n;            // unknowns in the item
     int32_t nlev;         // levels of the deepest cell in the item
     int64_t meta_off;     // offset (int32 units, multiple of 4) of the item's metadata blob
-    int32_t meta_len;     // int32 count (multiple of 4): [level_begin (nlev+1) | pad | desc 3*ndesc | pad]
-    int32_t desc_off;     // offset (int32 units, multiple of 4) of the descriptors inside the blob
+    int32_t meta_len;     // int32 count (multiple of 4): [level_begin (nlev+1) | pad | branch desc | segment desc]
+    int32_t desc_off;     // offset (int32 units, multiple of 4) of the branch descriptors inside the blob
+    int32_t seg_off;      // offset of the segment descriptors inside the blob
+    int32_t nseg_lanes;   // segment descriptors (lanes of the condensation / expansion sweeps)
+    int32_t nsep;         // separators (= segments) of the item
+    int32_t pad_;
 };
 
 // Streaming-path branch descriptor (24 bytes).
@@ -49,7 +53,8 @@ struct hines_plan {
         branch_level, cell_nlevels, level_count, level_list, child_ids;
     // policy tables
     std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc;
-    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets;
+    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets, item_seg_offsets;
+    std::vector<int32_t> item_seg, item_nsep;
     std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
     std::vector<int32_t> class_blocks_per_sm;
     std::vector<int64_t> class_first, class_count;     // ranges in item_launch_order
@@ -61,7 +66,7 @@ struct hines_plan {
     std::vector<int32_t> stream_child;                 // pairs {gstart, ws}
     int64_t n_stream_cells = 0, n_stream_unknowns = 0;
     int64_t n_resident_cells = 0, n_resident_unknowns = 0;
-    int64_t padded_lane_steps = 0;
+    int64_t padded_lane_steps = 0, useful_lane_steps = 0;
 
     hines::DeviceTables* dev = nullptr;                // null until uploaded
 };

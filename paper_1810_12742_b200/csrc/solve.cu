@@ -52,7 +52,6 @@ struct DeviceTables {
         }                                                                                      \
     } while (0)
 
-static const int32_t kAtomicFlag = 1 << 30;
 
 // ------------------------------------------------------------------------------------------------
 // PTX helpers: mbarrier + 1-D TMA bulk copies (SASS: UBLKCP, SYNCS)
@@ -112,9 +111,22 @@ template <> __device__ __forceinline__ float fnma<float>(float a, float b, float
 
 // ------------------------------------------------------------------------------------------------
 // Resident kernel: one block per work item (a contiguous run of cells held in shared memory).
-// Shared-memory image (bytes): [0,16) mbarrier | sd[L] | su[L] | sb[L] | meta[meta_len]
+// Shared-memory image (bytes): [0,16) mbarrier | sd[L] | su[L] | sb[L] | topd[S] | topb[S] | meta
 //   L = landed elements = item range widened to 16-byte boundaries; compartment j of the item sits
-//   at index j + off, off = comp_begin mod (16 / sizeof(T)).
+//   at index j + off, off = comp_begin mod (16 / sizeof(T)).  S = separators rounded up.
+//
+// Three phases:
+//   P1 condense   every segment's interior a..b-1 is eliminated top-down, independently of the tree
+//                 level (one lane per segment).  Node i keeps g = u[i+1]/D, h = e/D, c = B/D where e is
+//                 the fill-in coupling to the separator t above the segment; the separator b below gets
+//                 d[b] -= g u[b], b[b] -= g B and the new coupling U = -h u[b] to t; the contributions
+//                 to t (sum h e, sum h B) are parked per separator and ride along in P2's hand-off.
+//   P2 reduced    the level-synchronous Hines sweeps of the paper on the separators
+//                 only: one lane per branch, one step per segment, block barrier per level, sibling
+//                 hand-off at branch points by warp shuffle.
+//   P3 expand     x[i] = c - g x[i+1] - h x[t] for every interior, again one lane per segment.
+// Eliminating in this order is a symmetric permutation of the same LDL^T factorisation (the matrix is
+// SPD and strictly diagonally dominant, so any order is stable without pivoting).
 // ------------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, const int32_t* __restrict__ order,
@@ -131,12 +143,15 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
     // the last item may end beyond a 16-byte boundary of the arrays: copy that remainder by hand
     const int64_t avail = n_total - g0;
     const int Lb = (int)(avail >= L ? L : (avail / E * E)); // elements brought by the bulk copies
+    const int S = (it.nsep + E - 1) / E * E;
 
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
     T* sd = reinterpret_cast<T*>(smem + 16);
     T* su = sd + L;
     T* sb = su + L;
-    int32_t* smeta = reinterpret_cast<int32_t*>(sb + L);
+    T* topd = sb + L;
+    T* topb = topd + S;
+    int32_t* smeta = reinterpret_cast<int32_t*>(topb + S);
 
     if (tid == 0) mbar_init(bar, 1);
     __syncthreads();
@@ -145,58 +160,81 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
         mbar_expect_tx(bar, 3u * bytes + (uint32_t)it.meta_len * 4u);
         tma_load_1d(smeta, meta_g + it.meta_off, (uint32_t)it.meta_len * 4u, bar);
         if (bytes) {
-            tma_load_1d(sb, b + g0, bytes, bar);
             tma_load_1d(sd, d + g0, bytes, bar);
             tma_load_1d(su, u + g0, bytes, bar);
+            tma_load_1d(sb, b + g0, bytes, bar);
         }
     }
     // remainder of the very last item (fewer than E elements), plain loads
     for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
+    for (int i = tid; i < S; i += nthreads) { topd[i] = T(0); topb[i] = T(0); }
     mbar_wait(bar, 0);
     __syncthreads();
 
     const int32_t* lvl = smeta;
-    const int32_t* desc = smeta + it.desc_off;
+    const int4* desc = reinterpret_cast<const int4*>(smeta + it.desc_off);
+    const int4* seg = reinterpret_cast<const int4*>(smeta + it.seg_off);
     const unsigned FULL = 0xffffffffu;
 
-    // ---- backward elimination, deepest level first ----
-    for (int lev = it.nlev - 1; lev >= 0; --lev) {
-        const int eb = lvl[lev], ee = lvl[lev + 1];
-        for (int base = eb + (tid & ~31); base < ee; base += nthreads) {
-            const int e = base + lane;
-            int start = 0, len = 0, pc = -1; bool atomic_handoff = false;
-            if (e < ee) {
-                start = desc[3 * e]; len = desc[3 * e + 1]; pc = desc[3 * e + 2];
-                atomic_handoff = len & kAtomicFlag; len &= ~kAtomicFlag;
+    // ---- P1: condense the interiors of all segments (no level dependency) ----
+    for (int base = (tid & ~31); base < it.nseg_lanes; base += nthreads) {
+        const int e = base + lane;
+        int4 sg = make_int4(0, 0, -1, 0);
+        if (e < it.nseg_lanes) sg = seg[e];
+        const int m = sg.y;
+        const int mmax = __reduce_max_sync(FULL, m);
+        int i = sg.x + off;
+        T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0);
+        if (m > 0) { D = sd[i]; B = sb[i]; if (sg.z >= 0) ee = su[i]; }
+        for (int s = 0; s < mmax; ++s) {
+            if (s < m) {
+                const T un = su[i + 1], dn = sd[i + 1], bn = sb[i + 1];
+                const T r = rcp<T>(D);
+                const T g = un * r, h = ee * r, c = B * r;
+                sd[i] = g; su[i] = h; sb[i] = c;
+                ddt = fnma<T>(-h, ee, ddt); dbt = fnma<T>(-h, B, dbt);
+                D = fnma<T>(g, un, dn); B = fnma<T>(g, B, bn); ee = -h * un;
+                ++i;
+                if (s == m - 1) { sd[i] = D; sb[i] = B; su[i] = ee; }     // the separator below
             }
-            const int maxlen = __reduce_max_sync(FULL, len);
-            int i = start + off + len - 1;                  // last compartment of the branch
+        }
+        if (m > 0) { topd[sg.w] = ddt; topb[sg.w] = dbt; }
+    }
+    __syncthreads();
+
+    // ---- P2 backward: reduced system, deepest level first ----
+    for (int lev = it.nlev - 1; lev >= 0; --lev) {
+        const int eb = lvl[lev], ee_ = lvl[lev + 1];
+        for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
+            const int e = base + lane;
+            int4 ds = make_int4(0, 0, -1, 0);
+            if (e < ee_) ds = desc[e];
+            const bool atomic_handoff = ds.y < 0;
+            const int nseg = ds.y & 0xfffff, sj = (ds.y >> 20) & 0x7ff, pc = ds.z;
+            const int nmax = __reduce_max_sync(FULL, nseg);
+            int i = ds.x + off;                                  // last compartment of the branch
             T D = T(1), B = T(0), dd = T(0), db = T(0);
-            if (len > 0) { D = sd[i]; B = sb[i]; }
-            for (int s = 0; s < maxlen; ++s) {              // lanes walk their branches in lock-step
-                if (s < len) {
+            if (nseg > 0) { D = sd[i]; B = sb[i]; }
+            for (int k = 0; k < nmax; ++k) {                     // lanes walk their separators in lock-step
+                if (k < nseg) {
                     const T r = rcp<T>(D);
                     const T c = B * r;
-                    if (s < len - 1) {                      // inside the branch: parent is i-1
-                        const T uk = su[i];
-                        const T f = uk * r;
+                    const bool last = k == nseg - 1;
+                    if (!last || pc >= 0) {
+                        const T U = su[i];
+                        const T f = U * r;
                         sd[i] = f; sb[i] = c;
-                        D = fnma<T>(f, uk, sd[i - 1]);
-                        B = fnma<T>(f, B, sb[i - 1]);
-                        --i;
-                    } else if (pc >= 0) {                   // first compartment: hand off to the parent branch
-                        const T uk = su[i];
-                        const T f = uk * r;
-                        sd[i] = f; sb[i] = c;
-                        dd = f * uk; db = f * B;
-                    } else {                                // root compartment: x0 = b'/d'; u[root] unread
+                        dd = fnma<T>(-f, U, topd[ds.w + k]);     // f U + parked contribution of the segment
+                        db = fnma<T>(-f, B, topb[ds.w + k]);
+                        if (!last) { i -= sj; D = sd[i] - dd; B = sb[i] - db; }
+                    } else {                                     // root of the reduced tree: x = b'/d'
                         sd[i] = T(0); sb[i] = c;
                     }
                 }
             }
             // hand-off at the branch point: siblings sit in one tile; the lowest lane of
             // each sibling group gathers the others' contributions by shuffle and updates the parent.
-            const int key = (len > 0 && pc >= 0) ? pc : -2 - lane;
+            const int key = (nseg > 0 && pc >= 0) ? pc : -2 - lane;
             const unsigned peers = __match_any_sync(FULL, key);
             const int leader = __ffs(peers) - 1;
             const int maxcnt = __reduce_max_sync(FULL, __popc(peers));
@@ -215,25 +253,45 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
         __syncthreads();
     }
 
-    // ---- forward substitution, root level first ----
+    // ---- P2 forward: root level first ----
     for (int lev = 0; lev < it.nlev; ++lev) {
-        const int eb = lvl[lev], ee = lvl[lev + 1];
-        for (int base = eb + (tid & ~31); base < ee; base += nthreads) {
+        const int eb = lvl[lev], ee_ = lvl[lev + 1];
+        for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
             const int e = base + lane;
-            int start = 0, len = 0, pc = -1;
-            if (e < ee) { start = desc[3 * e]; len = desc[3 * e + 1] & ~kAtomicFlag; pc = desc[3 * e + 2]; }
-            const int maxlen = __reduce_max_sync(FULL, len);
-            T xp = (len > 0 && pc >= 0) ? sb[pc + off] : T(0);
-            int i = start + off;
-            for (int s = 0; s < maxlen; ++s) {
-                if (s < len) {
+            int4 ds = make_int4(0, 0, -1, 0);
+            if (e < ee_) ds = desc[e];
+            const int nseg = ds.y & 0xfffff, sj = (ds.y >> 20) & 0x7ff, pc = ds.z;
+            const int nmax = __reduce_max_sync(FULL, nseg);
+            T xp = (nseg > 0 && pc >= 0) ? sb[pc + off] : T(0);
+            int i = ds.x + off - (nseg - 1) * sj;                // first (top-most) separator of the branch
+            for (int k = 0; k < nmax; ++k) {
+                if (k < nseg) {
                     xp = fnma<T>(sd[i], xp, sb[i]);
                     sb[i] = xp;
-                    ++i;
+                    i += sj;
                 }
             }
         }
         __syncthreads();
+    }
+
+    // ---- P3: expand the interiors (lanes aligned at the segment start so that the shared-memory
+    //      addresses of a wavefront keep their distinct residues) ----
+    for (int base = (tid & ~31); base < it.nseg_lanes; base += nthreads) {
+        const int e = base + lane;
+        int4 sg = make_int4(0, 0, -1, 0);
+        if (e < it.nseg_lanes) sg = seg[e];
+        const int m = sg.y;
+        const int mmax = __reduce_max_sync(FULL, m);
+        T xt = T(0), xn = T(0);
+        if (m > 0) { xn = sb[sg.x + off + m]; if (sg.z >= 0) xt = sb[sg.z + off]; }
+        for (int j = mmax - 1; j >= 0; --j) {
+            if (j < m) {
+                const int i = sg.x + off + j;
+                xn = fnma<T>(su[i], xt, fnma<T>(sd[i], xn, sb[i]));
+                sb[i] = xn;
+            }
+        }
     }
 
     // ---- store x (natural order): bulk store of the 16-byte aligned interior, edges by hand ----

@@ -15,7 +15,7 @@ import paper_1810_12742_b200 as hb
 from helpers import random_parent
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-ATOMIC = 1 << 30
+ATOMIC = -(1 << 31)      # bit 31 of the packed descriptor word (int32)
 
 
 def test_library_exports_every_declared_symbol():
@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
         assert getattr(lib, name) is not None
     assert "sm_100a" in hb.version()
     # struct sizes agree with the header's layout
-    assert ctypes.sizeof(hb.Options) == 24 and ctypes.sizeof(hb.PlanInfo) == 128
+    assert ctypes.sizeof(hb.Options) == 28 and ctypes.sizeof(hb.PlanInfo) == 128
 
 
 def _plan_cfg(cfg, scale, **kw):
@@ -92,11 +92,11 @@ def test_validation_errors():
     assert lib.hines_status_string(4) == b"CUDA error"
 
 
-def _check_policy(m, plan):
+def _check_policy(m, plan, max_segment=64):
     """Validity invariants (policy-free): every branch exactly once, all branches of a resident cell
-    in one item, sibling groups inside one 32-lane tile (or flagged), lengths non-increasing by
-    sibling-group key inside a level, parents strictly on the previous level, smem need within the
-    class, launch order a permutation."""
+    in one item, sibling groups inside one 32-lane tile (or flagged), parents strictly on the previous
+    level, segments tile every branch exactly (one separator per segment, interiors disjoint), every
+    non-empty interior listed exactly once, smem need within the class, launch order a permutation."""
     T = oracle.tables(m.parent, m.cell_offsets)
     w = 8 if plan.dtype == hb.F64 else 4
     cell_item = plan.table("cell_item")
@@ -104,7 +104,10 @@ def _check_policy(m, plan):
     desc_off = plan.table("item_desc_offsets")
     lvl_off = plan.table("item_level_offsets")
     lvl_begin = plan.table("item_level_begin")
-    desc = plan.table("item_desc").reshape(-1, 3)
+    desc = plan.table("item_desc").reshape(-1, 4)
+    seg_off = plan.table("item_seg_offsets")
+    segs = plan.table("item_seg").reshape(-1, 4)
+    nsep_tab = plan.table("item_nsep")
     cls = plan.table("item_class")
     cls_smem = plan.table("class_smem_bytes")
     order = plan.table("item_launch_order")
@@ -115,55 +118,75 @@ def _check_policy(m, plan):
     assert info.n_resident_items == nitems
     seen_cells = np.zeros(m.ncells, bool)
     useful = 0
+    nsep_total = 0
     for it in range(nitems):
         c0, c1 = rng_[it]
         assert c1 > c0 and (cell_item[c0:c1] == it).all()
         seen_cells[c0:c1] = True
         comp0 = m.cell_offsets[c0]; n_it = m.cell_offsets[c1] - comp0
         dsc = desc[desc_off[it]:desc_off[it + 1]]
+        sg = segs[seg_off[it]:seg_off[it + 1]]
         lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
         nlev = len(lb) - 1
         assert nlev == T.cell_nlevels[c0:c1].max() and lb[0] == 0 and lb[-1] == len(dsc)
-        # expected multiset of (start, len, pc, level)
-        want = set()
+        # expected set of (end, len, pc, level)
+        want = {}
         for c in range(c0, c1):
             sh = m.cell_offsets[c] - comp0
             for j in range(T.cell_branch_offsets[c], T.cell_branch_offsets[c + 1]):
                 pc = T.branch_parent_comp[j]
-                want.add((T.branch_start[j] + sh, T.branch_len[j], -1 if pc < 0 else pc + sh, T.branch_level[j]))
-        got = set()
-        level_of_comp = {}
+                want[int(T.branch_start[j] + sh + T.branch_len[j] - 1)] = (
+                    int(T.branch_len[j]), -1 if pc < 0 else int(pc + sh), int(T.branch_level[j]))
+        got = {}
+        sep_of = {}                       # separator id -> (node, top separator node or -1)
+        covered = np.zeros(n_it, int)
         for l in range(nlev):
-            seg = dsc[lb[l]:lb[l + 1]]
-            ln = seg[:, 1] & ~ATOMIC
-            real = ln > 0
-            for (s, _, pc), n_ in zip(seg[real], ln[real]):
-                assert (s, n_, pc, l) not in got
-                got.add((int(s), int(n_), int(pc), l))
-                level_of_comp[int(s) + int(n_) - 1] = l
-            # siblings share a tile unless flagged
-            pcs = seg[:, 2]
+            seg_l = dsc[lb[l]:lb[l + 1]]
+            nseg = seg_l[:, 1] & 0xfffff
+            sj = (seg_l[:, 1] >> 20) & 0x7ff
+            real = nseg > 0
+            for (end, word, pc, sbase), ns, s_ in zip(seg_l[real], nseg[real], sj[real]):
+                ln, pcw, lw = want[int(end)]
+                assert int(end) not in got and pcw == pc and lw == l
+                got[int(end)] = 1
+                assert ns == -(-ln // max_segment) and s_ == -(-ln // ns)
+                start = end - ln + 1
+                for k in range(ns):
+                    b = end - k * s_
+                    a = max(start, b - s_ + 1)
+                    t = b - s_ if k < ns - 1 else pc
+                    assert (sbase + k) not in sep_of
+                    sep_of[int(sbase + k)] = (int(a), int(b - a), int(t))
+                    covered[a:b + 1] += 1
+            pcs = seg_l[:, 2]
             for pcv in np.unique(pcs[real & (pcs >= 0)]):
                 idx = np.nonzero(real & (pcs == pcv))[0]
-                flagged = (seg[idx, 1] & ATOMIC) != 0
+                flagged = seg_l[idx, 1] < 0
                 if flagged.any():
                     assert flagged.all() and len(idx) > 32
                 else:
-                    assert idx.min() // 32 == idx.max() // 32
-                    assert (np.diff(idx) == 1).all()                  # contiguous lanes
-            # tiles: sibling-group keys (longest member) non-increasing => tile maxima non-increasing
-            tile_max = [ln[t:t + 32].max() for t in range(0, len(ln), 32)]
-            assert all(a >= b for a, b in zip(tile_max, tile_max[1:]))
-            useful += int(ln.sum())
-        assert got == want
-        for (s, n_, pc, l) in got:
+                    assert idx.min() // 32 == idx.max() // 32 and (np.diff(idx) == 1).all()
+        assert set(got) == set(want) and (covered == 1).all()
+        assert nsep_tab[it] == len(sep_of) and sorted(sep_of) == list(range(len(sep_of)))
+        # parents are separators of the level above
+        ends_level = {e: v[2] for e, v in want.items()}
+        for e, (ln, pc, l) in want.items():
             if pc >= 0:
-                assert level_of_comp[pc] == l - 1                      # parent = last compartment, level above
+                assert ends_level[pc] == l - 1
+        # segment lane list: exactly the non-empty interiors, once each
+        real = sg[:, 1] > 0
+        listed = {int(sid): (int(a), int(mm), int(t)) for a, mm, t, sid in sg[real]}
+        assert len(listed) == real.sum()
+        assert listed == {k: v for k, v in sep_of.items() if v[1] > 0}
+        useful += int(sg[real, 1].sum())
+        nsep_total += len(sep_of)
+        # wavefront groups (16 lanes fp64 / 32 lanes fp32) mostly have distinct start residues
+        R = 128 // w
         # shared-memory need within the class
         E = 16 // w
         L = -(-(comp0 % E + n_it) // E) * E
-        meta = -(-(nlev + 1) // 4) * 4 + -(-(3 * len(dsc)) // 4) * 4
-        assert 16 + 3 * L * w + 4 * meta <= cls_smem[cls[it]] <= 232448
+        meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + 4 * len(sg)
+        assert 16 + 3 * L * w + 2 * (-(-len(sep_of) // E) * E) * w + 4 * meta <= cls_smem[cls[it]] <= 232448
     assert (seen_cells == (cell_item >= 0)).all()
     # streaming path: every branch of every non-resident cell exactly once, children complete
     sd = plan.table("stream_desc").reshape(-1, 6)
@@ -191,20 +214,21 @@ def _check_policy(m, plan):
                 assert want[int(cgs)][1] == gs + ln - 1 and want[int(cgs)][2] == l + 1
                 assert cws - ws == cgs - gs                           # same cell, same shift
             useful += int(ln)
-    assert useful == m.n == info.useful_lane_steps
+    assert useful + nsep_total == m.n and useful == info.useful_lane_steps
     assert info.n_resident_unknowns + info.n_stream_unknowns == m.n
-    assert info.padded_lane_steps >= m.n
+    assert info.padded_lane_steps >= useful
 
 
 @pytest.mark.parametrize("cfg,scale,kw", [
     (0, 1.0, {}), (0, 1.0, dict(policy_flags=hb.POLICY_NO_GROUPING)),
     (2, 0.004, {}), (2, 0.004, dict(smem_bytes_per_block=60000)),
     (2, 0.003, dict(policy_flags=hb.POLICY_FORCE_STREAM)),
-    (3, 0.002, {}), (3, 0.002, dict(dtype=hb.F32)), (1, 0.002, {}),
+    (3, 0.002, {}), (3, 0.002, dict(dtype=hb.F32)), (1, 0.002, {}), (1, 0.002, dict(max_segment=7)),
+    (2, 0.003, dict(max_segment=2)), (3, 0.002, dict(max_segment=16)),
 ])
 def test_policy_tables_valid(cfg, scale, kw):
     m, plan = _plan_cfg(cfg, scale, **kw)
-    _check_policy(m, plan)
+    _check_policy(m, plan, kw.get("max_segment", 64))
 
 
 def test_policy_star_with_many_siblings_and_odd_offsets():
@@ -215,7 +239,7 @@ def test_policy_star_with_many_siblings_and_odd_offsets():
     for kw in ({}, dict(dtype=hb.F32), dict(policy_flags=hb.POLICY_NO_GROUPING)):
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
         _check_policy(m, plan)
-        assert (plan.table("item_desc").reshape(-1, 3)[:, 1] & ATOMIC).any()
+        assert (plan.table("item_desc").reshape(-1, 4)[:, 1] < 0).any()
 
 
 def test_config4_goes_to_streaming_path_and_grouping_is_greedy_in_order():
