@@ -194,6 +194,17 @@ hines_status_t hines_plan_get_table(const hines_plan_t* plan, int32_t table_id, 
 hines_status_t hines_plan_enable_timing(hines_plan_t* plan, int32_t enable);
 hines_status_t hines_plan_get_timing(hines_plan_t* plan, float* resident_ms, float* stream_ms);
 
+/* Load-imbalance / phase hook (debug; SURVEY.md §8(d) "per-work-item cycle counts").  With phase clocks
+ * enabled every shared-memory work item records, per solve, 8 x uint64: %globaltimer (ns) at
+ * [0] block start, [1] inputs landed in shared memory, [2] segment interiors condensed, [3] backward
+ * level sweeps done, [4] forward level sweeps done, [5] interiors expanded, [6] x stored;
+ * [7] = (SM id << 32) | unknowns of the item.  Rows are in launch order (HINES_TABLE_ITEM_LAUNCH_ORDER).
+ * hines_plan_get_phase_clocks synchronises the device and copies the rows of the last solve
+ * (host_dst may be NULL to query the size).  Errors: INVALID_ARG, CUDA, ALLOC. */
+hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* plan, int32_t enable);
+hines_status_t hines_plan_get_phase_clocks(hines_plan_t* plan, uint64_t* host_dst, int64_t capacity_bytes,
+                                           int64_t* needed_bytes);
+
 /* Number of kernel launches one hines_solve enqueues with this plan (bench.py's gpu_launches). */
 hines_status_t hines_plan_launches_per_solve(const hines_plan_t* plan, int32_t* out);
 

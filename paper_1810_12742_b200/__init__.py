@@ -41,6 +41,7 @@ TABLES = {
 ABI_SYMBOLS = ["hines_plan_create", "hines_plan_upload", "hines_solve", "hines_solve_host",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
+               "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
                "hines_status_string", "hines_last_error", "hines_version"]
 
 
@@ -91,6 +92,8 @@ def load_library(build_if_missing: bool = True):
     lib.hines_plan_launches_per_solve.argtypes = [vp, C.POINTER(i32)]
     lib.hines_plan_enable_timing.argtypes = [vp, i32]
     lib.hines_plan_get_timing.argtypes = [vp, C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    lib.hines_plan_enable_phase_clocks.argtypes = [vp, i32]
+    lib.hines_plan_get_phase_clocks.argtypes = [vp, vp, i64, C.POINTER(i64)]
     for f in ("hines_status_string", "hines_last_error", "hines_version"):
         getattr(lib, f).restype = C.c_char_p
     lib.hines_status_string.argtypes = [i32]
@@ -165,6 +168,18 @@ class Plan:
         a, b = C.c_float(), C.c_float()
         _check(load_library().hines_plan_get_timing(self._h, C.byref(a), C.byref(b)))
         return a.value, b.value
+
+    # hines_plan_enable_phase_clocks / hines_plan_get_phase_clocks
+    def enable_phase_clocks(self, enable=True):
+        _check(load_library().hines_plan_enable_phase_clocks(self._h, int(bool(enable))))
+
+    def phase_clocks(self) -> np.ndarray:
+        """uint64[nitems, 8] of the last solve (launch order); waits for the device."""
+        need = C.c_int64()
+        _check(load_library().hines_plan_get_phase_clocks(self._h, None, 0, C.byref(need)))
+        out = np.zeros(need.value // 8, dtype=np.uint64)
+        _check(load_library().hines_plan_get_phase_clocks(self._h, out.ctypes.data, need.value, C.byref(need)))
+        return out.reshape(-1, 8)
 
     def upload(self):
         _check(load_library().hines_plan_upload(self._h))

@@ -40,6 +40,8 @@ struct DeviceTables {
     void* host_stage[4] = {nullptr, nullptr, nullptr, nullptr};   // hines_solve_host device buffers d,u,b,x
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};              // timing hook
     bool timing = false, timed_once = false;
+    unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident item, launch order
+    bool prof_on = false;
     int64_t bytes = 0;
 };
 
@@ -101,6 +103,19 @@ __device__ __forceinline__ void fence_proxy_async()
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
 
+__device__ __forceinline__ unsigned long long globaltimer_ns()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ unsigned smid()
+{
+    unsigned r;
+    asm volatile("mov.u32 %0, %smid;" : "=r"(r));
+    return r;
+}
+
 template <typename T> __device__ __forceinline__ T rcp(T v);
 template <> __device__ __forceinline__ double rcp<double>(double v) { return 1.0 / v; }
 template <> __device__ __forceinline__ float rcp<float>(float v) { return 1.0f / v; }
@@ -131,9 +146,14 @@ template <> __device__ __forceinline__ float fnma<float>(float a, float b, float
 template <typename T>
 __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, const int32_t* __restrict__ order,
                                       const int32_t* __restrict__ meta_g, const T* __restrict__ d,
-                                      const T* __restrict__ u, const T* __restrict__ b, T* x, int64_t n_total)
+                                      const T* __restrict__ u, const T* __restrict__ b, T* x, int64_t n_total,
+                                      unsigned long long* prof)
 {
     extern __shared__ __align__(128) unsigned char smem[];
+    // phase clocks (debug hook, prof == nullptr in normal runs): thread 0 stamps %globaltimer
+    unsigned long long stamp[7];
+#define HINES_STAMP(k) do { if (prof && threadIdx.x == 0) stamp[k] = globaltimer_ns(); } while (0)
+    HINES_STAMP(0);
     constexpr int E = 16 / (int)sizeof(T);
     const ItemHeader it = items[order[blockIdx.x]];
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
@@ -170,6 +190,7 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
     for (int i = tid; i < S; i += nthreads) { topd[i] = T(0); topb[i] = T(0); }
     mbar_wait(bar, 0);
     __syncthreads();
+    HINES_STAMP(1);
 
     const int32_t* lvl = smeta;
     const int4* desc = reinterpret_cast<const int4*>(smeta + it.desc_off);
@@ -201,6 +222,7 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
         if (m > 0) { topd[sg.w] = ddt; topb[sg.w] = dbt; }
     }
     __syncthreads();
+    HINES_STAMP(2);
 
     // ---- P2 backward: reduced system, deepest level first ----
     for (int lev = it.nlev - 1; lev >= 0; --lev) {
@@ -253,6 +275,7 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
         __syncthreads();
     }
 
+    HINES_STAMP(3);
     // ---- P2 forward: root level first ----
     for (int lev = 0; lev < it.nlev; ++lev) {
         const int eb = lvl[lev], ee_ = lvl[lev + 1];
@@ -275,6 +298,7 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
         __syncthreads();
     }
 
+    HINES_STAMP(4);
     // ---- P3: expand the interiors (lanes aligned at the segment start so that the shared-memory
     //      addresses of a wavefront keep their distinct residues) ----
     for (int base = (tid & ~31); base < it.nseg_lanes; base += nthreads) {
@@ -299,12 +323,20 @@ __global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, cons
     const int tail_begin = max(head_end, (int)(((off + it.n) / E) * E) - off);   // item-local [tail_begin, n)
     fence_proxy_async();
     __syncthreads();
+    HINES_STAMP(5);
     if (tid == 0 && tail_begin > head_end) {
         tma_store_1d(x + it.comp_begin + head_end, sb + off + head_end, (uint32_t)(tail_begin - head_end) * sizeof(T));
         tma_store_commit_wait();
     }
     for (int j = tid; j < head_end; j += nthreads) x[it.comp_begin + j] = sb[off + j];
     for (int j = tail_begin + tid; j < it.n; j += nthreads) x[it.comp_begin + j] = sb[off + j];
+    if (prof && tid == 0) {
+        stamp[6] = globaltimer_ns();
+        unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
+        for (int k = 0; k < 7; ++k) o[k] = stamp[k];
+        o[7] = ((unsigned long long)smid() << 32) | (unsigned)it.n;
+    }
+#undef HINES_STAMP
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -375,7 +407,7 @@ static void free_device(DeviceTables* D)
 {
     if (!D) return;
     cudaFree(D->items); cudaFree(D->launch_order); cudaFree(D->item_meta); cudaFree(D->stream_desc);
-    cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c);
+    cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
     delete D;
@@ -439,7 +471,8 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         const int64_t cnt = P->class_count[q];
         if (!cnt) continue;
         hines_resident_kernel<T><<<(unsigned)cnt, nthreads, P->class_smem_bytes[q], stream>>>(
-            D->items, D->launch_order + P->class_first[q], D->item_meta, d, u, b, x, P->n);
+            D->items, D->launch_order + P->class_first[q], D->item_meta, d, u, b, x, P->n,
+            D->prof_on ? D->prof + 8 * P->class_first[q] : nullptr);
     }
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
     const int nlev = (int)P->stream_level_begin.size() - 1;
@@ -533,6 +566,35 @@ hines_status_t hines_plan_get_timing(hines_plan_t* P, float* resident_ms, float*
     CUDA_TRY(cudaEventSynchronize(D->ev[2]));
     CUDA_TRY(cudaEventElapsedTime(resident_ms, D->ev[0], D->ev[1]));
     CUDA_TRY(cudaEventElapsedTime(stream_ms, D->ev[1], D->ev[2]));
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* P, int32_t enable)
+{
+    if (!P) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    hines_status_t st = upload(P);
+    if (st != HINES_OK) return st;
+    DeviceTables* D = P->dev;
+    const size_t bytes = P->item_headers.size() * 8 * sizeof(unsigned long long);
+    if (enable && !D->prof && bytes) {
+        CUDA_TRY(cudaMalloc(&D->prof, bytes));
+        CUDA_TRY(cudaMemset(D->prof, 0, bytes));
+        D->bytes += (int64_t)bytes;
+    }
+    D->prof_on = enable != 0 && D->prof;
+    return HINES_OK;
+}
+
+hines_status_t hines_plan_get_phase_clocks(hines_plan_t* P, uint64_t* host_dst, int64_t capacity_bytes, int64_t* needed_bytes)
+{
+    if (!P || !needed_bytes) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    const int64_t bytes = (int64_t)(P->item_headers.size() * 8 * sizeof(unsigned long long));
+    *needed_bytes = bytes;
+    if (!host_dst) return HINES_OK;
+    if (!P->dev || !P->dev->prof) { set_error("phase clocks not enabled"); return HINES_ERR_INVALID_ARG; }
+    if (capacity_bytes < bytes) { set_error("buffer too small"); return HINES_ERR_INVALID_ARG; }
+    CUDA_TRY(cudaDeviceSynchronize());
+    CUDA_TRY(cudaMemcpy(host_dst, P->dev->prof, (size_t)bytes, cudaMemcpyDeviceToHost));
     return HINES_OK;
 }
 
