@@ -54,13 +54,16 @@ enum {
     HINES_POLICY_DEFAULT      = 0,
     HINES_POLICY_FORCE_STREAM = 1,   /* every cell through the streaming (global-memory) path           */
     HINES_POLICY_NO_GROUPING  = 2,   /* one cell per shared-memory work item (paper: >= 1 cell per block) */
-    HINES_POLICY_INPUT_ORDER  = 4    /* launch work items in input order, not heaviest first (PAPER.md:128
+    HINES_POLICY_INPUT_ORDER  = 4,   /* launch work items in input order, not heaviest first (PAPER.md:128
                                         "greedy": cells are taken in the order given)                     */
+    HINES_POLICY_NO_CLUSTER   = 8    /* never spread a cell over a thread-block cluster: a cell either fits one
+                                        block's shared memory or goes to the streaming path               */
 };
 
 typedef struct {
     int32_t struct_size;            /* = sizeof(hines_options_t); lets the struct grow                     */
-    int32_t threads_per_block;      /* 0 = default (256); multiple of 32, <= 1024                          */
+    int32_t threads_per_block;      /* 0 = default (per size class: one lane per segment of the widest work item,
+                                       128..1024, within the register file); else multiple of 32, <= 1024  */
     int32_t smem_bytes_per_block;   /* 0 = default (227 KiB: sm_100 opt-in maximum); upper bound for the
                                        shared memory one resident work item may use                       */
     int32_t policy_flags;           /* HINES_POLICY_*                                                      */
@@ -70,6 +73,11 @@ typedef struct {
                                        block as possible")                                                 */
     int32_t max_segment;            /* 0 = default (64), 2..2047: branches longer than this are cut into
                                        chained segments ("we split branches that are too long") */
+    int32_t cluster_max;            /* 0 = default (8), 1..16: largest thread-block cluster a cell may be spread
+                                       over (powers of two are used; 16 needs the non-portable cluster size)  */
+    int32_t chunk_smem_bytes;       /* 0 = default (113 KiB, two blocks per SM): shared memory one block of a
+                                       cluster item aims to stay within; also the size above which a cell is
+                                       spread over a cluster instead of taking a whole SM's shared memory      */
 } hines_options_t;
 
 typedef struct {
@@ -93,7 +101,10 @@ typedef struct {
                                    (PAPER.md:138); the roofline numerator                                  */
     int64_t bytes_literal;      /* n*(4*w + 4): one parent per compartment (Listing 2 as printed)          */
     int32_t breadth_first;      /* 1 if every cell's branches are numbered level by level    */
-    int32_t n_classes;          /* shared-memory size classes in use                                       */
+    int32_t n_classes;          /* size classes in use = resident kernel launches per solve                */
+    int64_t n_cluster_cells;    /* cells spread over a thread-block cluster (counted in n_resident_* too)  */
+    int64_t n_cluster_unknowns;
+    int64_t n_chunks;           /* blocks the resident launches start per solve                            */
 } hines_plan_info_t;
 
 /* Canonical, policy-free tables (bit-exact against the table oracle); all indices cell-local.
@@ -111,28 +122,39 @@ typedef enum {
     HINES_TABLE_LEVEL_LIST           = 9,   /* int32[nbranches]  per cell: ids by (level, length desc, id)  */
     HINES_TABLE_CHILD_OFFSETS        = 10,  /* int64[nbranches+1] CSR over global branch index              */
     HINES_TABLE_CHILD_IDS            = 11,  /* int32[nbranches-ncells] ascending                            */
-    /* Policy tables (depend on options; validity-checked in tests) */
-    HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  resident work item of the cell, -1 = streaming path     */
+    /* Policy tables (depend on options; validity-checked in tests).
+     * A work item is a run of whole cells in ONE block's shared memory, or one cell cut into the chunks
+     * of a thread-block cluster.  Its reduced tree has one node per segment (the segment's last
+     * compartment, the "separator"); node ids are item-local: the top node of the branch in lane e has
+     * id e, the other nodes of a branch with nseg > 1 have ids rest, rest+1, ... from the top. */
+    HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  on-chip work item of the cell, -1 = streaming path       */
     HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
-    HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  shared-memory size class                                */
+    HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  size class                                              */
     HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
-    HINES_TABLE_ITEM_DESC_OFFSETS    = 36,  /* int64[nitems+1] into ITEM_DESC (in units of descriptors)               */
+    HINES_TABLE_ITEM_DESC_OFFSETS    = 36,  /* int64[nitems+1] into ITEM_DESC / ITEM_PNODE (in units of lanes)        */
     HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
-    HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] descriptor index (item-local) where each
-                                               level's lane list begins                                               */
-    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*ndesc] per branch {end = last compartment (item-local),
-                                               nseg | Sj<<20 | spans-tiles flag<<31, parent compartment (item-local,
-                                               -1 = root branch), first separator id}; nseg = 0 marks a padding lane   */
-    HINES_TABLE_ITEM_SEG_OFFSETS     = 44,  /* int64[nitems+1] into ITEM_SEG (in units of descriptors)                */
-    HINES_TABLE_ITEM_SEG             = 45,  /* int32[4*nseglanes] per segment with a non-empty interior {a = first
-                                               interior compartment, m = interior length, t = separator above (-1 = none),
-                                               separator id}; m = 0 marks a padding lane                               */
-    HINES_TABLE_ITEM_NSEP            = 46,  /* int32[nitems] separators (= segments) per item                          */
+    HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] lane index (item-local) where each level's
+                                               lane list begins                                                        */
+    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane {nseg | nafter<<16 | tile max nafter<<24,
+                                               rest, cfirst, nlead | tile max nseg<<16}: nseg = 0 marks a padding lane;
+                                               nafter = sibling lanes to the right whose hand-off values this lane
+                                               absorbs by warp shuffle; cfirst, nlead = the hand-off slots (lane ids)
+                                               the branch's last node pulls from                                       */
+    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[nlanes] last node of the parent branch, -1 = root branch / padding */
+    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] node ids in use (>= lanes)                                 */
+    HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
+    HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
+    HINES_TABLE_CHUNK_SEG_OFFSETS    = 48,  /* int64[nchunks+1] into CHUNK_SEG (in units of descriptors)                */
+    HINES_TABLE_CHUNK_SEG            = 49,  /* int32[4*nseglanes] per segment {a = first compartment (chunk-local),
+                                               m = interior length (separator = a+m), node, node of the separator above
+                                               (-1 = none)}; node = -1 marks a padding lane                             */
     HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
     HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment
                                                (-1 root), workspace start, child_begin, nchild}                       */
     HINES_TABLE_STREAM_CHILD         = 42,  /* int32[2*nstream_children] {global start, workspace start} of each child */
-    HINES_TABLE_CLASS_SMEM_BYTES     = 43   /* int32[n_classes] dynamic shared memory per block of each class          */
+    HINES_TABLE_CLASS_SMEM_BYTES     = 43,  /* int32[n_classes] dynamic shared memory per block of each class          */
+    HINES_TABLE_CLASS_CLUSTER        = 50,  /* int32[n_classes] blocks per item = cluster size (1 = no cluster)        */
+    HINES_TABLE_CLASS_THREADS        = 51   /* int32[n_classes] threads per block                                      */
 } hines_table_id_t;
 
 /*

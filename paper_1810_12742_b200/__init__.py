@@ -18,7 +18,7 @@ import numpy as np
 from ._build import LIB as _LIB_PATH, build as build_library
 
 F64, F32 = 0, 1
-POLICY_DEFAULT, POLICY_FORCE_STREAM, POLICY_NO_GROUPING, POLICY_INPUT_ORDER = 0, 1, 2, 4
+POLICY_DEFAULT, POLICY_FORCE_STREAM, POLICY_NO_GROUPING, POLICY_INPUT_ORDER, POLICY_NO_CLUSTER = 0, 1, 2, 4, 8
 
 STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",
           4: "HINES_ERR_CUDA", 5: "HINES_ERR_UNSUPPORTED"}
@@ -33,8 +33,9 @@ TABLES = {
     "item_launch_order": (35, np.int32), "item_desc_offsets": (36, np.int64),
     "item_level_offsets": (37, np.int64), "item_level_begin": (38, np.int32), "item_desc": (39, np.int32),
     "stream_level_begin": (40, np.int64), "stream_desc": (41, np.int32), "stream_child": (42, np.int32),
-    "class_smem_bytes": (43, np.int32), "item_seg_offsets": (44, np.int64), "item_seg": (45, np.int32),
-    "item_nsep": (46, np.int32),
+    "class_smem_bytes": (43, np.int32), "item_pnode": (44, np.int32), "item_nnode": (45, np.int32),
+    "item_chunk_offsets": (46, np.int64), "chunk_comp_range": (47, np.int64), "chunk_seg_offsets": (48, np.int64),
+    "chunk_seg": (49, np.int32), "class_cluster": (50, np.int32), "class_threads": (51, np.int32),
 }
 
 # every symbol include/hines.h declares
@@ -48,7 +49,8 @@ ABI_SYMBOLS = ["hines_plan_create", "hines_plan_upload", "hines_solve", "hines_s
 class Options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("threads_per_block", C.c_int32),
                 ("smem_bytes_per_block", C.c_int32), ("policy_flags", C.c_int32),
-                ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32), ("max_segment", C.c_int32)]
+                ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32), ("max_segment", C.c_int32),
+                ("cluster_max", C.c_int32), ("chunk_smem_bytes", C.c_int32)]
 
 
 class PlanInfo(C.Structure):
@@ -59,7 +61,8 @@ class PlanInfo(C.Structure):
                 ("n_stream_unknowns", C.c_int64), ("n_stream_branches", C.c_int64),
                 ("padded_lane_steps", C.c_int64), ("useful_lane_steps", C.c_int64),
                 ("workspace_bytes", C.c_int64), ("bytes_min", C.c_int64), ("bytes_literal", C.c_int64),
-                ("breadth_first", C.c_int32), ("n_classes", C.c_int32)]
+                ("breadth_first", C.c_int32), ("n_classes", C.c_int32),
+                ("n_cluster_cells", C.c_int64), ("n_cluster_unknowns", C.c_int64), ("n_chunks", C.c_int64)]
 
 
 class HinesError(RuntimeError):
@@ -123,12 +126,13 @@ class Plan:
     """hines_plan_create(parent arrays, cell offsets) -- setup-time scheduler."""
 
     def __init__(self, parent, cell_offsets, dtype=F64, threads_per_block=0, smem_bytes_per_block=0,
-                 policy_flags=0, stream_threads=0, group_smem_bytes=0, max_segment=0):
+                 policy_flags=0, stream_threads=0, group_smem_bytes=0, max_segment=0, cluster_max=0,
+                 chunk_smem_bytes=0):
         lib = load_library()
         parent = np.ascontiguousarray(parent, dtype=np.int32)
         offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
         opt = Options(C.sizeof(Options), threads_per_block, smem_bytes_per_block, policy_flags,
-                      stream_threads, group_smem_bytes, max_segment)
+                      stream_threads, group_smem_bytes, max_segment, cluster_max, chunk_smem_bytes)
         h = C.c_void_p()
         self._h = None
         _check(lib.hines_plan_create(parent.ctypes.data, offs.ctypes.data, len(offs) - 1, int(dtype),
@@ -174,7 +178,7 @@ class Plan:
         _check(load_library().hines_plan_enable_phase_clocks(self._h, int(bool(enable))))
 
     def phase_clocks(self) -> np.ndarray:
-        """uint64[nitems, 8] of the last solve (launch order); waits for the device."""
+        """uint64[nblocks, 8] of the last solve (launch order); waits for the device."""
         need = C.c_int64()
         _check(load_library().hines_plan_get_phase_clocks(self._h, None, 0, C.byref(need)))
         out = np.zeros(need.value // 8, dtype=np.uint64)

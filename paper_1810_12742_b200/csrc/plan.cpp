@@ -11,12 +11,14 @@
 //          into a Cuda block any longer, we start a new Cuda block"); the fit test here is bytes of
 //          shared memory instead of "branches per level <= threads", because a B200 block loops over
 //          a level's lane list and is limited by its 227 KB of shared memory, not its thread count.
-//          Cells that do not fit any block go to the streaming path (the paper has no such path:
-//          PAPER.md:114 requires one matrix per block).
-//   P3     per (item, level): lane list of the level-synchronous part.  Sibling branches (same parent
-//          compartment) are kept in one 32-lane tile so the hand-off at the branch point
-//           is a warp shuffle; sibling groups are sorted by their longest member,
-//          descending (Fig 4.1).
+//          A cell too large for one block is cut into chunks held by the blocks of one thread-block
+//          cluster (the paper requires one matrix per block; distributed shared memory
+//          lifts that).  Cells that fit no cluster go to the streaming path.
+//   P3     per (item, level): lane list of the level-synchronous part, one lane per branch.  Sibling
+//          branches are kept in one 32-lane tile so their hand-off values at the branch point
+//           are summed by warp shuffles; sibling groups are sorted by their longest
+//          member, descending (Fig 4.1).  The parent pulls the sum from the slot of
+//          the group's first lane.
 //   P4     segments.  Every branch is cut, from its end, into nseg = ceil(len / max_segment) segments
 //          of Sj = ceil(len / nseg) compartments (the paper's branch splitting, with a
 //          fixed bound instead of the level average).  The last compartment of a segment is its
@@ -41,9 +43,10 @@ void set_error(const std::string& msg) { g_last_error = msg; }
 
 static const int64_t kSmemPerSM = 233472;       // 228 KiB
 static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
-static const int32_t kAtomicFlag = (int32_t)0x80000000u;   // descriptor bit 31: sibling group spans tiles
 static const int kClassK[] = {1, 2, 3, 4, 6, 8};
 static const int kNumClassK = 6;
+static const int kRegsPerThread = 64;           // __launch_bounds__ of the resident kernel
+static const int kMaxClusterClass = 16;
 
 static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
@@ -53,145 +56,244 @@ static int64_t class_cap(int k, int64_t max_smem)
     return std::min(cap, max_smem);
 }
 
-struct Entry { int32_t start, len, pc, ord; int64_t key; int32_t nseg, sj, sep_base; };
-
-// Lane lists of one work item (cells [c0,c1)), policies P3 + P4.
-struct ItemBuild {
-    int64_t comp_begin = 0, n = 0;
-    int32_t nlev = 0, nsep = 0;
-    std::vector<int32_t> level_begin;   // nlev+1, in branch descriptors
-    std::vector<int32_t> desc;          // 4 per branch descriptor: {end, nseg | sj<<20 | flag, pc, sep_base}
-    std::vector<int32_t> seg;           // 4 per segment descriptor: {a, m, t, sep_id}; m = 0 is a padding lane
-    int64_t padded_steps = 0;           // lane-steps of the segment sweeps incl. idle lanes
-    int64_t smem_need = 0;
+// One branch of the item while its lists are built.
+struct Br {
+    int32_t start, len, pc, level, parent;   // item-local positions; parent = index into the item's branch array
+    int32_t nseg, sj;                        // segments, compartments per segment (the first may be shorter)
+    int32_t e = -1, rest = -1;               // lane index (= id of the top node); id of the second node from the top
+    int32_t cfirst = 0, nlead = 0;           // hand-off slots the branch's last node pulls from
+    int32_t nafter = 0;                      // siblings to the right whose contributions this lane absorbs by shuffle
 };
 
-static void build_item(const hines_plan& P, int64_t c0, int64_t c1, ItemBuild& out)
-{
-    const int32_t smax = P.opt.max_segment;
-    out.comp_begin = P.cell_offsets[c0];
-    out.n = P.cell_offsets[c1] - out.comp_begin;
-    out.nlev = 0;
-    for (int64_t c = c0; c < c1; ++c) out.nlev = std::max(out.nlev, P.cell_nlevels[c]);
-    std::vector<std::vector<Entry>> lv(out.nlev);
-    int32_t ord = 0, nsep = 0;
-    struct Seg { int32_t a, m, t, sid; };
-    std::vector<Seg> segs;
-    for (int64_t c = c0; c < c1; ++c) {
-        const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
-        const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
-        for (int64_t j = b0; j < b1; ++j, ++ord) {
-            Entry e;
-            e.start = P.branch_start[j] + shift;
-            e.len = P.branch_len[j];
-            e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
-            e.ord = ord;                                    // (cell, branch id) order
-            e.key = e.pc >= 0 ? (int64_t)e.pc : -(int64_t)ord - 1;   // roots are singletons
-            e.nseg = (e.len + smax - 1) / smax;
-            e.sj = (e.len + e.nseg - 1) / e.nseg;
-            e.sep_base = nsep;
-            const int32_t end = e.start + e.len - 1;
-            for (int32_t k = 0; k < e.nseg; ++k) {          // segments counted from the branch's end
-                const int32_t b = end - k * e.sj;
-                const int32_t a = std::max(e.start, b - e.sj + 1);
-                const int32_t t = k < e.nseg - 1 ? b - e.sj : e.pc;
-                if (b - a > 0) segs.push_back({a, b - a, t, nsep + k});
-            }
-            nsep += e.nseg;
-            lv[P.branch_level[j]].push_back(e);
-        }
-    }
-    out.nsep = nsep;
-    out.level_begin.assign(out.nlev + 1, 0);
-    out.desc.clear();
-    struct Group { int32_t first, count, maxseg, minord; };
-    std::vector<Group> groups;
-    for (int32_t l = 0; l < out.nlev; ++l) {
-        auto& v = lv[l];
-        // siblings contiguous; inside a group: segment count descending, then (cell, id)
-        std::sort(v.begin(), v.end(), [](const Entry& a, const Entry& b) {
-            if (a.key != b.key) return a.key < b.key;
-            if (a.nseg != b.nseg) return a.nseg > b.nseg;
-            return a.ord < b.ord;
-        });
-        groups.clear();
-        for (int32_t i = 0; i < (int32_t)v.size();) {
-            int32_t j = i, mo = v[i].ord;
-            while (j < (int32_t)v.size() && v[j].key == v[i].key) { mo = std::min(mo, v[j].ord); ++j; }
-            groups.push_back({i, j - i, v[i].nseg, mo});
-            i = j;
-        }
-        // groups by their longest member (in level-synchronous steps) descending
-        std::sort(groups.begin(), groups.end(), [](const Group& a, const Group& b) {
-            if (a.maxseg != b.maxseg) return a.maxseg > b.maxseg;
-            return a.minord < b.minord;
-        });
-        out.level_begin[l] = (int32_t)(out.desc.size() / 4);
-        int32_t pos = 0;
-        for (const Group& g : groups) {
-            const bool spans = g.count > 32;
-            if (!spans && (pos % 32) + g.count > 32) {          // keep the sibling group in one tile
-                while (pos % 32) { out.desc.insert(out.desc.end(), {0, 0, -1, 0}); ++pos; }
-            }
-            for (int32_t i = 0; i < g.count; ++i) {
-                const Entry& e = v[g.first + i];
-                out.desc.push_back(e.start + e.len - 1);
-                out.desc.push_back(e.nseg | (e.sj << 20) | (spans ? kAtomicFlag : 0));
-                out.desc.push_back(e.pc);
-                out.desc.push_back(e.sep_base);
-                ++pos;
-            }
-        }
-    }
-    out.level_begin[out.nlev] = (int32_t)(out.desc.size() / 4);
+// Lists of one work item: cells [c0,c1) in nchunks chunks, policies P3 + P4.
+struct ItemBuild {
+    int64_t comp_begin = 0, n = 0;
+    int32_t nlev = 0, ndesc = 0, nnode = 0, nchunks = 1;
+    bool ok = true;                          // false: a field overflows its descriptor bits -> streaming path
+    std::vector<int32_t> level_begin;        // nlev+1, in branch lanes
+    std::vector<int32_t> desc;               // 4 per branch lane
+    std::vector<int32_t> pnode;              // 1 per branch lane: last node of the parent branch, -1 = root / padding
+    struct Chunk {
+        int32_t begin = 0, n = 0;            // item-local compartment range
+        std::vector<int32_t> seg;            // 4 per segment lane {a (chunk-local), m, node, tnode}; node = -1 padding
+        int64_t smem_need = 0;
+    };
+    std::vector<Chunk> chunks;
+    int64_t padded_steps = 0, useful_steps = 0;
+    int64_t leader_extra = 0;                // bytes of the reduced arrays + item metadata (rank 0 only)
+    int64_t smem_need = 0;                   // max over the chunks (rank 0 includes leader_extra)
+    int32_t max_lanes = 0;                   // widest segment lane list of a chunk
+};
 
-    // P4: segment lane list.  R lanes access shared memory in one wavefront (16 x 8 B or 32 x 4 B);
-    // give them distinct start residues mod R (then they stay distinct while all lanes advance in
-    // lock-step) and similar lengths: bucket by residue, each bucket longest first, one round = the
-    // heads of all buckets, topped up from the fullest buckets when some are exhausted.
-    const int R = 128 / P.width;
-    std::vector<std::vector<Seg>> bucket(R);
-    for (const Seg& sg : segs) bucket[sg.a % R].push_back(sg);
+struct SegTmp { int32_t a, m, node, tnode; };
+
+// Segment lane list of one chunk.  R lanes access shared memory in one wavefront (16 x 8 B or
+// 32 x 4 B); give them distinct start residues mod R (they stay distinct while all lanes advance in
+// lock-step) and similar lengths: bucket by residue, each bucket longest first, one round = the heads
+// of all buckets, topped up from the fullest buckets when some are exhausted.
+static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
+{
+    std::vector<std::vector<SegTmp>> bucket(R);
+    for (const SegTmp& sg : segs) bucket[(sg.a + off) % R].push_back(sg);
     for (auto& bk : bucket)
-        std::stable_sort(bk.begin(), bk.end(), [](const Seg& x, const Seg& y) { return x.m > y.m; });
+        std::stable_sort(bk.begin(), bk.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
     std::vector<size_t> head(R, 0);
     size_t remaining = segs.size();
-    out.seg.clear();
+    out.clear();
     std::vector<int> pick;
+    std::vector<int> used(R);
     while (remaining) {
         pick.clear();
         for (int r = 0; r < R; ++r) if (head[r] < bucket[r].size()) pick.push_back(r);
         size_t taken = pick.size();
+        std::fill(used.begin(), used.end(), 0);
+        for (int q : pick) used[q]++;
         // top up: second helpings from the buckets with most left (conflicts only in these tail rounds)
         while (taken < (size_t)R && taken < remaining) {
             int best = -1; size_t left = 0;
             for (int r = 0; r < R; ++r) {
-                size_t used = 0;
-                for (int q : pick) used += (q == r);
-                const size_t l = bucket[r].size() - head[r] > used ? bucket[r].size() - head[r] - used : 0;
+                const size_t avail = bucket[r].size() - head[r];
+                const size_t l = avail > (size_t)used[r] ? avail - used[r] : 0;
                 if (l > left) { left = l; best = r; }
             }
             if (best < 0) break;
-            pick.push_back(best); ++taken;
+            pick.push_back(best); used[best]++; ++taken;
         }
+        // longest first inside the round as well, so that the final order is close to length-descending
         for (int r : pick) {
-            const Seg& sg = bucket[r][head[r]++];
-            out.seg.insert(out.seg.end(), {sg.a, sg.m, sg.t, sg.sid});
+            const SegTmp& sg = bucket[r][head[r]++];
+            out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
             --remaining;
         }
-        if (remaining) while ((out.seg.size() / 4) % R) out.seg.insert(out.seg.end(), {0, 0, -1, 0});
+        if (remaining) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
     }
-    out.padded_steps = 0;
-    const int32_t ns = (int32_t)(out.seg.size() / 4);
-    for (int32_t t = 0; t < ns; t += 32) {
-        int32_t mx = 0;
-        for (int32_t i = t; i < std::min(ns, t + 32); ++i) mx = std::max(mx, out.seg[4 * i + 1]);
-        out.padded_steps += 32 * (int64_t)mx;
+}
+
+static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchunks, ItemBuild& out)
+{
+    const int32_t smax = P.opt.max_segment;
+    const int E = 16 / P.width, R = 128 / P.width;
+    out = ItemBuild();
+    out.nchunks = nchunks;
+    out.comp_begin = P.cell_offsets[c0];
+    out.n = P.cell_offsets[c1] - out.comp_begin;
+    for (int64_t c = c0; c < c1; ++c) out.nlev = std::max(out.nlev, P.cell_nlevels[c]);
+    const int64_t B0 = P.cell_branch_offsets[c0];
+    const int32_t nb = (int32_t)(P.cell_branch_offsets[c1] - B0);
+    std::vector<Br> br(nb);
+    std::vector<std::vector<int32_t>> lv(out.nlev);
+    for (int64_t c = c0; c < c1; ++c) {
+        const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
+        const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
+        for (int64_t j = b0; j < b1; ++j) {
+            Br& e = br[j - B0];
+            e.start = P.branch_start[j] + shift;
+            e.len = P.branch_len[j];
+            e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
+            e.level = P.branch_level[j];
+            e.parent = P.branch_parent_branch[j] < 0 ? -1 : (int32_t)(b0 + P.branch_parent_branch[j] - B0);
+            e.nseg = (e.len + smax - 1) / smax;
+            e.sj = (e.len + e.nseg - 1) / e.nseg;
+            if (e.nseg > 0xffff) out.ok = false;
+            lv[e.level].push_back((int32_t)(j - B0));
+        }
     }
-    const int E = 16 / P.width;
-    const int64_t L = round_up(out.comp_begin % E + out.n, E);
-    const int64_t meta = round_up(out.nlev + 1, 4) + (int64_t)out.desc.size() + (int64_t)out.seg.size();
-    out.smem_need = 16 + 3 * L * P.width + 2 * round_up(out.nsep, E) * P.width + meta * 4;
+    // ---- P3: lane lists of the level-synchronous part -----------------------------------------
+    // Sibling branches (same parent branch) are contiguous and, when there are at most 32 of them,
+    // inside one 32-lane tile (tiles counted from the level's first lane), so that their hand-off
+    // values are summed by warp shuffles; sibling groups are ordered by their longest member in
+    // level-synchronous steps, descending, ties by (cell, branch id).
+    out.level_begin.assign(out.nlev + 1, 0);
+    std::vector<int32_t> lane_br;                       // branch of every lane, -1 = padding
+    struct Group { int32_t first, count, maxseg, minord; };
+    std::vector<Group> groups;
+    for (int32_t l = 0; l < out.nlev; ++l) {
+        auto& v = lv[l];
+        auto key = [&](int32_t i) { return br[i].parent >= 0 ? (int64_t)br[i].parent : -(int64_t)i - 1; };
+        std::sort(v.begin(), v.end(), [&](int32_t a, int32_t b) {
+            if (key(a) != key(b)) return key(a) < key(b);
+            if (br[a].nseg != br[b].nseg) return br[a].nseg > br[b].nseg;
+            return a < b;
+        });
+        groups.clear();
+        for (int32_t i = 0; i < (int32_t)v.size();) {
+            int32_t j = i, mo = v[i];
+            while (j < (int32_t)v.size() && key(v[j]) == key(v[i])) { mo = std::min(mo, v[j]); ++j; }
+            groups.push_back({i, j - i, br[v[i]].nseg, mo});
+            i = j;
+        }
+        std::sort(groups.begin(), groups.end(), [](const Group& a, const Group& b) {
+            if (a.maxseg != b.maxseg) return a.maxseg > b.maxseg;
+            return a.minord < b.minord;
+        });
+        const int32_t lb = (int32_t)lane_br.size();
+        out.level_begin[l] = lb;
+        for (const Group& g : groups) {
+            const bool shuffled = g.count <= 32;
+            int32_t pos = (int32_t)lane_br.size() - lb;
+            if (shuffled && (pos % 32) + g.count > 32)
+                while (pos % 32) { lane_br.push_back(-1); ++pos; }
+            const int32_t first_lane = (int32_t)lane_br.size();
+            for (int32_t i = 0; i < g.count; ++i) {
+                Br& e = br[v[g.first + i]];
+                e.e = (int32_t)lane_br.size();
+                e.nafter = shuffled ? g.count - 1 - i : 0;
+                lane_br.push_back(v[g.first + i]);
+            }
+            const int32_t par = br[v[g.first]].parent;
+            if (par >= 0) {
+                br[par].cfirst = first_lane;
+                br[par].nlead = shuffled ? 1 : g.count;
+                if (g.count > 0xffff) out.ok = false;
+            }
+        }
+    }
+    out.ndesc = (int32_t)lane_br.size();
+    out.level_begin[out.nlev] = out.ndesc;
+    int32_t next_id = out.ndesc;
+    for (int32_t e = 0; e < out.ndesc; ++e) {
+        if (lane_br[e] < 0) continue;
+        Br& b = br[lane_br[e]];
+        if (b.nseg > 1) { b.rest = next_id; next_id += b.nseg - 1; }
+    }
+    out.nnode = next_id;
+    auto last_node = [&](const Br& b) { return b.nseg > 1 ? b.rest + b.nseg - 2 : b.e; };
+    out.desc.assign(4 * (size_t)out.ndesc, 0);
+    out.pnode.assign(out.ndesc, -1);
+    for (int32_t l = 0; l < out.nlev; ++l) {
+        const int32_t lb = out.level_begin[l], le = out.level_begin[l + 1];
+        for (int32_t t = lb; t < le; t += 32) {
+            int32_t wmax = 0, smx = 0;
+            for (int32_t e = t; e < std::min(le, t + 32); ++e)
+                if (lane_br[e] >= 0) { wmax = std::max(wmax, br[lane_br[e]].nafter); smx = std::max(smx, br[lane_br[e]].nseg); }
+            for (int32_t e = t; e < std::min(le, t + 32); ++e) {
+                if (lane_br[e] < 0) { out.desc[4 * e + 3] = smx << 16; out.desc[4 * e] = wmax << 24; continue; }
+                const Br& b = br[lane_br[e]];
+                out.desc[4 * e + 0] = b.nseg | (b.nafter << 16) | (wmax << 24);
+                out.desc[4 * e + 1] = b.rest;
+                out.desc[4 * e + 2] = b.cfirst;
+                out.desc[4 * e + 3] = b.nlead | (smx << 16);
+                out.pnode[e] = b.parent >= 0 ? last_node(br[b.parent]) : -1;
+            }
+        }
+    }
+    // ---- P4: segments, in compartment order ------------------------------------------------------
+    // Branch cut from its end into nseg segments of sj compartments (the paper's branch splitting,
+    // PAPER.md:151, with a fixed bound); node ids from the top of the branch: e, rest, rest+1, ...
+    std::vector<SegTmp> segs;                          // a item-local here
+    segs.reserve(nb);
+    for (int32_t i = 0; i < nb; ++i) {
+        const Br& b = br[i];
+        const int32_t end = b.start + b.len - 1;
+        for (int32_t k = 0; k < b.nseg; ++k) {          // k-th segment from the top
+            const int32_t q = b.nseg - 1 - k;           // counted from the branch's end
+            const int32_t sb = end - q * b.sj;
+            const int32_t sa = std::max(b.start, sb - b.sj + 1);
+            const int32_t node = k == 0 ? b.e : b.rest + k - 1;
+            const int32_t tnode = k > 0 ? (k == 1 ? b.e : b.rest + k - 2) : (b.parent >= 0 ? last_node(br[b.parent]) : -1);
+            segs.push_back({sa, sb - sa, node, tnode});
+            out.useful_steps += sb - sa;
+        }
+    }
+    // ---- chunks: consecutive segments, balanced in shared-memory bytes -----------------------------
+    const int64_t meta_item = round_up(out.nlev + 1, 4) + 4 * (int64_t)out.ndesc + round_up(out.ndesc, 4);
+    out.leader_extra = 5 * round_up(out.nnode, E) * P.width + 4 * meta_item;
+    out.chunks.assign(nchunks, ItemBuild::Chunk());
+    const int64_t per_comp = 3 * P.width, per_seg = 16;
+    const int64_t total = out.leader_extra + per_comp * out.n + per_seg * (int64_t)segs.size();
+    size_t si = 0;
+    int64_t acc = 0;
+    std::vector<SegTmp> mine;
+    for (int32_t r = 0; r < nchunks; ++r) {
+        ItemBuild::Chunk& ch = out.chunks[r];
+        const int64_t target = total * (r + 1) / nchunks;            // cumulative, so rounding does not pile up
+        if (r == 0) acc = out.leader_extra;
+        ch.begin = si < segs.size() ? segs[si].a : (int32_t)out.n;
+        mine.clear();
+        while (si < segs.size()) {
+            const int64_t cost = per_comp * (segs[si].m + 1) + per_seg;
+            const size_t left_chunks = (size_t)(nchunks - 1 - r);
+            const bool must_take = mine.empty() && segs.size() - si > left_chunks;   // no empty chunk while segments remain
+            const bool must_leave = segs.size() - si <= left_chunks;                   // keep one for every later chunk
+            if (r == nchunks - 1 || must_take || (!must_leave && acc + cost / 2 <= target)) {
+                mine.push_back(segs[si]); acc += cost; ++si;
+            } else break;
+        }
+        ch.n = mine.empty() ? 0 : mine.back().a + mine.back().m + 1 - ch.begin;
+        for (SegTmp& sg : mine) sg.a -= ch.begin;
+        const int32_t off = (int32_t)((out.comp_begin + ch.begin) % E);
+        order_segments(mine, R, off, ch.seg);
+        const int32_t ns = (int32_t)(ch.seg.size() / 4);
+        out.max_lanes = std::max(out.max_lanes, ns);
+        for (int32_t t = 0; t < ns; t += 32) {
+            int32_t mx = 0;
+            for (int32_t i = t; i < std::min(ns, t + 32); ++i) mx = std::max(mx, ch.seg[4 * i + 1]);
+            out.padded_steps += 32 * (int64_t)mx;
+        }
+        const int64_t L = round_up(off + ch.n, E);
+        ch.smem_need = 16 + (r == 0 ? out.leader_extra : 0) + 3 * L * P.width + 16 * (int64_t)ns;
+        out.smem_need = std::max(out.smem_need, ch.smem_need);
+    }
 }
 
 static hines_status_t canonical_tables(hines_plan& P, const int32_t* parent)
@@ -296,95 +398,153 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_level_begin.insert(P.item_level_begin.end(), ib.level_begin.begin(), ib.level_begin.end());
     P.item_level_offsets.push_back((int64_t)P.item_level_begin.size());
     P.item_desc.insert(P.item_desc.end(), ib.desc.begin(), ib.desc.end());
+    P.item_pnode.insert(P.item_pnode.end(), ib.pnode.begin(), ib.pnode.end());
     P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 4);
-    P.item_seg.insert(P.item_seg.end(), ib.seg.begin(), ib.seg.end());
-    P.item_seg_offsets.push_back((int64_t)P.item_seg.size() / 4);
-    P.item_nsep.push_back(ib.nsep);
-    // device blob: [level_begin | pad4 | branch desc | segment desc]
-    hines::ItemHeader h;
-    h.comp_begin = ib.comp_begin;
-    h.n = (int32_t)ib.n;
-    h.nlev = ib.nlev;
+    P.item_nnode.push_back(ib.nnode);
+    // device blob of the item: [level_begin | pad4 | branch desc | pnode | pad4]
+    hines::ItemHeader h{};
     h.meta_off = (int64_t)P.item_meta.size();
     P.item_meta.insert(P.item_meta.end(), ib.level_begin.begin(), ib.level_begin.end());
     P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
-    h.desc_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    h.bdesc_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
     P.item_meta.insert(P.item_meta.end(), ib.desc.begin(), ib.desc.end());
-    h.seg_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    P.item_meta.insert(P.item_meta.end(), ib.seg.begin(), ib.seg.end());
+    h.pnode_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
+    P.item_meta.insert(P.item_meta.end(), ib.pnode.begin(), ib.pnode.end());
+    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
     h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    h.nseg_lanes = (int32_t)(ib.seg.size() / 4);
-    h.nsep = ib.nsep;
+    h.nlev = ib.nlev; h.ndesc = ib.ndesc; h.nnode = ib.nnode;
+    h.first_chunk = (int32_t)P.chunk_headers.size();
+    h.nchunks = ib.nchunks;
+    h.n = (int32_t)ib.n;
     P.item_headers.push_back(h);
+    for (int32_t r = 0; r < ib.nchunks; ++r) {
+        const ItemBuild::Chunk& ch = ib.chunks[r];
+        hines::ChunkHeader k{};
+        k.comp_begin = ib.comp_begin + ch.begin;
+        k.n = ch.n;
+        k.nseg_lanes = (int32_t)(ch.seg.size() / 4);
+        k.item = item; k.rank = r;
+        k.seg_off = (int64_t)P.item_meta.size();
+        P.item_meta.insert(P.item_meta.end(), ch.seg.begin(), ch.seg.end());
+        P.chunk_headers.push_back(k);
+        P.chunk_comp_range.push_back(k.comp_begin);
+        P.chunk_comp_range.push_back(k.comp_begin + k.n);
+        P.chunk_seg.insert(P.chunk_seg.end(), ch.seg.begin(), ch.seg.end());
+        P.chunk_seg_offsets.push_back((int64_t)P.chunk_seg.size() / 4);
+    }
+    P.item_chunk_offsets.push_back((int64_t)P.chunk_headers.size());
     P.padded_lane_steps += ib.padded_steps;
-    for (size_t q = 1; q < ib.seg.size(); q += 4) P.useful_lane_steps += ib.seg[q];
+    P.useful_lane_steps += ib.useful_steps;
+    if (ib.nchunks > 1) { P.n_cluster_cells += c1 - c0; P.n_cluster_unknowns += ib.n; }
     P.n_resident_cells += c1 - c0;
     P.n_resident_unknowns += ib.n;
 }
 
-static void pack_items(hines_plan& P, std::vector<int64_t>& item_need, std::vector<char>& is_stream)
+struct ItemNeed { int64_t smem; int32_t lanes; int32_t nchunks; };
+
+// P1 + P2: cells -> work items, greedy in input order.  A cell whose lists fit the
+// group budget joins the open group while the group still fits; a cell that fits one block's budget
+// gets its own item; a larger cell is spread over a cluster of 2, 4, 8 or 16 blocks ("long branches
+// of large cells kept on their own blocks"); what fits nowhere goes to the streaming path.
+static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<char>& is_stream)
 {
     const int64_t nc = P.ncells;
     const int64_t max_smem = P.opt.smem_bytes_per_block;
     const int64_t group_cap = std::min<int64_t>(P.opt.group_smem_bytes, max_smem);
     const bool force_stream = P.opt.policy_flags & HINES_POLICY_FORCE_STREAM;
     const bool no_group = P.opt.policy_flags & HINES_POLICY_NO_GROUPING;
+    const bool no_cluster = (P.opt.policy_flags & HINES_POLICY_NO_CLUSTER) || P.opt.cluster_max < 2;
+    // a cell alone in a block may use up to single_cap; beyond that a cluster is preferred, because
+    // blocks of at most chunk_smem_bytes leave room for a second resident block per SM
+    const int64_t chunk_cap = std::min<int64_t>(P.opt.chunk_smem_bytes, max_smem);
+    const int64_t single_cap = no_cluster ? max_smem : chunk_cap;
     P.cell_item.assign(nc, -1);
     P.item_level_offsets.assign(1, 0);
     P.item_desc_offsets.assign(1, 0);
-    P.item_seg_offsets.assign(1, 0);
+    P.item_chunk_offsets.assign(1, 0);
+    P.chunk_seg_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
-    ItemBuild cur, cand;
+    ItemBuild cur, cand, alone;
     int64_t g0 = -1;                                   // first cell of the open group
-    auto flush = [&](int64_t c_end) {
-        if (g0 >= 0) { emit_item(P, g0, c_end, cur); item_need.push_back(cur.smem_need); g0 = -1; }
+    auto push = [&](int64_t a, int64_t b, const ItemBuild& ib) {
+        emit_item(P, a, b, ib);
+        need.push_back({ib.smem_need, ib.max_lanes, ib.nchunks});
     };
+    auto flush = [&](int64_t c_end) { if (g0 >= 0) { push(g0, c_end, cur); g0 = -1; } };
     for (int64_t c = 0; c < nc; ++c) {
         const int64_t ncomp = P.cell_offsets[c + 1] - P.cell_offsets[c];
-        // quick reject before building lists: the three arrays alone
-        bool fits_alone = !force_stream && 16 + 3 * ncomp * P.width <= max_smem;
-        ItemBuild alone;
-        if (fits_alone) { build_item(P, c, c + 1, alone); fits_alone = alone.smem_need <= max_smem; }
-        if (!fits_alone) { flush(c); is_stream[c] = 1; continue; }
-        if (no_group || alone.smem_need > group_cap) {            // its own item
-            flush(c);
-            emit_item(P, c, c + 1, alone); item_need.push_back(alone.smem_need);
-            continue;
+        bool placed = false, is_single = false;
+        if (!force_stream) {
+            const int64_t arrays = 16 + 3 * ncomp * P.width;             // lower bound of the need
+            if (arrays <= single_cap) {
+                build_item(P, c, c + 1, 1, alone);
+                is_single = alone.ok && alone.smem_need <= single_cap;
+            }
+            if (!is_single && !no_cluster) {
+                for (int32_t k = 2; k <= P.opt.cluster_max && !placed; k *= 2) {
+                    if (arrays / k > chunk_cap) continue;
+                    build_item(P, c, c + 1, k, cand);
+                    if (!cand.ok) break;
+                    if (cand.smem_need <= chunk_cap || (k * 2 > P.opt.cluster_max && cand.smem_need <= max_smem)) {
+                        flush(c); push(c, c + 1, cand); placed = true;
+                    }
+                }
+                if (!placed && arrays <= max_smem) {                      // last resort before streaming: one big block
+                    build_item(P, c, c + 1, 1, alone);
+                    is_single = alone.ok && alone.smem_need <= max_smem;
+                }
+            }
         }
-        if (g0 < 0) { g0 = c; cur = std::move(alone); continue; }
-        build_item(P, g0, c + 1, cand);                           // greedy: does the next cell still fit?
-        if (cand.smem_need <= group_cap) { std::swap(cur, cand); continue; }
+        if (placed) continue;
+        if (!is_single) { flush(c); is_stream[c] = 1; continue; }
+        if (no_group || alone.smem_need > group_cap) { flush(c); push(c, c + 1, alone); continue; }
+        if (g0 < 0) { g0 = c; std::swap(cur, alone); continue; }
+        build_item(P, g0, c + 1, 1, cand);                                // greedy: does the next cell still fit?
+        if (cand.ok && cand.smem_need <= group_cap) { std::swap(cur, cand); continue; }
         flush(c);
-        g0 = c; cur = std::move(alone);
+        g0 = c; std::swap(cur, alone);
     }
     flush(nc);
 }
 
-static void assign_classes(hines_plan& P, const std::vector<int64_t>& item_need)
+// Size classes.  Single-block items: by how many blocks of that size fit one SM (1, 2, 3, 4, 6, 8).
+// Cluster items: one class per cluster size.  Threads per block: enough lanes for the widest segment
+// list of the class, within what the register file allows for that many resident blocks.
+static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
 {
-    const int64_t nitems = (int64_t)item_need.size();
+    const int64_t nitems = (int64_t)need.size();
     const int64_t max_smem = P.opt.smem_bytes_per_block;
-    std::vector<int> item_k(nitems, 1);
-    int64_t need_max[kNumClassK] = {0};
-    int64_t count[kNumClassK] = {0};
+    const int nq = kNumClassK + kMaxClusterClass + 1;
+    std::vector<int> item_q(nitems, 0);
+    std::vector<int64_t> need_max(nq, 0), count(nq, 0);
+    std::vector<int32_t> lanes_max(nq, 0);
     for (int64_t i = 0; i < nitems; ++i) {
-        int best = 0;
-        for (int q = 0; q < kNumClassK; ++q)
-            if (item_need[i] <= class_cap(kClassK[q], max_smem)) best = q;
-        item_k[i] = best;
-        need_max[best] = std::max(need_max[best], item_need[i]);
-        count[best]++;
+        int q = 0;
+        if (need[i].nchunks > 1) q = kNumClassK + need[i].nchunks;
+        else for (int t = 0; t < kNumClassK; ++t) if (need[i].smem <= class_cap(kClassK[t], max_smem)) q = t;
+        item_q[i] = q;
+        need_max[q] = std::max(need_max[q], need[i].smem);
+        lanes_max[q] = std::max(lanes_max[q], need[i].lanes);
+        count[q]++;
     }
-    // classes in launch order: biggest blocks first
-    int cls_of_q[kNumClassK];
-    for (int q = 0; q < kNumClassK; ++q) {
-        cls_of_q[q] = -1;
-        if (!count[q]) continue;
+    // launch order of the classes: clusters first (largest first), then single blocks, biggest first
+    std::vector<int> qs;
+    for (int q = nq - 1; q >= kNumClassK; --q) if (count[q]) qs.push_back(q);
+    for (int q = 0; q < kNumClassK; ++q) if (count[q]) qs.push_back(q);
+    std::vector<int> cls_of_q(nq, -1);
+    for (int q : qs) {
         cls_of_q[q] = (int)P.class_smem_bytes.size();
-        P.class_smem_bytes.push_back((int32_t)round_up(need_max[q], 128));
-        P.class_blocks_per_sm.push_back(kClassK[q]);
+        const int64_t smem = round_up(need_max[q], 128);
+        P.class_smem_bytes.push_back((int32_t)smem);
+        P.class_cluster.push_back(q >= kNumClassK ? q - kNumClassK : 1);
+        const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
+        int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
+        tmax = std::max<int64_t>(128, std::min<int64_t>(1024, tmax));
+        int64_t t = P.opt.threads_per_block ? P.opt.threads_per_block : round_up(std::max(lanes_max[q], 1), 32);
+        t = std::max<int64_t>(P.opt.threads_per_block ? 32 : 128, std::min(t, tmax));
+        P.class_threads.push_back((int32_t)t);
     }
-    for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[item_k[i]];
+    for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[item_q[i]];
     const int ncls = (int)P.class_smem_bytes.size();
     P.class_first.assign(ncls, 0);
     P.class_count.assign(ncls, 0);
@@ -476,15 +636,17 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         }
         std::memcpy(&o, opt, (size_t)opt->struct_size);
     }
-    if (o.threads_per_block == 0) o.threads_per_block = 256;
     if (o.smem_bytes_per_block == 0) o.smem_bytes_per_block = (int32_t)kSmemMaxOptin;
     if (o.stream_threads == 0) o.stream_threads = 128;
     if (o.group_smem_bytes == 0) o.group_smem_bytes = 57344;
     if (o.max_segment == 0) o.max_segment = 64;
-    if (o.threads_per_block < 32 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
+    if (o.cluster_max == 0) o.cluster_max = 8;
+    if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 113 * 1024;
+    if (o.threads_per_block < 0 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~7)) {
+        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~15) ||
+        o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }
     if (cell_offsets[0] != 0) { set_error("cell_offsets[0] must be 0"); return HINES_ERR_BAD_TOPOLOGY; }
@@ -501,7 +663,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         P->cell_offsets.assign(cell_offsets, cell_offsets + ncells + 1);
         hines_status_t st = canonical_tables(*P, parent);
         if (st != HINES_OK) { delete P; return st; }
-        std::vector<int64_t> item_need;
+        std::vector<ItemNeed> item_need;
         std::vector<char> is_stream;
         pack_items(*P, item_need, is_stream);
         assign_classes(*P, item_need);
@@ -527,12 +689,15 @@ hines_status_t hines_plan_get_info(const hines_plan_t* P, hines_plan_info_t* out
     out->n_stream_branches = (int64_t)P->stream_desc.size();
     out->padded_lane_steps = P->padded_lane_steps; out->useful_lane_steps = P->useful_lane_steps;
     out->workspace_bytes = (int64_t)(P->item_meta.size() * 4 + P->item_headers.size() * sizeof(ItemHeader) +
+                                     P->chunk_headers.size() * sizeof(ChunkHeader) +
                                      P->item_launch_order.size() * 4 + P->stream_desc.size() * sizeof(StreamDesc) +
                                      P->stream_child.size() * 4 + 2 * P->n_stream_unknowns * P->width);
     out->bytes_min = P->n * 4 * P->width + 4 * P->nbranches;
     out->bytes_literal = P->n * (4 * P->width + 4);
     out->breadth_first = P->breadth_first;
     out->n_classes = (int32_t)P->class_smem_bytes.size();
+    out->n_cluster_cells = P->n_cluster_cells; out->n_cluster_unknowns = P->n_cluster_unknowns;
+    out->n_chunks = (int64_t)P->chunk_headers.size();
     return HINES_OK;
 }
 
@@ -562,9 +727,14 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_LEVEL_OFFSETS, P->item_level_offsets)
         TBL(HINES_TABLE_ITEM_LEVEL_BEGIN, P->item_level_begin)
         TBL(HINES_TABLE_ITEM_DESC, P->item_desc)
-        TBL(HINES_TABLE_ITEM_SEG_OFFSETS, P->item_seg_offsets)
-        TBL(HINES_TABLE_ITEM_SEG, P->item_seg)
-        TBL(HINES_TABLE_ITEM_NSEP, P->item_nsep)
+        TBL(HINES_TABLE_ITEM_PNODE, P->item_pnode)
+        TBL(HINES_TABLE_ITEM_NNODE, P->item_nnode)
+        TBL(HINES_TABLE_ITEM_CHUNK_OFFSETS, P->item_chunk_offsets)
+        TBL(HINES_TABLE_CHUNK_COMP_RANGE, P->chunk_comp_range)
+        TBL(HINES_TABLE_CHUNK_SEG_OFFSETS, P->chunk_seg_offsets)
+        TBL(HINES_TABLE_CHUNK_SEG, P->chunk_seg)
+        TBL(HINES_TABLE_CLASS_CLUSTER, P->class_cluster)
+        TBL(HINES_TABLE_CLASS_THREADS, P->class_threads)
         TBL(HINES_TABLE_STREAM_LEVEL_BEGIN, P->stream_level_begin)
         TBL(HINES_TABLE_STREAM_DESC, P->stream_desc)
         TBL(HINES_TABLE_STREAM_CHILD, P->stream_child)

@@ -8,19 +8,33 @@
 
 namespace hines {
 
-// One shared-memory work item = a contiguous run of cells (cells are packed into a
-// block in the order given).  32 bytes, read by one thread per block.
-struct ItemHeader {
-    int64_t comp_begin;   // global index of the item's first compartment
-    int32_t n;            // unknowns in the item
-    int32_t nlev;         // levels of the deepest cell in the item
-    int64_t meta_off;     // offset (int32 units, multiple of 4) of the item's metadata blob
-    int32_t meta_len;     // int32 count (multiple of 4): [level_begin (nlev+1) | pad | branch desc | segment desc]
-    int32_t desc_off;     // offset (int32 units, multiple of 4) of the branch descriptors inside the blob
-    int32_t seg_off;      // offset of the segment descriptors inside the blob
-    int32_t nseg_lanes;   // segment descriptors (lanes of the condensation / expansion sweeps)
-    int32_t nsep;         // separators (= segments) of the item
+// One on-chip work item = a contiguous run of whole cells held in the shared memory of one block
+// (nchunks == 1; cells are packed into a block in the order given), or ONE cell too
+// large for that, spread over the shared memories of a thread-block cluster (nchunks == cluster
+// size; chunk r lives in the block of cluster rank r, the level-synchronous part runs in rank 0).
+struct ItemHeader {          // 48 bytes
+    int64_t meta_off;        // offset (int32 units, multiple of 4) of the item's metadata blob:
+                             //   [level_begin (nlev+1) | pad4 | branch desc 4*ndesc | pnode ndesc | pad4]
+    int32_t meta_len;        // int32 count (multiple of 4)
+    int32_t bdesc_off;       // offset of the branch descriptors inside the blob (multiple of 4)
+    int32_t pnode_off;       // offset of the parent-node list inside the blob
+    int32_t nlev;            // levels of the deepest cell in the item
+    int32_t ndesc;           // branch lanes (incl. padding lanes) = ids of the branches' top nodes
+    int32_t nnode;           // nodes of the reduced tree (separators incl. the unused ids of padding lanes)
+    int32_t first_chunk;     // index of the item's first chunk
+    int32_t nchunks;
+    int32_t n;               // unknowns of the item
     int32_t pad_;
+};
+
+// One chunk = the contiguous compartment range one block stages into its shared memory.
+struct ChunkHeader {         // 32 bytes
+    int64_t comp_begin;      // global index of the chunk's first compartment
+    int64_t seg_off;         // offset (int32 units, multiple of 4) of the chunk's segment descriptors
+    int32_t n;               // unknowns in the chunk
+    int32_t nseg_lanes;      // segment descriptors (lanes of the condensation / expansion sweeps)
+    int32_t item;
+    int32_t rank;            // position inside the item = cluster rank
 };
 
 // Streaming-path branch descriptor (24 bytes).
@@ -52,20 +66,23 @@ struct hines_plan {
     std::vector<int32_t> branch_start, branch_len, branch_parent_comp, branch_parent_branch,
         branch_level, cell_nlevels, level_count, level_list, child_ids;
     // policy tables
-    std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc;
-    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets, item_seg_offsets;
-    std::vector<int32_t> item_seg, item_nsep;
+    std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc, item_pnode,
+        item_nnode, chunk_seg;
+    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets, item_chunk_offsets,
+        chunk_comp_range, chunk_seg_offsets;
     std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
-    std::vector<int32_t> class_blocks_per_sm;
+    std::vector<int32_t> class_cluster;                // per class: blocks per item (cluster size), 1 = no cluster
+    std::vector<int32_t> class_threads;                // per class: threads per block
     std::vector<int64_t> class_first, class_count;     // ranges in item_launch_order
     std::vector<hines::ItemHeader> item_headers;       // indexed by item id
+    std::vector<hines::ChunkHeader> chunk_headers;     // indexed by chunk id
     std::vector<int32_t> item_meta;                    // device blob
     // streaming path
     std::vector<int64_t> stream_level_begin;           // [nstream_levels+1]
     std::vector<hines::StreamDesc> stream_desc;
     std::vector<int32_t> stream_child;                 // pairs {gstart, ws}
     int64_t n_stream_cells = 0, n_stream_unknowns = 0;
-    int64_t n_resident_cells = 0, n_resident_unknowns = 0;
+    int64_t n_resident_cells = 0, n_resident_unknowns = 0, n_cluster_cells = 0, n_cluster_unknowns = 0;
     int64_t padded_lane_steps = 0, useful_lane_steps = 0;
 
     hines::DeviceTables* dev = nullptr;                // null until uploaded

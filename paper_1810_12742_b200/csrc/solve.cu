@@ -18,7 +18,9 @@
 //   forward:   x[i] = (b'[i] - u[i] x[q]) / d'[i] = c - f x[q]
 // f overwrites d and c, then x, overwrite b in the on-chip copy; the caller's d,u,b are not written.
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 
+#include <algorithm>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -31,6 +33,7 @@ namespace hines {
 struct DeviceTables {
     int device = -1;
     ItemHeader* items = nullptr;
+    ChunkHeader* chunks = nullptr;
     int32_t* launch_order = nullptr;
     int32_t* item_meta = nullptr;
     StreamDesc* stream_desc = nullptr;
@@ -40,7 +43,7 @@ struct DeviceTables {
     void* host_stage[4] = {nullptr, nullptr, nullptr, nullptr};   // hines_solve_host device buffers d,u,b,x
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};              // timing hook
     bool timing = false, timed_once = false;
-    unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident item, launch order
+    unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident block, launch order
     bool prof_on = false;
     int64_t bytes = 0;
 };
@@ -116,226 +119,274 @@ __device__ __forceinline__ unsigned smid()
     return r;
 }
 
+// fast reciprocal: hardware seed + Newton steps (no slow-path branch on the dependent chain; the
+// pivots of a strictly diagonally dominant matrix are finite, non-zero and in the normal range)
 template <typename T> __device__ __forceinline__ T rcp(T v);
-template <> __device__ __forceinline__ double rcp<double>(double v) { return 1.0 / v; }
-template <> __device__ __forceinline__ float rcp<float>(float v) { return 1.0f / v; }
+template <> __device__ __forceinline__ double rcp<double>(double v)
+{
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(v));      // MUFU.RCP64H: ~20 bits
+    double e = fma(-v, r, 1.0); r = fma(r, e, r);               // ~40 bits
+    e = fma(-v, r, 1.0); r = fma(r, e, r);                      // full double
+    return r;
+}
+template <> __device__ __forceinline__ float rcp<float>(float v)
+{
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(v));
+    const float e = fmaf(-v, r, 1.0f);
+    return fmaf(r, e, r);
+}
 
 template <typename T> __device__ __forceinline__ T fnma(T a, T b, T c);   // c - a*b
 template <> __device__ __forceinline__ double fnma<double>(double a, double b, double c) { return fma(-a, b, c); }
 template <> __device__ __forceinline__ float fnma<float>(float a, float b, float c) { return fmaf(-a, b, c); }
+template <typename T> __device__ __forceinline__ T fmad(T a, T b, T c);   // c + a*b
+template <> __device__ __forceinline__ double fmad<double>(double a, double b, double c) { return fma(a, b, c); }
+template <> __device__ __forceinline__ float fmad<float>(float a, float b, float c) { return fmaf(a, b, c); }
 
 // ------------------------------------------------------------------------------------------------
-// Resident kernel: one block per work item (a contiguous run of cells held in shared memory).
-// Shared-memory image (bytes): [0,16) mbarrier | sd[L] | su[L] | sb[L] | topd[S] | topb[S] | meta
-//   L = landed elements = item range widened to 16-byte boundaries; compartment j of the item sits
-//   at index j + off, off = comp_begin mod (16 / sizeof(T)).  S = separators rounded up.
+// Resident kernel: one block per chunk; an item is one block, or one cluster of blocks (CL).
 //
-// Three phases:
+// Shared memory of a block (bytes):
+//   [0,16) mbarrier
+//   rank 0 only:  rD[NN] rB[NN] rU[NN] pd[NN] pb[NN]  the reduced tree (one node per segment: its
+//                 separator), NN = nodes rounded up | item metadata (level_begin, branch desc, pnode)
+//   sd[L] su[L] sb[L]  the chunk's d, u, b in natural order, L = chunk range widened to 16-byte
+//                 boundaries; compartment j of the chunk sits at index j + off | segment descriptors
+// Blocks of rank > 0 write their separators into rank 0's reduced arrays through distributed shared
+// memory and read the separators' solution back from there.
+//
+// Phases:
 //   P1 condense   every segment's interior a..b-1 is eliminated top-down, independently of the tree
 //                 level (one lane per segment).  Node i keeps g = u[i+1]/D, h = e/D, c = B/D where e is
-//                 the fill-in coupling to the separator t above the segment; the separator b below gets
-//                 d[b] -= g u[b], b[b] -= g B and the new coupling U = -h u[b] to t; the contributions
-//                 to t (sum h e, sum h B) are parked per separator and ride along in P2's hand-off.
-//   P2 reduced    the level-synchronous Hines sweeps of the paper on the separators
-//                 only: one lane per branch, one step per segment, block barrier per level, sibling
-//                 hand-off at branch points by warp shuffle.
+//                 the fill-in coupling to the separator t above the segment.  What is left of the
+//                 separator b (pivot, right-hand side, coupling U to t) and the interior's contribution
+//                 to t (sum h e, sum h B) go to the reduced arrays.
+//   P2 reduced    the level-synchronous Hines sweeps of the paper on the reduced
+//                 tree: one lane per branch, one step per segment, block barrier per level; at a branch
+//                 point the siblings' hand-off values are summed by warp shuffles and the parent pulls
+//                 the sum.
 //   P3 expand     x[i] = c - g x[i+1] - h x[t] for every interior, again one lane per segment.
 // Eliminating in this order is a symmetric permutation of the same LDL^T factorisation (the matrix is
 // SPD and strictly diagonally dominant, so any order is stable without pivoting).
 // ------------------------------------------------------------------------------------------------
-template <typename T>
-__global__ void hines_resident_kernel(const ItemHeader* __restrict__ items, const int32_t* __restrict__ order,
-                                      const int32_t* __restrict__ meta_g, const T* __restrict__ d,
-                                      const T* __restrict__ u, const T* __restrict__ b, T* x, int64_t n_total,
-                                      unsigned long long* prof)
+template <typename T, bool CL>
+__global__ void __launch_bounds__(1024, 1)
+hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* __restrict__ chunks,
+                      const int32_t* __restrict__ order, const int32_t* __restrict__ meta_g,
+                      const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
+                      int64_t n_total, unsigned long long* prof)
 {
     extern __shared__ __align__(128) unsigned char smem[];
+    namespace cg = cooperative_groups;
     // phase clocks (debug hook, prof == nullptr in normal runs): thread 0 stamps %globaltimer
     unsigned long long stamp[7];
 #define HINES_STAMP(k) do { if (prof && threadIdx.x == 0) stamp[k] = globaltimer_ns(); } while (0)
     HINES_STAMP(0);
     constexpr int E = 16 / (int)sizeof(T);
-    const ItemHeader it = items[order[blockIdx.x]];
+    unsigned rank = 0, csize = 1;
+    if (CL) { rank = cg::this_cluster().block_rank(); csize = cg::this_cluster().num_blocks(); }
+    const ItemHeader it = items[order[blockIdx.x / csize]];
+    const ChunkHeader ch = chunks[it.first_chunk + rank];
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
-    const int off = (int)(it.comp_begin % E);
-    const int64_t g0 = it.comp_begin - off;                 // 16-byte aligned global element index
-    const int L = (off + it.n + E - 1) / E * E;             // landed elements
-    // the last item may end beyond a 16-byte boundary of the arrays: copy that remainder by hand
+    const int off = (int)(ch.comp_begin % E);
+    const int64_t g0 = ch.comp_begin - off;                 // 16-byte aligned global element index
+    const int L = (off + ch.n + E - 1) / E * E;             // landed elements
+    // the last chunk may end beyond a 16-byte boundary of the arrays: copy that remainder by hand
     const int64_t avail = n_total - g0;
     const int Lb = (int)(avail >= L ? L : (avail / E * E)); // elements brought by the bulk copies
-    const int S = (it.nsep + E - 1) / E * E;
+    const int NN = (it.nnode + E - 1) / E * E;
 
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
-    T* sd = reinterpret_cast<T*>(smem + 16);
+    // rank 0's layout of the reduced arrays; the same offsets address rank 0's memory from any rank
+    T* rD = reinterpret_cast<T*>(smem + 16);
+    T* rB = rD + NN;
+    T* rU = rB + NN;
+    T* pd = rU + NN;
+    T* pb = pd + NN;
+    int32_t* imeta = reinterpret_cast<int32_t*>(pb + NN);
+    unsigned char* chunk_base = rank == 0 ? reinterpret_cast<unsigned char*>(imeta + it.meta_len) : smem + 16;
+    T* sd = reinterpret_cast<T*>(chunk_base);
     T* su = sd + L;
     T* sb = su + L;
-    T* topd = sb + L;
-    T* topb = topd + S;
-    int32_t* smeta = reinterpret_cast<int32_t*>(topb + S);
+    const int4* seg = reinterpret_cast<const int4*>(sb + L);
 
     if (tid == 0) mbar_init(bar, 1);
     __syncthreads();
     if (tid == 0) {
         const uint32_t bytes = (uint32_t)Lb * sizeof(T);
-        mbar_expect_tx(bar, 3u * bytes + (uint32_t)it.meta_len * 4u);
-        tma_load_1d(smeta, meta_g + it.meta_off, (uint32_t)it.meta_len * 4u, bar);
+        const uint32_t mbytes = rank == 0 ? (uint32_t)it.meta_len * 4u : 0u;
+        const uint32_t sbytes = (uint32_t)ch.nseg_lanes * 16u;
+        mbar_expect_tx(bar, 3u * bytes + mbytes + sbytes);
+        if (sbytes) tma_load_1d(const_cast<int4*>(seg), meta_g + ch.seg_off, sbytes, bar);
         if (bytes) {
             tma_load_1d(sd, d + g0, bytes, bar);
-            tma_load_1d(su, u + g0, bytes, bar);
             tma_load_1d(sb, b + g0, bytes, bar);
+            tma_load_1d(su, u + g0, bytes, bar);
         }
+        if (mbytes) tma_load_1d(imeta, meta_g + it.meta_off, mbytes, bar);
     }
-    // remainder of the very last item (fewer than E elements), plain loads
+    // remainder of the very last chunk (fewer than E elements), plain loads
     for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
-    for (int i = tid; i < S; i += nthreads) { topd[i] = T(0); topb[i] = T(0); }
+    // reduced arrays as seen from this block
+    T *RD = rD, *RB = rB, *RU = rU, *PD = pd, *PB = pb;
+    if (CL) {
+        cg::cluster_group cluster = cg::this_cluster();
+        RD = cluster.map_shared_rank(rD, 0); RB = cluster.map_shared_rank(rB, 0); RU = cluster.map_shared_rank(rU, 0);
+        PD = cluster.map_shared_rank(pd, 0); PB = cluster.map_shared_rank(pb, 0);
+        cluster.sync();                                     // every block of the cluster is running
+    }
     mbar_wait(bar, 0);
     __syncthreads();
     HINES_STAMP(1);
-
-    const int32_t* lvl = smeta;
-    const int4* desc = reinterpret_cast<const int4*>(smeta + it.desc_off);
-    const int4* seg = reinterpret_cast<const int4*>(smeta + it.seg_off);
     const unsigned FULL = 0xffffffffu;
 
     // ---- P1: condense the interiors of all segments (no level dependency) ----
-    for (int base = (tid & ~31); base < it.nseg_lanes; base += nthreads) {
+    for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
         const int e = base + lane;
-        int4 sg = make_int4(0, 0, -1, 0);
-        if (e < it.nseg_lanes) sg = seg[e];
+        int4 sg = make_int4(0, 0, -1, -1);
+        if (e < ch.nseg_lanes) sg = seg[e];
         const int m = sg.y;
         const int mmax = __reduce_max_sync(FULL, m);
         int i = sg.x + off;
-        T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0);
-        if (m > 0) { D = sd[i]; B = sb[i]; if (sg.z >= 0) ee = su[i]; }
+        T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(1), bn = T(0);
+        if (sg.z >= 0) { D = sd[i]; B = sb[i]; if (sg.w >= 0) ee = su[i]; }
+        if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; bn = sb[i + 1]; }
         for (int s = 0; s < mmax; ++s) {
             if (s < m) {
-                const T un = su[i + 1], dn = sd[i + 1], bn = sb[i + 1];
+                T un2 = T(0), dn2 = T(1), bn2 = T(0);
+                if (s + 1 < m) { un2 = su[i + 2]; dn2 = sd[i + 2]; bn2 = sb[i + 2]; }     // next step's inputs
                 const T r = rcp<T>(D);
                 const T g = un * r, h = ee * r, c = B * r;
                 sd[i] = g; su[i] = h; sb[i] = c;
-                ddt = fnma<T>(-h, ee, ddt); dbt = fnma<T>(-h, B, dbt);
+                ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);
                 D = fnma<T>(g, un, dn); B = fnma<T>(g, B, bn); ee = -h * un;
-                ++i;
-                if (s == m - 1) { sd[i] = D; sb[i] = B; su[i] = ee; }     // the separator below
+                ++i; un = un2; dn = dn2; bn = bn2;
             }
         }
-        if (m > 0) { topd[sg.w] = ddt; topb[sg.w] = dbt; }
+        if (sg.z >= 0) { RD[sg.z] = D; RB[sg.z] = B; RU[sg.z] = ee; PD[sg.z] = ddt; PB[sg.z] = dbt; }
     }
-    __syncthreads();
+    if (CL) cg::this_cluster().sync(); else __syncthreads();
     HINES_STAMP(2);
 
-    // ---- P2 backward: reduced system, deepest level first ----
-    for (int lev = it.nlev - 1; lev >= 0; --lev) {
-        const int eb = lvl[lev], ee_ = lvl[lev + 1];
-        for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
-            const int e = base + lane;
-            int4 ds = make_int4(0, 0, -1, 0);
-            if (e < ee_) ds = desc[e];
-            const bool atomic_handoff = ds.y < 0;
-            const int nseg = ds.y & 0xfffff, sj = (ds.y >> 20) & 0x7ff, pc = ds.z;
-            const int nmax = __reduce_max_sync(FULL, nseg);
-            int i = ds.x + off;                                  // last compartment of the branch
-            T D = T(1), B = T(0), dd = T(0), db = T(0);
-            if (nseg > 0) { D = sd[i]; B = sb[i]; }
-            for (int k = 0; k < nmax; ++k) {                     // lanes walk their separators in lock-step
-                if (k < nseg) {
-                    const T r = rcp<T>(D);
-                    const T c = B * r;
-                    const bool last = k == nseg - 1;
-                    if (!last || pc >= 0) {
-                        const T U = su[i];
+    if (rank == 0) {
+        const int32_t* lvl = imeta;
+        const int4* bdesc = reinterpret_cast<const int4*>(imeta + it.bdesc_off);
+        const int32_t* pnode = imeta + it.pnode_off;
+        // ---- P2 backward: reduced tree, deepest level first ----
+        for (int lev = it.nlev - 1; lev >= 0; --lev) {
+            const int eb = lvl[lev], ee_ = lvl[lev + 1];
+            for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
+                const int e = base + lane;
+                int4 ds = make_int4(0, 0, 0, 0);
+                if (e < ee_) ds = bdesc[e];
+                const int4 d0 = bdesc[base];                     // tile-uniform fields (same in every lane of the tile)
+                const int nseg = ds.x & 0xffff, nafter = (ds.x >> 16) & 0xff, wmax = (d0.x >> 24) & 0xff;
+                const int nlead = ds.w & 0xffff, nmax = (d0.w >> 16) & 0xffff;
+                int node = nseg > 1 ? ds.y + nseg - 2 : e;       // last node of the branch
+                T D = T(1), B = T(0), dd = T(0), db = T(0);
+                if (nseg > 0) {
+                    D = rD[node]; B = rB[node];
+                    for (int c = 0; c < nlead; ++c) { D -= pd[ds.z + c]; B -= pb[ds.z + c]; }   // pull
+                }
+                for (int k = 0; k < nmax; ++k) {                 // lanes walk their nodes in lock-step
+                    if (k < nseg) {
+                        const T r = rcp<T>(D);
+                        const T U = rU[node];
                         const T f = U * r;
-                        sd[i] = f; sb[i] = c;
-                        dd = fnma<T>(-f, U, topd[ds.w + k]);     // f U + parked contribution of the segment
-                        db = fnma<T>(-f, B, topb[ds.w + k]);
-                        if (!last) { i -= sj; D = sd[i] - dd; B = sb[i] - db; }
-                    } else {                                     // root of the reduced tree: x = b'/d'
-                        sd[i] = T(0); sb[i] = c;
+                        rD[node] = f; rB[node] = B * r;
+                        dd = fmad<T>(f, U, pd[node]);            // f U + parked contribution of the segment
+                        db = fmad<T>(f, B, pb[node]);
+                        if (k + 1 < nseg) {
+                            node = (k + 2 == nseg) ? e : node - 1;
+                            D = rD[node] - dd; B = rB[node] - db;
+                        }
+                    }
+                }
+                // hand-off at the branch point: siblings sit in one tile, the group's first lane sums
+                // their values by shuffle (fixed order) and leaves the sum in its slot
+                const T dd0 = dd, db0 = db;
+                for (int k = 1; k <= wmax; ++k) {
+                    const T vd = __shfl_down_sync(FULL, dd0, k);
+                    const T vb = __shfl_down_sync(FULL, db0, k);
+                    if (k <= nafter) { dd += vd; db += vb; }
+                }
+                if (nseg > 0) { pd[e] = dd; pb[e] = db; }
+            }
+            __syncthreads();
+        }
+        HINES_STAMP(3);
+        // ---- P2 forward: root level first; a root has f = 0, so x = c ----
+        for (int lev = 0; lev < it.nlev; ++lev) {
+            const int eb = lvl[lev], ee_ = lvl[lev + 1];
+            for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
+                const int e = base + lane;
+                int4 ds = make_int4(0, 0, 0, 0);
+                int pn = -1;
+                if (e < ee_) { ds = bdesc[e]; pn = pnode[e]; }
+                const int nseg = ds.x & 0xffff, nmax = (ds.w >> 16) & 0xffff;
+                T xp = pn >= 0 ? rB[pn] : T(0);
+                int node = e;
+                for (int k = 0; k < nmax; ++k) {
+                    if (k < nseg) {
+                        xp = fnma<T>(rD[node], xp, rB[node]);
+                        rB[node] = xp;
+                        node = k == 0 ? ds.y : node + 1;
                     }
                 }
             }
-            // hand-off at the branch point: siblings sit in one tile; the lowest lane of
-            // each sibling group gathers the others' contributions by shuffle and updates the parent.
-            const int key = (nseg > 0 && pc >= 0) ? pc : -2 - lane;
-            const unsigned peers = __match_any_sync(FULL, key);
-            const int leader = __ffs(peers) - 1;
-            const int maxcnt = __reduce_max_sync(FULL, __popc(peers));
-            unsigned rest = (lane == leader) ? (peers & ~(1u << lane)) : 0u;
-            for (int t = 1; t < maxcnt; ++t) {
-                const int src = rest ? (__ffs(rest) - 1) : lane;
-                const T vd = __shfl_sync(FULL, dd, src);
-                const T vb = __shfl_sync(FULL, db, src);
-                if (rest) { dd += vd; db += vb; rest &= rest - 1; }
-            }
-            if (lane == leader && key >= 0) {
-                if (!atomic_handoff) { sd[pc + off] -= dd; sb[pc + off] -= db; }
-                else { atomicAdd(&sd[pc + off], -dd); atomicAdd(&sb[pc + off], -db); }
-            }
+            __syncthreads();
         }
-        __syncthreads();
+    } else {
+        HINES_STAMP(3);
     }
-
-    HINES_STAMP(3);
-    // ---- P2 forward: root level first ----
-    for (int lev = 0; lev < it.nlev; ++lev) {
-        const int eb = lvl[lev], ee_ = lvl[lev + 1];
-        for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
-            const int e = base + lane;
-            int4 ds = make_int4(0, 0, -1, 0);
-            if (e < ee_) ds = desc[e];
-            const int nseg = ds.y & 0xfffff, sj = (ds.y >> 20) & 0x7ff, pc = ds.z;
-            const int nmax = __reduce_max_sync(FULL, nseg);
-            T xp = (nseg > 0 && pc >= 0) ? sb[pc + off] : T(0);
-            int i = ds.x + off - (nseg - 1) * sj;                // first (top-most) separator of the branch
-            for (int k = 0; k < nmax; ++k) {
-                if (k < nseg) {
-                    xp = fnma<T>(sd[i], xp, sb[i]);
-                    sb[i] = xp;
-                    i += sj;
-                }
-            }
-        }
-        __syncthreads();
-    }
-
+    if (CL) cg::this_cluster().sync();
     HINES_STAMP(4);
+
     // ---- P3: expand the interiors (lanes aligned at the segment start so that the shared-memory
     //      addresses of a wavefront keep their distinct residues) ----
-    for (int base = (tid & ~31); base < it.nseg_lanes; base += nthreads) {
+    for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
         const int e = base + lane;
-        int4 sg = make_int4(0, 0, -1, 0);
-        if (e < it.nseg_lanes) sg = seg[e];
+        int4 sg = make_int4(0, 0, -1, -1);
+        if (e < ch.nseg_lanes) sg = seg[e];
         const int m = sg.y;
         const int mmax = __reduce_max_sync(FULL, m);
+        const int a = sg.x + off;
         T xt = T(0), xn = T(0);
-        if (m > 0) { xn = sb[sg.x + off + m]; if (sg.z >= 0) xt = sb[sg.z + off]; }
+        if (sg.z >= 0) { xn = RB[sg.z]; if (sg.w >= 0) xt = RB[sg.w]; sb[a + m] = xn; }
+        T g1 = T(0), h1 = T(0), c1 = T(0);
+        if (m > 0) { g1 = sd[a + m - 1]; h1 = su[a + m - 1]; c1 = sb[a + m - 1]; }
         for (int j = mmax - 1; j >= 0; --j) {
             if (j < m) {
-                const int i = sg.x + off + j;
-                xn = fnma<T>(su[i], xt, fnma<T>(sd[i], xn, sb[i]));
-                sb[i] = xn;
+                T g2 = T(0), h2 = T(0), c2 = T(0);
+                if (j > 0) { g2 = sd[a + j - 1]; h2 = su[a + j - 1]; c2 = sb[a + j - 1]; }
+                xn = fnma<T>(g1, xn, fnma<T>(h1, xt, c1));       // one FMA on the dependent chain
+                sb[a + j] = xn;
+                g1 = g2; h1 = h2; c1 = c2;
             }
         }
     }
 
     // ---- store x (natural order): bulk store of the 16-byte aligned interior, edges by hand ----
-    const int head_end = min(it.n, (E - off) % E);                     // item-local [0, head_end)
-    const int tail_begin = max(head_end, (int)(((off + it.n) / E) * E) - off);   // item-local [tail_begin, n)
+    const int head_end = min(ch.n, (E - off) % E);                     // chunk-local [0, head_end)
+    const int tail_begin = max(head_end, (int)(((off + ch.n) / E) * E) - off);   // chunk-local [tail_begin, n)
     fence_proxy_async();
     __syncthreads();
     HINES_STAMP(5);
     if (tid == 0 && tail_begin > head_end) {
-        tma_store_1d(x + it.comp_begin + head_end, sb + off + head_end, (uint32_t)(tail_begin - head_end) * sizeof(T));
+        tma_store_1d(x + ch.comp_begin + head_end, sb + off + head_end, (uint32_t)(tail_begin - head_end) * sizeof(T));
         tma_store_commit_wait();
     }
-    for (int j = tid; j < head_end; j += nthreads) x[it.comp_begin + j] = sb[off + j];
-    for (int j = tail_begin + tid; j < it.n; j += nthreads) x[it.comp_begin + j] = sb[off + j];
+    for (int j = tid; j < head_end; j += nthreads) x[ch.comp_begin + j] = sb[off + j];
+    for (int j = tail_begin + tid; j < ch.n; j += nthreads) x[ch.comp_begin + j] = sb[off + j];
     if (prof && tid == 0) {
         stamp[6] = globaltimer_ns();
         unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
         for (int k = 0; k < 7; ++k) o[k] = stamp[k];
-        o[7] = ((unsigned long long)smid() << 32) | (unsigned)it.n;
+        o[7] = ((unsigned long long)smid() << 32) | (unsigned)ch.n;
     }
+    if (CL) cg::this_cluster().sync();          // rank 0's shared memory stays alive while others read it
 #undef HINES_STAMP
 }
 
@@ -406,7 +457,7 @@ static hines_status_t upload_vec(const V& v, void** dst, int64_t& total)
 static void free_device(DeviceTables* D)
 {
     if (!D) return;
-    cudaFree(D->items); cudaFree(D->launch_order); cudaFree(D->item_meta); cudaFree(D->stream_desc);
+    cudaFree(D->items); cudaFree(D->chunks); cudaFree(D->launch_order); cudaFree(D->item_meta); cudaFree(D->stream_desc);
     cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
@@ -435,6 +486,7 @@ static hines_status_t upload(hines_plan* P)
                 return HINES_ERR_UNSUPPORTED;
             }
         if ((st = upload_vec(P->item_headers, (void**)&D->items, D->bytes))) return st;
+        if ((st = upload_vec(P->chunk_headers, (void**)&D->chunks, D->bytes))) return st;
         if ((st = upload_vec(P->item_launch_order, (void**)&D->launch_order, D->bytes))) return st;
         if ((st = upload_vec(P->item_meta, (void**)&D->item_meta, D->bytes))) return st;
         if ((st = upload_vec(P->stream_desc, (void**)&D->stream_desc, D->bytes))) return st;
@@ -445,13 +497,21 @@ static hines_status_t upload(hines_plan* P)
             CUDA_TRY(cudaMalloc(&D->ws_c, wb));
             D->bytes += 2 * (int64_t)wb;
         }
-        int32_t max_smem = 0;
-        for (int32_t s : P->class_smem_bytes) max_smem = s > max_smem ? s : max_smem;
-        if (max_smem) {
-            if (P->dtype == HINES_F64)
-                CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
-            else
-                CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem));
+        int32_t max_smem[2] = {0, 0};
+        bool nonportable = false;
+        for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
+            const int cl = P->class_cluster[q] > 1;
+            max_smem[cl] = std::max(max_smem[cl], P->class_smem_bytes[q]);
+            nonportable |= P->class_cluster[q] > 8;
+        }
+        if (P->dtype == HINES_F64) {
+            if (max_smem[0]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[0]));
+            if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
+            if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        } else {
+            if (max_smem[0]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[0]));
+            if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
+            if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         }
         return HINES_OK;
     };
@@ -465,14 +525,32 @@ template <typename T>
 static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T* b, T* x, cudaStream_t stream)
 {
     DeviceTables* D = P->dev;
-    const int nthreads = P->opt.threads_per_block;
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
+    int64_t first_block = 0;
     for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
         const int64_t cnt = P->class_count[q];
         if (!cnt) continue;
-        hines_resident_kernel<T><<<(unsigned)cnt, nthreads, P->class_smem_bytes[q], stream>>>(
-            D->items, D->launch_order + P->class_first[q], D->item_meta, d, u, b, x, P->n,
-            D->prof_on ? D->prof + 8 * P->class_first[q] : nullptr);
+        const int cl = P->class_cluster[q];
+        unsigned long long* prof = D->prof_on ? D->prof + 8 * first_block : nullptr;
+        const int32_t* ord = D->launch_order + P->class_first[q];
+        if (cl == 1) {
+            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], stream>>>(
+                D->items, D->chunks, ord, D->item_meta, d, u, b, x, P->n, prof);
+        } else {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)(cnt * cl));
+            cfg.blockDim = dim3((unsigned)P->class_threads[q]);
+            cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
+            cfg.stream = stream;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, (const ItemHeader*)D->items,
+                                        (const ChunkHeader*)D->chunks, ord, (const int32_t*)D->item_meta, d, u, b, x,
+                                        (int64_t)P->n, prof));
+        }
+        first_block += cnt * cl;
     }
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
     const int nlev = (int)P->stream_level_begin.size() - 1;
@@ -575,7 +653,7 @@ hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* P, int32_t enable)
     hines_status_t st = upload(P);
     if (st != HINES_OK) return st;
     DeviceTables* D = P->dev;
-    const size_t bytes = P->item_headers.size() * 8 * sizeof(unsigned long long);
+    const size_t bytes = P->chunk_headers.size() * 8 * sizeof(unsigned long long);
     if (enable && !D->prof && bytes) {
         CUDA_TRY(cudaMalloc(&D->prof, bytes));
         CUDA_TRY(cudaMemset(D->prof, 0, bytes));
@@ -588,7 +666,7 @@ hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* P, int32_t enable)
 hines_status_t hines_plan_get_phase_clocks(hines_plan_t* P, uint64_t* host_dst, int64_t capacity_bytes, int64_t* needed_bytes)
 {
     if (!P || !needed_bytes) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
-    const int64_t bytes = (int64_t)(P->item_headers.size() * 8 * sizeof(unsigned long long));
+    const int64_t bytes = (int64_t)(P->chunk_headers.size() * 8 * sizeof(unsigned long long));
     *needed_bytes = bytes;
     if (!host_dst) return HINES_OK;
     if (!P->dev || !P->dev->prof) { set_error("phase clocks not enabled"); return HINES_ERR_INVALID_ARG; }

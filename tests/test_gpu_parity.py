@@ -61,7 +61,7 @@ def test_small_configs_streaming_path(cfg, scale):
     assert info.n_resident_items == 0 and info.n_stream_cells == m.ncells
 
 
-@pytest.mark.parametrize("kw", [dict(policy_flags=2), dict(policy_flags=4), dict(smem_bytes_per_block=48 * 1024),
+@pytest.mark.parametrize("kw", [dict(policy_flags=2), dict(policy_flags=4), dict(smem_bytes_per_block=48 * 1024, policy_flags=8),
                                 dict(threads_per_block=64), dict(threads_per_block=1024, group_smem_bytes=200 * 1024),
                                 dict(group_smem_bytes=8 * 1024, stream_threads=32)])
 def test_policy_variants_mixed_paths(kw):
@@ -71,6 +71,18 @@ def test_policy_variants_mixed_paths(kw):
     _, info = _check(m, d, u, b, **kw)
     if kw.get("smem_bytes_per_block"):
         assert info.n_stream_cells > 0 and info.n_resident_items > 0
+
+
+@pytest.mark.parametrize("kw", [dict(chunk_smem_bytes=40 * 1024), dict(chunk_smem_bytes=24 * 1024, cluster_max=16),
+                                dict(chunk_smem_bytes=30 * 1024, cluster_max=2, max_segment=9),
+                                dict(chunk_smem_bytes=16 * 1024, cluster_max=16, max_segment=3, threads_per_block=64)])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_cluster_path(kw, dtype):
+    """Cells cut into chunks over a thread-block cluster (distributed shared memory), sizes 2..16."""
+    m = mg.make_config(2, 0.006)
+    d, u, b = mg.system(m)
+    _, info = _check(m, d, u, b, dtype, **kw)
+    assert info.n_cluster_cells > 0 and info.n_chunks > info.n_resident_items
 
 
 def _edge_morphology():

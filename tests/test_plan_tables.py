@@ -15,7 +15,6 @@ import paper_1810_12742_b200 as hb
 from helpers import random_parent
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-ATOMIC = -(1 << 31)      # bit 31 of the packed descriptor word (int32)
 
 
 def test_library_exports_every_declared_symbol():
@@ -28,7 +27,7 @@ def test_library_exports_every_declared_symbol():
         assert getattr(lib, name) is not None
     assert "sm_100a" in hb.version()
     # struct sizes agree with the header's layout
-    assert ctypes.sizeof(hb.Options) == 28 and ctypes.sizeof(hb.PlanInfo) == 128
+    assert ctypes.sizeof(hb.Options) == 36 and ctypes.sizeof(hb.PlanInfo) == 152
 
 
 def _plan_cfg(cfg, scale, **kw):
@@ -93,29 +92,38 @@ def test_validation_errors():
 
 
 def _check_policy(m, plan, max_segment=64):
-    """Validity invariants (policy-free): every branch exactly once, all branches of a resident cell
-    in one item, sibling groups inside one 32-lane tile (or flagged), parents strictly on the previous
-    level, segments tile every branch exactly (one separator per segment, interiors disjoint), every
-    non-empty interior listed exactly once, smem need within the class, launch order a permutation."""
+    """Validity invariants (policy-free): every cell in exactly one on-chip item or on the streaming
+    path; the chunks of an item tile its compartment range; segments tile every branch exactly, each
+    inside one chunk and listed once; node ids are unique; a segment's upper node is the node of the
+    compartment above it; every branch has one lane on its level; sibling groups of at most 32 sit in
+    one 32-lane tile and their first lane absorbs the others, larger groups are pulled one by one;
+    shared-memory need within the class; launch order a permutation."""
     T = oracle.tables(m.parent, m.cell_offsets)
     w = 8 if plan.dtype == hb.F64 else 4
+    E = 16 // w
     cell_item = plan.table("cell_item")
     rng_ = plan.table("item_cell_range").reshape(-1, 2)
     desc_off = plan.table("item_desc_offsets")
     lvl_off = plan.table("item_level_offsets")
     lvl_begin = plan.table("item_level_begin")
     desc = plan.table("item_desc").reshape(-1, 4)
-    seg_off = plan.table("item_seg_offsets")
-    segs = plan.table("item_seg").reshape(-1, 4)
-    nsep_tab = plan.table("item_nsep")
+    pnode = plan.table("item_pnode")
+    nnode = plan.table("item_nnode")
+    ch_off = plan.table("item_chunk_offsets")
+    ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
+    seg_off = plan.table("chunk_seg_offsets")
+    segs = plan.table("chunk_seg").reshape(-1, 4)
     cls = plan.table("item_class")
     cls_smem = plan.table("class_smem_bytes")
+    cls_cluster = plan.table("class_cluster")
+    cls_threads = plan.table("class_threads")
     order = plan.table("item_launch_order")
     nitems = len(cls)
     assert sorted(order.tolist()) == list(range(nitems))
     assert (np.diff(cls[order]) >= 0).all()
+    assert ((cls_threads % 32 == 0) & (cls_threads >= 32) & (cls_threads <= 1024)).all()
     info = plan.info
-    assert info.n_resident_items == nitems
+    assert info.n_resident_items == nitems and info.n_chunks == len(ch_rng)
     seen_cells = np.zeros(m.ncells, bool)
     useful = 0
     nsep_total = 0
@@ -124,69 +132,91 @@ def _check_policy(m, plan, max_segment=64):
         assert c1 > c0 and (cell_item[c0:c1] == it).all()
         seen_cells[c0:c1] = True
         comp0 = m.cell_offsets[c0]; n_it = m.cell_offsets[c1] - comp0
+        nch = ch_off[it + 1] - ch_off[it]
+        assert nch == cls_cluster[cls[it]] and (nch == 1 or c1 - c0 == 1)
+        cr = ch_rng[ch_off[it]:ch_off[it + 1]]
+        assert cr[0, 0] == comp0 and cr[-1, 1] == comp0 + n_it and (cr[1:, 0] == cr[:-1, 1]).all()
         dsc = desc[desc_off[it]:desc_off[it + 1]]
-        sg = segs[seg_off[it]:seg_off[it + 1]]
+        pn = pnode[desc_off[it]:desc_off[it + 1]]
         lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
         nlev = len(lb) - 1
         assert nlev == T.cell_nlevels[c0:c1].max() and lb[0] == 0 and lb[-1] == len(dsc)
-        # expected set of (end, len, pc, level)
+        # segments of all chunks -> node of every separator compartment (item-local position)
+        node_at = {}                     # separator position -> node
+        seg_of_node = {}
+        covered = np.zeros(n_it, int)
+        nlanes_max = 0
+        for r, ch in enumerate(range(ch_off[it], ch_off[it + 1])):
+            sg = segs[seg_off[ch]:seg_off[ch + 1]]
+            nlanes_max = max(nlanes_max, len(sg))
+            base = cr[r, 0] - comp0
+            for a, mm, node, tnode in sg:
+                if node < 0:
+                    assert mm == 0
+                    continue
+                assert 0 <= node < nnode[it] and node not in seg_of_node
+                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < max_segment
+                seg_of_node[int(node)] = (int(base + a), int(mm), int(tnode))
+                node_at[int(base + a + mm)] = int(node)
+                covered[base + a:base + a + mm + 1] += 1
+                useful += int(mm)
+            L = -(-(cr[r, 0] % E + cr[r, 1] - cr[r, 0]) // E) * E
+            meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + -(-len(dsc) // 4) * 4
+            need = 16 + 3 * L * w + 16 * len(sg) + (5 * (-(-nnode[it] // E) * E) * w + 4 * meta if r == 0 else 0)
+            assert need <= cls_smem[cls[it]] <= 232448
+        assert (covered == 1).all()
+        nsep_total += len(seg_of_node)
+        # branches: one lane each, on its level; node chain from the top: e, rest, rest+1, ...
         want = {}
         for c in range(c0, c1):
             sh = m.cell_offsets[c] - comp0
             for j in range(T.cell_branch_offsets[c], T.cell_branch_offsets[c + 1]):
                 pc = T.branch_parent_comp[j]
-                want[int(T.branch_start[j] + sh + T.branch_len[j] - 1)] = (
-                    int(T.branch_len[j]), -1 if pc < 0 else int(pc + sh), int(T.branch_level[j]))
-        got = {}
-        sep_of = {}                       # separator id -> (node, top separator node or -1)
-        covered = np.zeros(n_it, int)
+                want[int(T.branch_start[j] + sh)] = (int(T.branch_len[j]), -1 if pc < 0 else int(pc + sh), int(T.branch_level[j]))
+        top_node_pos = {node: a for node, (a, mm, t) in seg_of_node.items()}
+        lanes_seen = set()
         for l in range(nlev):
-            seg_l = dsc[lb[l]:lb[l + 1]]
-            nseg = seg_l[:, 1] & 0xfffff
-            sj = (seg_l[:, 1] >> 20) & 0x7ff
-            real = nseg > 0
-            for (end, word, pc, sbase), ns, s_ in zip(seg_l[real], nseg[real], sj[real]):
-                ln, pcw, lw = want[int(end)]
-                assert int(end) not in got and pcw == pc and lw == l
-                got[int(end)] = 1
-                assert ns == -(-ln // max_segment) and s_ == -(-ln // ns)
-                start = end - ln + 1
-                for k in range(ns):
-                    b = end - k * s_
-                    a = max(start, b - s_ + 1)
-                    t = b - s_ if k < ns - 1 else pc
-                    assert (sbase + k) not in sep_of
-                    sep_of[int(sbase + k)] = (int(a), int(b - a), int(t))
-                    covered[a:b + 1] += 1
-            pcs = seg_l[:, 2]
-            for pcv in np.unique(pcs[real & (pcs >= 0)]):
-                idx = np.nonzero(real & (pcs == pcv))[0]
-                flagged = seg_l[idx, 1] < 0
-                if flagged.any():
-                    assert flagged.all() and len(idx) > 32
+            tile_l = dsc[lb[l]:lb[l + 1]]
+            for e in range(lb[l], lb[l + 1]):
+                w0, rest, cfirst, w3 = (int(v) for v in dsc[e])
+                nseg, nafter, wmax = w0 & 0xffff, (w0 >> 16) & 0xff, (w0 >> 24) & 0xff
+                nlead, smx = w3 & 0xffff, (w3 >> 16) & 0xffff
+                t0 = lb[l] + (e - lb[l]) // 32 * 32
+                tl = dsc[t0:min(t0 + 32, lb[l + 1])]
+                assert wmax == ((tl[:, 0] >> 16) & 0xff).max() and smx == (tl[:, 0] & 0xffff).max()
+                if nseg == 0:
+                    assert pn[e] == -1 and nafter == 0
+                    continue
+                start = top_node_pos[e]                      # the top segment starts at the branch start
+                ln, pc, lw = want[start]
+                assert lw == l and start not in lanes_seen
+                lanes_seen.add(start)
+                assert nseg == -(-ln // max_segment)
+                sj = -(-ln // nseg)
+                end = start + ln - 1
+                for k in range(nseg):                        # k-th segment from the top
+                    q = nseg - 1 - k
+                    b_ = end - q * sj
+                    a_ = max(start, b_ - sj + 1)
+                    node = e if k == 0 else rest + k - 1
+                    tn = (e if k == 1 else rest + k - 2) if k > 0 else (node_at[pc] if pc >= 0 else -1)
+                    assert seg_of_node[node] == (a_, b_ - a_, tn), (it, e, k)
+                assert pn[e] == (node_at[pc] if pc >= 0 else -1)
+                # the children of this branch hang off its last compartment
+                kids = sorted(s_ for s_, (ln2, pc2, l2) in want.items() if pc2 == end)
+                if not kids:
+                    assert nlead == 0
                 else:
-                    assert idx.min() // 32 == idx.max() // 32 and (np.diff(idx) == 1).all()
-        assert set(got) == set(want) and (covered == 1).all()
-        assert nsep_tab[it] == len(sep_of) and sorted(sep_of) == list(range(len(sep_of)))
-        # parents are separators of the level above
-        ends_level = {e: v[2] for e, v in want.items()}
-        for e, (ln, pc, l) in want.items():
-            if pc >= 0:
-                assert ends_level[pc] == l - 1
-        # segment lane list: exactly the non-empty interiors, once each
-        real = sg[:, 1] > 0
-        listed = {int(sid): (int(a), int(mm), int(t)) for a, mm, t, sid in sg[real]}
-        assert len(listed) == real.sum()
-        assert listed == {k: v for k, v in sep_of.items() if v[1] > 0}
-        useful += int(sg[real, 1].sum())
-        nsep_total += len(sep_of)
-        # wavefront groups (16 lanes fp64 / 32 lanes fp32) mostly have distinct start residues
-        R = 128 // w
-        # shared-memory need within the class
-        E = 16 // w
-        L = -(-(comp0 % E + n_it) // E) * E
-        meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + 4 * len(sg)
-        assert 16 + 3 * L * w + 2 * (-(-len(sep_of) // E) * E) * w + 4 * meta <= cls_smem[cls[it]] <= 232448
+                    kid_lanes = sorted(node_at_start for node_at_start in
+                                       (n_ for n_, pos in top_node_pos.items() if pos in kids and n_ < len(dsc)))
+                    assert len(kid_lanes) == len(kids) and kid_lanes == list(range(kid_lanes[0], kid_lanes[0] + len(kids)))
+                    assert cfirst == kid_lanes[0] and lb[l + 1] <= cfirst < lb[l + 2]
+                    if len(kids) <= 32:
+                        assert nlead == 1 and (cfirst - lb[l + 1]) // 32 == (kid_lanes[-1] - lb[l + 1]) // 32
+                        assert [(int(dsc[q_, 0]) >> 16) & 0xff for q_ in kid_lanes] == list(range(len(kids) - 1, -1, -1))
+                    else:
+                        assert nlead == len(kids) and all(((int(dsc[q_, 0]) >> 16) & 0xff) == 0 for q_ in kid_lanes)
+        assert len(lanes_seen) == len(want)
     assert (seen_cells == (cell_item >= 0)).all()
     # streaming path: every branch of every non-resident cell exactly once, children complete
     sd = plan.table("stream_desc").reshape(-1, 6)
@@ -219,27 +249,55 @@ def _check_policy(m, plan, max_segment=64):
     assert info.padded_lane_steps >= useful
 
 
+def _check_interpreted(m, plan):
+    """The tables, executed lane by lane on the CPU (tests/plan_interpreter.py), solve the systems."""
+    from plan_interpreter import solve_with_tables
+    d, u, b = mg.system(m)
+    x = solve_with_tables(plan, m, d, u, b)
+    xr = oracle.hines_solve(m.parent, m.cell_offsets, d, u, b)
+    sel = np.repeat(plan.table("cell_item") >= 0, np.diff(m.cell_offsets))
+    assert np.isfinite(x[sel]).all() and np.isnan(x[~sel]).all()
+    if sel.any():
+        assert np.abs(x[sel] - xr[sel]).max() < 1e-12
+
+
 @pytest.mark.parametrize("cfg,scale,kw", [
     (0, 1.0, {}), (0, 1.0, dict(policy_flags=hb.POLICY_NO_GROUPING)),
-    (2, 0.004, {}), (2, 0.004, dict(smem_bytes_per_block=60000)),
+    (2, 0.004, {}), (2, 0.004, dict(smem_bytes_per_block=60000, policy_flags=hb.POLICY_NO_CLUSTER)),
     (2, 0.003, dict(policy_flags=hb.POLICY_FORCE_STREAM)),
     (3, 0.002, {}), (3, 0.002, dict(dtype=hb.F32)), (1, 0.002, {}), (1, 0.002, dict(max_segment=7)),
     (2, 0.003, dict(max_segment=2)), (3, 0.002, dict(max_segment=16)),
+    (2, 0.004, dict(chunk_smem_bytes=30000, cluster_max=16)), (1, 0.002, dict(max_segment=5, chunk_smem_bytes=8000)),
+    (3, 0.002, dict(chunk_smem_bytes=40000, cluster_max=4)),
 ])
 def test_policy_tables_valid(cfg, scale, kw):
     m, plan = _plan_cfg(cfg, scale, **kw)
     _check_policy(m, plan, kw.get("max_segment", 64))
+    _check_interpreted(m, plan)
 
 
 def test_policy_star_with_many_siblings_and_odd_offsets():
-    star = np.array([-1] + [0] * 70, np.int32)                        # 70 siblings: group spans tiles -> flagged
-    ps = [star, random_parent(33, 1), np.array([-1], np.int32), random_parent(200, 2, .7), star[:40]]
+    star = np.array([-1] + [0] * 70, np.int32)                        # 70 siblings: more than a tile -> pulled one by one
+    ps = [star, random_parent(33, 1), np.array([-1], np.int32), random_parent(200, 2, .7), star[:40],
+          random_parent(1001, 3, .97)]
     offs = np.concatenate([[0], np.cumsum([len(p) for p in ps])])
     m = mg.Morphology(np.concatenate(ps), offs)
-    for kw in ({}, dict(dtype=hb.F32), dict(policy_flags=hb.POLICY_NO_GROUPING)):
+    for kw in ({}, dict(dtype=hb.F32), dict(policy_flags=hb.POLICY_NO_GROUPING), dict(max_segment=3),
+               dict(chunk_smem_bytes=6000, max_segment=4)):
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
-        _check_policy(m, plan)
-        assert (plan.table("item_desc").reshape(-1, 4)[:, 1] < 0).any()
+        _check_policy(m, plan, kw.get("max_segment", 64))
+        _check_interpreted(m, plan)
+        assert ((plan.table("item_desc").reshape(-1, 4)[:, 3] & 0xffff) == 70).any()
+
+
+def test_clusters_take_the_cells_too_large_for_one_block():
+    m, plan = _plan_cfg(3, 0.004)
+    info = plan.info
+    assert info.n_cluster_cells > 0 and info.n_stream_cells == 0
+    cl = plan.table("class_cluster")
+    assert set(cl.tolist()) <= {1, 2, 4, 8} and (np.diff(cl) <= 0).all()
+    m, plan = _plan_cfg(3, 0.004, policy_flags=hb.POLICY_NO_CLUSTER)
+    assert plan.info.n_cluster_cells == 0 and (plan.table("class_cluster") == 1).all()
 
 
 def test_config4_goes_to_streaming_path_and_grouping_is_greedy_in_order():
