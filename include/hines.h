@@ -135,13 +135,18 @@ typedef enum {
     HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
     HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] lane index (item-local) where each level's
                                                lane list begins                                                        */
-    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane {nseg | nafter<<16 | tile max nafter<<24,
+    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane {nseg | nafter<<16 | tile max nafter<<24 | fast tile<<30,
                                                rest, cfirst, nlead | tile max nseg<<16}: nseg = 0 marks a padding lane;
                                                nafter = sibling lanes to the right whose hand-off values this lane
                                                absorbs by warp shuffle; cfirst, nlead = the hand-off slots (lane ids)
                                                the branch's last node pulls from                                       */
-    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[nlanes] last node of the parent branch, -1 = root branch / padding */
-    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] node ids in use (>= lanes)                                 */
+    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node above it in the reduced tree (a root and
+                                               an unused id: itself)                                                    */
+    HINES_TABLE_ITEM_NODE_OFFSETS    = 52,  /* int64[nitems+1] into ITEM_PNODE                                          */
+    HINES_TABLE_ITEM_ROUNDS          = 53,  /* int32[nitems] pointer-jumping rounds of the forward sweep: 2^rounds >= nodes
+                                               on the longest root path of the reduced tree                             */
+    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] node ids (>= lanes; the last one is an all-zero node that
+                                               branches without children pull: their cfirst)                           */
     HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
     HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
     HINES_TABLE_CHUNK_SEG_OFFSETS    = 48,  /* int64[nchunks+1] into CHUNK_SEG (in units of descriptors)                */

@@ -47,6 +47,7 @@ static const int kClassK[] = {1, 2, 3, 4, 6, 8};
 static const int kNumClassK = 6;
 static const int kRegsPerThread = 64;           // __launch_bounds__ of the resident kernel
 static const int kMaxClusterClass = 16;
+static const int32_t kFastTile = 1 << 30;        // descriptor word 0, bit 30
 
 static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
@@ -72,7 +73,8 @@ struct ItemBuild {
     bool ok = true;                          // false: a field overflows its descriptor bits -> streaming path
     std::vector<int32_t> level_begin;        // nlev+1, in branch lanes
     std::vector<int32_t> desc;               // 4 per branch lane
-    std::vector<int32_t> pnode;              // 1 per branch lane: last node of the parent branch, -1 = root / padding
+    std::vector<int32_t> pnode;              // 1 per node: the node above it in the reduced tree; itself for a root / an unused id
+    int32_t rounds = 0;                      // pointer-jumping rounds of the forward sweep: 2^rounds >= nodes on the longest root path
     struct Chunk {
         int32_t begin = 0, n = 0;            // item-local compartment range
         std::vector<int32_t> seg;            // 4 per segment lane {a (chunk-local), m, node, tnode}; node = -1 padding
@@ -216,27 +218,43 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         Br& b = br[lane_br[e]];
         if (b.nseg > 1) { b.rest = next_id; next_id += b.nseg - 1; }
     }
-    out.nnode = next_id;
+    const int32_t dummy = next_id;                     // an all-zero node: what a branch without children pulls
+    out.nnode = next_id + 1;
     auto last_node = [&](const Br& b) { return b.nseg > 1 ? b.rest + b.nseg - 2 : b.e; };
     out.desc.assign(4 * (size_t)out.ndesc, 0);
-    out.pnode.assign(out.ndesc, -1);
+    out.pnode.resize(out.nnode);
+    std::iota(out.pnode.begin(), out.pnode.end(), 0);
+    std::vector<int32_t> depth(out.nnode, 1);          // nodes on the path from the root, inclusive
+    int32_t height = 1;
     for (int32_t l = 0; l < out.nlev; ++l) {
         const int32_t lb = out.level_begin[l], le = out.level_begin[l + 1];
         for (int32_t t = lb; t < le; t += 32) {
-            int32_t wmax = 0, smx = 0;
+            int32_t wmax = 0, smx = 0, lmx = 0;
             for (int32_t e = t; e < std::min(le, t + 32); ++e)
-                if (lane_br[e] >= 0) { wmax = std::max(wmax, br[lane_br[e]].nafter); smx = std::max(smx, br[lane_br[e]].nseg); }
+                if (lane_br[e] >= 0) {
+                    const Br& b = br[lane_br[e]];
+                    wmax = std::max(wmax, b.nafter); smx = std::max(smx, b.nseg); lmx = std::max(lmx, b.nlead);
+                }
+            // fast tile: one node per branch, sibling groups of at most two, one hand-off slot to pull
+            const int32_t fast = (smx <= 1 && wmax <= 1 && lmx <= 1) ? kFastTile : 0;
             for (int32_t e = t; e < std::min(le, t + 32); ++e) {
-                if (lane_br[e] < 0) { out.desc[4 * e + 3] = smx << 16; out.desc[4 * e] = wmax << 24; continue; }
+                out.desc[4 * e + 2] = dummy;
+                if (lane_br[e] < 0) { out.desc[4 * e + 3] = smx << 16; out.desc[4 * e] = (wmax << 24) | fast; continue; }
                 const Br& b = br[lane_br[e]];
-                out.desc[4 * e + 0] = b.nseg | (b.nafter << 16) | (wmax << 24);
+                out.desc[4 * e + 0] = b.nseg | (b.nafter << 16) | (wmax << 24) | fast;
                 out.desc[4 * e + 1] = b.rest;
-                out.desc[4 * e + 2] = b.cfirst;
+                if (b.nlead) out.desc[4 * e + 2] = b.cfirst;
                 out.desc[4 * e + 3] = b.nlead | (smx << 16);
-                out.pnode[e] = b.parent >= 0 ? last_node(br[b.parent]) : -1;
+                if (b.parent >= 0) { out.pnode[e] = last_node(br[b.parent]); depth[e] = depth[out.pnode[e]] + 1; }
+                for (int32_t k = 1; k < b.nseg; ++k) {          // a root keeps itself as parent: its f is 0
+                    out.pnode[b.rest + k - 1] = k == 1 ? e : b.rest + k - 2;
+                    depth[b.rest + k - 1] = depth[e] + k;
+                }
+                height = std::max(height, depth[e] + b.nseg - 1);
             }
         }
     }
+    while ((1 << out.rounds) < height) ++out.rounds;
     // ---- P4: segments, in compartment order ------------------------------------------------------
     // Branch cut from its end into nseg segments of sj compartments (the paper's branch splitting,
     // PAPER.md:151, with a fixed bound); node ids from the top of the branch: e, rest, rest+1, ...
@@ -256,8 +274,8 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         }
     }
     // ---- chunks: consecutive segments, balanced in shared-memory bytes -----------------------------
-    const int64_t meta_item = round_up(out.nlev + 1, 4) + 4 * (int64_t)out.ndesc + round_up(out.ndesc, 4);
-    out.leader_extra = 5 * round_up(out.nnode, E) * P.width + 4 * meta_item;
+    const int64_t meta_item = round_up(out.nlev + 1, 4) + 4 * (int64_t)out.ndesc + round_up(out.nnode, 4);
+    out.leader_extra = 6 * round_up(out.nnode, E) * P.width + 4 * meta_item;
     out.chunks.assign(nchunks, ItemBuild::Chunk());
     const int64_t per_comp = 3 * P.width, per_seg = 16;
     const int64_t total = out.leader_extra + per_comp * out.n + per_seg * (int64_t)segs.size();
@@ -400,6 +418,8 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_desc.insert(P.item_desc.end(), ib.desc.begin(), ib.desc.end());
     P.item_pnode.insert(P.item_pnode.end(), ib.pnode.begin(), ib.pnode.end());
     P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 4);
+    P.item_node_offsets.push_back((int64_t)P.item_pnode.size());
+    P.item_rounds.push_back(ib.rounds);
     P.item_nnode.push_back(ib.nnode);
     // device blob of the item: [level_begin | pad4 | branch desc | pnode | pad4]
     hines::ItemHeader h{};
@@ -412,7 +432,7 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_meta.insert(P.item_meta.end(), ib.pnode.begin(), ib.pnode.end());
     P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
     h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    h.nlev = ib.nlev; h.ndesc = ib.ndesc; h.nnode = ib.nnode;
+    h.nlev = ib.nlev; h.ndesc = ib.ndesc; h.nnode = ib.nnode; h.rounds = ib.rounds;
     h.first_chunk = (int32_t)P.chunk_headers.size();
     h.nchunks = ib.nchunks;
     h.n = (int32_t)ib.n;
@@ -461,6 +481,7 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     P.cell_item.assign(nc, -1);
     P.item_level_offsets.assign(1, 0);
     P.item_desc_offsets.assign(1, 0);
+    P.item_node_offsets.assign(1, 0);
     P.item_chunk_offsets.assign(1, 0);
     P.chunk_seg_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
@@ -728,6 +749,8 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_LEVEL_BEGIN, P->item_level_begin)
         TBL(HINES_TABLE_ITEM_DESC, P->item_desc)
         TBL(HINES_TABLE_ITEM_PNODE, P->item_pnode)
+        TBL(HINES_TABLE_ITEM_NODE_OFFSETS, P->item_node_offsets)
+        TBL(HINES_TABLE_ITEM_ROUNDS, P->item_rounds)
         TBL(HINES_TABLE_ITEM_NNODE, P->item_nnode)
         TBL(HINES_TABLE_ITEM_CHUNK_OFFSETS, P->item_chunk_offsets)
         TBL(HINES_TABLE_CHUNK_COMP_RANGE, P->chunk_comp_range)

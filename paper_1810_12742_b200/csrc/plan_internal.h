@@ -14,7 +14,7 @@ namespace hines {
 // size; chunk r lives in the block of cluster rank r, the level-synchronous part runs in rank 0).
 struct ItemHeader {          // 48 bytes
     int64_t meta_off;        // offset (int32 units, multiple of 4) of the item's metadata blob:
-                             //   [level_begin (nlev+1) | pad4 | branch desc 4*ndesc | pnode ndesc | pad4]
+                             //   [level_begin (nlev+1) | pad4 | branch desc 4*ndesc | pnode nnode | pad4]
     int32_t meta_len;        // int32 count (multiple of 4)
     int32_t bdesc_off;       // offset of the branch descriptors inside the blob (multiple of 4)
     int32_t pnode_off;       // offset of the parent-node list inside the blob
@@ -24,7 +24,7 @@ struct ItemHeader {          // 48 bytes
     int32_t first_chunk;     // index of the item's first chunk
     int32_t nchunks;
     int32_t n;               // unknowns of the item
-    int32_t pad_;
+    int32_t rounds;          // pointer-jumping rounds of the forward sweep over the reduced tree
 };
 
 // One chunk = the contiguous compartment range one block stages into its shared memory.
@@ -67,8 +67,8 @@ struct hines_plan {
         branch_level, cell_nlevels, level_count, level_list, child_ids;
     // policy tables
     std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc, item_pnode,
-        item_nnode, chunk_seg;
-    std::vector<int64_t> item_cell_range, item_desc_offsets, item_level_offsets, item_chunk_offsets,
+        item_nnode, item_rounds, chunk_seg;
+    std::vector<int64_t> item_cell_range, item_desc_offsets, item_node_offsets, item_level_offsets, item_chunk_offsets,
         chunk_comp_range, chunk_seg_offsets;
     std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
     std::vector<int32_t> class_cluster;                // per class: blocks per item (cluster size), 1 = no cluster

@@ -30,6 +30,13 @@
 
 namespace hines {
 
+#ifdef HINES_P2_TRACE
+__device__ long long g_trace[1024];
+#define TR(i) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (i) < 1024) g_trace[(i)] = clock64(); } while (0)
+#else
+#define TR(i) do {} while (0)
+#endif
+
 struct DeviceTables {
     int device = -1;
     ItemHeader* items = nullptr;
@@ -141,6 +148,9 @@ template <> __device__ __forceinline__ float rcp<float>(float v)
 template <typename T> __device__ __forceinline__ T fnma(T a, T b, T c);   // c - a*b
 template <> __device__ __forceinline__ double fnma<double>(double a, double b, double c) { return fma(-a, b, c); }
 template <> __device__ __forceinline__ float fnma<float>(float a, float b, float c) { return fmaf(-a, b, c); }
+template <typename T> struct Vec2;
+template <> struct Vec2<double> { typedef double2 type; };
+template <> struct Vec2<float> { typedef float2 type; };
 template <typename T> __device__ __forceinline__ T fmad(T a, T b, T c);   // c + a*b
 template <> __device__ __forceinline__ double fmad<double>(double a, double b, double c) { return fma(a, b, c); }
 template <> __device__ __forceinline__ float fmad<float>(float a, float b, float c) { return fmaf(a, b, c); }
@@ -150,8 +160,9 @@ template <> __device__ __forceinline__ float fmad<float>(float a, float b, float
 //
 // Shared memory of a block (bytes):
 //   [0,16) mbarrier
-//   rank 0 only:  rD[NN] rB[NN] rU[NN] pd[NN] pb[NN]  the reduced tree (one node per segment: its
-//                 separator), NN = nodes rounded up | item metadata (level_begin, branch desc, pnode)
+//   rank 0 only:  nd[5 NN]  the reduced tree (one node per segment: its separator; per node the
+//                 record {D -> f, B -> c -> x, U, pd, pb}), NN = nodes rounded up | item metadata
+//                 (level_begin, branch desc, pnode)
 //   sd[L] su[L] sb[L]  the chunk's d, u, b in natural order, L = chunk range widened to 16-byte
 //                 boundaries; compartment j of the chunk sits at index j + off | segment descriptors
 // Blocks of rank > 0 write their separators into rank 0's reduced arrays through distributed shared
@@ -200,12 +211,10 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
 
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
     // rank 0's layout of the reduced arrays; the same offsets address rank 0's memory from any rank
-    T* rD = reinterpret_cast<T*>(smem + 16);
-    T* rB = rD + NN;
-    T* rU = rB + NN;
-    T* pd = rU + NN;
-    T* pb = pd + NN;
-    int32_t* imeta = reinterpret_cast<int32_t*>(pb + NN);
+    // node record: 6 values {D -> -f, B -> c, U, -, pd, pb}; the forward sweep reuses them as two
+    // {g, c} buffers and two parent ids
+    T* nd = reinterpret_cast<T*>(smem + 16);
+    int32_t* imeta = reinterpret_cast<int32_t*>(nd + 6 * NN);
     unsigned char* chunk_base = rank == 0 ? reinterpret_cast<unsigned char*>(imeta + it.meta_len) : smem + 16;
     T* sd = reinterpret_cast<T*>(chunk_base);
     T* su = sd + L;
@@ -227,14 +236,14 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
         }
         if (mbytes) tma_load_1d(imeta, meta_g + it.meta_off, mbytes, bar);
     }
+    if (rank == 0 && tid < 6) nd[6 * (it.nnode - 1) + tid] = T(0);      // the zero node (what a childless branch pulls)
     // remainder of the very last chunk (fewer than E elements), plain loads
     for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
     // reduced arrays as seen from this block
-    T *RD = rD, *RB = rB, *RU = rU, *PD = pd, *PB = pb;
+    T* ND = nd;
     if (CL) {
         cg::cluster_group cluster = cg::this_cluster();
-        RD = cluster.map_shared_rank(rD, 0); RB = cluster.map_shared_rank(rB, 0); RU = cluster.map_shared_rank(rU, 0);
-        PD = cluster.map_shared_rank(pd, 0); PB = cluster.map_shared_rank(pb, 0);
+        ND = cluster.map_shared_rank(nd, 0);
         cluster.sync();                                     // every block of the cluster is running
     }
     mbar_wait(bar, 0);
@@ -265,7 +274,7 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
                 ++i; un = un2; dn = dn2; bn = bn2;
             }
         }
-        if (sg.z >= 0) { RD[sg.z] = D; RB[sg.z] = B; RU[sg.z] = ee; PD[sg.z] = ddt; PB[sg.z] = dbt; }
+        if (sg.z >= 0) { T* q = ND + 6 * sg.z; q[0] = D; q[1] = B; q[2] = ee; q[4] = ddt; q[5] = dbt; }
     }
     if (CL) cg::this_cluster().sync(); else __syncthreads();
     HINES_STAMP(2);
@@ -275,66 +284,119 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
         const int4* bdesc = reinterpret_cast<const int4*>(imeta + it.bdesc_off);
         const int32_t* pnode = imeta + it.pnode_off;
         // ---- P2 backward: reduced tree, deepest level first ----
-        for (int lev = it.nlev - 1; lev >= 0; --lev) {
-            const int eb = lvl[lev], ee_ = lvl[lev + 1];
-            for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
-                const int e = base + lane;
-                int4 ds = make_int4(0, 0, 0, 0);
-                if (e < ee_) ds = bdesc[e];
-                const int4 d0 = bdesc[base];                     // tile-uniform fields (same in every lane of the tile)
-                const int nseg = ds.x & 0xffff, nafter = (ds.x >> 16) & 0xff, wmax = (d0.x >> 24) & 0xff;
-                const int nlead = ds.w & 0xffff, nmax = (d0.w >> 16) & 0xffff;
-                int node = nseg > 1 ? ds.y + nseg - 2 : e;       // last node of the branch
-                T D = T(1), B = T(0), dd = T(0), db = T(0);
-                if (nseg > 0) {
-                    D = rD[node]; B = rB[node];
-                    for (int c = 0; c < nlead; ++c) { D -= pd[ds.z + c]; B -= pb[ds.z + c]; }   // pull
+        // One lane per branch.  After a level's barrier the only new data a lane needs is the hand-off
+        // slot of its children; its descriptor is fetched one level ahead.  The working warp's
+        // instruction count per level is what bounds this phase, hence the lean "fast tile" path.
+        typedef typename Vec2<T>::type V2;
+        auto backward_general = [&](int e, int4 ds, int x0, int w0) {
+            const int nseg = ds.x & 0xffff, nafter = (ds.x >> 16) & 0xff;
+            const int wmax = (x0 >> 24) & 0x1f, nlead = ds.w & 0xffff, nmax = (w0 >> 16) & 0xffff;
+            const T* cq = nd + 6 * ds.z;                         // hand-off slots of the children (the zero node if none)
+            T* q = nd + 6 * (nseg > 1 ? ds.y + nseg - 2 : e);    // last node of the branch
+            T D = T(1), B = T(0), U = T(0), dd = T(0), db = T(0);
+            if (nseg > 0) {
+                D = q[0]; B = q[1]; U = q[2]; dd = q[4]; db = q[5];
+                D -= cq[4]; B -= cq[5];                          // pull; the zero node if no children
+                for (int c = 1; c < nlead; ++c) { D -= cq[6 * c + 4]; B -= cq[6 * c + 5]; }
+                const T r = rcp<T>(D);
+                const T f = U * r;
+                q[0] = -f; q[1] = B * r;
+                dd = fmad<T>(f, U, dd);                          // f U + parked contribution of the segment
+                db = fmad<T>(f, B, db);
+            }
+            for (int k = 1; k < nmax; ++k) {                     // branches of several segments: walk up in lock-step
+                if (k < nseg) {
+                    q = (k + 1 == nseg) ? nd + 6 * e : q - 6;
+                    D = q[0] - dd; B = q[1] - db; U = q[2];
+                    const T r = rcp<T>(D);
+                    const T f = U * r;
+                    q[0] = -f; q[1] = B * r;
+                    dd = fmad<T>(f, U, q[4]);
+                    db = fmad<T>(f, B, q[5]);
                 }
-                for (int k = 0; k < nmax; ++k) {                 // lanes walk their nodes in lock-step
-                    if (k < nseg) {
-                        const T r = rcp<T>(D);
-                        const T U = rU[node];
-                        const T f = U * r;
-                        rD[node] = f; rB[node] = B * r;
-                        dd = fmad<T>(f, U, pd[node]);            // f U + parked contribution of the segment
-                        db = fmad<T>(f, B, pb[node]);
-                        if (k + 1 < nseg) {
-                            node = (k + 2 == nseg) ? e : node - 1;
-                            D = rD[node] - dd; B = rB[node] - db;
-                        }
-                    }
-                }
-                // hand-off at the branch point: siblings sit in one tile, the group's first lane sums
-                // their values by shuffle (fixed order) and leaves the sum in its slot
+            }
+            // hand-off at the branch point: siblings sit in one tile, the group's first lane sums
+            // their values by shuffle (fixed order) and leaves the sum in its slot
+            if (wmax > 0) {
                 const T dd0 = dd, db0 = db;
                 for (int k = 1; k <= wmax; ++k) {
                     const T vd = __shfl_down_sync(FULL, dd0, k);
                     const T vb = __shfl_down_sync(FULL, db0, k);
                     if (k <= nafter) { dd += vd; db += vb; }
                 }
-                if (nseg > 0) { pd[e] = dd; pb[e] = db; }
             }
-            __syncthreads();
-        }
-        HINES_STAMP(3);
-        // ---- P2 forward: root level first; a root has f = 0, so x = c ----
-        for (int lev = 0; lev < it.nlev; ++lev) {
-            const int eb = lvl[lev], ee_ = lvl[lev + 1];
-            for (int base = eb + (tid & ~31); base < ee_; base += nthreads) {
-                const int e = base + lane;
-                int4 ds = make_int4(0, 0, 0, 0);
-                int pn = -1;
-                if (e < ee_) { ds = bdesc[e]; pn = pnode[e]; }
-                const int nseg = ds.x & 0xffff, nmax = (ds.w >> 16) & 0xffff;
-                T xp = pn >= 0 ? rB[pn] : T(0);
-                int node = e;
-                for (int k = 0; k < nmax; ++k) {
-                    if (k < nseg) {
-                        xp = fnma<T>(rD[node], xp, rB[node]);
-                        rB[node] = xp;
-                        node = k == 0 ? ds.y : node + 1;
+            if (nseg > 0) { T* t = nd + 6 * e; t[4] = dd; t[5] = db; }
+        };
+        {
+            const int wbase = tid & ~31;
+            const int dummy = it.nnode - 1;
+            int eb = lvl[it.nlev - 1], ee_ = lvl[it.nlev];
+            int nb = it.nlev > 1 ? lvl[it.nlev - 2] : 0;
+            int4 ds = make_int4(0, 0, dummy, 0);
+            if (eb + tid < ee_) ds = bdesc[eb + tid];
+            for (int lev = it.nlev - 1; lev >= 0; --lev) {
+                const int e = eb + tid;
+                TR(8 * lev + 0);
+                if (eb + wbase < ee_) {                          // this warp has lanes on the level
+                    const int x0 = __shfl_sync(FULL, ds.x, 0), w0 = __shfl_sync(FULL, ds.w, 0);   // tile-uniform fields
+                    if (x0 & (1 << 30)) {
+                        // fast tile: one node per branch, at most two siblings, one slot to pull
+                        V2* q = reinterpret_cast<V2*>(nd + 6 * e);
+                        const bool act = (ds.x & 0xffff) != 0;
+                        T dd = T(0), db = T(0);
+                        if (act) {
+                            const V2 c2 = *reinterpret_cast<const V2*>(nd + 6 * ds.z + 4);
+                            const V2 a0 = q[0], a2 = q[2];
+                            const T U = nd[6 * e + 2];
+                            const T D = a0.x - c2.x, B = a0.y - c2.y;
+                            TR(8 * lev + 1);
+                            const T r = rcp<T>(D);
+                            const T f = U * r;
+                            V2 o; o.x = -f; o.y = B * r;
+                            q[0] = o;
+                            dd = fmad<T>(f, U, a2.x); db = fmad<T>(f, B, a2.y);
+                        }
+                        TR(8 * lev + 2);
+                        const T vd = __shfl_down_sync(FULL, dd, 1), vb = __shfl_down_sync(FULL, db, 1);
+                        if (ds.x & 0x10000) { dd += vd; db += vb; }
+                        if (act) { V2 o; o.x = dd; o.y = db; q[2] = o; }
+                        TR(8 * lev + 3);
+                    } else {
+                        backward_general(e, ds, x0, w0);
                     }
                 }
+                for (int base = eb + wbase + nthreads; base < ee_; base += nthreads) {   // levels wider than the block
+                    int4 d2 = make_int4(0, 0, dummy, 0);
+                    if (base + lane < ee_) d2 = bdesc[base + lane];
+                    backward_general(base + lane, d2, __shfl_sync(FULL, d2.x, 0), __shfl_sync(FULL, d2.w, 0));
+                }
+                // next level's descriptor, in flight across the barrier
+                ee_ = eb; eb = nb;
+                nb = lev > 1 ? lvl[lev - 2] : 0;
+                ds = make_int4(0, 0, dummy, 0);
+                if (lev > 0 && eb + tid < ee_) ds = bdesc[eb + tid];
+                TR(8 * lev + 4);
+                __syncthreads();
+                TR(8 * lev + 5);
+            }
+        }
+        HINES_STAMP(3);
+        // ---- P2 forward by pointer jumping over the reduced tree --------------
+        // x_v = c_v + g_v x_p(v), g = -f, g_root = 0.  One round replaces (g_v, c_v, p(v)) by
+        // (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds >= nodes on the longest
+        // root path) every g is 0 and c is x.  All nodes work in every round, with one barrier per
+        // round instead of one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
+        for (int r = 0; r < it.rounds; ++r) {
+            const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
+            for (int v = tid; v < it.nnode; v += nthreads) {
+                int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
+                const int p = r == 0 ? pnode[v] : ip[(r - 1) & 1];
+                const V2 a = *reinterpret_cast<const V2*>(nd + 6 * v + sbuf);
+                const V2 ap = *reinterpret_cast<const V2*>(nd + 6 * p + sbuf);
+                const int pp = r == 0 ? pnode[p] : reinterpret_cast<const int*>(nd + 6 * p + 4)[(r - 1) & 1];
+                V2 o; o.x = a.x * ap.x; o.y = fmad<T>(a.x, ap.y, a.y);
+                *reinterpret_cast<V2*>(nd + 6 * v + dbuf) = o;
+                ip[r & 1] = pp;
             }
             __syncthreads();
         }
@@ -344,6 +406,7 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
     if (CL) cg::this_cluster().sync();
     HINES_STAMP(4);
 
+    const int xs = 2 * (it.rounds & 1) + 1;               // record slot that holds x after the forward sweep
     // ---- P3: expand the interiors (lanes aligned at the segment start so that the shared-memory
     //      addresses of a wavefront keep their distinct residues) ----
     for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
@@ -354,7 +417,7 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
         const int mmax = __reduce_max_sync(FULL, m);
         const int a = sg.x + off;
         T xt = T(0), xn = T(0);
-        if (sg.z >= 0) { xn = RB[sg.z]; if (sg.w >= 0) xt = RB[sg.w]; sb[a + m] = xn; }
+        if (sg.z >= 0) { xn = ND[6 * sg.z + xs]; if (sg.w >= 0) xt = ND[6 * sg.w + xs]; sb[a + m] = xn; }
         T g1 = T(0), h1 = T(0), c1 = T(0);
         if (m > 0) { g1 = sd[a + m - 1]; h1 = su[a + m - 1]; c1 = sb[a + m - 1]; }
         for (int j = mmax - 1; j >= 0; --j) {
@@ -582,6 +645,10 @@ static hines_status_t check_ptrs(const hines_plan* P, const void* d, const void*
 using namespace hines;
 
 extern "C" {
+
+#ifdef HINES_P2_TRACE
+int hines_debug_read_trace(long long* dst) { return (int)cudaMemcpyFromSymbol(dst, hines::g_trace, sizeof(long long) * 1024); }
+#endif
 
 hines_status_t hines_plan_upload(hines_plan_t* P)
 {

@@ -21,6 +21,8 @@ def solve_with_tables(plan, m, d, u, b):
     desc = plan.table("item_desc").reshape(-1, 4)
     pnode_all = plan.table("item_pnode")
     nnode = plan.table("item_nnode")
+    node_off = plan.table("item_node_offsets")
+    rounds = plan.table("item_rounds")
     ch_off = plan.table("item_chunk_offsets")
     ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
     seg_off = plan.table("chunk_seg_offsets")
@@ -54,7 +56,8 @@ def solve_with_tables(plan, m, d, u, b):
             work.append((g0, g1, sd, su, sb, sg))
         # P2
         dsc = desc[desc_off[it]:desc_off[it + 1]]
-        pn = pnode_all[desc_off[it]:desc_off[it + 1]]
+        pn = pnode_all[node_off[it]:node_off[it + 1]]
+        assert len(pn) == NN
         lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
         nlev = len(lb) - 1
         for lev in range(nlev - 1, -1, -1):
@@ -87,18 +90,14 @@ def solve_with_tables(plan, m, d, u, b):
                 j = e - lb[lev]
                 assert j % 32 + nafter < 32, "sibling group leaves its tile"
                 pd[e] = dd[j] + sum(dd[j + 1:j + 1 + nafter]); pb[e] = db[j] + sum(db[j + 1:j + 1 + nafter])
-        for lev in range(nlev):
-            for e in range(lb[lev], lb[lev + 1]):
-                w0, rest = int(dsc[e, 0]), int(dsc[e, 1])
-                nseg = w0 & 0xffff
-                if nseg == 0:
-                    continue
-                xp = rB[pn[e]] if pn[e] >= 0 else 0.0
-                node = e
-                for k in range(nseg):
-                    xp = rB[node] - rD[node] * xp
-                    rB[node] = xp
-                    node = rest if k == 0 else node + 1
+        # forward sweep by pointer jumping: x_v = c_v + g_v x_p(v), g = -f (a root: g = 0, p = itself)
+        real = ~np.isnan(rD)
+        g = np.where(real, -rD, 0.0); c = np.where(real, rB, 0.0); par = pn.astype(np.int64).copy()
+        assert (par[~real] == np.nonzero(~real)[0]).all() and real[par[real]].all()
+        for _ in range(int(rounds[it])):
+            g, c, par = g * g[par], c + g * c[par], par[par]
+        assert (g[real] == 0).all(), "not enough pointer-jumping rounds"
+        rB = c
         # P3
         for g0, g1, sd, su, sb, sg in work:
             for a, mm, node, tnode in sg:

@@ -109,6 +109,8 @@ def _check_policy(m, plan, max_segment=64):
     desc = plan.table("item_desc").reshape(-1, 4)
     pnode = plan.table("item_pnode")
     nnode = plan.table("item_nnode")
+    node_off = plan.table("item_node_offsets")
+    rounds = plan.table("item_rounds")
     ch_off = plan.table("item_chunk_offsets")
     ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
     seg_off = plan.table("chunk_seg_offsets")
@@ -137,7 +139,8 @@ def _check_policy(m, plan, max_segment=64):
         cr = ch_rng[ch_off[it]:ch_off[it + 1]]
         assert cr[0, 0] == comp0 and cr[-1, 1] == comp0 + n_it and (cr[1:, 0] == cr[:-1, 1]).all()
         dsc = desc[desc_off[it]:desc_off[it + 1]]
-        pn = pnode[desc_off[it]:desc_off[it + 1]]
+        pn = pnode[node_off[it]:node_off[it + 1]]
+        assert len(pn) == nnode[it]
         lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
         nlev = len(lb) - 1
         assert nlev == T.cell_nlevels[c0:c1].max() and lb[0] == 0 and lb[-1] == len(dsc)
@@ -179,13 +182,14 @@ def _check_policy(m, plan, max_segment=64):
             tile_l = dsc[lb[l]:lb[l + 1]]
             for e in range(lb[l], lb[l + 1]):
                 w0, rest, cfirst, w3 = (int(v) for v in dsc[e])
-                nseg, nafter, wmax = w0 & 0xffff, (w0 >> 16) & 0xff, (w0 >> 24) & 0xff
+                nseg, nafter, wmax, fast = w0 & 0xffff, (w0 >> 16) & 0xff, (w0 >> 24) & 0x1f, (w0 >> 30) & 1
                 nlead, smx = w3 & 0xffff, (w3 >> 16) & 0xffff
                 t0 = lb[l] + (e - lb[l]) // 32 * 32
                 tl = dsc[t0:min(t0 + 32, lb[l + 1])]
                 assert wmax == ((tl[:, 0] >> 16) & 0xff).max() and smx == (tl[:, 0] & 0xffff).max()
+                assert fast == int(smx <= 1 and wmax <= 1 and (tl[:, 3] & 0xffff).max() <= 1)
                 if nseg == 0:
-                    assert pn[e] == -1 and nafter == 0
+                    assert pn[e] == e and nafter == 0
                     continue
                 start = top_node_pos[e]                      # the top segment starts at the branch start
                 ln, pc, lw = want[start]
@@ -201,11 +205,12 @@ def _check_policy(m, plan, max_segment=64):
                     node = e if k == 0 else rest + k - 1
                     tn = (e if k == 1 else rest + k - 2) if k > 0 else (node_at[pc] if pc >= 0 else -1)
                     assert seg_of_node[node] == (a_, b_ - a_, tn), (it, e, k)
-                assert pn[e] == (node_at[pc] if pc >= 0 else -1)
+                    assert k == 0 or pn[node] == tn
+                assert pn[e] == (node_at[pc] if pc >= 0 else e)          # a root reads itself (its f is 0)
                 # the children of this branch hang off its last compartment
                 kids = sorted(s_ for s_, (ln2, pc2, l2) in want.items() if pc2 == end)
                 if not kids:
-                    assert nlead == 0
+                    assert nlead == 0 and cfirst == nnode[it] - 1        # pulls the all-zero node
                 else:
                     kid_lanes = sorted(node_at_start for node_at_start in
                                        (n_ for n_, pos in top_node_pos.items() if pos in kids and n_ < len(dsc)))
