@@ -151,55 +151,39 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------------
-def main():
-    ap = argparse.ArgumentParser()
-    ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
-    ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[] index (default 2)")
-    ap.add_argument("--scale", type=float, default=1.0)
-    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--threads", type=int, default=0)
-    ap.add_argument("--policy", type=int, default=0)
-    ap.add_argument("--group-smem", type=int, default=0)
-    ap.add_argument("--smem", type=int, default=0)
-    args = ap.parse_args()
-    if args.warmup < 3:
-        args.warmup = 3
-    if args.impl == "reference":
-        return run_reference(args)
-
+def reduce_over_ranks(ms: float, e2e_s_per_step: float, units: float, dist=None, device="cpu"):
+    """Whole-job numbers from per-rank ones: time = MAX over ranks, units = SUM over ranks.
+    Cells are independent: this is the only communication of a multi-GPU run, and it
+    is outside the timed region.  Works on any backend (nccl on GPUs, gloo in the CPU test)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return ms, e2e_s_per_step, units
     import torch
-    import torch.distributed as dist
+    t = torch.tensor([ms, e2e_s_per_step], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    n = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(n, op=dist.ReduceOp.SUM)
+    return float(t[0]), float(t[1]), float(n[0])
+
+
+def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrier):
+    """One config on this rank's GPU: device-resident timing, per-path device time, optional e2e."""
+    import torch
     import paper_1810_12742_b200 as hb
-
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
-    torch.cuda.set_device(local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    np_dtype = np.float64 if args.dtype == "f64" else np.float32
+    np_dtype = np.float64 if dtype == "f64" else np.float32
     w = np.dtype(np_dtype).itemsize
-
-    m, d, u, b, seed = workload(args.config, args.scale, rank)
+    m, d, u, b, seed = workload(cfg, args.scale, rank)
     t0 = time.perf_counter()
-    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if args.dtype == "f64" else hb.F32,
+    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32,
                    threads_per_block=args.threads, policy_flags=args.policy, group_smem_bytes=args.group_smem,
-                   smem_bytes_per_block=args.smem)
+                   smem_bytes_per_block=args.smem, max_segment=args.max_segment, chunk_smem_bytes=args.chunk_smem,
+                   cluster_max=args.cluster_max)
     plan.upload()
     plan_s = time.perf_counter() - t0
     info = plan.info
     bytes_min = info.bytes_min
-
-    # device-resident inputs.  Working sets smaller than L2 rotate through >= 256 MB of distinct
-    # buffer sets so that no step finds its inputs in L2 ("cold"); larger ones exceed L2 by themselves.
-    nsets = 1 if bytes_min > L2_BYTES else int(np.ceil(2 * L2_BYTES / max(bytes_min, 1))) + 1
-    nsets = min(nsets, 64)
+    # device-resident inputs.  Working sets smaller than L2 rotate through > 2x L2 of distinct buffer
+    # sets so that no step finds its inputs in L2 ("cold"); larger ones exceed L2 by themselves.
+    nsets = 1 if bytes_min > L2_BYTES else min(64, int(np.ceil(2 * L2_BYTES / max(bytes_min, 1))) + 1)
     dd = torch.from_numpy(d.astype(np_dtype)).cuda()
     du = torch.from_numpy(u.astype(np_dtype)).cuda()
     sets = []
@@ -213,41 +197,33 @@ def main():
         a = sets[i % nsets]
         plan.solve(a[0], a[1], a[2], a[3], stream)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-
-    sampler = ClockSampler(local) if rank == 0 else None
-    for i in range(args.warmup):
+    for i in range(warmup):
         step(i)
     torch.cuda.synchronize()
-
-    # ---- timed region: exactly K steps -----------------------------------------------------
+    # ---- timed region: exactly `steps` steps, CUDA events on the launching stream -----------
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier(); torch.cuda.synchronize()
     w0 = time.time()
     e0.record()
-    for i in range(args.steps):
+    for i in range(steps):
         step(i)
     e1.record()
     torch.cuda.synchronize(); barrier()
     w1 = time.time()
     ms = e0.elapsed_time(e1)
     windows = [(w0, w1)]
-
-    # ---- parity of what was just timed (full batch, against the oracle) ----------------------
+    # ---- parity of what was just timed (full batch, against the oracle) -----------------------
     parity = None
-    if rank == 0 and not args.no_cpu:
+    if want_parity:
         import oracle
         dr, ur, br = (a.cpu().numpy().astype(np.float64) for a in sets[0][:3])
         xr = oracle.hines_solve(m.parent, m.cell_offsets, dr, ur, br)
         parity = float(oracle.rel_err(m.cell_offsets, sets[0][3].cpu().numpy().astype(np.float64), xr).max())
-
-    # ---- per-path device time (roofline): same steps with the library's event hook ------------
+    # ---- per-path device time (roofline): the library's event hook, events on the same stream ----
     plan.enable_timing(True)
     res_ms, str_ms = [], []
     w2 = time.time()
-    for i in range(min(args.steps, 50)):
+    for i in range(min(steps, 50)):
         step(i)
         r_, s_ = plan.timing()
         res_ms.append(r_); str_ms.append(s_)
@@ -255,61 +231,135 @@ def main():
     plan.enable_timing(False)
     windows.append((w2, w3))
     res_ms, str_ms = float(np.mean(res_ms)), float(np.mean(str_ms))
-
     # ---- end to end: pinned host buffers through hines_solve_host -----------------------------
     e2e = None
-    if not args.no_e2e:
+    if want_e2e:
         hd, hu, hb_, hx = (torch.from_numpy(np.ascontiguousarray(a, np_dtype)).pin_memory() for a in (d, u, b, np.empty_like(b)))
-        k_e2e = max(3, min(args.steps, int(np.ceil(3e9 / max(4 * m.n * w, 1)))))    # ~3 GB of traffic
+        k_e2e = max(3, min(steps, int(np.ceil(3e9 / max(4 * m.n * w, 1)))))    # ~3 GB of traffic
         for _ in range(2):
             plan.solve_host(hd, hu, hb_, hx, stream)
         barrier()
         t0 = time.perf_counter()
         for _ in range(k_e2e):
             plan.solve_host(hd, hu, hb_, hx, stream)
-        e2e_s = time.perf_counter() - t0
+        e2e_s = (time.perf_counter() - t0) / k_e2e
         barrier()
-        e2e = (m.n * k_e2e / e2e_s, k_e2e, 3 * m.n * w, m.n * w)
-    clocks = sampler.stop(windows) if sampler else None
+        e2e = {"s_per_step": e2e_s, "steps": k_e2e, "h2d": 3 * m.n * w, "d2h": m.n * w}
+    launches = plan.launches_per_solve
+    out = {"m": m, "d": d, "u": u, "b": b, "info": info, "ms": ms, "res_ms": res_ms, "str_ms": str_ms,
+           "parity": parity, "e2e": e2e, "plan_s": plan_s, "nsets": nsets, "launches": launches,
+           "windows": windows, "bytes_min": bytes_min, "bytes_literal": info.bytes_literal,
+           "classes": [int(v) for v in plan.table("class_cluster")]}
+    plan.close()
+    del sets, dd, du
+    torch.cuda.empty_cache()
+    return out
 
-    # ---- reduce over ranks: max time, sum of units -------------------------------------------
-    tot_units = m.n
+
+def load_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    ncu --set full capture (profiles/traffic.json, written by hand from that capture), or None."""
+    try:
+        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(key)
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[] index (default 1)")
+    ap.add_argument("--scale", type=float, default=1.0)
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--threads", type=int, default=0)
+    ap.add_argument("--policy", type=int, default=0)
+    ap.add_argument("--group-smem", type=int, default=0)
+    ap.add_argument("--smem", type=int, default=0)
+    ap.add_argument("--max-segment", type=int, default=0)
+    ap.add_argument("--chunk-smem", type=int, default=0)
+    ap.add_argument("--cluster-max", type=int, default=0)
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local)
     if world > 1:
-        t = torch.tensor([ms, (m.n / e2e[0]) if e2e else 0.0], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        nn = torch.tensor([m.n], dtype=torch.float64, device="cuda")
-        dist.all_reduce(nn, op=dist.ReduceOp.SUM)
-        ms, tot_units = float(t[0]), float(nn[0])
-        if e2e:
-            e2e = (tot_units / float(t[1]), e2e[1], e2e[2], e2e[3])
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    r = measure(args.config, args.dtype, args.steps, args.warmup, rank, args,
+                want_e2e=not args.no_e2e, want_parity=(rank == 0 and not args.no_cpu), barrier=barrier)
+    clocks = sampler.stop(r["windows"]) if sampler else None
+    m, info = r["m"], r["info"]
+    ms, e2e_s, tot_units = reduce_over_ranks(r["ms"], r["e2e"]["s_per_step"] if r["e2e"] else 0.0, float(m.n),
+                                             dist if world > 1 else None, "cuda")
+
+    # the other configs, short runs (parity-test cases, not bench lines): context for the headline
+    others = {}
+    if not args.no_others and world == 1 and args.scale == 1.0:
+        for cfg, dt in ((0, "f64"), (1, "f64"), (2, "f64"), (2, "f32"), (3, "f64"), (4, "f64")):
+            if cfg == args.config and dt == args.dtype:
+                continue
+            try:
+                o = measure(cfg, dt, min(args.steps, 20), 3, rank, args, False, False, barrier)
+                others[f"cfg{cfg}_{dt}"] = {
+                    "unknowns": o["m"].n, "ms_per_step": o["ms"] / min(args.steps, 20),
+                    "value": o["m"].n * min(args.steps, 20) / (o["ms"] * 1e-3),
+                    "hbm_frac": o["bytes_min"] / (o["ms"] / min(args.steps, 20) * 1e-3) / 1e9 / peak_hbm()[0],
+                    "resident_ms": o["res_ms"], "stream_ms": o["str_ms"], "launches_per_step": o["launches"],
+                    "cluster_sizes": o["classes"], "stream_cells": o["info"].n_stream_cells}
+                del o
+            except Exception as ex:                       # a context line must never kill the headline
+                others[f"cfg{cfg}_{dt}"] = {"error": str(ex)[:200]}
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
+    w = 8 if args.dtype == "f64" else 4
     ms_step = ms / args.steps
     value = tot_units * args.steps / (ms * 1e-3)
     peak, peak_src = peak_hbm()
+    res_ms, str_ms = r["res_ms"], r["str_ms"]
     kern_ms = res_ms + str_ms                       # device time of all kernels of one step (this rank)
-    achieved = bytes_min / (kern_ms * 1e-3) / 1e9
+    achieved = r["bytes_min"] / (kern_ms * 1e-3) / 1e9
     dominant = "hines_resident_kernel" if res_ms >= str_ms else "hines_stream_backward/forward"
-    traffic = None
-    try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tr.get(f"cfg{args.config}_{args.dtype}")
-    except Exception:
-        pass
 
     cpu = None
     if not args.no_cpu and world == 1:
         cores = os.cpu_count() or 1
-        t1, _, _ = cpu_oracle_time(m, d.astype(np_dtype).astype(np.float64), u.astype(np_dtype).astype(np.float64),
-                                   b.astype(np_dtype).astype(np.float64), 1, 3)
-        tn, used, _ = cpu_oracle_time(m, d, u, b, cores, 5)
-        cpu = {"value": m.n / tn, "unit": UNIT, "cores": used, "kind": "oracle",
-               "sample": f"whole workload ({m.n} unknowns), best of 5 after warm-up, parallel-for over cells",
-               "single_thread_value": m.n / t1, "cpu_count": cores}
+        # bounded sample: whole cells from the start of the batch, at most ~40 M unknowns
+        ncs = int(np.searchsorted(m.cell_offsets, min(m.n, 40_000_000), side="left"))
+        ncs = max(1, min(ncs, m.ncells))
+        ms_ = mg.Morphology(m.parent[:m.cell_offsets[ncs]], m.cell_offsets[:ncs + 1])
+        ns = ms_.n
+        t1, _, _ = cpu_oracle_time(ms_, r["d"][:ns], r["u"][:ns], r["b"][:ns], 1, 2)
+        tn, used, _ = cpu_oracle_time(ms_, r["d"][:ns], r["u"][:ns], r["b"][:ns], cores, 5)
+        cpu = {"value": ns / tn, "unit": UNIT, "cores": used, "kind": "oracle",
+               "sample": f"first {ncs} cells ({ns} unknowns) of the workload, best of 5 after warm-up, parallel-for over cells",
+               "single_thread_value": ns / t1, "cpu_count": cores}
 
+    e2e = r["e2e"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -317,25 +367,29 @@ def main():
         "config": {"workload": mg.CONFIG_NAMES[args.config], "scale": args.scale, "unknowns_per_gpu": m.n,
                    "cells_per_gpu": m.ncells, "branches_per_gpu": info.nbranches, "max_levels": info.max_levels,
                    "parallelism": f"independent cells, {world} replica(s), no collective",
-                   "l2": "inputs_exceed_l2" if nsets == 1 else f"rotating {nsets} distinct buffer sets (> 2x L2)",
-                   "resident_items": info.n_resident_items, "resident_unknowns": info.n_resident_unknowns,
+                   "l2": "inputs_exceed_l2" if r["nsets"] == 1 else f"rotating {r['nsets']} distinct buffer sets (> 2x L2)",
+                   "resident_items": info.n_resident_items, "resident_blocks": info.n_chunks,
+                   "resident_unknowns": info.n_resident_unknowns, "cluster_cells": info.n_cluster_cells,
+                   "cluster_unknowns": info.n_cluster_unknowns, "cluster_sizes_per_class": r["classes"],
                    "stream_cells": info.n_stream_cells, "stream_unknowns": info.n_stream_unknowns,
                    "size_classes": info.n_classes,
                    "lane_efficiency": info.useful_lane_steps / max(1, info.padded_lane_steps),
-                   "plan_create_s": plan_s},
-        "achieved_hbm_gbs": bytes_min * world / (ms_step * 1e-3) / 1e9,
-        "hbm_frac_of_peak_per_gpu": bytes_min / (ms_step * 1e-3) / 1e9 / peak,
-        "bytes_min_per_step": bytes_min, "bytes_literal_per_step": info.bytes_literal,
-        "gpu_launches": plan.launches_per_solve * args.steps,
+                   "plan_create_s": r["plan_s"]},
+        "achieved_hbm_gbs": r["bytes_min"] * world / (ms_step * 1e-3) / 1e9,
+        "hbm_frac_of_peak_per_gpu": r["bytes_min"] / (ms_step * 1e-3) / 1e9 / peak,
+        "bytes_min_per_step": r["bytes_min"], "bytes_literal_per_step": r["bytes_literal"],
+        "gpu_launches": r["launches"] * args.steps,
         "clocks": clocks,
-        "e2e": None if e2e is None else {"value": e2e[0], "unit": UNIT, "steps": e2e[1],
-                                         "h2d_bytes_per_step": e2e[2] * world, "d2h_bytes_per_step": e2e[3] * world},
+        "e2e": None if e2e is None else {"value": tot_units / e2e_s, "unit": UNIT, "steps": e2e["steps"],
+                                         "h2d_bytes_per_step": e2e["h2d"] * world, "d2h_bytes_per_step": e2e["d2h"] * world},
         "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                     "resident_ms": res_ms, "stream_ms": str_ms,
-                     "note": "achieved = bytes_min / device time of one step's kernels (library event hook)"},
+                     "frac": achieved / peak, "traffic": load_traffic(f"cfg{args.config}_{args.dtype}"),
+                     "peak_source": peak_src, "resident_ms": res_ms, "stream_ms": str_ms,
+                     "note": "achieved = bytes_min (N*4w + 4*branches, all launches of one step) / device time of one "
+                             "step's kernels, CUDA events recorded by the library on the launching stream"},
         "cpu_baseline": cpu,
-        "parity_max_rel_err": parity,
+        "parity_max_rel_err": r["parity"],
+        "other_configs": others,
     }
     print(json.dumps(line))
     if world > 1:
