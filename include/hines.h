@@ -56,6 +56,8 @@ enum {
     HINES_POLICY_NO_GROUPING  = 2,   /* one cell per shared-memory work item (paper: >= 1 cell per block) */
     HINES_POLICY_INPUT_ORDER  = 4,   /* launch work items in input order, not heaviest first (PAPER.md:128
                                         "greedy": cells are taken in the order given)                     */
+    HINES_POLICY_SERIAL_CLASSES = 16, /* launch the size classes one after the other on the caller's stream instead
+                                        of concurrently on plan-owned side streams (forked from / joined to it)  */
     HINES_POLICY_NO_CLUSTER   = 8    /* never spread a cell over a thread-block cluster: a cell either fits one
                                         block's shared memory or goes to the streaming path               */
 };

@@ -49,6 +49,9 @@ struct DeviceTables {
     void* ws_c = nullptr;           // streaming workspace: c
     void* host_stage[4] = {nullptr, nullptr, nullptr, nullptr};   // hines_solve_host device buffers d,u,b,x
     cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};              // timing hook
+    static const int kSide = 3;                                   // side streams: size classes run concurrently
+    cudaStream_t side[kSide] = {nullptr, nullptr, nullptr};
+    cudaEvent_t fork = nullptr, join[kSide] = {nullptr, nullptr, nullptr};
     bool timing = false, timed_once = false;
     unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident block, launch order
     bool prof_on = false;
@@ -524,6 +527,9 @@ static void free_device(DeviceTables* D)
     cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
+    for (cudaStream_t t : D->side) if (t) cudaStreamDestroy(t);
+    for (cudaEvent_t e : D->join) if (e) cudaEventDestroy(e);
+    if (D->fork) cudaEventDestroy(D->fork);
     delete D;
 }
 
@@ -576,6 +582,13 @@ static hines_status_t upload(hines_plan* P)
             if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
             if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         }
+        if (P->class_smem_bytes.size() > 1 && !(P->opt.policy_flags & HINES_POLICY_SERIAL_CLASSES)) {
+            CUDA_TRY(cudaEventCreateWithFlags(&D->fork, cudaEventDisableTiming));
+            for (int k = 0; k < DeviceTables::kSide; ++k) {
+                CUDA_TRY(cudaStreamCreateWithFlags(&D->side[k], cudaStreamNonBlocking));
+                CUDA_TRY(cudaEventCreateWithFlags(&D->join[k], cudaEventDisableTiming));
+            }
+        }
         return HINES_OK;
     };
     st = run();
@@ -589,22 +602,35 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
 {
     DeviceTables* D = P->dev;
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
+    // size classes are independent: the first runs on the caller's stream, the others on side streams
+    // forked from it and joined back, so that their blocks share the SMs and fill each other's tails
     int64_t first_block = 0;
+    const bool forked = D->fork != nullptr;
+    bool used[DeviceTables::kSide] = {false, false, false};
+    if (forked) CUDA_TRY(cudaEventRecord(D->fork, stream));
+    int nth = 0;
     for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
         const int64_t cnt = P->class_count[q];
         if (!cnt) continue;
         const int cl = P->class_cluster[q];
+        cudaStream_t ls = stream;
+        if (forked && nth > 0) {
+            const int k = (nth - 1) % DeviceTables::kSide;
+            ls = D->side[k];
+            if (!used[k]) { CUDA_TRY(cudaStreamWaitEvent(ls, D->fork, 0)); used[k] = true; }
+        }
+        ++nth;
         unsigned long long* prof = D->prof_on ? D->prof + 8 * first_block : nullptr;
         const int32_t* ord = D->launch_order + P->class_first[q];
         if (cl == 1) {
-            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], stream>>>(
+            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], ls>>>(
                 D->items, D->chunks, ord, D->item_meta, d, u, b, x, P->n, prof);
         } else {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3((unsigned)(cnt * cl));
             cfg.blockDim = dim3((unsigned)P->class_threads[q]);
             cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
-            cfg.stream = stream;
+            cfg.stream = ls;
             cudaLaunchAttribute attr[1];
             attr[0].id = cudaLaunchAttributeClusterDimension;
             attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
@@ -615,6 +641,8 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         }
         first_block += cnt * cl;
     }
+    for (int k = 0; k < DeviceTables::kSide; ++k)
+        if (used[k]) { CUDA_TRY(cudaEventRecord(D->join[k], D->side[k])); CUDA_TRY(cudaStreamWaitEvent(stream, D->join[k], 0)); }
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
     const int nlev = (int)P->stream_level_begin.size() - 1;
     const int st = P->opt.stream_threads;
