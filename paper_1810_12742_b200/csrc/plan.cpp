@@ -47,6 +47,7 @@ static const int kClassK[] = {1, 2, 3, 4, 6, 8};
 static const int kNumClassK = 6;
 static const int kRegsPerThread = 64;           // __launch_bounds__ of the resident kernel
 static const int kMaxClusterClass = 16;
+static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descriptor word 1, bits 24-25)
 static const int32_t kFastTile = 1 << 30;        // descriptor word 0, bit 30
 
 static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
@@ -89,19 +90,17 @@ struct ItemBuild {
 
 struct SegTmp { int32_t a, m, node, tnode; };
 
-// Segment lane list of one chunk.  R lanes access shared memory in one wavefront (16 x 8 B or
-// 32 x 4 B); give them distinct start residues mod R (they stay distinct while all lanes advance in
-// lock-step) and similar lengths: bucket by residue, each bucket longest first, one round = the heads
-// of all buckets, topped up from the fullest buckets when some are exhausted.
-static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
+// Segment lane list of one chunk.  R lanes access shared memory in one wavefront; they should start at
+// distinct residues mod R (they stay distinct while all lanes advance in lock-step) AND have similar
+// lengths (a warp runs as long as its longest lane).  Segments are sorted by length,
+// longest first, and cut into windows of 4 R; inside a window they are bucketed by start residue, and a
+// round takes the longest remaining segment of every bucket, topped up from the fullest buckets.
+static void order_window(const SegTmp* segs, size_t n, int R, int32_t off, bool last, std::vector<int32_t>& out)
 {
     std::vector<std::vector<SegTmp>> bucket(R);
-    for (const SegTmp& sg : segs) bucket[(sg.a + off) % R].push_back(sg);
-    for (auto& bk : bucket)
-        std::stable_sort(bk.begin(), bk.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
+    for (size_t k = 0; k < n; ++k) bucket[(segs[k].a + off) % R].push_back(segs[k]);     // stays longest first
     std::vector<size_t> head(R, 0);
-    size_t remaining = segs.size();
-    out.clear();
+    size_t remaining = n;
     std::vector<int> pick;
     std::vector<int> used(R);
     while (remaining) {
@@ -110,8 +109,7 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
         size_t taken = pick.size();
         std::fill(used.begin(), used.end(), 0);
         for (int q : pick) used[q]++;
-        // top up: second helpings from the buckets with most left (conflicts only in these tail rounds)
-        while (taken < (size_t)R && taken < remaining) {
+        while (taken < (size_t)R && taken < remaining) {          // second helpings: conflicts only here
             int best = -1; size_t left = 0;
             for (int r = 0; r < R; ++r) {
                 const size_t avail = bucket[r].size() - head[r];
@@ -121,20 +119,31 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
             if (best < 0) break;
             pick.push_back(best); used[best]++; ++taken;
         }
-        // longest first inside the round as well, so that the final order is close to length-descending
         for (int r : pick) {
             const SegTmp& sg = bucket[r][head[r]++];
             out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
             --remaining;
         }
-        if (remaining) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
+        if (remaining || !last) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
+    }
+}
+
+static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
+{
+    std::vector<SegTmp> sorted(segs);
+    std::stable_sort(sorted.begin(), sorted.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
+    out.clear();
+    const size_t W = 4 * (size_t)R;
+    for (size_t w0 = 0; w0 < sorted.size(); w0 += W) {
+        const size_t n = std::min(W, sorted.size() - w0);
+        order_window(sorted.data() + w0, n, R, off, w0 + n == sorted.size(), out);
     }
 }
 
 static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchunks, ItemBuild& out)
 {
     const int32_t smax = P.opt.max_segment;
-    const int E = 16 / P.width, R = 128 / P.width;
+    const int E = 16 / P.width;
     out = ItemBuild();
     out.nchunks = nchunks;
     out.comp_begin = P.cell_offsets[c0];
@@ -277,7 +286,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
     const int64_t meta_item = round_up(out.nlev + 1, 4) + 4 * (int64_t)out.ndesc + round_up(out.nnode, 4);
     out.leader_extra = 6 * round_up(out.nnode, E) * P.width + 4 * meta_item;
     out.chunks.assign(nchunks, ItemBuild::Chunk());
-    const int64_t per_comp = 3 * P.width, per_seg = 16;
+    const int64_t per_comp = 3 * P.width, per_seg = 32;   // two lanes per segment
     const int64_t total = out.leader_extra + per_comp * out.n + per_seg * (int64_t)segs.size();
     size_t si = 0;
     int64_t acc = 0;
@@ -300,14 +309,32 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         ch.n = mine.empty() ? 0 : mine.back().a + mine.back().m + 1 - ch.begin;
         for (SegTmp& sg : mine) sg.a -= ch.begin;
         const int32_t off = (int32_t)((out.comp_begin + ch.begin) % E);
-        order_segments(mine, R, off, ch.seg);
+        // two lanes per segment: lane A eliminates the upper half of the interior top-down, lane B the
+        // lower half bottom-up, they meet at the middle node q, which A eliminates last.  A warp holds
+        // 16 segments: A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
+        std::vector<int32_t> ord;
+        order_segments(mine, 16, off, ord);
+        while ((ord.size() / 4) % 16) ord.insert(ord.end(), {0, 0, -1, -1});
+        const int32_t ngroups = (int32_t)(ord.size() / 64);
+        ch.seg.assign((size_t)ngroups * 128, 0);
+        for (int32_t gidx = 0; gidx < ngroups; ++gidx) {
+            int32_t mx = 0;
+            for (int32_t k = 0; k < 16; ++k) {
+                const int32_t* sgp = &ord[(size_t)(gidx * 16 + k) * 4];
+                int32_t* A = &ch.seg[(size_t)(gidx * 32 + k) * 4];
+                int32_t* B = &ch.seg[(size_t)(gidx * 32 + 16 + k) * 4];
+                const int32_t a = sgp[0], mm = sgp[1], node = sgp[2], tnode = sgp[3];
+                if (node < 0) { A[2] = A[3] = B[2] = B[3] = -1; continue; }
+                const int32_t hasq = mm > 0, mt = hasq ? mm / 2 : 0, mb = hasq ? mm - 1 - mt : 0;
+                const int32_t word = mt | (mb << 12) | (hasq << 26);
+                A[0] = a; A[1] = word | (kSegA << 24); A[2] = node; A[3] = tnode;
+                B[0] = a + mm - 1; B[1] = word | (kSegB << 24); B[2] = node; B[3] = -1;
+                mx = std::max(mx, std::max(mt, mb));
+            }
+            out.padded_steps += 32 * (int64_t)(mx + 1);     // the loop steps of the warp + the step for q
+        }
         const int32_t ns = (int32_t)(ch.seg.size() / 4);
         out.max_lanes = std::max(out.max_lanes, ns);
-        for (int32_t t = 0; t < ns; t += 32) {
-            int32_t mx = 0;
-            for (int32_t i = t; i < std::min(ns, t + 32); ++i) mx = std::max(mx, ch.seg[4 * i + 1]);
-            out.padded_steps += 32 * (int64_t)mx;
-        }
         const int64_t L = round_up(off + ch.n, E);
         ch.smem_need = 16 + (r == 0 ? out.leader_extra : 0) + 3 * L * P.width + 16 * (int64_t)ns;
         out.smem_need = std::max(out.smem_need, ch.smem_need);

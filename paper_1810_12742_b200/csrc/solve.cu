@@ -22,9 +22,11 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
+#include <vector>
 
 #include "plan_internal.h"
 
@@ -255,29 +257,56 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
     const unsigned FULL = 0xffffffffu;
 
     // ---- P1: condense the interiors of all segments (no level dependency) ----
+    // Two lanes per segment [a..b] (b = separator, t = separator above): lane A eliminates the upper
+    // half a..q-1 top-down (fill-in coupling to t), lane B = A ^ 16 the lower half b-1..q+1 bottom-up
+    // (fill-in coupling to b); A then takes B's update of the middle node q, eliminates q and writes
+    // the node record of b.  Lane: node i = base + sgn s at step s.
     for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
-        const int e = base + lane;
-        int4 sg = make_int4(0, 0, -1, -1);
-        if (e < ch.nseg_lanes) sg = seg[e];
-        const int m = sg.y;
+        const int4 sg = seg[base + lane];
+        const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
+        const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
+        const bool isB = kind == 2;
+        const int m = isB ? mb : (kind == 1 ? mt : 0);
+        const int sgn = isB ? -1 : 1, uo = isB ? 0 : 1;
+        const int mload = isB ? m - 1 : m;                  // B's last step: only the update of q is wanted
         const int mmax = __reduce_max_sync(FULL, m);
         int i = sg.x + off;
-        T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(1), bn = T(0);
-        if (sg.z >= 0) { D = sd[i]; B = sb[i]; if (sg.w >= 0) ee = su[i]; }
-        if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; bn = sb[i + 1]; }
+        T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
+        if (kind == 1) { D = sd[i]; B = sb[i]; if (sg.w >= 0) ee = su[i]; }
+        if (isB && hasq) { ee = su[i + 1]; D = T(0); if (m > 0) { D = sd[i]; B = sb[i]; } }
+        if (m > 0) un = su[i + uo];
+        if (mload > 0) { dn = sd[i + sgn]; bn = sb[i + sgn]; }
         for (int s = 0; s < mmax; ++s) {
             if (s < m) {
-                T un2 = T(0), dn2 = T(1), bn2 = T(0);
-                if (s + 1 < m) { un2 = su[i + 2]; dn2 = sd[i + 2]; bn2 = sb[i + 2]; }     // next step's inputs
+                T un2 = T(0), dn2 = T(0), bn2 = T(0);
+                if (s + 1 < m) un2 = su[i + sgn + uo];                                       // next step's inputs
+                if (s + 1 < mload) { dn2 = sd[i + 2 * sgn]; bn2 = sb[i + 2 * sgn]; }
                 const T r = rcp<T>(D);
                 const T g = un * r, h = ee * r, c = B * r;
                 sd[i] = g; su[i] = h; sb[i] = c;
                 ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);
                 D = fnma<T>(g, un, dn); B = fnma<T>(g, B, bn); ee = -h * un;
-                ++i; un = un2; dn = dn2; bn = bn2;
+                i += sgn; un = un2; dn = dn2; bn = bn2;
             }
         }
-        if (sg.z >= 0) { T* q = ND + 6 * sg.z; q[0] = D; q[1] = B; q[2] = ee; q[4] = ddt; q[5] = dbt; }
+        // B -> A: update of q (pD, pB), coupling q-b (pe), contribution parked for b (pdd, pdb)
+        const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
+        T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
+        if (kind == 1) {
+            T* q = ND + 6 * sg.z;
+            if (hasq) {                                     // i is q now
+                const T Dq = D + pD, Bq = B + pB;
+                const T r = rcp<T>(Dq);
+                const T gq = pe * r, hq = ee * r;
+                sd[i] = gq; su[i] = hq; sb[i] = Bq * r;
+                ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
+                pdd = fmad<T>(gq, pe, pdd); pdb = fmad<T>(gq, Bq, pdb);
+                const int bp = i + 1 + mb;
+                q[0] = sd[bp] - pdd; q[1] = sb[bp] - pdb; q[2] = -hq * pe; q[4] = ddt; q[5] = dbt;
+            } else {                                        // a segment of one compartment: the separator as it is
+                q[0] = D; q[1] = B; q[2] = ee; q[4] = T(0); q[5] = T(0);
+            }
+        }
     }
     if (CL) cg::this_cluster().sync(); else __syncthreads();
     HINES_STAMP(2);
@@ -410,25 +439,39 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
     HINES_STAMP(4);
 
     const int xs = 2 * (it.rounds & 1) + 1;               // record slot that holds x after the forward sweep
-    // ---- P3: expand the interiors (lanes aligned at the segment start so that the shared-memory
-    //      addresses of a wavefront keep their distinct residues) ----
+    // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t], then A walks up from q-1 to a
+    //      and B walks down from q+1 to b-1, one FMA on the dependent chain per step ----
     for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
-        const int e = base + lane;
-        int4 sg = make_int4(0, 0, -1, -1);
-        if (e < ch.nseg_lanes) sg = seg[e];
-        const int m = sg.y;
+        const int4 sg = seg[base + lane];
+        const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
+        const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
+        const bool isB = kind == 2;
+        const int m = isB ? mb : (kind == 1 ? mt : 0);
+        const int sgn = isB ? -1 : 1;
         const int mmax = __reduce_max_sync(FULL, m);
-        const int a = sg.x + off;
-        T xt = T(0), xn = T(0);
-        if (sg.z >= 0) { xn = ND[6 * sg.z + xs]; if (sg.w >= 0) xt = ND[6 * sg.w + xs]; sb[a + m] = xn; }
+        const int p0 = sg.x + off;
+        T xb = T(0), xt = T(0), xn = T(0);
+        if (kind != 0) xb = ND[6 * sg.z + xs];
+        if (kind == 1) {
+            if (sg.w >= 0) xt = ND[6 * sg.w + xs];
+            if (hasq) {
+                const int iq = p0 + mt;
+                xn = fnma<T>(sd[iq], xb, fnma<T>(su[iq], xt, sb[iq]));
+                sb[iq] = xn; sb[iq + 1 + mb] = xb;
+            } else {
+                sb[p0] = xb;
+            }
+        }
+        const T xq = __shfl_xor_sync(FULL, xn, 16);
+        if (isB) { xn = xq; xt = xb; }
         T g1 = T(0), h1 = T(0), c1 = T(0);
-        if (m > 0) { g1 = sd[a + m - 1]; h1 = su[a + m - 1]; c1 = sb[a + m - 1]; }
+        if (m > 0) { const int i = p0 + sgn * (m - 1); g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
         for (int j = mmax - 1; j >= 0; --j) {
             if (j < m) {
                 T g2 = T(0), h2 = T(0), c2 = T(0);
-                if (j > 0) { g2 = sd[a + j - 1]; h2 = su[a + j - 1]; c2 = sb[a + j - 1]; }
+                if (j > 0) { const int i2 = p0 + sgn * (j - 1); g2 = sd[i2]; h2 = su[i2]; c2 = sb[i2]; }
                 xn = fnma<T>(g1, xn, fnma<T>(h1, xt, c1));       // one FMA on the dependent chain
-                sb[a + j] = xn;
+                sb[p0 + sgn * j] = xn;
                 g1 = g2; h1 = h2; c1 = c2;
             }
         }

@@ -11,6 +11,23 @@ from __future__ import annotations
 import numpy as np
 
 
+def pairs(sg):
+    """Segments of a chunk's lane list: groups of 32 lanes = 16 A lanes + their 16 B partners.
+    Yields (a, mt, mb, hasq, node, tnode) per segment and checks the pairing."""
+    for g in range(0, len(sg), 32):
+        for k in range(16):
+            A, B = sg[g + k], sg[g + 16 + k]
+            ka, kb = (int(A[1]) >> 24) & 3, (int(B[1]) >> 24) & 3
+            if ka == 0:
+                assert kb == 0 and A[2] == -1 and B[2] == -1
+                continue
+            assert ka == 1 and kb == 2 and (int(A[1]) & ~(3 << 24)) == (int(B[1]) & ~(3 << 24)) and A[2] == B[2]
+            mt, mb, hasq = int(A[1]) & 0xfff, (int(A[1]) >> 12) & 0xfff, (int(A[1]) >> 26) & 1
+            mm = mt + mb + hasq
+            assert B[0] == A[0] + mm - 1 and (hasq or (mt == 0 and mb == 0)) and abs(mt - mb) <= 1
+            yield int(A[0]), mt, mb, hasq, int(A[2]), int(A[3])
+
+
 def solve_with_tables(plan, m, d, u, b):
     """x for every cell that sits in an on-chip work item (NaN elsewhere)."""
     x = np.full(m.n, np.nan)
@@ -36,14 +53,14 @@ def solve_with_tables(plan, m, d, u, b):
             g0, g1 = ch_rng[ch]
             sd = d[g0:g1].astype(np.float64).copy(); su = u[g0:g1].astype(np.float64).copy(); sb = b[g0:g1].astype(np.float64).copy()
             sg = segs[seg_off[ch]:seg_off[ch + 1]]
-            for a, mm, node, tnode in sg:
-                if node < 0:
-                    continue
+            assert len(sg) % 32 == 0
+            for a, mt, mb, hasq, node, tnode in pairs(sg):
+                # lane A: upper half a..q-1 top-down, fill-in coupling to t
                 i = a
                 D, B = sd[i], sb[i]
                 ee = su[i] if tnode >= 0 else 0.0
                 ddt = dbt = 0.0
-                for _ in range(mm):
+                for _ in range(mt):
                     un, dn, bn = su[i + 1], sd[i + 1], sb[i + 1]
                     r = 1.0 / D
                     g, h, c = un * r, ee * r, B * r
@@ -51,8 +68,34 @@ def solve_with_tables(plan, m, d, u, b):
                     ddt += h * ee; dbt += h * B
                     D, B, ee = dn - g * un, bn - g * B, -h * un
                     i += 1
+                if hasq:
+                    q = a + mt; bp = q + 1 + mb
+                    # lane B: lower half b-1..q+1 bottom-up, fill-in coupling to b
+                    eb = su[bp]; pD = pB = pdd = pdb = 0.0
+                    if mb > 0:
+                        j = bp - 1
+                        Db, Bb = sd[j], sb[j]
+                        for s_ in range(mb):
+                            un = su[j]
+                            dn, bn = (sd[j - 1], sb[j - 1]) if s_ + 1 < mb else (0.0, 0.0)
+                            r = 1.0 / Db
+                            g, h, c = un * r, eb * r, Bb * r
+                            sd[j], su[j], sb[j] = g, h, c
+                            pdd += h * eb; pdb += h * Bb
+                            Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
+                            j -= 1
+                        pD, pB = Db, Bb
+                    Dq, Bq = D + pD, B + pB
+                    r = 1.0 / Dq
+                    gq, hq = eb * r, ee * r
+                    sd[q], su[q], sb[q] = gq, hq, Bq * r
+                    ddt += hq * ee; dbt += hq * Bq
+                    pdd += gq * eb; pdb += gq * Bq
+                    rec = (sd[bp] - pdd, sb[bp] - pdb, -hq * eb, ddt, dbt)
+                else:
+                    rec = (D, B, ee, 0.0, 0.0)
                 assert np.isnan(rD[node]), "node written twice"
-                rD[node], rB[node], rU[node], pd[node], pb[node] = D, B, ee, ddt, dbt
+                rD[node], rB[node], rU[node], pd[node], pb[node] = rec
             work.append((g0, g1, sd, su, sb, sg))
         # P2
         dsc = desc[desc_off[it]:desc_off[it + 1]]
@@ -100,14 +143,22 @@ def solve_with_tables(plan, m, d, u, b):
         rB = c
         # P3
         for g0, g1, sd, su, sb, sg in work:
-            for a, mm, node, tnode in sg:
-                if node < 0:
-                    continue
-                xn = rB[node]
+            for a, mt, mb, hasq, node, tnode in pairs(sg):
+                xb = rB[node]
                 xt = rB[tnode] if tnode >= 0 else 0.0
-                sb[a + mm] = xn
-                for j in range(mm - 1, -1, -1):
-                    xn = (sb[a + j] - su[a + j] * xt) - sd[a + j] * xn
-                    sb[a + j] = xn
+                if not hasq:
+                    sb[a] = xb
+                    continue
+                q = a + mt; bp = q + 1 + mb
+                xq = (sb[q] - su[q] * xt) - sd[q] * xb
+                sb[q] = xq; sb[bp] = xb
+                xn = xq
+                for j in range(q - 1, a - 1, -1):
+                    xn = (sb[j] - su[j] * xt) - sd[j] * xn
+                    sb[j] = xn
+                xn = xq
+                for j in range(q + 1, bp):
+                    xn = (sb[j] - su[j] * xb) - sd[j] * xn
+                    sb[j] = xn
             x[g0:g1] = sb
     return x

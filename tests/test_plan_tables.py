@@ -13,6 +13,7 @@ import morphgen as mg
 import oracle
 import paper_1810_12742_b200 as hb
 from helpers import random_parent
+from plan_interpreter import pairs
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -153,10 +154,8 @@ def _check_policy(m, plan, max_segment=64):
             sg = segs[seg_off[ch]:seg_off[ch + 1]]
             nlanes_max = max(nlanes_max, len(sg))
             base = cr[r, 0] - comp0
-            for a, mm, node, tnode in sg:
-                if node < 0:
-                    assert mm == 0
-                    continue
+            for a, mt_, mb_, hasq_, node, tnode in pairs(sg):
+                mm = mt_ + mb_ + hasq_
                 assert 0 <= node < nnode[it] and node not in seg_of_node
                 assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < max_segment
                 seg_of_node[int(node)] = (int(base + a), int(mm), int(tnode))
@@ -164,8 +163,8 @@ def _check_policy(m, plan, max_segment=64):
                 covered[base + a:base + a + mm + 1] += 1
                 useful += int(mm)
             L = -(-(cr[r, 0] % E + cr[r, 1] - cr[r, 0]) // E) * E
-            meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + -(-len(dsc) // 4) * 4
-            need = 16 + 3 * L * w + 16 * len(sg) + (5 * (-(-nnode[it] // E) * E) * w + 4 * meta if r == 0 else 0)
+            meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + -(-nnode[it] // 4) * 4
+            need = 16 + 3 * L * w + 16 * len(sg) + (6 * (-(-nnode[it] // E) * E) * w + 4 * meta if r == 0 else 0)
             assert need <= cls_smem[cls[it]] <= 232448
         assert (covered == 1).all()
         nsep_total += len(seg_of_node)
