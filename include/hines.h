@@ -75,8 +75,8 @@ typedef struct {
                                        block as possible")                                                 */
     int32_t max_segment;            /* 0 = default (64), 2..2047: branches longer than this are cut into
                                        chained segments ("we split branches that are too long") */
-    int32_t cluster_max;            /* 0 = default (8), 1..16: largest thread-block cluster a cell may be spread
-                                       over (powers of two are used; 16 needs the non-portable cluster size)  */
+    int32_t cluster_max;            /* 0 = default (16), 1..16: largest thread-block cluster a cell may be spread
+                                       over (powers of two are used; 16 is the non-portable cluster size)      */
     int32_t chunk_smem_bytes;       /* 0 = default (113 KiB, two blocks per SM): shared memory one block of a
                                        cluster item aims to stay within; also the size above which a cell is
                                        spread over a cluster instead of taking a whole SM's shared memory      */

@@ -555,21 +555,21 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     flush(nc);
 }
 
-// Size classes.  Single-block items: by how many blocks of that size fit one SM (1, 2, 3, 4, 6, 8).
-// Cluster items: one class per cluster size.  Threads per block: enough lanes for the widest segment
+// Size classes.  By how many blocks of that size fit one SM (1, 2, 3, 4, 6, 8), separately for single-block
+// items and for every cluster size.  Threads per block: enough lanes for the widest segment
 // list of the class, within what the register file allows for that many resident blocks.
 static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
 {
     const int64_t nitems = (int64_t)need.size();
     const int64_t max_smem = P.opt.smem_bytes_per_block;
-    const int nq = kNumClassK + kMaxClusterClass + 1;
+    const int nq = kNumClassK * (kMaxClusterClass + 2);   // single blocks, then per cluster size, each by blocks per SM
     std::vector<int> item_q(nitems, 0);
     std::vector<int64_t> need_max(nq, 0), count(nq, 0);
     std::vector<int32_t> lanes_max(nq, 0);
     for (int64_t i = 0; i < nitems; ++i) {
         int q = 0;
-        if (need[i].nchunks > 1) q = kNumClassK + need[i].nchunks;
-        else for (int t = 0; t < kNumClassK; ++t) if (need[i].smem <= class_cap(kClassK[t], max_smem)) q = t;
+        for (int t = 0; t < kNumClassK; ++t) if (need[i].smem <= class_cap(kClassK[t], max_smem)) q = t;
+        if (need[i].nchunks > 1) q += kNumClassK * need[i].nchunks;
         item_q[i] = q;
         need_max[q] = std::max(need_max[q], need[i].smem);
         lanes_max[q] = std::max(lanes_max[q], need[i].lanes);
@@ -577,14 +577,15 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
     }
     // launch order of the classes: clusters first (largest first), then single blocks, biggest first
     std::vector<int> qs;
-    for (int q = nq - 1; q >= kNumClassK; --q) if (count[q]) qs.push_back(q);
+    for (int k = kMaxClusterClass; k >= 2; --k)
+        for (int t = 0; t < kNumClassK; ++t) if (count[kNumClassK * k + t]) qs.push_back(kNumClassK * k + t);
     for (int q = 0; q < kNumClassK; ++q) if (count[q]) qs.push_back(q);
     std::vector<int> cls_of_q(nq, -1);
     for (int q : qs) {
         cls_of_q[q] = (int)P.class_smem_bytes.size();
         const int64_t smem = round_up(need_max[q], 128);
         P.class_smem_bytes.push_back((int32_t)smem);
-        P.class_cluster.push_back(q >= kNumClassK ? q - kNumClassK : 1);
+        P.class_cluster.push_back(q >= kNumClassK ? q / kNumClassK : 1);
         const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
         int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
         tmax = std::max<int64_t>(128, std::min<int64_t>(1024, tmax));
@@ -688,7 +689,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.stream_threads == 0) o.stream_threads = 128;
     if (o.group_smem_bytes == 0) o.group_smem_bytes = 57344;
     if (o.max_segment == 0) o.max_segment = 64;
-    if (o.cluster_max == 0) o.cluster_max = 8;
+    if (o.cluster_max == 0) o.cluster_max = 16;
     if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 113 * 1024;
     if (o.threads_per_block < 0 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||

@@ -39,11 +39,11 @@ __device__ long long g_trace[1024];
 #define TR(i) do {} while (0)
 #endif
 
+struct BlockRec { ItemHeader it; ChunkHeader ch; };   // 80 bytes
+
 struct DeviceTables {
     int device = -1;
-    ItemHeader* items = nullptr;
-    ChunkHeader* chunks = nullptr;
-    int32_t* launch_order = nullptr;
+    BlockRec* recs = nullptr;                                     // one per resident block, launch order
     int32_t* item_meta = nullptr;
     StreamDesc* stream_desc = nullptr;
     int32_t* stream_child = nullptr;
@@ -54,6 +54,8 @@ struct DeviceTables {
     static const int kSide = 3;                                   // side streams: size classes run concurrently
     cudaStream_t side[kSide] = {nullptr, nullptr, nullptr};
     cudaEvent_t fork = nullptr, join[kSide] = {nullptr, nullptr, nullptr};
+    cudaStream_t sstream = nullptr;                               // the streaming path runs beside the resident classes
+    cudaEvent_t sjoin = nullptr;
     bool timing = false, timed_once = false;
     unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident block, launch order
     bool prof_on = false;
@@ -189,8 +191,7 @@ template <> __device__ __forceinline__ float fmad<float>(float a, float b, float
 // ------------------------------------------------------------------------------------------------
 template <typename T, bool CL>
 __global__ void __launch_bounds__(1024, 1)
-hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* __restrict__ chunks,
-                      const int32_t* __restrict__ order, const int32_t* __restrict__ meta_g,
+hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restrict__ meta_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
                       int64_t n_total, unsigned long long* prof)
 {
@@ -203,8 +204,11 @@ hines_resident_kernel(const ItemHeader* __restrict__ items, const ChunkHeader* _
     constexpr int E = 16 / (int)sizeof(T);
     unsigned rank = 0, csize = 1;
     if (CL) { rank = cg::this_cluster().block_rank(); csize = cg::this_cluster().num_blocks(); }
-    const ItemHeader it = items[order[blockIdx.x / csize]];
-    const ChunkHeader ch = chunks[it.first_chunk + rank];
+    // one record per block, in launch order: the block's item and chunk headers side by side, so that
+    // a single dependent global load stands between the block's start and its bulk copies
+    const ItemHeader it = recs[blockIdx.x].it;
+    const ChunkHeader ch = recs[blockIdx.x].ch;
+    (void)csize;
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
     const int off = (int)(ch.comp_begin % E);
     const int64_t g0 = ch.comp_begin - off;                 // 16-byte aligned global element index
@@ -566,13 +570,15 @@ static hines_status_t upload_vec(const V& v, void** dst, int64_t& total)
 static void free_device(DeviceTables* D)
 {
     if (!D) return;
-    cudaFree(D->items); cudaFree(D->chunks); cudaFree(D->launch_order); cudaFree(D->item_meta); cudaFree(D->stream_desc);
+    cudaFree(D->recs); cudaFree(D->item_meta); cudaFree(D->stream_desc);
     cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
     for (cudaStream_t t : D->side) if (t) cudaStreamDestroy(t);
     for (cudaEvent_t e : D->join) if (e) cudaEventDestroy(e);
     if (D->fork) cudaEventDestroy(D->fork);
+    if (D->sstream) cudaStreamDestroy(D->sstream);
+    if (D->sjoin) cudaEventDestroy(D->sjoin);
     delete D;
 }
 
@@ -597,9 +603,15 @@ static hines_status_t upload(hines_plan* P)
                 set_error("device offers " + std::to_string(max_optin) + " bytes of shared memory per block, plan needs " + std::to_string(s));
                 return HINES_ERR_UNSUPPORTED;
             }
-        if ((st = upload_vec(P->item_headers, (void**)&D->items, D->bytes))) return st;
-        if ((st = upload_vec(P->chunk_headers, (void**)&D->chunks, D->bytes))) return st;
-        if ((st = upload_vec(P->item_launch_order, (void**)&D->launch_order, D->bytes))) return st;
+        {
+            std::vector<BlockRec> recs;
+            recs.reserve(P->chunk_headers.size());
+            for (int32_t item : P->item_launch_order) {
+                const ItemHeader& h = P->item_headers[item];
+                for (int32_t r = 0; r < h.nchunks; ++r) recs.push_back(BlockRec{h, P->chunk_headers[h.first_chunk + r]});
+            }
+            if ((st = upload_vec(recs, (void**)&D->recs, D->bytes))) return st;
+        }
         if ((st = upload_vec(P->item_meta, (void**)&D->item_meta, D->bytes))) return st;
         if ((st = upload_vec(P->stream_desc, (void**)&D->stream_desc, D->bytes))) return st;
         if ((st = upload_vec(P->stream_child, (void**)&D->stream_child, D->bytes))) return st;
@@ -625,8 +637,13 @@ static hines_status_t upload(hines_plan* P)
             if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
             if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         }
-        if (P->class_smem_bytes.size() > 1 && !(P->opt.policy_flags & HINES_POLICY_SERIAL_CLASSES)) {
+        const bool has_stream_path = P->stream_level_begin.size() > 1;
+        if (P->class_smem_bytes.size() + (has_stream_path ? 1 : 0) > 1 && !(P->opt.policy_flags & HINES_POLICY_SERIAL_CLASSES)) {
             CUDA_TRY(cudaEventCreateWithFlags(&D->fork, cudaEventDisableTiming));
+            if (has_stream_path && !P->class_smem_bytes.empty()) {
+                CUDA_TRY(cudaStreamCreateWithFlags(&D->sstream, cudaStreamNonBlocking));
+                CUDA_TRY(cudaEventCreateWithFlags(&D->sjoin, cudaEventDisableTiming));
+            }
             for (int k = 0; k < DeviceTables::kSide; ++k) {
                 CUDA_TRY(cudaStreamCreateWithFlags(&D->side[k], cudaStreamNonBlocking));
                 CUDA_TRY(cudaEventCreateWithFlags(&D->join[k], cudaEventDisableTiming));
@@ -645,12 +662,34 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
 {
     DeviceTables* D = P->dev;
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
+    auto launch_streaming = [&](cudaStream_t ss) -> hines_status_t {
+        const int nlev = (int)P->stream_level_begin.size() - 1;
+        const int st = P->opt.stream_threads;
+        T* wf = static_cast<T*>(D->ws_f); T* wc = static_cast<T*>(D->ws_c);
+        for (int l = nlev - 1; l >= 0; --l) {
+            const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
+            hines_stream_backward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, ss>>>(
+                D->stream_desc, b0, b1, reinterpret_cast<const int2*>(D->stream_child), d, u, b, wf, wc);
+        }
+        for (int l = 0; l < nlev; ++l) {
+            const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
+            hines_stream_forward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, ss>>>(
+                D->stream_desc, b0, b1, wf, wc, x);
+        }
+        CUDA_TRY(cudaGetLastError());
+        return HINES_OK;
+    };
     // size classes are independent: the first runs on the caller's stream, the others on side streams
     // forked from it and joined back, so that their blocks share the SMs and fill each other's tails
     int64_t first_block = 0;
     const bool forked = D->fork != nullptr;
     bool used[DeviceTables::kSide] = {false, false, false};
     if (forked) CUDA_TRY(cudaEventRecord(D->fork, stream));
+    if (D->sstream) {                                   // cells of the streaming path are independent of the rest
+        CUDA_TRY(cudaStreamWaitEvent(D->sstream, D->fork, 0));
+        if (hines_status_t sst = launch_streaming(D->sstream)) return sst;
+        CUDA_TRY(cudaEventRecord(D->sjoin, D->sstream));
+    }
     int nth = 0;
     for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
         const int64_t cnt = P->class_count[q];
@@ -664,10 +703,10 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         }
         ++nth;
         unsigned long long* prof = D->prof_on ? D->prof + 8 * first_block : nullptr;
-        const int32_t* ord = D->launch_order + P->class_first[q];
+        const BlockRec* recs = D->recs + first_block;
         if (cl == 1) {
             hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], ls>>>(
-                D->items, D->chunks, ord, D->item_meta, d, u, b, x, P->n, prof);
+                recs, D->item_meta, d, u, b, x, P->n, prof);
         } else {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3((unsigned)(cnt * cl));
@@ -678,8 +717,7 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
             attr[0].id = cudaLaunchAttributeClusterDimension;
             attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
             cfg.attrs = attr; cfg.numAttrs = 1;
-            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, (const ItemHeader*)D->items,
-                                        (const ChunkHeader*)D->chunks, ord, (const int32_t*)D->item_meta, d, u, b, x,
+            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, recs, (const int32_t*)D->item_meta, d, u, b, x,
                                         (int64_t)P->n, prof));
         }
         first_block += cnt * cl;
@@ -687,19 +725,8 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
     for (int k = 0; k < DeviceTables::kSide; ++k)
         if (used[k]) { CUDA_TRY(cudaEventRecord(D->join[k], D->side[k])); CUDA_TRY(cudaStreamWaitEvent(stream, D->join[k], 0)); }
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
-    const int nlev = (int)P->stream_level_begin.size() - 1;
-    const int st = P->opt.stream_threads;
-    T* wf = static_cast<T*>(D->ws_f); T* wc = static_cast<T*>(D->ws_c);
-    for (int l = nlev - 1; l >= 0; --l) {
-        const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
-        hines_stream_backward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, stream>>>(
-            D->stream_desc, b0, b1, reinterpret_cast<const int2*>(D->stream_child), d, u, b, wf, wc);
-    }
-    for (int l = 0; l < nlev; ++l) {
-        const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
-        hines_stream_forward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, stream>>>(
-            D->stream_desc, b0, b1, wf, wc, x);
-    }
+    if (D->sstream) CUDA_TRY(cudaStreamWaitEvent(stream, D->sjoin, 0));
+    else if (hines_status_t sst = launch_streaming(stream)) return sst;
     if (D->timing) { CUDA_TRY(cudaEventRecord(D->ev[2], stream)); D->timed_once = true; }
     CUDA_TRY(cudaGetLastError());
     return HINES_OK;
