@@ -58,6 +58,8 @@ enum {
                                         "greedy": cells are taken in the order given)                     */
     HINES_POLICY_SERIAL_CLASSES = 16, /* launch the size classes one after the other on the caller's stream instead
                                         of concurrently on plan-owned side streams (forked from / joined to it)  */
+    HINES_POLICY_POW2_CLUSTERS = 32, /* cluster sizes 2, 4, 8, 16 only (default: any size up to cluster_max, the one
+                                        whose blocks fill their shared-memory slot best)                     */
     HINES_POLICY_NO_CLUSTER   = 8    /* never spread a cell over a thread-block cluster: a cell either fits one
                                         block's shared memory or goes to the streaming path               */
 };
@@ -76,7 +78,7 @@ typedef struct {
     int32_t max_segment;            /* 0 = default (64), 2..2047: branches longer than this are cut into
                                        chained segments ("we split branches that are too long") */
     int32_t cluster_max;            /* 0 = default (16), 1..16: largest thread-block cluster a cell may be spread
-                                       over (powers of two are used; 16 is the non-portable cluster size)      */
+                                       over (more than 8 needs the non-portable cluster size)                  */
     int32_t chunk_smem_bytes;       /* 0 = default (113 KiB, two blocks per SM): shared memory one block of a
                                        cluster item aims to stay within; also the size above which a cell is
                                        spread over a cluster instead of taking a whole SM's shared memory      */

@@ -20,6 +20,7 @@ from ._build import LIB as _LIB_PATH, build as build_library
 F64, F32 = 0, 1
 POLICY_DEFAULT, POLICY_FORCE_STREAM, POLICY_NO_GROUPING, POLICY_INPUT_ORDER, POLICY_NO_CLUSTER = 0, 1, 2, 4, 8
 POLICY_SERIAL_CLASSES = 16
+POLICY_POW2_CLUSTERS = 32
 
 STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",
           4: "HINES_ERR_CUDA", 5: "HINES_ERR_UNSUPPORTED"}

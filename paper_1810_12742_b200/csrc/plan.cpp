@@ -85,6 +85,7 @@ struct ItemBuild {
     int64_t padded_steps = 0, useful_steps = 0;
     int64_t leader_extra = 0;                // bytes of the reduced arrays + item metadata (rank 0 only)
     int64_t smem_need = 0;                   // max over the chunks (rank 0 includes leader_extra)
+    int64_t total_bytes = 0;                 // shared memory of the whole item, all chunks together
     int32_t max_lanes = 0;                   // widest segment lane list of a chunk
 };
 
@@ -288,6 +289,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
     out.chunks.assign(nchunks, ItemBuild::Chunk());
     const int64_t per_comp = 3 * P.width, per_seg = 32;   // two lanes per segment
     const int64_t total = out.leader_extra + per_comp * out.n + per_seg * (int64_t)segs.size();
+    out.total_bytes = total;
     size_t si = 0;
     int64_t acc = 0;
     std::vector<SegTmp> mine;
@@ -505,6 +507,7 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     // blocks of at most chunk_smem_bytes leave room for a second resident block per SM
     const int64_t chunk_cap = std::min<int64_t>(P.opt.chunk_smem_bytes, max_smem);
     const int64_t single_cap = no_cluster ? max_smem : chunk_cap;
+    const bool pow2_only = P.opt.policy_flags & HINES_POLICY_POW2_CLUSTERS;
     P.cell_item.assign(nc, -1);
     P.item_level_offsets.assign(1, 0);
     P.item_desc_offsets.assign(1, 0);
@@ -529,12 +532,29 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
                 is_single = alone.ok && alone.smem_need <= single_cap;
             }
             if (!is_single && !no_cluster) {
-                for (int32_t k = 2; k <= P.opt.cluster_max && !placed; k *= 2) {
-                    if (arrays / k > chunk_cap) continue;
-                    build_item(P, c, c + 1, k, cand);
-                    if (!cand.ok) break;
-                    if (cand.smem_need <= chunk_cap || (k * 2 > P.opt.cluster_max && cand.smem_need <= max_smem)) {
-                        flush(c); push(c, c + 1, cand); placed = true;
+                // cluster size: the one whose blocks fill their shared-memory slot best (slots = an SM's
+                // shared memory divided by 1, 2, 3, 4, 6, 8); close calls go to the smaller cluster
+                build_item(P, c, c + 1, 2, cand);
+                if (cand.ok) {
+                    const int64_t total = cand.total_bytes;
+                    std::vector<std::pair<double, int32_t>> opts;                 // (-score, k)
+                    for (int t = 1; t <= 3; ++t) {                                // slots of 1/2, 1/3, 1/4 of an SM
+                        const int64_t slot = class_cap(kClassK[t], max_smem);
+                        if (slot > chunk_cap) continue;
+                        int32_t k = (int32_t)std::max<int64_t>(2, (total + slot - 2048 - 1) / (slot - 2048));
+                        if (pow2_only) while (k & (k - 1)) ++k;
+                        if (k > P.opt.cluster_max) continue;
+                        opts.push_back({-((double)total / (double)(k * slot) - 0.01 * t), k});
+                    }
+                    if (opts.empty() && total / P.opt.cluster_max + 2048 <= max_smem) opts.push_back({0.0, P.opt.cluster_max});
+                    std::sort(opts.begin(), opts.end());
+                    for (size_t o = 0; o < opts.size() && o < 3 && !placed; ++o) {
+                        const int32_t k = opts[o].second;
+                        if (k != 2) build_item(P, c, c + 1, k, cand);
+                        int64_t slot = 0;
+                        for (int t = 0; t < kNumClassK; ++t) if (cand.smem_need <= class_cap(kClassK[t], chunk_cap)) slot = 1;
+                        if (slot || (k == P.opt.cluster_max && cand.smem_need <= max_smem)) { flush(c); push(c, c + 1, cand); placed = true; }
+                        else if (k == 2 && o + 1 < opts.size()) { /* rebuilt below for the next option */ }
                     }
                 }
                 if (!placed && arrays <= max_smem) {                      // last resort before streaming: one big block
@@ -694,7 +714,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.threads_per_block < 0 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~31) ||
+        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~63) ||
         o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }

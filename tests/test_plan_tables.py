@@ -299,7 +299,9 @@ def test_clusters_take_the_cells_too_large_for_one_block():
     info = plan.info
     assert info.n_cluster_cells > 0 and info.n_stream_cells == 0
     cl = plan.table("class_cluster")
-    assert set(cl.tolist()) <= {1, 2, 4, 8} and (np.diff(cl) <= 0).all()
+    assert cl.min() == 1 and cl.max() <= 16 and (np.diff(cl) <= 0).all()
+    m, plan = _plan_cfg(3, 0.004, policy_flags=hb.POLICY_POW2_CLUSTERS)
+    assert set(plan.table("class_cluster").tolist()) <= {1, 2, 4, 8, 16}
     m, plan = _plan_cfg(3, 0.004, policy_flags=hb.POLICY_NO_CLUSTER)
     assert plan.info.n_cluster_cells == 0 and (plan.table("class_cluster") == 1).all()
 
