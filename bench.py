@@ -257,12 +257,16 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
 
 
 def load_traffic(key):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    ncu --set full capture (profiles/traffic.json, written by hand from that capture), or None."""
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per step, from the committed
+    ncu --set full capture (profiles/traffic.csv, see profiles/traffic.md), or None."""
     try:
-        return json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(key)
+        for line in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
+            k, v = line.split(",")
+            if k == key:
+                return int(v)
     except Exception:
-        return None
+        pass
+    return None
 
 
 # ------------------------------------------------------------------------------------------------
