@@ -154,9 +154,12 @@ typedef enum {
     HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
     HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
     HINES_TABLE_CHUNK_SEG_OFFSETS    = 48,  /* int64[nchunks+1] into CHUNK_SEG (in units of descriptors)                */
-    HINES_TABLE_CHUNK_SEG            = 49,  /* int32[4*nseglanes] per segment {a = first compartment (chunk-local),
-                                               m = interior length (separator = a+m), node, node of the separator above
-                                               (-1 = none)}; node = -1 marks a padding lane                             */
+    HINES_TABLE_CHUNK_SEG            = 49,  /* int32[4*nseglanes] two lanes per segment, in groups of 32: lanes 0-15 the
+                                               A halves, lanes 16-31 their B partners (lane ^ 16).  A: {a = first
+                                               compartment (chunk-local), word, node, node of the separator above (-1 =
+                                               none)}; B: {b-1, word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26
+                                               (kind 0 padding, 1 A, 2 B; mt/mb = compartments A / B eliminate; the
+                                               middle node q = a+mt exists iff hasq; separator b = a+mt+mb+hasq)        */
     HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
     HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment
                                                (-1 root), workspace start, child_begin, nchild}                       */
@@ -226,10 +229,11 @@ hines_status_t hines_plan_enable_timing(hines_plan_t* plan, int32_t enable);
 hines_status_t hines_plan_get_timing(hines_plan_t* plan, float* resident_ms, float* stream_ms);
 
 /* Load-imbalance / phase hook (debug; SURVEY.md §8(d) "per-work-item cycle counts").  With phase clocks
- * enabled every shared-memory work item records, per solve, 8 x uint64: %globaltimer (ns) at
+ * enabled every block of the shared-memory kernel records, per solve, 8 x uint64: %globaltimer (ns) at
  * [0] block start, [1] inputs landed in shared memory, [2] segment interiors condensed, [3] backward
- * level sweeps done, [4] forward level sweeps done, [5] interiors expanded, [6] x stored;
- * [7] = (SM id << 32) | unknowns of the item.  Rows are in launch order (HINES_TABLE_ITEM_LAUNCH_ORDER).
+ * level sweep done, [4] forward sweep done (blocks of rank > 0: the wait for rank 0), [5] interiors expanded,
+ * [6] x stored; [7] = (SM id << 32) | unknowns of the block.  Rows are in launch order (classes in order, inside a
+ * class HINES_TABLE_ITEM_LAUNCH_ORDER, the blocks of a cluster item consecutive).
  * hines_plan_get_phase_clocks synchronises the device and copies the rows of the last solve
  * (host_dst may be NULL to query the size).  Errors: INVALID_ARG, CUDA, ALLOC. */
 hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* plan, int32_t enable);
