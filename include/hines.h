@@ -67,7 +67,7 @@ enum {
 typedef struct {
     int32_t struct_size;            /* = sizeof(hines_options_t); lets the struct grow                     */
     int32_t threads_per_block;      /* 0 = default (per size class: one lane per segment of the widest work item,
-                                       128..1024, within the register file); else multiple of 32, <= 1024  */
+                                       64..384, within the register file); else multiple of 32, <= 384      */
     int32_t smem_bytes_per_block;   /* 0 = default (227 KiB: sm_100 opt-in maximum); upper bound for the
                                        shared memory one resident work item may use                       */
     int32_t policy_flags;           /* HINES_POLICY_*                                                      */
@@ -139,18 +139,15 @@ typedef enum {
     HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
     HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] lane index (item-local) where each level's
                                                lane list begins                                                        */
-    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane {nseg | nafter<<16 | tile max nafter<<24 | fast tile<<30,
-                                               rest, cfirst, nlead | tile max nseg<<16}: nseg = 0 marks a padding lane;
-                                               nafter = sibling lanes to the right whose hand-off values this lane
-                                               absorbs by warp shuffle; cfirst, nlead = the hand-off slots (lane ids)
-                                               the branch's last node pulls from                                       */
+    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane (levels in order, siblings contiguous, sibling
+                                               groups by their longest member in segments): {nseg, rest, lane of the first
+                                               child branch, child branches}                                            */
     HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node above it in the reduced tree (a root and
                                                an unused id: itself)                                                    */
     HINES_TABLE_ITEM_NODE_OFFSETS    = 52,  /* int64[nitems+1] into ITEM_PNODE                                          */
     HINES_TABLE_ITEM_ROUNDS          = 53,  /* int32[nitems] pointer-jumping rounds of the forward sweep: 2^rounds >= nodes
                                                on the longest root path of the reduced tree                             */
-    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] node ids (>= lanes; the last one is an all-zero node that
-                                               branches without children pull: their cfirst)                           */
+    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] nodes of the reduced tree (>= lanes)                          */
     HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
     HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
     HINES_TABLE_CHUNK_SEG_OFFSETS    = 48,  /* int64[nchunks+1] into CHUNK_SEG (in units of descriptors)                */
@@ -165,6 +162,16 @@ typedef enum {
                                                (-1 root), workspace start, child_begin, nchild}                       */
     HINES_TABLE_STREAM_CHILD         = 42,  /* int32[2*nstream_children] {global start, workspace start} of each child */
     HINES_TABLE_CLASS_SMEM_BYTES     = 43,  /* int32[n_classes] dynamic shared memory per block of each class          */
+    HINES_TABLE_ITEM_TASK_OFFSETS    = 54,  /* int64[nitems+1] into ITEM_TASK_BLOB                                         */
+    HINES_TABLE_ITEM_TASK_BLOB       = 55,  /* int32[] per item, the backward sweep of the reduced tree: sub-trees of at
+                                               most 32 leaves, one warp per group of sub-trees, lock-step over the height
+                                               above the leaves, a node in the lane of its first child:
+                                               [ntier, tier_begin (ntier+1), pad4 | groups: 36 ints each = lane_begin[33]
+                                               (entry index), steps, byte offset (in the blob) of the per-step shuffle
+                                               counts, pad | entries: 4 ints per node, by lane then step = {node |
+                                               step<<20, lane mask of the other children in the group, first, count in
+                                               the pull list} | pull list: nodes swept in an earlier tier whose hand-off
+                                               slot is added, pad4 | shuffle counts (bytes), pad]                         */
     HINES_TABLE_CLASS_CLUSTER        = 50,  /* int32[n_classes] blocks per item = cluster size (1 = no cluster)        */
     HINES_TABLE_CLASS_THREADS        = 51   /* int32[n_classes] threads per block                                      */
 } hines_table_id_t;

@@ -39,6 +39,7 @@ TABLES = {
     "item_chunk_offsets": (46, np.int64), "chunk_comp_range": (47, np.int64), "chunk_seg_offsets": (48, np.int64),
     "chunk_seg": (49, np.int32), "class_cluster": (50, np.int32), "class_threads": (51, np.int32),
     "item_node_offsets": (52, np.int64), "item_rounds": (53, np.int32),
+    "item_task_offsets": (54, np.int64), "item_task_blob": (55, np.int32),
 }
 
 # every symbol include/hines.h declares

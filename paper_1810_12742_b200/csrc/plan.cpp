@@ -45,7 +45,8 @@ static const int64_t kSmemPerSM = 233472;       // 228 KiB
 static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
 static const int kClassK[] = {1, 2, 3, 4, 6, 8};
 static const int kNumClassK = 6;
-static const int kRegsPerThread = 64;           // __launch_bounds__ of the resident kernel
+static const int kRegsPerThread = 80;           // the resident kernel is built for __launch_bounds__(384, 2): up to 85
+static const int kMaxThreads = 384;
 static const int kMaxClusterClass = 16;
 static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descriptor word 1, bits 24-25)
 static const int32_t kFastTile = 1 << 30;        // descriptor word 0, bit 30
@@ -75,6 +76,11 @@ struct ItemBuild {
     std::vector<int32_t> level_begin;        // nlev+1, in branch lanes
     std::vector<int32_t> desc;               // 4 per branch lane
     std::vector<int32_t> pnode;              // 1 per node: the node above it in the reduced tree; itself for a root / an unused id
+    std::vector<int32_t> perm;               // node id used while the lists were built -> final node id (build_tasks)
+    std::vector<int32_t> task_blob;          // device tables of the backward sweep (build_tasks), multiple of 4 ints
+    int32_t ntier = 0, grp_off = 0, ent_off = 0, pull_off = 0, ngroups = 0;
+    std::vector<int32_t> task_entry, task_group, task_pull, task_tier_begin;   // the same, for the table getters
+    std::vector<unsigned char> task_nsh;
     int32_t rounds = 0;                      // pointer-jumping rounds of the forward sweep: 2^rounds >= nodes on the longest root path
     struct Chunk {
         int32_t begin = 0, n = 0;            // item-local compartment range
@@ -141,6 +147,143 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     }
 }
 
+// Backward sweep over the reduced tree (policy P3).  The tree is cut into sub-trees of at most 32 leaves;
+// a sub-tree is swept by the lanes of ONE warp in lock-step over the node's height (PAPER.md:110-112 with
+// height above the leaves in place of depth below the root): a node sits in the lane of its first child,
+// so the first child's hand-off value is already in that lane's registers and the other children's values
+// come by warp shuffle from their lanes -- no shared memory and no barrier on the dependent
+// chain.  Sub-trees of a tier are packed into groups of at most 32 lanes (one warp each); what lies above
+// the sub-trees forms the next tier, whose leaves pull the hand-off values of the tier below from shared
+// memory after a block barrier.
+//   group   36 ints: lane_begin[33] (into the item's entries), steps, offset of the per-step shuffle
+//           counts (bytes), pad
+//   entry   4 ints per node, by lane then step: node | step << 20, lanes of the other children in the
+//           same group (bit mask, summed in ascending lane order), first / count of the pull list
+//   pull    node ids whose hand-off slot the node adds (children swept in an earlier tier)
+static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
+{
+    const int32_t nn = out.nnode;
+    std::vector<std::vector<int32_t>> kids(nn);
+    std::vector<int32_t> order(nn);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return depth[a] > depth[b]; });   // deepest first
+    for (int32_t v = 0; v < nn; ++v) if (out.pnode[v] != v) kids[out.pnode[v]].push_back(v);                   // ascending id
+    std::vector<int32_t> tier(nn, -1), leaves(nn), group_of(nn, -1), lane_of(nn, -1), step_of(nn, 0);
+    struct Group { std::vector<int32_t> roots; int32_t lanes = 0, steps = 0; std::vector<std::vector<int32_t>> chain; };
+    std::vector<Group> groups;
+    std::vector<int32_t> tier_begin(1, 0);
+    int32_t remaining = nn;
+    for (int32_t t = 0; remaining > 0; ++t) {
+        if (t >= 64) { out.ok = false; break; }
+        // leaves of the remaining forest below every remaining node
+        for (int32_t v : order) {
+            if (tier[v] >= 0) continue;
+            int32_t l = 0;
+            for (int32_t c : kids[v]) if (tier[c] < 0) l += leaves[c];
+            leaves[v] = l ? l : 1;
+        }
+        // sub-tree roots of this tier: at most 32 leaves, parent (if any) has more
+        std::vector<int32_t> roots;
+        for (int32_t v = 0; v < nn; ++v)
+            if (tier[v] < 0 && leaves[v] <= 32 && (out.pnode[v] == v || leaves[out.pnode[v]] > 32)) roots.push_back(v);
+        // pack into groups (first fit in id order), assign lanes and steps
+        const size_t g0 = groups.size();
+        for (int32_t r : roots) {
+            size_t g = g0;
+            while (g < groups.size() && groups[g].lanes + leaves[r] > 32) ++g;
+            if (g == groups.size()) { groups.push_back(Group()); groups[g].chain.resize(32); }
+            Group& G = groups[g];
+            // iterative DFS: a node takes the lane of its first remaining child, a leaf the next free lane
+            std::vector<std::pair<int32_t, int32_t>> stack(1, {r, 0});      // (node, phase)
+            while (!stack.empty()) {
+                auto [v, ph] = stack.back(); stack.pop_back();
+                if (ph == 0) {
+                    stack.push_back({v, 1});
+                    for (auto it = kids[v].rbegin(); it != kids[v].rend(); ++it) if (tier[*it] < 0) stack.push_back({*it, 0});
+                } else {
+                    int32_t first = -1, h = 0;
+                    for (int32_t c : kids[v]) if (tier[c] < 0) { if (first < 0) first = c; h = std::max(h, step_of[c] + 1); }
+                    // in a sub-tree that is a plain chain (one leaf) every node continues its child's run: same
+                    // step, no shuffle, no pull -- the lane walks the chain without waiting for the lock-step of
+                    // the other lanes (in a branching sub-tree runs would make a step as long as its longest run)
+                    if (leaves[r] == 1 && first >= 0) h = step_of[first];
+                    lane_of[v] = first < 0 ? G.lanes++ : lane_of[first];
+                    step_of[v] = h; group_of[v] = (int32_t)g;
+                    G.chain[lane_of[v]].push_back(v);
+                    G.steps = std::max(G.steps, h + 1);
+                }
+            }
+            G.roots.push_back(r);
+        }
+        // commit the tier (after the DFS, which tests tier[] < 0 for "remaining")
+        for (size_t g = g0; g < groups.size(); ++g)
+            for (auto& ch : groups[g].chain) for (int32_t v : ch) { tier[v] = t; --remaining; }
+        tier_begin.push_back((int32_t)groups.size());
+        if (roots.empty()) { out.ok = false; break; }
+    }
+    if (!out.ok) { out.task_blob.assign(4, 0); return; }
+    // tables
+    out.ntier = (int32_t)tier_begin.size() - 1;
+    out.ngroups = (int32_t)groups.size();
+    out.task_tier_begin = tier_begin;
+    out.task_entry.clear(); out.task_group.clear(); out.task_pull.clear(); out.task_nsh.clear();
+    for (Group& G : groups) {
+        std::vector<unsigned char> nsh(G.steps, 0);
+        const size_t gh = out.task_group.size();
+        out.task_group.resize(gh + 36, 0);
+        for (int32_t l = 0; l < 32; ++l) {
+            out.task_group[gh + l] = (int32_t)(out.task_entry.size() / 4);
+            for (int32_t v : G.chain[l]) {
+                if (step_of[v] >= 4096) out.ok = false;
+                uint32_t mask = 0; int32_t first = -1;
+                const int32_t pull0 = (int32_t)out.task_pull.size();
+                for (int32_t c : kids[v]) {
+                    if (tier[c] == tier[v]) { if (first < 0) first = c; else mask |= 1u << lane_of[c]; }
+                    else out.task_pull.push_back(c);
+                }
+                int32_t pc = 0; for (uint32_t m = mask; m; m &= m - 1) ++pc;
+                nsh[step_of[v]] = std::max<unsigned char>(nsh[step_of[v]], (unsigned char)pc);
+                out.task_entry.insert(out.task_entry.end(), {v | (step_of[v] << 20), (int32_t)mask, pull0, (int32_t)out.task_pull.size() - pull0});
+            }
+        }
+        out.task_group[gh + 32] = (int32_t)(out.task_entry.size() / 4);
+        out.task_group[gh + 33] = G.steps;
+        out.task_group[gh + 34] = (int32_t)out.task_nsh.size();      // byte offset, made absolute below
+        out.task_nsh.insert(out.task_nsh.end(), nsh.begin(), nsh.end());
+    }
+    // Renumber the nodes in entry order (group, lane, position in the lane's chain): the records of a lane's
+    // chain are then consecutive in shared memory, so the address of the lane's next record does not wait for
+    // a descriptor.  From here on node id = entry index.
+    out.perm.assign(nn, -1);
+    for (size_t k = 0; k < out.task_entry.size() / 4; ++k) out.perm[out.task_entry[4 * k] & 0xfffff] = (int32_t)k;
+    for (int32_t v = 0; v < nn; ++v) if (out.perm[v] < 0) { out.ok = false; out.task_blob.assign(4, 0); return; }
+    for (size_t k = 0; k < out.task_entry.size() / 4; ++k)
+        out.task_entry[4 * k] = (int32_t)k | (out.task_entry[4 * k] & ~0xfffff);
+    for (int32_t& c : out.task_pull) c = out.perm[c];
+    {
+        std::vector<int32_t> np(nn);
+        for (int32_t v = 0; v < nn; ++v) np[out.perm[v]] = out.perm[out.pnode[v]];
+        out.pnode.swap(np);
+    }
+    // blob: [ntier, tier_begin (ntier+1), pad4 | groups | entries | pull, pad4 | shuffle counts, pad4]
+    std::vector<int32_t>& B = out.task_blob;
+    B.clear();
+    B.push_back(out.ntier);
+    B.insert(B.end(), tier_begin.begin(), tier_begin.end());
+    B.resize(round_up((int64_t)B.size(), 4), 0);
+    out.grp_off = (int32_t)B.size();
+    B.insert(B.end(), out.task_group.begin(), out.task_group.end());
+    out.ent_off = (int32_t)B.size();
+    B.insert(B.end(), out.task_entry.begin(), out.task_entry.end());
+    out.pull_off = (int32_t)B.size();
+    B.insert(B.end(), out.task_pull.begin(), out.task_pull.end());
+    B.resize(round_up((int64_t)B.size(), 4), 0);
+    const int32_t nsh_off = (int32_t)B.size();
+    B.resize(B.size() + round_up((int64_t)out.task_nsh.size(), 16) / 4, 0);
+    if (!out.task_nsh.empty()) std::memcpy(&B[nsh_off], out.task_nsh.data(), out.task_nsh.size());
+    for (int32_t g = 0; g < out.ngroups; ++g) B[out.grp_off + 36 * g + 34] += nsh_off * 4;     // byte offset inside the blob
+}
+
 static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchunks, ItemBuild& out)
 {
     const int32_t smax = P.opt.max_segment;
@@ -201,23 +344,14 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         const int32_t lb = (int32_t)lane_br.size();
         out.level_begin[l] = lb;
         for (const Group& g : groups) {
-            const bool shuffled = g.count <= 32;
-            int32_t pos = (int32_t)lane_br.size() - lb;
-            if (shuffled && (pos % 32) + g.count > 32)
-                while (pos % 32) { lane_br.push_back(-1); ++pos; }
             const int32_t first_lane = (int32_t)lane_br.size();
             for (int32_t i = 0; i < g.count; ++i) {
                 Br& e = br[v[g.first + i]];
                 e.e = (int32_t)lane_br.size();
-                e.nafter = shuffled ? g.count - 1 - i : 0;
                 lane_br.push_back(v[g.first + i]);
             }
             const int32_t par = br[v[g.first]].parent;
-            if (par >= 0) {
-                br[par].cfirst = first_lane;
-                br[par].nlead = shuffled ? 1 : g.count;
-                if (g.count > 0xffff) out.ok = false;
-            }
+            if (par >= 0) { br[par].cfirst = first_lane; br[par].nlead = g.count; }
         }
     }
     out.ndesc = (int32_t)lane_br.size();
@@ -228,43 +362,29 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         Br& b = br[lane_br[e]];
         if (b.nseg > 1) { b.rest = next_id; next_id += b.nseg - 1; }
     }
-    const int32_t dummy = next_id;                     // an all-zero node: what a branch without children pulls
-    out.nnode = next_id + 1;
+    out.nnode = next_id;
+    if (out.nnode >= (1 << 20)) out.ok = false;
     auto last_node = [&](const Br& b) { return b.nseg > 1 ? b.rest + b.nseg - 2 : b.e; };
+    // per branch lane: {segments, id of the second node, lane of the first child branch, child branches}
     out.desc.assign(4 * (size_t)out.ndesc, 0);
     out.pnode.resize(out.nnode);
     std::iota(out.pnode.begin(), out.pnode.end(), 0);
     std::vector<int32_t> depth(out.nnode, 1);          // nodes on the path from the root, inclusive
     int32_t height = 1;
-    for (int32_t l = 0; l < out.nlev; ++l) {
-        const int32_t lb = out.level_begin[l], le = out.level_begin[l + 1];
-        for (int32_t t = lb; t < le; t += 32) {
-            int32_t wmax = 0, smx = 0, lmx = 0;
-            for (int32_t e = t; e < std::min(le, t + 32); ++e)
-                if (lane_br[e] >= 0) {
-                    const Br& b = br[lane_br[e]];
-                    wmax = std::max(wmax, b.nafter); smx = std::max(smx, b.nseg); lmx = std::max(lmx, b.nlead);
-                }
-            // fast tile: one node per branch, sibling groups of at most two, one hand-off slot to pull
-            const int32_t fast = (smx <= 1 && wmax <= 1 && lmx <= 1) ? kFastTile : 0;
-            for (int32_t e = t; e < std::min(le, t + 32); ++e) {
-                out.desc[4 * e + 2] = dummy;
-                if (lane_br[e] < 0) { out.desc[4 * e + 3] = smx << 16; out.desc[4 * e] = (wmax << 24) | fast; continue; }
-                const Br& b = br[lane_br[e]];
-                out.desc[4 * e + 0] = b.nseg | (b.nafter << 16) | (wmax << 24) | fast;
-                out.desc[4 * e + 1] = b.rest;
-                if (b.nlead) out.desc[4 * e + 2] = b.cfirst;
-                out.desc[4 * e + 3] = b.nlead | (smx << 16);
-                if (b.parent >= 0) { out.pnode[e] = last_node(br[b.parent]); depth[e] = depth[out.pnode[e]] + 1; }
-                for (int32_t k = 1; k < b.nseg; ++k) {          // a root keeps itself as parent: its f is 0
-                    out.pnode[b.rest + k - 1] = k == 1 ? e : b.rest + k - 2;
-                    depth[b.rest + k - 1] = depth[e] + k;
-                }
-                height = std::max(height, depth[e] + b.nseg - 1);
-            }
+    for (int32_t e = 0; e < out.ndesc; ++e) {           // lanes are in level order: parents come first
+        const Br& b = br[lane_br[e]];
+        out.desc[4 * e + 0] = b.nseg; out.desc[4 * e + 1] = b.rest;
+        out.desc[4 * e + 2] = b.cfirst; out.desc[4 * e + 3] = b.nlead;
+        if (b.parent >= 0) { out.pnode[e] = last_node(br[b.parent]); depth[e] = depth[out.pnode[e]] + 1; }
+        for (int32_t k = 1; k < b.nseg; ++k) {          // a root keeps itself as parent: its f is 0
+            out.pnode[b.rest + k - 1] = k == 1 ? e : b.rest + k - 2;
+            depth[b.rest + k - 1] = depth[e] + k;
         }
+        height = std::max(height, depth[e] + b.nseg - 1);
     }
     while ((1 << out.rounds) < height) ++out.rounds;
+    build_tasks(out, depth);
+    if (!out.ok) { out.perm.resize(out.nnode); std::iota(out.perm.begin(), out.perm.end(), 0); }
     // ---- P4: segments, in compartment order ------------------------------------------------------
     // Branch cut from its end into nseg segments of sj compartments (the paper's branch splitting,
     // PAPER.md:151, with a fixed bound); node ids from the top of the branch: e, rest, rest+1, ...
@@ -279,12 +399,12 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             const int32_t sa = std::max(b.start, sb - b.sj + 1);
             const int32_t node = k == 0 ? b.e : b.rest + k - 1;
             const int32_t tnode = k > 0 ? (k == 1 ? b.e : b.rest + k - 2) : (b.parent >= 0 ? last_node(br[b.parent]) : -1);
-            segs.push_back({sa, sb - sa, node, tnode});
+            segs.push_back({sa, sb - sa, out.perm[node], tnode < 0 ? -1 : out.perm[tnode]});
             out.useful_steps += sb - sa;
         }
     }
     // ---- chunks: consecutive segments, balanced in shared-memory bytes -----------------------------
-    const int64_t meta_item = round_up(out.nlev + 1, 4) + 4 * (int64_t)out.ndesc + round_up(out.nnode, 4);
+    const int64_t meta_item = (int64_t)out.task_blob.size() + round_up(out.nnode, 4);
     out.leader_extra = 6 * round_up(out.nnode, E) * P.width + 4 * meta_item;
     out.chunks.assign(nchunks, ItemBuild::Chunk());
     const int64_t per_comp = 3 * P.width, per_seg = 32;   // two lanes per segment
@@ -450,18 +570,18 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_node_offsets.push_back((int64_t)P.item_pnode.size());
     P.item_rounds.push_back(ib.rounds);
     P.item_nnode.push_back(ib.nnode);
-    // device blob of the item: [level_begin | pad4 | branch desc | pnode | pad4]
+    P.item_task_blob.insert(P.item_task_blob.end(), ib.task_blob.begin(), ib.task_blob.end());
+    P.item_task_offsets.push_back((int64_t)P.item_task_blob.size());
+    // device blob of the item: [task blob | pnode | pad4]
     hines::ItemHeader h{};
     h.meta_off = (int64_t)P.item_meta.size();
-    P.item_meta.insert(P.item_meta.end(), ib.level_begin.begin(), ib.level_begin.end());
-    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
-    h.bdesc_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    P.item_meta.insert(P.item_meta.end(), ib.desc.begin(), ib.desc.end());
+    P.item_meta.insert(P.item_meta.end(), ib.task_blob.begin(), ib.task_blob.end());
+    h.grp_off = ib.grp_off; h.ent_off = ib.ent_off; h.pull_off = ib.pull_off; h.ntier = ib.ntier;
     h.pnode_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
     P.item_meta.insert(P.item_meta.end(), ib.pnode.begin(), ib.pnode.end());
     P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
     h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    h.nlev = ib.nlev; h.ndesc = ib.ndesc; h.nnode = ib.nnode; h.rounds = ib.rounds;
+    h.nnode = ib.nnode; h.rounds = ib.rounds;
     h.first_chunk = (int32_t)P.chunk_headers.size();
     h.nchunks = ib.nchunks;
     h.n = (int32_t)ib.n;
@@ -512,6 +632,7 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     P.item_level_offsets.assign(1, 0);
     P.item_desc_offsets.assign(1, 0);
     P.item_node_offsets.assign(1, 0);
+    P.item_task_offsets.assign(1, 0);
     P.item_chunk_offsets.assign(1, 0);
     P.chunk_seg_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
@@ -608,9 +729,9 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
         P.class_cluster.push_back(q >= kNumClassK ? q / kNumClassK : 1);
         const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
         int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
-        tmax = std::max<int64_t>(128, std::min<int64_t>(1024, tmax));
+        tmax = std::max<int64_t>(64, std::min<int64_t>(kMaxThreads, tmax));
         int64_t t = P.opt.threads_per_block ? P.opt.threads_per_block : round_up(std::max(lanes_max[q], 1), 32);
-        t = std::max<int64_t>(P.opt.threads_per_block ? 32 : 128, std::min(t, tmax));
+        t = std::max<int64_t>(P.opt.threads_per_block ? 32 : std::min<int64_t>(128, tmax), std::min(t, tmax));
         P.class_threads.push_back((int32_t)t);
     }
     for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[item_q[i]];
@@ -711,7 +832,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.max_segment == 0) o.max_segment = 64;
     if (o.cluster_max == 0) o.cluster_max = 16;
     if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 113 * 1024;
-    if (o.threads_per_block < 0 || o.threads_per_block > 1024 || o.threads_per_block % 32 ||
+    if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
         o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~63) ||
@@ -799,6 +920,8 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_PNODE, P->item_pnode)
         TBL(HINES_TABLE_ITEM_NODE_OFFSETS, P->item_node_offsets)
         TBL(HINES_TABLE_ITEM_ROUNDS, P->item_rounds)
+        TBL(HINES_TABLE_ITEM_TASK_OFFSETS, P->item_task_offsets)
+        TBL(HINES_TABLE_ITEM_TASK_BLOB, P->item_task_blob)
         TBL(HINES_TABLE_ITEM_NNODE, P->item_nnode)
         TBL(HINES_TABLE_ITEM_CHUNK_OFFSETS, P->item_chunk_offsets)
         TBL(HINES_TABLE_CHUNK_COMP_RANGE, P->chunk_comp_range)

@@ -12,19 +12,21 @@ namespace hines {
 // (nchunks == 1; cells are packed into a block in the order given), or ONE cell too
 // large for that, spread over the shared memories of a thread-block cluster (nchunks == cluster
 // size; chunk r lives in the block of cluster rank r, the level-synchronous part runs in rank 0).
-struct ItemHeader {          // 48 bytes
+struct ItemHeader {          // 56 bytes
     int64_t meta_off;        // offset (int32 units, multiple of 4) of the item's metadata blob:
-                             //   [level_begin (nlev+1) | pad4 | branch desc 4*ndesc | pnode nnode | pad4]
+                             //   [task blob (plan.cpp build_tasks) | pnode nnode | pad4]
     int32_t meta_len;        // int32 count (multiple of 4)
-    int32_t bdesc_off;       // offset of the branch descriptors inside the blob (multiple of 4)
-    int32_t pnode_off;       // offset of the parent-node list inside the blob
-    int32_t nlev;            // levels of the deepest cell in the item
-    int32_t ndesc;           // branch lanes (incl. padding lanes) = ids of the branches' top nodes
-    int32_t nnode;           // nodes of the reduced tree (separators incl. the unused ids of padding lanes)
+    int32_t grp_off;         // offsets inside the blob: group headers (36 ints each),
+    int32_t ent_off;         //   entries (4 ints per node),
+    int32_t pull_off;        //   pull list,
+    int32_t pnode_off;       //   parent-node list
+    int32_t ntier;           // tiers of the backward sweep (block barrier between tiers)
+    int32_t nnode;           // nodes of the reduced tree
     int32_t first_chunk;     // index of the item's first chunk
     int32_t nchunks;
     int32_t n;               // unknowns of the item
     int32_t rounds;          // pointer-jumping rounds of the forward sweep over the reduced tree
+    int32_t pad_;
 };
 
 // One chunk = the contiguous compartment range one block stages into its shared memory.
@@ -67,8 +69,8 @@ struct hines_plan {
         branch_level, cell_nlevels, level_count, level_list, child_ids;
     // policy tables
     std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc, item_pnode,
-        item_nnode, item_rounds, chunk_seg;
-    std::vector<int64_t> item_cell_range, item_desc_offsets, item_node_offsets, item_level_offsets, item_chunk_offsets,
+        item_nnode, item_rounds, item_task_blob, chunk_seg;
+    std::vector<int64_t> item_cell_range, item_desc_offsets, item_node_offsets, item_task_offsets, item_level_offsets, item_chunk_offsets,
         chunk_comp_range, chunk_seg_offsets;
     std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
     std::vector<int32_t> class_cluster;                // per class: blocks per item (cluster size), 1 = no cluster

@@ -32,13 +32,6 @@
 
 namespace hines {
 
-#ifdef HINES_P2_TRACE
-__device__ long long g_trace[1024];
-#define TR(i) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (i) < 1024) g_trace[(i)] = clock64(); } while (0)
-#else
-#define TR(i) do {} while (0)
-#endif
-
 struct BlockRec { ItemHeader it; ChunkHeader ch; };   // 80 bytes
 
 struct DeviceTables {
@@ -158,6 +151,22 @@ template <> __device__ __forceinline__ float fnma<float>(float a, float b, float
 template <typename T> struct Vec2;
 template <> struct Vec2<double> { typedef double2 type; };
 template <> struct Vec2<float> { typedef float2 type; };
+// shared-memory accesses by 32-bit shared address (no generic-to-shared conversion on the dependent chain)
+template <typename T> __device__ __forceinline__ typename Vec2<T>::type lds2(uint32_t a);
+template <> __device__ __forceinline__ double2 lds2<double>(uint32_t a)
+{ double2 v; asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a) : "memory"); return v; }
+template <> __device__ __forceinline__ float2 lds2<float>(uint32_t a)
+{ float2 v; asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(a) : "memory"); return v; }
+template <typename T> __device__ __forceinline__ T lds1(uint32_t a);
+template <> __device__ __forceinline__ double lds1<double>(uint32_t a)
+{ double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory"); return v; }
+template <> __device__ __forceinline__ float lds1<float>(uint32_t a)
+{ float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; }
+template <typename T> __device__ __forceinline__ void sts2(uint32_t a, typename Vec2<T>::type v);
+template <> __device__ __forceinline__ void sts2<double>(uint32_t a, double2 v)
+{ asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory"); }
+template <> __device__ __forceinline__ void sts2<float>(uint32_t a, float2 v)
+{ asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(a), "f"(v.x), "f"(v.y) : "memory"); }
 template <typename T> __device__ __forceinline__ T fmad(T a, T b, T c);   // c + a*b
 template <> __device__ __forceinline__ double fmad<double>(double a, double b, double c) { return fma(a, b, c); }
 template <> __device__ __forceinline__ float fmad<float>(float a, float b, float c) { return fmaf(a, b, c); }
@@ -190,7 +199,7 @@ template <> __device__ __forceinline__ float fmad<float>(float a, float b, float
 // SPD and strictly diagonally dominant, so any order is stable without pivoting).
 // ------------------------------------------------------------------------------------------------
 template <typename T, bool CL>
-__global__ void __launch_bounds__(1024, 1)
+__global__ void __launch_bounds__(384, 2)
 hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restrict__ meta_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
                       int64_t n_total, unsigned long long* prof)
@@ -245,7 +254,6 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         }
         if (mbytes) tma_load_1d(imeta, meta_g + it.meta_off, mbytes, bar);
     }
-    if (rank == 0 && tid < 6) nd[6 * (it.nnode - 1) + tid] = T(0);      // the zero node (what a childless branch pulls)
     // remainder of the very last chunk (fewer than E elements), plain loads
     for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
     // reduced arrays as seen from this block
@@ -316,104 +324,94 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
     HINES_STAMP(2);
 
     if (rank == 0) {
-        const int32_t* lvl = imeta;
-        const int4* bdesc = reinterpret_cast<const int4*>(imeta + it.bdesc_off);
         const int32_t* pnode = imeta + it.pnode_off;
-        // ---- P2 backward: reduced tree, deepest level first ----
-        // One lane per branch.  After a level's barrier the only new data a lane needs is the hand-off
-        // slot of its children; its descriptor is fetched one level ahead.  The working warp's
-        // instruction count per level is what bounds this phase, hence the lean "fast tile" path.
         typedef typename Vec2<T>::type V2;
-        auto backward_general = [&](int e, int4 ds, int x0, int w0) {
-            const int nseg = ds.x & 0xffff, nafter = (ds.x >> 16) & 0xff;
-            const int wmax = (x0 >> 24) & 0x1f, nlead = ds.w & 0xffff, nmax = (w0 >> 16) & 0xffff;
-            const T* cq = nd + 6 * ds.z;                         // hand-off slots of the children (the zero node if none)
-            T* q = nd + 6 * (nseg > 1 ? ds.y + nseg - 2 : e);    // last node of the branch
-            T D = T(1), B = T(0), U = T(0), dd = T(0), db = T(0);
-            if (nseg > 0) {
-                D = q[0]; B = q[1]; U = q[2]; dd = q[4]; db = q[5];
-                D -= cq[4]; B -= cq[5];                          // pull; the zero node if no children
-                for (int c = 1; c < nlead; ++c) { D -= cq[6 * c + 4]; B -= cq[6 * c + 5]; }
-                const T r = rcp<T>(D);
-                const T f = U * r;
-                q[0] = -f; q[1] = B * r;
-                dd = fmad<T>(f, U, dd);                          // f U + parked contribution of the segment
-                db = fmad<T>(f, B, db);
-            }
-            for (int k = 1; k < nmax; ++k) {                     // branches of several segments: walk up in lock-step
-                if (k < nseg) {
-                    q = (k + 1 == nseg) ? nd + 6 * e : q - 6;
-                    D = q[0] - dd; B = q[1] - db; U = q[2];
-                    const T r = rcp<T>(D);
-                    const T f = U * r;
-                    q[0] = -f; q[1] = B * r;
-                    dd = fmad<T>(f, U, q[4]);
-                    db = fmad<T>(f, B, q[5]);
-                }
-            }
-            // hand-off at the branch point: siblings sit in one tile, the group's first lane sums
-            // their values by shuffle (fixed order) and leaves the sum in its slot
-            if (wmax > 0) {
-                const T dd0 = dd, db0 = db;
-                for (int k = 1; k <= wmax; ++k) {
-                    const T vd = __shfl_down_sync(FULL, dd0, k);
-                    const T vb = __shfl_down_sync(FULL, db0, k);
-                    if (k <= nafter) { dd += vd; db += vb; }
-                }
-            }
-            if (nseg > 0) { T* t = nd + 6 * e; t[4] = dd; t[5] = db; }
-        };
+        // ---- P2 backward on the reduced tree --------------------------------------
+        // Sub-trees of at most 32 leaves, one warp per group of sub-trees, lock-step over the height above
+        // the leaves.  A node sits in the lane of its first child: that child's hand-off value (f U + parked,
+        // f B + parked) is already in the lane's registers, the other children's values come by warp shuffle
+        // from their lanes, in ascending lane order.  No shared memory and no barrier on the dependent chain
+        // inside a tier; between tiers a block barrier, and the leaves of the upper tier pull the hand-off
+        // slots of the tier below.
         {
-            const int wbase = tid & ~31;
-            const int dummy = it.nnode - 1;
-            int eb = lvl[it.nlev - 1], ee_ = lvl[it.nlev];
-            int nb = it.nlev > 1 ? lvl[it.nlev - 2] : 0;
-            int4 ds = make_int4(0, 0, dummy, 0);
-            if (eb + tid < ee_) ds = bdesc[eb + tid];
-            for (int lev = it.nlev - 1; lev >= 0; --lev) {
-                const int e = eb + tid;
-                TR(8 * lev + 0);
-                if (eb + wbase < ee_) {                          // this warp has lanes on the level
-                    const int x0 = __shfl_sync(FULL, ds.x, 0), w0 = __shfl_sync(FULL, ds.w, 0);   // tile-uniform fields
-                    if (x0 & (1 << 30)) {
-                        // fast tile: one node per branch, at most two siblings, one slot to pull
-                        V2* q = reinterpret_cast<V2*>(nd + 6 * e);
-                        const bool act = (ds.x & 0xffff) != 0;
-                        T dd = T(0), db = T(0);
-                        if (act) {
-                            const V2 c2 = *reinterpret_cast<const V2*>(nd + 6 * ds.z + 4);
-                            const V2 a0 = q[0], a2 = q[2];
-                            const T U = nd[6 * e + 2];
-                            const T D = a0.x - c2.x, B = a0.y - c2.y;
-                            TR(8 * lev + 1);
+            const int4* ents = reinterpret_cast<const int4*>(imeta + it.ent_off);
+            const int32_t* pull = imeta + it.pull_off;
+            const int warp = tid >> 5, nwarps = nthreads >> 5;
+            const uint32_t nd_sa = smem_u32(nd);
+            for (int tier = 0; tier < it.ntier; ++tier) {
+                const int gb = imeta[1 + tier], ge = imeta[2 + tier];
+                for (int g = gb + warp; g < ge; g += nwarps) {
+                    const int32_t* gh = imeta + it.grp_off + 36 * g;
+                    int pos = gh[lane];
+                    const int end = gh[lane + 1], nsteps = gh[33];
+                    const unsigned char* nshb = reinterpret_cast<const unsigned char*>(imeta) + gh[34];
+                    T outd = T(0), outb = T(0);
+                    // Node ids are entry indices, so the records of the lane's chain are consecutive: the next
+                    // record's address is known without its descriptor (one shared-memory hop, not two).
+                    constexpr uint32_t RS = 6u * (uint32_t)sizeof(T), W = (uint32_t)sizeof(T);
+                    int4 en = make_int4(0, 0, 0, 0);
+                    uint32_t qa = nd_sa + (uint32_t)pos * RS;
+                    V2 a0, a2; T U = T(0);
+                    a0.x = T(1); a0.y = T(0); a2.x = T(0); a2.y = T(0);
+                    int estep = 0x7fffffff;                         // step of the lane's next node
+                    if (pos < end) {
+                        en = ents[pos];
+                        a0 = lds2<T>(qa); U = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
+                        estep = en.x >> 20;
+                    }
+                    int nsh = nshb[0];
+#pragma unroll 1
+                    for (int h = 0; h < nsteps; ++h) {
+                        const int nsh_next = h + 1 < nsteps ? nshb[h + 1] : 0;
+                        const bool act = estep == h;
+                        T sd_ = outd, sb_ = outb;                       // the first child (own lane), or 0 at a leaf
+                        if (nsh) {                                      // the other children, by shuffle
+                            unsigned m = act ? (unsigned)en.y : 0u;
+#pragma unroll 1
+                            for (int t = 0; t < nsh; ++t) {
+                                const int src = m ? __ffs(m) - 1 : lane;
+                                const T vd = __shfl_sync(FULL, outd, src), vb = __shfl_sync(FULL, outb, src);
+                                if (m) { sd_ += vd; sb_ += vb; m &= m - 1; }
+                            }
+                        }
+                        // a run = a node and the single-child nodes above it, all on this step (no shuffle, no pull
+                        // after the first): the lane walks it node by node
+                        while (estep == h) {
+                            if (en.w) {                                 // children swept in an earlier tier
+#pragma unroll 1
+                                for (int k = 0; k < en.w; ++k) {
+                                    const V2 c2 = lds2<T>(nd_sa + (uint32_t)pull[en.z + k] * RS + 4u * W);
+                                    sd_ += c2.x; sb_ += c2.y;
+                                }
+                            }
+                            const T D = a0.x - sd_, B = a0.y - sb_;
+                            ++pos;
+                            const bool more = pos < end;
+                            if (more) {                                 // next node: what its step needs first
+                                en = ents[pos];
+                                a0 = lds2<T>(qa + RS);
+                                estep = en.x >> 20;
+                            } else {
+                                estep = 0x7fffffff;
+                            }
                             const T r = rcp<T>(D);
                             const T f = U * r;
                             V2 o; o.x = -f; o.y = B * r;
-                            q[0] = o;
-                            dd = fmad<T>(f, U, a2.x); db = fmad<T>(f, B, a2.y);
+                            sts2<T>(qa, o);
+                            outd = fmad<T>(f, U, a2.x); outb = fmad<T>(f, B, a2.y);
+                            if (more) {                                 // ... and what it needs after its reciprocal
+                                qa += RS;
+                                U = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
+                            } else {                                    // end of the lane's chain: leave the hand-off in the slot
+                                V2 s2; s2.x = outd; s2.y = outb;
+                                sts2<T>(qa + 4u * W, s2);
+                            }
+                            sd_ = outd; sb_ = outb;                     // the next node of the run has this one as its only child
                         }
-                        TR(8 * lev + 2);
-                        const T vd = __shfl_down_sync(FULL, dd, 1), vb = __shfl_down_sync(FULL, db, 1);
-                        if (ds.x & 0x10000) { dd += vd; db += vb; }
-                        if (act) { V2 o; o.x = dd; o.y = db; q[2] = o; }
-                        TR(8 * lev + 3);
-                    } else {
-                        backward_general(e, ds, x0, w0);
+                        nsh = nsh_next;
                     }
                 }
-                for (int base = eb + wbase + nthreads; base < ee_; base += nthreads) {   // levels wider than the block
-                    int4 d2 = make_int4(0, 0, dummy, 0);
-                    if (base + lane < ee_) d2 = bdesc[base + lane];
-                    backward_general(base + lane, d2, __shfl_sync(FULL, d2.x, 0), __shfl_sync(FULL, d2.w, 0));
-                }
-                // next level's descriptor, in flight across the barrier
-                ee_ = eb; eb = nb;
-                nb = lev > 1 ? lvl[lev - 2] : 0;
-                ds = make_int4(0, 0, dummy, 0);
-                if (lev > 0 && eb + tid < ee_) ds = bdesc[eb + tid];
-                TR(8 * lev + 4);
                 __syncthreads();
-                TR(8 * lev + 5);
             }
         }
         HINES_STAMP(3);
@@ -743,10 +741,6 @@ static hines_status_t check_ptrs(const hines_plan* P, const void* d, const void*
 using namespace hines;
 
 extern "C" {
-
-#ifdef HINES_P2_TRACE
-int hines_debug_read_trace(long long* dst) { return (int)cudaMemcpyFromSymbol(dst, hines::g_trace, sizeof(long long) * 1024); }
-#endif
 
 hines_status_t hines_plan_upload(hines_plan_t* P)
 {

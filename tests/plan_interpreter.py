@@ -1,7 +1,8 @@
 """Test-side interpreter of the plan's policy tables (pure Python, fp64).
 
 Executes exactly what the tables tell the resident kernel to do -- condense every segment (P1),
-level-synchronous sweeps over the reduced tree with the pull hand-off (P2), expand (P3) -- one
+the backward sweep over the reduced tree (tiers of warp groups in lock-step over the height, shuffle and
+pull hand-off) and the pointer-jumping forward sweep (P2), expand (P3) -- one
 "lane" at a time, so that a wrong table (a missing segment, a wrong node id, a child group the parent
 does not pull) shows up on the CPU box as a wrong solution, before any GPU run.  It shares no code
 with the library: it only reads tables through hines_plan_get_table.
@@ -28,6 +29,30 @@ def pairs(sg):
             yield int(A[0]), mt, mb, hasq, int(A[2]), int(A[3])
 
 
+def parse_tasks(blob):
+    """Per tier: (tier, [(lane_begin[33], steps, shuffle counts per step)], entries, pull list, raw bytes)."""
+    ntier = int(blob[0])
+    tb = blob[1:2 + ntier]
+    grp_off = -(-(2 + ntier) // 4) * 4
+    ngroups = int(tb[-1])
+    ent_off = grp_off + 36 * ngroups
+    nent = int(blob[grp_off + 36 * (ngroups - 1) + 32]) if ngroups else 0
+    ents = blob[ent_off:ent_off + 4 * nent].reshape(-1, 4)
+    pull_off = ent_off + 4 * nent
+    npull = int((ents[:, 3]).sum()) if nent else 0
+    pull = blob[pull_off:pull_off + npull]
+    raw = blob.view(np.uint8)
+    out = []
+    for t in range(ntier):
+        groups = []
+        for g in range(int(tb[t]), int(tb[t + 1])):
+            gh = blob[grp_off + 36 * g:grp_off + 36 * g + 36]
+            nsteps, boff = int(gh[33]), int(gh[34])
+            groups.append((gh[:33], nsteps, raw[boff:boff + nsteps]))
+        out.append((t, groups, ents, pull, raw))
+    return out
+
+
 def solve_with_tables(plan, m, d, u, b):
     """x for every cell that sits in an on-chip work item (NaN elsewhere)."""
     x = np.full(m.n, np.nan)
@@ -40,6 +65,8 @@ def solve_with_tables(plan, m, d, u, b):
     nnode = plan.table("item_nnode")
     node_off = plan.table("item_node_offsets")
     rounds = plan.table("item_rounds")
+    task_off = plan.table("item_task_offsets")
+    task_blob = plan.table("item_task_blob")
     ch_off = plan.table("item_chunk_offsets")
     ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
     seg_off = plan.table("chunk_seg_offsets")
@@ -97,42 +124,51 @@ def solve_with_tables(plan, m, d, u, b):
                 assert np.isnan(rD[node]), "node written twice"
                 rD[node], rB[node], rU[node], pd[node], pb[node] = rec
             work.append((g0, g1, sd, su, sb, sg))
-        # P2
-        dsc = desc[desc_off[it]:desc_off[it + 1]]
+        # P2 backward: tiers of warp groups, lock-step over the height, a node in the lane of its first child
         pn = pnode_all[node_off[it]:node_off[it + 1]]
         assert len(pn) == NN
-        lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
-        nlev = len(lb) - 1
-        for lev in range(nlev - 1, -1, -1):
-            dd = np.zeros(lb[lev + 1] - lb[lev]); db = dd.copy()
-            for e in range(lb[lev], lb[lev + 1]):
-                w0, rest, cfirst, w3 = (int(v) for v in dsc[e])
-                nseg, nlead = w0 & 0xffff, w3 & 0xffff
-                if nseg == 0:
-                    continue
-                node = rest + nseg - 2 if nseg > 1 else e
-                D, B = rD[node], rB[node]
-                for c in range(nlead):
-                    D -= pd[cfirst + c]; B -= pb[cfirst + c]
-                for k in range(nseg):
-                    r = 1.0 / D
-                    U = rU[node]
-                    f = U * r
-                    rD[node], rB[node] = f, B * r
-                    dde, dbe = f * U + pd[node], f * B + pb[node]
-                    if k + 1 < nseg:
-                        node = e if k + 2 == nseg else node - 1
-                        D, B = rD[node] - dde, rB[node] - dbe
-                dd[e - lb[lev]], db[e - lb[lev]] = dde, dbe
-            # shuffle stage: lane e absorbs the nafter lanes to its right (same 32-lane tile)
-            for e in range(lb[lev], lb[lev + 1]):
-                w0 = int(dsc[e, 0])
-                nseg, nafter = w0 & 0xffff, (w0 >> 16) & 0xff
-                if nseg == 0:
-                    continue
-                j = e - lb[lev]
-                assert j % 32 + nafter < 32, "sibling group leaves its tile"
-                pd[e] = dd[j] + sum(dd[j + 1:j + 1 + nafter]); pb[e] = db[j] + sum(db[j + 1:j + 1 + nafter])
+        blob = task_blob[task_off[it]:task_off[it + 1]]
+        done = np.zeros(NN, bool)
+        for tier, groups, ents, pull, nshb in parse_tasks(blob):
+            for gh, nsteps, nsh in groups:
+                outd = np.zeros(32); outb = np.zeros(32)
+                pos = [int(gh[l]) for l in range(32)]
+                for h in range(nsteps):
+                    newd, newb = outd.copy(), outb.copy()
+                    for lane in range(32):
+                        first = True
+                        while pos[lane] < gh[lane + 1]:
+                            w0, mask, p0, pcount = (int(v) for v in ents[pos[lane]])
+                            node, step = w0 & 0xfffff, (w0 >> 20) & 0xfff
+                            if step != h:
+                                assert step > h
+                                break
+                            if first:
+                                sd_, sb_ = outd[lane], outb[lane]
+                                srcs = [l2 for l2 in range(32) if (mask >> l2) & 1]
+                                assert len(srcs) <= nsh[h] and lane not in srcs
+                                for l2 in srcs:
+                                    sd_ += outd[l2]; sb_ += outb[l2]
+                            else:                           # continuation of a run: only child = the node just computed
+                                assert mask == 0
+                                sd_, sb_ = newd[lane], newb[lane]
+                            for c in pull[p0:p0 + pcount]:
+                                assert done[c]
+                                sd_ += pd[c]; sb_ += pb[c]
+                            D, B = rD[node] - sd_, rB[node] - sb_
+                            r = 1.0 / D
+                            f = rU[node] * r
+                            rD[node], rB[node] = f, B * r
+                            newd[lane], newb[lane] = f * rU[node] + pd[node], f * B + pb[node]
+                            assert not done[node]
+                            done[node] = True
+                            pos[lane] += 1
+                            first = False
+                            if pos[lane] >= gh[lane + 1]:
+                                pd[node], pb[node] = newd[lane], newb[lane]       # hand-off slot
+                    outd, outb = newd, newb
+                assert all(pos[l] == gh[l + 1] for l in range(32))
+        assert done.all()
         # forward sweep by pointer jumping: x_v = c_v + g_v x_p(v), g = -f (a root: g = 0, p = itself)
         real = ~np.isnan(rD)
         g = np.where(real, -rD, 0.0); c = np.where(real, rB, 0.0); par = pn.astype(np.int64).copy()

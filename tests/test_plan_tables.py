@@ -13,7 +13,7 @@ import morphgen as mg
 import oracle
 import paper_1810_12742_b200 as hb
 from helpers import random_parent
-from plan_interpreter import pairs
+from plan_interpreter import pairs, parse_tasks
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -163,7 +163,8 @@ def _check_policy(m, plan, max_segment=64):
                 covered[base + a:base + a + mm + 1] += 1
                 useful += int(mm)
             L = -(-(cr[r, 0] % E + cr[r, 1] - cr[r, 0]) // E) * E
-            meta = -(-(nlev + 1) // 4) * 4 + 4 * len(dsc) + -(-nnode[it] // 4) * 4
+            tb = plan.table("item_task_offsets")
+            meta = int(tb[it + 1] - tb[it]) + -(-nnode[it] // 4) * 4
             need = 16 + 3 * L * w + 16 * len(sg) + (6 * (-(-nnode[it] // E) * E) * w + 4 * meta if r == 0 else 0)
             assert need <= cls_smem[cls[it]] <= 232448
         assert (covered == 1).all()
@@ -175,52 +176,61 @@ def _check_policy(m, plan, max_segment=64):
             for j in range(T.cell_branch_offsets[c], T.cell_branch_offsets[c + 1]):
                 pc = T.branch_parent_comp[j]
                 want[int(T.branch_start[j] + sh)] = (int(T.branch_len[j]), -1 if pc < 0 else int(pc + sh), int(T.branch_level[j]))
-        top_node_pos = {node: a for node, (a, mm, t) in seg_of_node.items()}
+        seg_at = {a: (mm, node, t) for node, (a, mm, t) in seg_of_node.items()}       # by first compartment
         lanes_seen = set()
-        for l in range(nlev):
-            tile_l = dsc[lb[l]:lb[l + 1]]
-            for e in range(lb[l], lb[l + 1]):
-                w0, rest, cfirst, w3 = (int(v) for v in dsc[e])
-                nseg, nafter, wmax, fast = w0 & 0xffff, (w0 >> 16) & 0xff, (w0 >> 24) & 0x1f, (w0 >> 30) & 1
-                nlead, smx = w3 & 0xffff, (w3 >> 16) & 0xffff
-                t0 = lb[l] + (e - lb[l]) // 32 * 32
-                tl = dsc[t0:min(t0 + 32, lb[l + 1])]
-                assert wmax == ((tl[:, 0] >> 16) & 0xff).max() and smx == (tl[:, 0] & 0xffff).max()
-                assert fast == int(smx <= 1 and wmax <= 1 and (tl[:, 3] & 0xffff).max() <= 1)
-                if nseg == 0:
-                    assert pn[e] == e and nafter == 0
-                    continue
-                start = top_node_pos[e]                      # the top segment starts at the branch start
-                ln, pc, lw = want[start]
-                assert lw == l and start not in lanes_seen
-                lanes_seen.add(start)
-                assert nseg == -(-ln // max_segment)
-                sj = -(-ln // nseg)
-                end = start + ln - 1
-                for k in range(nseg):                        # k-th segment from the top
-                    q = nseg - 1 - k
-                    b_ = end - q * sj
-                    a_ = max(start, b_ - sj + 1)
-                    node = e if k == 0 else rest + k - 1
-                    tn = (e if k == 1 else rest + k - 2) if k > 0 else (node_at[pc] if pc >= 0 else -1)
-                    assert seg_of_node[node] == (a_, b_ - a_, tn), (it, e, k)
-                    assert k == 0 or pn[node] == tn
-                assert pn[e] == (node_at[pc] if pc >= 0 else e)          # a root reads itself (its f is 0)
-                # the children of this branch hang off its last compartment
-                kids = sorted(s_ for s_, (ln2, pc2, l2) in want.items() if pc2 == end)
-                if not kids:
-                    assert nlead == 0 and cfirst == nnode[it] - 1        # pulls the all-zero node
+        for start, (ln, pc, lw) in want.items():
+            nseg = -(-ln // max_segment)
+            sj = -(-ln // nseg)
+            end = start + ln - 1
+            prev = node_at[pc] if pc >= 0 else -1
+            for k in range(nseg):                            # k-th segment from the top
+                q = nseg - 1 - k
+                b_ = end - q * sj
+                a_ = max(start, b_ - sj + 1)
+                mm, node, tn = seg_at[a_]
+                assert mm == b_ - a_ and tn == prev, (it, start, k)
+                assert pn[node] == (prev if prev >= 0 else node)             # a root reads itself (its f is 0)
+                prev = node
+            lanes_seen.add(start)
+        assert len(lanes_seen) == len(want) and len(seg_of_node) == nnode[it]
+        # backward-sweep tasks: every node once; a node's step is above its children's; children of the same
+        # tier sit in the same group: the first in the node's own lane, the others in its lane mask; children
+        # of earlier tiers are in its pull list; at most 32 lanes per group
+        blob = plan.table("item_task_blob")[plan.table("item_task_offsets")[it]:plan.table("item_task_offsets")[it + 1]]
+        where = {}
+        for tier, groups, ents, pull, raw in parse_tasks(blob):
+            for gi, (gh, nsteps, nsh) in enumerate(groups):
+                for lane in range(32):
+                    prev = None
+                    for k in range(int(gh[lane]), int(gh[lane + 1])):
+                        node, step = int(ents[k, 0]) & 0xfffff, (int(ents[k, 0]) >> 20) & 0xfff
+                        assert node not in where and step < nsteps
+                        where[node] = (tier, gi, lane, step, k)
+                        if prev is not None:                 # the lane's chain: each node the parent of the one before
+                            assert pn[prev[0]] == node and step >= prev[1]
+                        prev = (node, step)
+        assert sorted(where) == list(range(nnode[it]))
+        kids_of = {}
+        for v in range(nnode[it]):
+            if pn[v] != v:
+                kids_of.setdefault(int(pn[v]), []).append(v)
+        _, _, ents, pull, _ = parse_tasks(blob)[0]
+        for v, (tier, gi, lane, step, k) in where.items():
+            same = [c for c in kids_of.get(v, []) if where[c][0] == tier]
+            lower = [c for c in kids_of.get(v, []) if where[c][0] != tier]
+            assert all(where[c][0] < tier for c in lower)
+            assert sorted(int(c) for c in pull[int(ents[k, 2]):int(ents[k, 2]) + int(ents[k, 3])]) == sorted(lower)
+            mask = int(ents[k, 1]) & 0xffffffff
+            if same:
+                assert all(where[c][1] == gi for c in same)
+                if where[same[0]][3] == step:                # a run (plain chains only): the single child's step
+                    assert len(same) == 1 and mask == 0
                 else:
-                    kid_lanes = sorted(node_at_start for node_at_start in
-                                       (n_ for n_, pos in top_node_pos.items() if pos in kids and n_ < len(dsc)))
-                    assert len(kid_lanes) == len(kids) and kid_lanes == list(range(kid_lanes[0], kid_lanes[0] + len(kids)))
-                    assert cfirst == kid_lanes[0] and lb[l + 1] <= cfirst < lb[l + 2]
-                    if len(kids) <= 32:
-                        assert nlead == 1 and (cfirst - lb[l + 1]) // 32 == (kid_lanes[-1] - lb[l + 1]) // 32
-                        assert [(int(dsc[q_, 0]) >> 16) & 0xff for q_ in kid_lanes] == list(range(len(kids) - 1, -1, -1))
-                    else:
-                        assert nlead == len(kids) and all(((int(dsc[q_, 0]) >> 16) & 0xff) == 0 for q_ in kid_lanes)
-        assert len(lanes_seen) == len(want)
+                    assert all(where[c][3] < step for c in same)
+                assert where[min(same)][2] == lane
+                assert mask == sum(1 << where[c][2] for c in same if c != min(same))
+            else:
+                assert mask == 0 and (lower or step == 0)
     assert (seen_cells == (cell_item >= 0)).all()
     # streaming path: every branch of every non-resident cell exactly once, children complete
     sd = plan.table("stream_desc").reshape(-1, 6)
@@ -291,7 +301,7 @@ def test_policy_star_with_many_siblings_and_odd_offsets():
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
         _check_policy(m, plan, kw.get("max_segment", 64))
         _check_interpreted(m, plan)
-        assert ((plan.table("item_desc").reshape(-1, 4)[:, 3] & 0xffff) == 70).any()
+        assert (plan.table("item_desc").reshape(-1, 4)[:, 3] == 70).any()
 
 
 def test_clusters_take_the_cells_too_large_for_one_block():
