@@ -307,8 +307,9 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
             e.level = P.branch_level[j];
             e.parent = P.branch_parent_branch[j] < 0 ? -1 : (int32_t)(b0 + P.branch_parent_branch[j] - B0);
-            e.nseg = (e.len + smax - 1) / smax;
+            e.nseg = std::max<int32_t>(1, (int32_t)((5 * (int64_t)e.len + 2 * smax) / (5 * (int64_t)smax)));   // len/smax + 0.4, cut off
             e.sj = (e.len + e.nseg - 1) / e.nseg;
+            e.nseg = (e.len + e.sj - 1) / e.sj;             // no empty segment
             if (e.nseg > 0xffff) out.ok = false;
             lv[e.level].push_back((int32_t)(j - B0));
         }
@@ -835,7 +836,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 2047 || (o.policy_flags & ~63) ||
+        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~63) ||
         o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }

@@ -157,7 +157,7 @@ def _check_policy(m, plan, max_segment=64):
             for a, mt_, mb_, hasq_, node, tnode in pairs(sg):
                 mm = mt_ + mb_ + hasq_
                 assert 0 <= node < nnode[it] and node not in seg_of_node
-                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < max_segment
+                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < 2 * max_segment
                 seg_of_node[int(node)] = (int(base + a), int(mm), int(tnode))
                 node_at[int(base + a + mm)] = int(node)
                 covered[base + a:base + a + mm + 1] += 1
@@ -179,8 +179,9 @@ def _check_policy(m, plan, max_segment=64):
         seg_at = {a: (mm, node, t) for node, (a, mm, t) in seg_of_node.items()}       # by first compartment
         lanes_seen = set()
         for start, (ln, pc, lw) in want.items():
-            nseg = -(-ln // max_segment)
+            nseg = max(1, (5 * ln + 2 * max_segment) // (5 * max_segment))       # len / max_segment + 0.4, cut off
             sj = -(-ln // nseg)
+            nseg = -(-ln // sj)                              # no empty segment
             end = start + ln - 1
             prev = node_at[pc] if pc >= 0 else -1
             for k in range(nseg):                            # k-th segment from the top
