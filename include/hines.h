@@ -131,19 +131,12 @@ typedef enum {
     /* Policy tables (depend on options; validity-checked in tests).
      * A work item is a run of whole cells in ONE block's shared memory, or one cell cut into the chunks
      * of a thread-block cluster.  Its reduced tree has one node per segment (the segment's last
-     * compartment, the "separator"); node ids are item-local: the top node of the branch in lane e has
-     * id e, the other nodes of a branch with nseg > 1 have ids rest, rest+1, ... from the top. */
+     * compartment, the "separator"); node ids are item-local, in the order of the backward sweep's
+     * entries (ITEM_TASK_BLOB). */
     HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  on-chip work item of the cell, -1 = streaming path       */
     HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
     HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  size class                                              */
     HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
-    HINES_TABLE_ITEM_DESC_OFFSETS    = 36,  /* int64[nitems+1] into ITEM_DESC / ITEM_PNODE (in units of lanes)        */
-    HINES_TABLE_ITEM_LEVEL_OFFSETS   = 37,  /* int64[nitems+1] into ITEM_LEVEL_BEGIN                                   */
-    HINES_TABLE_ITEM_LEVEL_BEGIN     = 38,  /* int32[sum (nlevels_item+1)] lane index (item-local) where each level's
-                                               lane list begins                                                        */
-    HINES_TABLE_ITEM_DESC            = 39,  /* int32[4*nlanes] per branch lane (levels in order, siblings contiguous, sibling
-                                               groups by their longest member in segments): {nseg, rest, lane of the first
-                                               child branch, child branches}                                            */
     HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node above it in the reduced tree (a root and
                                                an unused id: itself)                                                    */
     HINES_TABLE_ITEM_NODE_OFFSETS    = 52,  /* int64[nitems+1] into ITEM_PNODE                                          */

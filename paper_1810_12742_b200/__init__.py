@@ -32,8 +32,7 @@ TABLES = {
     "cell_nlevels": (6, np.int32), "cell_level_offsets": (7, np.int64), "level_count": (8, np.int32),
     "level_list": (9, np.int32), "child_offsets": (10, np.int64), "child_ids": (11, np.int32),
     "cell_item": (32, np.int32), "item_cell_range": (33, np.int64), "item_class": (34, np.int32),
-    "item_launch_order": (35, np.int32), "item_desc_offsets": (36, np.int64),
-    "item_level_offsets": (37, np.int64), "item_level_begin": (38, np.int32), "item_desc": (39, np.int32),
+    "item_launch_order": (35, np.int32),
     "stream_level_begin": (40, np.int64), "stream_desc": (41, np.int32), "stream_child": (42, np.int32),
     "class_smem_bytes": (43, np.int32), "item_pnode": (44, np.int32), "item_nnode": (45, np.int32),
     "item_chunk_offsets": (46, np.int64), "chunk_comp_range": (47, np.int64), "chunk_seg_offsets": (48, np.int64),

@@ -14,11 +14,10 @@
 //          A cell too large for one block is cut into chunks held by the blocks of one thread-block
 //          cluster (the paper requires one matrix per block; distributed shared memory
 //          lifts that).  Cells that fit no cluster go to the streaming path.
-//   P3     per (item, level): lane list of the level-synchronous part, one lane per branch.  Sibling
-//          branches are kept in one 32-lane tile so their hand-off values at the branch point
-//           are summed by warp shuffles; sibling groups are sorted by their longest
-//          member, descending (Fig 4.1).  The parent pulls the sum from the slot of
-//          the group's first lane.
+//   P3     the reduced tree (one node per segment) and its backward sweep: sub-trees of at most 32 leaves,
+//          one warp per group of sub-trees, lock-step over the height above the leaves (PAPER.md:110-112
+//          with height in place of depth), a node in the lane of its first child so that the hand-off at
+//          the branch point stays in registers or is a warp shuffle (build_tasks).
 //   P4     segments.  Every branch is cut, from its end, into nseg = ceil(len / max_segment) segments
 //          of Sj = ceil(len / nseg) compartments (the paper's branch splitting, with a
 //          fixed bound instead of the level average).  The last compartment of a segment is its
@@ -49,7 +48,6 @@ static const int kRegsPerThread = 80;           // the resident kernel is built 
 static const int kMaxThreads = 384;
 static const int kMaxClusterClass = 16;
 static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descriptor word 1, bits 24-25)
-static const int32_t kFastTile = 1 << 30;        // descriptor word 0, bit 30
 
 static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
@@ -65,7 +63,6 @@ struct Br {
     int32_t nseg, sj;                        // segments, compartments per segment (the first may be shorter)
     int32_t e = -1, rest = -1;               // lane index (= id of the top node); id of the second node from the top
     int32_t cfirst = 0, nlead = 0;           // hand-off slots the branch's last node pulls from
-    int32_t nafter = 0;                      // siblings to the right whose contributions this lane absorbs by shuffle
 };
 
 // Lists of one work item: cells [c0,c1) in nchunks chunks, policies P3 + P4.
@@ -314,11 +311,10 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             lv[e.level].push_back((int32_t)(j - B0));
         }
     }
-    // ---- P3: lane lists of the level-synchronous part -----------------------------------------
-    // Sibling branches (same parent branch) are contiguous and, when there are at most 32 of them,
-    // inside one 32-lane tile (tiles counted from the level's first lane), so that their hand-off
-    // values are summed by warp shuffles; sibling groups are ordered by their longest member in
-    // level-synchronous steps, descending, ties by (cell, branch id).
+    // ---- P3: nodes of the reduced tree ----------------------------------------------------------
+    // Branches level by level, siblings contiguous, sibling groups by their longest member in segments,
+    // descending, ties by (cell, branch id): the provisional node numbering from which
+    // build_tasks derives the sweep (and the final numbering).
     out.level_begin.assign(out.nlev + 1, 0);
     std::vector<int32_t> lane_br;                       // branch of every lane, -1 = padding
     struct Group { int32_t first, count, maxseg, minord; };
@@ -914,10 +910,6 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_CELL_RANGE, P->item_cell_range)
         TBL(HINES_TABLE_ITEM_CLASS, P->item_class)
         TBL(HINES_TABLE_ITEM_LAUNCH_ORDER, P->item_launch_order)
-        TBL(HINES_TABLE_ITEM_DESC_OFFSETS, P->item_desc_offsets)
-        TBL(HINES_TABLE_ITEM_LEVEL_OFFSETS, P->item_level_offsets)
-        TBL(HINES_TABLE_ITEM_LEVEL_BEGIN, P->item_level_begin)
-        TBL(HINES_TABLE_ITEM_DESC, P->item_desc)
         TBL(HINES_TABLE_ITEM_PNODE, P->item_pnode)
         TBL(HINES_TABLE_ITEM_NODE_OFFSETS, P->item_node_offsets)
         TBL(HINES_TABLE_ITEM_ROUNDS, P->item_rounds)

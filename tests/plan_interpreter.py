@@ -57,10 +57,6 @@ def solve_with_tables(plan, m, d, u, b):
     """x for every cell that sits in an on-chip work item (NaN elsewhere)."""
     x = np.full(m.n, np.nan)
     rng_ = plan.table("item_cell_range").reshape(-1, 2)
-    desc_off = plan.table("item_desc_offsets")
-    lvl_off = plan.table("item_level_offsets")
-    lvl_begin = plan.table("item_level_begin")
-    desc = plan.table("item_desc").reshape(-1, 4)
     pnode_all = plan.table("item_pnode")
     nnode = plan.table("item_nnode")
     node_off = plan.table("item_node_offsets")

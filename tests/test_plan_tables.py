@@ -104,10 +104,6 @@ def _check_policy(m, plan, max_segment=64):
     E = 16 // w
     cell_item = plan.table("cell_item")
     rng_ = plan.table("item_cell_range").reshape(-1, 2)
-    desc_off = plan.table("item_desc_offsets")
-    lvl_off = plan.table("item_level_offsets")
-    lvl_begin = plan.table("item_level_begin")
-    desc = plan.table("item_desc").reshape(-1, 4)
     pnode = plan.table("item_pnode")
     nnode = plan.table("item_nnode")
     node_off = plan.table("item_node_offsets")
@@ -139,12 +135,8 @@ def _check_policy(m, plan, max_segment=64):
         assert nch == cls_cluster[cls[it]] and (nch == 1 or c1 - c0 == 1)
         cr = ch_rng[ch_off[it]:ch_off[it + 1]]
         assert cr[0, 0] == comp0 and cr[-1, 1] == comp0 + n_it and (cr[1:, 0] == cr[:-1, 1]).all()
-        dsc = desc[desc_off[it]:desc_off[it + 1]]
         pn = pnode[node_off[it]:node_off[it + 1]]
         assert len(pn) == nnode[it]
-        lb = lvl_begin[lvl_off[it]:lvl_off[it + 1]]
-        nlev = len(lb) - 1
-        assert nlev == T.cell_nlevels[c0:c1].max() and lb[0] == 0 and lb[-1] == len(dsc)
         # segments of all chunks -> node of every separator compartment (item-local position)
         node_at = {}                     # separator position -> node
         seg_of_node = {}
@@ -302,7 +294,8 @@ def test_policy_star_with_many_siblings_and_odd_offsets():
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
         _check_policy(m, plan, kw.get("max_segment", 64))
         _check_interpreted(m, plan)
-        assert (plan.table("item_desc").reshape(-1, 4)[:, 3] == 70).any()
+        blob = plan.table("item_task_blob")[:plan.table("item_task_offsets")[1]]
+        assert any(int(e[3]) == 70 for t in parse_tasks(blob)[:1] for e in t[2])      # the star's root pulls its 70 children
 
 
 def test_clusters_take_the_cells_too_large_for_one_block():
