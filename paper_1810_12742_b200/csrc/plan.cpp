@@ -103,30 +103,32 @@ static void order_window(const SegTmp* segs, size_t n, int R, int32_t off, bool 
 {
     std::vector<std::vector<SegTmp>> bucket(R);
     for (size_t k = 0; k < n; ++k) bucket[(segs[k].a + off) % R].push_back(segs[k]);     // stays longest first
-    std::vector<size_t> head(R, 0);
     size_t remaining = n;
-    std::vector<int> pick;
-    std::vector<int> used(R);
-    while (remaining) {
-        pick.clear();
-        for (int r = 0; r < R; ++r) if (head[r] < bucket[r].size()) pick.push_back(r);
-        size_t taken = pick.size();
-        std::fill(used.begin(), used.end(), 0);
-        for (int q : pick) used[q]++;
-        while (taken < (size_t)R && taken < remaining) {          // second helpings: conflicts only here
-            int best = -1; size_t left = 0;
-            for (int r = 0; r < R; ++r) {
-                const size_t avail = bucket[r].size() - head[r];
-                const size_t l = avail > (size_t)used[r] ? avail - used[r] : 0;
-                if (l > left) { left = l; best = r; }
-            }
-            if (best < 0) break;
-            pick.push_back(best); used[best]++; ++taken;
+    std::vector<char> used_b(R);
+    auto take = [&](int r) {
+        // from bucket r the longest segment whose B lane (start b-1) lands on a bank residue not yet used
+        // in this round; if there is none, the longest
+        auto& bk = bucket[r];
+        size_t pick = 0;
+        for (size_t k = 0; k < bk.size(); ++k) {
+            const int rb = (bk[k].a + bk[k].m - 1 + off + R) % R;
+            if (bk[k].m < 3 || !used_b[rb]) { pick = k; break; }
         }
-        for (int r : pick) {
-            const SegTmp& sg = bucket[r][head[r]++];
-            out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
-            --remaining;
+        const SegTmp sg = bk[pick];
+        bk.erase(bk.begin() + (long)pick);
+        if (sg.m >= 3) used_b[(sg.a + sg.m - 1 + off + R) % R] = 1;
+        out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
+        --remaining;
+    };
+    while (remaining) {
+        std::fill(used_b.begin(), used_b.end(), 0);
+        size_t taken = 0;
+        for (int r = 0; r < R; ++r) if (!bucket[r].empty()) { take(r); ++taken; }
+        while (taken < (size_t)R && remaining) {                   // second helpings: conflicts only here
+            int best = -1; size_t left = 0;
+            for (int r = 0; r < R; ++r) if (bucket[r].size() > left) { left = bucket[r].size(); best = r; }
+            if (best < 0) break;
+            take(best); ++taken;
         }
         if (remaining || !last) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
     }

@@ -162,6 +162,11 @@ template <> __device__ __forceinline__ double lds1<double>(uint32_t a)
 { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory"); return v; }
 template <> __device__ __forceinline__ float lds1<float>(uint32_t a)
 { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; }
+template <typename T> __device__ __forceinline__ void sts1(uint32_t a, T v);
+template <> __device__ __forceinline__ void sts1<double>(uint32_t a, double v)
+{ asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
+template <> __device__ __forceinline__ void sts1<float>(uint32_t a, float v)
+{ asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
 template <typename T> __device__ __forceinline__ void sts2(uint32_t a, typename Vec2<T>::type v);
 template <> __device__ __forceinline__ void sts2<double>(uint32_t a, double2 v)
 { asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory"); }
@@ -288,18 +293,34 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         if (isB && hasq) { ee = su[i + 1]; D = T(0); if (m > 0) { D = sd[i]; B = sb[i]; } }
         if (m > 0) un = su[i + uo];
         if (mload > 0) { dn = sd[i + sgn]; bn = sb[i + sgn]; }
-        for (int s = 0; s < mmax; ++s) {
-            if (s < m) {
-                T un2 = T(0), dn2 = T(0), bn2 = T(0);
-                if (s + 1 < m) un2 = su[i + sgn + uo];                                       // next step's inputs
-                if (s + 1 < mload) { dn2 = sd[i + 2 * sgn]; bn2 = sb[i + 2 * sgn]; }
-                const T r = rcp<T>(D);
-                const T g = un * r, h = ee * r, c = B * r;
-                sd[i] = g; su[i] = h; sb[i] = c;
-                ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);
-                D = fnma<T>(g, un, dn); B = fnma<T>(g, B, bn); ee = -h * un;
-                i += sgn; un = un2; dn = dn2; bn = bn2;
+        {
+            // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
+            // loop is unrolled by two with the two register sets swapping roles (no register rotation).
+            const uint32_t LW = (uint32_t)L * (uint32_t)sizeof(T);
+            uint32_t pa = smem_u32(sd + i);
+            const int stp = sgn * (int)sizeof(T);
+            const uint32_t o_u = (uint32_t)(stp + (int)LW + uo * (int)sizeof(T));      // u of the next step
+            const uint32_t o_d = (uint32_t)(2 * stp), o_b = (uint32_t)(2 * stp) + 2u * LW;   // d, b of the node after next
+            T un2 = T(0), dn2 = T(0), bn2 = T(0);
+#define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2)                                                     \
+            if (s < m) {                                                                             \
+                UN2 = T(0); DN2 = T(0); BN2 = T(0);                                                  \
+                if (s + 1 < m) UN2 = lds1<T>(pa + o_u);                                              \
+                if (s + 1 < mload) { DN2 = lds1<T>(pa + o_d); BN2 = lds1<T>(pa + o_b); }             \
+                const T r = rcp<T>(D);                                                               \
+                const T g = UN * r, h = ee * r, c = B * r;                                           \
+                sts1<T>(pa, g); sts1<T>(pa + LW, h); sts1<T>(pa + 2u * LW, c);                       \
+                ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);                                 \
+                D = fnma<T>(g, UN, DN); B = fnma<T>(g, B, BN); ee = -h * UN;                         \
+                pa += (uint32_t)stp;                                                                 \
+            }                                                                                        \
+            ++s;
+            for (int s = 0; s < mmax;) {
+                HINES_P1_STEP(un, dn, bn, un2, dn2, bn2)
+                HINES_P1_STEP(un2, dn2, bn2, un, dn, bn)
             }
+#undef HINES_P1_STEP
+            i += sgn * m;
         }
         // B -> A: update of q (pD, pB), coupling q-b (pe), contribution parked for b (pdd, pdb)
         const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
