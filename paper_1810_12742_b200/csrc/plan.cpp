@@ -94,55 +94,52 @@ struct ItemBuild {
 
 struct SegTmp { int32_t a, m, node, tnode; };
 
-// Segment lane list of one chunk.  R lanes access shared memory in one wavefront; they should start at
-// distinct residues mod R (they stay distinct while all lanes advance in lock-step) AND have similar
-// lengths (a warp runs as long as its longest lane).  Segments are sorted by length,
-// longest first, and cut into windows of 4 R; inside a window they are bucketed by start residue, and a
-// round takes the longest remaining segment of every bucket, topped up from the fullest buckets.
-static void order_window(const SegTmp* segs, size_t n, int R, int32_t off, bool last, std::vector<int32_t>& out)
-{
-    std::vector<std::vector<SegTmp>> bucket(R);
-    for (size_t k = 0; k < n; ++k) bucket[(segs[k].a + off) % R].push_back(segs[k]);     // stays longest first
-    size_t remaining = n;
-    std::vector<char> used_b(R);
-    auto take = [&](int r) {
-        // from bucket r the longest segment whose B lane (start b-1) lands on a bank residue not yet used
-        // in this round; if there is none, the longest
-        auto& bk = bucket[r];
-        size_t pick = 0;
-        for (size_t k = 0; k < bk.size(); ++k) {
-            const int rb = (bk[k].a + bk[k].m - 1 + off + R) % R;
-            if (bk[k].m < 3 || !used_b[rb]) { pick = k; break; }
-        }
-        const SegTmp sg = bk[pick];
-        bk.erase(bk.begin() + (long)pick);
-        if (sg.m >= 3) used_b[(sg.a + sg.m - 1 + off + R) % R] = 1;
-        out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
-        --remaining;
-    };
-    while (remaining) {
-        std::fill(used_b.begin(), used_b.end(), 0);
-        size_t taken = 0;
-        for (int r = 0; r < R; ++r) if (!bucket[r].empty()) { take(r); ++taken; }
-        while (taken < (size_t)R && remaining) {                   // second helpings: conflicts only here
-            int best = -1; size_t left = 0;
-            for (int r = 0; r < R; ++r) if (bucket[r].size() > left) { left = bucket[r].size(); best = r; }
-            if (best < 0) break;
-            take(best); ++taken;
-        }
-        if (remaining || !last) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
-    }
-}
-
+// Segment lane list of one chunk.  R = 16 segments share a warp (A lanes 0-15, B lanes 16-31); the lanes of a
+// half-warp access shared memory in one wavefront if they start at distinct residues mod R (they stay
+// distinct while all lanes advance in lock-step), and a warp runs as long as its longest lane.
+// Segments are sorted by length, longest first; a group takes, scanning from the longest remaining segment,
+// up to R segments whose A lane (start a) AND B lane (start b-1) fall on residues not yet used in the group;
+// the scan looks at most 6 R segments ahead, then relaxes the B lanes, then fills up with the longest remaining.
 static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
 {
     std::vector<SegTmp> sorted(segs);
     std::stable_sort(sorted.begin(), sorted.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
+    const size_t n = sorted.size();
+    std::vector<int32_t> next(n + 1);                       // singly linked list over the sorted order, n = end
+    for (size_t k = 0; k <= n; ++k) next[k] = (int32_t)k + 1;
+    int32_t head = n ? 0 : (int32_t)n;
     out.clear();
-    const size_t W = 4 * (size_t)R;
-    for (size_t w0 = 0; w0 < sorted.size(); w0 += W) {
-        const size_t n = std::min(W, sorted.size() - w0);
-        order_window(sorted.data() + w0, n, R, off, w0 + n == sorted.size(), out);
+    std::vector<char> ua(R), ub(R);
+    size_t remaining = n;
+    auto emit = [&](int32_t k) {
+        const SegTmp& sg = sorted[k];
+        out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
+        --remaining;
+    };
+    while (remaining) {
+        std::fill(ua.begin(), ua.end(), 0); std::fill(ub.begin(), ub.end(), 0);
+        int taken = 0;
+        // pass 0: A and B lanes conflict-free; pass 1: A lanes only; pass 2: fill up (measured: idle lanes cost
+        // more than the conflicts they avoid, the sweeps are bound by warp-steps, not by shared-memory wavefronts)
+        for (int pass = 0; pass < 3 && taken < R && remaining; ++pass) {
+            int32_t prev = -1, k = head;
+            for (int looked = 0; k < (int32_t)n && taken < R && looked < 6 * R; ++looked) {
+                const SegTmp& sg = sorted[k];
+                const int ra = (sg.a + off) % R, rb = (sg.a + sg.m - 1 + off + R) % R;
+                const bool usesB = sg.m >= 3;
+                const bool ok = pass == 2 || (!ua[ra] && (pass == 1 || !usesB || !ub[rb]));
+                const int32_t nx = next[k];
+                if (ok) {
+                    ua[ra] = 1; if (usesB) ub[rb] = 1;
+                    emit(k); ++taken;
+                    if (prev < 0) head = nx; else next[prev] = nx;       // unlink
+                } else {
+                    prev = k;
+                }
+                k = nx;
+            }
+        }
+        if (remaining || (out.size() / 4) % R) while ((out.size() / 4) % R) out.insert(out.end(), {0, 0, -1, -1});
     }
 }
 
