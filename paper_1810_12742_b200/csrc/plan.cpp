@@ -92,7 +92,7 @@ struct ItemBuild {
     int32_t max_lanes = 0;                   // widest segment lane list of a chunk
 };
 
-struct SegTmp { int32_t a, m, node, tnode; };
+struct SegTmp { int32_t a, m, node, tnode, mt = -1; };   // mt: interior nodes lane A takes (-1: half)
 
 // Segment lane list of one chunk.  R = 16 segments share a warp (A lanes 0-15, B lanes 16-31); the lanes of a
 // half-warp access shared memory in one wavefront if they start at distinct residues mod R (they stay
@@ -113,7 +113,7 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     size_t remaining = n;
     auto emit = [&](int32_t k) {
         const SegTmp& sg = sorted[k];
-        out.insert(out.end(), {sg.a, sg.m, sg.node, sg.tnode});
+        out.insert(out.end(), {sg.a, sg.m | (sg.mt << 16), sg.node, sg.tnode});
         --remaining;
     };
     while (remaining) {
@@ -124,10 +124,23 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
         for (int pass = 0; pass < 3 && taken < R && remaining; ++pass) {
             int32_t prev = -1, k = head;
             for (int looked = 0; k < (int32_t)n && taken < R && looked < 6 * R; ++looked) {
-                const SegTmp& sg = sorted[k];
-                const int ra = (sg.a + off) % R, rb = (sg.a + sg.m - 1 + off + R) % R;
+                SegTmp& sg = sorted[k];
+                const int ra = (sg.a + off) % R;
+                // lane B starts at q + 1 = a + mt + 1: the split point may move by up to two nodes off the middle
+                // to put B on a free residue
                 const bool usesB = sg.m >= 3;
+                int mt = sg.m / 2, rb = (sg.a + mt + 1 + off) % R;
+                if (usesB && pass == 0 && ub[rb]) {
+                    static const int kDelta[4] = {1, -1, 2, -2};
+                    for (int t = 0; t < 4; ++t) {
+                        const int cand = sg.m / 2 + kDelta[t];
+                        if (cand < 0 || cand > sg.m - 2) continue;
+                        const int r2 = (sg.a + cand + 1 + off) % R;
+                        if (!ub[r2]) { mt = cand; rb = r2; break; }
+                    }
+                }
                 const bool ok = pass == 2 || (!ua[ra] && (pass == 1 || !usesB || !ub[rb]));
+                if (ok) sg.mt = mt;
                 const int32_t nx = next[k];
                 if (ok) {
                     ua[ra] = 1; if (usesB) ub[rb] = 1;
@@ -441,12 +454,12 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
                 const int32_t* sgp = &ord[(size_t)(gidx * 16 + k) * 4];
                 int32_t* A = &ch.seg[(size_t)(gidx * 32 + k) * 4];
                 int32_t* B = &ch.seg[(size_t)(gidx * 32 + 16 + k) * 4];
-                const int32_t a = sgp[0], mm = sgp[1], node = sgp[2], tnode = sgp[3];
+                const int32_t a = sgp[0], mm = sgp[1] & 0xffff, node = sgp[2], tnode = sgp[3];
                 if (node < 0) { A[2] = A[3] = B[2] = B[3] = -1; continue; }
-                const int32_t hasq = mm > 0, mt = hasq ? mm / 2 : 0, mb = hasq ? mm - 1 - mt : 0;
+                const int32_t hasq = mm > 0, mt = hasq ? std::min(sgp[1] >> 16, mm - 1) : 0, mb = hasq ? mm - 1 - mt : 0;
                 const int32_t word = mt | (mb << 12) | (hasq << 26);
                 A[0] = a; A[1] = word | (kSegA << 24); A[2] = node; A[3] = tnode;
-                B[0] = a + mm - 1; B[1] = word | (kSegB << 24); B[2] = node; B[3] = -1;
+                B[0] = a + mt + 1; B[1] = word | (kSegB << 24); B[2] = node; B[3] = -1;   // B starts below q = a + mt
                 mx = std::max(mx, std::max(mt, mb));
             }
             out.padded_steps += 32 * (int64_t)(mx + 1);     // the loop steps of the warp + the step for q

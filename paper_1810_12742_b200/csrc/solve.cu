@@ -274,45 +274,37 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
     const unsigned FULL = 0xffffffffu;
 
     // ---- P1: condense the interiors of all segments (no level dependency) ----
-    // Two lanes per segment [a..b] (b = separator, t = separator above): lane A eliminates the upper
-    // half a..q-1 top-down (fill-in coupling to t), lane B = A ^ 16 the lower half b-1..q+1 bottom-up
-    // (fill-in coupling to b); A then takes B's update of the middle node q, eliminates q and writes
-    // the node record of b.  Lane: node i = base + sgn s at step s.
+    // Two lanes per segment [a..b] (b = separator, t = separator above), split at a middle node q: lane A
+    // eliminates a..q-1 top-down with fill-in coupling to t and arrives at q; lane B = A ^ 16 eliminates
+    // q+1..b-1 top-down with fill-in coupling to q and arrives at b.  A then takes B's contribution to q,
+    // eliminates q (couplings to t and to b) and writes the node record of b.  Both lanes run the same code.
     for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
         const bool isB = kind == 2;
         const int m = isB ? mb : (kind == 1 ? mt : 0);
-        const int sgn = isB ? -1 : 1, uo = isB ? 0 : 1;
-        const int mload = isB ? m - 1 : m;                  // B's last step: only the update of q is wanted
         const int mmax = __reduce_max_sync(FULL, m);
         int i = sg.x + off;
         T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
-        if (kind == 1) { D = sd[i]; B = sb[i]; if (sg.w >= 0) ee = su[i]; }
-        if (isB && hasq) { ee = su[i + 1]; D = T(0); if (m > 0) { D = sd[i]; B = sb[i]; } }
-        if (m > 0) un = su[i + uo];
-        if (mload > 0) { dn = sd[i + sgn]; bn = sb[i + sgn]; }
+        if (kind == 1 || (isB && hasq)) { D = sd[i]; B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
+        if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; bn = sb[i + 1]; }
         {
             // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
             // loop is unrolled by two with the two register sets swapping roles (no register rotation).
-            const uint32_t LW = (uint32_t)L * (uint32_t)sizeof(T);
-            uint32_t pa = smem_u32(sd + i);
-            const int stp = sgn * (int)sizeof(T);
-            const uint32_t o_u = (uint32_t)(stp + (int)LW + uo * (int)sizeof(T));      // u of the next step
-            const uint32_t o_d = (uint32_t)(2 * stp), o_b = (uint32_t)(2 * stp) + 2u * LW;   // d, b of the node after next
+            constexpr uint32_t W = (uint32_t)sizeof(T);
+            const uint32_t LW = (uint32_t)L * W;
+            uint32_t pa = smem_u32(sd + i), pu = pa + LW, pb = pa + 2u * LW;
             T un2 = T(0), dn2 = T(0), bn2 = T(0);
 #define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2)                                                     \
             if (s < m) {                                                                             \
-                UN2 = T(0); DN2 = T(0); BN2 = T(0);                                                  \
-                if (s + 1 < m) UN2 = lds1<T>(pa + o_u);                                              \
-                if (s + 1 < mload) { DN2 = lds1<T>(pa + o_d); BN2 = lds1<T>(pa + o_b); }             \
+                if (s + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); BN2 = lds1<T>(pb + 2u * W); } \
                 const T r = rcp<T>(D);                                                               \
                 const T g = UN * r, h = ee * r, c = B * r;                                           \
-                sts1<T>(pa, g); sts1<T>(pa + LW, h); sts1<T>(pa + 2u * LW, c);                       \
+                sts1<T>(pa, g); sts1<T>(pu, h); sts1<T>(pb, c);                                      \
                 ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);                                 \
                 D = fnma<T>(g, UN, DN); B = fnma<T>(g, B, BN); ee = -h * UN;                         \
-                pa += (uint32_t)stp;                                                                 \
+                pa += W; pu += W; pb += W;                                                           \
             }                                                                                        \
             ++s;
             for (int s = 0; s < mmax;) {
@@ -320,22 +312,20 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                 HINES_P1_STEP(un2, dn2, bn2, un, dn, bn)
             }
 #undef HINES_P1_STEP
-            i += sgn * m;
+            i += m;
         }
-        // B -> A: update of q (pD, pB), coupling q-b (pe), contribution parked for b (pdd, pdb)
+        // B -> A: what is left of b (pD, pB), its coupling to q (pe), B's contribution parked for q (pdd, pdb)
         const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
-        T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
+        const T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
         if (kind == 1) {
             T* q = ND + 6 * sg.z;
             if (hasq) {                                     // i is q now
-                const T Dq = D + pD, Bq = B + pB;
+                const T Dq = D - pdd, Bq = B - pdb;
                 const T r = rcp<T>(Dq);
                 const T gq = pe * r, hq = ee * r;
                 sd[i] = gq; su[i] = hq; sb[i] = Bq * r;
                 ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
-                pdd = fmad<T>(gq, pe, pdd); pdb = fmad<T>(gq, Bq, pdb);
-                const int bp = i + 1 + mb;
-                q[0] = sd[bp] - pdd; q[1] = sb[bp] - pdb; q[2] = -hq * pe; q[4] = ddt; q[5] = dbt;
+                q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = -hq * pe; q[4] = ddt; q[5] = dbt;
             } else {                                        // a segment of one compartment: the separator as it is
                 q[0] = D; q[1] = B; q[2] = ee; q[4] = T(0); q[5] = T(0);
             }
@@ -462,15 +452,15 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
     HINES_STAMP(4);
 
     const int xs = 2 * (it.rounds & 1) + 1;               // record slot that holds x after the forward sweep
-    // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t], then A walks up from q-1 to a
-    //      and B walks down from q+1 to b-1, one FMA on the dependent chain per step ----
+    // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t]; then A walks up from q-1 to a
+    //      (x[i] = c - g x[i+1] - h x[t]) and B walks up from b-1 to q+1 (x[i] = c - g x[i+1] - h x[q]), one FMA
+    //      on the dependent chain per step ----
     for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
         const bool isB = kind == 2;
         const int m = isB ? mb : (kind == 1 ? mt : 0);
-        const int sgn = isB ? -1 : 1;
         const int mmax = __reduce_max_sync(FULL, m);
         const int p0 = sg.x + off;
         T xb = T(0), xt = T(0), xn = T(0);
@@ -486,15 +476,15 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
             }
         }
         const T xq = __shfl_xor_sync(FULL, xn, 16);
-        if (isB) { xn = xq; xt = xb; }
+        if (isB) { xn = xb; xt = xq; }
         T g1 = T(0), h1 = T(0), c1 = T(0);
-        if (m > 0) { const int i = p0 + sgn * (m - 1); g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
+        if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
         for (int j = mmax - 1; j >= 0; --j) {
             if (j < m) {
                 T g2 = T(0), h2 = T(0), c2 = T(0);
-                if (j > 0) { const int i2 = p0 + sgn * (j - 1); g2 = sd[i2]; h2 = su[i2]; c2 = sb[i2]; }
+                if (j > 0) { const int i2 = p0 + j - 1; g2 = sd[i2]; h2 = su[i2]; c2 = sb[i2]; }
                 xn = fnma<T>(g1, xn, fnma<T>(h1, xt, c1));       // one FMA on the dependent chain
-                sb[p0 + sgn * j] = xn;
+                sb[p0 + j] = xn;
                 g1 = g2; h1 = h2; c1 = c2;
             }
         }

@@ -25,7 +25,7 @@ def pairs(sg):
             assert ka == 1 and kb == 2 and (int(A[1]) & ~(3 << 24)) == (int(B[1]) & ~(3 << 24)) and A[2] == B[2]
             mt, mb, hasq = int(A[1]) & 0xfff, (int(A[1]) >> 12) & 0xfff, (int(A[1]) >> 26) & 1
             mm = mt + mb + hasq
-            assert B[0] == A[0] + mm - 1 and (hasq or (mt == 0 and mb == 0)) and abs(mt - mb) <= 1
+            assert (B[0] == A[0] + mt + 1 or not hasq) and (hasq or (mt == 0 and mb == 0)) and abs(mt - mb) <= 5
             yield int(A[0]), mt, mb, hasq, int(A[2]), int(A[3])
 
 
@@ -93,28 +93,25 @@ def solve_with_tables(plan, m, d, u, b):
                     i += 1
                 if hasq:
                     q = a + mt; bp = q + 1 + mb
-                    # lane B: lower half b-1..q+1 bottom-up, fill-in coupling to b
-                    eb = su[bp]; pD = pB = pdd = pdb = 0.0
-                    if mb > 0:
-                        j = bp - 1
-                        Db, Bb = sd[j], sb[j]
-                        for s_ in range(mb):
-                            un = su[j]
-                            dn, bn = (sd[j - 1], sb[j - 1]) if s_ + 1 < mb else (0.0, 0.0)
-                            r = 1.0 / Db
-                            g, h, c = un * r, eb * r, Bb * r
-                            sd[j], su[j], sb[j] = g, h, c
-                            pdd += h * eb; pdb += h * Bb
-                            Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
-                            j -= 1
-                        pD, pB = Db, Bb
-                    Dq, Bq = D + pD, B + pB
+                    # lane B: q+1..b-1 top-down, fill-in coupling to q; arrives at b
+                    j = q + 1
+                    Db, Bb, eb = sd[j], sb[j], su[j]
+                    pdd = pdb = 0.0
+                    for _ in range(mb):
+                        un, dn, bn = su[j + 1], sd[j + 1], sb[j + 1]
+                        r = 1.0 / Db
+                        g, h, c = un * r, eb * r, Bb * r
+                        sd[j], su[j], sb[j] = g, h, c
+                        pdd += h * eb; pdb += h * Bb
+                        Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
+                        j += 1
+                    assert j == bp
+                    Dq, Bq = D - pdd, B - pdb
                     r = 1.0 / Dq
                     gq, hq = eb * r, ee * r
                     sd[q], su[q], sb[q] = gq, hq, Bq * r
                     ddt += hq * ee; dbt += hq * Bq
-                    pdd += gq * eb; pdb += gq * Bq
-                    rec = (sd[bp] - pdd, sb[bp] - pdb, -hq * eb, ddt, dbt)
+                    rec = (Db - gq * eb, Bb - gq * Bq, -hq * eb, ddt, dbt)
                 else:
                     rec = (D, B, ee, 0.0, 0.0)
                 assert np.isnan(rD[node]), "node written twice"
@@ -188,9 +185,9 @@ def solve_with_tables(plan, m, d, u, b):
                 for j in range(q - 1, a - 1, -1):
                     xn = (sb[j] - su[j] * xt) - sd[j] * xn
                     sb[j] = xn
-                xn = xq
-                for j in range(q + 1, bp):
-                    xn = (sb[j] - su[j] * xb) - sd[j] * xn
+                xn = xb
+                for j in range(bp - 1, q, -1):
+                    xn = (sb[j] - su[j] * xq) - sd[j] * xn
                     sb[j] = xn
             x[g0:g1] = sb
     return x
