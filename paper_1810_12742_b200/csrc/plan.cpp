@@ -121,9 +121,11 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
         int taken = 0;
         // pass 0: A and B lanes conflict-free; pass 1: A lanes only; pass 2: fill up (measured: idle lanes cost
         // more than the conflicts they avoid, the sweeps are bound by warp-steps, not by shared-memory wavefronts)
+        const int kLook = 6, kMinFill = R - 2;             // a group that is nearly full is not filled up with conflicts
         for (int pass = 0; pass < 3 && taken < R && remaining; ++pass) {
+            if (pass > 0 && taken >= kMinFill) break;
             int32_t prev = -1, k = head;
-            for (int looked = 0; k < (int32_t)n && taken < R && looked < 6 * R; ++looked) {
+            for (int looked = 0; k < (int32_t)n && taken < R && looked < kLook * R; ++looked) {
                 SegTmp& sg = sorted[k];
                 const int ra = (sg.a + off) % R;
                 // lane B starts at q + 1 = a + mt + 1: the split point may move by up to two nodes off the middle
