@@ -149,8 +149,8 @@ typedef enum {
     HINES_TABLE_CHUNK_SEG            = 49,  /* int32[4*nseglanes] two lanes per segment, in groups of 32: lanes 0-15 the
                                                A halves, lanes 16-31 their B partners (lane ^ 16).  A: {a = first
                                                compartment (chunk-local), word, node, node of the separator above (-1 =
-                                               none)}; B: {b-1, word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26
-                                               (kind 0 padding, 1 A, 2 B; mt/mb = compartments A / B eliminate; the
+                                               none)}; B: {a+mt+1, word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26
+                                               (kind 0 padding, 1 A, 2 B; mt/mb = compartments A / B eliminate, both top-down; the
                                                middle node q = a+mt exists iff hasq; separator b = a+mt+mb+hasq)        */
     HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
     HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment

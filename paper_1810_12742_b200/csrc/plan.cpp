@@ -62,7 +62,6 @@ struct Br {
     int32_t start, len, pc, level, parent;   // item-local positions; parent = index into the item's branch array
     int32_t nseg, sj;                        // segments, compartments per segment (the first may be shorter)
     int32_t e = -1, rest = -1;               // lane index (= id of the top node); id of the second node from the top
-    int32_t cfirst = 0, nlead = 0;           // hand-off slots the branch's last node pulls from
 };
 
 // Lists of one work item: cells [c0,c1) in nchunks chunks, policies P3 + P4.
@@ -70,8 +69,6 @@ struct ItemBuild {
     int64_t comp_begin = 0, n = 0;
     int32_t nlev = 0, ndesc = 0, nnode = 0, nchunks = 1;
     bool ok = true;                          // false: a field overflows its descriptor bits -> streaming path
-    std::vector<int32_t> level_begin;        // nlev+1, in branch lanes
-    std::vector<int32_t> desc;               // 4 per branch lane
     std::vector<int32_t> pnode;              // 1 per node: the node above it in the reduced tree; itself for a root / an unused id
     std::vector<int32_t> perm;               // node id used while the lists were built -> final node id (build_tasks)
     std::vector<int32_t> task_blob;          // device tables of the backward sweep (build_tasks), multiple of 4 ints
@@ -98,7 +95,7 @@ struct SegTmp { int32_t a, m, node, tnode, mt = -1; };   // mt: interior nodes l
 // half-warp access shared memory in one wavefront if they start at distinct residues mod R (they stay
 // distinct while all lanes advance in lock-step), and a warp runs as long as its longest lane.
 // Segments are sorted by length, longest first; a group takes, scanning from the longest remaining segment,
-// up to R segments whose A lane (start a) AND B lane (start b-1) fall on residues not yet used in the group;
+// up to R segments whose A lane (start a) AND B lane (start q+1) fall on residues not yet used in the group;
 // the scan looks at most 6 R segments ahead, then relaxes the B lanes, then fills up with the longest remaining.
 static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
 {
@@ -119,8 +116,8 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     while (remaining) {
         std::fill(ua.begin(), ua.end(), 0); std::fill(ub.begin(), ub.end(), 0);
         int taken = 0;
-        // pass 0: A and B lanes conflict-free; pass 1: A lanes only; pass 2: fill up (measured: idle lanes cost
-        // more than the conflicts they avoid, the sweeps are bound by warp-steps, not by shared-memory wavefronts)
+        // pass 0: A and B lanes conflict-free; pass 1: A lanes only; pass 2: fill up a group that is far from
+        // full (measured: many idle lanes cost more than the conflicts they avoid)
         const int kLook = 6, kMinFill = R - 2;             // a group that is nearly full is not filled up with conflicts
         for (int pass = 0; pass < 3 && taken < R && remaining; ++pass) {
             if (pass > 0 && taken >= kMinFill) break;
@@ -329,7 +326,6 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
     // Branches level by level, siblings contiguous, sibling groups by their longest member in segments,
     // descending, ties by (cell, branch id): the provisional node numbering from which
     // build_tasks derives the sweep (and the final numbering).
-    out.level_begin.assign(out.nlev + 1, 0);
     std::vector<int32_t> lane_br;                       // branch of every lane, -1 = padding
     struct Group { int32_t first, count, maxseg, minord; };
     std::vector<Group> groups;
@@ -352,21 +348,14 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             if (a.maxseg != b.maxseg) return a.maxseg > b.maxseg;
             return a.minord < b.minord;
         });
-        const int32_t lb = (int32_t)lane_br.size();
-        out.level_begin[l] = lb;
-        for (const Group& g : groups) {
-            const int32_t first_lane = (int32_t)lane_br.size();
+        for (const Group& g : groups)
             for (int32_t i = 0; i < g.count; ++i) {
                 Br& e = br[v[g.first + i]];
                 e.e = (int32_t)lane_br.size();
                 lane_br.push_back(v[g.first + i]);
             }
-            const int32_t par = br[v[g.first]].parent;
-            if (par >= 0) { br[par].cfirst = first_lane; br[par].nlead = g.count; }
-        }
     }
     out.ndesc = (int32_t)lane_br.size();
-    out.level_begin[out.nlev] = out.ndesc;
     int32_t next_id = out.ndesc;
     for (int32_t e = 0; e < out.ndesc; ++e) {
         if (lane_br[e] < 0) continue;
@@ -376,16 +365,12 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
     out.nnode = next_id;
     if (out.nnode >= (1 << 20)) out.ok = false;
     auto last_node = [&](const Br& b) { return b.nseg > 1 ? b.rest + b.nseg - 2 : b.e; };
-    // per branch lane: {segments, id of the second node, lane of the first child branch, child branches}
-    out.desc.assign(4 * (size_t)out.ndesc, 0);
     out.pnode.resize(out.nnode);
     std::iota(out.pnode.begin(), out.pnode.end(), 0);
     std::vector<int32_t> depth(out.nnode, 1);          // nodes on the path from the root, inclusive
     int32_t height = 1;
     for (int32_t e = 0; e < out.ndesc; ++e) {           // lanes are in level order: parents come first
         const Br& b = br[lane_br[e]];
-        out.desc[4 * e + 0] = b.nseg; out.desc[4 * e + 1] = b.rest;
-        out.desc[4 * e + 2] = b.cfirst; out.desc[4 * e + 3] = b.nlead;
         if (b.parent >= 0) { out.pnode[e] = last_node(br[b.parent]); depth[e] = depth[out.pnode[e]] + 1; }
         for (int32_t k = 1; k < b.nseg; ++k) {          // a root keeps itself as parent: its f is 0
             out.pnode[b.rest + k - 1] = k == 1 ? e : b.rest + k - 2;
@@ -442,8 +427,8 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         ch.n = mine.empty() ? 0 : mine.back().a + mine.back().m + 1 - ch.begin;
         for (SegTmp& sg : mine) sg.a -= ch.begin;
         const int32_t off = (int32_t)((out.comp_begin + ch.begin) % E);
-        // two lanes per segment: lane A eliminates the upper half of the interior top-down, lane B the
-        // lower half bottom-up, they meet at the middle node q, which A eliminates last.  A warp holds
+        // two lanes per segment: lane A eliminates the interior above the middle node q, lane B the interior
+        // below it, both top-down (fill-in to t resp. q); A eliminates q last.  A warp holds
         // 16 segments: A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
         std::vector<int32_t> ord;
         order_segments(mine, 16, off, ord);
@@ -573,11 +558,7 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     P.item_cell_range.push_back(c0);
     P.item_cell_range.push_back(c1);
     P.item_class.push_back(0);                     // filled by assign_classes
-    P.item_level_begin.insert(P.item_level_begin.end(), ib.level_begin.begin(), ib.level_begin.end());
-    P.item_level_offsets.push_back((int64_t)P.item_level_begin.size());
-    P.item_desc.insert(P.item_desc.end(), ib.desc.begin(), ib.desc.end());
     P.item_pnode.insert(P.item_pnode.end(), ib.pnode.begin(), ib.pnode.end());
-    P.item_desc_offsets.push_back((int64_t)P.item_desc.size() / 4);
     P.item_node_offsets.push_back((int64_t)P.item_pnode.size());
     P.item_rounds.push_back(ib.rounds);
     P.item_nnode.push_back(ib.nnode);
@@ -640,8 +621,6 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     const int64_t single_cap = no_cluster ? max_smem : chunk_cap;
     const bool pow2_only = P.opt.policy_flags & HINES_POLICY_POW2_CLUSTERS;
     P.cell_item.assign(nc, -1);
-    P.item_level_offsets.assign(1, 0);
-    P.item_desc_offsets.assign(1, 0);
     P.item_node_offsets.assign(1, 0);
     P.item_task_offsets.assign(1, 0);
     P.item_chunk_offsets.assign(1, 0);

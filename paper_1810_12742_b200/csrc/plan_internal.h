@@ -68,9 +68,9 @@ struct hines_plan {
     std::vector<int32_t> branch_start, branch_len, branch_parent_comp, branch_parent_branch,
         branch_level, cell_nlevels, level_count, level_list, child_ids;
     // policy tables
-    std::vector<int32_t> cell_item, item_class, item_launch_order, item_level_begin, item_desc, item_pnode,
+    std::vector<int32_t> cell_item, item_class, item_launch_order, item_pnode,
         item_nnode, item_rounds, item_task_blob, chunk_seg;
-    std::vector<int64_t> item_cell_range, item_desc_offsets, item_node_offsets, item_task_offsets, item_level_offsets, item_chunk_offsets,
+    std::vector<int64_t> item_cell_range, item_node_offsets, item_task_offsets, item_chunk_offsets,
         chunk_comp_range, chunk_seg_offsets;
     std::vector<int32_t> class_smem_bytes;             // per class: dynamic smem per block
     std::vector<int32_t> class_cluster;                // per class: blocks per item (cluster size), 1 = no cluster
