@@ -92,11 +92,15 @@ struct ItemBuild {
 struct SegTmp { int32_t a, m, node, tnode, mt = -1; };   // mt: interior nodes lane A takes (-1: half)
 
 // Segment lane list of one chunk.  R = 16 segments share a warp (A lanes 0-15, B lanes 16-31); the lanes of a
-// half-warp access shared memory in one wavefront if they start at distinct residues mod R (they stay
-// distinct while all lanes advance in lock-step), and a warp runs as long as its longest lane.
-// Segments are sorted by length, longest first; a group takes, scanning from the longest remaining segment,
-// up to R segments whose A lane (start a) AND B lane (start q+1) fall on residues not yet used in the group;
-// the scan looks at most 6 R segments ahead, then relaxes the B lanes, then fills up with the longest remaining.
+// half-warp access shared memory in one wavefront if, at every step, they sit on distinct residues mod R, and
+// a warp runs as long as its longest lane.  Segments are sorted by length, longest first, and
+// a group is cut from the head of the list: its step count is the longer half of the head segment.  A lane
+// that is shorter than the group may START LATE: a delay of dl steps moves its residue by -dl in every step,
+// at no cost.  For each of the next kLook candidates the split point (off the middle by up to two nodes) and
+// the delays of both lanes are chosen so that the A lanes and the B lanes of the group keep distinct residues;
+// a candidate that cannot be placed stays in the list.  A group that ends up far from full is filled up with
+// the longest remaining segments, conflicts and all.
+// out: 4 ints per segment {a, m | mt << 12 | dA << 24 | dB << 28, node, tnode}, groups padded to R with node -1.
 static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
 {
     std::vector<SegTmp> sorted(segs);
@@ -108,42 +112,41 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     out.clear();
     std::vector<char> ua(R), ub(R);
     size_t remaining = n;
-    auto emit = [&](int32_t k) {
+    auto emit = [&](int32_t k, int mt, int dA, int dB) {
         const SegTmp& sg = sorted[k];
-        out.insert(out.end(), {sg.a, sg.m | (sg.mt << 16), sg.node, sg.tnode});
+        const uint32_t word = (uint32_t)sg.m | ((uint32_t)mt << 12) | ((uint32_t)dA << 24) | ((uint32_t)dB << 28);
+        out.insert(out.end(), {sg.a, (int32_t)word, sg.node, sg.tnode});
         --remaining;
     };
+    const int kLook = 2 * R, kMinFill = R - 2, kMaxDelay = 15;
+    static const int kDelta[5] = {0, 1, -1, 2, -2};
     while (remaining) {
         std::fill(ua.begin(), ua.end(), 0); std::fill(ub.begin(), ub.end(), 0);
         int taken = 0;
-        // pass 0: A and B lanes conflict-free; pass 1: A lanes only; pass 2: fill up a group that is far from
-        // full (measured: many idle lanes cost more than the conflicts they avoid)
-        const int kLook = 6, kMinFill = R - 2;             // a group that is nearly full is not filled up with conflicts
-        for (int pass = 0; pass < 3 && taken < R && remaining; ++pass) {
+        const int nhalf = sorted[head].m / 2;              // steps of the group: mt = m/2 >= mb = m-1-mt of the head
+        for (int pass = 0; pass < 2 && taken < R && remaining; ++pass) {
             if (pass > 0 && taken >= kMinFill) break;
             int32_t prev = -1, k = head;
-            for (int looked = 0; k < (int32_t)n && taken < R && looked < kLook * R; ++looked) {
-                SegTmp& sg = sorted[k];
-                const int ra = (sg.a + off) % R;
-                // lane B starts at q + 1 = a + mt + 1: the split point may move by up to two nodes off the middle
-                // to put B on a free residue
-                const bool usesB = sg.m >= 3;
-                int mt = sg.m / 2, rb = (sg.a + mt + 1 + off) % R;
-                if (usesB && pass == 0 && ub[rb]) {
-                    static const int kDelta[4] = {1, -1, 2, -2};
-                    for (int t = 0; t < 4; ++t) {
-                        const int cand = sg.m / 2 + kDelta[t];
-                        if (cand < 0 || cand > sg.m - 2) continue;
-                        const int r2 = (sg.a + cand + 1 + off) % R;
-                        if (!ub[r2]) { mt = cand; rb = r2; break; }
-                    }
+            for (int looked = 0; k < (int32_t)n && taken < R && looked < kLook; ++looked) {
+                const SegTmp& sg = sorted[k];
+                int mt = sg.m / 2, dA = 0, dB = 0;
+                bool ok = pass == 1 || sg.m == 0;
+                for (int t = 0; t < 5 && !ok; ++t) {
+                    const int cmt = sg.m / 2 + kDelta[t], cmb = sg.m - 1 - cmt;
+                    if (cmt < 0 || cmb < 0 || cmt > nhalf || cmb > nhalf) continue;
+                    int fa = -1, fb = -1;
+                    for (int dl = 0; dl <= std::min(kMaxDelay, nhalf - cmt) && fa < 0; ++dl)
+                        if (cmt == 0 || !ua[((sg.a + off - dl) % R + R) % R]) fa = dl;
+                    for (int dl = 0; dl <= std::min(kMaxDelay, nhalf - cmb) && fb < 0; ++dl)
+                        if (cmb == 0 || !ub[((sg.a + cmt + 1 + off - dl) % R + R) % R]) fb = dl;
+                    if (fa >= 0 && fb >= 0) { ok = true; mt = cmt; dA = cmt ? fa : 0; dB = cmb ? fb : 0; }
                 }
-                const bool ok = pass == 2 || (!ua[ra] && (pass == 1 || !usesB || !ub[rb]));
-                if (ok) sg.mt = mt;
                 const int32_t nx = next[k];
                 if (ok) {
-                    ua[ra] = 1; if (usesB) ub[rb] = 1;
-                    emit(k); ++taken;
+                    const int mb = sg.m - 1 - mt;
+                    if (mt > 0) ua[((sg.a + off - dA) % R + R) % R] = 1;
+                    if (mb > 0) ub[((sg.a + mt + 1 + off - dB) % R + R) % R] = 1;
+                    emit(k, mt, dA, dB); ++taken;
                     if (prev < 0) head = nx; else next[prev] = nx;       // unlink
                 } else {
                     prev = k;
@@ -441,13 +444,15 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
                 const int32_t* sgp = &ord[(size_t)(gidx * 16 + k) * 4];
                 int32_t* A = &ch.seg[(size_t)(gidx * 32 + k) * 4];
                 int32_t* B = &ch.seg[(size_t)(gidx * 32 + 16 + k) * 4];
-                const int32_t a = sgp[0], mm = sgp[1] & 0xffff, node = sgp[2], tnode = sgp[3];
+                const uint32_t ow = (uint32_t)sgp[1];
+                const int32_t a = sgp[0], mm = (int32_t)(ow & 0xfff), node = sgp[2], tnode = sgp[3];
                 if (node < 0) { A[2] = A[3] = B[2] = B[3] = -1; continue; }
-                const int32_t hasq = mm > 0, mt = hasq ? std::min(sgp[1] >> 16, mm - 1) : 0, mb = hasq ? mm - 1 - mt : 0;
+                const int32_t hasq = mm > 0, mt = hasq ? std::min<int32_t>((ow >> 12) & 0xfff, mm - 1) : 0, mb = hasq ? mm - 1 - mt : 0;
+                const int32_t dA = (int32_t)((ow >> 24) & 15), dB = (int32_t)(ow >> 28);
                 const int32_t word = mt | (mb << 12) | (hasq << 26);
-                A[0] = a; A[1] = word | (kSegA << 24); A[2] = node; A[3] = tnode;
-                B[0] = a + mt + 1; B[1] = word | (kSegB << 24); B[2] = node; B[3] = -1;   // B starts below q = a + mt
-                mx = std::max(mx, std::max(mt, mb));
+                A[0] = a; A[1] = word | (kSegA << 24) | (dA << 27); A[2] = node; A[3] = tnode;
+                B[0] = a + mt + 1; B[1] = (int32_t)((uint32_t)word | ((uint32_t)kSegB << 24) | ((uint32_t)dB << 27)); B[2] = node; B[3] = -1;   // B starts below q = a + mt
+                mx = std::max(mx, std::max(mt + dA, mb + dB));
             }
             out.padded_steps += 32 * (int64_t)(mx + 1);     // the loop steps of the warp + the step for q
         }

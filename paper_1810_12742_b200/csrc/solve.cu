@@ -284,7 +284,8 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
         const bool isB = kind == 2;
         const int m = isB ? mb : (kind == 1 ? mt : 0);
-        const int mmax = __reduce_max_sync(FULL, m);
+        const int dl = (sg.y >> 27) & 15;                   // the lane starts dl steps late (bank residues, plan.cpp)
+        const int mmax = __reduce_max_sync(FULL, m + dl);
         int i = sg.x + off;
         T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
         if (kind == 1 || (isB && hasq)) { D = sd[i]; B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
@@ -295,10 +296,10 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
             constexpr uint32_t W = (uint32_t)sizeof(T);
             const uint32_t LW = (uint32_t)L * W;
             uint32_t pa = smem_u32(sd + i), pu = pa + LW, pb = pa + 2u * LW;
-            T un2 = T(0), dn2 = T(0), bn2 = T(0);
+            T un2 = un, dn2 = dn, bn2 = bn;                 // a lane's first step may fall on either half of the loop body
 #define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2)                                                     \
-            if (s < m) {                                                                             \
-                if (s + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); BN2 = lds1<T>(pb + 2u * W); } \
+            if ((unsigned)sl < (unsigned)m) {                                                        \
+                if (sl + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); BN2 = lds1<T>(pb + 2u * W); } \
                 const T r = rcp<T>(D);                                                               \
                 const T g = UN * r, h = ee * r, c = B * r;                                           \
                 sts1<T>(pa, g); sts1<T>(pu, h); sts1<T>(pb, c);                                      \
@@ -306,8 +307,9 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                 D = fnma<T>(g, UN, DN); B = fnma<T>(g, B, BN); ee = -h * UN;                         \
                 pa += W; pu += W; pb += W;                                                           \
             }                                                                                        \
-            ++s;
-            for (int s = 0; s < mmax;) {
+            ++sl;
+            int sl = -dl;
+            for (int s = 0; s < mmax; s += 2) {
                 HINES_P1_STEP(un, dn, bn, un2, dn2, bn2)
                 HINES_P1_STEP(un2, dn2, bn2, un, dn, bn)
             }
@@ -461,7 +463,8 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
         const bool isB = kind == 2;
         const int m = isB ? mb : (kind == 1 ? mt : 0);
-        const int mmax = __reduce_max_sync(FULL, m);
+        const int dl = (sg.y >> 27) & 15;
+        const int mmax = __reduce_max_sync(FULL, m + dl);
         const int p0 = sg.x + off;
         T xb = T(0), xt = T(0), xn = T(0);
         if (kind != 0) xb = ND[6 * sg.z + xs];
@@ -479,8 +482,9 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         if (isB) { xn = xb; xt = xq; }
         T g1 = T(0), h1 = T(0), c1 = T(0);
         if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
-        for (int j = mmax - 1; j >= 0; --j) {
-            if (j < m) {
+        for (int jj = mmax - 1; jj >= 0; --jj) {
+            const int j = jj - dl;                          // the lane's own step: the same residue shift as in P1
+            if ((unsigned)j < (unsigned)m) {
                 T g2 = T(0), h2 = T(0), c2 = T(0);
                 if (j > 0) { const int i2 = p0 + j - 1; g2 = sd[i2]; h2 = su[i2]; c2 = sb[i2]; }
                 xn = fnma<T>(g1, xn, fnma<T>(h1, xt, c1));       // one FMA on the dependent chain

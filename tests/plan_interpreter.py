@@ -22,7 +22,8 @@ def pairs(sg):
             if ka == 0:
                 assert kb == 0 and A[2] == -1 and B[2] == -1
                 continue
-            assert ka == 1 and kb == 2 and (int(A[1]) & ~(3 << 24)) == (int(B[1]) & ~(3 << 24)) and A[2] == B[2]
+            msk = ~((3 << 24) | (15 << 27))                # kind and the lane's start delay differ between A and B
+            assert ka == 1 and kb == 2 and (int(A[1]) & msk) == (int(B[1]) & msk) and A[2] == B[2]
             mt, mb, hasq = int(A[1]) & 0xfff, (int(A[1]) >> 12) & 0xfff, (int(A[1]) >> 26) & 1
             mm = mt + mb + hasq
             assert (B[0] == A[0] + mt + 1 or not hasq) and (hasq or (mt == 0 and mb == 0)) and abs(mt - mb) <= 5
