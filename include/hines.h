@@ -77,8 +77,9 @@ typedef struct {
                                        block as possible")                                                 */
     int32_t max_segment;            /* 0 = default (64), 2..1023: target segment length.  A branch of len compartments
                                        is cut into max(1, floor(len / max_segment + 0.4)) chained segments of equal
-                                       length (so a segment is at most 1.4 x max_segment + 1 long) (PAPER.md:151
-                                       "we split branches that are too long")                                   */
+                                       length, made odd when there are several (their starts then fall on
+                                       distinct shared-memory banks), so a segment is at most 1.4 x max_segment + 2
+                                       long ("we split branches that are too long")               */
     int32_t cluster_max;            /* 0 = default (16), 1..16: largest thread-block cluster a cell may be spread
                                        over (more than 8 needs the non-portable cluster size)                  */
     int32_t chunk_smem_bytes;       /* 0 = default (113 KiB, two blocks per SM): shared memory one block of a

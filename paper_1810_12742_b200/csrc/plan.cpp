@@ -97,11 +97,13 @@ struct SegTmp { int32_t a, m, node, tnode, mt = -1; };   // mt: interior nodes l
 // a group is cut from the head of the list: its step count is the longer half of the head segment.  A lane
 // that is shorter than the group may START LATE: a delay of dl steps moves its residue by -dl in every step,
 // at no cost.  For each of the next kLook candidates the split point (off the middle by up to two nodes) and
-// the delays of both lanes are chosen so that the A lanes and the B lanes of the group keep distinct residues;
+// the delays of both lanes are chosen so that the A lanes and the B lanes of the group keep distinct residues
+// mod NB (fp64: NB = 16 banks of 8 bytes, A and B lanes are different wavefronts; fp32: NB = 32, all 32 lanes
+// are one wavefront and share one set of residues);
 // a candidate that cannot be placed stays in the list.  A group that ends up far from full is filled up with
 // the longest remaining segments, conflicts and all.
 // out: 4 ints per segment {a, m | mt << 12 | dA << 24 | dB << 28, node, tnode}, groups padded to R with node -1.
-static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, std::vector<int32_t>& out)
+static void order_segments(const std::vector<SegTmp>& segs, int R, int NB, int32_t off, std::vector<int32_t>& out)
 {
     std::vector<SegTmp> sorted(segs);
     std::stable_sort(sorted.begin(), sorted.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
@@ -110,7 +112,9 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     for (size_t k = 0; k <= n; ++k) next[k] = (int32_t)k + 1;
     int32_t head = n ? 0 : (int32_t)n;
     out.clear();
-    std::vector<char> ua(R), ub(R);
+    std::vector<char> ua_(NB), ub_(NB);
+    std::vector<char>& ua = ua_;
+    std::vector<char>& ub = NB > R ? ua_ : ub_;            // one wavefront: one set
     size_t remaining = n;
     auto emit = [&](int32_t k, int mt, int dA, int dB) {
         const SegTmp& sg = sorted[k];
@@ -121,7 +125,7 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
     const int kLook = 2 * R, kMinFill = R - 2, kMaxDelay = 15;
     static const int kDelta[5] = {0, 1, -1, 2, -2};
     while (remaining) {
-        std::fill(ua.begin(), ua.end(), 0); std::fill(ub.begin(), ub.end(), 0);
+        std::fill(ua_.begin(), ua_.end(), 0); std::fill(ub_.begin(), ub_.end(), 0);
         int taken = 0;
         const int nhalf = sorted[head].m / 2;              // steps of the group: mt = m/2 >= mb = m-1-mt of the head
         for (int pass = 0; pass < 2 && taken < R && remaining; ++pass) {
@@ -136,16 +140,19 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int32_t off, 
                     if (cmt < 0 || cmb < 0 || cmt > nhalf || cmb > nhalf) continue;
                     int fa = -1, fb = -1;
                     for (int dl = 0; dl <= std::min(kMaxDelay, nhalf - cmt) && fa < 0; ++dl)
-                        if (cmt == 0 || !ua[((sg.a + off - dl) % R + R) % R]) fa = dl;
-                    for (int dl = 0; dl <= std::min(kMaxDelay, nhalf - cmb) && fb < 0; ++dl)
-                        if (cmb == 0 || !ub[((sg.a + cmt + 1 + off - dl) % R + R) % R]) fb = dl;
+                        if (cmt == 0 || !ua[((sg.a + off - dl) % NB + NB) % NB]) fa = dl;
+                    const int ra = NB > R && cmt > 0 && fa >= 0 ? ((sg.a + off - fa) % NB + NB) % NB : -1;
+                    for (int dl = 0; dl <= std::min(kMaxDelay, nhalf - cmb) && fb < 0; ++dl) {
+                        const int rb = ((sg.a + cmt + 1 + off - dl) % NB + NB) % NB;
+                        if (cmb == 0 || (!ub[rb] && rb != ra)) fb = dl;
+                    }
                     if (fa >= 0 && fb >= 0) { ok = true; mt = cmt; dA = cmt ? fa : 0; dB = cmb ? fb : 0; }
                 }
                 const int32_t nx = next[k];
                 if (ok) {
                     const int mb = sg.m - 1 - mt;
-                    if (mt > 0) ua[((sg.a + off - dA) % R + R) % R] = 1;
-                    if (mb > 0) ub[((sg.a + mt + 1 + off - dB) % R + R) % R] = 1;
+                    if (mt > 0) ua[((sg.a + off - dA) % NB + NB) % NB] = 1;
+                    if (mb > 0) ub[((sg.a + mt + 1 + off - dB) % NB + NB) % NB] = 1;
                     emit(k, mt, dA, dB); ++taken;
                     if (prev < 0) head = nx; else next[prev] = nx;       // unlink
                 } else {
@@ -320,6 +327,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             e.parent = P.branch_parent_branch[j] < 0 ? -1 : (int32_t)(b0 + P.branch_parent_branch[j] - B0);
             e.nseg = std::max<int32_t>(1, (int32_t)((5 * (int64_t)e.len + 2 * smax) / (5 * (int64_t)smax)));   // len/smax + 0.4, cut off
             e.sj = (e.len + e.nseg - 1) / e.nseg;
+            if (e.nseg > 1 && e.sj % 2 == 0) ++e.sj;        // odd: the segments of one branch start on distinct banks
             e.nseg = (e.len + e.sj - 1) / e.sj;             // no empty segment
             if (e.nseg > 0xffff) out.ok = false;
             lv[e.level].push_back((int32_t)(j - B0));
@@ -434,7 +442,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         // below it, both top-down (fill-in to t resp. q); A eliminates q last.  A warp holds
         // 16 segments: A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
         std::vector<int32_t> ord;
-        order_segments(mine, 16, off, ord);
+        order_segments(mine, 16, P.width == 8 ? 16 : 32, off, ord);
         while ((ord.size() / 4) % 16) ord.insert(ord.end(), {0, 0, -1, -1});
         const int32_t ngroups = (int32_t)(ord.size() / 64);
         ch.seg.assign((size_t)ngroups * 128, 0);

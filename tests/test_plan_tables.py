@@ -173,6 +173,8 @@ def _check_policy(m, plan, max_segment=64):
         for start, (ln, pc, lw) in want.items():
             nseg = max(1, (5 * ln + 2 * max_segment) // (5 * max_segment))       # len / max_segment + 0.4, cut off
             sj = -(-ln // nseg)
+            if nseg > 1 and sj % 2 == 0:
+                sj += 1                                      # odd: the segments of a branch start on distinct banks
             nseg = -(-ln // sj)                              # no empty segment
             end = start + ln - 1
             prev = node_at[pc] if pc >= 0 else -1
