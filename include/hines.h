@@ -75,7 +75,8 @@ typedef struct {
     int32_t group_smem_bytes;       /* 0 = default (56 KiB): small cells are grouped into work items up to
                                        this much shared memory ("fit as many matrices into one
                                        block as possible")                                                 */
-    int32_t max_segment;            /* 0 = default (64), 2..1023: target segment length.  A branch of len compartments
+    int32_t max_segment;            /* 0 = default (40 for a cell in a block of its own, 64 for a cell spread over a
+                                       cluster), 2..1023: target segment length.  A branch of len compartments
                                        is cut into max(1, floor(len / max_segment + 0.4)) chained segments of equal
                                        length, made odd when there are several (their starts then fall on
                                        distinct shared-memory banks), so a segment is at most 1.4 x max_segment + 2

@@ -304,7 +304,7 @@ static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
 
 static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchunks, ItemBuild& out)
 {
-    const int32_t smax = P.opt.max_segment;
+    const int32_t smax = nchunks > 1 ? P.seg_cluster : P.seg_single;
     const int E = 16 / P.width;
     out = ItemBuild();
     out.nchunks = nchunks;
@@ -832,7 +832,8 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.smem_bytes_per_block == 0) o.smem_bytes_per_block = (int32_t)kSmemMaxOptin;
     if (o.stream_threads == 0) o.stream_threads = 128;
     if (o.group_smem_bytes == 0) o.group_smem_bytes = 57344;
-    if (o.max_segment == 0) o.max_segment = 64;
+    const bool auto_segment = o.max_segment == 0;     // default: 40 in a block of its own, 64 in the blocks of a cluster
+    if (auto_segment) o.max_segment = 64;
     if (o.cluster_max == 0) o.cluster_max = 16;
     if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 113 * 1024;
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
@@ -853,6 +854,8 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         hines_plan* P = new hines_plan();
         P->n = cell_offsets[ncells]; P->ncells = ncells; P->dtype = dtype; P->width = dtype == HINES_F64 ? 8 : 4;
         P->opt = o;
+        P->seg_cluster = o.max_segment;
+        P->seg_single = auto_segment ? 40 : o.max_segment;
         P->cell_offsets.assign(cell_offsets, cell_offsets + ncells + 1);
         hines_status_t st = canonical_tables(*P, parent);
         if (st != HINES_OK) { delete P; return st; }

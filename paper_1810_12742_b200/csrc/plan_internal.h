@@ -61,6 +61,7 @@ struct hines_plan {
     hines_options_t opt{};
     int32_t max_levels = 0;
     int32_t breadth_first = 1;
+    int32_t seg_single = 64, seg_cluster = 64;         // segment target (max_segment) of single-block / cluster items
 
     std::vector<int64_t> cell_offsets;
     // canonical tables T1-T7

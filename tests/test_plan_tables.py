@@ -92,7 +92,7 @@ def test_validation_errors():
     assert lib.hines_status_string(4) == b"CUDA error"
 
 
-def _check_policy(m, plan, max_segment=64):
+def _check_policy(m, plan, max_segment=0):
     """Validity invariants (policy-free): every cell in exactly one on-chip item or on the streaming
     path; the chunks of an item tile its compartment range; segments tile every branch exactly, each
     inside one chunk and listed once; node ids are unique; a segment's upper node is the node of the
@@ -142,6 +142,8 @@ def _check_policy(m, plan, max_segment=64):
         seg_of_node = {}
         covered = np.zeros(n_it, int)
         nlanes_max = 0
+        # segment target of the item: the option, or by default 40 in a block of its own, 64 in a cluster
+        S_it = max_segment if max_segment else (40 if ch_off[it + 1] - ch_off[it] == 1 else 64)
         for r, ch in enumerate(range(ch_off[it], ch_off[it + 1])):
             sg = segs[seg_off[ch]:seg_off[ch + 1]]
             nlanes_max = max(nlanes_max, len(sg))
@@ -149,7 +151,7 @@ def _check_policy(m, plan, max_segment=64):
             for a, mt_, mb_, hasq_, node, tnode in pairs(sg):
                 mm = mt_ + mb_ + hasq_
                 assert 0 <= node < nnode[it] and node not in seg_of_node
-                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < 2 * max_segment
+                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < 2 * S_it
                 seg_of_node[int(node)] = (int(base + a), int(mm), int(tnode))
                 node_at[int(base + a + mm)] = int(node)
                 covered[base + a:base + a + mm + 1] += 1
@@ -171,7 +173,7 @@ def _check_policy(m, plan, max_segment=64):
         seg_at = {a: (mm, node, t) for node, (a, mm, t) in seg_of_node.items()}       # by first compartment
         lanes_seen = set()
         for start, (ln, pc, lw) in want.items():
-            nseg = max(1, (5 * ln + 2 * max_segment) // (5 * max_segment))       # len / max_segment + 0.4, cut off
+            nseg = max(1, (5 * ln + 2 * S_it) // (5 * S_it))       # len / max_segment + 0.4, cut off
             sj = -(-ln // nseg)
             if nseg > 1 and sj % 2 == 0:
                 sj += 1                                      # odd: the segments of a branch start on distinct banks
@@ -281,7 +283,7 @@ def _check_interpreted(m, plan):
 ])
 def test_policy_tables_valid(cfg, scale, kw):
     m, plan = _plan_cfg(cfg, scale, **kw)
-    _check_policy(m, plan, kw.get("max_segment", 64))
+    _check_policy(m, plan, kw.get("max_segment", 0))
     _check_interpreted(m, plan)
 
 
@@ -294,7 +296,7 @@ def test_policy_star_with_many_siblings_and_odd_offsets():
     for kw in ({}, dict(dtype=hb.F32), dict(policy_flags=hb.POLICY_NO_GROUPING), dict(max_segment=3),
                dict(chunk_smem_bytes=6000, max_segment=4)):
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
-        _check_policy(m, plan, kw.get("max_segment", 64))
+        _check_policy(m, plan, kw.get("max_segment", 0))
         _check_interpreted(m, plan)
         blob = plan.table("item_task_blob")[:plan.table("item_task_offsets")[1]]
         assert any(int(e[3]) == 70 for t in parse_tasks(blob)[:1] for e in t[2])      # the star's root pulls its 70 children
