@@ -337,7 +337,6 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
     HINES_STAMP(2);
 
     if (rank == 0) {
-        const int32_t* pnode = imeta + it.pnode_off;
         typedef typename Vec2<T>::type V2;
         // ---- P2 backward on the reduced tree --------------------------------------
         // Sub-trees of at most 32 leaves, one warp per group of sub-trees, lock-step over the height above
@@ -427,7 +426,11 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                 __syncthreads();
             }
         }
-        HINES_STAMP(3);
+    }
+    HINES_STAMP(3);                 // outside the rank test: a stamp in both arms of it splits warp 0 for all of P2
+    if (rank == 0) {
+        const int32_t* pnode = imeta + it.pnode_off;
+        typedef typename Vec2<T>::type V2;
         // ---- P2 forward by pointer jumping over the reduced tree --------------
         // x_v = c_v + g_v x_p(v), g = -f, g_root = 0.  One round replaces (g_v, c_v, p(v)) by
         // (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds >= nodes on the longest
@@ -447,8 +450,6 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
             }
             __syncthreads();
         }
-    } else {
-        HINES_STAMP(3);
     }
     if (CL) cg::this_cluster().sync();
     HINES_STAMP(4);
