@@ -166,8 +166,10 @@ typedef enum {
                                                [ntier, tier_begin (ntier+1), pad4 | groups: 36 ints each = lane_begin[33]
                                                (entry index), steps, byte offset (in the blob) of the per-step shuffle
                                                counts, pad | entries: 4 ints per node, by lane then step = {node |
-                                               step<<20, lane mask of the other children in the group, first, count in
-                                               the pull list} | pull list: nodes swept in an earlier tier whose hand-off
+                                               step<<20, lane mask of the other children in the group, first in the
+                                               pull list, count in the pull list | (entries right behind that continue
+                                               the run with nothing to pull)<<16} | pull list: nodes swept in an earlier
+                                               tier whose hand-off
                                                slot is added, pad4 | shuffle counts (bytes), pad]                         */
     HINES_TABLE_CLASS_CLUSTER        = 50,  /* int32[n_classes] blocks per item = cluster size (1 = no cluster)        */
     HINES_TABLE_CLASS_THREADS        = 51   /* int32[n_classes] threads per block                                      */

@@ -176,7 +176,8 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int NB, int32
 //   group   36 ints: lane_begin[33] (into the item's entries), steps, offset of the per-step shuffle
 //           counts (bytes), pad
 //   entry   4 ints per node, by lane then step: node | step << 20, lanes of the other children in the
-//           same group (bit mask, summed in ascending lane order), first / count of the pull list
+//           same group (bit mask, summed in ascending lane order), first of the pull list, count of the pull
+//           list | (entries behind this one that continue its run with nothing to pull) << 16
 //   pull    node ids whose hand-off slot the node adds (children swept in an earlier tier)
 static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
 {
@@ -261,7 +262,19 @@ static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
                 }
                 int32_t pc = 0; for (uint32_t m = mask; m; m &= m - 1) ++pc;
                 nsh[step_of[v]] = std::max<unsigned char>(nsh[step_of[v]], (unsigned char)pc);
-                out.task_entry.insert(out.task_entry.end(), {v | (step_of[v] << 20), (int32_t)mask, pull0, (int32_t)out.task_pull.size() - pull0});
+                const int32_t npull = (int32_t)out.task_pull.size() - pull0;
+                if (npull > 0xffff) out.ok = false;
+                out.task_entry.insert(out.task_entry.end(), {v | (step_of[v] << 20), (int32_t)mask, pull0, npull});
+            }
+            // upper half of the last word: how many entries right behind this one continue its run with
+            // nothing to pull (same step, only child = the node before): the kernel walks those in a tight loop
+            const size_t e0 = (size_t)out.task_group[gh + l], e1 = out.task_entry.size() / 4;
+            int32_t more = 0;
+            for (size_t k = e1; k-- > e0;) {
+                out.task_entry[4 * k + 3] |= std::min(more, 0xffff) << 16;
+                const bool plain = (out.task_entry[4 * k + 3] & 0xffff) == 0 && k > e0 &&
+                                   (out.task_entry[4 * k] >> 20) == (out.task_entry[4 * (k - 1)] >> 20);
+                more = plain ? more + 1 : 0;
             }
         }
         out.task_group[gh + 32] = (int32_t)(out.task_entry.size() / 4);

@@ -389,9 +389,11 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                         // a run = a node and the single-child nodes above it, all on this step (no shuffle, no pull
                         // after the first): the lane walks it node by node
                         while (estep == h) {
-                            if (en.w) {                                 // children swept in an earlier tier
+                            const int npull = en.w & 0xffff;
+                            int run = en.w >> 16;                       // plain nodes behind this one (same step, nothing to pull)
+                            if (npull) {                                // children swept in an earlier tier
 #pragma unroll 1
-                                for (int k = 0; k < en.w; ++k) {
+                                for (int k = 0; k < npull; ++k) {
                                     const V2 c2 = lds2<T>(nd_sa + (uint32_t)pull[en.z + k] * RS + 4u * W);
                                     sd_ += c2.x; sb_ += c2.y;
                                 }
@@ -417,6 +419,42 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                             } else {                                    // end of the lane's chain: leave the hand-off in the slot
                                 V2 s2; s2.x = outd; s2.y = outb;
                                 sts2<T>(qa + 4u * W, s2);
+                            }
+                            if (run) {
+                                // The plain part of the run in a tight loop: records are consecutive, no descriptor is
+                                // read, the next record is fetched while this one's reciprocal runs; two register
+                                // sets swap roles.  On entry {a0, U, a2} hold the record at qa (= entry pos).
+                                V2 b0, b2; T V;
+                                b0 = a0; b2 = a2; V = U;
+                                pos += run;
+                                const bool ends = pos >= end;           // the run takes the lane's chain to its end
+#define HINES_RUN_NODE(A0, UU, A2, B0, VV, B2)                                                               \
+                                {                                                                            \
+                                    const T D_ = A0.x - outd, B_ = A0.y - outb;                              \
+                                    if (run > 1 || !ends) { B0 = lds2<T>(qa + RS); VV = lds1<T>(qa + RS + 2u * W); B2 = lds2<T>(qa + RS + 4u * W); } \
+                                    const T r_ = rcp<T>(D_);                                                 \
+                                    const T f_ = UU * r_;                                                    \
+                                    V2 o_; o_.x = -f_; o_.y = B_ * r_;                                       \
+                                    sts2<T>(qa, o_);                                                         \
+                                    outd = fmad<T>(f_, UU, A2.x); outb = fmad<T>(f_, B_, A2.y);              \
+                                    qa += RS;                                                                \
+                                }
+#pragma unroll 1
+                                while (true) {
+                                    HINES_RUN_NODE(a0, U, a2, b0, V, b2)
+                                    if (--run == 0) { a0 = b0; U = V; a2 = b2; break; }
+                                    HINES_RUN_NODE(b0, V, b2, a0, U, a2)
+                                    if (--run == 0) break;
+                                }
+#undef HINES_RUN_NODE
+                                if (ends) {
+                                    V2 s2; s2.x = outd; s2.y = outb;
+                                    sts2<T>(qa - RS + 4u * W, s2);
+                                    estep = 0x7fffffff;
+                                } else {
+                                    en = ents[pos];
+                                    estep = en.x >> 20;
+                                }
                             }
                             sd_ = outd; sb_ = outb;                     // the next node of the run has this one as its only child
                         }

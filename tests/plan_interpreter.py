@@ -40,7 +40,7 @@ def parse_tasks(blob):
     nent = int(blob[grp_off + 36 * (ngroups - 1) + 32]) if ngroups else 0
     ents = blob[ent_off:ent_off + 4 * nent].reshape(-1, 4)
     pull_off = ent_off + 4 * nent
-    npull = int((ents[:, 3]).sum()) if nent else 0
+    npull = int((ents[:, 3] & 0xffff).sum()) if nent else 0
     pull = blob[pull_off:pull_off + npull]
     raw = blob.view(np.uint8)
     out = []
@@ -132,8 +132,14 @@ def solve_with_tables(plan, m, d, u, b):
                     for lane in range(32):
                         first = True
                         while pos[lane] < gh[lane + 1]:
-                            w0, mask, p0, pcount = (int(v) for v in ents[pos[lane]])
+                            w0, mask, p0, w3 = (int(v) for v in ents[pos[lane]])
                             node, step = w0 & 0xfffff, (w0 >> 20) & 0xfff
+                            pcount, run = w3 & 0xffff, w3 >> 16
+                            # the run the kernel walks in its tight loop: entries right behind, same step, nothing to pull
+                            assert pos[lane] + run < gh[lane + 1] or run == 0
+                            for k in range(1, run + 1):
+                                wk = [int(v) for v in ents[pos[lane] + k]]
+                                assert (wk[0] >> 20) & 0xfff == step and wk[1] == 0 and wk[3] & 0xffff == 0 and wk[3] >> 16 == run - k
                             if step != h:
                                 assert step > h
                                 break

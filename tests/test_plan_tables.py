@@ -216,7 +216,7 @@ def _check_policy(m, plan, max_segment=0):
             same = [c for c in kids_of.get(v, []) if where[c][0] == tier]
             lower = [c for c in kids_of.get(v, []) if where[c][0] != tier]
             assert all(where[c][0] < tier for c in lower)
-            assert sorted(int(c) for c in pull[int(ents[k, 2]):int(ents[k, 2]) + int(ents[k, 3])]) == sorted(lower)
+            assert sorted(int(c) for c in pull[int(ents[k, 2]):int(ents[k, 2]) + (int(ents[k, 3]) & 0xffff)]) == sorted(lower)
             mask = int(ents[k, 1]) & 0xffffffff
             if same:
                 assert all(where[c][1] == gi for c in same)
