@@ -139,11 +139,14 @@ typedef enum {
     HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
     HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  size class                                              */
     HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
-    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node above it in the reduced tree (a root and
-                                               an unused id: itself)                                                    */
+    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node the FORWARD sweep reads = the node above it
+                                               in the reduced tree; itself for a root, and for every node of a lane chain
+                                               that turns around at a root (ITEM_TASK_BLOB): those are final before the
+                                               pointer jumping starts                                                   */
     HINES_TABLE_ITEM_NODE_OFFSETS    = 52,  /* int64[nitems+1] into ITEM_PNODE                                          */
-    HINES_TABLE_ITEM_ROUNDS          = 53,  /* int32[nitems] pointer-jumping rounds of the forward sweep: 2^rounds >= nodes
-                                               on the longest root path of the reduced tree                             */
+    HINES_TABLE_ITEM_ROUNDS          = 53,  /* int32[nitems] pointer-jumping rounds of the forward sweep: 2^rounds > the
+                                               largest distance of a node to the nearest node that reads itself (0 rounds
+                                               when every chain turns around, e.g. unbranched cables)                   */
     HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] nodes of the reduced tree (>= lanes)                          */
     HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
     HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
@@ -165,7 +168,10 @@ typedef enum {
                                                above the leaves, a node in the lane of its first child:
                                                [ntier, tier_begin (ntier+1), pad4 | groups: 36 ints each = lane_begin[33]
                                                (entry index), steps, byte offset (in the blob) of the per-step shuffle
-                                               counts, pad | entries: 4 ints per node, by lane then step = {node |
+                                               counts, mask of the lanes whose chain ends in a root and turns around
+                                               there (x_root = c_root, then x = c - f x_parent down the lane's chain,
+                                               straight after the backward sweep; all root chains of an item or none:
+                                               only where it saves a pointer-jumping round) | entries: 4 ints per node, by lane then step = {node |
                                                step<<20, lane mask of the other children in the group, first in the
                                                pull list, count in the pull list | (entries right behind that continue
                                                the run with nothing to pull)<<16} | pull list: nodes swept in an earlier

@@ -296,6 +296,46 @@ static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
         for (int32_t v = 0; v < nn; ++v) np[out.perm[v]] = out.perm[out.pnode[v]];
         out.pnode.swap(np);
     }
+    // A lane whose chain ends in a root turns around there: x_root = c_root, then x = c - f x_parent down its own
+    // chain, straight after the backward sweep (group word 35 = mask of such lanes).  Those nodes are final before
+    // the pointer jumping starts and read themselves in it; the rounds follow from the distance of the other nodes
+    // to their nearest final ancestor (2^rounds > distance; none left: no round at all, e.g. unbranched cables).
+    {
+        std::vector<char> fin(nn, 0);
+        for (int32_t g = 0; g < out.ngroups; ++g) {
+            int32_t* gh = &out.task_group[36 * (size_t)g];
+            uint32_t mask = 0;
+            for (int32_t l = 0; l < 32; ++l) {
+                const int32_t b = gh[l], e = gh[l + 1];
+                if (e > b && out.pnode[e - 1] == e - 1) { mask |= 1u << l; for (int32_t k = b; k < e; ++k) fin[k] = 1; }
+            }
+            gh[35] = (int32_t)mask;
+        }
+        std::vector<int32_t> byd(nn), dnew(nn), dist(nn, 0);
+        for (int32_t v = 0; v < nn; ++v) dnew[out.perm[v]] = depth[v];
+        std::iota(byd.begin(), byd.end(), 0);
+        std::stable_sort(byd.begin(), byd.end(), [&](int32_t a, int32_t b) { return dnew[a] < dnew[b]; });   // parents first
+        auto rounds_for = [&](bool turn) {
+            int32_t maxdist = 0;
+            for (int32_t v : byd) {
+                const bool f = turn ? fin[v] != 0 : out.pnode[v] == v;
+                dist[v] = f ? 0 : dist[out.pnode[v]] + 1;
+                maxdist = std::max(maxdist, dist[v]);
+            }
+            int32_t r = 0;
+            while ((1 << r) <= maxdist) ++r;
+            return r;
+        };
+        // the turn-around lengthens the backward sweep by the root chains: taken only where it saves a round
+        const int32_t r_plain = rounds_for(false), r_turn = rounds_for(true);
+        if (r_turn < r_plain) {
+            out.rounds = r_turn;
+            for (int32_t v = 0; v < nn; ++v) if (fin[v]) out.pnode[v] = v;
+        } else {
+            out.rounds = r_plain;
+            for (int32_t g = 0; g < out.ngroups; ++g) out.task_group[36 * (size_t)g + 35] = 0;
+        }
+    }
     // blob: [ntier, tier_begin (ntier+1), pad4 | groups | entries | pull, pad4 | shuffle counts, pad4]
     std::vector<int32_t>& B = out.task_blob;
     B.clear();
@@ -402,8 +442,8 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
         }
         height = std::max(height, depth[e] + b.nseg - 1);
     }
-    while ((1 << out.rounds) < height) ++out.rounds;
-    build_tasks(out, depth);
+    (void)height;
+    build_tasks(out, depth);                            // also sets out.rounds
     if (!out.ok) { out.perm.resize(out.nnode); std::iota(out.perm.begin(), out.perm.end(), 0); }
     // ---- P4: segments, in compartment order ------------------------------------------------------
     // Branch cut from its end into nseg segments of sj compartments (the paper's branch splitting,

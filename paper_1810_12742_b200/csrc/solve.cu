@@ -460,6 +460,22 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                         }
                         nsh = nsh_next;
                     }
+                    // A chain that ended in a root turns around: x_root = c_root, then x = c - f x_parent down the
+                    // lane's own chain (records consecutive, loads independent of the chain); these nodes are final
+                    // before the pointer jumping ({g, c} := {0, x}).
+                    if ((gh[35] >> lane) & 1) {
+                        const int begin = gh[lane];
+                        uint32_t qk = nd_sa + (uint32_t)(end - 1) * RS;
+                        T xv = lds1<T>(qk + W);
+#pragma unroll 4
+                        for (int k = end - 2; k >= begin; --k) {
+                            qk -= RS;
+                            const V2 gc = lds2<T>(qk);
+                            xv = fmad<T>(gc.x, xv, gc.y);
+                            V2 o; o.x = T(0); o.y = xv;
+                            sts2<T>(qk, o);
+                        }
+                    }
                 }
                 __syncthreads();
             }

@@ -31,7 +31,7 @@ def pairs(sg):
 
 
 def parse_tasks(blob):
-    """Per tier: (tier, [(lane_begin[33], steps, shuffle counts per step)], entries, pull list, raw bytes)."""
+    """Per tier: (tier, [(lane_begin[33], steps, shuffle counts per step, turn-around lane mask)], entries, pull list, raw bytes)."""
     ntier = int(blob[0])
     tb = blob[1:2 + ntier]
     grp_off = -(-(2 + ntier) // 4) * 4
@@ -49,7 +49,7 @@ def parse_tasks(blob):
         for g in range(int(tb[t]), int(tb[t + 1])):
             gh = blob[grp_off + 36 * g:grp_off + 36 * g + 36]
             nsteps, boff = int(gh[33]), int(gh[34])
-            groups.append((gh[:33], nsteps, raw[boff:boff + nsteps]))
+            groups.append((gh[:33], nsteps, raw[boff:boff + nsteps], int(gh[35]) & 0xffffffff))
         out.append((t, groups, ents, pull, raw))
     return out
 
@@ -123,8 +123,11 @@ def solve_with_tables(plan, m, d, u, b):
         assert len(pn) == NN
         blob = task_blob[task_off[it]:task_off[it + 1]]
         done = np.zeros(NN, bool)
-        for tier, groups, ents, pull, nshb in parse_tasks(blob):
-            for gh, nsteps, nsh in groups:
+        final = np.zeros(NN, bool)
+        tiers = parse_tasks(blob)
+        any_turn = any(g_[3] for t_ in tiers for g_ in t_[1])      # all root chains of an item turn around, or none
+        for tier, groups, ents, pull, nshb in tiers:
+            for gh, nsteps, nsh, turn in groups:
                 outd = np.zeros(32); outb = np.zeros(32)
                 pos = [int(gh[l]) for l in range(32)]
                 for h in range(nsteps):
@@ -168,11 +171,26 @@ def solve_with_tables(plan, m, d, u, b):
                                 pd[node], pb[node] = newd[lane], newb[lane]       # hand-off slot
                     outd, outb = newd, newb
                 assert all(pos[l] == gh[l + 1] for l in range(32))
+                # a chain that ended in a root turns around: x_root = c_root, x = c - f x_parent down the lane's chain
+                for l in range(32):
+                    b_, e_ = int(gh[l]), int(gh[l + 1])
+                    if (turn >> l) & 1:
+                        assert e_ > b_ and rU[e_ - 1] == 0, "turn-around lane does not end in a root"
+                        xv = rB[e_ - 1]
+                        rD[e_ - 1] = 0.0
+                        final[e_ - 1] = True
+                        for k in range(e_ - 2, b_ - 1, -1):
+                            xv = rB[k] - rD[k] * xv
+                            rD[k], rB[k] = 0.0, xv
+                            final[k] = True
+                    elif e_ > b_ and any_turn:
+                        assert pn[e_ - 1] != e_ - 1, "a chain that ends in a root must turn around"
         assert done.all()
         # forward sweep by pointer jumping: x_v = c_v + g_v x_p(v), g = -f (a root: g = 0, p = itself)
         real = ~np.isnan(rD)
         g = np.where(real, -rD, 0.0); c = np.where(real, rB, 0.0); par = pn.astype(np.int64).copy()
         assert (par[~real] == np.nonzero(~real)[0]).all() and real[par[real]].all()
+        assert (par[final] == np.nonzero(final)[0]).all(), "a final node reads itself"
         for _ in range(int(rounds[it])):
             g, c, par = g * g[par], c + g * c[par], par[par]
         assert (g[real] == 0).all(), "not enough pointer-jumping rounds"

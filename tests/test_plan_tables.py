@@ -135,7 +135,23 @@ def _check_policy(m, plan, max_segment=0):
         assert nch == cls_cluster[cls[it]] and (nch == 1 or c1 - c0 == 1)
         cr = ch_rng[ch_off[it]:ch_off[it + 1]]
         assert cr[0, 0] == comp0 and cr[-1, 1] == comp0 + n_it and (cr[1:, 0] == cr[:-1, 1]).all()
-        pn = pnode[node_off[it]:node_off[it + 1]]
+        pn_sweep = pnode[node_off[it]:node_off[it + 1]]
+        # ITEM_PNODE is the parent the FORWARD sweep reads: a node of a lane chain that ends in a root is final
+        # after the backward sweep's turn-around and reads itself.  pn = the parent in the reduced tree: for those
+        # nodes the next entry of the lane's chain (node id = entry index).
+        pn = pn_sweep.copy()
+        blob_ = plan.table("item_task_blob")[plan.table("item_task_offsets")[it]:plan.table("item_task_offsets")[it + 1]]
+        tiers_ = parse_tasks(blob_)
+        any_turn = any(g_[3] for t_ in tiers_ for g_ in t_[1])     # all root chains of an item turn around, or none
+        for _t, groups_, _e, _p, _r in tiers_:
+            for gh_, _ns, _nsh, turn_ in groups_:
+                for l_ in range(32):
+                    b_, e_ = int(gh_[l_]), int(gh_[l_ + 1])
+                    if (turn_ >> l_) & 1:
+                        assert e_ > b_ and (pn_sweep[b_:e_] == np.arange(b_, e_)).all()
+                        pn[b_:e_ - 1] = np.arange(b_ + 1, e_)
+                    elif e_ > b_ and any_turn:
+                        assert pn_sweep[e_ - 1] != e_ - 1          # a chain that ends in a root turns around
         assert len(pn) == nnode[it]
         # segments of all chunks -> node of every separator compartment (item-local position)
         node_at = {}                     # separator position -> node
@@ -196,7 +212,7 @@ def _check_policy(m, plan, max_segment=0):
         blob = plan.table("item_task_blob")[plan.table("item_task_offsets")[it]:plan.table("item_task_offsets")[it + 1]]
         where = {}
         for tier, groups, ents, pull, raw in parse_tasks(blob):
-            for gi, (gh, nsteps, nsh) in enumerate(groups):
+            for gi, (gh, nsteps, nsh, _turn) in enumerate(groups):
                 for lane in range(32):
                     prev = None
                     for k in range(int(gh[lane]), int(gh[lane + 1])):
