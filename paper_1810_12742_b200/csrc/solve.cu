@@ -467,8 +467,17 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
                         const int begin = gh[lane];
                         uint32_t qk = nd_sa + (uint32_t)(end - 1) * RS;
                         T xv = lds1<T>(qk + W);
-#pragma unroll 4
-                        for (int k = end - 2; k >= begin; --k) {
+                        int k = end - 2;
+                        for (; k - 3 >= begin; k -= 4) {                // four records in flight under one chain
+                            const V2 g0 = lds2<T>(qk - RS), g1 = lds2<T>(qk - 2u * RS), g2 = lds2<T>(qk - 3u * RS), g3 = lds2<T>(qk - 4u * RS);
+                            V2 o; o.x = T(0);
+                            xv = fmad<T>(g0.x, xv, g0.y); o.y = xv; sts2<T>(qk - RS, o);
+                            xv = fmad<T>(g1.x, xv, g1.y); o.y = xv; sts2<T>(qk - 2u * RS, o);
+                            xv = fmad<T>(g2.x, xv, g2.y); o.y = xv; sts2<T>(qk - 3u * RS, o);
+                            xv = fmad<T>(g3.x, xv, g3.y); o.y = xv; sts2<T>(qk - 4u * RS, o);
+                            qk -= 4u * RS;
+                        }
+                        for (; k >= begin; --k) {
                             qk -= RS;
                             const V2 gc = lds2<T>(qk);
                             xv = fmad<T>(gc.x, xv, gc.y);
