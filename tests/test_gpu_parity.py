@@ -85,6 +85,17 @@ def test_cluster_path(kw, dtype):
     assert info.n_cluster_cells > 0 and info.n_chunks > info.n_resident_items
 
 
+@pytest.mark.parametrize("max_segment", [0, 2, 7, 48, 64, 200, 1023])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_long_cables_segment_targets(max_segment, dtype):
+    """Unbranched cables cut into 1..500 segments: odd segment lengths, late-starting lanes, the tight run loop of
+    the backward sweep and the turn-around at the root in place of the pointer-jumping rounds."""
+    m = mg.make_config(1, 0.002)
+    d, u, b = mg.system(m)
+    _, info = _check(m, d, u, b, dtype, max_segment=max_segment)
+    assert info.n_resident_items > 0 and info.n_stream_cells == 0
+
+
 def _edge_morphology():
     star = np.array([-1] + [0] * 70, np.int32)            # 70 siblings: hand-off spans tiles (atomic path)
     ps = [np.array([-1], np.int32), star, random_parent(33, 1), np.array([-1], np.int32),
