@@ -23,7 +23,10 @@
  *
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): dense LAPACK solve on every tree with
  * n <= 7 and on random trees; scipy banded solver and the constant-coefficient closed form on
- * cables; star-tree closed form; residual; x = 1 for b = A 1; M-matrix invariants.
+ * cables; star-tree closed form; residual; x = 1 for b = A 1; M-matrix invariants; oracle_rel_err
+ * against a numpy per-cell max-norm (NaN at the first / middle / last element of a cell, zero
+ * reference); oracle_hines_solve_range bit-equal to oracle_hines_solve over splits of the cells and
+ * against dense solves; oracle_pivots against Schur complements from dense inverses.
  */
 #include <stdint.h>
 #include <stddef.h>
@@ -138,7 +141,9 @@ void oracle_pivots(int64_t ncells, const int64_t* cell_offsets, const int32_t* p
     }
 }
 
-/* per cell relative max-norm error  ||xa - xb||_inf / ||xb||_inf  (reading S15). */
+/* per cell relative max-norm error  ||xa - xb||_inf / ||xb||_inf  (reading S15); the absolute error
+ * where xb is identically zero.  A NaN anywhere in a cell's xa (or xb) makes that cell's error NaN, and
+ * only that cell's.  Pinned by tests/test_oracle_solve.py against numpy, cell by cell. */
 void oracle_rel_err(int64_t ncells, const int64_t* cell_offsets, const double* xa,
                     const double* xb, double* err)
 {
@@ -146,7 +151,7 @@ void oracle_rel_err(int64_t ncells, const int64_t* cell_offsets, const double* x
         double e = 0.0, nrm = 0.0;
         for (int64_t i = cell_offsets[c]; i < cell_offsets[c + 1]; ++i) {
             double t = fabs(xa[i] - xb[i]);
-            if (!(t <= e)) e = t;            /* NaN-propagating max */
+            if (t != t || (e == e && t > e)) e = t;   /* NaN-sticky max: once NaN, stays NaN */
             double a = fabs(xb[i]); if (a > nrm) nrm = a;
         }
         err[c] = (nrm > 0.0) ? e / nrm : e;

@@ -124,6 +124,7 @@ def test_in_place_and_nan_poisoned_root_u():
     for kw in ({}, dict(policy_flags=1)):
         x1, _ = _gpu_solve(m, d, u2, b, inplace=True, **kw)
         xr = oracle.hines_solve(m.parent, m.cell_offsets, d, u, b)
+        assert np.isfinite(x1).all()
         assert oracle.rel_err(m.cell_offsets, x1, xr).max() < 1e-10
     assert np.array_equal(x0, _gpu_solve(m, d, u, b)[0])     # run-to-run deterministic
 
@@ -179,5 +180,7 @@ def test_config4_fresh_rhs_steps():
         b = mg.rhs(m, step=step)
         plan.solve(dd, du, torch.from_numpy(b).cuda(), x)
         xr = oracle.hines_solve(m.parent, m.cell_offsets, d, u, b)
-        assert oracle.rel_err(m.cell_offsets, x.cpu().numpy(), xr).max() < 1e-10
+        xg = x.cpu().numpy()
+        assert np.isfinite(xg).all()
+        assert oracle.rel_err(m.cell_offsets, xg, xr).max() < 1e-10
     plan.close()

@@ -223,3 +223,94 @@ def test_linearity_and_renumbering():
     perm, p_new = dfs_renumber(p)
     x_new = _solve1(p_new, d[perm], np.where(np.arange(len(p)) == 0, 0.0, u[perm]), b[perm])
     np.testing.assert_allclose(x_new, x1[perm], rtol=0, atol=1e-14)
+
+
+# ---- the parity metric itself (reading S15) and the range entry: pinned against numpy, not against themselves ----
+def _rel_err_numpy(offs, xa, xb):
+    out = np.empty(len(offs) - 1)
+    for c in range(len(offs) - 1):
+        a, b_ = xa[offs[c]:offs[c + 1]], xb[offs[c]:offs[c + 1]]
+        diff = np.abs(a - b_)
+        e = np.nan if np.isnan(diff).any() else diff.max()
+        nrm = np.abs(b_).max()
+        out[c] = e / nrm if nrm > 0 else e
+    return out
+
+
+def test_rel_err_matches_numpy_per_cell():
+    offs = np.array([0, 3, 4, 10, 210, 211], np.int64)
+    r = mg.rng.uniform(5, 91, np.arange(2 * offs[-1], dtype=np.uint64), -2.0, 2.0)
+    xb = r[:offs[-1]].copy()
+    xa = xb + 1e-9 * r[offs[-1]:]
+    err = oracle.rel_err(offs, xa, xb)
+    np.testing.assert_allclose(err, _rel_err_numpy(offs, xa, xb), rtol=1e-15, atol=0)
+    assert err.shape == (5,) and (err > 0).all()
+    # the value is the per-cell ratio, not a global one: scaling one cell's reference scales only that cell's error
+    xb2, xa2 = xb.copy(), xa.copy()
+    xb2[3:4] *= 1e6; xa2[3:4] = xb2[3:4] + (xa[3:4] - xb[3:4])
+    err2 = oracle.rel_err(offs, xa2, xb2)
+    assert err2[1] == pytest.approx(err[1] * 1e-6, rel=1e-6) and np.array_equal(np.delete(err2, 1), np.delete(err, 1))
+
+
+@pytest.mark.parametrize("pos", ["first", "middle", "last"])
+def test_rel_err_nan_is_sticky_and_local(pos):
+    """A NaN at any position of a cell gives NaN for that cell and only for that cell (the round-1 checker
+    let a later finite element overwrite it)."""
+    offs = np.array([0, 3, 8, 11], np.int64)
+    xb = np.array([1, 2, 4, 0.5, 2, 3, 1, 1, 7, 8, 9], np.float64)
+    xa = xb + 1e-3
+    k = {"first": 3, "middle": 5, "last": 7}[pos]
+    xa[k] = np.nan
+    err = oracle.rel_err(offs, xa, xb)
+    assert np.isnan(err[1]) and np.isfinite(err[0]) and np.isfinite(err[2])
+    np.testing.assert_allclose(err[[0, 2]], [1e-3 / 4, 1e-3 / 9], rtol=1e-12)
+    # the probe of VERDICT.md round 1: an isolated NaN followed by finite elements
+    e2 = oracle.rel_err(np.array([0, 3, 5], np.int64), np.array([1, np.nan, 3, 0, 0.0]), np.array([1, 2, 4, 0, 1e-3]))
+    assert np.isnan(e2[0]) and e2[1] == 1.0
+    # NaN in the reference is not hidden either
+    e3 = oracle.rel_err(np.array([0, 2], np.int64), np.array([1.0, 2.0]), np.array([np.nan, 2.0]))
+    assert np.isnan(e3[0])
+
+
+def test_rel_err_zero_reference_is_absolute():
+    offs = np.array([0, 2, 4], np.int64)
+    err = oracle.rel_err(offs, np.array([1e-3, -2e-3, 1.0, 1.0]), np.array([0.0, 0.0, 1.0, 1.0]))
+    assert err[0] == 2e-3 and err[1] == 0.0
+
+
+def test_solve_range_equals_dense_and_full_solve():
+    """hines_solve_range over any split of the cells: bit-equal to hines_solve, and each range on its own equal to
+    dense solves of its cells; cells outside the range are not touched."""
+    ps = [random_parent(n, 30 + n, 0.6) for n in (1, 17, 40, 5, 64, 2, 33)]
+    offs = np.concatenate([[0], np.cumsum([len(p) for p in ps])]).astype(np.int64)
+    m, d, u, b = system_for(np.concatenate(ps), seed=21, cell_offsets=offs)
+    x_full = oracle.hines_solve(m.parent, offs, d, u, b)
+    par = np.ascontiguousarray(m.parent, np.int32)
+    for cuts in ([0, 7], [0, 3, 7], [0, 1, 2, 6, 7], [0, 5, 5, 7]):
+        x = np.full(m.n, -77.0); dw = np.empty(m.n)
+        for c0, c1 in zip(cuts[:-1], cuts[1:]):
+            before = x.copy()
+            oracle.hines_solve_range(c0, c1, par, offs, d, u, b, x, dw)
+            untouched = np.ones(m.n, bool); untouched[offs[c0]:offs[c1]] = False
+            assert np.array_equal(x[untouched], before[untouched])
+        assert np.array_equal(x, x_full)
+    for c in range(len(ps)):
+        A = dense_from_hines(ps[c], d[offs[c]:offs[c + 1]], u[offs[c]:offs[c + 1]])
+        np.testing.assert_allclose(x_full[offs[c]:offs[c + 1]], np.linalg.solve(A, b[offs[c]:offs[c + 1]]), rtol=0, atol=2e-15)
+
+
+def test_pivots_equal_schur_complements():
+    """oracle_pivots: d'[i] is the Schur complement of the sub-tree below i onto i, i.e. 1 / [A_sub^-1]_{ii} for
+    the principal sub-matrix of i and its descendants (dense inverse), not only the inequalities I1/I2."""
+    p = random_parent(40, 3, 0.5)
+    m, d, u, _ = system_for(p, seed=4)
+    dw = oracle.pivots(m.parent, m.cell_offsets, d, u)
+    A = dense_from_hines(p, d, u)
+    n = len(p)
+    desc = [[i] for i in range(n)]
+    for i in range(n - 1, 0, -1):
+        desc[p[i]] += desc[i]
+    for i in range(n):
+        idx = sorted(desc[i])
+        S = np.linalg.inv(A[np.ix_(idx, idx)])
+        assert dw[i] == pytest.approx(1.0 / S[idx.index(i), idx.index(i)], rel=1e-13)
