@@ -375,7 +375,7 @@ def main():
                    "cells_per_gpu": m.ncells, "branches_per_gpu": info.nbranches, "max_levels": info.max_levels,
                    "parallelism": f"independent cells, {world} replica(s), no collective",
                    "l2": "inputs_exceed_l2" if r["nsets"] == 1 else f"rotating {r['nsets']} distinct buffer sets (> 2x L2)",
-                   "resident_items": info.n_resident_items, "resident_blocks": info.n_chunks,
+                   "resident_items": info.n_resident_items, "resident_blocks": info.n_blocks,
                    "resident_unknowns": info.n_resident_unknowns, "cluster_cells": info.n_cluster_cells,
                    "cluster_unknowns": info.n_cluster_unknowns, "cluster_sizes_per_class": r["classes"],
                    "stream_cells": info.n_stream_cells, "stream_unknowns": info.n_stream_unknowns,

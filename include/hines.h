@@ -60,8 +60,17 @@ enum {
                                         of concurrently on plan-owned side streams (forked from / joined to it)  */
     HINES_POLICY_POW2_CLUSTERS = 32, /* cluster sizes 2, 4, 8, 16 only (default: any size up to cluster_max, the one
                                         whose blocks fill their shared-memory slot best)                     */
-    HINES_POLICY_NO_CLUSTER   = 8    /* never spread a cell over a thread-block cluster: a cell either fits one
-                                        block's shared memory or goes to the streaming path               */
+    HINES_POLICY_NO_CLUSTER   = 8,   /* never cut a cell into parts: a cell either fits one block's shared memory
+                                        or goes to the streaming path                                     */
+    HINES_POLICY_NO_PCR       = 256, /* unbranched cables: the reduced chains go through the level sweeps like every other tree,
+                                        not through parallel cyclic reduction                                          */
+    HINES_POLICY_NO_SPLIT     = 64,  /* no split items: a cell that fits no cluster goes to the streaming path  */
+    HINES_POLICY_SPLIT_LEVEL_MEAN = 128 /* f1: cut branches by the paper's own rule first (level by
+                                        level from the root, over all cells of the batch, a branch longer than
+                                        c = ceil(mean length on the level) is cut into a head of c compartments and
+                                        a rest that moves, with the branch's children, one level down); every piece is
+                                        then still bounded by max_segment (set max_segment = 1023 for the paper's rule
+                                        alone).  Tables HINES_TABLE_SPLIT_* hold the pieces with or without the flag  */
 };
 
 typedef struct {
@@ -86,6 +95,8 @@ typedef struct {
     int32_t chunk_smem_bytes;       /* 0 = default (113 KiB, two blocks per SM): shared memory one block of a
                                        cluster item aims to stay within; also the size above which a cell is
                                        spread over a cluster instead of taking a whole SM's shared memory      */
+    int32_t split_smem_bytes;       /* 0 = default (113 KiB): shared memory of one sub-tree part of a split item
+                                       (a cell beyond the largest cluster, run as three dependent launches)     */
 } hines_options_t;
 
 typedef struct {
@@ -112,7 +123,11 @@ typedef struct {
     int32_t n_classes;          /* size classes in use = resident kernel launches per solve                */
     int64_t n_cluster_cells;    /* cells spread over a thread-block cluster (counted in n_resident_* too)  */
     int64_t n_cluster_unknowns;
-    int64_t n_chunks;           /* blocks the resident launches start per solve                            */
+    int64_t n_parts;            /* parts (= blocks' worth of shared memory) of all on-chip items           */
+    int64_t n_split_cells;      /* cells run as split items: three dependent launches (counted in n_resident_* too) */
+    int64_t n_split_unknowns;
+    int64_t n_exports;          /* sub-tree roots that hand their value to another part (cluster + split items)    */
+    int64_t n_blocks;           /* blocks the resident launches start per solve (split sub-tree parts count twice) */
 } hines_plan_info_t;
 
 /* Canonical, policy-free tables (bit-exact against the table oracle); all indices cell-local.
@@ -130,53 +145,62 @@ typedef enum {
     HINES_TABLE_LEVEL_LIST           = 9,   /* int32[nbranches]  per cell: ids by (level, length desc, id)  */
     HINES_TABLE_CHILD_OFFSETS        = 10,  /* int64[nbranches+1] CSR over global branch index              */
     HINES_TABLE_CHILD_IDS            = 11,  /* int32[nbranches-ncells] ascending                            */
-    /* Policy tables (depend on options; validity-checked in tests).
-     * A work item is a run of whole cells in ONE block's shared memory, or one cell cut into the chunks
-     * of a thread-block cluster.  Its reduced tree has one node per segment (the segment's last
-     * compartment, the "separator"); node ids are item-local, in the order of the backward sweep's
-     * entries (ITEM_TASK_BLOB). */
+    /* Policy tables (depend on options; validity-checked in tests and executed
+     * lane by lane on the CPU by tests/plan_interpreter.py).  A PART is what one block stages into its shared
+     * memory: whole branches, as runs of consecutive compartments.  A work item is one part (a run of whole
+     * cells), or one cell cut into a top part (the root region) and parts that are unions of complete
+     * sub-trees (cluster item: one part per block of a thread-block cluster; split item: three launches).
+     * A part's reduced forest has one node per segment (the segment's last compartment, the "separator");
+     * node ids are part-local. */
     HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  on-chip work item of the cell, -1 = streaming path       */
     HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
     HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  size class                                              */
     HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
-    HINES_TABLE_ITEM_PNODE           = 44,  /* int32[sum nnode] per node: the node the FORWARD sweep reads = the node above it
-                                               in the reduced tree; itself for a root, and for every node of a lane chain
-                                               that turns around at a root (ITEM_TASK_BLOB): those are final before the
-                                               pointer jumping starts                                                   */
-    HINES_TABLE_ITEM_NODE_OFFSETS    = 52,  /* int64[nitems+1] into ITEM_PNODE                                          */
-    HINES_TABLE_ITEM_ROUNDS          = 53,  /* int32[nitems] pointer-jumping rounds of the forward sweep: 2^rounds > the
-                                               largest distance of a node to the nearest node that reads itself (0 rounds
-                                               when every chain turns around, e.g. unbranched cables)                   */
-    HINES_TABLE_ITEM_NNODE           = 45,  /* int32[nitems] nodes of the reduced tree (>= lanes)                          */
-    HINES_TABLE_ITEM_CHUNK_OFFSETS   = 46,  /* int64[nitems+1] into the chunk tables; chunks of an item = cluster size  */
-    HINES_TABLE_CHUNK_COMP_RANGE     = 47,  /* int64[2*nchunks] global compartment range [begin, end) of each chunk     */
-    HINES_TABLE_CHUNK_SEG_OFFSETS    = 48,  /* int64[nchunks+1] into CHUNK_SEG (in units of descriptors)                */
-    HINES_TABLE_CHUNK_SEG            = 49,  /* int32[4*nseglanes] two lanes per segment, in groups of 32: lanes 0-15 the
-                                               A halves, lanes 16-31 their B partners (lane ^ 16).  A: {a = first
-                                               compartment (chunk-local), word, node, node of the separator above (-1 =
-                                               none)}; B: {a+mt+1, word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26
-                                               (kind 0 padding, 1 A, 2 B; mt/mb = compartments A / B eliminate, both top-down; the
-                                               middle node q = a+mt exists iff hasq; separator b = a+mt+mb+hasq)        */
+    HINES_TABLE_ITEM_KIND            = 36,  /* int32[nitems]  0 = one part (a run of whole cells in one block), 1 = one cell cut
+                                               into the parts of a thread-block cluster, 2 = split item (three launches)      */
+    HINES_TABLE_ITEM_XCH             = 44,  /* int32[nitems]  first slot of the item in the global exchange buffers (split items)  */
+    HINES_TABLE_ITEM_PART_OFFSETS    = 46,  /* int64[nitems+1] into the part tables; part 0 of a multi-part item is its top part    */
+    HINES_TABLE_PART_HEADER          = 47,  /* int32[32*nparts] the 128-byte device record of each part:
+                                               [0,1] meta_off (int64), [2] meta_len, [3] run_off, [4] nrun, [5] tx_elems, [6] L,
+                                               [7] n, [8] nnode, [9] nlevnode, [10] nlev, [11] rounds, [12] kp_off, [13] exp_off,
+                                               [14] gh_off, [15] seg_off, [16] nexp, [17] nghost, [18] nseg_lanes, [19] xch_base,
+                                               [20] xs0, [21] item, [22] rank, [23] flags, [24] ntoplev, [25] lowlev                */
+    HINES_TABLE_PART_META            = 48,  /* int32[] per part one blob (meta_off, meta_len), every section padded to 4 ints:
+                                               lb[nlev+1]   first node of each local level (level = depth in the cell - smallest
+                                                            depth in the part; level nodes are numbered level by level, the children
+                                                            of a node consecutive, sorted by parent);
+                                               kp[2*nnode]  per node {kids, pnode}: kids = first child | (children << 20), -1 for a
+                                                            ghost child (a stand-in, in part 0, for the root of a sub-tree held by
+                                                            another part: only its hand-off slot is used); pnode = the node the forward
+                                                            sweep reads: the parent, itself for a root / ghost, for an exported sub-tree
+                                                            root the ghost parent (ids >= nlevnode) that receives the parent's x; bit 30 set
+                                                            for a top node (an ancestor of a ghost child: swept after the exchange);
+                                               exps[4*nexp] per exported root {node, ghost child in part 0 (cluster) or exchange slot
+                                                            (split), parent node in part 0, ghost parent};
+                                               ghosts[4*nghost] {ghost child, exchange slot, its parent node, 0};
+                                               seg[4*nseg_lanes] two lanes per segment, in groups of 32: lanes 0-15 the A halves, lanes
+                                                            16-31 their B partners (lane ^ 16).  A: {a = staged index of the first
+                                                            compartment, word, node, node of the separator above (-1 = none)}; B: {a+mt+1,
+                                                            word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26 | delay<<27 (kind 0
+                                                            padding, 1 A, 2 B; mt/mb = compartments A / B eliminate, both top-down; the
+                                                            middle node q = a+mt exists iff hasq; separator b = a+mt+mb+hasq)            */
+    HINES_TABLE_PART_RUNS            = 49,  /* int32[4*nruns] {global first compartment, length, staged index of it, 0}: the runs of
+                                               consecutive compartments a part stages (run_off, nrun in its header)            */
+    HINES_TABLE_CLASS_PHASE          = 52,  /* int32[n_classes] 0 = ordinary; split items: 1 = sub-tree parts, backward sweep + export,
+                                               2 = top parts, 3 = sub-tree parts again: backward sweep, import, forward sweep      */
+    HINES_TABLE_CLASS_FIRST          = 53,  /* int64[n_classes] into CLASS_PARTS                                                */
+    HINES_TABLE_CLASS_COUNT          = 54,  /* int64[n_classes] blocks of the class                                             */
+    HINES_TABLE_CLASS_PARTS          = 55,  /* int32[] part ids in launch order, class by class (the blocks of a cluster item consecutive,
+                                               rank 0 first)                                                                    */
+    HINES_TABLE_SPLIT_PIECE_OFFSETS  = 60,  /* int64[nbranches+1] f1: pieces of every branch under the level-mean rule  */
+    HINES_TABLE_SPLIT_PIECE_LEN      = 61,  /* int32[npieces] compartments of each piece, from the top of the branch             */
+    HINES_TABLE_SPLIT_PIECE_LEVEL    = 62,  /* int32[npieces] level of the piece in the split dependency tree                    */
+    HINES_TABLE_SPLIT_LEVEL_STAT     = 63,  /* int64[2*nsplit_levels] {sum of the piece lengths, pieces} on each level: cut = ceil(sum/count) */
     HINES_TABLE_STREAM_LEVEL_BEGIN   = 40,  /* int64[max_stream_levels+1] into STREAM_DESC                             */
     HINES_TABLE_STREAM_DESC          = 41,  /* int32[6*nstream_branches] {global start, len, global parent compartment
                                                (-1 root), workspace start, child_begin, nchild}                       */
     HINES_TABLE_STREAM_CHILD         = 42,  /* int32[2*nstream_children] {global start, workspace start} of each child */
     HINES_TABLE_CLASS_SMEM_BYTES     = 43,  /* int32[n_classes] dynamic shared memory per block of each class          */
-    HINES_TABLE_ITEM_TASK_OFFSETS    = 54,  /* int64[nitems+1] into ITEM_TASK_BLOB                                         */
-    HINES_TABLE_ITEM_TASK_BLOB       = 55,  /* int32[] per item, the backward sweep of the reduced tree: sub-trees of at
-                                               most 32 leaves, one warp per group of sub-trees, lock-step over the height
-                                               above the leaves, a node in the lane of its first child:
-                                               [ntier, tier_begin (ntier+1), pad4 | groups: 36 ints each = lane_begin[33]
-                                               (entry index), steps, byte offset (in the blob) of the per-step shuffle
-                                               counts, mask of the lanes whose chain ends in a root and turns around
-                                               there (x_root = c_root, then x = c - f x_parent down the lane's chain,
-                                               straight after the backward sweep; all root chains of an item or none:
-                                               only where it saves a pointer-jumping round) | entries: 4 ints per node, by lane then step = {node |
-                                               step<<20, lane mask of the other children in the group, first in the
-                                               pull list, count in the pull list | (entries right behind that continue
-                                               the run with nothing to pull)<<16} | pull list: nodes swept in an earlier
-                                               tier whose hand-off
-                                               slot is added, pad4 | shuffle counts (bytes), pad]                         */
     HINES_TABLE_CLASS_CLUSTER        = 50,  /* int32[n_classes] blocks per item = cluster size (1 = no cluster)        */
     HINES_TABLE_CLASS_THREADS        = 51   /* int32[n_classes] threads per block                                      */
 } hines_table_id_t;

@@ -21,6 +21,10 @@ F64, F32 = 0, 1
 POLICY_DEFAULT, POLICY_FORCE_STREAM, POLICY_NO_GROUPING, POLICY_INPUT_ORDER, POLICY_NO_CLUSTER = 0, 1, 2, 4, 8
 POLICY_SERIAL_CLASSES = 16
 POLICY_POW2_CLUSTERS = 32
+POLICY_NO_SPLIT = 64
+POLICY_SPLIT_LEVEL_MEAN = 128
+POLICY_NO_PCR = 256
+ITEM_SINGLE, ITEM_CLUSTER, ITEM_SPLIT = 0, 1, 2
 
 STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",
           4: "HINES_ERR_CUDA", 5: "HINES_ERR_UNSUPPORTED"}
@@ -32,13 +36,15 @@ TABLES = {
     "cell_nlevels": (6, np.int32), "cell_level_offsets": (7, np.int64), "level_count": (8, np.int32),
     "level_list": (9, np.int32), "child_offsets": (10, np.int64), "child_ids": (11, np.int32),
     "cell_item": (32, np.int32), "item_cell_range": (33, np.int64), "item_class": (34, np.int32),
-    "item_launch_order": (35, np.int32),
+    "item_launch_order": (35, np.int32), "item_kind": (36, np.int32), "item_xch": (44, np.int32),
+    "item_part_offsets": (46, np.int64), "part_header": (47, np.int32), "part_meta": (48, np.int32),
+    "part_runs": (49, np.int32),
     "stream_level_begin": (40, np.int64), "stream_desc": (41, np.int32), "stream_child": (42, np.int32),
-    "class_smem_bytes": (43, np.int32), "item_pnode": (44, np.int32), "item_nnode": (45, np.int32),
-    "item_chunk_offsets": (46, np.int64), "chunk_comp_range": (47, np.int64), "chunk_seg_offsets": (48, np.int64),
-    "chunk_seg": (49, np.int32), "class_cluster": (50, np.int32), "class_threads": (51, np.int32),
-    "item_node_offsets": (52, np.int64), "item_rounds": (53, np.int32),
-    "item_task_offsets": (54, np.int64), "item_task_blob": (55, np.int32),
+    "class_smem_bytes": (43, np.int32), "class_cluster": (50, np.int32), "class_threads": (51, np.int32),
+    "class_phase": (52, np.int32), "class_first": (53, np.int64), "class_count": (54, np.int64),
+    "class_parts": (55, np.int32),
+    "split_piece_offsets": (60, np.int64), "split_piece_len": (61, np.int32), "split_piece_level": (62, np.int32),
+    "split_level_stat": (63, np.int64),
 }
 
 # every symbol include/hines.h declares
@@ -53,7 +59,7 @@ class Options(C.Structure):
     _fields_ = [("struct_size", C.c_int32), ("threads_per_block", C.c_int32),
                 ("smem_bytes_per_block", C.c_int32), ("policy_flags", C.c_int32),
                 ("stream_threads", C.c_int32), ("group_smem_bytes", C.c_int32), ("max_segment", C.c_int32),
-                ("cluster_max", C.c_int32), ("chunk_smem_bytes", C.c_int32)]
+                ("cluster_max", C.c_int32), ("chunk_smem_bytes", C.c_int32), ("split_smem_bytes", C.c_int32)]
 
 
 class PlanInfo(C.Structure):
@@ -65,7 +71,9 @@ class PlanInfo(C.Structure):
                 ("padded_lane_steps", C.c_int64), ("useful_lane_steps", C.c_int64),
                 ("workspace_bytes", C.c_int64), ("bytes_min", C.c_int64), ("bytes_literal", C.c_int64),
                 ("breadth_first", C.c_int32), ("n_classes", C.c_int32),
-                ("n_cluster_cells", C.c_int64), ("n_cluster_unknowns", C.c_int64), ("n_chunks", C.c_int64)]
+                ("n_cluster_cells", C.c_int64), ("n_cluster_unknowns", C.c_int64), ("n_parts", C.c_int64),
+                ("n_split_cells", C.c_int64), ("n_split_unknowns", C.c_int64), ("n_exports", C.c_int64),
+                ("n_blocks", C.c_int64)]
 
 
 class HinesError(RuntimeError):
@@ -130,12 +138,12 @@ class Plan:
 
     def __init__(self, parent, cell_offsets, dtype=F64, threads_per_block=0, smem_bytes_per_block=0,
                  policy_flags=0, stream_threads=0, group_smem_bytes=0, max_segment=0, cluster_max=0,
-                 chunk_smem_bytes=0):
+                 chunk_smem_bytes=0, split_smem_bytes=0):
         lib = load_library()
         parent = np.ascontiguousarray(parent, dtype=np.int32)
         offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
         opt = Options(C.sizeof(Options), threads_per_block, smem_bytes_per_block, policy_flags,
-                      stream_threads, group_smem_bytes, max_segment, cluster_max, chunk_smem_bytes)
+                      stream_threads, group_smem_bytes, max_segment, cluster_max, chunk_smem_bytes, split_smem_bytes)
         h = C.c_void_p()
         self._h = None
         _check(lib.hines_plan_create(parent.ctypes.data, offs.ctypes.data, len(offs) - 1, int(dtype),

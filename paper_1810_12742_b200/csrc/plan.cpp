@@ -10,25 +10,31 @@
 //          ("we assign matrices to a Cuda block as long as ... When a matrix doesn't fit
 //          into a Cuda block any longer, we start a new Cuda block"); the fit test here is bytes of
 //          shared memory instead of "branches per level <= threads", because a B200 block loops over
-//          a level's lane list and is limited by its 227 KB of shared memory, not its thread count.
-//          A cell too large for one block is cut into chunks held by the blocks of one thread-block
-//          cluster (the paper requires one matrix per block; distributed shared memory
-//          lifts that).  Cells that fit no cluster go to the streaming path.
-//   P3     the reduced tree (one node per segment) and its backward sweep: sub-trees of at most 32 leaves,
-//          one warp per group of sub-trees, lock-step over the height above the leaves (PAPER.md:110-112
-//          with height in place of depth), a node in the lane of its first child so that the hand-off at
-//          the branch point stays in registers or is a warp shuffle (build_tasks).
-//   P4     segments.  Every branch is cut, from its end, into nseg = ceil(len / max_segment) segments
-//          of Sj = ceil(len / nseg) compartments (the paper's branch splitting, with a
-//          fixed bound instead of the level average).  The last compartment of a segment is its
-//          separator; the compartments above it are its interior.  Interiors are eliminated
-//          independently of the tree level (one lane per segment, all segments of the item at once),
-//          which leaves the level-synchronous sweeps with one node per segment.  The segment lane list
-//          is ordered so that the 16 (fp64) / 32 (fp32) lanes that access shared memory together start
-//          at different bank residues and have similar lengths.
+//          a level's node list and is limited by its 227 KB of shared memory, not its thread count.
+//          A cell too large for one block is cut into PARTS made of whole branches: a top part (the
+//          root region) and parts that are unions of complete sub-trees, balanced in bytes.  The parts
+//          are held by the blocks of one thread-block cluster (the paper requires one matrix per block,
+//          PAPER.md:114; distributed shared memory lifts that), or, beyond the largest cluster, run as
+//          three dependent launches (sub-trees backward / top / sub-trees forward).  With breadth-first
+//          branch numbering a complete sub-tree is ONE run of consecutive compartments per
+//          level, so a part is a short list of runs, each moved by bulk copies.
+//   P3     the reduced forest of a part (one node per segment), numbered level by level with the children
+//          of a node consecutive: the backward sweep is the paper's level-synchronous sweep
+//          over these nodes, a node pulling its children's hand-off values.
+//   P4     segments.  Every branch is cut, from its end, into nseg = max(1, floor(len / max_segment + 0.4))
+//          segments of ceil(len / nseg) compartments, one more if that is even and nseg > 1 (the paper's
+//          branch splitting, with a fixed bound), or, with HINES_POLICY_SPLIT_LEVEL_MEAN,
+//          first by the paper's own rule (per level, cut what is longer than the level's mean).
+//          The last compartment of a segment is its separator; the compartments above it are its interior.
+//          Interiors are eliminated independently of the tree level (two lanes per segment, all segments of
+//          the part at once), which leaves the level-synchronous sweeps with one node per segment.  The
+//          segment lane list is ordered so that the 16 (fp64) / 32 (fp32) lanes that access shared memory
+//          together start at different bank residues and have similar lengths.
 // Written policy: DESIGN.md "Scheduler policy".
 #include <algorithm>
+#include <cmath>
 #include <cstring>
+#include <memory>
 #include <new>
 #include <numeric>
 #include <string>
@@ -57,39 +63,8 @@ static int64_t class_cap(int k, int64_t max_smem)
     return std::min(cap, max_smem);
 }
 
-// One branch of the item while its lists are built.
-struct Br {
-    int32_t start, len, pc, level, parent;   // item-local positions; parent = index into the item's branch array
-    int32_t nseg, sj;                        // segments, compartments per segment (the first may be shorter)
-    int32_t e = -1, rest = -1;               // lane index (= id of the top node); id of the second node from the top
-};
-
-// Lists of one work item: cells [c0,c1) in nchunks chunks, policies P3 + P4.
-struct ItemBuild {
-    int64_t comp_begin = 0, n = 0;
-    int32_t nlev = 0, ndesc = 0, nnode = 0, nchunks = 1;
-    bool ok = true;                          // false: a field overflows its descriptor bits -> streaming path
-    std::vector<int32_t> pnode;              // 1 per node: the node above it in the reduced tree; itself for a root / an unused id
-    std::vector<int32_t> perm;               // node id used while the lists were built -> final node id (build_tasks)
-    std::vector<int32_t> task_blob;          // device tables of the backward sweep (build_tasks), multiple of 4 ints
-    int32_t ntier = 0, grp_off = 0, ent_off = 0, pull_off = 0, ngroups = 0;
-    std::vector<int32_t> task_entry, task_group, task_pull, task_tier_begin;   // the same, for the table getters
-    std::vector<unsigned char> task_nsh;
-    int32_t rounds = 0;                      // pointer-jumping rounds of the forward sweep: 2^rounds >= nodes on the longest root path
-    struct Chunk {
-        int32_t begin = 0, n = 0;            // item-local compartment range
-        std::vector<int32_t> seg;            // 4 per segment lane {a (chunk-local), m, node, tnode}; node = -1 padding
-        int64_t smem_need = 0;
-    };
-    std::vector<Chunk> chunks;
-    int64_t padded_steps = 0, useful_steps = 0;
-    int64_t leader_extra = 0;                // bytes of the reduced arrays + item metadata (rank 0 only)
-    int64_t smem_need = 0;                   // max over the chunks (rank 0 includes leader_extra)
-    int64_t total_bytes = 0;                 // shared memory of the whole item, all chunks together
-    int32_t max_lanes = 0;                   // widest segment lane list of a chunk
-};
-
 struct SegTmp { int32_t a, m, node, tnode, mt = -1; };   // mt: interior nodes lane A takes (-1: half)
+
 
 // Segment lane list of one chunk.  R = 16 segments share a warp (A lanes 0-15, B lanes 16-31); the lanes of a
 // half-warp access shared memory in one wavefront if, at every step, they sit on distinct residues mod R, and
@@ -165,209 +140,73 @@ static void order_segments(const std::vector<SegTmp>& segs, int R, int NB, int32
     }
 }
 
-// Backward sweep over the reduced tree (policy P3).  The tree is cut into sub-trees of at most 32 leaves;
-// a sub-tree is swept by the lanes of ONE warp in lock-step over the node's height (PAPER.md:110-112 with
-// height above the leaves in place of depth below the root): a node sits in the lane of its first child,
-// so the first child's hand-off value is already in that lane's registers and the other children's values
-// come by warp shuffle from their lanes -- no shared memory and no barrier on the dependent
-// chain.  Sub-trees of a tier are packed into groups of at most 32 lanes (one warp each); what lies above
-// the sub-trees forms the next tier, whose leaves pull the hand-off values of the tier below from shared
-// memory after a block barrier.
-//   group   36 ints: lane_begin[33] (into the item's entries), steps, offset of the per-step shuffle
-//           counts (bytes), pad
-//   entry   4 ints per node, by lane then step: node | step << 20, lanes of the other children in the
-//           same group (bit mask, summed in ascending lane order), first of the pull list, count of the pull
-//           list | (entries behind this one that continue its run with nothing to pull) << 16
-//   pull    node ids whose hand-off slot the node adds (children swept in an earlier tier)
-static void build_tasks(ItemBuild& out, const std::vector<int32_t>& depth)
+// One branch of the item while its lists are built.
+struct Br {
+    int32_t start, len, pc, level, parent;   // item-local positions; parent = index into the item's branch array
+    int32_t nseg = 1;                        // segments (pieces) of the branch
+    int32_t piece0 = 0;                      // first of its piece lengths (top-down) in the item's piece list
+    int32_t node0 = 0;                       // provisional id of its top node: nodes node0 .. node0+nseg-1, top-down
+    int32_t part = 0;
+    int32_t soff = 0;                        // staged (shared-memory) index of its first compartment
+};
+
+// Tables of one part (policies P3 + P4).
+struct PartBuild {
+    std::vector<int32_t> runs;               // 4 per run {item-local first compartment, length, staged index, 0}
+    int32_t L = 0, n = 0, tx_elems = 0;
+    int32_t nnode = 0, nlevnode = 0, nlev = 0, rounds = 0, nexp = 0, nghost = 0, nlanes = 0, flags = 0, ntoplev = 0, lowlev = 0, maxwidth = 0;
+    std::vector<int32_t> lb, kp, exps, ghosts, seg;
+    int64_t smem_need = 0;
+};
+
+// Lists of one work item: cells [c0,c1).
+struct ItemBuild {
+    int64_t comp_begin = 0, n = 0;
+    int32_t kind = kItemSingle;
+    bool ok = true;                          // false: does not fit the descriptor fields / the shared memory -> next option
+    std::vector<PartBuild> parts;
+    int32_t nxch = 0;                        // exchange slots (= exported sub-tree roots)
+    int32_t nnode = 0;
+    int64_t padded_steps = 0, useful_steps = 0;
+    int64_t smem_need = 0;                   // max over the parts (split items: over the sub-tree parts)
+    int64_t smem_top = 0;                    // split items: the top part
+    int64_t total_bytes = 0;                 // estimate of the shared memory of the whole item, all parts together
+    int32_t max_lanes = 0, max_lanes_top = 0;
+};
+
+// Pieces of a branch under the fixed-bound rule (P4), top-down: nseg = max(1, floor(len/S + 0.4)) pieces of
+// ceil(len/nseg) compartments (one more if that is even and nseg > 1), cut from the branch's END, so the
+// first (top) piece takes what is left.
+static void fixed_bound_pieces(int32_t len, int32_t smax, std::vector<int32_t>& out)
 {
-    const int32_t nn = out.nnode;
-    std::vector<std::vector<int32_t>> kids(nn);
-    std::vector<int32_t> order(nn);
-    std::iota(order.begin(), order.end(), 0);
-    std::stable_sort(order.begin(), order.end(), [&](int32_t a, int32_t b) { return depth[a] > depth[b]; });   // deepest first
-    for (int32_t v = 0; v < nn; ++v) if (out.pnode[v] != v) kids[out.pnode[v]].push_back(v);                   // ascending id
-    std::vector<int32_t> tier(nn, -1), leaves(nn), group_of(nn, -1), lane_of(nn, -1), step_of(nn, 0);
-    struct Group { std::vector<int32_t> roots; int32_t lanes = 0, steps = 0; std::vector<std::vector<int32_t>> chain; };
-    std::vector<Group> groups;
-    std::vector<int32_t> tier_begin(1, 0);
-    int32_t remaining = nn;
-    for (int32_t t = 0; remaining > 0; ++t) {
-        if (t >= 64) { out.ok = false; break; }
-        // leaves of the remaining forest below every remaining node
-        for (int32_t v : order) {
-            if (tier[v] >= 0) continue;
-            int32_t l = 0;
-            for (int32_t c : kids[v]) if (tier[c] < 0) l += leaves[c];
-            leaves[v] = l ? l : 1;
-        }
-        // sub-tree roots of this tier: at most 32 leaves, parent (if any) has more
-        std::vector<int32_t> roots;
-        for (int32_t v = 0; v < nn; ++v)
-            if (tier[v] < 0 && leaves[v] <= 32 && (out.pnode[v] == v || leaves[out.pnode[v]] > 32)) roots.push_back(v);
-        // pack into groups (first fit in id order), assign lanes and steps
-        const size_t g0 = groups.size();
-        for (int32_t r : roots) {
-            size_t g = g0;
-            while (g < groups.size() && groups[g].lanes + leaves[r] > 32) ++g;
-            if (g == groups.size()) { groups.push_back(Group()); groups[g].chain.resize(32); }
-            Group& G = groups[g];
-            // iterative DFS: a node takes the lane of its first remaining child, a leaf the next free lane
-            std::vector<std::pair<int32_t, int32_t>> stack(1, {r, 0});      // (node, phase)
-            while (!stack.empty()) {
-                auto [v, ph] = stack.back(); stack.pop_back();
-                if (ph == 0) {
-                    stack.push_back({v, 1});
-                    for (auto it = kids[v].rbegin(); it != kids[v].rend(); ++it) if (tier[*it] < 0) stack.push_back({*it, 0});
-                } else {
-                    int32_t first = -1, h = 0;
-                    for (int32_t c : kids[v]) if (tier[c] < 0) { if (first < 0) first = c; h = std::max(h, step_of[c] + 1); }
-                    // in a sub-tree that is a plain chain (one leaf) every node continues its child's run: same
-                    // step, no shuffle, no pull -- the lane walks the chain without waiting for the lock-step of
-                    // the other lanes (in a branching sub-tree runs would make a step as long as its longest run)
-                    if (leaves[r] == 1 && first >= 0) h = step_of[first];
-                    lane_of[v] = first < 0 ? G.lanes++ : lane_of[first];
-                    step_of[v] = h; group_of[v] = (int32_t)g;
-                    G.chain[lane_of[v]].push_back(v);
-                    G.steps = std::max(G.steps, h + 1);
-                }
-            }
-            G.roots.push_back(r);
-        }
-        // commit the tier (after the DFS, which tests tier[] < 0 for "remaining")
-        for (size_t g = g0; g < groups.size(); ++g)
-            for (auto& ch : groups[g].chain) for (int32_t v : ch) { tier[v] = t; --remaining; }
-        tier_begin.push_back((int32_t)groups.size());
-        if (roots.empty()) { out.ok = false; break; }
-    }
-    if (!out.ok) { out.task_blob.assign(4, 0); return; }
-    // tables
-    out.ntier = (int32_t)tier_begin.size() - 1;
-    out.ngroups = (int32_t)groups.size();
-    out.task_tier_begin = tier_begin;
-    out.task_entry.clear(); out.task_group.clear(); out.task_pull.clear(); out.task_nsh.clear();
-    for (Group& G : groups) {
-        std::vector<unsigned char> nsh(G.steps, 0);
-        const size_t gh = out.task_group.size();
-        out.task_group.resize(gh + 36, 0);
-        for (int32_t l = 0; l < 32; ++l) {
-            out.task_group[gh + l] = (int32_t)(out.task_entry.size() / 4);
-            for (int32_t v : G.chain[l]) {
-                if (step_of[v] >= 4096) out.ok = false;
-                uint32_t mask = 0; int32_t first = -1;
-                const int32_t pull0 = (int32_t)out.task_pull.size();
-                for (int32_t c : kids[v]) {
-                    if (tier[c] == tier[v]) { if (first < 0) first = c; else mask |= 1u << lane_of[c]; }
-                    else out.task_pull.push_back(c);
-                }
-                int32_t pc = 0; for (uint32_t m = mask; m; m &= m - 1) ++pc;
-                nsh[step_of[v]] = std::max<unsigned char>(nsh[step_of[v]], (unsigned char)pc);
-                const int32_t npull = (int32_t)out.task_pull.size() - pull0;
-                if (npull > 0xffff) out.ok = false;
-                out.task_entry.insert(out.task_entry.end(), {v | (step_of[v] << 20), (int32_t)mask, pull0, npull});
-            }
-            // upper half of the last word: how many entries right behind this one continue its run with
-            // nothing to pull (same step, only child = the node before): the kernel walks those in a tight loop
-            const size_t e0 = (size_t)out.task_group[gh + l], e1 = out.task_entry.size() / 4;
-            int32_t more = 0;
-            for (size_t k = e1; k-- > e0;) {
-                out.task_entry[4 * k + 3] |= std::min(more, 0xffff) << 16;
-                const bool plain = (out.task_entry[4 * k + 3] & 0xffff) == 0 && k > e0 &&
-                                   (out.task_entry[4 * k] >> 20) == (out.task_entry[4 * (k - 1)] >> 20);
-                more = plain ? more + 1 : 0;
-            }
-        }
-        out.task_group[gh + 32] = (int32_t)(out.task_entry.size() / 4);
-        out.task_group[gh + 33] = G.steps;
-        out.task_group[gh + 34] = (int32_t)out.task_nsh.size();      // byte offset, made absolute below
-        out.task_nsh.insert(out.task_nsh.end(), nsh.begin(), nsh.end());
-    }
-    // Renumber the nodes in entry order (group, lane, position in the lane's chain): the records of a lane's
-    // chain are then consecutive in shared memory, so the address of the lane's next record does not wait for
-    // a descriptor.  From here on node id = entry index.
-    out.perm.assign(nn, -1);
-    for (size_t k = 0; k < out.task_entry.size() / 4; ++k) out.perm[out.task_entry[4 * k] & 0xfffff] = (int32_t)k;
-    for (int32_t v = 0; v < nn; ++v) if (out.perm[v] < 0) { out.ok = false; out.task_blob.assign(4, 0); return; }
-    for (size_t k = 0; k < out.task_entry.size() / 4; ++k)
-        out.task_entry[4 * k] = (int32_t)k | (out.task_entry[4 * k] & ~0xfffff);
-    for (int32_t& c : out.task_pull) c = out.perm[c];
-    {
-        std::vector<int32_t> np(nn);
-        for (int32_t v = 0; v < nn; ++v) np[out.perm[v]] = out.perm[out.pnode[v]];
-        out.pnode.swap(np);
-    }
-    // A lane whose chain ends in a root turns around there: x_root = c_root, then x = c - f x_parent down its own
-    // chain, straight after the backward sweep (group word 35 = mask of such lanes).  Those nodes are final before
-    // the pointer jumping starts and read themselves in it; the rounds follow from the distance of the other nodes
-    // to their nearest final ancestor (2^rounds > distance; none left: no round at all, e.g. unbranched cables).
-    {
-        std::vector<char> fin(nn, 0);
-        for (int32_t g = 0; g < out.ngroups; ++g) {
-            int32_t* gh = &out.task_group[36 * (size_t)g];
-            uint32_t mask = 0;
-            for (int32_t l = 0; l < 32; ++l) {
-                const int32_t b = gh[l], e = gh[l + 1];
-                if (e > b && out.pnode[e - 1] == e - 1) { mask |= 1u << l; for (int32_t k = b; k < e; ++k) fin[k] = 1; }
-            }
-            gh[35] = (int32_t)mask;
-        }
-        std::vector<int32_t> byd(nn), dnew(nn), dist(nn, 0);
-        for (int32_t v = 0; v < nn; ++v) dnew[out.perm[v]] = depth[v];
-        std::iota(byd.begin(), byd.end(), 0);
-        std::stable_sort(byd.begin(), byd.end(), [&](int32_t a, int32_t b) { return dnew[a] < dnew[b]; });   // parents first
-        auto rounds_for = [&](bool turn) {
-            int32_t maxdist = 0;
-            for (int32_t v : byd) {
-                const bool f = turn ? fin[v] != 0 : out.pnode[v] == v;
-                dist[v] = f ? 0 : dist[out.pnode[v]] + 1;
-                maxdist = std::max(maxdist, dist[v]);
-            }
-            int32_t r = 0;
-            while ((1 << r) <= maxdist) ++r;
-            return r;
-        };
-        // the turn-around lengthens the backward sweep by the root chains: taken only where it saves a round
-        const int32_t r_plain = rounds_for(false), r_turn = rounds_for(true);
-        if (r_turn < r_plain) {
-            out.rounds = r_turn;
-            for (int32_t v = 0; v < nn; ++v) if (fin[v]) out.pnode[v] = v;
-        } else {
-            out.rounds = r_plain;
-            for (int32_t g = 0; g < out.ngroups; ++g) out.task_group[36 * (size_t)g + 35] = 0;
-        }
-    }
-    // blob: [ntier, tier_begin (ntier+1), pad4 | groups | entries | pull, pad4 | shuffle counts, pad4]
-    std::vector<int32_t>& B = out.task_blob;
-    B.clear();
-    B.push_back(out.ntier);
-    B.insert(B.end(), tier_begin.begin(), tier_begin.end());
-    B.resize(round_up((int64_t)B.size(), 4), 0);
-    out.grp_off = (int32_t)B.size();
-    B.insert(B.end(), out.task_group.begin(), out.task_group.end());
-    out.ent_off = (int32_t)B.size();
-    B.insert(B.end(), out.task_entry.begin(), out.task_entry.end());
-    out.pull_off = (int32_t)B.size();
-    B.insert(B.end(), out.task_pull.begin(), out.task_pull.end());
-    B.resize(round_up((int64_t)B.size(), 4), 0);
-    const int32_t nsh_off = (int32_t)B.size();
-    B.resize(B.size() + round_up((int64_t)out.task_nsh.size(), 16) / 4, 0);
-    if (!out.task_nsh.empty()) std::memcpy(&B[nsh_off], out.task_nsh.data(), out.task_nsh.size());
-    for (int32_t g = 0; g < out.ngroups; ++g) B[out.grp_off + 36 * g + 34] += nsh_off * 4;     // byte offset inside the blob
+    int32_t nseg = std::max<int32_t>(1, (int32_t)((5 * (int64_t)len + 2 * smax) / (5 * (int64_t)smax)));   // len/smax + 0.4, cut off
+    int32_t sj = (len + nseg - 1) / nseg;
+    if (nseg > 1 && sj % 2 == 0) ++sj;       // odd: the segments of one branch start on distinct banks
+    nseg = (len + sj - 1) / sj;              // no empty segment
+    out.push_back(len - (nseg - 1) * sj);
+    for (int32_t k = 1; k < nseg; ++k) out.push_back(sj);
 }
 
-static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchunks, ItemBuild& out)
+struct NodeTmp { int32_t depth, pkey, gid, ghost; };
+
+// kind = single: cells [c0,c1) in one part.  kind = cluster: ONE cell in K parts, part 0 = top + sub-trees.
+// kind = split: ONE cell, part 0 = top alone, the sub-trees packed into parts of at most `slot` bytes (K is
+// then the result).
+static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t kind, int32_t K, int64_t slot, ItemBuild& out)
 {
-    const int32_t smax = nchunks > 1 ? P.seg_cluster : P.seg_single;
-    const int E = 16 / P.width;
+    const int32_t w = P.width, E = 16 / w;
+    const int32_t smax = kind == kItemSingle ? P.seg_single : P.seg_cluster;
+    const bool level_mean = (P.opt.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN) != 0;
     out = ItemBuild();
-    out.nchunks = nchunks;
+    out.kind = kind;
     out.comp_begin = P.cell_offsets[c0];
     out.n = P.cell_offsets[c1] - out.comp_begin;
-    for (int64_t c = c0; c < c1; ++c) out.nlev = std::max(out.nlev, P.cell_nlevels[c]);
     const int64_t B0 = P.cell_branch_offsets[c0];
     const int32_t nb = (int32_t)(P.cell_branch_offsets[c1] - B0);
     std::vector<Br> br(nb);
-    std::vector<std::vector<int32_t>> lv(out.nlev);
+    std::vector<int32_t> pieces;
+    pieces.reserve(nb + nb / 4);
+    int32_t nn = 0;
     for (int64_t c = c0; c < c1; ++c) {
         const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
         const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
@@ -378,133 +217,272 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
             e.level = P.branch_level[j];
             e.parent = P.branch_parent_branch[j] < 0 ? -1 : (int32_t)(b0 + P.branch_parent_branch[j] - B0);
-            e.nseg = std::max<int32_t>(1, (int32_t)((5 * (int64_t)e.len + 2 * smax) / (5 * (int64_t)smax)));   // len/smax + 0.4, cut off
-            e.sj = (e.len + e.nseg - 1) / e.nseg;
-            if (e.nseg > 1 && e.sj % 2 == 0) ++e.sj;        // odd: the segments of one branch start on distinct banks
-            e.nseg = (e.len + e.sj - 1) / e.sj;             // no empty segment
+            e.piece0 = (int32_t)pieces.size();
+            if (level_mean) {                           // the paper's pieces first, each then bounded
+                for (int64_t q = P.split_piece_offsets[j]; q < P.split_piece_offsets[j + 1]; ++q)
+                    fixed_bound_pieces(P.split_piece_len[q], smax, pieces);
+            } else {
+                fixed_bound_pieces(e.len, smax, pieces);
+            }
+            e.nseg = (int32_t)pieces.size() - e.piece0;
             if (e.nseg > 0xffff) out.ok = false;
-            lv[e.level].push_back((int32_t)(j - B0));
+            e.node0 = nn;
+            nn += e.nseg;
         }
     }
-    // ---- P3: nodes of the reduced tree ----------------------------------------------------------
-    // Branches level by level, siblings contiguous, sibling groups by their longest member in segments,
-    // descending, ties by (cell, branch id): the provisional node numbering from which
-    // build_tasks derives the sweep (and the final numbering).
-    std::vector<int32_t> lane_br;                       // branch of every lane, -1 = padding
-    struct Group { int32_t first, count, maxseg, minord; };
-    std::vector<Group> groups;
-    for (int32_t l = 0; l < out.nlev; ++l) {
-        auto& v = lv[l];
-        auto key = [&](int32_t i) { return br[i].parent >= 0 ? (int64_t)br[i].parent : -(int64_t)i - 1; };
-        std::sort(v.begin(), v.end(), [&](int32_t a, int32_t b) {
-            if (key(a) != key(b)) return key(a) < key(b);
-            if (br[a].nseg != br[b].nseg) return br[a].nseg > br[b].nseg;
-            return a < b;
-        });
-        groups.clear();
-        for (int32_t i = 0; i < (int32_t)v.size();) {
-            int32_t j = i, mo = v[i];
-            while (j < (int32_t)v.size() && key(v[j]) == key(v[i])) { mo = std::min(mo, v[j]); ++j; }
-            groups.push_back({i, j - i, br[v[i]].nseg, mo});
+    out.nnode = nn;
+    if (nn >= (1 << 20)) { out.ok = false; return; }
+    // ---- nodes of the reduced forest: one per segment; (branch, k) -> node0 + k, top-down ------------------
+    std::vector<int32_t> nparent(nn), ndepth(nn), nbr(nn);
+    for (int32_t b = 0; b < nb; ++b) {                  // parents come first (parent_branch < branch)
+        const Br& e = br[b];
+        const int32_t pn = e.parent >= 0 ? br[e.parent].node0 + br[e.parent].nseg - 1 : -1;
+        for (int32_t k = 0; k < e.nseg; ++k) {
+            const int32_t g = e.node0 + k;
+            nparent[g] = k == 0 ? pn : g - 1;
+            ndepth[g] = nparent[g] < 0 ? 0 : ndepth[nparent[g]] + 1;
+            nbr[g] = b;
+        }
+    }
+    // ---- parts ----------------------------------------------------------------------------------------------
+    const int64_t per_node = 6 * w + 32 + 8;            // record + two segment lanes + {kids, parent}
+    std::vector<int64_t> bytes(nb), sub(nb);
+    int64_t total = 0;
+    for (int32_t b = 0; b < nb; ++b) { bytes[b] = 3 * (int64_t)w * br[b].len + per_node * br[b].nseg; total += bytes[b]; }
+    out.total_bytes = total + 1024;
+    int32_t nparts = 1;
+    if (kind != kItemSingle) {
+        // Frontier of sub-trees: walking down from the root, a sub-tree heavier than Tsub gives its root branch
+        // to the top and is replaced by its children's sub-trees.  Frontier roots in branch order (= breadth-first
+        // order: neighbours share runs) are dealt to the parts in sequence, balanced in bytes.
+        sub = bytes;
+        for (int32_t b = nb - 1; b > 0; --b) if (br[b].parent >= 0) sub[br[b].parent] += sub[b];
+        std::vector<int32_t> root_of(nb, -2), best_root, part_of_root(nb, 0), best_part;   // root_of: -2 = top, else its frontier root
+        std::vector<int32_t> frontier;
+        std::vector<int64_t> load;
+        int64_t best_max = -1; int32_t best_nparts = 1;
+        // cluster items: the finer the frontier, the better the parts balance but the heavier the top (all in part 0):
+        // several thresholds are tried and the one with the lightest heaviest part is kept
+        const int ntry = kind == kItemCluster ? 4 : 1;
+        for (int t = 0; t < ntry; ++t) {
+            static const int kNum[4] = {1, 1, 1, 2}, kDen[4] = {4, 3, 2, 3};
+            const int64_t Tsub = kind == kItemCluster ? std::max<int64_t>(total * kNum[t] / (kDen[t] * (int64_t)K), 2048)
+                                                      : std::max<int64_t>(slot * 4 / 5, 2048);
+            frontier.clear();
+            int64_t top_bytes = 0;
+            for (int32_t b = 0; b < nb; ++b) {
+                if (br[b].parent < 0 || root_of[br[b].parent] == -2) {
+                    if (sub[b] > Tsub) { root_of[b] = -2; top_bytes += bytes[b]; }
+                    else { root_of[b] = b; frontier.push_back(b); }
+                } else root_of[b] = root_of[br[b].parent];
+            }
+            int32_t np = 1;
+            if (kind == kItemCluster) {
+                np = K;
+                load.assign(K, 0); load[0] = top_bytes;
+                int64_t acc = top_bytes; int32_t r = 0;
+                for (int32_t f : frontier) {
+                    while (r < K - 1 && acc + sub[f] / 2 > total * (r + 1) / K) ++r;
+                    part_of_root[f] = r; acc += sub[f]; load[r] += sub[f];
+                }
+            } else {
+                int32_t r = 1; int64_t acc = 0;
+                load.assign(1, top_bytes);
+                for (int32_t f : frontier) {
+                    if (acc > 0 && acc + sub[f] > slot) { ++r; acc = 0; }
+                    part_of_root[f] = r; acc += sub[f];
+                }
+                np = frontier.empty() ? 1 : r + 1;
+                if (np > 65535) { out.ok = false; return; }
+            }
+            const int64_t mx = *std::max_element(load.begin(), load.end());
+            if (best_max < 0 || mx < best_max) { best_max = mx; best_root = root_of; best_part = part_of_root; best_nparts = np; }
+        }
+        nparts = best_nparts;
+        root_of.swap(best_root); part_of_root.swap(best_part);
+        for (int32_t b = 0; b < nb; ++b) br[b].part = root_of[b] == -2 ? 0 : part_of_root[root_of[b]];
+    }
+    out.parts.assign(nparts, PartBuild());
+    // exported sub-tree roots (branches whose parent branch lies in another part, which must be part 0)
+    std::vector<int32_t> g0_of_branch, p0_of_branch, x_of_branch, gp_of_branch;
+    if (nparts > 1) {
+        g0_of_branch.assign(nb, -1); p0_of_branch.assign(nb, -1); x_of_branch.assign(nb, -1); gp_of_branch.assign(nb, -1);
+        for (int32_t b = 0; b < nb; ++b)
+            if (br[b].parent >= 0 && br[br[b].parent].part != br[b].part && br[br[b].parent].part != 0) { out.ok = false; return; }
+    }
+    std::vector<int32_t> lmap(nn, -1);                  // provisional node id -> local id in the part being built
+    std::vector<std::vector<int32_t>> part_br(nparts);
+    for (int32_t b = 0; b < nb; ++b) part_br[br[b].part].push_back(b);
+    std::vector<NodeTmp> nodes;
+    std::vector<SegTmp> segs;
+    std::vector<int32_t> ord, first, cnt, dist;
+    for (int32_t p = 0; p < nparts; ++p) {
+        PartBuild& pb = out.parts[p];
+        const std::vector<int32_t>& mine = part_br[p];
+        // ---- runs of consecutive compartments, staged one after the other; the staged index of a run has the
+        //      parity of its global index, so that the 16-byte words of both sides coincide (bulk copies) ----
+        int64_t cursor = 0;
+        for (size_t i = 0; i < mine.size();) {
+            size_t j = i; int32_t end = br[mine[i]].start;
+            while (j < mine.size() && br[mine[j]].start == end) { end += br[mine[j]].len; ++j; }
+            const int32_t start = br[mine[i]].start, len = end - start;
+            const int64_t g = out.comp_begin + start;
+            const int64_t so = round_up(cursor, E) + g % E;
+            if (so + len >= ((int64_t)1 << 30)) { out.ok = false; return; }
+            pb.runs.insert(pb.runs.end(), {start, len, (int32_t)so, 0});
+            for (size_t k = i; k < j; ++k) br[mine[k]].soff = (int32_t)(so + br[mine[k]].start - start);
+            cursor = so + len;
+            const int64_t ga = g - g % E, ge = std::min<int64_t>(round_up(g + len, E), P.n / E * E);
+            if (ge > ga) pb.tx_elems += (int32_t)(ge - ga);
+            pb.n += len;
             i = j;
         }
-        std::sort(groups.begin(), groups.end(), [](const Group& a, const Group& b) {
-            if (a.maxseg != b.maxseg) return a.maxseg > b.maxseg;
-            return a.minord < b.minord;
-        });
-        for (const Group& g : groups)
-            for (int32_t i = 0; i < g.count; ++i) {
-                Br& e = br[v[g.first + i]];
-                e.e = (int32_t)lane_br.size();
-                lane_br.push_back(v[g.first + i]);
+        pb.L = (int32_t)round_up(cursor, E);
+        // ---- P3: the part's reduced forest, level by level, children of a node consecutive --------------------
+        nodes.clear();
+        for (int32_t b : mine) for (int32_t k = 0; k < br[b].nseg; ++k) nodes.push_back({ndepth[br[b].node0 + k], -1, br[b].node0 + k, 0});
+        if (p == 0 && nparts > 1)
+            for (int32_t b = 0; b < nb; ++b)
+                if (br[b].part != 0 && br[b].parent >= 0 && br[br[b].parent].part == 0) nodes.push_back({ndepth[br[b].node0], -1, br[b].node0, 1});
+        std::stable_sort(nodes.begin(), nodes.end(), [](const NodeTmp& x, const NodeTmp& y) { return x.depth < y.depth; });
+        pb.lb.assign(1, 0);
+        int32_t next = 0;
+        for (size_t i = 0; i < nodes.size();) {
+            size_t j = i;
+            while (j < nodes.size() && nodes[j].depth == nodes[i].depth) ++j;
+            for (size_t k = i; k < j; ++k) {
+                const int32_t pg = nparent[nodes[k].gid];
+                nodes[k].pkey = pg >= 0 ? lmap[pg] : -1;                     // -1: root of the cell, or parent outside the part
             }
-    }
-    out.ndesc = (int32_t)lane_br.size();
-    int32_t next_id = out.ndesc;
-    for (int32_t e = 0; e < out.ndesc; ++e) {
-        if (lane_br[e] < 0) continue;
-        Br& b = br[lane_br[e]];
-        if (b.nseg > 1) { b.rest = next_id; next_id += b.nseg - 1; }
-    }
-    out.nnode = next_id;
-    if (out.nnode >= (1 << 20)) out.ok = false;
-    auto last_node = [&](const Br& b) { return b.nseg > 1 ? b.rest + b.nseg - 2 : b.e; };
-    out.pnode.resize(out.nnode);
-    std::iota(out.pnode.begin(), out.pnode.end(), 0);
-    std::vector<int32_t> depth(out.nnode, 1);          // nodes on the path from the root, inclusive
-    int32_t height = 1;
-    for (int32_t e = 0; e < out.ndesc; ++e) {           // lanes are in level order: parents come first
-        const Br& b = br[lane_br[e]];
-        if (b.parent >= 0) { out.pnode[e] = last_node(br[b.parent]); depth[e] = depth[out.pnode[e]] + 1; }
-        for (int32_t k = 1; k < b.nseg; ++k) {          // a root keeps itself as parent: its f is 0
-            out.pnode[b.rest + k - 1] = k == 1 ? e : b.rest + k - 2;
-            depth[b.rest + k - 1] = depth[e] + k;
+            std::sort(nodes.begin() + i, nodes.begin() + j, [](const NodeTmp& x, const NodeTmp& y) {
+                return x.pkey != y.pkey ? x.pkey < y.pkey : x.gid < y.gid; });
+            for (size_t k = i; k < j; ++k) {
+                if (nodes[k].ghost) g0_of_branch[nbr[nodes[k].gid]] = next; else lmap[nodes[k].gid] = next;
+                ++next;
+            }
+            pb.lb.push_back(next);
+            i = j;
         }
-        height = std::max(height, depth[e] + b.nseg - 1);
-    }
-    (void)height;
-    build_tasks(out, depth);                            // also sets out.rounds
-    if (!out.ok) { out.perm.resize(out.nnode); std::iota(out.perm.begin(), out.perm.end(), 0); }
-    // ---- P4: segments, in compartment order ------------------------------------------------------
-    // Branch cut from its end into nseg segments of sj compartments (the paper's branch splitting,
-    // PAPER.md:151, with a fixed bound); node ids from the top of the branch: e, rest, rest+1, ...
-    std::vector<SegTmp> segs;                          // a item-local here
-    segs.reserve(nb);
-    for (int32_t i = 0; i < nb; ++i) {
-        const Br& b = br[i];
-        const int32_t end = b.start + b.len - 1;
-        for (int32_t k = 0; k < b.nseg; ++k) {          // k-th segment from the top
-            const int32_t q = b.nseg - 1 - k;           // counted from the branch's end
-            const int32_t sb = end - q * b.sj;
-            const int32_t sa = std::max(b.start, sb - b.sj + 1);
-            const int32_t node = k == 0 ? b.e : b.rest + k - 1;
-            const int32_t tnode = k > 0 ? (k == 1 ? b.e : b.rest + k - 2) : (b.parent >= 0 ? last_node(br[b.parent]) : -1);
-            segs.push_back({sa, sb - sa, out.perm[node], tnode < 0 ? -1 : out.perm[tnode]});
-            out.useful_steps += sb - sa;
+        pb.nlev = (int32_t)pb.lb.size() - 1;
+        pb.nlevnode = next;
+        first.assign(next, 0); cnt.assign(next, 0);
+        for (int32_t v = 0; v < next; ++v)
+            if (nodes[v].pkey >= 0) { if (!cnt[nodes[v].pkey]) first[nodes[v].pkey] = v; ++cnt[nodes[v].pkey]; }
+        // every cell of the part an unbranched cable of at most 32 nodes: the reduced systems are solved by
+        // parallel cyclic reduction, one warp per cable; nodes are then numbered cable by cable (lb[] = first
+        // node of each cable) instead of level by level
+        bool chains = kind == kItemSingle && next > 0 && (int64_t)mine.size() == c1 - c0;
+        if (chains) for (int32_t b : mine) if (br[b].nseg > 32 || br[b].parent >= 0) chains = false;
+        if (chains && !(P.opt.policy_flags & HINES_POLICY_NO_PCR)) {
+            pb.flags |= kPartFlagChains;
+            pb.lb.assign(1, 0);
+            int32_t id = 0;
+            for (int32_t b : mine) {
+                for (int32_t k = 0; k < br[b].nseg; ++k) lmap[br[b].node0 + k] = id++;
+                pb.lb.push_back(id);
+            }
+            pb.nlev = (int32_t)mine.size();
+            pb.kp.assign(4 * (size_t)next, 0);
+            for (int32_t b : mine)
+                for (int32_t k = 0; k < br[b].nseg; ++k) {
+                    const int32_t v = lmap[br[b].node0 + k];
+                    pb.kp[4 * v + 2] = k + 1 < br[b].nseg ? 1 : 0;
+                    pb.kp[4 * v + 3] = k > 0 ? v - 1 : v;
+                }
+            pb.nnode = next; pb.rounds = 0; pb.ntoplev = 0; pb.lowlev = 0; pb.maxwidth = 0;
+        } else {
+        // per node {slot0, slot1, info, pnode}: slot0/slot1 = byte offsets (in the record array) of the hand-off
+        // slots of its first two children, or of the all-zero record behind the last node; info = children |
+        // top << 29, or -1 for a ghost child; pnode = the node the forward sweep reads
+        const int32_t RSb = 6 * w, zero_slot = 0;             // the zero record sits at index nnode: patched below
+        (void)zero_slot;
+        pb.kp.assign(4 * (size_t)next, 0);
+        dist.assign(next, 0);
+        int32_t maxdist = 0;
+        for (int32_t v = 0; v < next; ++v) {
+            const NodeTmp& nt = nodes[v];
+            int32_t pn = v;
+            if (nt.ghost) {
+                pb.kp[4 * v + 2] = -1;
+                p0_of_branch[nbr[nt.gid]] = nt.pkey;
+                x_of_branch[nbr[nt.gid]] = pb.nghost;
+                pb.ghosts.insert(pb.ghosts.end(), {v, pb.nghost, nt.pkey, 0});
+                ++pb.nghost;
+            } else {
+                if (cnt[v] > 4095) { out.ok = false; return; }
+                pb.kp[4 * v] = cnt[v] > 0 ? first[v] : -1;             // node index for now, byte offset below
+                pb.kp[4 * v + 1] = cnt[v] > 1 ? first[v] + 1 : -1;
+                pb.kp[4 * v + 2] = cnt[v];
+                if (nt.pkey >= 0) pn = nt.pkey;
+                else if (nparent[nt.gid] >= 0) {                               // exported sub-tree root: its parent is a ghost
+                    const int32_t b = nbr[nt.gid];
+                    pn = next + pb.nexp;
+                    gp_of_branch[b] = pn;
+                    if (kind == kItemCluster) pb.exps.insert(pb.exps.end(), {v, g0_of_branch[b], p0_of_branch[b], pn});
+                    else pb.exps.insert(pb.exps.end(), {v, x_of_branch[b], 0, pn});
+                    if (g0_of_branch[b] < 0) { out.ok = false; return; }
+                    ++pb.nexp;
+                }
+            }
+            pb.kp[4 * v + 3] = pn;
+            dist[v] = pn == v ? 0 : (pn >= next ? 1 : dist[pn] + 1);
+            maxdist = std::max(maxdist, dist[v]);
         }
-    }
-    // ---- chunks: consecutive segments, balanced in shared-memory bytes -----------------------------
-    const int64_t meta_item = (int64_t)out.task_blob.size() + round_up(out.nnode, 4);
-    out.leader_extra = 6 * round_up(out.nnode, E) * P.width + 4 * meta_item;
-    out.chunks.assign(nchunks, ItemBuild::Chunk());
-    const int64_t per_comp = 3 * P.width, per_seg = 32;   // two lanes per segment
-    const int64_t total = out.leader_extra + per_comp * out.n + per_seg * (int64_t)segs.size();
-    out.total_bytes = total;
-    size_t si = 0;
-    int64_t acc = 0;
-    std::vector<SegTmp> mine;
-    for (int32_t r = 0; r < nchunks; ++r) {
-        ItemBuild::Chunk& ch = out.chunks[r];
-        const int64_t target = total * (r + 1) / nchunks;            // cumulative, so rounding does not pile up
-        if (r == 0) acc = out.leader_extra;
-        ch.begin = si < segs.size() ? segs[si].a : (int32_t)out.n;
-        mine.clear();
-        while (si < segs.size()) {
-            const int64_t cost = per_comp * (segs[si].m + 1) + per_seg;
-            const size_t left_chunks = (size_t)(nchunks - 1 - r);
-            const bool must_take = mine.empty() && segs.size() - si > left_chunks;   // no empty chunk while segments remain
-            const bool must_leave = segs.size() - si <= left_chunks;                   // keep one for every later chunk
-            if (r == nchunks - 1 || must_take || (!must_leave && acc + cost / 2 <= target)) {
-                mine.push_back(segs[si]); acc += cost; ++si;
-            } else break;
+        pb.nnode = next + pb.nexp;
+        for (int32_t e = 0; e < pb.nexp; ++e) pb.kp.insert(pb.kp.end(), {0, 0, 0, next + e});    // ghost parents read themselves
+        for (int32_t v = 0; v < next; ++v)
+            for (int q = 0; q < 2; ++q) pb.kp[4 * v + q] = (pb.kp[4 * v + q] < 0 ? pb.nnode : pb.kp[4 * v + q]) * RSb + 4 * w;
+        while ((1 << pb.rounds) <= maxdist) ++pb.rounds;
+        pb.maxwidth = 0;
+        for (int32_t l = 0; l < pb.nlev; ++l) pb.maxwidth = std::max(pb.maxwidth, pb.lb[l + 1] - pb.lb[l]);
+        // top nodes = the ancestors of ghost children (bit 29 of info): they wait for the other parts' hand-off values;
+        // everything else in the part is swept before that.  ntoplev: levels [0, ntoplev) hold top nodes; lowlev: the
+        // smallest level with a node that is not a top node.
+        pb.ntoplev = 0; pb.lowlev = pb.nlev;
+        if (pb.nghost) {
+            std::vector<char> top(next, 0);
+            for (int32_t v = next - 1; v >= 0; --v)
+                if (nodes[v].pkey >= 0 && (nodes[v].ghost || top[v])) top[nodes[v].pkey] = 1;
+            int32_t l = 0;
+            for (int32_t v = 0; v < next; ++v) {
+                while (v >= pb.lb[l + 1]) ++l;
+                if (top[v]) { pb.kp[4 * v + 2] |= 1 << 29; pb.ntoplev = std::max(pb.ntoplev, l + 1); }
+                else if (!nodes[v].ghost) pb.lowlev = std::min(pb.lowlev, l);
+            }
+        } else if (next > 0) pb.lowlev = 0;
         }
-        ch.n = mine.empty() ? 0 : mine.back().a + mine.back().m + 1 - ch.begin;
-        for (SegTmp& sg : mine) sg.a -= ch.begin;
-        const int32_t off = (int32_t)((out.comp_begin + ch.begin) % E);
+        if (p == 0) out.nxch = pb.nghost;
+        // ---- P4: segments, in compartment order ---------------------------------------------------------------
+        segs.clear();
+        for (int32_t b : mine) {
+            const Br& e = br[b];
+            int32_t pos = e.soff;
+            for (int32_t k = 0; k < e.nseg; ++k) {
+                const int32_t plen = pieces[e.piece0 + k];
+                const int32_t node = lmap[e.node0 + k];
+                int32_t tnode;
+                if (k > 0) tnode = lmap[e.node0 + k - 1];
+                else if (e.parent < 0) tnode = -1;
+                else if (br[e.parent].part == p) tnode = lmap[br[e.parent].node0 + br[e.parent].nseg - 1];
+                else tnode = gp_of_branch[b];
+                segs.push_back({pos, plen - 1, node, tnode});
+                out.useful_steps += plen - 1;
+                pos += plen;
+            }
+        }
         // two lanes per segment: lane A eliminates the interior above the middle node q, lane B the interior
-        // below it, both top-down (fill-in to t resp. q); A eliminates q last.  A warp holds
-        // 16 segments: A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
-        std::vector<int32_t> ord;
-        order_segments(mine, 16, P.width == 8 ? 16 : 32, off, ord);
+        // below it, both top-down (fill-in to t resp. q); A eliminates q last.  A warp holds 16 segments:
+        // A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
+        order_segments(segs, 16, w == 8 ? 16 : 32, 0, ord);
         while ((ord.size() / 4) % 16) ord.insert(ord.end(), {0, 0, -1, -1});
         const int32_t ngroups = (int32_t)(ord.size() / 64);
-        ch.seg.assign((size_t)ngroups * 128, 0);
+        pb.seg.assign((size_t)ngroups * 128, 0);
         for (int32_t gidx = 0; gidx < ngroups; ++gidx) {
             int32_t mx = 0;
             for (int32_t k = 0; k < 16; ++k) {
                 const int32_t* sgp = &ord[(size_t)(gidx * 16 + k) * 4];
-                int32_t* A = &ch.seg[(size_t)(gidx * 32 + k) * 4];
-                int32_t* B = &ch.seg[(size_t)(gidx * 32 + 16 + k) * 4];
+                int32_t* A = &pb.seg[(size_t)(gidx * 32 + k) * 4];
+                int32_t* B = &pb.seg[(size_t)(gidx * 32 + 16 + k) * 4];
                 const uint32_t ow = (uint32_t)sgp[1];
                 const int32_t a = sgp[0], mm = (int32_t)(ow & 0xfff), node = sgp[2], tnode = sgp[3];
                 if (node < 0) { A[2] = A[3] = B[2] = B[3] = -1; continue; }
@@ -517,11 +495,14 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t nchu
             }
             out.padded_steps += 32 * (int64_t)(mx + 1);     // the loop steps of the warp + the step for q
         }
-        const int32_t ns = (int32_t)(ch.seg.size() / 4);
-        out.max_lanes = std::max(out.max_lanes, ns);
-        const int64_t L = round_up(off + ch.n, E);
-        ch.smem_need = 16 + (r == 0 ? out.leader_extra : 0) + 3 * L * P.width + 16 * (int64_t)ns;
-        out.smem_need = std::max(out.smem_need, ch.smem_need);
+        pb.nlanes = ngroups * 32;
+        for (const SegTmp& sg : segs) if (sg.m >= 0xfff) out.ok = false;
+        const int64_t meta = round_up(pb.nlev + 1, 4) + 4 * (int64_t)pb.nnode + 4 * (int64_t)pb.nexp +
+                             4 * (int64_t)pb.nghost + 4 * (int64_t)pb.nlanes;
+        pb.smem_need = 16 + 512 + 6 * round_up(pb.nnode + 1, E) * w + 4 * meta + 3 * (int64_t)pb.L * w;
+        if (kind == kItemSplit && p == 0) { out.smem_top = pb.smem_need; out.max_lanes_top = pb.nlanes; }
+        else { out.smem_need = std::max(out.smem_need, pb.smem_need); out.max_lanes = std::max(out.max_lanes, pb.nlanes); }
+        for (int32_t b : mine) for (int32_t k = 0; k < br[b].nseg; ++k) lmap[br[b].node0 + k] = -1;
     }
 }
 
@@ -617,62 +598,110 @@ static hines_status_t canonical_tables(hines_plan& P, const int32_t* parent)
     return HINES_OK;
 }
 
+// f1: the paper's branch splitting (reading F1).  Level by level from the root, over
+// ALL cells of the batch ("the average length of all dendritic branches on this level"): c = ceil(mean length of
+// the pieces on the level); a piece longer than c is cut into a head of c compartments, which stays on the level,
+// and the rest, which becomes its only child on the next level ("two shorter branches that are attached to each
+// other") and takes the branch's children along ("causes all child branches to move one level down"); the rest
+// may be cut again there.  Integer arithmetic throughout: c = (sum + count - 1) / count.
+static void level_mean_split(hines_plan& P)
+{
+    const int64_t nbr = P.nbranches;
+    std::vector<int64_t> base(nbr);                               // first branch of the branch's cell
+    for (int64_t c = 0; c < P.ncells; ++c)
+        for (int64_t j = P.cell_branch_offsets[c]; j < P.cell_branch_offsets[c + 1]; ++j) base[j] = P.cell_branch_offsets[c];
+    struct It { int64_t j; int32_t rem; };
+    std::vector<It> cur, nxt;
+    struct Piece { int64_t j; int32_t len, level; };
+    std::vector<Piece> out;
+    out.reserve((size_t)nbr + (size_t)nbr / 2);
+    for (int64_t c = 0; c < P.ncells; ++c) cur.push_back({P.cell_branch_offsets[c], P.branch_len[P.cell_branch_offsets[c]]});
+    P.split_level_stat.clear();
+    for (int32_t level = 0; !cur.empty(); ++level) {
+        int64_t sum = 0;
+        for (const It& it : cur) sum += it.rem;
+        const int64_t cnt = (int64_t)cur.size();
+        const int64_t cut = (sum + cnt - 1) / cnt;
+        P.split_level_stat.push_back(sum); P.split_level_stat.push_back(cnt);
+        nxt.clear();
+        for (const It& it : cur) {
+            if (it.rem > cut) {
+                out.push_back({it.j, (int32_t)cut, level});
+                nxt.push_back({it.j, (int32_t)(it.rem - cut)});
+            } else {
+                out.push_back({it.j, it.rem, level});
+                for (int64_t k = P.child_offsets[it.j]; k < P.child_offsets[it.j + 1]; ++k) {
+                    const int64_t ch = base[it.j] + P.child_ids[k];
+                    nxt.push_back({ch, P.branch_len[ch]});
+                }
+            }
+        }
+        cur.swap(nxt);
+    }
+    P.split_piece_offsets.assign(nbr + 1, 0);
+    for (const Piece& p : out) P.split_piece_offsets[p.j + 1]++;
+    for (int64_t j = 0; j < nbr; ++j) P.split_piece_offsets[j + 1] += P.split_piece_offsets[j];
+    P.split_piece_len.assign(out.size(), 0);
+    P.split_piece_level.assign(out.size(), 0);
+    std::vector<int64_t> fill(P.split_piece_offsets.begin(), P.split_piece_offsets.end() - 1);
+    for (const Piece& p : out) { const int64_t q = fill[p.j]++; P.split_piece_len[q] = p.len; P.split_piece_level[q] = p.level; }
+}
+
 static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib)
 {
-    const int32_t item = (int32_t)P.item_class.size();
+    const int32_t item = (int32_t)P.item_kind.size();
     for (int64_t c = c0; c < c1; ++c) P.cell_item[c] = item;
     P.item_cell_range.push_back(c0);
     P.item_cell_range.push_back(c1);
     P.item_class.push_back(0);                     // filled by assign_classes
-    P.item_pnode.insert(P.item_pnode.end(), ib.pnode.begin(), ib.pnode.end());
-    P.item_node_offsets.push_back((int64_t)P.item_pnode.size());
-    P.item_rounds.push_back(ib.rounds);
-    P.item_nnode.push_back(ib.nnode);
-    P.item_task_blob.insert(P.item_task_blob.end(), ib.task_blob.begin(), ib.task_blob.end());
-    P.item_task_offsets.push_back((int64_t)P.item_task_blob.size());
-    // device blob of the item: [task blob | pnode | pad4]
-    hines::ItemHeader h{};
-    h.meta_off = (int64_t)P.item_meta.size();
-    P.item_meta.insert(P.item_meta.end(), ib.task_blob.begin(), ib.task_blob.end());
-    h.grp_off = ib.grp_off; h.ent_off = ib.ent_off; h.pull_off = ib.pull_off; h.ntier = ib.ntier;
-    h.pnode_off = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    P.item_meta.insert(P.item_meta.end(), ib.pnode.begin(), ib.pnode.end());
-    P.item_meta.resize(round_up((int64_t)P.item_meta.size(), 4), 0);
-    h.meta_len = (int32_t)((int64_t)P.item_meta.size() - h.meta_off);
-    h.nnode = ib.nnode; h.rounds = ib.rounds;
-    h.first_chunk = (int32_t)P.chunk_headers.size();
-    h.nchunks = ib.nchunks;
-    h.n = (int32_t)ib.n;
-    P.item_headers.push_back(h);
-    for (int32_t r = 0; r < ib.nchunks; ++r) {
-        const ItemBuild::Chunk& ch = ib.chunks[r];
-        hines::ChunkHeader k{};
-        k.comp_begin = ib.comp_begin + ch.begin;
-        k.n = ch.n;
-        k.nseg_lanes = (int32_t)(ch.seg.size() / 4);
-        k.item = item; k.rank = r;
-        k.seg_off = (int64_t)P.item_meta.size();
-        P.item_meta.insert(P.item_meta.end(), ch.seg.begin(), ch.seg.end());
-        P.chunk_headers.push_back(k);
-        P.chunk_comp_range.push_back(k.comp_begin);
-        P.chunk_comp_range.push_back(k.comp_begin + k.n);
-        P.chunk_seg.insert(P.chunk_seg.end(), ch.seg.begin(), ch.seg.end());
-        P.chunk_seg_offsets.push_back((int64_t)P.chunk_seg.size() / 4);
+    P.item_kind.push_back(ib.kind);
+    P.item_xch.push_back((int32_t)P.n_xch);
+    const int32_t xs0 = 2 * (ib.parts[0].rounds & 1) + 1;
+    for (size_t r = 0; r < ib.parts.size(); ++r) {
+        const PartBuild& pb = ib.parts[r];
+        hines::PartHeader h{};
+        h.meta_off = (int64_t)P.part_meta.size();
+        std::vector<int32_t>& M = P.part_meta;
+        auto pad4 = [&]() { M.resize((size_t)round_up((int64_t)M.size(), 4), 0); };
+        M.insert(M.end(), pb.lb.begin(), pb.lb.end()); pad4();
+        h.kp_off = (int32_t)((int64_t)M.size() - h.meta_off);
+        M.insert(M.end(), pb.kp.begin(), pb.kp.end()); pad4();
+        h.exp_off = (int32_t)((int64_t)M.size() - h.meta_off);
+        M.insert(M.end(), pb.exps.begin(), pb.exps.end());
+        h.gh_off = (int32_t)((int64_t)M.size() - h.meta_off);
+        M.insert(M.end(), pb.ghosts.begin(), pb.ghosts.end());
+        h.seg_off = (int32_t)((int64_t)M.size() - h.meta_off);
+        M.insert(M.end(), pb.seg.begin(), pb.seg.end());
+        h.meta_len = (int32_t)((int64_t)M.size() - h.meta_off);
+        h.run_off = (int32_t)(P.part_runs.size() / 4);
+        h.nrun = (int32_t)(pb.runs.size() / 4);
+        for (int32_t k = 0; k < h.nrun; ++k)
+            P.part_runs.insert(P.part_runs.end(), {(int32_t)(ib.comp_begin + pb.runs[4 * k]), pb.runs[4 * k + 1], pb.runs[4 * k + 2], 0});
+        h.tx_elems = pb.tx_elems; h.L = pb.L; h.n = pb.n;
+        h.nnode = pb.nnode; h.nlevnode = pb.nlevnode; h.nlev = pb.nlev; h.rounds = pb.rounds;
+        h.nexp = pb.nexp; h.nghost = pb.nghost; h.nseg_lanes = pb.nlanes;
+        h.xch_base = (int32_t)P.n_xch; h.xs0 = xs0;
+        h.item = item; h.rank = (int32_t)r; h.flags = pb.flags; h.ntoplev = pb.ntoplev; h.lowlev = pb.lowlev; h.maxwidth = pb.maxwidth;
+        P.part_headers.push_back(h);
+        P.n_exports += pb.nexp;
     }
-    P.item_chunk_offsets.push_back((int64_t)P.chunk_headers.size());
+    P.item_part_offsets.push_back((int64_t)P.part_headers.size());
+    if (ib.kind == kItemSplit) P.n_xch += ib.nxch;
     P.padded_lane_steps += ib.padded_steps;
     P.useful_lane_steps += ib.useful_steps;
-    if (ib.nchunks > 1) { P.n_cluster_cells += c1 - c0; P.n_cluster_unknowns += ib.n; }
+    if (ib.kind == kItemCluster) { P.n_cluster_cells += c1 - c0; P.n_cluster_unknowns += ib.n; }
+    if (ib.kind == kItemSplit) { P.n_split_cells += c1 - c0; P.n_split_unknowns += ib.n; }
     P.n_resident_cells += c1 - c0;
     P.n_resident_unknowns += ib.n;
 }
 
-struct ItemNeed { int64_t smem; int32_t lanes; int32_t nchunks; };
+struct ItemNeed { int64_t smem; int32_t lanes; int32_t nparts; int32_t kind; int64_t smem_top; int32_t lanes_top; };
 
-// P1 + P2: cells -> work items, greedy in input order.  A cell whose lists fit the
-// group budget joins the open group while the group still fits; a cell that fits one block's budget
-// gets its own item; a larger cell is spread over a cluster of 2, 4, 8 or 16 blocks ("long branches
-// of large cells kept on their own blocks"); what fits nowhere goes to the streaming path.
+// P1 + P2: cells -> work items, greedy in input order.  A cell whose lists fit the group budget
+// joins the open group while the group still fits; a cell that fits one block's budget gets its own item; a
+// larger cell is cut into the parts of a cluster of up to cluster_max blocks ("long branches of large cells kept
+// on their own blocks"), beyond that into the parts of a split item (three launches); what fits nowhere goes to
+// the streaming path.
 static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<char>& is_stream)
 {
     const int64_t nc = P.ncells;
@@ -681,108 +710,158 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     const bool force_stream = P.opt.policy_flags & HINES_POLICY_FORCE_STREAM;
     const bool no_group = P.opt.policy_flags & HINES_POLICY_NO_GROUPING;
     const bool no_cluster = (P.opt.policy_flags & HINES_POLICY_NO_CLUSTER) || P.opt.cluster_max < 2;
+    const bool no_split = (P.opt.policy_flags & HINES_POLICY_NO_SPLIT) != 0;
     // a cell alone in a block may use up to single_cap; beyond that a cluster is preferred, because
     // blocks of at most chunk_smem_bytes leave room for a second resident block per SM
     const int64_t chunk_cap = std::min<int64_t>(P.opt.chunk_smem_bytes, max_smem);
     const int64_t single_cap = no_cluster ? max_smem : chunk_cap;
     const bool pow2_only = P.opt.policy_flags & HINES_POLICY_POW2_CLUSTERS;
+    const bool level_mean = (P.opt.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN) != 0;
+    const int32_t w = P.width;
     P.cell_item.assign(nc, -1);
-    P.item_node_offsets.assign(1, 0);
-    P.item_task_offsets.assign(1, 0);
-    P.item_chunk_offsets.assign(1, 0);
-    P.chunk_seg_offsets.assign(1, 0);
+    P.item_part_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
     ItemBuild cur, cand, alone;
-    int64_t g0 = -1;                                   // first cell of the open group
     auto push = [&](int64_t a, int64_t b, const ItemBuild& ib) {
         emit_item(P, a, b, ib);
-        need.push_back({ib.smem_need, ib.max_lanes, ib.nchunks});
+        need.push_back({ib.smem_need, ib.max_lanes, (int32_t)ib.parts.size(), ib.kind, ib.smem_top, ib.max_lanes_top});
     };
-    auto flush = [&](int64_t c_end) { if (g0 >= 0) { push(g0, c_end, cur); g0 = -1; } };
+    // additive estimate of a cell's shared-memory need as a single part (upper side): arrays + per node the
+    // record, two segment lanes and {kids, parent}; decides group membership without building the group
+    std::vector<int32_t> tmp;
+    auto estimate = [&](int64_t c) -> int64_t {
+        int64_t nodes = 0;
+        for (int64_t j = P.cell_branch_offsets[c]; j < P.cell_branch_offsets[c + 1]; ++j) {
+            tmp.clear();
+            if (level_mean) for (int64_t q = P.split_piece_offsets[j]; q < P.split_piece_offsets[j + 1]; ++q) fixed_bound_pieces(P.split_piece_len[q], P.seg_single, tmp);
+            else fixed_bound_pieces(P.branch_len[j], P.seg_single, tmp);
+            nodes += (int64_t)tmp.size();
+        }
+        return 3 * (int64_t)w * (P.cell_offsets[c + 1] - P.cell_offsets[c]) + nodes * (6 * w + 32 + 8) + 4 * (P.cell_nlevels[c] + 1);
+    };
+    const int64_t group_fixed = 16 + 2048;          // mbarrier, alignment slack, padding of the lane list to whole warps
+    int64_t g0 = -1, gacc = 0;                      // first cell of the open group, its estimated need
+    // flush the open group [a, b): built once; should the build exceed the cap after all, halve it
+    std::function<void(int64_t, int64_t)> flush_range = [&](int64_t a, int64_t b) {
+        if (a >= b) return;
+        ItemBuild ib;
+        build_item(P, a, b, kItemSingle, 1, 0, ib);
+        if ((!ib.ok || ib.smem_need > group_cap) && b - a > 1) { const int64_t mid = (a + b) / 2; flush_range(a, mid); flush_range(mid, b); return; }
+        if (!ib.ok || ib.smem_need > max_smem) { for (int64_t c = a; c < b; ++c) is_stream[c] = 1; return; }
+        push(a, b, ib);
+    };
+    auto flush = [&](int64_t c_end) { if (g0 >= 0) { flush_range(g0, c_end); g0 = -1; gacc = 0; } };
     for (int64_t c = 0; c < nc; ++c) {
-        const int64_t ncomp = P.cell_offsets[c + 1] - P.cell_offsets[c];
+        if (force_stream) { is_stream[c] = 1; continue; }
+        const int64_t est = estimate(c);
+        if (!no_group && est + group_fixed <= group_cap) {                  // a small cell: joins the open group, greedy in input order
+            if (g0 >= 0 && gacc + est + group_fixed > group_cap) flush(c);
+            if (g0 < 0) { g0 = c; gacc = 0; }
+            gacc += est;
+            continue;
+        }
+        flush(c);
         bool placed = false, is_single = false;
-        if (!force_stream) {
-            const int64_t arrays = 16 + 3 * ncomp * P.width;             // lower bound of the need
-            if (arrays <= single_cap) {
-                build_item(P, c, c + 1, 1, alone);
-                is_single = alone.ok && alone.smem_need <= single_cap;
+        if (est <= single_cap + 4096) {
+            build_item(P, c, c + 1, kItemSingle, 1, 0, alone);
+            is_single = alone.ok && alone.smem_need <= single_cap;
+        }
+        if (!is_single && !no_cluster) {
+            // cluster size: the one whose blocks fill their shared-memory slot best (slots = an SM's
+            // shared memory divided by 2, 3, 4); close calls go to the smaller cluster
+            const int64_t total = est + 1024;
+            struct Opt { double score; int32_t k; int64_t slot; };
+            std::vector<Opt> opts;
+            for (int t = 1; t <= 3; ++t) {                                // slots of 1/2, 1/3, 1/4 of an SM
+                const int64_t slot = class_cap(kClassK[t], max_smem);
+                if (slot > chunk_cap) continue;
+                int32_t k = (int32_t)std::max<int64_t>(2, (total + slot - 4096 - 1) / (slot - 4096));
+                if (pow2_only) while (k & (k - 1)) ++k;
+                if (k > P.opt.cluster_max) continue;
+                opts.push_back({-((double)total / (double)(k * slot) - 0.01 * t), k, slot});
             }
-            if (!is_single && !no_cluster) {
-                // cluster size: the one whose blocks fill their shared-memory slot best (slots = an SM's
-                // shared memory divided by 1, 2, 3, 4, 6, 8); close calls go to the smaller cluster
-                build_item(P, c, c + 1, 2, cand);
-                if (cand.ok) {
-                    const int64_t total = cand.total_bytes;
-                    std::vector<std::pair<double, int32_t>> opts;                 // (-score, k)
-                    for (int t = 1; t <= 3; ++t) {                                // slots of 1/2, 1/3, 1/4 of an SM
-                        const int64_t slot = class_cap(kClassK[t], max_smem);
-                        if (slot > chunk_cap) continue;
-                        int32_t k = (int32_t)std::max<int64_t>(2, (total + slot - 2048 - 1) / (slot - 2048));
-                        if (pow2_only) while (k & (k - 1)) ++k;
-                        if (k > P.opt.cluster_max) continue;
-                        opts.push_back({-((double)total / (double)(k * slot) - 0.01 * t), k});
-                    }
-                    if (opts.empty() && total / P.opt.cluster_max + 2048 <= max_smem) opts.push_back({0.0, P.opt.cluster_max});
-                    std::sort(opts.begin(), opts.end());
-                    for (size_t o = 0; o < opts.size() && o < 3 && !placed; ++o) {
-                        const int32_t k = opts[o].second;
-                        if (k != 2) build_item(P, c, c + 1, k, cand);
-                        int64_t slot = 0;
-                        for (int t = 0; t < kNumClassK; ++t) if (cand.smem_need <= class_cap(kClassK[t], chunk_cap)) slot = 1;
-                        if (slot || (k == P.opt.cluster_max && cand.smem_need <= max_smem)) { flush(c); push(c, c + 1, cand); placed = true; }
-                        else if (k == 2 && o + 1 < opts.size()) { /* rebuilt below for the next option */ }
-                    }
+            if (opts.empty() && total / P.opt.cluster_max + 4096 <= max_smem) opts.push_back({0.0, P.opt.cluster_max, max_smem});
+            std::sort(opts.begin(), opts.end(), [](const Opt& a, const Opt& b) { return a.score < b.score; });
+            for (size_t o = 0; o < opts.size() && o < 3 && !placed; ++o) {
+                // the sub-trees may not balance as well as the estimate assumes: one or two blocks more are tried too,
+                // and an option counts only if every part fits the slot it was chosen for
+                for (int32_t k = opts[o].k; k <= std::min<int32_t>(P.opt.cluster_max, opts[o].k + 2) && !placed; ++k) {
+                    if (pow2_only && (k & (k - 1))) continue;
+                    build_item(P, c, c + 1, kItemCluster, k, 0, cand);
+                    if (cand.ok && cand.smem_need <= opts[o].slot) { push(c, c + 1, cand); placed = true; }
                 }
-                if (!placed && arrays <= max_smem) {                      // last resort before streaming: one big block
-                    build_item(P, c, c + 1, 1, alone);
-                    is_single = alone.ok && alone.smem_need <= max_smem;
+            }
+            if (!placed) {                                                // anything that fits a block
+                for (int32_t k = opts.empty() ? P.opt.cluster_max : std::min<int32_t>(P.opt.cluster_max, opts[0].k + 3); k <= P.opt.cluster_max && !placed; k += std::max(1, k / 4)) {
+                    if (pow2_only && (k & (k - 1))) continue;
+                    build_item(P, c, c + 1, kItemCluster, k, 0, cand);
+                    if (cand.ok && cand.smem_need <= max_smem) { push(c, c + 1, cand); placed = true; }
                 }
+            }
+            if (!placed && est <= max_smem) {                             // one big block
+                build_item(P, c, c + 1, kItemSingle, 1, 0, alone);
+                is_single = alone.ok && alone.smem_need <= max_smem;
             }
         }
+        if (!placed && !is_single && !no_cluster && !no_split) {
+            // beyond the largest cluster: sub-tree parts of at most a split_smem_bytes slot + the top part in one block
+            const int64_t sslot = std::min<int64_t>(P.opt.split_smem_bytes, max_smem);
+            build_item(P, c, c + 1, kItemSplit, 0, sslot - 6144, cand);
+            if (cand.ok && cand.parts.size() > 1 && cand.smem_need <= sslot && cand.smem_top <= max_smem) { push(c, c + 1, cand); placed = true; }
+        }
         if (placed) continue;
-        if (!is_single) { flush(c); is_stream[c] = 1; continue; }
-        if (no_group || alone.smem_need > group_cap) { flush(c); push(c, c + 1, alone); continue; }
-        if (g0 < 0) { g0 = c; std::swap(cur, alone); continue; }
-        build_item(P, g0, c + 1, 1, cand);                                // greedy: does the next cell still fit?
-        if (cand.ok && cand.smem_need <= group_cap) { std::swap(cur, cand); continue; }
-        flush(c);
-        g0 = c; std::swap(cur, alone);
+        if (!is_single) { is_stream[c] = 1; continue; }
+        push(c, c + 1, alone);
     }
     flush(nc);
 }
 
 // Size classes.  By how many blocks of that size fit one SM (1, 2, 3, 4, 6, 8), separately for single-block
-// items and for every cluster size.  Threads per block: enough lanes for the widest segment
-// list of the class, within what the register file allows for that many resident blocks.
+// items, for every cluster size, and for the three launch phases of split items.  Threads per block: enough
+// lanes for the widest segment list of the class, within what the register file allows for that many resident blocks.
 static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
 {
     const int64_t nitems = (int64_t)need.size();
     const int64_t max_smem = P.opt.smem_bytes_per_block;
-    const int nq = kNumClassK * (kMaxClusterClass + 2);   // single blocks, then per cluster size, each by blocks per SM
+    // queue index: [0, 6) single blocks; 6*k + t cluster of k; then split: sub-tree parts, top parts
+    const int qSplitSub = kNumClassK * (kMaxClusterClass + 1), qSplitTop = qSplitSub + kNumClassK, nq = qSplitTop + kNumClassK;
+    auto slot_of = [&](int64_t smem) { int q = 0; for (int t = 0; t < kNumClassK; ++t) if (smem <= class_cap(kClassK[t], max_smem)) q = t; return q; };
     std::vector<int> item_q(nitems, 0);
     std::vector<int64_t> need_max(nq, 0), count(nq, 0);
     std::vector<int32_t> lanes_max(nq, 0);
     for (int64_t i = 0; i < nitems; ++i) {
-        int q = 0;
-        for (int t = 0; t < kNumClassK; ++t) if (need[i].smem <= class_cap(kClassK[t], max_smem)) q = t;
-        if (need[i].nchunks > 1) q += kNumClassK * need[i].nchunks;
+        int q = slot_of(need[i].smem);
+        if (need[i].kind == kItemCluster) q += kNumClassK * need[i].nparts;
+        if (need[i].kind == kItemSplit) {
+            q += qSplitSub;
+            const int qt = qSplitTop + slot_of(need[i].smem_top);
+            need_max[qt] = std::max(need_max[qt], need[i].smem_top);
+            lanes_max[qt] = std::max(lanes_max[qt], need[i].lanes_top);
+            count[qt]++;
+        }
         item_q[i] = q;
         need_max[q] = std::max(need_max[q], need[i].smem);
         lanes_max[q] = std::max(lanes_max[q], need[i].lanes);
         count[q]++;
     }
-    // launch order of the classes: clusters first (largest first), then single blocks, biggest first
-    std::vector<int> qs;
+    // launch order of the classes: clusters first (largest first), then single blocks, biggest first; the
+    // classes of split items on a stream of their own: phase A, then B, then C
+    struct Cls { int q, phase; };
+    std::vector<Cls> qs;
     for (int k = kMaxClusterClass; k >= 2; --k)
-        for (int t = 0; t < kNumClassK; ++t) if (count[kNumClassK * k + t]) qs.push_back(kNumClassK * k + t);
-    for (int q = 0; q < kNumClassK; ++q) if (count[q]) qs.push_back(q);
+        for (int t = 0; t < kNumClassK; ++t) if (count[kNumClassK * k + t]) qs.push_back({kNumClassK * k + t, kPhaseAll});
+    for (int q = 0; q < kNumClassK; ++q) if (count[q]) qs.push_back({q, kPhaseAll});
+    for (int q = qSplitSub; q < qSplitSub + kNumClassK; ++q) if (count[q]) qs.push_back({q, kPhaseA});
+    for (int q = qSplitTop; q < qSplitTop + kNumClassK; ++q) if (count[q]) qs.push_back({q, kPhaseB});
+    for (int q = qSplitSub; q < qSplitSub + kNumClassK; ++q) if (count[q]) qs.push_back({q, kPhaseC});
     std::vector<int> cls_of_q(nq, -1);
-    for (int q : qs) {
-        cls_of_q[q] = (int)P.class_smem_bytes.size();
+    for (const Cls& c : qs) {
+        const int q = c.q;
+        if (c.phase != kPhaseC) cls_of_q[q] = (int)P.class_smem_bytes.size();
         const int64_t smem = round_up(need_max[q], 128);
         P.class_smem_bytes.push_back((int32_t)smem);
-        P.class_cluster.push_back(q >= kNumClassK ? q / kNumClassK : 1);
+        P.class_cluster.push_back(q >= kNumClassK && q < qSplitSub ? q / kNumClassK : 1);
+        P.class_phase.push_back(c.phase);
         const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
         int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
         tmax = std::max<int64_t>(64, std::min<int64_t>(kMaxThreads, tmax));
@@ -790,20 +869,35 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
         t = std::max<int64_t>(P.opt.threads_per_block ? 32 : std::min<int64_t>(128, tmax), std::min(t, tmax));
         P.class_threads.push_back((int32_t)t);
     }
-    for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[item_q[i]];
-    const int ncls = (int)P.class_smem_bytes.size();
-    P.class_first.assign(ncls, 0);
-    P.class_count.assign(ncls, 0);
+    for (int64_t i = 0; i < nitems; ++i) P.item_class[i] = cls_of_q[need[i].kind == kItemSplit ? qSplitTop + slot_of(need[i].smem_top) : item_q[i]];
     P.item_launch_order.resize(nitems);
     std::iota(P.item_launch_order.begin(), P.item_launch_order.end(), 0);
     const bool input_order = P.opt.policy_flags & HINES_POLICY_INPUT_ORDER;
+    auto weight = [&](int32_t it) { return P.cell_offsets[P.item_cell_range[2 * (size_t)it + 1]] - P.cell_offsets[P.item_cell_range[2 * (size_t)it]]; };
     std::stable_sort(P.item_launch_order.begin(), P.item_launch_order.end(), [&](int32_t a, int32_t b) {
         if (P.item_class[a] != P.item_class[b]) return P.item_class[a] < P.item_class[b];
         if (input_order) return false;
-        return P.item_headers[a].n > P.item_headers[b].n;          // heaviest first
+        return weight(a) > weight(b);                                  // heaviest first
     });
-    for (int64_t i = 0; i < nitems; ++i) P.class_count[P.item_class[P.item_launch_order[i]]]++;
-    for (int q = 1; q < ncls; ++q) P.class_first[q] = P.class_first[q - 1] + P.class_count[q - 1];
+    // blocks of every class in launch order
+    const int ncls = (int)P.class_smem_bytes.size();
+    P.class_first.assign(ncls, 0);
+    P.class_count.assign(ncls, 0);
+    for (int k = 0; k < ncls; ++k) {
+        const Cls& c = qs[k];
+        P.class_first[k] = (int64_t)P.class_parts.size();
+        for (int32_t it : P.item_launch_order) {
+            const int64_t p0 = P.item_part_offsets[it], p1 = P.item_part_offsets[it + 1];
+            if (c.phase == kPhaseAll) {
+                if (need[it].kind == kItemSplit || item_q[it] != c.q) continue;
+                for (int64_t p = p0; p < p1; ++p) P.class_parts.push_back((int32_t)p);
+            } else if (need[it].kind == kItemSplit) {
+                if (c.phase == kPhaseB) { if (qSplitTop + slot_of(need[it].smem_top) == c.q) P.class_parts.push_back((int32_t)p0); }
+                else if (item_q[it] == c.q) for (int64_t p = p0 + 1; p < p1; ++p) P.class_parts.push_back((int32_t)p);
+            }
+        }
+        P.class_count[k] = (int64_t)P.class_parts.size() - P.class_first[k];
+    }
 }
 
 static void build_stream(hines_plan& P, const std::vector<char>& is_stream)
@@ -860,7 +954,6 @@ static void build_stream(hines_plan& P, const std::vector<char>& is_stream)
     }
     P.stream_level_begin[maxlev] = (int64_t)P.stream_desc.size();
 }
-
 }  // namespace hines
 
 using namespace hines;
@@ -889,11 +982,12 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (auto_segment) o.max_segment = 64;
     if (o.cluster_max == 0) o.cluster_max = 16;
     if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 113 * 1024;
+    if (o.split_smem_bytes == 0) o.split_smem_bytes = 113 * 1024;
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~63) ||
-        o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024) {
+        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~1023) ||
+        o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024 || o.split_smem_bytes < 8192) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }
     if (cell_offsets[0] != 0) { set_error("cell_offsets[0] must be 0"); return HINES_ERR_BAD_TOPOLOGY; }
@@ -904,20 +998,22 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         }
     if (cell_offsets[ncells] >= (int64_t)1 << 31) { set_error("N >= 2^31 is not supported"); return HINES_ERR_INVALID_ARG; }
     try {
-        hines_plan* P = new hines_plan();
+        std::unique_ptr<hines_plan> holder(new hines_plan());
+        hines_plan* P = holder.get();
         P->n = cell_offsets[ncells]; P->ncells = ncells; P->dtype = dtype; P->width = dtype == HINES_F64 ? 8 : 4;
         P->opt = o;
         P->seg_cluster = o.max_segment;
         P->seg_single = auto_segment ? 40 : o.max_segment;
         P->cell_offsets.assign(cell_offsets, cell_offsets + ncells + 1);
         hines_status_t st = canonical_tables(*P, parent);
-        if (st != HINES_OK) { delete P; return st; }
+        if (st != HINES_OK) return st;
+        level_mean_split(*P);
         std::vector<ItemNeed> item_need;
         std::vector<char> is_stream;
         pack_items(*P, item_need, is_stream);
         assign_classes(*P, item_need);
         build_stream(*P, is_stream);
-        *out_plan = P;
+        *out_plan = holder.release();
         return HINES_OK;
     } catch (const std::bad_alloc&) {
         set_error("host allocation failed while building the plan"); return HINES_ERR_ALLOC;
@@ -932,21 +1028,23 @@ hines_status_t hines_plan_get_info(const hines_plan_t* P, hines_plan_info_t* out
     std::memset(out, 0, sizeof(*out));
     out->n = P->n; out->ncells = P->ncells; out->nbranches = P->nbranches;
     out->max_levels = P->max_levels; out->dtype = P->dtype;
-    out->n_resident_items = (int64_t)P->item_class.size();
+    out->n_resident_items = (int64_t)P->item_kind.size();
     out->n_resident_cells = P->n_resident_cells; out->n_resident_unknowns = P->n_resident_unknowns;
     out->n_stream_cells = P->n_stream_cells; out->n_stream_unknowns = P->n_stream_unknowns;
     out->n_stream_branches = (int64_t)P->stream_desc.size();
     out->padded_lane_steps = P->padded_lane_steps; out->useful_lane_steps = P->useful_lane_steps;
-    out->workspace_bytes = (int64_t)(P->item_meta.size() * 4 + P->item_headers.size() * sizeof(ItemHeader) +
-                                     P->chunk_headers.size() * sizeof(ChunkHeader) +
-                                     P->item_launch_order.size() * 4 + P->stream_desc.size() * sizeof(StreamDesc) +
+    out->workspace_bytes = (int64_t)(P->part_meta.size() * 4 + P->part_runs.size() * 4 + P->class_parts.size() * sizeof(PartHeader) +
+                                     3 * P->n_xch * P->width + P->class_parts.size() * (sizeof(BlockRecord) - sizeof(PartHeader)) + P->stream_desc.size() * sizeof(StreamDesc) +
                                      P->stream_child.size() * 4 + 2 * P->n_stream_unknowns * P->width);
     out->bytes_min = P->n * 4 * P->width + 4 * P->nbranches;
     out->bytes_literal = P->n * (4 * P->width + 4);
     out->breadth_first = P->breadth_first;
     out->n_classes = (int32_t)P->class_smem_bytes.size();
     out->n_cluster_cells = P->n_cluster_cells; out->n_cluster_unknowns = P->n_cluster_unknowns;
-    out->n_chunks = (int64_t)P->chunk_headers.size();
+    out->n_parts = (int64_t)P->part_headers.size();
+    out->n_split_cells = P->n_split_cells; out->n_split_unknowns = P->n_split_unknowns;
+    out->n_exports = P->n_exports;
+    out->n_blocks = (int64_t)P->class_parts.size();
     return HINES_OK;
 }
 
@@ -972,16 +1070,20 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_ITEM_CELL_RANGE, P->item_cell_range)
         TBL(HINES_TABLE_ITEM_CLASS, P->item_class)
         TBL(HINES_TABLE_ITEM_LAUNCH_ORDER, P->item_launch_order)
-        TBL(HINES_TABLE_ITEM_PNODE, P->item_pnode)
-        TBL(HINES_TABLE_ITEM_NODE_OFFSETS, P->item_node_offsets)
-        TBL(HINES_TABLE_ITEM_ROUNDS, P->item_rounds)
-        TBL(HINES_TABLE_ITEM_TASK_OFFSETS, P->item_task_offsets)
-        TBL(HINES_TABLE_ITEM_TASK_BLOB, P->item_task_blob)
-        TBL(HINES_TABLE_ITEM_NNODE, P->item_nnode)
-        TBL(HINES_TABLE_ITEM_CHUNK_OFFSETS, P->item_chunk_offsets)
-        TBL(HINES_TABLE_CHUNK_COMP_RANGE, P->chunk_comp_range)
-        TBL(HINES_TABLE_CHUNK_SEG_OFFSETS, P->chunk_seg_offsets)
-        TBL(HINES_TABLE_CHUNK_SEG, P->chunk_seg)
+        TBL(HINES_TABLE_ITEM_KIND, P->item_kind)
+        TBL(HINES_TABLE_ITEM_XCH, P->item_xch)
+        TBL(HINES_TABLE_ITEM_PART_OFFSETS, P->item_part_offsets)
+        TBL(HINES_TABLE_PART_HEADER, P->part_headers)
+        TBL(HINES_TABLE_PART_META, P->part_meta)
+        TBL(HINES_TABLE_PART_RUNS, P->part_runs)
+        TBL(HINES_TABLE_CLASS_PHASE, P->class_phase)
+        TBL(HINES_TABLE_CLASS_FIRST, P->class_first)
+        TBL(HINES_TABLE_CLASS_COUNT, P->class_count)
+        TBL(HINES_TABLE_CLASS_PARTS, P->class_parts)
+        TBL(HINES_TABLE_SPLIT_PIECE_OFFSETS, P->split_piece_offsets)
+        TBL(HINES_TABLE_SPLIT_PIECE_LEN, P->split_piece_len)
+        TBL(HINES_TABLE_SPLIT_PIECE_LEVEL, P->split_piece_level)
+        TBL(HINES_TABLE_SPLIT_LEVEL_STAT, P->split_level_stat)
         TBL(HINES_TABLE_CLASS_CLUSTER, P->class_cluster)
         TBL(HINES_TABLE_CLASS_THREADS, P->class_threads)
         TBL(HINES_TABLE_STREAM_LEVEL_BEGIN, P->stream_level_begin)
@@ -1001,7 +1103,9 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
 hines_status_t hines_plan_launches_per_solve(const hines_plan_t* P, int32_t* out)
 {
     if (!P || !out) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
-    *out = (int32_t)P->class_smem_bytes.size() + 2 * (int32_t)(P->stream_level_begin.size() - 1);
+    int32_t k = 0;
+    for (size_t q = 0; q < P->class_count.size(); ++q) if (P->class_count[q]) ++k;
+    *out = k + 2 * (int32_t)(P->stream_level_begin.size() - 1);
     return HINES_OK;
 }
 
@@ -1019,6 +1123,6 @@ const char* hines_status_string(hines_status_t s)
 }
 
 const char* hines_last_error(void) { return g_last_error.c_str(); }
-const char* hines_version(void) { return "hines-b200 0.1 (sm_100a)"; }
+const char* hines_version(void) { return "hines-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

@@ -1,15 +1,18 @@
 // hines_solve: the per-step kernels (sm_100a) and their host launcher.
 //
 // Two paths, chosen per cell by the plan:
-//   resident  whole cells / cell groups staged into shared memory by TMA bulk copies
-//             (cp.async.bulk + mbarrier), level-synchronous sweeps with one lane per branch
-//             (PAPER.md:110-114), block barrier per level, sibling hand-off by warp shuffle,
-//             x written back by a bulk store.  d,u,b are read from and x written to the caller's
-//             natural-order arrays directly: the paper's separate permute kernels
-//             do not exist here.
-//   stream    cells too large for one block's shared memory: one launch per level over all such
-//             cells (global synchronisation = kernel boundary, which PAPER.md:114 avoids by
-//             requiring one matrix per block), intermediates in a plan-owned global workspace.
+//   resident  whole cells / cell groups, or the parts of a large cell, staged into shared memory by TMA bulk
+//             copies (cp.async.bulk + mbarrier) of their runs of consecutive compartments.  Segment interiors
+//             are condensed before (P1) and expanded after (P3) the level-synchronous sweeps (P2) over the
+//             reduced forest of the part: one node per segment, one thread per node, a block barrier per
+//             level, the parent pulling its children's hand-off values.
+//             Parts of one cell exchange two values per exported sub-tree root through distributed shared
+//             memory (cluster items) or a global exchange buffer between launches (split items).  d,u,b are
+//             read from and x written to the caller's natural-order arrays directly: the paper's separate
+//             permute kernels do not exist here.
+//   stream    cells that fit none of this: one launch per level over all such cells (global synchronisation
+//             = kernel boundary, which PAPER.md:114 avoids by requiring one matrix per block), intermediates
+//             in a plan-owned global workspace.
 //
 // Arithmetic per compartment i with parent/previous compartment q (Listing 2 read
 // with u[i], reading G1), written with the reciprocal r = 1/d'[i] (reading S12):
@@ -32,25 +35,30 @@
 
 namespace hines {
 
-struct BlockRec { ItemHeader it; ChunkHeader ch; };   // 80 bytes
-
 struct DeviceTables {
-    int device = -1;
-    BlockRec* recs = nullptr;                                     // one per resident block, launch order
-    int32_t* item_meta = nullptr;
+    int device = -1, num_sms = 148;
+    BlockRecord* recs = nullptr;                                  // one per launched block, launch order (class by class)
+    int32_t* meta = nullptr;
+    int4* runs = nullptr;
+    void* xch_h = nullptr;          // split items: exported hand-off values (2 per slot)
+    void* xch_x = nullptr;          // split items: the parent's x of every exported sub-tree root
     StreamDesc* stream_desc = nullptr;
     int32_t* stream_child = nullptr;
     void* ws_f = nullptr;           // streaming workspace: f (n_stream_unknowns elements)
     void* ws_c = nullptr;           // streaming workspace: c
     void* host_stage[4] = {nullptr, nullptr, nullptr, nullptr};   // hines_solve_host device buffers d,u,b,x
-    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};              // timing hook
+    cudaStream_t copy_stream = nullptr;                           // hines_solve_host: D2H of x beside the H2D of the next slice
+    cudaEvent_t slice_ev[2] = {nullptr, nullptr};
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};     // timing hook: resident start/end on the caller's stream, streaming start/end
     static const int kSide = 3;                                   // side streams: size classes run concurrently
     cudaStream_t side[kSide] = {nullptr, nullptr, nullptr};
     cudaEvent_t fork = nullptr, join[kSide] = {nullptr, nullptr, nullptr};
     cudaStream_t sstream = nullptr;                               // the streaming path runs beside the resident classes
     cudaEvent_t sjoin = nullptr;
+    cudaStream_t pstream = nullptr;                               // the three phases of split items, in order, beside the rest
+    cudaEvent_t pjoin = nullptr;
     bool timing = false, timed_once = false;
-    unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per resident block, launch order
+    unsigned long long* prof = nullptr;                           // phase clocks: 8 x u64 per launched block, launch order
     bool prof_on = false;
     int64_t bytes = 0;
 };
@@ -63,7 +71,6 @@ struct DeviceTables {
             return e_ == cudaErrorMemoryAllocation ? HINES_ERR_ALLOC : HINES_ERR_CUDA;         \
         }                                                                                      \
     } while (0)
-
 
 // ------------------------------------------------------------------------------------------------
 // PTX helpers: mbarrier + 1-D TMA bulk copies (SASS: UBLKCP, SYNCS)
@@ -162,6 +169,10 @@ template <> __device__ __forceinline__ double lds1<double>(uint32_t a)
 { double v; asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a) : "memory"); return v; }
 template <> __device__ __forceinline__ float lds1<float>(uint32_t a)
 { float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ int ldsi1(uint32_t a)
+{ int v; asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
+__device__ __forceinline__ int4 ldsi4(uint32_t a)
+{ int4 v; asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(a) : "memory"); return v; }
 template <typename T> __device__ __forceinline__ void sts1(uint32_t a, T v);
 template <> __device__ __forceinline__ void sts1<double>(uint32_t a, double v)
 { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
@@ -176,98 +187,306 @@ template <typename T> __device__ __forceinline__ T fmad(T a, T b, T c);   // c +
 template <> __device__ __forceinline__ double fmad<double>(double a, double b, double c) { return fma(a, b, c); }
 template <> __device__ __forceinline__ float fmad<float>(float a, float b, float c) { return fmaf(a, b, c); }
 
+// split-phase cluster barrier (every thread of every block of the cluster arrives and waits, in turn)
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+
+
+// P2 backward over the levels lfrom .. lto of a part's reduced forest: deepest level first, one
+// thread per node, a block barrier per level; a node pulls the hand-off values of its children.
+// topsel selects the nodes of this sweep: 0 = nodes that do not wait for another part, 1 = top nodes (the
+// ancestors of ghost children).  What the critical warp executes between two barriers is what a level costs
+// (a lone warp issues dependent code at about 5 cycles per instruction), so the step is kept short: the plan
+// stores, per node, the byte offsets of its first two children's hand-off slots (the all-zero record when there is
+// none: no branch), more than two children are rare and take a loop; the record and descriptor of a thread's node
+// on the NEXT level are fetched after this level's stores and land while the barrier is pending.
+// Node record: {D -> g = -f, B -> c, -U, -, parked d -> hand-off d, parked b -> hand-off b}.
+__device__ __forceinline__ void named_barrier(int nthreads_in)
+{
+    asm volatile("bar.sync 1, %0;" ::"r"(nthreads_in) : "memory");
+}
+
+template <typename T>
+__device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int lfrom, int lto,
+                                               int topsel, int maxwidth, int tid, int nthreads)
+{
+    typedef typename Vec2<T>::type V2;
+    constexpr uint32_t W = (uint32_t)sizeof(T), RS = 6u * W;
+    if (lfrom < lto) return;
+    if (maxwidth <= nthreads) {
+        // No level is wider than the block: at most one node per thread and level, and only the warps that can ever
+        // hold a node take part (named barrier over those; the others wait at the block barrier behind the sweep).
+        const int pthreads = (maxwidth + 31) & ~31;
+        if (tid < pthreads) {
+            int lo = ldsi1(lb_sa + 4u * (uint32_t)lfrom), hi = ldsi1(lb_sa + 4u * (uint32_t)(lfrom + 1));
+            int lo_n = lfrom > lto ? ldsi1(lb_sa + 4u * (uint32_t)(lfrom - 1)) : 0;
+            int v = lo + tid;
+            int4 k = make_int4(0, 0, -1, 0);
+            V2 a0, a2; T Un = T(0);
+            a0.x = T(1); a0.y = T(0); a2.x = T(0); a2.y = T(0);
+            uint32_t qa = nd_sa + (uint32_t)v * RS;
+            bool have = false;
+            if (v < hi) {
+                k = ldsi4(kp_sa + 16u * (uint32_t)v); a0 = lds2<T>(qa); Un = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
+                have = k.z >= 0 && ((k.z >> 29) & 1) == topsel;
+            }
+#pragma unroll 1
+            for (int l = lfrom; l >= lto; --l) {
+                const int lo_nn = l > lto + 1 ? ldsi1(lb_sa + 4u * (uint32_t)(l - 2)) : 0;     // two levels ahead: off the chain
+                if (have) {
+                    const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
+                    T D = a0.x - h0.x, B = a0.y - h0.y;
+                    D -= h1.x; B -= h1.y;
+                    int nc = k.z & 0xfff;
+                    if (nc > 2) {                           // more than two children: the rest, consecutive records
+                        uint32_t ca = nd_sa + (uint32_t)k.y + RS;
+                        for (nc -= 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
+                    }
+                    const T r = rcp<T>(D);
+                    const T g = Un * r;                     // -f
+                    V2 o; o.x = g; o.y = B * r;
+                    sts2<T>(qa, o);
+                    V2 s2; s2.x = fmad<T>(g, Un, a2.x); s2.y = fnma<T>(g, B, a2.y);
+                    sts2<T>(qa + 4u * W, s2);
+                }
+                hi = lo; lo = lo_n; lo_n = lo_nn;
+                v = lo + tid;
+                qa = nd_sa + (uint32_t)v * RS;
+                have = false;
+                if (l > lto && v < hi) {                    // this thread's node on the next level: lands while the barrier is pending
+                    k = ldsi4(kp_sa + 16u * (uint32_t)v); a0 = lds2<T>(qa); Un = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
+                    have = k.z >= 0 && ((k.z >> 29) & 1) == topsel;
+                }
+                named_barrier(pthreads);
+            }
+        }
+        __syncthreads();
+        return;
+    }
+    // a level wider than the block: every thread loops over the level's nodes
+#pragma unroll 1
+    for (int l = lfrom; l >= lto; --l) {
+        const int hi = ldsi1(lb_sa + 4u * (uint32_t)(l + 1));
+        for (int v = ldsi1(lb_sa + 4u * (uint32_t)l) + tid; v < hi; v += nthreads) {
+            const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
+            if (k.z >= 0 && ((k.z >> 29) & 1) == topsel) {
+                const uint32_t qa = nd_sa + (uint32_t)v * RS;
+                const V2 a0 = lds2<T>(qa), a2 = lds2<T>(qa + 4u * W);
+                const T Un = lds1<T>(qa + 2u * W);
+                const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
+                T D = a0.x - h0.x, B = a0.y - h0.y;
+                D -= h1.x; B -= h1.y;
+                uint32_t ca = nd_sa + (uint32_t)k.y + RS;
+                for (int nc = (k.z & 0xfff) - 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
+                const T r = rcp<T>(D);
+                const T g = Un * r;
+                V2 o; o.x = g; o.y = B * r;
+                sts2<T>(qa, o);
+                V2 s2; s2.x = fmad<T>(g, Un, a2.x); s2.y = fnma<T>(g, B, a2.y);
+                sts2<T>(qa + 4u * W, s2);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// P2 forward over the top nodes only, level by level from the root: x_v = c_v + g_v x_parent.
+// The other parts of the cell wait for exactly these values; everything below the top nodes follows by pointer
+// jumping afterwards.  A finished node holds {g, c} = {0, x}.
+template <typename T>
+__device__ __forceinline__ void sweep_forward_top(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int ntoplev, int maxwidth,
+                                                  int tid, int nthreads)
+{
+    typedef typename Vec2<T>::type V2;
+    constexpr uint32_t W = (uint32_t)sizeof(T), RS = 6u * W;
+    if (ntoplev <= 0) return;
+    if (maxwidth <= nthreads) {                             // one node per thread and level at most: see sweep_backward
+        const int pthreads = (maxwidth + 31) & ~31;
+        if (tid < pthreads) {
+            int lo = ldsi1(lb_sa), hi = ldsi1(lb_sa + 4u), hi_n = ldsi1(lb_sa + 8u);
+            int v = lo + tid;
+            uint32_t qa = nd_sa + (uint32_t)v * RS, pa = qa + W;
+            V2 gc; gc.x = T(0); gc.y = T(0);
+            bool have = false;
+            if (v < hi) {
+                const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
+                gc = lds2<T>(qa); pa = nd_sa + (uint32_t)k.w * RS + W;
+                have = k.z >= 0 && ((k.z >> 29) & 1);
+            }
+#pragma unroll 1
+            for (int l = 0; l < ntoplev; ++l) {
+                const int hi_nn = l + 2 < ntoplev ? ldsi1(lb_sa + 4u * (uint32_t)(l + 3)) : 0;
+                if (have) {
+                    const T xp = lds1<T>(pa);               // a root reads its own c: g = 0 there
+                    V2 o; o.x = T(0); o.y = fmad<T>(gc.x, xp, gc.y);
+                    sts2<T>(qa, o);
+                }
+                lo = hi; hi = hi_n; hi_n = hi_nn;
+                v = lo + tid;
+                qa = nd_sa + (uint32_t)v * RS;
+                have = false;
+                if (l + 1 < ntoplev && v < hi) {
+                    const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
+                    gc = lds2<T>(qa); pa = nd_sa + (uint32_t)k.w * RS + W;
+                    have = k.z >= 0 && ((k.z >> 29) & 1);
+                }
+                named_barrier(pthreads);
+            }
+        }
+        __syncthreads();
+        return;
+    }
+#pragma unroll 1
+    for (int l = 0; l < ntoplev; ++l) {
+        const int hi = ldsi1(lb_sa + 4u * (uint32_t)(l + 1));
+        for (int v = ldsi1(lb_sa + 4u * (uint32_t)l) + tid; v < hi; v += nthreads) {
+            const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
+            if (k.z >= 0 && ((k.z >> 29) & 1)) {
+                const uint32_t qa = nd_sa + (uint32_t)v * RS;
+                const V2 gc = lds2<T>(qa);
+                const T xp = lds1<T>(nd_sa + (uint32_t)k.w * RS + W);
+                V2 o; o.x = T(0); o.y = fmad<T>(gc.x, xp, gc.y);
+                sts2<T>(qa, o);
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Unbranched cables (the degenerate single-branch case): the reduced system of a cable is tridiagonal, one row per
+// segment, and is solved inside ONE warp by parallel cyclic reduction: lane i holds row i = {a, b, c, d} (couplings
+// to rows i-1 and i+1, pivot, right-hand side); a step with stride s eliminates the couplings to i-s and i+s
+// (a' = -a ra[i-s], c' = -c rc[i+s], b' = b - a rc[i-s] - c ra[i+s], d' = d - a rd[i-s] - c rd[i+s], with
+// ra = a/b, rc = c/b, rd = d/b of the source rows); after ceil(log2 m) steps x = d / b.  5 steps for the 25
+// segments of a 1,000-compartment cable, instead of 25 dependent levels.  The matrix is strictly diagonally
+// dominant and every step keeps it so.
+template <typename T>
+__device__ __forceinline__ void solve_cables_pcr(T* nd, const int32_t* cb, int ncables, int tid, int nthreads)
+{
+    const unsigned FULL = 0xffffffffu;
+    const int lane = tid & 31, nwarps = nthreads >> 5;
+    for (int c = tid >> 5; c < ncables; c += nwarps) {
+        const int n0 = cb[c], m = cb[c + 1] - n0;
+        T a = T(0), bb = T(1), cc = T(0), dd = T(0), pd = T(0), pb = T(0);
+        if (lane < m) {
+            const T* q = nd + 6 * (n0 + lane);
+            bb = q[0]; dd = q[1]; a = -q[2]; pd = q[4]; pb = q[5];      // record slot 2 holds -U
+        }
+        // the interior of segment i+1 left its contribution to its top = row i; row i+1's coupling is row i's c
+        const T pdn = __shfl_down_sync(FULL, pd, 1), pbn = __shfl_down_sync(FULL, pb, 1), an = __shfl_down_sync(FULL, a, 1);
+        if (lane + 1 < m) { bb -= pdn; dd -= pbn; cc = an; }
+        if (lane == 0) a = T(0);
+#pragma unroll 1
+        for (int s = 1; s < m; s <<= 1) {
+            const T r = rcp<T>(bb);
+            const T ra = a * r, rc = cc * r, rd = dd * r;
+            const T ra_u = __shfl_up_sync(FULL, ra, s), rc_u = __shfl_up_sync(FULL, rc, s), rd_u = __shfl_up_sync(FULL, rd, s);
+            const T ra_d = __shfl_down_sync(FULL, ra, s), rc_d = __shfl_down_sync(FULL, rc, s), rd_d = __shfl_down_sync(FULL, rd, s);
+            const bool up = lane >= s, dn = lane + s < 32;
+            const T au = up ? a : T(0), cd = dn ? cc : T(0);
+            bb = fnma<T>(au, rc_u, fnma<T>(cd, ra_d, bb));
+            dd = fnma<T>(au, rd_u, fnma<T>(cd, rd_d, dd));
+            a = -au * ra_u;
+            cc = -cd * rc_d;
+        }
+        if (lane < m) nd[6 * (n0 + lane) + 1] = dd * rcp<T>(bb);
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
-// Resident kernel: one block per chunk; an item is one block, or one cluster of blocks (CL).
+// Resident kernel: one block per part; an item is one block, one cluster of blocks (CL), or the
+// blocks of three launches (split items, `phase`).
 //
 // Shared memory of a block (bytes):
-//   [0,16) mbarrier
-//   rank 0 only:  nd[5 NN]  the reduced tree (one node per segment: its separator; per node the
-//                 record {D -> f, B -> c -> x, U, pd, pb}), NN = nodes rounded up | item metadata
-//                 (level_begin, branch desc, pnode)
-//   sd[L] su[L] sb[L]  the chunk's d, u, b in natural order, L = chunk range widened to 16-byte
-//                 boundaries; compartment j of the chunk sits at index j + off | segment descriptors
-// Blocks of rank > 0 write their separators into rank 0's reduced arrays through distributed shared
-// memory and read the separators' solution back from there.
+//   [0,16) mbarrier | [16,528) the block's record (header + first runs) | nd[6 NN] node records of the part's reduced forest
+//   {D -> -f, B -> c -> x, U, -, parked d -> hand-off d, parked b -> hand-off b}, NN = nodes rounded up |
+//   metadata blob (level starts, {kids, parent} per node, exports, ghosts, segment lanes) |
+//   sd[L] su[L] sb[L]  the part's runs of d, u, b, one after the other, each at an index with the parity
+//   of its global index.
 //
-// Phases (DESIGN.md "Condensation"):
+// Phases (DESIGN.md section 4):
 //   P1 condense   every segment's interior a..b-1 is eliminated top-down, independently of the tree
-//                 level (one lane per segment).  Node i keeps g = u[i+1]/D, h = e/D, c = B/D where e is
+//                 level (two lanes per segment).  Node i keeps g = u[i+1]/D, h = e/D, c = B/D where e is
 //                 the fill-in coupling to the separator t above the segment.  What is left of the
 //                 separator b (pivot, right-hand side, coupling U to t) and the interior's contribution
-//                 to t (sum h e, sum h B) go to the reduced arrays.
-//   P2 reduced    the level-synchronous Hines sweeps of the paper on the reduced
-//                 tree: one lane per branch, one step per segment, block barrier per level; at a branch
-//                 point the siblings' hand-off values are summed by warp shuffles and the parent pulls
-//                 the sum.
-//   P3 expand     x[i] = c - g x[i+1] - h x[t] for every interior, again one lane per segment.
+//                 to t (sum h e, sum h B) go to the segment's node record.
+//   P2 backward   the level-synchronous sweep of the paper over the reduced forest,
+//                 deepest level first: one thread per node, a block barrier per level; a node pulls the
+//                 hand-off values of its children (consecutive records), in ascending order:
+//                 D -= sum hd; B -= sum hb; r = 1/D; f = U r; c = B r; hand-off = (f U + parked d, f B + parked b).
+//                 A root has U = 0, so f = 0 and x = c.
+//      exchange   the root of a sub-tree held by another block hands its value to a ghost child in the
+//                 top part and later reads its parent's x into a ghost parent (cluster: distributed
+//                 shared memory; split items: global exchange buffers between launches).
+//   P2 forward    x_v = c_v - f_v x_parent by pointer jumping over the forest.
+//   P3 expand     x[i] = c - g x[i+1] - h x[t] for every interior, the same two lanes per segment.
 // Eliminating in this order is a symmetric permutation of the same LDL^T factorisation (the matrix is
 // SPD and strictly diagonally dominant, so any order is stable without pivoting).
 // ------------------------------------------------------------------------------------------------
 template <typename T, bool CL>
 __global__ void __launch_bounds__(384, 2)
-hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restrict__ meta_g,
+hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __restrict__ meta_g, const int4* __restrict__ runs_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
-                      int64_t n_total, unsigned long long* prof)
+                      int64_t n_total, T* xch_h, T* xch_x, int phase, unsigned long long* prof)
 {
     extern __shared__ __align__(128) unsigned char smem[];
     namespace cg = cooperative_groups;
+    typedef typename Vec2<T>::type V2;
     // phase clocks (debug hook, prof == nullptr in normal runs): thread 0 stamps %globaltimer
     unsigned long long stamp[7];
 #define HINES_STAMP(k) do { if (prof && threadIdx.x == 0) stamp[k] = globaltimer_ns(); } while (0)
     HINES_STAMP(0);
     constexpr int E = 16 / (int)sizeof(T);
-    unsigned rank = 0, csize = 1;
-    if (CL) { rank = cg::this_cluster().block_rank(); csize = cg::this_cluster().num_blocks(); }
-    // one record per block, in launch order: the block's item and chunk headers side by side, so that
-    // a single dependent global load stands between the block's start and its bulk copies
-    const ItemHeader it = recs[blockIdx.x].it;
-    const ChunkHeader ch = recs[blockIdx.x].ch;
-    (void)csize;
+    constexpr uint32_t W = (uint32_t)sizeof(T);
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
-    const int off = (int)(ch.comp_begin % E);
-    const int64_t g0 = ch.comp_begin - off;                 // 16-byte aligned global element index
-    const int L = (off + ch.n + E - 1) / E * E;             // landed elements
-    // the last chunk may end beyond a 16-byte boundary of the arrays: copy that remainder by hand
-    const int64_t avail = n_total - g0;
-    const int Lb = (int)(avail >= L ? L : (avail / E * E)); // elements brought by the bulk copies
-    const int NN = (it.nnode + E - 1) / E * E;
-
+    unsigned rank = 0;
+    if (CL) { rank = cg::this_cluster().block_rank(); cluster_arrive(); }     // barrier 0: every block of the cluster is running
+    // One 512-byte record per block, in launch order: the part's header and its first runs side by side, so that a
+    // single dependent global load stands between the block's start and its bulk copies.
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
-    // rank 0's layout of the reduced arrays; the same offsets address rank 0's memory from any rank
-    // node record: 6 values {D -> -f, B -> c, U, -, pd, pb}; the forward sweep reuses them as two
-    // {g, c} buffers and two parent ids
-    T* nd = reinterpret_cast<T*>(smem + 16);
-    int32_t* imeta = reinterpret_cast<int32_t*>(nd + 6 * NN);
-    unsigned char* chunk_base = rank == 0 ? reinterpret_cast<unsigned char*>(imeta + it.meta_len) : smem + 16;
-    T* sd = reinterpret_cast<T*>(chunk_base);
-    T* su = sd + L;
-    T* sb = su + L;
-    const int4* seg = reinterpret_cast<const int4*>(sb + L);
-
+    const PartHeader& H = *reinterpret_cast<const PartHeader*>(smem + 16);
+    const int4* myruns = reinterpret_cast<const int4*>(smem + 16 + sizeof(PartHeader));
+    if (tid < 32) reinterpret_cast<int4*>(smem + 16)[tid] = reinterpret_cast<const int4*>(recs + blockIdx.x)[tid];
     if (tid == 0) mbar_init(bar, 1);
     __syncthreads();
+    const int L = H.L, NN = (H.nnode + 1 + E - 1) / E * E;    // one all-zero record behind the last node
+    T* nd = reinterpret_cast<T*>(smem + 16 + sizeof(BlockRecord));
+    int32_t* meta = reinterpret_cast<int32_t*>(nd + 6 * NN);
+    T* sd = reinterpret_cast<T*>(meta + H.meta_len);
+    T* su = sd + L;
+    T* sb = su + L;
+    const int4* seg = reinterpret_cast<const int4*>(meta + H.seg_off);
+    const int nseg_lanes = H.nseg_lanes, nrun = H.nrun;
+
     if (tid == 0) {
-        const uint32_t bytes = (uint32_t)Lb * sizeof(T);
-        const uint32_t mbytes = rank == 0 ? (uint32_t)it.meta_len * 4u : 0u;
-        const uint32_t sbytes = (uint32_t)ch.nseg_lanes * 16u;
-        mbar_expect_tx(bar, 3u * bytes + mbytes + sbytes);
-        if (sbytes) tma_load_1d(const_cast<int4*>(seg), meta_g + ch.seg_off, sbytes, bar);
-        if (bytes) {
-            tma_load_1d(sd, d + g0, bytes, bar);
-            tma_load_1d(sb, b + g0, bytes, bar);
-            tma_load_1d(su, u + g0, bytes, bar);
+        mbar_expect_tx(bar, 3u * (uint32_t)H.tx_elems * W + (uint32_t)H.meta_len * 4u);
+        tma_load_1d(meta, meta_g + H.meta_off, (uint32_t)H.meta_len * 4u, bar);
+    }
+    __syncthreads();                                        // the expected byte count is set before any copy can complete
+    {
+        // a run [g, g+len) is brought as the 16-byte words that cover it (neighbouring compartments come along
+        // and are ignored); words beyond the end of the arrays are not touched: that remainder by plain loads
+        // (a bulk-copy instruction costs its warp ~70 cycles per active lane: one run per warp, its three arrays by
+        // lanes 0-2, so that the copies of a part with many runs are issued by all warps side by side)
+        const int64_t gemax = n_total / E * E;
+        const int nwarps = nthreads >> 5, warp = tid >> 5;
+        for (int r = warp; r < nrun; r += nwarps) {
+            const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
+            const int64_t g = rd.x, gend = g + rd.y;
+            const int64_t ga = g & ~(int64_t)(E - 1);
+            int64_t ge = (gend + E - 1) / E * E;
+            if (ge > gemax) ge = gemax;
+            const int sdst = rd.z - (int)(g - ga);
+            if (ge > ga && lane < 3) {
+                const uint32_t bytes = (uint32_t)(ge - ga) * W;
+                const T* src = lane == 0 ? d : (lane == 1 ? b : u);
+                T* dst = lane == 0 ? sd : (lane == 1 ? sb : su);
+                tma_load_1d(dst + sdst, src + ga, bytes, bar);
+            }
+            if (lane == 3) for (int64_t i = ge > ga ? ge : ga; i < gend; ++i) { const int k = sdst + (int)(i - ga); sd[k] = d[i]; su[k] = u[i]; sb[k] = b[i]; }
         }
-        if (mbytes) tma_load_1d(imeta, meta_g + it.meta_off, mbytes, bar);
     }
-    // remainder of the very last chunk (fewer than E elements), plain loads
-    for (int i = Lb + tid; i < L && g0 + i < n_total; i += nthreads) { sd[i] = d[g0 + i]; su[i] = u[g0 + i]; sb[i] = b[g0 + i]; }
-    // reduced arrays as seen from this block
-    T* ND = nd;
-    if (CL) {
-        cg::cluster_group cluster = cg::this_cluster();
-        ND = cluster.map_shared_rank(nd, 0);
-        cluster.sync();                                     // every block of the cluster is running
-    }
+    if (tid < 2) nd[6 * H.nnode + 4 + tid] = T(0);          // the all-zero record: hand-off slot of a child that is not there
     mbar_wait(bar, 0);
     __syncthreads();
     HINES_STAMP(1);
@@ -278,7 +497,7 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
     // eliminates a..q-1 top-down with fill-in coupling to t and arrives at q; lane B = A ^ 16 eliminates
     // q+1..b-1 top-down with fill-in coupling to q and arrives at b.  A then takes B's contribution to q,
     // eliminates q (couplings to t and to b) and writes the node record of b.  Both lanes run the same code.
-    for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
+    for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
@@ -286,14 +505,13 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         const int m = isB ? mb : (kind == 1 ? mt : 0);
         const int dl = (sg.y >> 27) & 15;                   // the lane starts dl steps late (bank residues, plan.cpp)
         const int mmax = __reduce_max_sync(FULL, m + dl);
-        int i = sg.x + off;
+        int i = sg.x;
         T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
         if (kind == 1 || (isB && hasq)) { D = sd[i]; B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
         if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; bn = sb[i + 1]; }
         {
             // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
             // loop is unrolled by two with the two register sets swapping roles (no register rotation).
-            constexpr uint32_t W = (uint32_t)sizeof(T);
             const uint32_t LW = (uint32_t)L * W;
             uint32_t pa = smem_u32(sd + i), pu = pa + LW, pb = pa + 2u * LW;
             T un2 = un, dn2 = dn, bn2 = bn;                 // a lane's first step may fall on either half of the loop body
@@ -320,208 +538,123 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
         const T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
         if (kind == 1) {
-            T* q = ND + 6 * sg.z;
+            T* q = nd + 6 * sg.z;
             if (hasq) {                                     // i is q now
                 const T Dq = D - pdd, Bq = B - pdb;
                 const T r = rcp<T>(Dq);
                 const T gq = pe * r, hq = ee * r;
                 sd[i] = gq; su[i] = hq; sb[i] = Bq * r;
                 ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
-                q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = -hq * pe; q[4] = ddt; q[5] = dbt;
+                q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = hq * pe; q[4] = ddt; q[5] = dbt;     // slot 2 = -U
             } else {                                        // a segment of one compartment: the separator as it is
-                q[0] = D; q[1] = B; q[2] = ee; q[4] = T(0); q[5] = T(0);
+                q[0] = D; q[1] = B; q[2] = -ee; q[4] = T(0); q[5] = T(0);
             }
         }
     }
-    if (CL) cg::this_cluster().sync(); else __syncthreads();
+    __syncthreads();
     HINES_STAMP(2);
 
-    if (rank == 0) {
-        typedef typename Vec2<T>::type V2;
-        // ---- P2 backward on the reduced tree --------------------------------------
-        // Sub-trees of at most 32 leaves, one warp per group of sub-trees, lock-step over the height above
-        // the leaves.  A node sits in the lane of its first child: that child's hand-off value (f U + parked,
-        // f B + parked) is already in the lane's registers, the other children's values come by warp shuffle
-        // from their lanes, in ascending lane order.  No shared memory and no barrier on the dependent chain
-        // inside a tier; between tiers a block barrier, and the leaves of the upper tier pull the hand-off
-        // slots of the tier below.
-        {
-            const int4* ents = reinterpret_cast<const int4*>(imeta + it.ent_off);
-            const int32_t* pull = imeta + it.pull_off;
-            const int warp = tid >> 5, nwarps = nthreads >> 5;
-            const uint32_t nd_sa = smem_u32(nd);
-            for (int tier = 0; tier < it.ntier; ++tier) {
-                const int gb = imeta[1 + tier], ge = imeta[2 + tier];
-                for (int g = gb + warp; g < ge; g += nwarps) {
-                    const int32_t* gh = imeta + it.grp_off + 36 * g;
-                    int pos = gh[lane];
-                    const int end = gh[lane + 1], nsteps = gh[33];
-                    const unsigned char* nshb = reinterpret_cast<const unsigned char*>(imeta) + gh[34];
-                    T outd = T(0), outb = T(0);
-                    // Node ids are entry indices, so the records of the lane's chain are consecutive: the next
-                    // record's address is known without its descriptor (one shared-memory hop, not two).
-                    constexpr uint32_t RS = 6u * (uint32_t)sizeof(T), W = (uint32_t)sizeof(T);
-                    int4 en = make_int4(0, 0, 0, 0);
-                    uint32_t qa = nd_sa + (uint32_t)pos * RS;
-                    V2 a0, a2; T U = T(0);
-                    a0.x = T(1); a0.y = T(0); a2.x = T(0); a2.y = T(0);
-                    int estep = 0x7fffffff;                         // step of the lane's next node
-                    if (pos < end) {
-                        en = ents[pos];
-                        a0 = lds2<T>(qa); U = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
-                        estep = en.x >> 20;
-                    }
-                    int nsh = nshb[0];
-#pragma unroll 1
-                    for (int h = 0; h < nsteps; ++h) {
-                        const int nsh_next = h + 1 < nsteps ? nshb[h + 1] : 0;
-                        const bool act = estep == h;
-                        T sd_ = outd, sb_ = outb;                       // the first child (own lane), or 0 at a leaf
-                        if (nsh) {                                      // the other children, by shuffle
-                            unsigned m = act ? (unsigned)en.y : 0u;
-#pragma unroll 1
-                            for (int t = 0; t < nsh; ++t) {
-                                const int src = m ? __ffs(m) - 1 : lane;
-                                const T vd = __shfl_sync(FULL, outd, src), vb = __shfl_sync(FULL, outb, src);
-                                if (m) { sd_ += vd; sb_ += vb; m &= m - 1; }
-                            }
-                        }
-                        // a run = a node and the single-child nodes above it, all on this step (no shuffle, no pull
-                        // after the first): the lane walks it node by node
-                        while (estep == h) {
-                            const int npull = en.w & 0xffff;
-                            int run = en.w >> 16;                       // plain nodes behind this one (same step, nothing to pull)
-                            if (npull) {                                // children swept in an earlier tier
-#pragma unroll 1
-                                for (int k = 0; k < npull; ++k) {
-                                    const V2 c2 = lds2<T>(nd_sa + (uint32_t)pull[en.z + k] * RS + 4u * W);
-                                    sd_ += c2.x; sb_ += c2.y;
-                                }
-                            }
-                            const T D = a0.x - sd_, B = a0.y - sb_;
-                            ++pos;
-                            const bool more = pos < end;
-                            if (more) {                                 // next node: what its step needs first
-                                en = ents[pos];
-                                a0 = lds2<T>(qa + RS);
-                                estep = en.x >> 20;
-                            } else {
-                                estep = 0x7fffffff;
-                            }
-                            const T r = rcp<T>(D);
-                            const T f = U * r;
-                            V2 o; o.x = -f; o.y = B * r;
-                            sts2<T>(qa, o);
-                            outd = fmad<T>(f, U, a2.x); outb = fmad<T>(f, B, a2.y);
-                            if (more) {                                 // ... and what it needs after its reciprocal
-                                qa += RS;
-                                U = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
-                            } else {                                    // end of the lane's chain: leave the hand-off in the slot
-                                V2 s2; s2.x = outd; s2.y = outb;
-                                sts2<T>(qa + 4u * W, s2);
-                            }
-                            if (run) {
-                                // The plain part of the run in a tight loop: records are consecutive, no descriptor is
-                                // read, the next record is fetched while this one's reciprocal runs; two register
-                                // sets swap roles.  On entry {a0, U, a2} hold the record at qa (= entry pos).
-                                V2 b0, b2; T V;
-                                b0 = a0; b2 = a2; V = U;
-                                pos += run;
-                                const bool ends = pos >= end;           // the run takes the lane's chain to its end
-#define HINES_RUN_NODE(A0, UU, A2, B0, VV, B2)                                                               \
-                                {                                                                            \
-                                    const T D_ = A0.x - outd, B_ = A0.y - outb;                              \
-                                    if (run > 1 || !ends) { B0 = lds2<T>(qa + RS); VV = lds1<T>(qa + RS + 2u * W); B2 = lds2<T>(qa + RS + 4u * W); } \
-                                    const T r_ = rcp<T>(D_);                                                 \
-                                    const T f_ = UU * r_;                                                    \
-                                    V2 o_; o_.x = -f_; o_.y = B_ * r_;                                       \
-                                    sts2<T>(qa, o_);                                                         \
-                                    outd = fmad<T>(f_, UU, A2.x); outb = fmad<T>(f_, B_, A2.y);              \
-                                    qa += RS;                                                                \
-                                }
-#pragma unroll 1
-                                while (true) {
-                                    HINES_RUN_NODE(a0, U, a2, b0, V, b2)
-                                    if (--run == 0) { a0 = b0; U = V; a2 = b2; break; }
-                                    HINES_RUN_NODE(b0, V, b2, a0, U, a2)
-                                    if (--run == 0) break;
-                                }
-#undef HINES_RUN_NODE
-                                if (ends) {
-                                    V2 s2; s2.x = outd; s2.y = outb;
-                                    sts2<T>(qa - RS + 4u * W, s2);
-                                    estep = 0x7fffffff;
-                                } else {
-                                    en = ents[pos];
-                                    estep = en.x >> 20;
-                                }
-                            }
-                            sd_ = outd; sb_ = outb;                     // the next node of the run has this one as its only child
-                        }
-                        nsh = nsh_next;
-                    }
-                    // A chain that ended in a root turns around: x_root = c_root, then x = c - f x_parent down the
-                    // lane's own chain (records consecutive, loads independent of the chain); these nodes are final
-                    // before the pointer jumping ({g, c} := {0, x}).
-                    if ((gh[35] >> lane) & 1) {
-                        const int begin = gh[lane];
-                        uint32_t qk = nd_sa + (uint32_t)(end - 1) * RS;
-                        T xv = lds1<T>(qk + W);
-                        int k = end - 2;
-                        for (; k - 3 >= begin; k -= 4) {                // four records in flight under one chain
-                            const V2 g0 = lds2<T>(qk - RS), g1 = lds2<T>(qk - 2u * RS), g2 = lds2<T>(qk - 3u * RS), g3 = lds2<T>(qk - 4u * RS);
-                            V2 o; o.x = T(0);
-                            xv = fmad<T>(g0.x, xv, g0.y); o.y = xv; sts2<T>(qk - RS, o);
-                            xv = fmad<T>(g1.x, xv, g1.y); o.y = xv; sts2<T>(qk - 2u * RS, o);
-                            xv = fmad<T>(g2.x, xv, g2.y); o.y = xv; sts2<T>(qk - 3u * RS, o);
-                            xv = fmad<T>(g3.x, xv, g3.y); o.y = xv; sts2<T>(qk - 4u * RS, o);
-                            qk -= 4u * RS;
-                        }
-                        for (; k >= begin; --k) {
-                            qk -= RS;
-                            const V2 gc = lds2<T>(qk);
-                            xv = fmad<T>(gc.x, xv, gc.y);
-                            V2 o; o.x = T(0); o.y = xv;
-                            sts2<T>(qk, o);
-                        }
-                    }
-                }
-                __syncthreads();
-            }
-        }
+    const int4* ex = reinterpret_cast<const int4*>(meta + H.exp_off);
+    const int4* gh = reinterpret_cast<const int4*>(meta + H.gh_off);
+    const uint32_t nd_sa = smem_u32(nd), lb_sa = smem_u32(meta), kp_sa = smem_u32(meta + H.kp_off);
+    const int nexp = H.nexp, nghost = H.nghost, nnode = H.nnode;
+    int rounds = H.rounds;
+    const bool cables = (H.flags & kPartFlagChains) != 0;
+    if (cables) {
+        // ---- unbranched cables: the reduced chains by parallel cyclic reduction, one warp per cable ----
+        solve_cables_pcr<T>(nd, meta, H.nlev, tid, nthreads);
+        __syncthreads();
+    } else {
+        // ---- P2 backward: what does not wait for another part, deepest level first ----
+        sweep_backward<T>(nd_sa, lb_sa, kp_sa, H.nlev - 1, H.lowlev, 0, H.maxwidth, tid, nthreads);
     }
-    HINES_STAMP(3);                 // outside the rank test: a stamp in both arms of it splits warp 0 for all of P2
-    if (rank == 0) {
-        const int32_t* pnode = imeta + it.pnode_off;
-        typedef typename Vec2<T>::type V2;
-        // ---- P2 forward by pointer jumping over the reduced tree --------------
-        // x_v = c_v + g_v x_p(v), g = -f, g_root = 0.  One round replaces (g_v, c_v, p(v)) by
-        // (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds >= nodes on the longest
-        // root path) every g is 0 and c is x.  All nodes work in every round, with one barrier per
-        // round instead of one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
-        for (int r = 0; r < it.rounds; ++r) {
-            const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
-            for (int v = tid; v < it.nnode; v += nthreads) {
-                int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
-                const int p = r == 0 ? pnode[v] : ip[(r - 1) & 1];
-                const V2 a = *reinterpret_cast<const V2*>(nd + 6 * v + sbuf);
-                const V2 ap = *reinterpret_cast<const V2*>(nd + 6 * p + sbuf);
-                const int pp = r == 0 ? pnode[p] : reinterpret_cast<const int*>(nd + 6 * p + 4)[(r - 1) & 1];
-                V2 o; o.x = a.x * ap.x; o.y = fmad<T>(a.x, ap.y, a.y);
-                *reinterpret_cast<V2*>(nd + 6 * v + dbuf) = o;
-                ip[r & 1] = pp;
+    // ---- hand-off values of the sub-trees held by other blocks, into the ghost children; then
+    //      the top nodes (the ancestors of the ghost children) ----
+    if (CL) {
+        if (rank == 0) { cluster_wait(); cluster_arrive(); cluster_wait(); }   // barrier 1: the other ranks have swept and exported
+    } else if (phase == kPhaseB) {
+        for (int e = tid; e < nghost; e += nthreads) {
+            const int4 g = gh[e];
+            *reinterpret_cast<V2*>(nd + 6 * g.x + 4) = reinterpret_cast<const V2*>(xch_h)[H.xch_base + g.y];
+        }
+        __syncthreads();
+    }
+    sweep_backward<T>(nd_sa, lb_sa, kp_sa, H.ntoplev - 1, 0, 1, H.maxwidth, tid, nthreads);
+    HINES_STAMP(3);
+    // ---- exchange: exported roots hand their value up and get their parent's x back ----
+    if (CL) {
+        if (rank != 0) {
+            T* nd0 = cg::this_cluster().map_shared_rank(nd, 0);
+            cluster_wait();                                 // barrier 0: rank 0 is running
+            for (int e = tid; e < nexp; e += nthreads) {
+                const int4 q = ex[e];
+                *reinterpret_cast<V2*>(nd0 + 6 * q.y + 4) = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
             }
+            cluster_arrive(); cluster_wait();               // barrier 1
+            cluster_arrive(); cluster_wait();               // barrier 2: rank 0 has finished its forward sweep
+            for (int e = tid; e < nexp; e += nthreads) {
+                const int4 q = ex[e];
+                nd[6 * q.w] = T(0); nd[6 * q.w + 1] = nd0[6 * q.z + 1];
+            }
+            cluster_arrive();                               // barrier 3: this block no longer reads rank 0's memory
             __syncthreads();
         }
+    } else if (phase == kPhaseA) {
+        for (int e = tid; e < nexp; e += nthreads) {
+            const int4 q = ex[e];
+            reinterpret_cast<V2*>(xch_h)[H.xch_base + q.y] = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
+        }
+        if (prof && tid == 0) {
+            unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
+            for (int k = 0; k < 4; ++k) o[k] = stamp[k];
+            o[4] = o[5] = o[6] = globaltimer_ns();
+            o[7] = ((unsigned long long)smid() << 32) | (unsigned)H.n;
+        }
+        return;
+    } else if (phase == kPhaseC) {
+        for (int e = tid; e < nexp; e += nthreads) {
+            const int4 q = ex[e];
+            nd[6 * q.w] = T(0); nd[6 * q.w + 1] = xch_x[H.xch_base + q.y];
+        }
+        __syncthreads();
     }
-    if (CL) cg::this_cluster().sync();
+    // ---- P2 forward: first the top nodes, level by level (the other parts of the cell wait
+    //      for their x), then everything by pointer jumping over the reduced forest.
+    // x_v = c_v + g_v x_p(v), g = -f, g = 0 at a root, at a finished node and at a ghost parent (c = the imported x).
+    // One round replaces (g_v, c_v, p(v)) by (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds > the
+    // longest path to such a node) every g is 0 and c is x.  All nodes work in every round, with one barrier per
+    // round instead of one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
+    sweep_forward_top<T>(nd_sa, lb_sa, kp_sa, H.ntoplev, H.maxwidth, tid, nthreads);
+    if (CL) {
+        if (rank == 0) { cluster_arrive(); cluster_wait(); cluster_arrive(); }   // barrier 2: x of the top nodes is there (slot 1); barrier 3 below
+    } else if (phase == kPhaseB) {
+        for (int e = tid; e < nghost; e += nthreads) {
+            const int4 g = gh[e];
+            xch_x[H.xch_base + g.y] = nd[6 * g.z + 1];
+        }
+    }
+    const int4* kp = reinterpret_cast<const int4*>(meta + H.kp_off);
+    for (int r = 0; r < rounds; ++r) {
+        const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
+        for (int v = tid; v < nnode; v += nthreads) {
+            int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
+            const int p = r == 0 ? kp[v].w : ip[(r - 1) & 1];
+            const V2 a = *reinterpret_cast<const V2*>(nd + 6 * v + sbuf);
+            const V2 ap = *reinterpret_cast<const V2*>(nd + 6 * p + sbuf);
+            const int pp = r == 0 ? kp[p].w : reinterpret_cast<const int*>(nd + 6 * p + 4)[(r - 1) & 1];
+            V2 o; o.x = a.x * ap.x; o.y = fmad<T>(a.x, ap.y, a.y);
+            *reinterpret_cast<V2*>(nd + 6 * v + dbuf) = o;
+            ip[r & 1] = pp;
+        }
+        __syncthreads();
+    }
+    const int xs = 2 * (rounds & 1) + 1;                  // record slot that holds x after the forward sweep
     HINES_STAMP(4);
 
-    const int xs = 2 * (it.rounds & 1) + 1;               // record slot that holds x after the forward sweep
     // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t]; then A walks up from q-1 to a
     //      (x[i] = c - g x[i+1] - h x[t]) and B walks up from b-1 to q+1 (x[i] = c - g x[i+1] - h x[q]), one FMA
     //      on the dependent chain per step ----
-    for (int base = (tid & ~31); base < ch.nseg_lanes; base += nthreads) {
+    for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
@@ -529,11 +662,11 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         const int m = isB ? mb : (kind == 1 ? mt : 0);
         const int dl = (sg.y >> 27) & 15;
         const int mmax = __reduce_max_sync(FULL, m + dl);
-        const int p0 = sg.x + off;
+        const int p0 = sg.x;
         T xb = T(0), xt = T(0), xn = T(0);
-        if (kind != 0) xb = ND[6 * sg.z + xs];
+        if (kind != 0) xb = nd[6 * sg.z + xs];
         if (kind == 1) {
-            if (sg.w >= 0) xt = ND[6 * sg.w + xs];
+            if (sg.w >= 0) xt = nd[6 * sg.w + xs];
             if (hasq) {
                 const int iq = p0 + mt;
                 xn = fnma<T>(sd[iq], xb, fnma<T>(su[iq], xt, sb[iq]));
@@ -558,25 +691,28 @@ hines_resident_kernel(const BlockRec* __restrict__ recs, const int32_t* __restri
         }
     }
 
-    // ---- store x (natural order): bulk store of the 16-byte aligned interior, edges by hand ----
-    const int head_end = min(ch.n, (E - off) % E);                     // chunk-local [0, head_end)
-    const int tail_begin = max(head_end, (int)(((off + ch.n) / E) * E) - off);   // chunk-local [tail_begin, n)
+    // ---- store x (natural order), run by run: bulk store of the 16-byte words inside the run, edges by hand ----
     fence_proxy_async();
     __syncthreads();
     HINES_STAMP(5);
-    if (tid == 0 && tail_begin > head_end) {
-        tma_store_1d(x + ch.comp_begin + head_end, sb + off + head_end, (uint32_t)(tail_begin - head_end) * sizeof(T));
-        tma_store_commit_wait();
+    for (int r = tid >> 5; r < nrun; r += nthreads >> 5) {
+        const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
+        const int64_t g = rd.x;
+        const int len = rd.y, so = rd.z;
+        const int head = min(len, (int)((E - (g & (E - 1))) & (E - 1)));                 // run-local [0, head)
+        const int tail = max(head, (int)(((g + len) & ~(int64_t)(E - 1)) - g));          // run-local [tail, len)
+        if (lane == 0 && tail > head) tma_store_1d(x + g + head, sb + so + head, (uint32_t)(tail - head) * W);
+        if (lane >= 1 && lane - 1 < head) x[g + lane - 1] = sb[so + lane - 1];
+        if (lane >= 8 && tail + lane - 8 < len) x[g + tail + lane - 8] = sb[so + tail + lane - 8];
     }
-    for (int j = tid; j < head_end; j += nthreads) x[ch.comp_begin + j] = sb[off + j];
-    for (int j = tail_begin + tid; j < ch.n; j += nthreads) x[ch.comp_begin + j] = sb[off + j];
+    tma_store_commit_wait();
     if (prof && tid == 0) {
         stamp[6] = globaltimer_ns();
         unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
         for (int k = 0; k < 7; ++k) o[k] = stamp[k];
-        o[7] = ((unsigned long long)smid() << 32) | (unsigned)ch.n;
+        o[7] = ((unsigned long long)smid() << 32) | (unsigned)H.n;
     }
-    if (CL) cg::this_cluster().sync();          // rank 0's shared memory stays alive while others read it
+    if (CL) cluster_wait();                     // barrier 3: rank 0's shared memory stays alive while the others read it
 #undef HINES_STAMP
 }
 
@@ -647,8 +783,8 @@ static hines_status_t upload_vec(const V& v, void** dst, int64_t& total)
 static void free_device(DeviceTables* D)
 {
     if (!D) return;
-    cudaFree(D->recs); cudaFree(D->item_meta); cudaFree(D->stream_desc);
-    cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
+    cudaFree(D->recs); cudaFree(D->meta); cudaFree(D->runs); cudaFree(D->xch_h); cudaFree(D->xch_x);
+    cudaFree(D->stream_desc); cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
     for (cudaStream_t t : D->side) if (t) cudaStreamDestroy(t);
@@ -656,7 +792,44 @@ static void free_device(DeviceTables* D)
     if (D->fork) cudaEventDestroy(D->fork);
     if (D->sstream) cudaStreamDestroy(D->sstream);
     if (D->sjoin) cudaEventDestroy(D->sjoin);
+    if (D->pstream) cudaStreamDestroy(D->pstream);
+    if (D->pjoin) cudaEventDestroy(D->pjoin);
     delete D;
+}
+
+// Per device and kernel instantiation, once per process: the opt-in maximum of dynamic shared memory and the
+// non-portable cluster size.  (Set to the device maximum, never to a plan's own need: several plans may be live.)
+template <typename T>
+static hines_status_t prepare_kernels(int max_optin)
+{
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    return HINES_OK;
+}
+
+template <typename T>
+static hines_status_t check_clusters(const hines_plan* P)
+{
+    for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
+        const int cl = P->class_cluster[q];
+        if (cl <= 1 || !P->class_count[q]) continue;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)cl); cfg.blockDim = dim3((unsigned)P->class_threads[q]);
+        cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        int nclusters = 0;
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, hines_resident_kernel<T, true>, &cfg));
+        if (nclusters < 1) {
+            set_error("this device cannot co-schedule a cluster of " + std::to_string(cl) + " blocks with " +
+                      std::to_string(P->class_smem_bytes[q]) + " bytes of shared memory each: create the plan with a smaller cluster_max");
+            return HINES_ERR_UNSUPPORTED;
+        }
+    }
+    return HINES_OK;
 }
 
 static hines_status_t upload(hines_plan* P)
@@ -673,6 +846,7 @@ static hines_status_t upload(hines_plan* P)
     hines_status_t st = HINES_OK;
     auto run = [&]() -> hines_status_t {
         CUDA_TRY(cudaGetDevice(&D->device));
+        CUDA_TRY(cudaDeviceGetAttribute(&D->num_sms, cudaDevAttrMultiProcessorCount, D->device));
         int max_optin = 0;
         CUDA_TRY(cudaDeviceGetAttribute(&max_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, D->device));
         for (int32_t s : P->class_smem_bytes)
@@ -680,46 +854,47 @@ static hines_status_t upload(hines_plan* P)
                 set_error("device offers " + std::to_string(max_optin) + " bytes of shared memory per block, plan needs " + std::to_string(s));
                 return HINES_ERR_UNSUPPORTED;
             }
+        if ((st = P->dtype == HINES_F64 ? prepare_kernels<double>(max_optin) : prepare_kernels<float>(max_optin))) return st;
+        if ((st = P->dtype == HINES_F64 ? check_clusters<double>(P) : check_clusters<float>(P))) return st;
         {
-            std::vector<BlockRec> recs;
-            recs.reserve(P->chunk_headers.size());
-            for (int32_t item : P->item_launch_order) {
-                const ItemHeader& h = P->item_headers[item];
-                for (int32_t r = 0; r < h.nchunks; ++r) recs.push_back(BlockRec{h, P->chunk_headers[h.first_chunk + r]});
+            std::vector<BlockRecord> recs(P->class_parts.size());
+            for (size_t k = 0; k < recs.size(); ++k) {
+                const PartHeader& h = P->part_headers[P->class_parts[k]];
+                recs[k].h = h;
+                std::memset(recs[k].runs, 0, sizeof(recs[k].runs));
+                const int nr = std::min<int>(h.nrun, kInlineRuns);
+                if (nr) std::memcpy(recs[k].runs, &P->part_runs[(size_t)h.run_off * 4], (size_t)nr * 16);
             }
             if ((st = upload_vec(recs, (void**)&D->recs, D->bytes))) return st;
         }
-        if ((st = upload_vec(P->item_meta, (void**)&D->item_meta, D->bytes))) return st;
+        if ((st = upload_vec(P->part_meta, (void**)&D->meta, D->bytes))) return st;
+        if ((st = upload_vec(P->part_runs, (void**)&D->runs, D->bytes))) return st;
         if ((st = upload_vec(P->stream_desc, (void**)&D->stream_desc, D->bytes))) return st;
         if ((st = upload_vec(P->stream_child, (void**)&D->stream_child, D->bytes))) return st;
+        if (P->n_xch) {
+            CUDA_TRY(cudaMalloc(&D->xch_h, 2 * (size_t)P->n_xch * P->width));
+            CUDA_TRY(cudaMalloc(&D->xch_x, (size_t)P->n_xch * P->width));
+            D->bytes += 3 * P->n_xch * P->width;
+        }
         if (P->n_stream_unknowns) {
             const size_t wb = (size_t)P->n_stream_unknowns * P->width;
             CUDA_TRY(cudaMalloc(&D->ws_f, wb));
             CUDA_TRY(cudaMalloc(&D->ws_c, wb));
             D->bytes += 2 * (int64_t)wb;
         }
-        int32_t max_smem[2] = {0, 0};
-        bool nonportable = false;
-        for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
-            const int cl = P->class_cluster[q] > 1;
-            max_smem[cl] = std::max(max_smem[cl], P->class_smem_bytes[q]);
-            nonportable |= P->class_cluster[q] > 8;
-        }
-        if (P->dtype == HINES_F64) {
-            if (max_smem[0]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[0]));
-            if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
-            if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<double, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        } else {
-            if (max_smem[0]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[0]));
-            if (max_smem[1]) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_smem[1]));
-            if (nonportable) CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<float, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        }
         const bool has_stream_path = P->stream_level_begin.size() > 1;
-        if (P->class_smem_bytes.size() + (has_stream_path ? 1 : 0) > 1 && !(P->opt.policy_flags & HINES_POLICY_SERIAL_CLASSES)) {
+        int n_ordinary = 0, n_split = 0;
+        for (size_t q = 0; q < P->class_phase.size(); ++q) if (P->class_count[q]) (P->class_phase[q] == kPhaseAll ? n_ordinary : n_split)++;
+        const int n_lines = n_ordinary + (n_split ? 1 : 0) + (has_stream_path ? 1 : 0);     // independent lines of work
+        if (n_lines > 1 && !(P->opt.policy_flags & HINES_POLICY_SERIAL_CLASSES)) {
             CUDA_TRY(cudaEventCreateWithFlags(&D->fork, cudaEventDisableTiming));
-            if (has_stream_path && !P->class_smem_bytes.empty()) {
+            if (has_stream_path) {
                 CUDA_TRY(cudaStreamCreateWithFlags(&D->sstream, cudaStreamNonBlocking));
                 CUDA_TRY(cudaEventCreateWithFlags(&D->sjoin, cudaEventDisableTiming));
+            }
+            if (n_split) {
+                CUDA_TRY(cudaStreamCreateWithFlags(&D->pstream, cudaStreamNonBlocking));
+                CUDA_TRY(cudaEventCreateWithFlags(&D->pjoin, cudaEventDisableTiming));
             }
             for (int k = 0; k < DeviceTables::kSide; ++k) {
                 CUDA_TRY(cudaStreamCreateWithFlags(&D->side[k], cudaStreamNonBlocking));
@@ -738,11 +913,11 @@ template <typename T>
 static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T* b, T* x, cudaStream_t stream)
 {
     DeviceTables* D = P->dev;
-    if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
     auto launch_streaming = [&](cudaStream_t ss) -> hines_status_t {
         const int nlev = (int)P->stream_level_begin.size() - 1;
         const int st = P->opt.stream_threads;
         T* wf = static_cast<T*>(D->ws_f); T* wc = static_cast<T*>(D->ws_c);
+        if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[2], ss));
         for (int l = nlev - 1; l >= 0; --l) {
             const int64_t b0 = P->stream_level_begin[l], b1 = P->stream_level_begin[l + 1];
             hines_stream_backward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, ss>>>(
@@ -753,12 +928,37 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
             hines_stream_forward<T><<<(unsigned)((b1 - b0 + st - 1) / st), st, 0, ss>>>(
                 D->stream_desc, b0, b1, wf, wc, x);
         }
+        if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[3], ss));
         CUDA_TRY(cudaGetLastError());
         return HINES_OK;
     };
-    // size classes are independent: the first runs on the caller's stream, the others on side streams
-    // forked from it and joined back, so that their blocks share the SMs and fill each other's tails
-    int64_t first_block = 0;
+    auto launch_class = [&](size_t q, cudaStream_t ls) -> hines_status_t {
+        const int64_t cnt = P->class_count[q], first = P->class_first[q];
+        const int cl = P->class_cluster[q];
+        unsigned long long* prof = D->prof_on ? D->prof + 8 * first : nullptr;
+        const BlockRecord* recs = D->recs + first;
+        T* xh = static_cast<T*>(D->xch_h); T* xx = static_cast<T*>(D->xch_x);
+        if (cl == 1) {
+            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], ls>>>(
+                recs, D->meta, D->runs, d, u, b, x, P->n, xh, xx, (int)P->class_phase[q], prof);
+        } else {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)cnt);
+            cfg.blockDim = dim3((unsigned)P->class_threads[q]);
+            cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
+            cfg.stream = ls;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, recs, (const int32_t*)D->meta, (const int4*)D->runs,
+                                        d, u, b, x, (int64_t)P->n, xh, xx, 0, prof));
+        }
+        return HINES_OK;
+    };
+    // Size classes are independent: the first runs on the caller's stream, the others on side streams forked
+    // from it and joined back, so that their blocks share the SMs and fill each other's tails.  The three phases
+    // of split items run in order on a stream of their own, the streaming path on another.
     const bool forked = D->fork != nullptr;
     bool used[DeviceTables::kSide] = {false, false, false};
     if (forked) CUDA_TRY(cudaEventRecord(D->fork, stream));
@@ -767,11 +967,20 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         if (hines_status_t sst = launch_streaming(D->sstream)) return sst;
         CUDA_TRY(cudaEventRecord(D->sjoin, D->sstream));
     }
+    if (D->pstream) {
+        CUDA_TRY(cudaStreamWaitEvent(D->pstream, D->fork, 0));
+        for (size_t q = 0; q < P->class_smem_bytes.size(); ++q)
+            if (P->class_phase[q] != kPhaseAll && P->class_count[q]) if (hines_status_t s2 = launch_class(q, D->pstream)) return s2;
+        CUDA_TRY(cudaEventRecord(D->pjoin, D->pstream));
+    }
+    if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[0], stream));
     int nth = 0;
     for (size_t q = 0; q < P->class_smem_bytes.size(); ++q) {
-        const int64_t cnt = P->class_count[q];
-        if (!cnt) continue;
-        const int cl = P->class_cluster[q];
+        if (!P->class_count[q]) continue;
+        if (P->class_phase[q] != kPhaseAll) {
+            if (!D->pstream) if (hines_status_t s2 = launch_class(q, stream)) return s2;      // in order on the caller's stream
+            continue;
+        }
         cudaStream_t ls = stream;
         if (forked && nth > 0) {
             const int k = (nth - 1) % DeviceTables::kSide;
@@ -779,32 +988,15 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
             if (!used[k]) { CUDA_TRY(cudaStreamWaitEvent(ls, D->fork, 0)); used[k] = true; }
         }
         ++nth;
-        unsigned long long* prof = D->prof_on ? D->prof + 8 * first_block : nullptr;
-        const BlockRec* recs = D->recs + first_block;
-        if (cl == 1) {
-            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], ls>>>(
-                recs, D->item_meta, d, u, b, x, P->n, prof);
-        } else {
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3((unsigned)(cnt * cl));
-            cfg.blockDim = dim3((unsigned)P->class_threads[q]);
-            cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
-            cfg.stream = ls;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-            cfg.attrs = attr; cfg.numAttrs = 1;
-            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, recs, (const int32_t*)D->item_meta, d, u, b, x,
-                                        (int64_t)P->n, prof));
-        }
-        first_block += cnt * cl;
+        if (hines_status_t s2 = launch_class(q, ls)) return s2;
     }
     for (int k = 0; k < DeviceTables::kSide; ++k)
         if (used[k]) { CUDA_TRY(cudaEventRecord(D->join[k], D->side[k])); CUDA_TRY(cudaStreamWaitEvent(stream, D->join[k], 0)); }
+    if (D->pstream) CUDA_TRY(cudaStreamWaitEvent(stream, D->pjoin, 0));
     if (D->timing) CUDA_TRY(cudaEventRecord(D->ev[1], stream));
     if (D->sstream) CUDA_TRY(cudaStreamWaitEvent(stream, D->sjoin, 0));
-    else if (hines_status_t sst = launch_streaming(stream)) return sst;
-    if (D->timing) { CUDA_TRY(cudaEventRecord(D->ev[2], stream)); D->timed_once = true; }
+    else if (P->stream_level_begin.size() > 1) { if (hines_status_t sst = launch_streaming(stream)) return sst; }
+    if (D->timing) D->timed_once = true;
     CUDA_TRY(cudaGetLastError());
     return HINES_OK;
 }
@@ -813,6 +1005,12 @@ static hines_status_t check_ptrs(const hines_plan* P, const void* d, const void*
 {
     if (!P || !d || !u || !b || !x) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
     return HINES_OK;
+}
+
+static bool overlaps(const void* a, const void* b, size_t bytes)
+{
+    const uintptr_t p = (uintptr_t)a, q = (uintptr_t)b;
+    return p < q + bytes && q < p + bytes;
 }
 
 }  // namespace hines
@@ -834,7 +1032,10 @@ hines_status_t hines_solve(hines_plan_t* P, const void* d, const void* u, const 
     if (((uintptr_t)d | (uintptr_t)u | (uintptr_t)b | (uintptr_t)x) & 15) {
         set_error("device pointers must be 16-byte aligned"); return HINES_ERR_INVALID_ARG;
     }
-    if (d == x || u == x) { set_error("x may alias b only"); return HINES_ERR_INVALID_ARG; }
+    const size_t bytes = (size_t)P->n * P->width;
+    if (overlaps(x, d, bytes) || overlaps(x, u, bytes) || (x != b && overlaps(x, b, bytes))) {
+        set_error("x may be exactly b (in place) or must not overlap d, u, b"); return HINES_ERR_INVALID_ARG;
+    }
     if ((st = upload(P)) != HINES_OK) return st;
     if (P->dtype == HINES_F64)
         return launch_all<double>(P, (const double*)d, (const double*)u, (const double*)b, (double*)x, (cudaStream_t)stream);
@@ -879,9 +1080,13 @@ hines_status_t hines_plan_get_timing(hines_plan_t* P, float* resident_ms, float*
     if (!P || !resident_ms || !stream_ms) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
     if (!P->dev || !P->dev->timing || !P->dev->timed_once) { set_error("timing not enabled or no solve yet"); return HINES_ERR_INVALID_ARG; }
     DeviceTables* D = P->dev;
-    CUDA_TRY(cudaEventSynchronize(D->ev[2]));
+    *resident_ms = 0.f; *stream_ms = 0.f;
+    CUDA_TRY(cudaEventSynchronize(D->ev[1]));
     CUDA_TRY(cudaEventElapsedTime(resident_ms, D->ev[0], D->ev[1]));
-    CUDA_TRY(cudaEventElapsedTime(stream_ms, D->ev[1], D->ev[2]));
+    if (P->stream_level_begin.size() > 1) {
+        CUDA_TRY(cudaEventSynchronize(D->ev[3]));
+        CUDA_TRY(cudaEventElapsedTime(stream_ms, D->ev[2], D->ev[3]));
+    }
     return HINES_OK;
 }
 
@@ -891,7 +1096,7 @@ hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* P, int32_t enable)
     hines_status_t st = upload(P);
     if (st != HINES_OK) return st;
     DeviceTables* D = P->dev;
-    const size_t bytes = P->chunk_headers.size() * 8 * sizeof(unsigned long long);
+    const size_t bytes = P->class_parts.size() * 8 * sizeof(unsigned long long);
     if (enable && !D->prof && bytes) {
         CUDA_TRY(cudaMalloc(&D->prof, bytes));
         CUDA_TRY(cudaMemset(D->prof, 0, bytes));
@@ -904,7 +1109,7 @@ hines_status_t hines_plan_enable_phase_clocks(hines_plan_t* P, int32_t enable)
 hines_status_t hines_plan_get_phase_clocks(hines_plan_t* P, uint64_t* host_dst, int64_t capacity_bytes, int64_t* needed_bytes)
 {
     if (!P || !needed_bytes) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
-    const int64_t bytes = (int64_t)(P->chunk_headers.size() * 8 * sizeof(unsigned long long));
+    const int64_t bytes = (int64_t)(P->class_parts.size() * 8 * sizeof(unsigned long long));
     *needed_bytes = bytes;
     if (!host_dst) return HINES_OK;
     if (!P->dev || !P->dev->prof) { set_error("phase clocks not enabled"); return HINES_ERR_INVALID_ARG; }

@@ -1,20 +1,68 @@
 """Test-side interpreter of the plan's policy tables (pure Python, fp64).
 
-Executes exactly what the tables tell the resident kernel to do -- condense every segment (P1),
-the backward sweep over the reduced tree (tiers of warp groups in lock-step over the height, shuffle and
-pull hand-off) and the pointer-jumping forward sweep (P2), expand (P3) -- one
-"lane" at a time, so that a wrong table (a missing segment, a wrong node id, a child group the parent
-does not pull) shows up on the CPU box as a wrong solution, before any GPU run.  It shares no code
-with the library: it only reads tables through hines_plan_get_table.
+Executes exactly what the tables tell the resident kernel to do -- stage the runs of every part, condense
+every segment (P1), the level-synchronous backward sweep over the part's reduced forest with the pull
+hand-off (P2), the exchange between the parts of one cell (exports -> ghost children, parent's x -> ghost
+parents), the pointer-jumping forward sweep, expand (P3), store run by run -- one "lane" at a time, so
+that a wrong table (a missing segment, a wrong node id, a child the parent does not pull, a wrong run)
+shows up on the CPU box as a wrong solution, before any GPU run.  It shares no code with the library: it
+only reads tables through hines_plan_get_table.
 """
 from __future__ import annotations
 
 import numpy as np
 
+HDR = {"meta_off": 0, "meta_len": 2, "run_off": 3, "nrun": 4, "tx_elems": 5, "L": 6, "n": 7, "nnode": 8,
+       "nlevnode": 9, "nlev": 10, "rounds": 11, "kp_off": 12, "exp_off": 13, "gh_off": 14, "seg_off": 15,
+       "nexp": 16, "nghost": 17, "nseg_lanes": 18, "xch_base": 19, "xs0": 20, "item": 21, "rank": 22, "flags": 23, "ntoplev": 24, "lowlev": 25, "maxwidth": 26}
+
+
+class Part:
+    """One part's tables, parsed from PART_HEADER / PART_META / PART_RUNS."""
+
+    def __init__(self, hdr, meta_all, runs_all):
+        h = {k: int(hdr[i]) for k, i in HDR.items()}
+        h["meta_off"] = int(hdr[0:2].view(np.int64)[0])
+        self.h = h
+        meta = meta_all[h["meta_off"]:h["meta_off"] + h["meta_len"]]
+        self.lb = meta[:h["nlev"] + 1]
+        kp4 = meta[h["kp_off"]:h["kp_off"] + 4 * h["nnode"]].reshape(-1, 4)
+        self.kp4 = kp4
+        info = kp4[:, 2]
+        self.ghost = info < 0
+        self.top = np.where(self.ghost, 0, (info >> 29) & 1)   # an ancestor of a ghost child
+        self.nc = np.where(self.ghost, 0, info & 0xfff)
+        self.pnode = kp4[:, 3]
+        self.chains = bool(h["flags"] & 1)
+        self.exps = meta[h["exp_off"]:h["exp_off"] + 4 * h["nexp"]].reshape(-1, 4)
+        self.ghosts = meta[h["gh_off"]:h["gh_off"] + 4 * h["nghost"]].reshape(-1, 4)
+        self.seg = meta[h["seg_off"]:h["seg_off"] + 4 * h["nseg_lanes"]].reshape(-1, 4)
+        assert h["seg_off"] + 4 * h["nseg_lanes"] == h["meta_len"] and h["meta_len"] % 4 == 0
+        assert all(h[k] % 4 == 0 for k in ("kp_off", "exp_off", "gh_off", "seg_off"))
+        self.runs = runs_all[h["run_off"]:h["run_off"] + h["nrun"]]
+        assert int(self.lb[-1]) == h["nlevnode"] and h["nnode"] == h["nlevnode"] + h["nexp"]
+
+    def children(self, v, w):
+        """Node ids of v's children from the byte offsets of their hand-off slots (record = 6 values of w bytes,
+        slot at value 4; the all-zero record sits at index nnode); children beyond the second are consecutive."""
+        nc = int(self.nc[v])
+        ids = []
+        for q in range(2):
+            off = int(self.kp4[v, q])
+            assert (off - 4 * w) % (6 * w) == 0
+            idx = (off - 4 * w) // (6 * w)
+            if q < nc:
+                ids.append(idx)
+            else:
+                assert idx == self.h["nnode"], "absent child points at the zero record"
+        ids += [ids[1] + k for k in range(1, nc - 1)]
+        return ids
+
 
 def pairs(sg):
-    """Segments of a chunk's lane list: groups of 32 lanes = 16 A lanes + their 16 B partners.
+    """Segments of a part's lane list: groups of 32 lanes = 16 A lanes + their 16 B partners.
     Yields (a, mt, mb, hasq, node, tnode) per segment and checks the pairing."""
+    assert len(sg) % 32 == 0
     for g in range(0, len(sg), 32):
         for k in range(16):
             A, B = sg[g + k], sg[g + 16 + k]
@@ -25,194 +73,238 @@ def pairs(sg):
             msk = ~((3 << 24) | (15 << 27))                # kind and the lane's start delay differ between A and B
             assert ka == 1 and kb == 2 and (int(A[1]) & msk) == (int(B[1]) & msk) and A[2] == B[2]
             mt, mb, hasq = int(A[1]) & 0xfff, (int(A[1]) >> 12) & 0xfff, (int(A[1]) >> 26) & 1
-            mm = mt + mb + hasq
             assert (B[0] == A[0] + mt + 1 or not hasq) and (hasq or (mt == 0 and mb == 0)) and abs(mt - mb) <= 5
             yield int(A[0]), mt, mb, hasq, int(A[2]), int(A[3])
 
 
-def parse_tasks(blob):
-    """Per tier: (tier, [(lane_begin[33], steps, shuffle counts per step, turn-around lane mask)], entries, pull list, raw bytes)."""
-    ntier = int(blob[0])
-    tb = blob[1:2 + ntier]
-    grp_off = -(-(2 + ntier) // 4) * 4
-    ngroups = int(tb[-1])
-    ent_off = grp_off + 36 * ngroups
-    nent = int(blob[grp_off + 36 * (ngroups - 1) + 32]) if ngroups else 0
-    ents = blob[ent_off:ent_off + 4 * nent].reshape(-1, 4)
-    pull_off = ent_off + 4 * nent
-    npull = int((ents[:, 3] & 0xffff).sum()) if nent else 0
-    pull = blob[pull_off:pull_off + npull]
-    raw = blob.view(np.uint8)
-    out = []
-    for t in range(ntier):
-        groups = []
-        for g in range(int(tb[t]), int(tb[t + 1])):
-            gh = blob[grp_off + 36 * g:grp_off + 36 * g + 36]
-            nsteps, boff = int(gh[33]), int(gh[34])
-            groups.append((gh[:33], nsteps, raw[boff:boff + nsteps], int(gh[35]) & 0xffffffff))
-        out.append((t, groups, ents, pull, raw))
-    return out
+def parts_of(plan):
+    hdrs = plan.table("part_header").reshape(-1, 32)
+    meta = plan.table("part_meta")
+    runs = plan.table("part_runs").reshape(-1, 4)
+    return [Part(h, meta, runs) for h in hdrs]
+
+
+class _PartState:
+    def __init__(self, part, d, u, b, n_total, E):
+        h = part.h
+        self.p = part
+        L = h["L"]
+        self.sd = np.full(L, np.nan); self.su = np.full(L, np.nan); self.sb = np.full(L, np.nan)
+        tx = 0
+        cursor = 0
+        for g, ln, so, _ in part.runs:
+            g, ln, so = int(g), int(ln), int(so)
+            assert ln > 0 and so % E == g % E and so >= cursor and so + ln <= L, "run staged at the parity of its global index"
+            cursor = so + ln
+            ga, ge = g - g % E, min(-(-(g + ln) // E) * E, n_total // E * E)
+            tx += max(0, ge - ga)
+            self.sd[so:so + ln] = d[g:g + ln]; self.su[so:so + ln] = u[g:g + ln]; self.sb[so:so + ln] = b[g:g + ln]
+        assert tx == h["tx_elems"] and L % E == 0 and sum(int(r[1]) for r in part.runs) == h["n"]
+        nn = h["nnode"]
+        self.rec = np.full((nn + 1, 6), np.nan)
+        self.rec[nn, 4:6] = 0.0                             # the all-zero record
+        self.w = 16 // E
+
+    def condense(self):
+        """P1: two lanes per segment, both top-down."""
+        sd, su, sb, rec = self.sd, self.su, self.sb, self.rec
+        for a, mt, mb, hasq, node, tnode in pairs(self.p.seg):
+            i = a
+            D, B = sd[i], sb[i]
+            ee = su[i] if tnode >= 0 else 0.0
+            ddt = dbt = 0.0
+            for _ in range(mt):
+                un, dn, bn = su[i + 1], sd[i + 1], sb[i + 1]
+                r = 1.0 / D
+                g, h, c = un * r, ee * r, B * r
+                sd[i], su[i], sb[i] = g, h, c
+                ddt += h * ee; dbt += h * B
+                D, B, ee = dn - g * un, bn - g * B, -h * un
+                i += 1
+            if hasq:
+                q = a + mt; bp = q + 1 + mb
+                j = q + 1
+                Db, Bb, eb = sd[j], sb[j], su[j]
+                pdd = pdb = 0.0
+                for _ in range(mb):
+                    un, dn, bn = su[j + 1], sd[j + 1], sb[j + 1]
+                    r = 1.0 / Db
+                    g, h, c = un * r, eb * r, Bb * r
+                    sd[j], su[j], sb[j] = g, h, c
+                    pdd += h * eb; pdb += h * Bb
+                    Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
+                    j += 1
+                assert j == bp
+                Dq, Bq = D - pdd, B - pdb
+                r = 1.0 / Dq
+                gq, hq = eb * r, ee * r
+                sd[q], su[q], sb[q] = gq, hq, Bq * r
+                ddt += hq * ee; dbt += hq * Bq
+                new = (Db - gq * eb, Bb - gq * Bq, hq * eb, ddt, dbt)      # slot 2 holds -U
+            else:
+                new = (D, B, -ee, 0.0, 0.0)
+            assert 0 <= node < self.p.h["nlevnode"] and np.isnan(rec[node, 0]), "node written twice"
+            assert not self.p.ghost[node], "a ghost child has no segment"
+            rec[node, 0], rec[node, 1], rec[node, 2], rec[node, 4], rec[node, 5] = new
+
+    def cables(self):
+        """A part of unbranched cables: lb[] = first node of each cable; the reduced chain of a cable is a
+        tridiagonal system (the kernel solves it by cyclic reduction inside a warp; any exact solve is the same)."""
+        p, rec = self.p, self.rec
+        x = np.zeros(p.h["nnode"])
+        for c in range(p.h["nlev"]):
+            n0, n1 = int(p.lb[c]), int(p.lb[c + 1])
+            m = n1 - n0
+            assert 1 <= m <= 32
+            A = np.zeros((m, m)); rhs = np.zeros(m)
+            for i in range(m):
+                A[i, i] = rec[n0 + i, 0] - (rec[n0 + i + 1, 4] if i + 1 < m else 0.0)
+                rhs[i] = rec[n0 + i, 1] - (rec[n0 + i + 1, 5] if i + 1 < m else 0.0)
+                if i > 0:
+                    A[i, i - 1] = A[i - 1, i] = -rec[n0 + i, 2]
+                    assert p.pnode[n0 + i] == n0 + i - 1
+                else:
+                    assert p.pnode[n0] == n0 and rec[n0, 2] == 0
+            x[n0:n1] = np.linalg.solve(A, rhs)
+        return x
+
+    def backward(self, sweep):
+        """P2 backward: deepest level first; a node pulls its children (first two by their slot offsets, the rest
+        consecutive, ascending).  sweep 0: everything that does not wait for another part (levels nlev-1 .. lowlev,
+        nodes that are not top nodes); sweep 1: the top nodes (levels ntoplev-1 .. 0), after the ghost children got
+        their hand-off."""
+        p, rec = self.p, self.rec
+        if sweep == 0:
+            self.done = np.zeros(p.h["nlevnode"], bool)
+        done = self.done
+        if sweep == 1:                                       # every ghost child has received its hand-off by now
+            gc = np.nonzero(p.ghost[:p.h["nlevnode"]])[0]
+            assert not np.isnan(rec[gc, 4]).any(), "ghost child without its hand-off"
+            done[gc] = True
+        lv = range(p.h["nlev"] - 1, p.h["lowlev"] - 1, -1) if sweep == 0 else range(p.h["ntoplev"] - 1, -1, -1)
+        for l in lv:
+            assert p.lb[l + 1] - p.lb[l] <= p.h["maxwidth"]
+            for v in range(int(p.lb[l]), int(p.lb[l + 1])):
+                if p.ghost[v] or p.top[v] != sweep:
+                    continue
+                D, B, Un = rec[v, 0], rec[v, 1], rec[v, 2]
+                assert not np.isnan(D), "node without a segment"
+                for c in p.children(v, self.w):
+                    assert done[c] and p.lb[l + 1] <= c < p.lb[l + 2], "children sit on the next level"
+                    assert p.pnode[c] == v or p.ghost[c]
+                    D -= rec[c, 4]; B -= rec[c, 5]
+                r = 1.0 / D
+                g = Un * r
+                rec[v, 0], rec[v, 1] = g, B * r
+                rec[v, 4], rec[v, 5] = g * Un + rec[v, 4], rec[v, 5] - g * B
+                assert not done[v]
+                done[v] = True
+        if sweep == 1:
+            assert done.all()
+
+    def forward_top(self):
+        """x of the top nodes, level by level from the root; a finished node holds {g, c} = {0, x}."""
+        p, rec = self.p, self.rec
+        for l in range(p.h["ntoplev"]):
+            for v in range(int(p.lb[l]), int(p.lb[l + 1])):
+                if p.ghost[v] or not p.top[v]:
+                    continue
+                pn = int(p.pnode[v])
+                xp = 0.0 if pn == v else rec[pn, 1]
+                assert pn == v or (p.top[pn] and rec[pn, 0] == 0.0), "a top node's parent is a finished top node"
+                rec[v, 0], rec[v, 1] = 0.0, rec[v, 1] + rec[v, 0] * xp
+
+    def forward(self):
+        """P2 forward by pointer jumping; returns x per node."""
+        p, rec = self.p, self.rec
+        nn = p.h["nnode"]
+        par = p.pnode.astype(np.int64).copy()
+        ghost_child = p.ghost
+        g = np.where(ghost_child, 0.0, rec[:nn, 0]); c = np.where(ghost_child, 0.0, rec[:nn, 1])
+        assert (par[ghost_child] == np.nonzero(ghost_child)[0]).all()
+        assert (par[p.h["nlevnode"]:] == np.arange(p.h["nlevnode"], nn)).all(), "a ghost parent reads itself"
+        assert not np.isnan(g[~ghost_child]).any() and not np.isnan(c[~ghost_child]).any()
+        for _ in range(p.h["rounds"]):
+            g, c, par = g * g[par], c + g * c[par], par[par]
+        assert (g[~ghost_child] == 0).all(), "not enough pointer-jumping rounds"
+        return c
+
+    def expand(self, xnode, x, E):
+        """P3 + the store, run by run."""
+        sd, su, sb = self.sd, self.su, self.sb
+        for a, mt, mb, hasq, node, tnode in pairs(self.p.seg):
+            xb = xnode[node]
+            xt = xnode[tnode] if tnode >= 0 else 0.0
+            if not hasq:
+                sb[a] = xb
+                continue
+            q = a + mt; bp = q + 1 + mb
+            xq = (sb[q] - su[q] * xt) - sd[q] * xb
+            sb[q] = xq; sb[bp] = xb
+            xn = xq
+            for j in range(q - 1, a - 1, -1):
+                xn = (sb[j] - su[j] * xt) - sd[j] * xn
+                sb[j] = xn
+            xn = xb
+            for j in range(bp - 1, q, -1):
+                xn = (sb[j] - su[j] * xq) - sd[j] * xn
+                sb[j] = xn
+        for g, ln, so, _ in self.p.runs:
+            assert np.isnan(x[g:g + ln]).all(), "compartment stored twice"
+            x[g:g + ln] = sb[so:so + ln]
 
 
 def solve_with_tables(plan, m, d, u, b):
     """x for every cell that sits in an on-chip work item (NaN elsewhere)."""
     x = np.full(m.n, np.nan)
-    rng_ = plan.table("item_cell_range").reshape(-1, 2)
-    pnode_all = plan.table("item_pnode")
-    nnode = plan.table("item_nnode")
-    node_off = plan.table("item_node_offsets")
-    rounds = plan.table("item_rounds")
-    task_off = plan.table("item_task_offsets")
-    task_blob = plan.table("item_task_blob")
-    ch_off = plan.table("item_chunk_offsets")
-    ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
-    seg_off = plan.table("chunk_seg_offsets")
-    segs = plan.table("chunk_seg").reshape(-1, 4)
-    for it in range(len(rng_)):
-        NN = int(nnode[it])
-        rD = np.full(NN, np.nan); rB = rD.copy(); rU = rD.copy(); pd = rD.copy(); pb = rD.copy()
-        work = []
-        # P1
-        for ch in range(ch_off[it], ch_off[it + 1]):
-            g0, g1 = ch_rng[ch]
-            sd = d[g0:g1].astype(np.float64).copy(); su = u[g0:g1].astype(np.float64).copy(); sb = b[g0:g1].astype(np.float64).copy()
-            sg = segs[seg_off[ch]:seg_off[ch + 1]]
-            assert len(sg) % 32 == 0
-            for a, mt, mb, hasq, node, tnode in pairs(sg):
-                # lane A: upper half a..q-1 top-down, fill-in coupling to t
-                i = a
-                D, B = sd[i], sb[i]
-                ee = su[i] if tnode >= 0 else 0.0
-                ddt = dbt = 0.0
-                for _ in range(mt):
-                    un, dn, bn = su[i + 1], sd[i + 1], sb[i + 1]
-                    r = 1.0 / D
-                    g, h, c = un * r, ee * r, B * r
-                    sd[i], su[i], sb[i] = g, h, c
-                    ddt += h * ee; dbt += h * B
-                    D, B, ee = dn - g * un, bn - g * B, -h * un
-                    i += 1
-                if hasq:
-                    q = a + mt; bp = q + 1 + mb
-                    # lane B: q+1..b-1 top-down, fill-in coupling to q; arrives at b
-                    j = q + 1
-                    Db, Bb, eb = sd[j], sb[j], su[j]
-                    pdd = pdb = 0.0
-                    for _ in range(mb):
-                        un, dn, bn = su[j + 1], sd[j + 1], sb[j + 1]
-                        r = 1.0 / Db
-                        g, h, c = un * r, eb * r, Bb * r
-                        sd[j], su[j], sb[j] = g, h, c
-                        pdd += h * eb; pdb += h * Bb
-                        Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
-                        j += 1
-                    assert j == bp
-                    Dq, Bq = D - pdd, B - pdb
-                    r = 1.0 / Dq
-                    gq, hq = eb * r, ee * r
-                    sd[q], su[q], sb[q] = gq, hq, Bq * r
-                    ddt += hq * ee; dbt += hq * Bq
-                    rec = (Db - gq * eb, Bb - gq * Bq, -hq * eb, ddt, dbt)
-                else:
-                    rec = (D, B, ee, 0.0, 0.0)
-                assert np.isnan(rD[node]), "node written twice"
-                rD[node], rB[node], rU[node], pd[node], pb[node] = rec
-            work.append((g0, g1, sd, su, sb, sg))
-        # P2 backward: tiers of warp groups, lock-step over the height, a node in the lane of its first child
-        pn = pnode_all[node_off[it]:node_off[it + 1]]
-        assert len(pn) == NN
-        blob = task_blob[task_off[it]:task_off[it + 1]]
-        done = np.zeros(NN, bool)
-        final = np.zeros(NN, bool)
-        tiers = parse_tasks(blob)
-        any_turn = any(g_[3] for t_ in tiers for g_ in t_[1])      # all root chains of an item turn around, or none
-        for tier, groups, ents, pull, nshb in tiers:
-            for gh, nsteps, nsh, turn in groups:
-                outd = np.zeros(32); outb = np.zeros(32)
-                pos = [int(gh[l]) for l in range(32)]
-                for h in range(nsteps):
-                    newd, newb = outd.copy(), outb.copy()
-                    for lane in range(32):
-                        first = True
-                        while pos[lane] < gh[lane + 1]:
-                            w0, mask, p0, w3 = (int(v) for v in ents[pos[lane]])
-                            node, step = w0 & 0xfffff, (w0 >> 20) & 0xfff
-                            pcount, run = w3 & 0xffff, w3 >> 16
-                            # the run the kernel walks in its tight loop: entries right behind, same step, nothing to pull
-                            assert pos[lane] + run < gh[lane + 1] or run == 0
-                            for k in range(1, run + 1):
-                                wk = [int(v) for v in ents[pos[lane] + k]]
-                                assert (wk[0] >> 20) & 0xfff == step and wk[1] == 0 and wk[3] & 0xffff == 0 and wk[3] >> 16 == run - k
-                            if step != h:
-                                assert step > h
-                                break
-                            if first:
-                                sd_, sb_ = outd[lane], outb[lane]
-                                srcs = [l2 for l2 in range(32) if (mask >> l2) & 1]
-                                assert len(srcs) <= nsh[h] and lane not in srcs
-                                for l2 in srcs:
-                                    sd_ += outd[l2]; sb_ += outb[l2]
-                            else:                           # continuation of a run: only child = the node just computed
-                                assert mask == 0
-                                sd_, sb_ = newd[lane], newb[lane]
-                            for c in pull[p0:p0 + pcount]:
-                                assert done[c]
-                                sd_ += pd[c]; sb_ += pb[c]
-                            D, B = rD[node] - sd_, rB[node] - sb_
-                            r = 1.0 / D
-                            f = rU[node] * r
-                            rD[node], rB[node] = f, B * r
-                            newd[lane], newb[lane] = f * rU[node] + pd[node], f * B + pb[node]
-                            assert not done[node]
-                            done[node] = True
-                            pos[lane] += 1
-                            first = False
-                            if pos[lane] >= gh[lane + 1]:
-                                pd[node], pb[node] = newd[lane], newb[lane]       # hand-off slot
-                    outd, outb = newd, newb
-                assert all(pos[l] == gh[l + 1] for l in range(32))
-                # a chain that ended in a root turns around: x_root = c_root, x = c - f x_parent down the lane's chain
-                for l in range(32):
-                    b_, e_ = int(gh[l]), int(gh[l + 1])
-                    if (turn >> l) & 1:
-                        assert e_ > b_ and rU[e_ - 1] == 0, "turn-around lane does not end in a root"
-                        xv = rB[e_ - 1]
-                        rD[e_ - 1] = 0.0
-                        final[e_ - 1] = True
-                        for k in range(e_ - 2, b_ - 1, -1):
-                            xv = rB[k] - rD[k] * xv
-                            rD[k], rB[k] = 0.0, xv
-                            final[k] = True
-                    elif e_ > b_ and any_turn:
-                        assert pn[e_ - 1] != e_ - 1, "a chain that ends in a root must turn around"
-        assert done.all()
-        # forward sweep by pointer jumping: x_v = c_v + g_v x_p(v), g = -f (a root: g = 0, p = itself)
-        real = ~np.isnan(rD)
-        g = np.where(real, -rD, 0.0); c = np.where(real, rB, 0.0); par = pn.astype(np.int64).copy()
-        assert (par[~real] == np.nonzero(~real)[0]).all() and real[par[real]].all()
-        assert (par[final] == np.nonzero(final)[0]).all(), "a final node reads itself"
-        for _ in range(int(rounds[it])):
-            g, c, par = g * g[par], c + g * c[par], par[par]
-        assert (g[real] == 0).all(), "not enough pointer-jumping rounds"
-        rB = c
-        # P3
-        for g0, g1, sd, su, sb, sg in work:
-            for a, mt, mb, hasq, node, tnode in pairs(sg):
-                xb = rB[node]
-                xt = rB[tnode] if tnode >= 0 else 0.0
-                if not hasq:
-                    sb[a] = xb
-                    continue
-                q = a + mt; bp = q + 1 + mb
-                xq = (sb[q] - su[q] * xt) - sd[q] * xb
-                sb[q] = xq; sb[bp] = xb
-                xn = xq
-                for j in range(q - 1, a - 1, -1):
-                    xn = (sb[j] - su[j] * xt) - sd[j] * xn
-                    sb[j] = xn
-                xn = xb
-                for j in range(bp - 1, q, -1):
-                    xn = (sb[j] - su[j] * xq) - sd[j] * xn
-                    sb[j] = xn
-            x[g0:g1] = sb
+    E = 2 if plan.np_dtype == np.float64 else 4
+    d = np.asarray(d, np.float64); u = np.asarray(u, np.float64); b = np.asarray(b, np.float64)
+    parts = parts_of(plan)
+    poff = plan.table("item_part_offsets")
+    kind = plan.table("item_kind")
+    for it in range(len(kind)):
+        ps = [_PartState(parts[k], d, u, b, m.n, E) for k in range(poff[it], poff[it + 1])]
+        assert (kind[it] == 0) == (len(ps) == 1)
+        for r, s in enumerate(ps):
+            assert s.p.h["item"] == it and s.p.h["rank"] == r
+            assert (r == 0 or s.p.h["nghost"] == 0) and (r > 0 or s.p.h["nexp"] == 0)
+        if ps[0].p.chains:
+            assert len(ps) == 1 and ps[0].p.h["rounds"] == 0
+            ps[0].condense()
+            ps[0].expand(ps[0].cables(), x, E)
+            continue
+        ps[0].condense(); ps[0].backward(0)              # part 0's own sub-trees do not wait for the others
+        # sub-tree parts: condense, sweep backward, export the roots' hand-off values to part 0's ghost children
+        exported = set()
+        for s in ps[1:]:
+            s.condense(); s.backward(0); s.backward(1)
+            assert not s.p.top.any() and not s.p.chains
+            for v, gx, p0, gp in s.p.exps:
+                if kind[it] == 1:
+                    ghost = int(gx)
+                else:                                            # split item: through exchange slot gx
+                    hit = [int(g[0]) for g in ps[0].p.ghosts if g[1] == gx]
+                    assert len(hit) == 1
+                    ghost = hit[0]
+                    p0 = int([g[2] for g in ps[0].p.ghosts if g[1] == gx][0])
+                assert ps[0].p.ghost[ghost] and ghost not in exported
+                exported.add(ghost)
+                ps[0].rec[ghost, 4], ps[0].rec[ghost, 5] = s.rec[v, 4], s.rec[v, 5]
+                # the ghost child's parent in part 0 is the node whose x the root reads back
+                gl = [g for g in ps[0].p.ghosts if g[0] == ghost][0]
+                assert int(gl[2]) == int(p0) and ps[0].p.top[int(p0)]
+        assert len(exported) == ps[0].p.h["nghost"]
+        ps[0].backward(1)
+        ps[0].forward_top()
+        xtop = ps[0].rec[:, 1].copy()                    # what the other parts read: x of the top nodes
+        x0 = ps[0].forward()
+        ps[0].expand(x0, x, E)
+        for s in ps[1:]:
+            for v, gx, p0, gp in s.p.exps:
+                if kind[it] != 1:
+                    p0 = int([g[2] for g in ps[0].p.ghosts if g[1] == gx][0])
+                assert gp >= s.p.h["nlevnode"] and s.p.pnode[v] == gp
+                assert xtop[p0] == x0[p0]
+                s.rec[gp, 0], s.rec[gp, 1] = 0.0, xtop[p0]
+            s.expand(s.forward(), x, E)
     return x

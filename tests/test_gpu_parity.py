@@ -82,7 +82,7 @@ def test_cluster_path(kw, dtype):
     m = mg.make_config(2, 0.006)
     d, u, b = mg.system(m)
     _, info = _check(m, d, u, b, dtype, **kw)
-    assert info.n_cluster_cells > 0 and info.n_chunks > info.n_resident_items
+    assert info.n_cluster_cells > 0 and info.n_parts > info.n_resident_items
 
 
 @pytest.mark.parametrize("max_segment", [0, 2, 7, 48, 64, 200, 1023])
