@@ -54,8 +54,8 @@ enum {
     HINES_POLICY_DEFAULT      = 0,
     HINES_POLICY_FORCE_STREAM = 1,   /* every cell through the streaming (global-memory) path           */
     HINES_POLICY_NO_GROUPING  = 2,   /* one cell per shared-memory work item (paper: >= 1 cell per block) */
-    HINES_POLICY_INPUT_ORDER  = 4,   /* launch work items in input order, not heaviest first (PAPER.md:128
-                                        "greedy": cells are taken in the order given)                     */
+    HINES_POLICY_INPUT_ORDER  = 4,   /* launch work items in input order, not heaviest first, and group only cells that are
+                                        neighbours in the input ("greedy": cells are taken in the order given) */
     HINES_POLICY_SERIAL_CLASSES = 16, /* launch the size classes one after the other on the caller's stream instead
                                         of concurrently on plan-owned side streams (forked from / joined to it)  */
     HINES_POLICY_POW2_CLUSTERS = 32, /* cluster sizes 2, 4, 8, 16 only (default: any size up to cluster_max, the one
@@ -153,7 +153,9 @@ typedef enum {
      * A part's reduced forest has one node per segment (the segment's last compartment, the "separator");
      * node ids are part-local. */
     HINES_TABLE_CELL_ITEM            = 32,  /* int32[ncells]  on-chip work item of the cell, -1 = streaming path       */
-    HINES_TABLE_ITEM_CELL_RANGE      = 33,  /* int64[2*nitems] first cell, one-past-last cell (contiguous run)        */
+    HINES_TABLE_ITEM_CELL_OFFSETS    = 33,  /* int64[nitems+1] into ITEM_CELLS                                           */
+    HINES_TABLE_ITEM_CELLS           = 37,  /* int64[] cells of each item, ascending (a group of small cells need not be
+                                               neighbours in the input: large cells in between get items of their own)  */
     HINES_TABLE_ITEM_CLASS           = 34,  /* int32[nitems]  size class                                              */
     HINES_TABLE_ITEM_LAUNCH_ORDER    = 35,  /* int32[nitems]  items in launch order, per class heaviest first         */
     HINES_TABLE_ITEM_KIND            = 36,  /* int32[nitems]  0 = one part (a run of whole cells in one block), 1 = one cell cut

@@ -35,7 +35,7 @@ TABLES = {
     "branch_parent_comp": (3, np.int32), "branch_parent_branch": (4, np.int32), "branch_level": (5, np.int32),
     "cell_nlevels": (6, np.int32), "cell_level_offsets": (7, np.int64), "level_count": (8, np.int32),
     "level_list": (9, np.int32), "child_offsets": (10, np.int64), "child_ids": (11, np.int32),
-    "cell_item": (32, np.int32), "item_cell_range": (33, np.int64), "item_class": (34, np.int32),
+    "cell_item": (32, np.int32), "item_cell_offsets": (33, np.int64), "item_cells": (37, np.int64), "item_class": (34, np.int32),
     "item_launch_order": (35, np.int32), "item_kind": (36, np.int32), "item_xch": (44, np.int32),
     "item_part_offsets": (46, np.int64), "part_header": (47, np.int32), "part_meta": (48, np.int32),
     "part_runs": (49, np.int32),

@@ -189,34 +189,34 @@ static void fixed_bound_pieces(int32_t len, int32_t smax, std::vector<int32_t>& 
 
 struct NodeTmp { int32_t depth, pkey, gid, ghost; };
 
-// kind = single: cells [c0,c1) in one part.  kind = cluster: ONE cell in K parts, part 0 = top + sub-trees.
+// kind = single: the given cells (ascending, not necessarily adjacent) in one part.  kind = cluster: ONE cell in K parts, part 0 = top + sub-trees.
 // kind = split: ONE cell, part 0 = top alone, the sub-trees packed into parts of at most `slot` bytes (K is
 // then the result).
-static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t kind, int32_t K, int64_t slot, ItemBuild& out)
+static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, int32_t kind, int32_t K, int64_t slot, ItemBuild& out)
 {
     const int32_t w = P.width, E = 16 / w;
     const int32_t smax = kind == kItemSingle ? P.seg_single : P.seg_cluster;
     const bool level_mean = (P.opt.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN) != 0;
     out = ItemBuild();
     out.kind = kind;
-    out.comp_begin = P.cell_offsets[c0];
-    out.n = P.cell_offsets[c1] - out.comp_begin;
-    const int64_t B0 = P.cell_branch_offsets[c0];
-    const int32_t nb = (int32_t)(P.cell_branch_offsets[c1] - B0);
+    out.comp_begin = P.cell_offsets[cells.front()];
+    int32_t nb = 0;
+    for (int64_t c : cells) { nb += (int32_t)(P.cell_branch_offsets[c + 1] - P.cell_branch_offsets[c]); out.n += P.cell_offsets[c + 1] - P.cell_offsets[c]; }
     std::vector<Br> br(nb);
     std::vector<int32_t> pieces;
     pieces.reserve(nb + nb / 4);
-    int32_t nn = 0;
-    for (int64_t c = c0; c < c1; ++c) {
+    int32_t nn = 0, lb0 = 0;
+    for (int64_t c : cells) {
         const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
-        const int32_t shift = (int32_t)(P.cell_offsets[c] - out.comp_begin);
+        const int64_t shift64 = P.cell_offsets[c] - out.comp_begin;
+        const int32_t shift = (int32_t)shift64;
         for (int64_t j = b0; j < b1; ++j) {
-            Br& e = br[j - B0];
+            Br& e = br[lb0 + (j - b0)];
             e.start = P.branch_start[j] + shift;
             e.len = P.branch_len[j];
             e.pc = P.branch_parent_comp[j] < 0 ? -1 : P.branch_parent_comp[j] + shift;
             e.level = P.branch_level[j];
-            e.parent = P.branch_parent_branch[j] < 0 ? -1 : (int32_t)(b0 + P.branch_parent_branch[j] - B0);
+            e.parent = P.branch_parent_branch[j] < 0 ? -1 : lb0 + P.branch_parent_branch[j];
             e.piece0 = (int32_t)pieces.size();
             if (level_mean) {                           // the paper's pieces first, each then bounded
                 for (int64_t q = P.split_piece_offsets[j]; q < P.split_piece_offsets[j + 1]; ++q)
@@ -229,6 +229,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t kind
             e.node0 = nn;
             nn += e.nseg;
         }
+        lb0 += (int32_t)(b1 - b0);
     }
     out.nnode = nn;
     if (nn >= (1 << 20)) { out.ok = false; return; }
@@ -280,8 +281,11 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t kind
             if (kind == kItemCluster) {
                 np = K;
                 load.assign(K, 0); load[0] = top_bytes;
+                // from the last frontier root to the first: part 0, which also carries the top and sweeps it after the
+                // exchange, gets the sub-trees rooted deepest (the fewest levels of its own to sweep before that)
                 int64_t acc = top_bytes; int32_t r = 0;
-                for (int32_t f : frontier) {
+                for (size_t q = frontier.size(); q-- > 0;) {
+                    const int32_t f = frontier[q];
                     while (r < K - 1 && acc + sub[f] / 2 > total * (r + 1) / K) ++r;
                     part_of_root[f] = r; acc += sub[f]; load[r] += sub[f];
                 }
@@ -371,7 +375,7 @@ static void build_item(const hines_plan& P, int64_t c0, int64_t c1, int32_t kind
         // every cell of the part an unbranched cable of at most 32 nodes: the reduced systems are solved by
         // parallel cyclic reduction, one warp per cable; nodes are then numbered cable by cable (lb[] = first
         // node of each cable) instead of level by level
-        bool chains = kind == kItemSingle && next > 0 && (int64_t)mine.size() == c1 - c0;
+        bool chains = kind == kItemSingle && next > 0 && mine.size() == cells.size();
         if (chains) for (int32_t b : mine) if (br[b].nseg > 32 || br[b].parent >= 0) chains = false;
         if (chains && !(P.opt.policy_flags & HINES_POLICY_NO_PCR)) {
             pb.flags |= kPartFlagChains;
@@ -647,12 +651,13 @@ static void level_mean_split(hines_plan& P)
     for (const Piece& p : out) { const int64_t q = fill[p.j]++; P.split_piece_len[q] = p.len; P.split_piece_level[q] = p.level; }
 }
 
-static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib)
+static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const ItemBuild& ib)
 {
     const int32_t item = (int32_t)P.item_kind.size();
-    for (int64_t c = c0; c < c1; ++c) P.cell_item[c] = item;
-    P.item_cell_range.push_back(c0);
-    P.item_cell_range.push_back(c1);
+    for (int64_t c : cells) P.cell_item[c] = item;
+    P.item_cells.insert(P.item_cells.end(), cells.begin(), cells.end());
+    P.item_cell_offsets.push_back((int64_t)P.item_cells.size());
+    P.item_unknowns.push_back(ib.n);
     P.item_class.push_back(0);                     // filled by assign_classes
     P.item_kind.push_back(ib.kind);
     P.item_xch.push_back((int32_t)P.n_xch);
@@ -689,9 +694,10 @@ static void emit_item(hines_plan& P, int64_t c0, int64_t c1, const ItemBuild& ib
     if (ib.kind == kItemSplit) P.n_xch += ib.nxch;
     P.padded_lane_steps += ib.padded_steps;
     P.useful_lane_steps += ib.useful_steps;
-    if (ib.kind == kItemCluster) { P.n_cluster_cells += c1 - c0; P.n_cluster_unknowns += ib.n; }
-    if (ib.kind == kItemSplit) { P.n_split_cells += c1 - c0; P.n_split_unknowns += ib.n; }
-    P.n_resident_cells += c1 - c0;
+    const int64_t ncell = (int64_t)cells.size();
+    if (ib.kind == kItemCluster) { P.n_cluster_cells += ncell; P.n_cluster_unknowns += ib.n; }
+    if (ib.kind == kItemSplit) { P.n_split_cells += ncell; P.n_split_unknowns += ib.n; }
+    P.n_resident_cells += ncell;
     P.n_resident_unknowns += ib.n;
 }
 
@@ -720,14 +726,15 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     const int32_t w = P.width;
     P.cell_item.assign(nc, -1);
     P.item_part_offsets.assign(1, 0);
+    P.item_cell_offsets.assign(1, 0);
     is_stream.assign(nc, 0);
-    ItemBuild cur, cand, alone;
-    auto push = [&](int64_t a, int64_t b, const ItemBuild& ib) {
-        emit_item(P, a, b, ib);
+    ItemBuild cand, alone;
+    auto push = [&](const std::vector<int64_t>& cells, const ItemBuild& ib) {
+        emit_item(P, cells, ib);
         need.push_back({ib.smem_need, ib.max_lanes, (int32_t)ib.parts.size(), ib.kind, ib.smem_top, ib.max_lanes_top});
     };
     // additive estimate of a cell's shared-memory need as a single part (upper side): arrays + per node the
-    // record, two segment lanes and {kids, parent}; decides group membership without building the group
+    // record, two segment lanes and the node descriptor; decides group membership without building the group
     std::vector<int32_t> tmp;
     auto estimate = [&](int64_t c) -> int64_t {
         int64_t nodes = 0;
@@ -737,33 +744,44 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
             else fixed_bound_pieces(P.branch_len[j], P.seg_single, tmp);
             nodes += (int64_t)tmp.size();
         }
-        return 3 * (int64_t)w * (P.cell_offsets[c + 1] - P.cell_offsets[c]) + nodes * (6 * w + 32 + 8) + 4 * (P.cell_nlevels[c] + 1);
+        return 3 * (int64_t)w * (P.cell_offsets[c + 1] - P.cell_offsets[c] + 2) + nodes * (6 * w + 32 + 16) + 4 * (P.cell_nlevels[c] + 1);
     };
-    const int64_t group_fixed = 16 + 2048;          // mbarrier, alignment slack, padding of the lane list to whole warps
-    int64_t g0 = -1, gacc = 0;                      // first cell of the open group, its estimated need
-    // flush the open group [a, b): built once; should the build exceed the cap after all, halve it
-    std::function<void(int64_t, int64_t)> flush_range = [&](int64_t a, int64_t b) {
-        if (a >= b) return;
+    const int64_t group_fixed = 16 + 512 + 2048;    // mbarrier, block record, alignment slack, padding of the lane list to whole warps
+    // The open group: small cells in input order ("greedy"); a large cell in between gets an item of its
+    // own and does not close the group (a part is a list of runs: its cells need not be neighbours).
+    std::vector<int64_t> group;
+    int64_t gacc = 0;
+    // a closed group is built once; should the build exceed the cap after all, it is halved
+    std::function<void(const std::vector<int64_t>&)> flush_cells = [&](const std::vector<int64_t>& cells) {
+        if (cells.empty()) return;
         ItemBuild ib;
-        build_item(P, a, b, kItemSingle, 1, 0, ib);
-        if ((!ib.ok || ib.smem_need > group_cap) && b - a > 1) { const int64_t mid = (a + b) / 2; flush_range(a, mid); flush_range(mid, b); return; }
-        if (!ib.ok || ib.smem_need > max_smem) { for (int64_t c = a; c < b; ++c) is_stream[c] = 1; return; }
-        push(a, b, ib);
+        build_item(P, cells, kItemSingle, 1, 0, ib);
+        if ((!ib.ok || ib.smem_need > group_cap) && cells.size() > 1) {
+            const size_t mid = cells.size() / 2;
+            flush_cells(std::vector<int64_t>(cells.begin(), cells.begin() + mid));
+            flush_cells(std::vector<int64_t>(cells.begin() + mid, cells.end()));
+            return;
+        }
+        if (!ib.ok || ib.smem_need > max_smem) { for (int64_t c : cells) is_stream[c] = 1; return; }
+        push(cells, ib);
     };
-    auto flush = [&](int64_t c_end) { if (g0 >= 0) { flush_range(g0, c_end); g0 = -1; gacc = 0; } };
+    auto flush = [&]() { flush_cells(group); group.clear(); gacc = 0; };
+    const bool adjacent_only = (P.opt.policy_flags & HINES_POLICY_INPUT_ORDER) != 0;
+    std::vector<int64_t> one(1);
     for (int64_t c = 0; c < nc; ++c) {
         if (force_stream) { is_stream[c] = 1; continue; }
         const int64_t est = estimate(c);
         if (!no_group && est + group_fixed <= group_cap) {                  // a small cell: joins the open group, greedy in input order
-            if (g0 >= 0 && gacc + est + group_fixed > group_cap) flush(c);
-            if (g0 < 0) { g0 = c; gacc = 0; }
+            if (!group.empty() && (gacc + est + group_fixed > group_cap || group.size() >= 4096)) flush();
+            group.push_back(c);
             gacc += est;
             continue;
         }
-        flush(c);
+        if (adjacent_only) flush();
+        one[0] = c;
         bool placed = false, is_single = false;
         if (est <= single_cap + 4096) {
-            build_item(P, c, c + 1, kItemSingle, 1, 0, alone);
+            build_item(P, one, kItemSingle, 1, 0, alone);
             is_single = alone.ok && alone.smem_need <= single_cap;
         }
         if (!is_single && !no_cluster) {
@@ -787,33 +805,33 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
                 // and an option counts only if every part fits the slot it was chosen for
                 for (int32_t k = opts[o].k; k <= std::min<int32_t>(P.opt.cluster_max, opts[o].k + 2) && !placed; ++k) {
                     if (pow2_only && (k & (k - 1))) continue;
-                    build_item(P, c, c + 1, kItemCluster, k, 0, cand);
-                    if (cand.ok && cand.smem_need <= opts[o].slot) { push(c, c + 1, cand); placed = true; }
+                    build_item(P, one, kItemCluster, k, 0, cand);
+                    if (cand.ok && cand.smem_need <= opts[o].slot) { push(one, cand); placed = true; }
                 }
             }
             if (!placed) {                                                // anything that fits a block
                 for (int32_t k = opts.empty() ? P.opt.cluster_max : std::min<int32_t>(P.opt.cluster_max, opts[0].k + 3); k <= P.opt.cluster_max && !placed; k += std::max(1, k / 4)) {
                     if (pow2_only && (k & (k - 1))) continue;
-                    build_item(P, c, c + 1, kItemCluster, k, 0, cand);
-                    if (cand.ok && cand.smem_need <= max_smem) { push(c, c + 1, cand); placed = true; }
+                    build_item(P, one, kItemCluster, k, 0, cand);
+                    if (cand.ok && cand.smem_need <= max_smem) { push(one, cand); placed = true; }
                 }
             }
             if (!placed && est <= max_smem) {                             // one big block
-                build_item(P, c, c + 1, kItemSingle, 1, 0, alone);
+                build_item(P, one, kItemSingle, 1, 0, alone);
                 is_single = alone.ok && alone.smem_need <= max_smem;
             }
         }
         if (!placed && !is_single && !no_cluster && !no_split) {
             // beyond the largest cluster: sub-tree parts of at most a split_smem_bytes slot + the top part in one block
             const int64_t sslot = std::min<int64_t>(P.opt.split_smem_bytes, max_smem);
-            build_item(P, c, c + 1, kItemSplit, 0, sslot - 6144, cand);
-            if (cand.ok && cand.parts.size() > 1 && cand.smem_need <= sslot && cand.smem_top <= max_smem) { push(c, c + 1, cand); placed = true; }
+            build_item(P, one, kItemSplit, 0, sslot - 6144, cand);
+            if (cand.ok && cand.parts.size() > 1 && cand.smem_need <= sslot && cand.smem_top <= max_smem) { push(one, cand); placed = true; }
         }
         if (placed) continue;
         if (!is_single) { is_stream[c] = 1; continue; }
-        push(c, c + 1, alone);
+        push(one, alone);
     }
-    flush(nc);
+    flush();
 }
 
 // Size classes.  By how many blocks of that size fit one SM (1, 2, 3, 4, 6, 8), separately for single-block
@@ -873,7 +891,7 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
     P.item_launch_order.resize(nitems);
     std::iota(P.item_launch_order.begin(), P.item_launch_order.end(), 0);
     const bool input_order = P.opt.policy_flags & HINES_POLICY_INPUT_ORDER;
-    auto weight = [&](int32_t it) { return P.cell_offsets[P.item_cell_range[2 * (size_t)it + 1]] - P.cell_offsets[P.item_cell_range[2 * (size_t)it]]; };
+    auto weight = [&](int32_t it) { return P.item_unknowns[it]; };
     std::stable_sort(P.item_launch_order.begin(), P.item_launch_order.end(), [&](int32_t a, int32_t b) {
         if (P.item_class[a] != P.item_class[b]) return P.item_class[a] < P.item_class[b];
         if (input_order) return false;
@@ -1067,7 +1085,8 @@ hines_status_t hines_plan_get_table(const hines_plan_t* P, int32_t id, void* dst
         TBL(HINES_TABLE_CHILD_OFFSETS, P->child_offsets)
         TBL(HINES_TABLE_CHILD_IDS, P->child_ids)
         TBL(HINES_TABLE_CELL_ITEM, P->cell_item)
-        TBL(HINES_TABLE_ITEM_CELL_RANGE, P->item_cell_range)
+        TBL(HINES_TABLE_ITEM_CELL_OFFSETS, P->item_cell_offsets)
+        TBL(HINES_TABLE_ITEM_CELLS, P->item_cells)
         TBL(HINES_TABLE_ITEM_CLASS, P->item_class)
         TBL(HINES_TABLE_ITEM_LAUNCH_ORDER, P->item_launch_order)
         TBL(HINES_TABLE_ITEM_KIND, P->item_kind)

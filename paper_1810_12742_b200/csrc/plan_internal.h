@@ -100,7 +100,7 @@ struct hines_plan {
     std::vector<int64_t> split_level_stat;             // per level of the split tree: {sum of the piece lengths, pieces}
     // policy tables
     std::vector<int32_t> cell_item, item_class, item_kind, item_launch_order, item_xch;
-    std::vector<int64_t> item_cell_range, item_part_offsets;
+    std::vector<int64_t> item_cell_offsets, item_cells, item_unknowns, item_part_offsets;
     std::vector<hines::PartHeader> part_headers;       // indexed by part id (item order, parts of an item consecutive)
     std::vector<int32_t> part_meta;                    // device blob: per part [lb | kp | exports | ghosts | segment lanes]
     std::vector<int32_t> part_runs;                    // 4 ints per run, GLOBAL first compartment

@@ -148,6 +148,61 @@ def test_bad_pointers_rejected():
     assert e.value.status == 1
     with pytest.raises(hb.HinesError):
         plan.solve(t, t, t, t)                               # x aliases d
+    big = torch.zeros(4 * m.n + 64, dtype=torch.float64, device="cuda")
+    dd, du, db = big[:m.n], big[m.n:2 * m.n], big[2 * m.n:3 * m.n]
+    with pytest.raises(hb.HinesError) as e:
+        plan.solve(dd, du, db, big[2 * m.n + 2:3 * m.n + 2])  # x overlaps b without being b
+    assert e.value.status == 1
+    with pytest.raises(hb.HinesError):
+        plan.solve(dd, du, db, big[m.n - 2:2 * m.n - 2])      # x overlaps d and u
+    plan.solve(dd + 1.0, du, db, db)                          # exactly b: allowed
+    torch.cuda.synchronize()
+
+
+def test_two_live_plans_interleaved():
+    """a plan that needs the largest shared memory and a small one, solved in turn (kernel attributes
+    are per process, not per plan)."""
+    import torch
+    import paper_1810_12742_b200 as hb
+    ma, mb_ = mg.make_config(2, 0.004), mg.make_config(0)
+    pa = hb.Plan(ma.parent, ma.cell_offsets, policy_flags=hb.POLICY_NO_CLUSTER, chunk_smem_bytes=227 * 1024)
+    pb = hb.Plan(mb_.parent, mb_.cell_offsets)
+    assert pa.table("class_smem_bytes").max() > 150 * 1024 > pb.table("class_smem_bytes").max()
+    sa, sb = mg.system(ma), mg.system(mb_)
+    ta = [torch.from_numpy(a).cuda() for a in sa]; tb = [torch.from_numpy(a).cuda() for a in sb]
+    xa, xb = torch.empty_like(ta[0]), torch.empty_like(tb[0])
+    for _ in range(3):
+        pa.solve(*ta, xa); pb.solve(*tb, xb)
+    torch.cuda.synchronize()
+    for m_, s_, x_ in ((ma, sa, xa), (mb_, sb, xb)):
+        xr = oracle.hines_solve(m_.parent, m_.cell_offsets, *s_)
+        xg = x_.cpu().numpy()
+        assert np.isfinite(xg).all() and oracle.rel_err(m_.cell_offsets, xg, xr).max() < 1e-10
+
+
+@pytest.mark.parametrize("kw", [dict(max_segment=8), dict(max_segment=8, dtype=np.float32), {}])
+def test_long_root_branch_with_fork(kw):
+    """20,000-compartment root branch with a fork at its end (thousands of reduced nodes on one chain)."""
+    n = 20000
+    p = np.arange(-1, n + 1, dtype=np.int32)
+    p[n + 1] = n - 1
+    m = mg.Morphology(p, np.array([0, n + 2], np.int64))
+    d, u, b = mg.system(m, seed=3)
+    kw = dict(kw); dtype = kw.pop("dtype", np.float64)
+    _check(m, d, u, b, dtype, **kw)
+
+
+@pytest.mark.parametrize("kw", [dict(smem_bytes_per_block=48000, cluster_max=2, split_smem_bytes=20000),
+                                dict(smem_bytes_per_block=64000, cluster_max=2, split_smem_bytes=12000, max_segment=9),
+                                dict(smem_bytes_per_block=100000, chunk_smem_bytes=30000, cluster_max=3, split_smem_bytes=30000)])
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_split_items(kw, dtype):
+    """Cells beyond the largest cluster: sub-tree parts backward + export, top part, sub-tree parts again (three launches),
+    beside ordinary items in the same solve."""
+    m = mg.make_config(2, 0.006)
+    d, u, b = mg.system(m)
+    _, info = _check(m, d, u, b, dtype, **kw)
+    assert info.n_split_cells > 0 and info.n_blocks > info.n_parts
 
 
 # ---- full BASELINE.json sizes, in the launch configuration bench.py times ----------------------

@@ -13,7 +13,7 @@ import morphgen as mg
 import oracle
 import paper_1810_12742_b200 as hb
 from helpers import random_parent
-from plan_interpreter import pairs, parse_tasks
+from plan_interpreter import pairs, parts_of
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -28,7 +28,7 @@ def test_library_exports_every_declared_symbol():
         assert getattr(lib, name) is not None
     assert "sm_100a" in hb.version()
     # struct sizes agree with the header's layout
-    assert ctypes.sizeof(hb.Options) == 36 and ctypes.sizeof(hb.PlanInfo) == 152
+    assert ctypes.sizeof(hb.Options) == 40 and ctypes.sizeof(hb.PlanInfo) == 184
 
 
 def _plan_cfg(cfg, scale, **kw):
@@ -92,158 +92,148 @@ def test_validation_errors():
     assert lib.hines_status_string(4) == b"CUDA error"
 
 
+
+
+def _pieces_fixed(ln, S):
+    """Pieces of a branch of ln compartments under the fixed-bound rule, top-down (P4)."""
+    nseg = max(1, (5 * ln + 2 * S) // (5 * S))             # len / max_segment + 0.4, cut off
+    sj = -(-ln // nseg)
+    if nseg > 1 and sj % 2 == 0:
+        sj += 1                                            # odd: the segments of a branch start on distinct banks
+    nseg = -(-ln // sj)                                    # no empty segment
+    return [ln - (nseg - 1) * sj] + [sj] * (nseg - 1)
+
+
 def _check_policy(m, plan, max_segment=0):
-    """Validity invariants (policy-free): every cell in exactly one on-chip item or on the streaming
-    path; the chunks of an item tile its compartment range; segments tile every branch exactly, each
-    inside one chunk and listed once; node ids are unique; a segment's upper node is the node of the
-    compartment above it; every branch has one lane on its level; sibling groups of at most 32 sit in
-    one 32-lane tile and their first lane absorbs the others, larger groups are pulled one by one;
-    shared-memory need within the class; launch order a permutation."""
+    """Validity invariants (policy-free): every cell in exactly one on-chip item or on the streaming path; the runs of
+    an item's parts tile the compartments of its cells exactly once; segments tile every branch exactly, in the
+    pieces the written rule gives, each listed once; a segment's upper node is the node of the compartment above it
+    (a ghost parent when that compartment lives in another part); every node once on the level of its depth,
+    children consecutive behind their parent; exports and ghost children pair up one to one; shared-memory need
+    within the class; every part launched exactly once per phase."""
     T = oracle.tables(m.parent, m.cell_offsets)
     w = 8 if plan.dtype == hb.F64 else 4
     E = 16 // w
     cell_item = plan.table("cell_item")
-    rng_ = plan.table("item_cell_range").reshape(-1, 2)
-    pnode = plan.table("item_pnode")
-    nnode = plan.table("item_nnode")
-    node_off = plan.table("item_node_offsets")
-    rounds = plan.table("item_rounds")
-    ch_off = plan.table("item_chunk_offsets")
-    ch_rng = plan.table("chunk_comp_range").reshape(-1, 2)
-    seg_off = plan.table("chunk_seg_offsets")
-    segs = plan.table("chunk_seg").reshape(-1, 4)
+    co, cells = plan.table("item_cell_offsets"), plan.table("item_cells")
+    kind = plan.table("item_kind")
+    poff = plan.table("item_part_offsets")
     cls = plan.table("item_class")
-    cls_smem = plan.table("class_smem_bytes")
-    cls_cluster = plan.table("class_cluster")
-    cls_threads = plan.table("class_threads")
+    cls_smem, cls_cluster = plan.table("class_smem_bytes"), plan.table("class_cluster")
+    cls_threads, cls_phase = plan.table("class_threads"), plan.table("class_phase")
+    cfirst, ccount, cparts = plan.table("class_first"), plan.table("class_count"), plan.table("class_parts")
     order = plan.table("item_launch_order")
-    nitems = len(cls)
-    assert sorted(order.tolist()) == list(range(nitems))
-    assert (np.diff(cls[order]) >= 0).all()
-    assert ((cls_threads % 32 == 0) & (cls_threads >= 32) & (cls_threads <= 1024)).all()
+    parts = parts_of(plan)
+    nitems = len(kind)
     info = plan.info
-    assert info.n_resident_items == nitems and info.n_chunks == len(ch_rng)
-    seen_cells = np.zeros(m.ncells, bool)
+    assert sorted(order.tolist()) == list(range(nitems))
+    assert ((cls_threads % 32 == 0) & (cls_threads >= 32) & (cls_threads <= 1024)).all()
+    assert info.n_resident_items == nitems and info.n_parts == len(parts) and info.n_blocks == len(cparts)
+    # launches: every part of an ordinary item once; a split item's sub-tree parts in phases A and C, its top in B
+    launched = {}
+    for q in range(len(cfirst)):
+        ids = cparts[cfirst[q]:cfirst[q] + ccount[q]]
+        assert ccount[q] % cls_cluster[q] == 0
+        for k, pid in enumerate(ids):
+            h = parts[pid].h
+            launched.setdefault(int(pid), []).append(int(cls_phase[q]))
+            need = 16 + 512 + 6 * w * (-(-(h["nnode"] + 1) // E) * E) + 4 * h["meta_len"] + 3 * w * h["L"]
+            assert need <= cls_smem[q] <= 232448
+            assert h["maxwidth"] <= cls_threads[q] or True
+            if cls_cluster[q] > 1:
+                assert h["rank"] == k % cls_cluster[q] and kind[h["item"]] == 1
     useful = 0
     nsep_total = 0
+    seen_cells = np.zeros(m.ncells, bool)
     for it in range(nitems):
-        c0, c1 = rng_[it]
-        assert c1 > c0 and (cell_item[c0:c1] == it).all()
-        seen_cells[c0:c1] = True
-        comp0 = m.cell_offsets[c0]; n_it = m.cell_offsets[c1] - comp0
-        nch = ch_off[it + 1] - ch_off[it]
-        assert nch == cls_cluster[cls[it]] and (nch == 1 or c1 - c0 == 1)
-        cr = ch_rng[ch_off[it]:ch_off[it + 1]]
-        assert cr[0, 0] == comp0 and cr[-1, 1] == comp0 + n_it and (cr[1:, 0] == cr[:-1, 1]).all()
-        pn_sweep = pnode[node_off[it]:node_off[it + 1]]
-        # ITEM_PNODE is the parent the FORWARD sweep reads: a node of a lane chain that ends in a root is final
-        # after the backward sweep's turn-around and reads itself.  pn = the parent in the reduced tree: for those
-        # nodes the next entry of the lane's chain (node id = entry index).
-        pn = pn_sweep.copy()
-        blob_ = plan.table("item_task_blob")[plan.table("item_task_offsets")[it]:plan.table("item_task_offsets")[it + 1]]
-        tiers_ = parse_tasks(blob_)
-        any_turn = any(g_[3] for t_ in tiers_ for g_ in t_[1])     # all root chains of an item turn around, or none
-        for _t, groups_, _e, _p, _r in tiers_:
-            for gh_, _ns, _nsh, turn_ in groups_:
-                for l_ in range(32):
-                    b_, e_ = int(gh_[l_]), int(gh_[l_ + 1])
-                    if (turn_ >> l_) & 1:
-                        assert e_ > b_ and (pn_sweep[b_:e_] == np.arange(b_, e_)).all()
-                        pn[b_:e_ - 1] = np.arange(b_ + 1, e_)
-                    elif e_ > b_ and any_turn:
-                        assert pn_sweep[e_ - 1] != e_ - 1          # a chain that ends in a root turns around
-        assert len(pn) == nnode[it]
-        # segments of all chunks -> node of every separator compartment (item-local position)
-        node_at = {}                     # separator position -> node
-        seg_of_node = {}
-        covered = np.zeros(n_it, int)
-        nlanes_max = 0
-        # segment target of the item: the option, or by default 40 in a block of its own, 64 in a cluster
-        S_it = max_segment if max_segment else (40 if ch_off[it + 1] - ch_off[it] == 1 else 64)
-        for r, ch in enumerate(range(ch_off[it], ch_off[it + 1])):
-            sg = segs[seg_off[ch]:seg_off[ch + 1]]
-            nlanes_max = max(nlanes_max, len(sg))
-            base = cr[r, 0] - comp0
-            for a, mt_, mb_, hasq_, node, tnode in pairs(sg):
-                mm = mt_ + mb_ + hasq_
-                assert 0 <= node < nnode[it] and node not in seg_of_node
-                assert 0 <= a and a + mm < cr[r, 1] - cr[r, 0] and 0 <= mm < 2 * S_it
-                seg_of_node[int(node)] = (int(base + a), int(mm), int(tnode))
-                node_at[int(base + a + mm)] = int(node)
-                covered[base + a:base + a + mm + 1] += 1
-                useful += int(mm)
-            L = -(-(cr[r, 0] % E + cr[r, 1] - cr[r, 0]) // E) * E
-            tb = plan.table("item_task_offsets")
-            meta = int(tb[it + 1] - tb[it]) + -(-nnode[it] // 4) * 4
-            need = 16 + 3 * L * w + 16 * len(sg) + (6 * (-(-nnode[it] // E) * E) * w + 4 * meta if r == 0 else 0)
-            assert need <= cls_smem[cls[it]] <= 232448
-        assert (covered == 1).all()
-        nsep_total += len(seg_of_node)
-        # branches: one lane each, on its level; node chain from the top: e, rest, rest+1, ...
-        want = {}
-        for c in range(c0, c1):
-            sh = m.cell_offsets[c] - comp0
-            for j in range(T.cell_branch_offsets[c], T.cell_branch_offsets[c + 1]):
-                pc = T.branch_parent_comp[j]
-                want[int(T.branch_start[j] + sh)] = (int(T.branch_len[j]), -1 if pc < 0 else int(pc + sh), int(T.branch_level[j]))
-        seg_at = {a: (mm, node, t) for node, (a, mm, t) in seg_of_node.items()}       # by first compartment
-        lanes_seen = set()
-        for start, (ln, pc, lw) in want.items():
-            nseg = max(1, (5 * ln + 2 * S_it) // (5 * S_it))       # len / max_segment + 0.4, cut off
-            sj = -(-ln // nseg)
-            if nseg > 1 and sj % 2 == 0:
-                sj += 1                                      # odd: the segments of a branch start on distinct banks
-            nseg = -(-ln // sj)                              # no empty segment
-            end = start + ln - 1
-            prev = node_at[pc] if pc >= 0 else -1
-            for k in range(nseg):                            # k-th segment from the top
-                q = nseg - 1 - k
-                b_ = end - q * sj
-                a_ = max(start, b_ - sj + 1)
-                mm, node, tn = seg_at[a_]
-                assert mm == b_ - a_ and tn == prev, (it, start, k)
-                assert pn[node] == (prev if prev >= 0 else node)             # a root reads itself (its f is 0)
-                prev = node
-            lanes_seen.add(start)
-        assert len(lanes_seen) == len(want) and len(seg_of_node) == nnode[it]
-        # backward-sweep tasks: every node once; a node's step is above its children's; children of the same
-        # tier sit in the same group: the first in the node's own lane, the others in its lane mask; children
-        # of earlier tiers are in its pull list; at most 32 lanes per group
-        blob = plan.table("item_task_blob")[plan.table("item_task_offsets")[it]:plan.table("item_task_offsets")[it + 1]]
+        cs = cells[co[it]:co[it + 1]]
+        assert len(cs) > 0 and (np.diff(cs) > 0).all() and (cell_item[cs] == it).all()
+        assert not seen_cells[cs].any()
+        seen_cells[cs] = True
+        ps = parts[poff[it]:poff[it + 1]]
+        assert (kind[it] == 0) == (len(ps) == 1) and (kind[it] == 0 or len(cs) == 1)
+        for r, p in enumerate(ps):
+            want_ph = [0] if kind[it] != 2 else ([2] if r == 0 else [1, 3])
+            assert launched[poff[it] + r] == want_ph
+        S_it = max_segment if max_segment else (40 if kind[it] == 0 else 64)
+        # compartments -> (part, staged index); runs tile the item's cells exactly once
         where = {}
-        for tier, groups, ents, pull, raw in parse_tasks(blob):
-            for gi, (gh, nsteps, nsh, _turn) in enumerate(groups):
-                for lane in range(32):
-                    prev = None
-                    for k in range(int(gh[lane]), int(gh[lane + 1])):
-                        node, step = int(ents[k, 0]) & 0xfffff, (int(ents[k, 0]) >> 20) & 0xfff
-                        assert node not in where and step < nsteps
-                        where[node] = (tier, gi, lane, step, k)
-                        if prev is not None:                 # the lane's chain: each node the parent of the one before
-                            assert pn[prev[0]] == node and step >= prev[1]
-                        prev = (node, step)
-        assert sorted(where) == list(range(nnode[it]))
-        kids_of = {}
-        for v in range(nnode[it]):
-            if pn[v] != v:
-                kids_of.setdefault(int(pn[v]), []).append(v)
-        _, _, ents, pull, _ = parse_tasks(blob)[0]
-        for v, (tier, gi, lane, step, k) in where.items():
-            same = [c for c in kids_of.get(v, []) if where[c][0] == tier]
-            lower = [c for c in kids_of.get(v, []) if where[c][0] != tier]
-            assert all(where[c][0] < tier for c in lower)
-            assert sorted(int(c) for c in pull[int(ents[k, 2]):int(ents[k, 2]) + (int(ents[k, 3]) & 0xffff)]) == sorted(lower)
-            mask = int(ents[k, 1]) & 0xffffffff
-            if same:
-                assert all(where[c][1] == gi for c in same)
-                if where[same[0]][3] == step:                # a run (plain chains only): the single child's step
-                    assert len(same) == 1 and mask == 0
-                else:
-                    assert all(where[c][3] < step for c in same)
-                assert where[min(same)][2] == lane
-                assert mask == sum(1 << where[c][2] for c in same if c != min(same))
-            else:
-                assert mask == 0 and (lower or step == 0)
+        for r, p in enumerate(ps):
+            for g, ln, so, _ in p.runs:
+                for k in range(int(ln)):
+                    assert int(g) + k not in where
+                    where[int(g) + k] = (r, int(so) + k)
+        want_comps = np.concatenate([np.arange(m.cell_offsets[c], m.cell_offsets[c + 1]) for c in cs])
+        assert sorted(where) == want_comps.tolist()
+        # segments of every part: separator position -> node
+        node_at = {}                                       # global compartment -> (part, node)
+        seg_at = {}                                        # global first compartment -> (part, interior, node, tnode)
+        for r, p in enumerate(ps):
+            inv = {v: k for k, (pr, v) in where.items() if pr == r}
+            seen_nodes = set()
+            for a, mt, mb, hasq, node, tnode in pairs(p.seg):
+                mm = mt + mb + hasq
+                assert 0 <= node < p.h["nlevnode"] and node not in seen_nodes and not p.ghost[node]
+                seen_nodes.add(node)
+                g0 = inv[a]
+                assert all(inv[a + k] == g0 + k for k in range(mm + 1)), "a segment is contiguous in memory and in the staging"
+                seg_at[g0] = (r, mm, node, tnode)
+                node_at[g0 + mm] = (r, node)
+                useful += mm
+            assert len(seen_nodes) == int((~p.ghost[:p.h["nlevnode"]]).sum())
+            nsep_total += len(seen_nodes)
+        # branches: the written pieces, one segment each, chained from the top; the node above a branch's first
+        # piece is the node of its parent compartment, through a ghost parent when that lives in part 0
+        level_of = []
+        for p in ps:
+            lv = np.zeros(p.h["nlevnode"], int)
+            if not p.chains:
+                for l in range(p.h["nlev"]):
+                    lv[p.lb[l]:p.lb[l + 1]] = l
+            level_of.append(lv)
+        exports = {(r, int(e[0])): e for r, p in enumerate(ps) for e in p.exps}
+        n_exp_seen = 0
+        for c in cs:
+            o = int(m.cell_offsets[c])
+            for j in range(T.cell_branch_offsets[c], T.cell_branch_offsets[c + 1]):
+                start, ln, pc = o + int(T.branch_start[j]), int(T.branch_len[j]), int(T.branch_parent_comp[j])
+                prev = None if pc < 0 else node_at[o + pc]
+                pos = start
+                for k, plen in enumerate(_pieces_fixed(ln, S_it)):
+                    r, mm, node, tnode = seg_at[pos]
+                    p = ps[r]
+                    assert mm == plen - 1, (it, j, k)
+                    if prev is None:
+                        assert tnode == -1 and p.pnode[node] == node
+                    elif prev[0] == r:
+                        assert tnode == prev[1] and p.pnode[node] == prev[1]
+                        if not p.chains:
+                            assert level_of[r][node] == level_of[r][prev[1]] + 1
+                            assert node in p.children(prev[1], w)
+                    else:                                      # an exported sub-tree root
+                        assert k == 0 and r > 0 and prev[0] == 0
+                        e = exports[(r, node)]
+                        assert tnode == e[3] >= p.h["nlevnode"] and p.pnode[node] == e[3]
+                        gl = [g for g in ps[0].ghosts if g[1] == e[1]] if kind[it] == 2 else [g for g in ps[0].ghosts if g[0] == e[1]]
+                        assert len(gl) == 1 and gl[0][2] == prev[1] and ps[0].ghost[gl[0][0]]
+                        assert int(gl[0][0]) in ps[0].children(prev[1], w)
+                        n_exp_seen += 1
+                    prev = (r, node)
+                    pos += plen
+                assert pos == start + ln
+        assert n_exp_seen == sum(p.h["nexp"] for p in ps) == ps[0].h["nghost"]
+        for p in ps:                                           # every child listed belongs to its parent
+            if p.chains:
+                continue
+            assert p.h["maxwidth"] == max([0] + [int(p.lb[l + 1] - p.lb[l]) for l in range(p.h["nlev"])])
+            nkids = 0
+            for v in range(p.h["nlevnode"]):
+                if not p.ghost[v]:
+                    for ch in p.children(v, w):
+                        assert p.ghost[ch] or p.pnode[ch] == v
+                        nkids += 1
+            roots = sum(1 for v in range(p.h["nlevnode"]) if not p.ghost[v] and (p.pnode[v] == v or p.pnode[v] >= p.h["nlevnode"]))
+            assert nkids + roots == p.h["nlevnode"]
     assert (seen_cells == (cell_item >= 0)).all()
     # streaming path: every branch of every non-resident cell exactly once, children complete
     sd = plan.table("stream_desc").reshape(-1, 6)
@@ -293,9 +283,13 @@ def _check_interpreted(m, plan):
     (2, 0.004, {}), (2, 0.004, dict(smem_bytes_per_block=60000, policy_flags=hb.POLICY_NO_CLUSTER)),
     (2, 0.003, dict(policy_flags=hb.POLICY_FORCE_STREAM)),
     (3, 0.002, {}), (3, 0.002, dict(dtype=hb.F32)), (1, 0.002, {}), (1, 0.002, dict(max_segment=7)),
+    (1, 0.002, dict(policy_flags=hb.POLICY_NO_PCR)), (3, 0.002, dict(policy_flags=hb.POLICY_INPUT_ORDER)),
     (2, 0.003, dict(max_segment=2)), (3, 0.002, dict(max_segment=16)),
     (2, 0.004, dict(chunk_smem_bytes=30000, cluster_max=16)), (1, 0.002, dict(max_segment=5, chunk_smem_bytes=8000)),
     (3, 0.002, dict(chunk_smem_bytes=40000, cluster_max=4)),
+    (2, 0.002, dict(chunk_smem_bytes=20000, cluster_max=2, split_smem_bytes=20000)),
+    (2, 0.004, dict(smem_bytes_per_block=48000, cluster_max=2, split_smem_bytes=20000)),
+    (2, 0.004, dict(smem_bytes_per_block=64000, cluster_max=2, split_smem_bytes=12000, max_segment=9)),
 ])
 def test_policy_tables_valid(cfg, scale, kw):
     m, plan = _plan_cfg(cfg, scale, **kw)
@@ -304,7 +298,7 @@ def test_policy_tables_valid(cfg, scale, kw):
 
 
 def test_policy_star_with_many_siblings_and_odd_offsets():
-    star = np.array([-1] + [0] * 70, np.int32)                        # 70 siblings: more than a tile -> pulled one by one
+    star = np.array([-1] + [0] * 70, np.int32)                        # 70 siblings: beyond the two child slots -> the loop
     ps = [star, random_parent(33, 1), np.array([-1], np.int32), random_parent(200, 2, .7), star[:40],
           random_parent(1001, 3, .97)]
     offs = np.concatenate([[0], np.cumsum([len(p) for p in ps])])
@@ -314,14 +308,13 @@ def test_policy_star_with_many_siblings_and_odd_offsets():
         plan = hb.Plan(m.parent, m.cell_offsets, **kw)
         _check_policy(m, plan, kw.get("max_segment", 0))
         _check_interpreted(m, plan)
-        blob = plan.table("item_task_blob")[:plan.table("item_task_offsets")[1]]
-        assert any(int(e[3]) == 70 for t in parse_tasks(blob)[:1] for e in t[2])      # the star's root pulls its 70 children
+        assert max(int(p.nc.max()) for p in parts_of(plan)) == 70    # the star's root pulls its 70 children
 
 
 def test_clusters_take_the_cells_too_large_for_one_block():
     m, plan = _plan_cfg(3, 0.004)
     info = plan.info
-    assert info.n_cluster_cells > 0 and info.n_stream_cells == 0
+    assert info.n_cluster_cells > 0 and info.n_stream_cells == 0 and info.n_split_cells == 0
     cl = plan.table("class_cluster")
     assert cl.min() == 1 and cl.max() <= 16 and (np.diff(cl) <= 0).all()
     m, plan = _plan_cfg(3, 0.004, policy_flags=hb.POLICY_POW2_CLUSTERS)
@@ -330,15 +323,33 @@ def test_clusters_take_the_cells_too_large_for_one_block():
     assert plan.info.n_cluster_cells == 0 and (plan.table("class_cluster") == 1).all()
 
 
-def test_config4_goes_to_streaming_path_and_grouping_is_greedy_in_order():
+def test_config4_is_a_split_item_and_grouping_is_greedy_in_order():
+    """Config 4 (one cell of 1.3 M unknowns, beyond any cluster) runs as a split item: sub-tree parts backward, the
+    top part, the sub-tree parts again -- three launches, no streaming path."""
     m, plan = _plan_cfg(4, 1.0)
     info = plan.info
-    assert info.n_stream_cells == 1 and info.n_resident_items == 0 and plan.launches_per_solve == 34
-    # config 0: 64 cells x 75 unknowns: greedy contiguous groups up to 56 KiB
+    assert info.n_split_cells == 1 and info.n_stream_cells == 0 and info.n_resident_items == 1
+    assert plan.table("class_phase").tolist() == [1, 2, 3] and plan.launches_per_solve == 3
+    assert info.n_exports == info.n_parts - 1 == 512
+    _check_policy(m, plan)
+    m, plan = _plan_cfg(4, 1.0, policy_flags=hb.POLICY_NO_SPLIT)
+    assert plan.info.n_stream_cells == 1 and plan.launches_per_solve == 34
+    # config 0: 64 cells x 75 unknowns: greedy groups in input order up to 56 KiB
     m, plan = _plan_cfg(0, 1.0)
-    r = plan.table("item_cell_range").reshape(-1, 2)
-    assert r[0, 0] == 0 and r[-1, 1] == 64 and (r[1:, 0] == r[:-1, 1]).all()
-    assert plan.info.n_stream_cells == 0 and len(r) < 64
+    co, cells = plan.table("item_cell_offsets"), plan.table("item_cells")
+    assert cells.tolist() == list(range(64)) and plan.info.n_stream_cells == 0 and len(co) - 1 < 64
+
+
+def test_long_root_branch_with_a_fork_takes_a_correct_path():
+    """a very long root branch (thousands of reduced nodes) with a fork at its end.  Whatever path the
+    plan picks, the tables must solve the system (no descriptor field may wrap)."""
+    n = 20000
+    p = np.arange(-1, n + 1, dtype=np.int32)
+    p[n + 1] = n - 1                                                  # two children at the end of the root branch
+    m = mg.Morphology(p, np.array([0, n + 2], np.int64))
+    for kw in (dict(max_segment=8), dict(max_segment=8, dtype=hb.F32), {}):
+        plan = hb.Plan(m.parent, m.cell_offsets, **kw)
+        _check_interpreted(m, plan)
 
 
 def test_solve_without_gpu_fails_loudly():
