@@ -4,16 +4,19 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--dtype f64|f32] [--impl ours|reference]
 
 A "step" is one pass of the whole hot path (hines_solve: load, backward elimination, hand-off, root
-solve, forward substitution, store; SURVEY.md §8(a) a5-a10) over one batch of synthetic input
-(BASELINE.json config C, seeded, morphgen/).  Prints ONE JSON line (rank 0).
+solve, forward substitution, store; SURVEY.md section 8(a) a5-a10) over one batch of synthetic input
+(BASELINE.json config C, seeded, morphgen/).  Default config: 3, the largest single-GPU configuration
+(BASELINE.json's metric names none).  Prints ONE JSON line (rank 0).
 
-  value      whole-job unknowns/s with inputs resident in HBM (CUDA events on the launching stream,
-             barrier + synchronize on both sides, max over ranks)
+  value      whole-job unknowns/s with inputs resident in HBM: exactly K steps between two CUDA events on the
+             launching stream, barrier + synchronize on both sides, max over ranks
+  timing     the same in >= 20 intervals of >= 50 ms each: median and best ms per step
   e2e        the same through hines_solve_host: pinned HOST buffers, H2D of d,u,b and D2H of x inside
              the timed region every step
   roofline   HBM: algorithmic bytes (bytes_min = N*4w + 4*branches) / device time of the kernels of one
              step, against MEASURED_PEAKS.json hbm_gbs
   cpu_baseline  the oracle as it stands, timed on this box's host cores (rank 0, N=1 only)
+  other_configs the remaining configs, each with its own roofline / parity / clocks block
 
 N > 1 (torchrun): cells are independent, so each rank solves its own batch of the same
 size with no collective on the data path: weak scaling.
@@ -22,6 +25,7 @@ size with no collective on the data path: weak scaling.
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -42,6 +46,8 @@ METRIC = "hines_unknowns_solved_per_sec"
 UNIT = "unknowns/s"
 L2_BYTES = 126 * 1024 * 1024
 FALLBACK_HBM_GBS = 6650.0     # /opt/skills/guides/B200_PROFILING.md fallback
+INTERVAL_MS = 50.0            # every timed interval at least this long
+N_INTERVALS = 20
 
 
 def peak_hbm():
@@ -60,6 +66,35 @@ def workload(cfg: int, scale: float, rank: int):
     return m, d, u, b, seed
 
 
+def config_block(cfg: int, scale: float, m):
+    """The keys both arms print under "config" (identical in the two arms)."""
+    return {"workload": mg.CONFIG_NAMES[cfg], "scale": scale, "unknowns": int(m.n), "cells": int(m.ncells)}
+
+
+def kernel_hash() -> str:
+    """Identifies the kernel + planner sources a measured traffic figure belongs to."""
+    h = hashlib.sha256()
+    for f in ("paper_1810_12742_b200/csrc/solve.cu", "paper_1810_12742_b200/csrc/plan.cpp",
+              "paper_1810_12742_b200/csrc/plan_internal.h"):
+        h.update(open(os.path.join(ROOT, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def load_traffic(key):
+    """dram__bytes_read.sum + dram__bytes_write.sum of all kernels of one step, from a committed ncu capture
+    (profiles/traffic.csv: key,bytes,source_hash,command; see profiles/traffic.md) -- or None when that capture
+    was made with other kernel sources than the ones in the tree (it would be stale)."""
+    try:
+        cur = kernel_hash()
+        for line in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
+            f = line.split(",", 3)
+            if f[0] == key and f[2] == cur:
+                return int(f[1])
+    except Exception:
+        pass
+    return None
+
+
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled while the GPU is under load."""
@@ -71,7 +106,7 @@ class ClockSampler:
         self.rows, self.proc = [], None
         try:
             self.proc = subprocess.Popen(
-                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(index)],
+                ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "20", "-i", str(index)],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -82,12 +117,10 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
-    def stop(self, windows):
+    def summary(self, windows):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.15)
-        self.proc.terminate()
-        rows = [r for (t, r) in self.rows if any(a <= t <= b for a, b in windows)] or [r for _, r in self.rows]
+        rows = [r for (t, r) in list(self.rows) if any(a <= t <= b for a, b in windows)]
         sm, mx, pw, reasons = [], [], [], set()
         for r in rows:
             f = [x.strip() for x in r.split(",")]
@@ -100,6 +133,11 @@ class ClockSampler:
                     reasons.add(name)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
                 "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+    def stop(self):
+        if self.proc is not None:
+            time.sleep(0.05)
+            self.proc.terminate()
 
 
 # ------------------------------------------------------------------------------------------------
@@ -124,26 +162,54 @@ def cpu_oracle_time(m, d, u, b, threads: int, reps: int):
     return best, len(jobs), x
 
 
+def head_sample(m, d, u, b, max_unknowns):
+    """Whole cells from the start of the batch, at most max_unknowns (at least one cell)."""
+    ncs = int(np.searchsorted(m.cell_offsets, min(m.n, max_unknowns), side="right")) - 1
+    ncs = max(1, min(ncs, m.ncells))
+    ns = int(m.cell_offsets[ncs])
+    return mg.Morphology(m.parent[:ns], m.cell_offsets[:ncs + 1]), d[:ns], u[:ns], b[:ns], ncs
+
+
+def sampled_parity(m, d, u, b, x_gpu, np_dtype, max_unknowns=12_000_000):
+    """Max per-cell relative max-norm error of the GPU solution against the oracle (reading S15), on every cell when
+    the batch is small, else on every k-th cell (about max_unknowns unknowns): the oracle solves exactly those cells."""
+    import oracle
+    k = max(1, int(np.ceil(m.n / max_unknowns)))
+    sel = np.arange(0, m.ncells, k)
+    lo, hi = m.cell_offsets[sel], m.cell_offsets[sel + 1]
+    idx = np.concatenate([np.arange(a, b_) for a, b_ in zip(lo, hi)]) if k > 1 else slice(None)
+    offs = np.concatenate([[0], np.cumsum(hi - lo)]).astype(np.int64)
+    rd = lambda a: np.ascontiguousarray(a[idx], np_dtype).astype(np.float64)       # the oracle sees the rounded inputs
+    xr = oracle.hines_solve(m.parent[idx], offs, rd(d), rd(u), rd(b))
+    xg = np.ascontiguousarray(x_gpu[idx], np.float64)
+    finite = bool(np.isfinite(x_gpu).all())
+    err = float(oracle.rel_err(offs, xg, xr).max())
+    return {"max_rel_err": err if finite else float("nan"), "finite": finite, "cells_checked": int(len(sel)),
+            "unknowns_checked": int(offs[-1]), "every_kth_cell": k}
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     m, d, u, b, _ = workload(args.config, args.scale, 0)
     cores = os.cpu_count() or 1
-    times = []
+    ms_, ds, us, bs, ncs = head_sample(m, d, u, b, 40_000_000)     # bounded sample of the workload per step
+    times, used = [], 1
     for i in range(args.warmup + args.steps):
-        t, used, _ = cpu_oracle_time(m, d, u, b, cores, 1)
+        t, used, _ = cpu_oracle_time(ms_, ds, us, bs, cores, 1)
         if i >= args.warmup:
             times.append(t)
     tot = sum(times)
-    value = m.n * len(times) / tot
+    value = ms_.n * len(times) / tot
+    sample = (f"each step = the first {ncs} cells ({ms_.n} unknowns) of the workload, parallel-for over cells "
+              f"(oracle/hines_oracle.c as it stands)")
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot / len(times),
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": mg.CONFIG_NAMES[args.config], "scale": args.scale, "unknowns": m.n, "cells": m.ncells},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle",
-                         "sample": "whole workload per step, parallel-for over cells (oracle/hines_oracle.c as it stands)"},
+        "config": config_block(args.config, args.scale, m),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -165,8 +231,9 @@ def reduce_over_ranks(ms: float, e2e_s_per_step: float, units: float, dist=None,
     return float(t[0]), float(t[1]), float(n[0])
 
 
-def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrier):
-    """One config on this rank's GPU: device-resident timing, per-path device time, optional e2e."""
+def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrier, intervals=N_INTERVALS):
+    """One config on this rank's GPU: exactly `steps` timed steps, then `intervals` intervals of >= 50 ms, the
+    per-path device time, parity of what was timed, optional e2e."""
     import torch
     import paper_1810_12742_b200 as hb
     np_dtype = np.float64 if dtype == "f64" else np.float32
@@ -176,7 +243,7 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32,
                    threads_per_block=args.threads, policy_flags=args.policy, group_smem_bytes=args.group_smem,
                    smem_bytes_per_block=args.smem, max_segment=args.max_segment, chunk_smem_bytes=args.chunk_smem,
-                   cluster_max=args.cluster_max)
+                   cluster_max=args.cluster_max, split_smem_bytes=args.split_smem)
     plan.upload()
     plan_s = time.perf_counter() - t0
     info = plan.info
@@ -197,39 +264,76 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
         a = sets[i % nsets]
         plan.solve(a[0], a[1], a[2], a[3], stream)
 
-    for i in range(warmup):
-        step(i)
+    # Launch-bound configs (a step of a few tens of microseconds: config 4's time loop, config 0) are replayed as a
+    # CUDA graph of one pass over the buffer sets, as SURVEY.md section 8(d) asks ("the 1,000 steps as one graph launch").
+    use_graph = nsets > 1 and not args.no_graph
+    graph = None
+    if use_graph:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            for i in range(nsets):
+                a = sets[i]
+                plan.solve(a[0], a[1], a[2], a[3], side.cuda_stream)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            for i in range(nsets):
+                a = sets[i]
+                plan.solve(a[0], a[1], a[2], a[3], side.cuda_stream)
+
+    def run_steps(k):
+        """k steps on the current stream (graph: whole passes over the buffer sets, k rounded up to one)."""
+        if graph is None:
+            for i in range(k):
+                step(i)
+            return k
+        n = -(-k // nsets)
+        for _ in range(n):
+            graph.replay()
+        return n * nsets
+
+    run_steps(max(warmup, 3))
     torch.cuda.synchronize()
     # ---- timed region: exactly `steps` steps, CUDA events on the launching stream -----------
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier(); torch.cuda.synchronize()
     w0 = time.time()
     e0.record()
-    for i in range(steps):
-        step(i)
+    done = run_steps(steps)
     e1.record()
     torch.cuda.synchronize(); barrier()
+    ms = e0.elapsed_time(e1) * steps / done                   # (graph replays are whole passes: scaled to `steps`)
+    # ---- >= 20 intervals of >= 50 ms each: median and best ------------------------------------
+    per_step = ms / steps
+    inner = max(1, int(np.ceil(INTERVAL_MS / max(per_step, 1e-6))))
+    iv = []
+    for _ in range(intervals):
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        n_ = run_steps(inner)
+        a1.record()
+        a1.synchronize()
+        iv.append(a0.elapsed_time(a1) / n_)
     w1 = time.time()
-    ms = e0.elapsed_time(e1)
     windows = [(w0, w1)]
-    # ---- parity of what was just timed (full batch, against the oracle) -----------------------
+    timing = {"intervals": intervals, "steps_per_interval": inner, "interval_ms": float(np.median(iv)) * inner,
+              "median_ms_per_step": float(np.median(iv)), "best_ms_per_step": float(np.min(iv)),
+              "worst_ms_per_step": float(np.max(iv))} if iv else None
+    # ---- parity of what was just timed (against the oracle, on the cells the oracle is given) ----
     parity = None
     if want_parity:
-        import oracle
-        dr, ur, br = (a.cpu().numpy().astype(np.float64) for a in sets[0][:3])
-        xr = oracle.hines_solve(m.parent, m.cell_offsets, dr, ur, br)
-        parity = float(oracle.rel_err(m.cell_offsets, sets[0][3].cpu().numpy().astype(np.float64), xr).max())
-    # ---- per-path device time (roofline): the library's event hook, events on the same stream ----
+        step(0); torch.cuda.synchronize()
+        parity = sampled_parity(m, d, u, b, sets[0][3].cpu().numpy(), np_dtype)
+    # ---- per-path device time: the library's event hook ----------------------------------------
     plan.enable_timing(True)
     res_ms, str_ms = [], []
-    w2 = time.time()
-    for i in range(min(steps, 50)):
+    for i in range(10):
         step(i)
         r_, s_ = plan.timing()
         res_ms.append(r_); str_ms.append(s_)
-    w3 = time.time()
     plan.enable_timing(False)
-    windows.append((w2, w3))
     res_ms, str_ms = float(np.mean(res_ms)), float(np.mean(str_ms))
     # ---- end to end: pinned host buffers through hines_solve_host -----------------------------
     e2e = None
@@ -245,43 +349,63 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
         e2e_s = (time.perf_counter() - t0) / k_e2e
         barrier()
         e2e = {"s_per_step": e2e_s, "steps": k_e2e, "h2d": 3 * m.n * w, "d2h": m.n * w}
-    launches = plan.launches_per_solve
+        del hd, hu, hb_, hx
     out = {"m": m, "d": d, "u": u, "b": b, "info": info, "ms": ms, "res_ms": res_ms, "str_ms": str_ms,
-           "parity": parity, "e2e": e2e, "plan_s": plan_s, "nsets": nsets, "launches": launches,
-           "windows": windows, "bytes_min": bytes_min, "bytes_literal": info.bytes_literal,
-           "classes": [int(v) for v in plan.table("class_cluster")]}
+           "parity": parity, "e2e": e2e, "plan_s": plan_s, "nsets": nsets, "launches": plan.launches_per_solve,
+           "windows": windows, "bytes_min": bytes_min, "bytes_literal": info.bytes_literal, "timing": timing,
+           "graph": graph is not None,
+           "classes": [int(v) for v in plan.table("class_cluster")], "phases": [int(v) for v in plan.table("class_phase")]}
+    del graph
     plan.close()
     del sets, dd, du
     torch.cuda.empty_cache()
     return out
 
 
-def load_traffic(key):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel per step, from the committed
-    ncu --set full capture (profiles/traffic.csv, see profiles/traffic.md), or None."""
-    try:
-        for line in open(os.path.join(ROOT, "profiles", "traffic.csv")).read().splitlines()[1:]:
-            k, v = line.split(",")
-            if k == key:
-                return int(v)
-    except Exception:
-        pass
-    return None
+def plan_block(r, world):
+    info = r["info"]
+    return {"branches": info.nbranches, "max_levels": info.max_levels,
+            "parallelism": f"independent cells, {world} replica(s), no collective",
+            "l2": "inputs_exceed_l2" if r["nsets"] == 1 else f"rotating {r['nsets']} distinct buffer sets of d,u,b,x (> 2x L2): cold",
+            "cuda_graph": r["graph"], "resident_items": info.n_resident_items, "parts": info.n_parts,
+            "blocks_per_step": info.n_blocks, "cluster_cells": info.n_cluster_cells,
+            "cluster_unknowns": info.n_cluster_unknowns, "split_cells": info.n_split_cells,
+            "split_unknowns": info.n_split_unknowns, "exports": info.n_exports,
+            "cluster_size_per_class": r["classes"], "phase_per_class": r["phases"],
+            "stream_cells": info.n_stream_cells, "stream_unknowns": info.n_stream_unknowns,
+            "launches_per_step": r["launches"],
+            "lane_efficiency": info.useful_lane_steps / max(1, info.padded_lane_steps), "plan_create_s": r["plan_s"]}
+
+
+def roofline_block(r, key, steps):
+    peak, peak_src = peak_hbm()
+    ms_step = r["ms"] / steps
+    achieved = r["bytes_min"] / (ms_step * 1e-3) / 1e9
+    best = r["bytes_min"] / (r["timing"]["median_ms_per_step"] * 1e-3) / 1e9 if r["timing"] else None
+    dominant = "hines_resident_kernel" if r["res_ms"] >= r["str_ms"] else "hines_stream_backward/forward"
+    return {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+            "frac_median_of_intervals": None if best is None else best / peak,
+            "traffic": load_traffic(key), "peak_source": peak_src, "resident_ms": r["res_ms"], "stream_ms": r["str_ms"],
+            "note": "achieved = bytes_min (N*4w + 4*branches, all launches of one step) / average device time of one step over "
+                    "the timed region (CUDA events on the launching stream); one kernel family fills the step; resident_ms / "
+                    "stream_ms = one isolated step per path (library event hook); traffic = measured DRAM bytes of one step from "
+                    "the committed ncu capture of these very sources (profiles/traffic.csv), else null"}
 
 
 # ------------------------------------------------------------------------------------------------
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=10)
-    ap.add_argument("--config", type=int, default=1, help="BASELINE.json configs[] index (default 1)")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json configs[] index (default 3: the largest single-GPU one)")
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
-    ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other configs")
+    ap.add_argument("--no-others", action="store_true", help="skip the runs of the other configs")
+    ap.add_argument("--no-graph", action="store_true", help="launch-bound configs step by step instead of as a CUDA graph")
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--policy", type=int, default=0)
     ap.add_argument("--group-smem", type=int, default=0)
@@ -289,6 +413,7 @@ def main():
     ap.add_argument("--max-segment", type=int, default=0)
     ap.add_argument("--chunk-smem", type=int, default=0)
     ap.add_argument("--cluster-max", type=int, default=0)
+    ap.add_argument("--split-smem", type=int, default=0)
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -313,90 +438,70 @@ def main():
     sampler = ClockSampler(local) if rank == 0 else None
     r = measure(args.config, args.dtype, args.steps, args.warmup, rank, args,
                 want_e2e=not args.no_e2e, want_parity=(rank == 0 and not args.no_cpu), barrier=barrier)
-    clocks = sampler.stop(r["windows"]) if sampler else None
-    m, info = r["m"], r["info"]
+    clocks = sampler.summary(r["windows"]) if sampler else None
+    m = r["m"]
     ms, e2e_s, tot_units = reduce_over_ranks(r["ms"], r["e2e"]["s_per_step"] if r["e2e"] else 0.0, float(m.n),
                                              dist if world > 1 else None, "cuda")
 
-    # the other configs, short runs (parity-test cases, not bench lines): context for the headline
+    # the other configs (parity-test cases, not bench lines): each with its own roofline / parity / clocks block
     others = {}
     if not args.no_others and world == 1 and args.scale == 1.0:
         for cfg, dt in ((0, "f64"), (1, "f64"), (2, "f64"), (2, "f32"), (3, "f64"), (4, "f64")):
             if cfg == args.config and dt == args.dtype:
                 continue
             try:
-                o = measure(cfg, dt, min(args.steps, 20), 3, rank, args, False, False, barrier)
+                k = max(20, min(args.steps, 100))
+                o = measure(cfg, dt, k, 5, rank, args, False, not args.no_cpu, barrier)
                 others[f"cfg{cfg}_{dt}"] = {
-                    "unknowns": o["m"].n, "ms_per_step": o["ms"] / min(args.steps, 20),
-                    "value": o["m"].n * min(args.steps, 20) / (o["ms"] * 1e-3),
-                    "hbm_frac": o["bytes_min"] / (o["ms"] / min(args.steps, 20) * 1e-3) / 1e9 / peak_hbm()[0],
-                    "resident_ms": o["res_ms"], "stream_ms": o["str_ms"], "launches_per_step": o["launches"],
-                    "cluster_sizes": o["classes"], "stream_cells": o["info"].n_stream_cells}
+                    "config": config_block(cfg, args.scale, o["m"]), "dtype": dt, "steps": k,
+                    "ms_per_step": o["ms"] / k, "value": o["m"].n * k / (o["ms"] * 1e-3), "unit": UNIT,
+                    "timing": o["timing"], "roofline": roofline_block(o, f"cfg{cfg}_{dt}", k),
+                    "parity": o["parity"], "clocks": sampler.summary(o["windows"]) if sampler else None,
+                    "bytes_min_per_step": o["bytes_min"], "gpu_launches": o["launches"] * k, "plan": plan_block(o, world)}
                 del o
             except Exception as ex:                       # a context line must never kill the headline
-                others[f"cfg{cfg}_{dt}"] = {"error": str(ex)[:200]}
+                others[f"cfg{cfg}_{dt}"] = {"error": str(ex)[:300]}
+    if sampler:
+        sampler.stop()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
-    w = 8 if args.dtype == "f64" else 4
     ms_step = ms / args.steps
     value = tot_units * args.steps / (ms * 1e-3)
-    peak, peak_src = peak_hbm()
-    res_ms, str_ms = r["res_ms"], r["str_ms"]
-    # The launches of one step are one kernel family (resident: one launch per size class, overlapping on side
-    # streams; or the streaming pair, one launch per level) and fill the step: their average duration over the
-    # timed region is the region divided by its steps.  res_ms / str_ms (one isolated step at a time, through
-    # the library's event hook, so each includes a cold start) say which path dominates.
-    achieved = r["bytes_min"] / (ms_step * 1e-3) / 1e9
-    dominant = "hines_resident_kernel" if res_ms >= str_ms else "hines_stream_backward/forward"
+    roof = roofline_block(r, f"cfg{args.config}_{args.dtype}", args.steps)
 
     cpu = None
     if not args.no_cpu and world == 1:
         cores = os.cpu_count() or 1
-        # bounded sample: whole cells from the start of the batch, at most ~40 M unknowns
-        ncs = int(np.searchsorted(m.cell_offsets, min(m.n, 40_000_000), side="left"))
-        ncs = max(1, min(ncs, m.ncells))
-        ms_ = mg.Morphology(m.parent[:m.cell_offsets[ncs]], m.cell_offsets[:ncs + 1])
-        ns = ms_.n
-        t1, _, _ = cpu_oracle_time(ms_, r["d"][:ns], r["u"][:ns], r["b"][:ns], 1, 2)
-        tn, used, _ = cpu_oracle_time(ms_, r["d"][:ns], r["u"][:ns], r["b"][:ns], cores, 5)
-        cpu = {"value": ns / tn, "unit": UNIT, "cores": used, "kind": "oracle",
-               "sample": f"first {ncs} cells ({ns} unknowns) of the workload, best of 5 after warm-up, parallel-for over cells",
-               "single_thread_value": ns / t1, "cpu_count": cores}
+        ms_, ds, us, bs, ncs = head_sample(m, r["d"], r["u"], r["b"], 40_000_000)      # bounded sample
+        t1, _, _ = cpu_oracle_time(ms_, ds, us, bs, 1, 1)
+        tn, used, _ = cpu_oracle_time(ms_, ds, us, bs, cores, 5)
+        cpu = {"value": ms_.n / tn, "unit": UNIT, "cores": used, "kind": "oracle",
+               "sample": f"first {ncs} cells ({ms_.n} unknowns) of the workload, best of 5 after warm-up, parallel-for over cells",
+               "single_thread_value": ms_.n / t1, "cpu_count": cores}
 
     e2e = r["e2e"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
-        "config": {"workload": mg.CONFIG_NAMES[args.config], "scale": args.scale, "unknowns_per_gpu": m.n,
-                   "cells_per_gpu": m.ncells, "branches_per_gpu": info.nbranches, "max_levels": info.max_levels,
-                   "parallelism": f"independent cells, {world} replica(s), no collective",
-                   "l2": "inputs_exceed_l2" if r["nsets"] == 1 else f"rotating {r['nsets']} distinct buffer sets (> 2x L2)",
-                   "resident_items": info.n_resident_items, "resident_blocks": info.n_blocks,
-                   "resident_unknowns": info.n_resident_unknowns, "cluster_cells": info.n_cluster_cells,
-                   "cluster_unknowns": info.n_cluster_unknowns, "cluster_sizes_per_class": r["classes"],
-                   "stream_cells": info.n_stream_cells, "stream_unknowns": info.n_stream_unknowns,
-                   "size_classes": info.n_classes,
-                   "lane_efficiency": info.useful_lane_steps / max(1, info.padded_lane_steps),
-                   "plan_create_s": r["plan_s"]},
+        "config": config_block(args.config, args.scale, m),
+        "plan": plan_block(r, world),
+        "timing": r["timing"],
         "achieved_hbm_gbs": r["bytes_min"] * world / (ms_step * 1e-3) / 1e9,
-        "hbm_frac_of_peak_per_gpu": r["bytes_min"] / (ms_step * 1e-3) / 1e9 / peak,
+        "hbm_frac_of_peak_per_gpu": roof["frac"],
         "bytes_min_per_step": r["bytes_min"], "bytes_literal_per_step": r["bytes_literal"],
         "gpu_launches": r["launches"] * args.steps,
         "clocks": clocks,
         "e2e": None if e2e is None else {"value": tot_units / e2e_s, "unit": UNIT, "steps": e2e["steps"],
                                          "h2d_bytes_per_step": e2e["h2d"] * world, "d2h_bytes_per_step": e2e["d2h"] * world},
-        "roofline": {"bound": "hbm", "kernel": dominant, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                     "frac": achieved / peak, "traffic": load_traffic(f"cfg{args.config}_{args.dtype}"),
-                     "peak_source": peak_src, "resident_ms": res_ms, "stream_ms": str_ms,
-                     "note": "achieved = bytes_min (N*4w + 4*branches, all launches of one step) / average device time "
-                             "of one step's launches over the timed region (CUDA events on the launching stream); "
-                             "resident_ms / stream_ms = one isolated step per path (library event hook, cold start)"},
+        "roofline": roof,
         "cpu_baseline": cpu,
-        "parity_max_rel_err": r["parity"],
+        "parity": r["parity"],
+        "parity_max_rel_err": None if r["parity"] is None else r["parity"]["max_rel_err"],
+        "kernel_source_hash": kernel_hash(),
         "other_configs": others,
     }
     print(json.dumps(line))
