@@ -147,3 +147,27 @@ def tables(parent, cell_offsets) -> Tables:
     assert rc == 0
     t.level_count = t.level_count[:nlc.value].copy()
     return t
+
+
+def level_mean_split(parent, cell_offsets):
+    """f1, the paper's branch splitting (reading F1): per branch the piece lengths (from the top of
+    the branch) and piece levels, plus the per-level {sum, count} statistics.  Returns (piece_offsets[nbranches+1],
+    piece_len, piece_level, level_stat[2*nlevels]) with pieces grouped by global branch index."""
+    t = tables(parent, cell_offsets)
+    nb = len(t.branch_len)
+    ncomp = int(np.asarray(cell_offsets)[-1])
+    pb = np.empty(ncomp, np.int64); pl = np.empty(ncomp, np.int32); pv = np.empty(ncomp, np.int32)
+    ls = np.empty(ncomp, np.int64); lc = np.empty(ncomp, np.int64)
+    nlev = C.c_int64(0)
+    lib().oracle_level_mean_split.restype = C.c_int64
+    npieces = lib().oracle_level_mean_split(
+        C.c_int64(len(t.cell_branch_offsets) - 1), _p(t.cell_branch_offsets, C.c_int64), _p(t.branch_len, C.c_int32),
+        _p(t.branch_parent_branch, C.c_int32), _p(pb, C.c_int64), _p(pl, C.c_int32), _p(pv, C.c_int32),
+        _p(ls, C.c_int64), _p(lc, C.c_int64), C.byref(nlev))
+    assert npieces >= nb
+    pb, pl, pv = pb[:npieces], pl[:npieces], pv[:npieces]
+    order = np.argsort(pb, kind="stable")                 # by branch; inside a branch the emission order = top-down
+    offs = np.concatenate([[0], np.cumsum(np.bincount(pb, minlength=nb))]).astype(np.int64)
+    stat = np.empty(2 * nlev.value, np.int64)
+    stat[0::2] = ls[:nlev.value]; stat[1::2] = lc[:nlev.value]
+    return offs, pl[order].copy(), pv[order].copy(), stat
