@@ -58,12 +58,35 @@ def peak_hbm():
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def workload(cfg: int, scale: float, rank: int):
-    seed = mg.rng.BASE_SEED + 7919 * rank           # every rank its own cells
+def workload(cfg: int, scale: float, rank: int, world: int = 1, scaling: str = "weak"):
+    """This rank's cells.  weak: every rank generates its own batch of the config's size (seed offset by rank).
+    strong: ONE batch of the config's size, its cells dealt to the ranks by hines_partition_cells (longest processing
+    time first on the cells' unknowns); the rank keeps its cells in input order."""
+    if scaling == "weak" or world == 1:
+        seed = mg.rng.BASE_SEED + 7919 * rank       # every rank its own cells
+        m = mg.make_config(cfg, scale, seed)
+        d, u, _ = mg.coefficients(m, seed)
+        b = mg.rhs(m, seed, 0)
+        return m, d, u, b, seed
+    seed = mg.rng.BASE_SEED
     m = mg.make_config(cfg, scale, seed)
     d, u, _ = mg.coefficients(m, seed)
     b = mg.rhs(m, seed, 0)
-    return m, d, u, b, seed
+    ms, idx = my_share(m, rank, world)
+    return ms, d[idx], u[idx], b[idx], seed
+
+
+def my_share(m, rank: int, world: int):
+    """(sub-morphology, compartment indices) of the cells hines_partition_cells gives to `rank` of `world`."""
+    import paper_1810_12742_b200 as hb
+    part, _ = hb.partition_cells(m.cell_offsets, world)
+    mine = np.nonzero(part == rank)[0]
+    lo, hi = m.cell_offsets[mine], m.cell_offsets[mine + 1]
+    idx = np.concatenate([np.arange(a, b_) for a, b_ in zip(lo, hi)]) if len(mine) else np.zeros(0, np.int64)
+    offs = np.concatenate([[0], np.cumsum(hi - lo)]).astype(np.int64)
+    ms = mg.Morphology(m.parent[idx], offs, name=m.name)
+    ms.meta["cells"] = mine
+    return ms, idx
 
 
 def config_block(cfg: int, scale: float, m):
@@ -238,7 +261,7 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     import paper_1810_12742_b200 as hb
     np_dtype = np.float64 if dtype == "f64" else np.float32
     w = np.dtype(np_dtype).itemsize
-    m, d, u, b, seed = workload(cfg, args.scale, rank)
+    m, d, u, b, seed = workload(cfg, args.scale, rank, args.world, args.scaling)
     t0 = time.perf_counter()
     plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32,
                    threads_per_block=args.threads, policy_flags=args.policy, group_smem_bytes=args.group_smem,
@@ -414,9 +437,12 @@ def main():
     ap.add_argument("--chunk-smem", type=int, default=0)
     ap.add_argument("--cluster-max", type=int, default=0)
     ap.add_argument("--split-smem", type=int, default=0)
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own batch of the config size; strong = one batch, cells dealt to the ranks")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
+    args.world = 1
     if args.impl == "reference":
         return run_reference(args)
 
@@ -424,6 +450,7 @@ def main():
     import torch.distributed as dist
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    args.world = world
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
@@ -485,7 +512,7 @@ def main():
     e2e = r["e2e"]
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None,
         "dtype": args.dtype, "data": "synthetic",
         "config": config_block(args.config, args.scale, m),
         "plan": plan_block(r, world),

@@ -250,6 +250,20 @@ hines_status_t hines_solve_host(hines_plan_t* plan, const void* d, const void* u
 
 hines_status_t hines_plan_destroy(hines_plan_t* plan);
 
+/*
+ * Multi-GPU: cells are independent, so a batch is spread over several devices by
+ * giving every device a subset of the cells -- no exchange step, no collective.  This helper deals the cells to
+ * nparts devices by longest-processing-time first on the per-cell cost (the cell's unknowns: the solve is linear in
+ * them): cells by cost descending (ties by index), each to the device with the least cost so far (ties to
+ * the lowest device).  The caller then builds one plan per device from that device's cells, in input order.
+ *   cell_offsets  HOST int64[ncells+1] as for hines_plan_create
+ *   cell_part     HOST int32[ncells]  out: device of every cell
+ *   part_cost     HOST int64[nparts]  out: unknowns per device (may be NULL)
+ * Errors: INVALID_ARG (null, ncells <= 0, nparts <= 0), BAD_TOPOLOGY (offsets not increasing).
+ */
+hines_status_t hines_partition_cells(const int64_t* cell_offsets, int64_t ncells, int32_t nparts,
+                                     int32_t* cell_part, int64_t* part_cost);
+
 /* Introspection: needed for the bit-exact table parity tests and for reporting. */
 hines_status_t hines_plan_get_info(const hines_plan_t* plan, hines_plan_info_t* out);
 

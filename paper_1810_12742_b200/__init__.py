@@ -48,7 +48,7 @@ TABLES = {
 }
 
 # every symbol include/hines.h declares
-ABI_SYMBOLS = ["hines_plan_create", "hines_plan_upload", "hines_solve", "hines_solve_host",
+ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_plan_upload", "hines_solve", "hines_solve_host",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
                "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
@@ -98,6 +98,7 @@ def load_library(build_if_missing: bool = True):
     vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
     lib.hines_plan_create.argtypes = [vp, vp, i64, i32, C.POINTER(Options), C.POINTER(vp)]
     lib.hines_plan_upload.argtypes = [vp]
+    lib.hines_partition_cells.argtypes = [vp, i64, i32, vp, vp]
     lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_plan_destroy.argtypes = [vp]
@@ -222,6 +223,16 @@ class Plan:
             self.close()
         except Exception:
             pass
+
+
+def partition_cells(cell_offsets, nparts: int):
+    """hines_partition_cells: (cell_part int32[ncells], part_cost int64[nparts]) -- longest-processing-time-first deal of
+    the cells to nparts devices by their unknowns (no exchange step: cells are independent)."""
+    offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
+    part = np.empty(len(offs) - 1, np.int32)
+    cost = np.empty(nparts, np.int64)
+    _check(load_library().hines_partition_cells(offs.ctypes.data, len(offs) - 1, int(nparts), part.ctypes.data, cost.ctypes.data))
+    return part, cost
 
 
 def version() -> str:

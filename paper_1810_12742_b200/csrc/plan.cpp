@@ -1040,6 +1040,36 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     }
 }
 
+hines_status_t hines_partition_cells(const int64_t* cell_offsets, int64_t ncells, int32_t nparts,
+                                     int32_t* cell_part, int64_t* part_cost)
+{
+    if (!cell_offsets || !cell_part) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    if (ncells <= 0 || nparts <= 0) { set_error("ncells and nparts must be positive"); return HINES_ERR_INVALID_ARG; }
+    for (int64_t c = 0; c < ncells; ++c)
+        if (cell_offsets[c + 1] <= cell_offsets[c]) { set_error("cell_offsets not strictly increasing at cell " + std::to_string(c)); return HINES_ERR_BAD_TOPOLOGY; }
+    try {
+        std::vector<int64_t> order(ncells);
+        std::iota(order.begin(), order.end(), 0);
+        auto cost = [&](int64_t c) { return cell_offsets[c + 1] - cell_offsets[c]; };
+        std::stable_sort(order.begin(), order.end(), [&](int64_t a, int64_t b) { return cost(a) > cost(b); });
+        // a heap of (cost so far, device): the lightest device first, ties to the lowest index
+        std::vector<std::pair<int64_t, int32_t>> heap;
+        for (int32_t p = 0; p < nparts; ++p) heap.push_back({0, p});
+        auto cmp = [](const std::pair<int64_t, int32_t>& a, const std::pair<int64_t, int32_t>& b) { return a > b; };
+        std::make_heap(heap.begin(), heap.end(), cmp);
+        for (int64_t c : order) {
+            std::pop_heap(heap.begin(), heap.end(), cmp);
+            cell_part[c] = heap.back().second;
+            heap.back().first += cost(c);
+            std::push_heap(heap.begin(), heap.end(), cmp);
+        }
+        if (part_cost) for (const auto& h : heap) part_cost[h.second] = h.first;
+        return HINES_OK;
+    } catch (const std::exception&) {
+        set_error("host allocation failed"); return HINES_ERR_ALLOC;
+    }
+}
+
 hines_status_t hines_plan_get_info(const hines_plan_t* P, hines_plan_info_t* out)
 {
     if (!P || !out) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
