@@ -171,3 +171,24 @@ def level_mean_split(parent, cell_offsets):
     stat = np.empty(2 * nlev.value, np.int64)
     stat[0::2] = ls[:nlev.value]; stat[1::2] = lc[:nlev.value]
     return offs, pl[order].copy(), pv[order].copy(), stat
+
+
+def hines_factor(parent, cell_offsets, d, u):
+    """f3: the part of Listing 2 that touches only d and u.  Returns (dw, f): pivots and multipliers."""
+    parent, offs, nc = _prep(parent, cell_offsets)
+    d = np.ascontiguousarray(d, np.float64); u = np.ascontiguousarray(u, np.float64)
+    dw = np.empty_like(d); f = np.empty_like(d)
+    lib().oracle_hines_factor(nc, _p(offs, C.c_int64), _p(parent, C.c_int32), _p(d, C.c_double), _p(u, C.c_double),
+                              _p(dw, C.c_double), _p(f, C.c_double))
+    return dw, f
+
+
+def hines_solve_rhs(parent, cell_offsets, dw, f, u, b):
+    """f3: x = A^-1 b from the factors of hines_factor (the part of Listing 2 that touches b)."""
+    parent, offs, nc = _prep(parent, cell_offsets)
+    dw = np.ascontiguousarray(dw, np.float64); f = np.ascontiguousarray(f, np.float64)
+    u = np.ascontiguousarray(u, np.float64); b = np.ascontiguousarray(b, np.float64)
+    x = np.empty_like(b)
+    lib().oracle_hines_solve_rhs(nc, _p(offs, C.c_int64), _p(parent, C.c_int32), _p(dw, C.c_double), _p(f, C.c_double),
+                                 _p(u, C.c_double), _p(b, C.c_double), _p(x, C.c_double))
+    return x

@@ -157,3 +157,51 @@ void oracle_rel_err(int64_t ncells, const int64_t* cell_offsets, const double* x
         err[c] = (nrm > 0.0) ? e / nrm : e;
     }
 }
+
+/* ---- f3: factor once, solve many (with a fixed time step the matrix does not change between steps,
+ * only the right-hand side does).  Listing 2 (reading G1) split in two: the part that touches only
+ * d and u, and the part that touches b.  Same operations in the same order as oracle_hines_cell, so the two
+ * together give bit-identical x (pinned in tests/test_oracle_solve.py). */
+
+/* dw[i] = the pivots d' after the backward sweep, f[i] = u[i] / dw[i] (f[0] unused, set to 0). */
+void oracle_hines_factor_cell(int64_t n, const int32_t* p, const double* d, const double* u,
+                              double* dw, double* f)
+{
+    for (int64_t i = 0; i < n; ++i) dw[i] = d[i];
+    f[0] = 0.0;
+    for (int64_t i = n - 1; i >= 1; --i) {
+        f[i] = u[i] / dw[i];
+        dw[p[i]] = dw[p[i]] - f[i] * u[i];
+    }
+}
+
+/* x = A^-1 b from the factors: backward x[p[i]] -= f[i] x[i]; root x[0] /= dw[0]; forward
+ * x[i] = (x[i] - u[i] x[p[i]]) / dw[i]. */
+void oracle_hines_solve_rhs_cell(int64_t n, const int32_t* p, const double* dw, const double* f,
+                                 const double* u, const double* b, double* x)
+{
+    for (int64_t i = 0; i < n; ++i) x[i] = b[i];
+    for (int64_t i = n - 1; i >= 1; --i) x[p[i]] = x[p[i]] - f[i] * x[i];
+    x[0] = x[0] / dw[0];
+    for (int64_t i = 1; i < n; ++i) x[i] = (x[i] - u[i] * x[p[i]]) / dw[i];
+}
+
+int oracle_hines_factor(int64_t ncells, const int64_t* cell_offsets, const int32_t* parent,
+                        const double* d, const double* u, double* dw, double* f)
+{
+    for (int64_t c = 0; c < ncells; ++c) {
+        int64_t o = cell_offsets[c], n = cell_offsets[c + 1] - o;
+        oracle_hines_factor_cell(n, parent + o, d + o, u + o, dw + o, f + o);
+    }
+    return 0;
+}
+
+int oracle_hines_solve_rhs(int64_t ncells, const int64_t* cell_offsets, const int32_t* parent,
+                           const double* dw, const double* f, const double* u, const double* b, double* x)
+{
+    for (int64_t c = 0; c < ncells; ++c) {
+        int64_t o = cell_offsets[c], n = cell_offsets[c + 1] - o;
+        oracle_hines_solve_rhs_cell(n, parent + o, dw + o, f + o, u + o, b + o, x + o);
+    }
+    return 0;
+}

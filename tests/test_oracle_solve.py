@@ -314,3 +314,27 @@ def test_pivots_equal_schur_complements():
         idx = sorted(desc[i])
         S = np.linalg.inv(A[np.ix_(idx, idx)])
         assert dw[i] == pytest.approx(1.0 / S[idx.index(i), idx.index(i)], rel=1e-13)
+
+
+# ---- f3: factor once / solve many ----------------------------------------------
+def test_factor_then_rhs_is_bit_equal_to_the_full_solve_and_to_dense():
+    ps = [random_parent(n, 50 + n, 0.6) for n in (1, 2, 30, 200, 9)]
+    offs = np.concatenate([[0], np.cumsum([len(p) for p in ps])]).astype(np.int64)
+    m, d, u, b = system_for(np.concatenate(ps), seed=31, cell_offsets=offs)
+    dw, f = oracle.hines_factor(m.parent, offs, d, u)
+    assert np.array_equal(dw, oracle.pivots(m.parent, offs, d, u))
+    for step in range(3):                                    # the same factors, a fresh right-hand side per step
+        bs = mg.rhs(m, step=step)
+        x = oracle.hines_solve_rhs(m.parent, offs, dw, f, u, bs)
+        assert np.array_equal(x, oracle.hines_solve(m.parent, offs, d, u, bs))
+        for c in range(len(ps)):
+            A = dense_from_hines(ps[c], d[offs[c]:offs[c + 1]], u[offs[c]:offs[c + 1]])
+            np.testing.assert_allclose(x[offs[c]:offs[c + 1]], np.linalg.solve(A, bs[offs[c]:offs[c + 1]]), rtol=0, atol=2e-15)
+    # the multipliers: f[i] = A[i,p] / d'[i]; L D L^T with L = I + (f placed at (p[i], i)) reproduces A
+    c = 3
+    p = ps[c]; sl = slice(offs[c], offs[c + 1])
+    n = len(p)
+    Lm = np.eye(n)
+    for i in range(1, n):
+        Lm[p[i], i] = f[sl][i]
+    np.testing.assert_allclose(Lm @ np.diag(dw[sl]) @ Lm.T, dense_from_hines(p, d[sl], u[sl]), rtol=0, atol=1e-13)
