@@ -64,6 +64,9 @@ enum {
                                         or goes to the streaming path                                     */
     HINES_POLICY_NO_PCR       = 256, /* unbranched cables: the reduced chains go through the level sweeps like every other tree,
                                         not through parallel cyclic reduction                                          */
+    HINES_POLICY_FACTORED     = 512, /* f3: the plan also serves hines_factor / hines_solve_rhs (with a fixed time
+                                        step only the right-hand side changes between steps): parts are sized for four
+                                        staged arrays (three factors + b) instead of three, and own N x 3 factor values  */
     HINES_POLICY_NO_SPLIT     = 64,  /* no split items: a cell that fits no cluster goes to the streaming path  */
     HINES_POLICY_SPLIT_LEVEL_MEAN = 128 /* f1: cut branches by the paper's own rule first (level by
                                         level from the root, over all cells of the batch, a branch longer than
@@ -239,6 +242,21 @@ hines_status_t hines_plan_upload(hines_plan_t* plan);
  */
 hines_status_t hines_solve(hines_plan_t* plan, const void* d, const void* u, const void* b, void* x,
                            hines_stream_t stream);
+
+/*
+ * f3, factor once / solve many ("the matrix ... " changes only with the time step; with a fixed step only
+ * the right-hand side changes between steps).  Needs a plan created with HINES_POLICY_FACTORED and no cell on the streaming path.
+ *   hines_factor     everything that depends only on d and u (all reciprocals, the pivot recurrences): three factor
+ *                    values per unknown, kept in plan-owned device memory (3*N*w bytes).  d, u DEVICE, read only.
+ *   hines_solve_rhs  x = A^-1 b from those factors: per unknown one multiply-add on every dependent chain, no division.
+ *                    b, x DEVICE; x may be exactly b.  Bytes moved per call: the factors (3w), b (w) read, x (w) written
+ *                    = 5*N*w (+ one parent per branch), against 4*N*w for hines_solve: the entry trades bytes for the
+ *                    dependent divide chain.
+ * Both only enqueue on `stream`.  Errors: UNSUPPORTED (plan without the flag / streaming cells), INVALID_ARG
+ * (null, misaligned, hines_solve_rhs before hines_factor, overlapping x), CUDA.
+ */
+hines_status_t hines_factor(hines_plan_t* plan, const void* d, const void* u, hines_stream_t stream);
+hines_status_t hines_solve_rhs(hines_plan_t* plan, const void* b, void* x, hines_stream_t stream);
 
 /*
  * Same solve with HOST buffers (pageable or pinned): copies d, u, b to plan-owned device buffers,

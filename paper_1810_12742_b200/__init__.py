@@ -24,6 +24,7 @@ POLICY_POW2_CLUSTERS = 32
 POLICY_NO_SPLIT = 64
 POLICY_SPLIT_LEVEL_MEAN = 128
 POLICY_NO_PCR = 256
+POLICY_FACTORED = 512
 ITEM_SINGLE, ITEM_CLUSTER, ITEM_SPLIT = 0, 1, 2
 
 STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",
@@ -48,7 +49,7 @@ TABLES = {
 }
 
 # every symbol include/hines.h declares
-ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_plan_upload", "hines_solve", "hines_solve_host",
+ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
                "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
@@ -101,6 +102,8 @@ def load_library(build_if_missing: bool = True):
     lib.hines_partition_cells.argtypes = [vp, i64, i32, vp, vp]
     lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hines_factor.argtypes = [vp, vp, vp, vp]
+    lib.hines_solve_rhs.argtypes = [vp, vp, vp, vp]
     lib.hines_plan_destroy.argtypes = [vp]
     lib.hines_plan_get_info.argtypes = [vp, C.POINTER(PlanInfo)]
     lib.hines_plan_get_table.argtypes = [vp, i32, vp, i64, C.POINTER(i64)]
@@ -206,6 +209,20 @@ class Plan:
             import torch
             stream = torch.cuda.current_stream().cuda_stream
         _check(load_library().hines_solve(self._h, _ptr(d), _ptr(u), _ptr(b), _ptr(x), stream))
+        return x
+
+    # hines_factor / hines_solve_rhs (f3; plan created with POLICY_FACTORED)
+    def factor(self, d, u, stream=None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        _check(load_library().hines_factor(self._h, _ptr(d), _ptr(u), stream))
+
+    def solve_rhs(self, b, x, stream=None):
+        if stream is None:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream
+        _check(load_library().hines_solve_rhs(self._h, _ptr(b), _ptr(x), stream))
         return x
 
     # hines_solve_host: host buffers (numpy arrays or pinned torch CPU tensors); synchronous

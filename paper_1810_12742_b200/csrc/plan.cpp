@@ -197,6 +197,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
     const int32_t w = P.width, E = 16 / w;
     const int32_t smax = kind == kItemSingle ? P.seg_single : P.seg_cluster;
     const bool level_mean = (P.opt.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN) != 0;
+    const int32_t narr = (P.opt.policy_flags & HINES_POLICY_FACTORED) ? 4 : 3;     // staged arrays: d,u,b, or the three factors + b
     out = ItemBuild();
     out.kind = kind;
     out.comp_begin = P.cell_offsets[cells.front()];
@@ -249,7 +250,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
     const int64_t per_node = 6 * w + 32 + 8;            // record + two segment lanes + {kids, parent}
     std::vector<int64_t> bytes(nb), sub(nb);
     int64_t total = 0;
-    for (int32_t b = 0; b < nb; ++b) { bytes[b] = 3 * (int64_t)w * br[b].len + per_node * br[b].nseg; total += bytes[b]; }
+    for (int32_t b = 0; b < nb; ++b) { bytes[b] = narr * (int64_t)w * br[b].len + per_node * br[b].nseg; total += bytes[b]; }
     out.total_bytes = total + 1024;
     int32_t nparts = 1;
     if (kind != kItemSingle) {
@@ -268,7 +269,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
         for (int t = 0; t < ntry; ++t) {
             static const int kNum[4] = {1, 1, 1, 2}, kDen[4] = {4, 3, 2, 3};
             const int64_t Tsub = kind == kItemCluster ? std::max<int64_t>(total * kNum[t] / (kDen[t] * (int64_t)K), 2048)
-                                                      : std::max<int64_t>(slot * 4 / 5, 2048);
+                                                      : std::max<int64_t>(slot * (K > 0 ? K : 80) / 100, 2048);   // split items: K = percent of the slot
             frontier.clear();
             int64_t top_bytes = 0;
             for (int32_t b = 0; b < nb; ++b) {
@@ -377,7 +378,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
         // node of each cable) instead of level by level
         bool chains = kind == kItemSingle && next > 0 && mine.size() == cells.size();
         if (chains) for (int32_t b : mine) if (br[b].nseg > 32 || br[b].parent >= 0) chains = false;
-        if (chains && !(P.opt.policy_flags & HINES_POLICY_NO_PCR)) {
+        if (chains && !(P.opt.policy_flags & (HINES_POLICY_NO_PCR | HINES_POLICY_FACTORED))) {
             pb.flags |= kPartFlagChains;
             pb.lb.assign(1, 0);
             int32_t id = 0;
@@ -503,7 +504,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
         for (const SegTmp& sg : segs) if (sg.m >= 0xfff) out.ok = false;
         const int64_t meta = round_up(pb.nlev + 1, 4) + 4 * (int64_t)pb.nnode + 4 * (int64_t)pb.nexp +
                              4 * (int64_t)pb.nghost + 4 * (int64_t)pb.nlanes;
-        pb.smem_need = 16 + 512 + 6 * round_up(pb.nnode + 1, E) * w + 4 * meta + 3 * (int64_t)pb.L * w;
+        pb.smem_need = 16 + 512 + 6 * round_up(pb.nnode + 1, E) * w + 4 * meta + narr * (int64_t)pb.L * w;
         if (kind == kItemSplit && p == 0) { out.smem_top = pb.smem_need; out.max_lanes_top = pb.nlanes; }
         else { out.smem_need = std::max(out.smem_need, pb.smem_need); out.max_lanes = std::max(out.max_lanes, pb.nlanes); }
         for (int32_t b : mine) for (int32_t k = 0; k < br[b].nseg; ++k) lmap[br[b].node0 + k] = -1;
@@ -686,7 +687,7 @@ static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const It
         h.nnode = pb.nnode; h.nlevnode = pb.nlevnode; h.nlev = pb.nlev; h.rounds = pb.rounds;
         h.nexp = pb.nexp; h.nghost = pb.nghost; h.nseg_lanes = pb.nlanes;
         h.xch_base = (int32_t)P.n_xch; h.xs0 = xs0;
-        h.item = item; h.rank = (int32_t)r; h.flags = pb.flags; h.ntoplev = pb.ntoplev; h.lowlev = pb.lowlev; h.maxwidth = pb.maxwidth;
+        h.item = item; h.rank = (int32_t)r; h.flags = pb.flags | ((P.opt.policy_flags & HINES_POLICY_FACTORED) ? kPartFlagFactored : 0); h.ntoplev = pb.ntoplev; h.lowlev = pb.lowlev; h.maxwidth = pb.maxwidth;
         P.part_headers.push_back(h);
         P.n_exports += pb.nexp;
     }
@@ -744,7 +745,7 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
             else fixed_bound_pieces(P.branch_len[j], P.seg_single, tmp);
             nodes += (int64_t)tmp.size();
         }
-        return 3 * (int64_t)w * (P.cell_offsets[c + 1] - P.cell_offsets[c] + 2) + nodes * (6 * w + 32 + 16) + 4 * (P.cell_nlevels[c] + 1);
+        return ((P.opt.policy_flags & HINES_POLICY_FACTORED) ? 4 : 3) * (int64_t)w * (P.cell_offsets[c + 1] - P.cell_offsets[c] + 2) + nodes * (6 * w + 32 + 16) + 4 * (P.cell_nlevels[c] + 1);
     };
     const int64_t group_fixed = 16 + 512 + 2048;    // mbarrier, block record, alignment slack, padding of the lane list to whole warps
     // The open group: small cells in input order ("greedy"); a large cell in between gets an item of its
@@ -823,9 +824,13 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
         }
         if (!placed && !is_single && !no_cluster && !no_split) {
             // beyond the largest cluster: sub-tree parts of at most a split_smem_bytes slot + the top part in one block
-            const int64_t sslot = std::min<int64_t>(P.opt.split_smem_bytes, max_smem);
-            build_item(P, one, kItemSplit, 0, sslot - 6144, cand);
-            if (cand.ok && cand.parts.size() > 1 && cand.smem_need <= sslot && cand.smem_top <= max_smem) { push(one, cand); placed = true; }
+            // (should the top part not fit one block, larger sub-trees leave a smaller top: the slot is raised once)
+            const int64_t sslots[3] = {std::min<int64_t>(P.opt.split_smem_bytes, max_smem), max_smem, max_smem};
+            const int32_t pct[3] = {80, 80, 97};
+            for (int t = 0; t < 3 && !placed; ++t) {
+                build_item(P, one, kItemSplit, pct[t], sslots[t] - 6144, cand);
+                if (cand.ok && cand.parts.size() > 1 && cand.smem_need <= sslots[t] && cand.smem_top <= max_smem) { push(one, cand); placed = true; }
+            }
         }
         if (placed) continue;
         if (!is_single) { is_stream[c] = 1; continue; }
@@ -1004,7 +1009,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~1023) ||
+        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~2047) ||
         o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024 || o.split_smem_bytes < 8192) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }

@@ -59,7 +59,7 @@ struct BlockRecord {         // 512 bytes
 };
 static_assert(sizeof(BlockRecord) == 512, "BlockRecord is read as 32 x int4");
 
-enum { kPartFlagChains = 1 };
+enum { kPartFlagChains = 1, kPartFlagFactored = 2 };     // factored: a fourth staged array follows sb
 enum { kItemSingle = 0, kItemCluster = 1, kItemSplit = 2 };
 // launch phases of a size class: 0 = ordinary (single / cluster items); split items: 1 = sub-tree parts
 // backward + export (A), 2 = top part (B), 3 = sub-tree parts again, import + forward (C)

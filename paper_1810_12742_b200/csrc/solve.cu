@@ -42,6 +42,8 @@ struct DeviceTables {
     int4* runs = nullptr;
     void* xch_h = nullptr;          // split items: exported hand-off values (2 per slot)
     void* xch_x = nullptr;          // split items: the parent's x of every exported sub-tree root
+    void* fac[3] = {nullptr, nullptr, nullptr};   // f3: the factor arrays of hines_factor (N values each)
+    bool factored = false;          // hines_factor has run
     StreamDesc* stream_desc = nullptr;
     int32_t* stream_child = nullptr;
     void* ws_f = nullptr;           // streaming workspace: f (n_stream_unknowns elements)
@@ -206,7 +208,39 @@ __device__ __forceinline__ void named_barrier(int nthreads_in)
     asm volatile("bar.sync 1, %0;" ::"r"(nthreads_in) : "memory");
 }
 
-template <typename T>
+// MODE 0: the whole step; 1 (factor): the pivot part only, the record keeps {g, r}; 2 (right-hand side): r comes from
+// record slot 3, g stays as it is, no reciprocal.
+template <typename T, int MODE>
+__device__ __forceinline__ void node_step(uint32_t nd_sa, uint32_t qa, const int4 k, typename Vec2<T>::type a0, T Un,
+                                          typename Vec2<T>::type a2)
+{
+    typedef typename Vec2<T>::type V2;
+    constexpr uint32_t W = (uint32_t)sizeof(T), RS = 6u * W;
+    const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
+    T D = a0.x - h0.x, B = a0.y - h0.y;
+    D -= h1.x; B -= h1.y;
+    int nc = k.z & 0xfff;
+    if (nc > 2) {                                           // more than two children: the rest, consecutive records
+        uint32_t ca = nd_sa + (uint32_t)k.y + RS;
+        for (nc -= 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
+    }
+    if (MODE == 2) {
+        const T r = lds1<T>(qa + 3u * W);
+        V2 o; o.x = a0.x; o.y = B * r;                      // g = -f is a factor; c = B r
+        sts2<T>(qa, o);
+        V2 s2; s2.x = T(0); s2.y = fnma<T>(a0.x, B, a2.y);
+        sts2<T>(qa + 4u * W, s2);
+    } else {
+        const T r = rcp<T>(D);
+        const T g = Un * r;                                 // -f
+        V2 o; o.x = g; o.y = MODE == 1 ? r : B * r;
+        sts2<T>(qa, o);
+        V2 s2; s2.x = fmad<T>(g, Un, a2.x); s2.y = fnma<T>(g, B, a2.y);
+        sts2<T>(qa + 4u * W, s2);
+    }
+}
+
+template <typename T, int MODE>
 __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int lfrom, int lto,
                                                int topsel, int maxwidth, int tid, int nthreads)
 {
@@ -233,22 +267,7 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
 #pragma unroll 1
             for (int l = lfrom; l >= lto; --l) {
                 const int lo_nn = l > lto + 1 ? ldsi1(lb_sa + 4u * (uint32_t)(l - 2)) : 0;     // two levels ahead: off the chain
-                if (have) {
-                    const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
-                    T D = a0.x - h0.x, B = a0.y - h0.y;
-                    D -= h1.x; B -= h1.y;
-                    int nc = k.z & 0xfff;
-                    if (nc > 2) {                           // more than two children: the rest, consecutive records
-                        uint32_t ca = nd_sa + (uint32_t)k.y + RS;
-                        for (nc -= 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
-                    }
-                    const T r = rcp<T>(D);
-                    const T g = Un * r;                     // -f
-                    V2 o; o.x = g; o.y = B * r;
-                    sts2<T>(qa, o);
-                    V2 s2; s2.x = fmad<T>(g, Un, a2.x); s2.y = fnma<T>(g, B, a2.y);
-                    sts2<T>(qa + 4u * W, s2);
-                }
+                if (have) node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
                 hi = lo; lo = lo_n; lo_n = lo_nn;
                 v = lo + tid;
                 qa = nd_sa + (uint32_t)v * RS;
@@ -273,17 +292,7 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
                 const uint32_t qa = nd_sa + (uint32_t)v * RS;
                 const V2 a0 = lds2<T>(qa), a2 = lds2<T>(qa + 4u * W);
                 const T Un = lds1<T>(qa + 2u * W);
-                const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
-                T D = a0.x - h0.x, B = a0.y - h0.y;
-                D -= h1.x; B -= h1.y;
-                uint32_t ca = nd_sa + (uint32_t)k.y + RS;
-                for (int nc = (k.z & 0xfff) - 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
-                const T r = rcp<T>(D);
-                const T g = Un * r;
-                V2 o; o.x = g; o.y = B * r;
-                sts2<T>(qa, o);
-                V2 s2; s2.x = fmad<T>(g, Un, a2.x); s2.y = fnma<T>(g, B, a2.y);
-                sts2<T>(qa + 4u * W, s2);
+                node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
             }
         }
         __syncthreads();
@@ -423,10 +432,18 @@ __device__ __forceinline__ void solve_cables_pcr(T* nd, const int32_t* cb, int n
 // Eliminating in this order is a symmetric permutation of the same LDL^T factorisation (the matrix is
 // SPD and strictly diagonally dominant, so any order is stable without pivoting).
 // ------------------------------------------------------------------------------------------------
-template <typename T, bool CL>
+// MODE (f3: with a fixed time step only the right-hand side changes):
+//   kModeSolve   the whole solve from d, u, b;
+//   kModeFactor  everything that touches only d and u: per interior g, h and r = 1/D, per separator g = -f, -U and r,
+//                written to the plan's factor arrays f0, f1, f2 (natural order);
+//   kModeRhs     the solve from those factors and b: no reciprocal, one FMA on every dependent chain.
+enum { kModeSolve = 0, kModeFactor = 1, kModeRhs = 2 };
+
+template <typename T, bool CL, int MODE>
 __global__ void __launch_bounds__(384, 2)
 hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __restrict__ meta_g, const int4* __restrict__ runs_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
+                      T* f0, T* f1, T* f2,
                       int64_t n_total, T* xch_h, T* xch_x, int phase, unsigned long long* prof)
 {
     extern __shared__ __align__(128) unsigned char smem[];
@@ -455,11 +472,13 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     T* sd = reinterpret_cast<T*>(meta + H.meta_len);
     T* su = sd + L;
     T* sb = su + L;
+    T* sr = sb + L;                                         // factored plans only (kPartFlagFactored): the fourth array
     const int4* seg = reinterpret_cast<const int4*>(meta + H.seg_off);
+    constexpr int NARR = MODE == kModeSolve ? 3 : (MODE == kModeFactor ? 2 : 4);
     const int nseg_lanes = H.nseg_lanes, nrun = H.nrun;
 
     if (tid == 0) {
-        mbar_expect_tx(bar, 3u * (uint32_t)H.tx_elems * W + (uint32_t)H.meta_len * 4u);
+        mbar_expect_tx(bar, (uint32_t)NARR * (uint32_t)H.tx_elems * W + (uint32_t)H.meta_len * 4u);
         tma_load_1d(meta, meta_g + H.meta_off, (uint32_t)H.meta_len * 4u, bar);
     }
     __syncthreads();                                        // the expected byte count is set before any copy can complete
@@ -477,13 +496,15 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             int64_t ge = (gend + E - 1) / E * E;
             if (ge > gemax) ge = gemax;
             const int sdst = rd.z - (int)(g - ga);
-            if (ge > ga && lane < 3) {
-                const uint32_t bytes = (uint32_t)(ge - ga) * W;
-                const T* src = lane == 0 ? d : (lane == 1 ? b : u);
-                T* dst = lane == 0 ? sd : (lane == 1 ? sb : su);
-                tma_load_1d(dst + sdst, src + ga, bytes, bar);
+            // lanes 0-3: the arrays this mode stages (solve: d, b, u; factor: d, u; right-hand side: f0, b, f1, f2)
+            const T* src = nullptr; T* dst = nullptr;
+            if (MODE == kModeSolve) { src = lane == 0 ? d : (lane == 1 ? b : (lane == 2 ? u : nullptr)); dst = lane == 0 ? sd : (lane == 1 ? sb : su); }
+            if (MODE == kModeFactor) { src = lane == 0 ? d : (lane == 2 ? u : nullptr); dst = lane == 0 ? sd : su; }
+            if (MODE == kModeRhs) { src = lane == 0 ? f0 : (lane == 1 ? b : (lane == 2 ? f1 : (lane == 3 ? f2 : nullptr))); dst = lane == 0 ? sd : (lane == 1 ? sb : (lane == 2 ? su : sr)); }
+            if (src != nullptr) {
+                if (ge > ga) tma_load_1d(dst + sdst, src + ga, (uint32_t)(ge - ga) * W, bar);
+                for (int64_t i = ge > ga ? ge : ga; i < gend; ++i) dst[sdst + (int)(i - ga)] = src[i];    // words beyond the arrays' end
             }
-            if (lane == 3) for (int64_t i = ge > ga ? ge : ga; i < gend; ++i) { const int k = sdst + (int)(i - ga); sd[k] = d[i]; su[k] = u[i]; sb[k] = b[i]; }
         }
     }
     if (tid < 2) nd[6 * H.nnode + 4 + tid] = T(0);          // the all-zero record: hand-off slot of a child that is not there
@@ -497,6 +518,52 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // eliminates a..q-1 top-down with fill-in coupling to t and arrives at q; lane B = A ^ 16 eliminates
     // q+1..b-1 top-down with fill-in coupling to q and arrives at b.  A then takes B's contribution to q,
     // eliminates q (couplings to t and to b) and writes the node record of b.  Both lanes run the same code.
+    if (MODE == kModeRhs) {
+        // The right-hand side alone (f3): the factors g, h, r of every interior sit in sd, su, sr; the chain of a lane is
+        // B' = b[i+1] - g B (one FMA); c = B r replaces b; the contribution sum h B to the top is accumulated.
+        for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
+            const int4 sg = seg[base + lane];
+            const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
+            const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
+            const bool isB = kind == 2;
+            const int m = isB ? mb : (kind == 1 ? mt : 0);
+            const int dl = (sg.y >> 27) & 15;
+            const int mmax = __reduce_max_sync(FULL, m + dl);
+            int i = sg.x;
+            T B = T(0), dbt = T(0);
+            if (kind == 1 || (isB && hasq)) B = sb[i];
+            T g1 = T(0), h1 = T(0), r1 = T(0), b1 = T(0);
+            if (m > 0) { g1 = sd[i]; h1 = su[i]; r1 = sr[i]; b1 = sb[i + 1]; }
+            for (int s = 0; s < mmax; ++s) {
+                const int sl = s - dl;
+                if ((unsigned)sl < (unsigned)m) {
+                    T g2 = T(0), h2 = T(0), r2 = T(0), b2 = T(0);
+                    if (sl + 1 < m) { g2 = sd[i + 1]; h2 = su[i + 1]; r2 = sr[i + 1]; b2 = sb[i + 2]; }
+                    sb[i] = B * r1;
+                    dbt = fmad<T>(h1, B, dbt);
+                    B = fnma<T>(g1, B, b1);
+                    g1 = g2; h1 = h2; r1 = r2; b1 = b2;
+                    ++i;
+                }
+            }
+            const T pB = __shfl_xor_sync(FULL, B, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
+            if (kind == 1) {
+                T* q = nd + 6 * sg.z;
+                int bpos = i;
+                if (hasq) {                                 // i is q now; the separator sits behind B's half
+                    const T Bq = B - pdb;
+                    sb[i] = Bq * sr[i];
+                    dbt = fmad<T>(su[i], Bq, dbt);
+                    q[1] = fnma<T>(sd[i], Bq, pB); q[5] = dbt;
+                    bpos = i + 1 + mb;
+                } else {
+                    q[1] = B; q[5] = T(0);
+                }
+                q[0] = sd[bpos]; q[2] = su[bpos]; q[3] = sr[bpos]; q[4] = T(0);    // the separator's factors: g = -f, -U, r
+            }
+        }
+    } else
+    {
     for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
@@ -507,8 +574,8 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         const int mmax = __reduce_max_sync(FULL, m + dl);
         int i = sg.x;
         T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
-        if (kind == 1 || (isB && hasq)) { D = sd[i]; B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
-        if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; bn = sb[i + 1]; }
+        if (kind == 1 || (isB && hasq)) { D = sd[i]; if (MODE == kModeSolve) B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
+        if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; if (MODE == kModeSolve) bn = sb[i + 1]; }
         {
             // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
             // loop is unrolled by two with the two register sets swapping roles (no register rotation).
@@ -517,10 +584,10 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             T un2 = un, dn2 = dn, bn2 = bn;                 // a lane's first step may fall on either half of the loop body
 #define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2)                                                     \
             if ((unsigned)sl < (unsigned)m) {                                                        \
-                if (sl + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); BN2 = lds1<T>(pb + 2u * W); } \
+                if (sl + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); if (MODE == kModeSolve) BN2 = lds1<T>(pb + 2u * W); } \
                 const T r = rcp<T>(D);                                                               \
                 const T g = UN * r, h = ee * r, c = B * r;                                           \
-                sts1<T>(pa, g); sts1<T>(pu, h); sts1<T>(pb, c);                                      \
+                sts1<T>(pa, g); sts1<T>(pu, h); sts1<T>(pb, MODE == kModeFactor ? r : c);            \
                 ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);                                 \
                 D = fnma<T>(g, UN, DN); B = fnma<T>(g, B, BN); ee = -h * UN;                         \
                 pa += W; pu += W; pb += W;                                                           \
@@ -543,13 +610,14 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
                 const T Dq = D - pdd, Bq = B - pdb;
                 const T r = rcp<T>(Dq);
                 const T gq = pe * r, hq = ee * r;
-                sd[i] = gq; su[i] = hq; sb[i] = Bq * r;
+                sd[i] = gq; su[i] = hq; sb[i] = MODE == kModeFactor ? r : Bq * r;
                 ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
                 q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = hq * pe; q[4] = ddt; q[5] = dbt;     // slot 2 = -U
             } else {                                        // a segment of one compartment: the separator as it is
                 q[0] = D; q[1] = B; q[2] = -ee; q[4] = T(0); q[5] = T(0);
             }
         }
+    }
     }
     __syncthreads();
     HINES_STAMP(2);
@@ -566,7 +634,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         __syncthreads();
     } else {
         // ---- P2 backward: what does not wait for another part, deepest level first ----
-        sweep_backward<T>(nd_sa, lb_sa, kp_sa, H.nlev - 1, H.lowlev, 0, H.maxwidth, tid, nthreads);
+        sweep_backward<T, MODE>(nd_sa, lb_sa, kp_sa, H.nlev - 1, H.lowlev, 0, H.maxwidth, tid, nthreads);
     }
     // ---- hand-off values of the sub-trees held by other blocks, into the ghost children; then
     //      the top nodes (the ancestors of the ghost children) ----
@@ -579,7 +647,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
         __syncthreads();
     }
-    sweep_backward<T>(nd_sa, lb_sa, kp_sa, H.ntoplev - 1, 0, 1, H.maxwidth, tid, nthreads);
+    sweep_backward<T, MODE>(nd_sa, lb_sa, kp_sa, H.ntoplev - 1, 0, 1, H.maxwidth, tid, nthreads);
     HINES_STAMP(3);
     // ---- exchange: exported roots hand their value up and get their parent's x back ----
     if (CL) {
@@ -604,13 +672,13 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             const int4 q = ex[e];
             reinterpret_cast<V2*>(xch_h)[H.xch_base + q.y] = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
         }
-        if (prof && tid == 0) {
+        if (MODE != kModeFactor && prof && tid == 0) {
             unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
             for (int k = 0; k < 4; ++k) o[k] = stamp[k];
             o[4] = o[5] = o[6] = globaltimer_ns();
             o[7] = ((unsigned long long)smid() << 32) | (unsigned)H.n;
         }
-        return;
+        if (MODE != kModeFactor) return;
     } else if (phase == kPhaseC) {
         for (int e = tid; e < nexp; e += nthreads) {
             const int4 q = ex[e];
@@ -624,10 +692,11 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // One round replaces (g_v, c_v, p(v)) by (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds > the
     // longest path to such a node) every g is 0 and c is x.  All nodes work in every round, with one barrier per
     // round instead of one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
-    sweep_forward_top<T>(nd_sa, lb_sa, kp_sa, H.ntoplev, H.maxwidth, tid, nthreads);
+    if (MODE == kModeFactor) rounds = 0;
+    else sweep_forward_top<T>(nd_sa, lb_sa, kp_sa, H.ntoplev, H.maxwidth, tid, nthreads);
     if (CL) {
         if (rank == 0) { cluster_arrive(); cluster_wait(); cluster_arrive(); }   // barrier 2: x of the top nodes is there (slot 1); barrier 3 below
-    } else if (phase == kPhaseB) {
+    } else if (phase == kPhaseB && MODE != kModeFactor) {
         for (int e = tid; e < nghost; e += nthreads) {
             const int4 g = gh[e];
             xch_x[H.xch_base + g.y] = nd[6 * g.z + 1];
@@ -654,6 +723,18 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t]; then A walks up from q-1 to a
     //      (x[i] = c - g x[i+1] - h x[t]) and B walks up from b-1 to q+1 (x[i] = c - g x[i+1] - h x[q]), one FMA
     //      on the dependent chain per step ----
+    if (MODE == kModeFactor) {
+        // the separators' factors go where their compartments are: g = -f, -U, r = 1 / pivot
+        __syncthreads();
+        for (int k = tid; k < nseg_lanes; k += nthreads) {
+            const int4 sg = seg[k];
+            if (((sg.y >> 24) & 3) != 1) continue;
+            const int hasq = (sg.y >> 26) & 1, mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
+            const int bpos = sg.x + (hasq ? mt + 1 + mb : 0);
+            const T* q = nd + 6 * sg.z;
+            sd[bpos] = q[0]; su[bpos] = q[2]; sb[bpos] = q[1];
+        }
+    } else
     for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
@@ -701,9 +782,14 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         const int len = rd.y, so = rd.z;
         const int head = min(len, (int)((E - (g & (E - 1))) & (E - 1)));                 // run-local [0, head)
         const int tail = max(head, (int)(((g + len) & ~(int64_t)(E - 1)) - g));          // run-local [tail, len)
-        if (lane == 0 && tail > head) tma_store_1d(x + g + head, sb + so + head, (uint32_t)(tail - head) * W);
-        if (lane >= 1 && lane - 1 < head) x[g + lane - 1] = sb[so + lane - 1];
-        if (lane >= 8 && tail + lane - 8 < len) x[g + tail + lane - 8] = sb[so + tail + lane - 8];
+#pragma unroll
+        for (int a = 0; a < (MODE == kModeFactor ? 3 : 1); ++a) {                        // x, or the three factor arrays
+            T* dstg = MODE == kModeFactor ? (a == 0 ? f0 : (a == 1 ? f1 : f2)) : x;
+            const T* srcs = MODE == kModeFactor ? (a == 0 ? sd : (a == 1 ? su : sb)) : sb;
+            if (lane == 0 && tail > head) tma_store_1d(dstg + g + head, srcs + so + head, (uint32_t)(tail - head) * W);
+            if (lane >= 1 && lane - 1 < head) dstg[g + lane - 1] = srcs[so + lane - 1];
+            if (lane >= 8 && tail + lane - 8 < len) dstg[g + tail + lane - 8] = srcs[so + tail + lane - 8];
+        }
     }
     tma_store_commit_wait();
     if (prof && tid == 0) {
@@ -783,7 +869,7 @@ static hines_status_t upload_vec(const V& v, void** dst, int64_t& total)
 static void free_device(DeviceTables* D)
 {
     if (!D) return;
-    cudaFree(D->recs); cudaFree(D->meta); cudaFree(D->runs); cudaFree(D->xch_h); cudaFree(D->xch_x);
+    cudaFree(D->recs); cudaFree(D->meta); cudaFree(D->runs); cudaFree(D->xch_h); cudaFree(D->xch_x); for (void* f : D->fac) cudaFree(f);
     cudaFree(D->stream_desc); cudaFree(D->stream_child); cudaFree(D->ws_f); cudaFree(D->ws_c); cudaFree(D->prof);
     for (void* p : D->host_stage) cudaFree(p);
     for (cudaEvent_t e : D->ev) if (e) cudaEventDestroy(e);
@@ -802,9 +888,12 @@ static void free_device(DeviceTables* D)
 template <typename T>
 static hines_status_t prepare_kernels(int max_optin)
 {
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+#define HINES_PREP(MODE)                                                                                                          \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, false, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin)); \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));  \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    HINES_PREP(kModeSolve) HINES_PREP(kModeFactor) HINES_PREP(kModeRhs)
+#undef HINES_PREP
     return HINES_OK;
 }
 
@@ -822,7 +911,7 @@ static hines_status_t check_clusters(const hines_plan* P)
         attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
         int nclusters = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, hines_resident_kernel<T, true>, &cfg));
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, hines_resident_kernel<T, true, kModeSolve>, &cfg));
         if (nclusters < 1) {
             set_error("this device cannot co-schedule a cluster of " + std::to_string(cl) + " blocks with " +
                       std::to_string(P->class_smem_bytes[q]) + " bytes of shared memory each: create the plan with a smaller cluster_max");
@@ -910,9 +999,10 @@ static hines_status_t upload(hines_plan* P)
 }
 
 template <typename T>
-static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T* b, T* x, cudaStream_t stream)
+static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T* b, T* x, cudaStream_t stream, int mode = kModeSolve)
 {
     DeviceTables* D = P->dev;
+    T* f0 = static_cast<T*>(D->fac[0]); T* f1 = static_cast<T*>(D->fac[1]); T* f2 = static_cast<T*>(D->fac[2]);
     auto launch_streaming = [&](cudaStream_t ss) -> hines_status_t {
         const int nlev = (int)P->stream_level_begin.size() - 1;
         const int st = P->opt.stream_threads;
@@ -938,9 +1028,17 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         unsigned long long* prof = D->prof_on ? D->prof + 8 * first : nullptr;
         const BlockRecord* recs = D->recs + first;
         T* xh = static_cast<T*>(D->xch_h); T* xx = static_cast<T*>(D->xch_x);
+        const int phase = (int)P->class_phase[q];
+        if (mode == kModeFactor && phase == kPhaseC) return HINES_OK;       // the factors of a sub-tree part are complete after phase A
         if (cl == 1) {
-            hines_resident_kernel<T, false><<<(unsigned)cnt, P->class_threads[q], P->class_smem_bytes[q], ls>>>(
-                recs, D->meta, D->runs, d, u, b, x, P->n, xh, xx, (int)P->class_phase[q], prof);
+            const unsigned grid = (unsigned)cnt, thr = (unsigned)P->class_threads[q];
+            const size_t sm = (size_t)P->class_smem_bytes[q];
+            if (mode == kModeSolve)
+                hines_resident_kernel<T, false, kModeSolve><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
+            else if (mode == kModeFactor)
+                hines_resident_kernel<T, false, kModeFactor><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
+            else
+                hines_resident_kernel<T, false, kModeRhs><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
         } else {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3((unsigned)cnt);
@@ -951,8 +1049,13 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
             attr[0].id = cudaLaunchAttributeClusterDimension;
             attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
             cfg.attrs = attr; cfg.numAttrs = 1;
-            CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true>, recs, (const int32_t*)D->meta, (const int4*)D->runs,
-                                        d, u, b, x, (int64_t)P->n, xh, xx, 0, prof));
+            const int32_t* mg_ = D->meta; const int4* rg_ = D->runs; const int64_t n_ = P->n;
+            if (mode == kModeSolve)
+                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeSolve>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
+            else if (mode == kModeFactor)
+                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeFactor>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
+            else
+                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeRhs>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
         }
         return HINES_OK;
     };
@@ -1040,6 +1143,35 @@ hines_status_t hines_solve(hines_plan_t* P, const void* d, const void* u, const 
     if (P->dtype == HINES_F64)
         return launch_all<double>(P, (const double*)d, (const double*)u, (const double*)b, (double*)x, (cudaStream_t)stream);
     return launch_all<float>(P, (const float*)d, (const float*)u, (const float*)b, (float*)x, (cudaStream_t)stream);
+}
+
+// f3: everything that depends only on d and u, once; then only the right-hand side per step.
+hines_status_t hines_factor(hines_plan_t* P, const void* d, const void* u, hines_stream_t stream)
+{
+    if (!P || !d || !u) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    if (!(P->opt.policy_flags & HINES_POLICY_FACTORED)) { set_error("hines_factor needs a plan created with HINES_POLICY_FACTORED"); return HINES_ERR_UNSUPPORTED; }
+    if (P->n_stream_cells) { set_error("hines_factor: cells on the streaming path are not supported"); return HINES_ERR_UNSUPPORTED; }
+    if (((uintptr_t)d | (uintptr_t)u) & 15) { set_error("device pointers must be 16-byte aligned"); return HINES_ERR_INVALID_ARG; }
+    hines_status_t st = upload(P);
+    if (st != HINES_OK) return st;
+    DeviceTables* D = P->dev;
+    const size_t bytes = ((size_t)P->n * P->width + 15) / 16 * 16;
+    for (void*& f : D->fac) if (!f) { CUDA_TRY(cudaMalloc(&f, bytes)); D->bytes += (int64_t)bytes; }
+    if (P->dtype == HINES_F64) st = launch_all<double>(P, (const double*)d, (const double*)u, nullptr, nullptr, (cudaStream_t)stream, kModeFactor);
+    else st = launch_all<float>(P, (const float*)d, (const float*)u, nullptr, nullptr, (cudaStream_t)stream, kModeFactor);
+    if (st == HINES_OK) D->factored = true;
+    return st;
+}
+
+hines_status_t hines_solve_rhs(hines_plan_t* P, const void* b, void* x, hines_stream_t stream)
+{
+    if (!P || !b || !x) { set_error("null pointer argument"); return HINES_ERR_INVALID_ARG; }
+    if (!P->dev || !P->dev->factored) { set_error("hines_solve_rhs: call hines_factor first"); return HINES_ERR_INVALID_ARG; }
+    if (((uintptr_t)b | (uintptr_t)x) & 15) { set_error("device pointers must be 16-byte aligned"); return HINES_ERR_INVALID_ARG; }
+    const size_t bytes = (size_t)P->n * P->width;
+    if (x != b && overlaps(x, b, bytes)) { set_error("x may be exactly b (in place) or must not overlap it"); return HINES_ERR_INVALID_ARG; }
+    if (P->dtype == HINES_F64) return launch_all<double>(P, nullptr, nullptr, (const double*)b, (double*)x, (cudaStream_t)stream, kModeRhs);
+    return launch_all<float>(P, nullptr, nullptr, (const float*)b, (float*)x, (cudaStream_t)stream, kModeRhs);
 }
 
 hines_status_t hines_solve_host(hines_plan_t* P, const void* d, const void* u, const void* b, void* x, hines_stream_t stream)

@@ -34,6 +34,7 @@ class Part:
         self.nc = np.where(self.ghost, 0, info & 0xfff)
         self.pnode = kp4[:, 3]
         self.chains = bool(h["flags"] & 1)
+        self.factored = bool(h["flags"] & 2)
         self.exps = meta[h["exp_off"]:h["exp_off"] + 4 * h["nexp"]].reshape(-1, 4)
         self.ghosts = meta[h["gh_off"]:h["gh_off"] + 4 * h["nghost"]].reshape(-1, 4)
         self.seg = meta[h["seg_off"]:h["seg_off"] + 4 * h["nseg_lanes"]].reshape(-1, 4)

@@ -241,3 +241,86 @@ def test_config4_fresh_rhs_steps():
         assert np.isfinite(xg).all()
         assert oracle.rel_err(m.cell_offsets, xg, xr).max() < 1e-10
     plan.close()
+
+
+# ---- f3: factor once / solve many ----------------------------------------------
+def _check_factored(m, d, u, dtype=np.float64, steps=(0, 1, 7), **kw):
+    """hines_factor once, hines_solve_rhs per step with a fresh b, against the oracle's two-function split of
+    Listing 2 (oracle.hines_factor / hines_solve_rhs) on the inputs as the GPU sees them."""
+    import torch
+    import paper_1810_12742_b200 as hb
+    flags = kw.pop("policy_flags", 0) | hb.POLICY_FACTORED
+    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == np.float64 else hb.F32, policy_flags=flags, **kw)
+    dd, du = (torch.from_numpy(np.ascontiguousarray(a, dtype)).cuda() for a in (d, u))
+    dr, ur = (np.ascontiguousarray(a, dtype).astype(np.float64) for a in (d, u))
+    dw, f = oracle.hines_factor(m.parent, m.cell_offsets, dr, ur)
+    plan.factor(dd, du)
+    dd.fill_(float("nan")); du.fill_(float("nan"))             # the factors are the plan's: d, u are not read again
+    worst = 0.0
+    for step in steps:
+        b = mg.rhs(m, step=step)
+        db = torch.from_numpy(np.ascontiguousarray(b, dtype)).cuda()
+        x = torch.full_like(db, float("nan"))
+        plan.solve_rhs(db, x)
+        torch.cuda.synchronize()
+        xg = x.cpu().numpy().astype(np.float64)
+        br = np.ascontiguousarray(b, dtype).astype(np.float64)
+        xr = oracle.hines_solve_rhs(m.parent, m.cell_offsets, dw, f, ur, br)
+        assert np.isfinite(xg).all()
+        err = oracle.rel_err(m.cell_offsets, xg, xr).max()
+        assert err <= TOL[dtype], (step, err)
+        worst = max(worst, err)
+        plan.solve_rhs(db, db)                                  # in place
+        torch.cuda.synchronize()
+        assert torch.equal(db, x)
+    info = plan.info
+    plan.close()
+    return worst, info
+
+
+@pytest.mark.parametrize("cfg,scale", SMALL)
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_factored_small_configs(cfg, scale, dtype):
+    m = mg.make_config(cfg, scale)
+    d, u, _ = mg.system(m)
+    _check_factored(m, d, u, dtype)
+
+
+@pytest.mark.parametrize("kw", [dict(chunk_smem_bytes=40 * 1024), dict(chunk_smem_bytes=24 * 1024, cluster_max=16, max_segment=9),
+                                dict(smem_bytes_per_block=80000, cluster_max=2, split_smem_bytes=26000),
+                                dict(policy_flags=2), dict(policy_flags=128)])
+def test_factored_clusters_split_items_policies(kw):
+    m = mg.make_config(2, 0.006)
+    d, u, _ = mg.system(m)
+    _check_factored(m, d, u, **kw)
+    me = _edge_morphology()
+    d, u, _ = mg.system(me, seed=11)
+    _check_factored(me, d, u, **{k: v for k, v in kw.items() if k == "policy_flags"})
+
+
+def test_factored_needs_the_flag_and_the_factor_call():
+    import torch
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(0)
+    d, u, b = (torch.from_numpy(a).cuda() for a in mg.system(m))
+    plan = hb.Plan(m.parent, m.cell_offsets)
+    with pytest.raises(hb.HinesError) as e:
+        plan.factor(d, u)
+    assert e.value.status == 5
+    plan = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_FACTORED)
+    with pytest.raises(hb.HinesError) as e:
+        plan.solve_rhs(b, torch.empty_like(b))
+    assert e.value.status == 1
+    x = torch.empty_like(b)                                     # a factored plan still serves the full solve
+    plan.solve(d, u, b, x)
+    torch.cuda.synchronize()
+    xr = oracle.hines_solve(m.parent, m.cell_offsets, *mg.system(m))
+    assert oracle.rel_err(m.cell_offsets, x.cpu().numpy(), xr).max() < 1e-10
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4])
+def test_factored_full_size(cfg):
+    m = mg.make_config(cfg, 1.0)
+    d, u, _ = mg.system(m)
+    err, info = _check_factored(m, d, u, steps=(0, 999) if cfg == 4 else (1,))
+    print(f"cfg{cfg} factored: n={m.n} max rel err {err:.3e} split_cells={info.n_split_cells} cluster_cells={info.n_cluster_cells}")

@@ -137,7 +137,7 @@ def _check_policy(m, plan, max_segment=0):
         for k, pid in enumerate(ids):
             h = parts[pid].h
             launched.setdefault(int(pid), []).append(int(cls_phase[q]))
-            need = 16 + 512 + 6 * w * (-(-(h["nnode"] + 1) // E) * E) + 4 * h["meta_len"] + 3 * w * h["L"]
+            need = 16 + 512 + 6 * w * (-(-(h["nnode"] + 1) // E) * E) + 4 * h["meta_len"] + (4 if parts[pid].factored else 3) * w * h["L"]
             assert need <= cls_smem[q] <= 232448
             assert h["maxwidth"] <= cls_threads[q] or True
             if cls_cluster[q] > 1:
