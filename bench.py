@@ -385,6 +385,79 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     return out
 
 
+def measure_factored(cfg, dtype, steps, rank, args, want_parity):
+    """f3: hines_factor once, then `steps` hines_solve_rhs calls with a fresh b per step, device-resident.
+    Roofline numerator of this entry: the factors (3w) + b (w) read, x (w) written = 5*N*w + 4*branches."""
+    import torch
+    import paper_1810_12742_b200 as hb
+    np_dtype = np.float64 if dtype == "f64" else np.float32
+    w = np.dtype(np_dtype).itemsize
+    m, d, u, b, seed = workload(cfg, args.scale, rank, args.world, args.scaling)
+    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32, policy_flags=args.policy | hb.POLICY_FACTORED)
+    info = plan.info
+    if info.n_stream_cells:
+        plan.close()
+        return {"error": "cells on the streaming path"}
+    dd, du = (torch.from_numpy(a.astype(np_dtype)).cuda() for a in (d, u))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.factor(dd, du); torch.cuda.synchronize()
+    e0.record(); plan.factor(dd, du); e1.record(); torch.cuda.synchronize()
+    factor_ms = e0.elapsed_time(e1)
+    del dd, du
+    bytes_rhs = 5 * m.n * w + 4 * info.nbranches
+    nsets = 1 if bytes_rhs > L2_BYTES else min(64, int(np.ceil(2 * L2_BYTES / max(2 * m.n * w, 1))) + 1)
+    sets = [(torch.from_numpy((b if s == 0 else mg.rhs(m, seed, s)).astype(np_dtype)).cuda(),
+             torch.empty(m.n, dtype=torch.float64 if dtype == "f64" else torch.float32, device="cuda")) for s in range(nsets)]
+    stream = torch.cuda.current_stream().cuda_stream
+    graph = None
+    if nsets > 1 and not args.no_graph:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            for bb, xx in sets:
+                plan.solve_rhs(bb, xx, side.cuda_stream)
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            for bb, xx in sets:
+                plan.solve_rhs(bb, xx, side.cuda_stream)
+
+    def run_steps(k):
+        if graph is None:
+            for i in range(k):
+                plan.solve_rhs(sets[i % nsets][0], sets[i % nsets][1], stream)
+            return k
+        n = -(-k // nsets)
+        for _ in range(n):
+            graph.replay()
+        return n * nsets
+
+    run_steps(5); torch.cuda.synchronize()
+    e0.record(); done = run_steps(steps); e1.record(); torch.cuda.synchronize()
+    ms_step = e0.elapsed_time(e1) / done
+    inner = max(1, int(np.ceil(INTERVAL_MS / max(ms_step, 1e-6))))
+    iv = []
+    for _ in range(N_INTERVALS):
+        e0.record(); n_ = run_steps(inner); e1.record(); e1.synchronize()
+        iv.append(e0.elapsed_time(e1) / n_)
+    parity = None
+    if want_parity:
+        plan.solve_rhs(sets[0][0], sets[0][1], stream); torch.cuda.synchronize()
+        parity = sampled_parity(m, d, u, b, sets[0][1].cpu().numpy(), np_dtype)["max_rel_err"]
+    peak, _ = peak_hbm()
+    out = {"entry": "hines_factor once + hines_solve_rhs per step (fresh b per step)", "ms_per_step": ms_step,
+           "median_ms_per_step": float(np.median(iv)), "best_ms_per_step": float(np.min(iv)),
+           "value": m.n / (ms_step * 1e-3), "unit": UNIT, "factor_ms": factor_ms, "cuda_graph": graph is not None,
+           "bytes_per_step": bytes_rhs, "achieved_gbs": bytes_rhs / (ms_step * 1e-3) / 1e9,
+           "frac_of_peak": bytes_rhs / (ms_step * 1e-3) / 1e9 / peak, "launches_per_step": plan.launches_per_solve,
+           "parity_max_rel_err": parity}
+    del graph, sets
+    plan.close()
+    torch.cuda.empty_cache()
+    return out
+
+
 def plan_block(r, world):
     info = r["info"]
     return {"branches": info.nbranches, "max_levels": info.max_levels,
@@ -428,6 +501,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the runs of the other configs")
+    ap.add_argument("--no-factored", action="store_true", help="skip the hines_factor / hines_solve_rhs entry (f3)")
     ap.add_argument("--no-graph", action="store_true", help="launch-bound configs step by step instead of as a CUDA graph")
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--policy", type=int, default=0)
@@ -486,8 +560,16 @@ def main():
                     "parity": o["parity"], "clocks": sampler.summary(o["windows"]) if sampler else None,
                     "bytes_min_per_step": o["bytes_min"], "gpu_launches": o["launches"] * k, "plan": plan_block(o, world)}
                 del o
+                if cfg in (3, 4) and not args.no_factored:
+                    others[f"cfg{cfg}_{dt}"]["factored"] = measure_factored(cfg, dt, k, rank, args, not args.no_cpu)
             except Exception as ex:                       # a context line must never kill the headline
                 others[f"cfg{cfg}_{dt}"] = {"error": str(ex)[:300]}
+    factored = None
+    if not args.no_factored and world == 1:
+        try:
+            factored = measure_factored(args.config, args.dtype, args.steps, rank, args, not args.no_cpu)
+        except Exception as ex:
+            factored = {"error": str(ex)[:300]}
     if sampler:
         sampler.stop()
     if rank != 0:
@@ -526,6 +608,7 @@ def main():
                                          "h2d_bytes_per_step": e2e["h2d"] * world, "d2h_bytes_per_step": e2e["d2h"] * world},
         "roofline": roof,
         "cpu_baseline": cpu,
+        "factored": factored,
         "parity": r["parity"],
         "parity_max_rel_err": None if r["parity"] is None else r["parity"]["max_rel_err"],
         "kernel_source_hash": kernel_hash(),
