@@ -332,7 +332,7 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     per_step = ms / steps
     inner = max(1, int(np.ceil(INTERVAL_MS / max(per_step, 1e-6))))
     iv = []
-    for _ in range(intervals):
+    for _ in range(0 if args.no_intervals else intervals):
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record()
         n_ = run_steps(inner)
@@ -352,7 +352,7 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     # ---- per-path device time: the library's event hook ----------------------------------------
     plan.enable_timing(True)
     res_ms, str_ms = [], []
-    for i in range(10):
+    for i in range(1 if args.no_intervals else 10):
         step(i)
         r_, s_ = plan.timing()
         res_ms.append(r_); str_ms.append(s_)
@@ -502,6 +502,7 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the runs of the other configs")
     ap.add_argument("--no-factored", action="store_true", help="skip the hines_factor / hines_solve_rhs entry (f3)")
+    ap.add_argument("--no-intervals", action="store_true", help="only the K timed steps (for runs under ncu)")
     ap.add_argument("--no-graph", action="store_true", help="launch-bound configs step by step instead of as a CUDA graph")
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--policy", type=int, default=0)

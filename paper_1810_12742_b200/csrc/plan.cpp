@@ -48,8 +48,11 @@ void set_error(const std::string& msg) { g_last_error = msg; }
 
 static const int64_t kSmemPerSM = 233472;       // 228 KiB
 static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
-static const int kClassK[] = {1, 2, 3, 4, 6, 8};
-static const int kNumClassK = 6;
+// size classes: shares of an SM's shared memory a block may take (num/den): the whole SM, 3/4 and 2/3 (such a block
+// shares its SM with a block of another, smaller class launched beside it), then 2, 3, 4, 6, 8 blocks per SM
+static const int kSlotNum[] = {1, 3, 2, 1, 1, 1, 1, 1};
+static const int kSlotDen[] = {1, 4, 3, 2, 3, 4, 6, 8};
+static const int kNumClassK = 8;
 static const int kRegsPerThread = 80;           // the resident kernel is built for __launch_bounds__(384, 2): up to 85
 static const int kMaxThreads = 384;
 static const int kMaxClusterClass = 16;
@@ -57,9 +60,9 @@ static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descr
 
 static inline int64_t round_up(int64_t v, int64_t m) { return (v + m - 1) / m * m; }
 
-static int64_t class_cap(int k, int64_t max_smem)
+static int64_t class_cap(int t, int64_t max_smem)
 {
-    int64_t cap = (kSmemPerSM / k - 1024) / 128 * 128;
+    int64_t cap = (kSmemPerSM * kSlotNum[t] / kSlotDen[t] - 1024) / 128 * 128;
     return std::min(cap, max_smem);
 }
 
@@ -791,8 +794,8 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
             const int64_t total = est + 1024;
             struct Opt { double score; int32_t k; int64_t slot; };
             std::vector<Opt> opts;
-            for (int t = 1; t <= 3; ++t) {                                // slots of 1/2, 1/3, 1/4 of an SM
-                const int64_t slot = class_cap(kClassK[t], max_smem);
+            for (int t = 3; t <= 5; ++t) {                                // slots of 1/2, 1/3, 1/4 of an SM
+                const int64_t slot = class_cap(t, max_smem);
                 if (slot > chunk_cap) continue;
                 int32_t k = (int32_t)std::max<int64_t>(2, (total + slot - 4096 - 1) / (slot - 4096));
                 if (pow2_only) while (k & (k - 1)) ++k;
@@ -848,7 +851,7 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
     const int64_t max_smem = P.opt.smem_bytes_per_block;
     // queue index: [0, 6) single blocks; 6*k + t cluster of k; then split: sub-tree parts, top parts
     const int qSplitSub = kNumClassK * (kMaxClusterClass + 1), qSplitTop = qSplitSub + kNumClassK, nq = qSplitTop + kNumClassK;
-    auto slot_of = [&](int64_t smem) { int q = 0; for (int t = 0; t < kNumClassK; ++t) if (smem <= class_cap(kClassK[t], max_smem)) q = t; return q; };
+    auto slot_of = [&](int64_t smem) { int q = 0; for (int t = 0; t < kNumClassK; ++t) if (smem <= class_cap(t, max_smem)) q = t; return q; };
     std::vector<int> item_q(nitems, 0);
     std::vector<int64_t> need_max(nq, 0), count(nq, 0);
     std::vector<int32_t> lanes_max(nq, 0);
