@@ -67,6 +67,8 @@ enum {
     HINES_POLICY_FACTORED     = 512, /* f3: the plan also serves hines_factor / hines_solve_rhs (with a fixed time
                                         step only the right-hand side changes between steps): parts are sized for four
                                         staged arrays (three factors + b) instead of three, and own N x 3 factor values  */
+    HINES_POLICY_NO_QUADS     = 1024, /* every segment gets two lanes (default: four lanes for segments with >= 24 interior
+                                        compartments: half the dependent steps in P1 / P3)                         */
     HINES_POLICY_NO_SPLIT     = 64,  /* no split items: a cell that fits no cluster goes to the streaming path  */
     HINES_POLICY_SPLIT_LEVEL_MEAN = 128 /* f1: cut branches by the paper's own rule first (level by
                                         level from the root, over all cells of the batch, a branch longer than
@@ -184,8 +186,11 @@ typedef enum {
                                                exps[4*nexp] per exported root {node, ghost child in part 0 (cluster) or exchange slot
                                                             (split), parent node in part 0, ghost parent};
                                                ghosts[4*nghost] {ghost child, exchange slot, its parent node, 0};
-                                               seg[4*nseg_lanes] two lanes per segment, in groups of 32: lanes 0-15 the A halves, lanes
-                                                            16-31 their B partners (lane ^ 16).  A: {a = staged index of the first
+                                               seg[4*nseg_lanes] groups of 32 lanes.  Four-lane groups (kind 3; long segments): lane k + 8 j is
+                                                            quarter j of segment k: {staged index of its first compartment, steps | j<<12 |
+                                                            3<<24 | 1<<26, node, node of the separator above (j = 0 only)}; the middle nodes
+                                                            q1, q2, q3 sit right above quarters 1, 2, 3.  Two-lane groups: lanes 0-15 the A
+                                                            halves, lanes 16-31 their B partners (lane ^ 16).  A: {a = staged index of the first
                                                             compartment, word, node, node of the separator above (-1 = none)}; B: {a+mt+1,
                                                             word, node, -1}; word = mt | mb<<12 | kind<<24 | hasq<<26 | delay<<27 (kind 0
                                                             padding, 1 A, 2 B; mt/mb = compartments A / B eliminate, both top-down; the

@@ -175,6 +175,7 @@ struct ItemBuild {
     int64_t smem_top = 0;                    // split items: the top part
     int64_t total_bytes = 0;                 // estimate of the shared memory of the whole item, all parts together
     int32_t max_lanes = 0, max_lanes_top = 0;
+    int32_t has_quads = 0;                   // some part has four-lane segment groups
 };
 
 // Pieces of a branch under the fixed-bound rule (P4), top-down: nseg = max(1, floor(len/S + 0.4)) pieces of
@@ -481,11 +482,77 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
         // two lanes per segment: lane A eliminates the interior above the middle node q, lane B the interior
         // below it, both top-down (fill-in to t resp. q); A eliminates q last.  A warp holds 16 segments:
         // A lanes 0..15, their B partners 16..31 (partner = lane ^ 16).
+        // Long segments (interior >= quad_min) get FOUR lanes instead: the interior is cut at three middle nodes
+        // q1 < q2 < q3 into quarters, lane j (= lane of the segment + 8 j) eliminates quarter j top-down with fill-in
+        // to its top (t, q1, q2, q3); the first lane then eliminates q1, q2, q3 in turn.  Half the dependent steps
+        // of the two-lane scheme for three more; a warp holds 8 such segments.
+        std::vector<SegTmp> quads;
+        if (P.quad_min > 0) {
+            // ... but only where warps are to spare: four lanes double the warps a segment keeps busy, and the lone
+            // warps of the level sweeps of the blocks beside it starve when the SM's schedulers fill up.  Estimate:
+            // (blocks of this size per SM) x (warps of P1 with four lanes) <= quad_max_warps.
+            size_t nlong = 0;
+            for (const SegTmp& sg : segs) nlong += sg.m >= P.quad_min;
+            const int64_t part_bytes = 16 + 512 + (int64_t)narr * w * pb.L + (int64_t)segs.size() * per_node;
+            const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (part_bytes + 2048));
+            const int64_t warps4 = (int64_t)((nlong + 7) / 8 + (segs.size() - nlong + 15) / 16);
+            if (per_sm * warps4 > P.quad_max_warps || warps4 > kMaxThreads / 32) nlong = 0;
+            std::vector<SegTmp> rest;
+            for (const SegTmp& sg : segs) (nlong && sg.m >= P.quad_min ? quads : rest).push_back(sg);
+            segs.swap(rest);
+            std::stable_sort(quads.begin(), quads.end(), [](const SegTmp& x, const SegTmp& y) { return x.m > y.m; });
+        }
         order_segments(segs, 16, w == 8 ? 16 : 32, 0, ord);
         while ((ord.size() / 4) % 16) ord.insert(ord.end(), {0, 0, -1, -1});
-        const int32_t ngroups = (int32_t)(ord.size() / 64);
+        const int32_t ngroups2 = (int32_t)(ord.size() / 64), nquadg = (int32_t)((quads.size() + 7) / 8);
+        if (nquadg) out.has_quads = 1;
+        const int32_t ngroups = ngroups2 + nquadg;
         pb.seg.assign((size_t)ngroups * 128, 0);
-        for (int32_t gidx = 0; gidx < ngroups; ++gidx) {
+        for (int32_t gq = 0; gq < nquadg; ++gq) {
+            int32_t* G = &pb.seg[(size_t)(ngroups2 + gq) * 128];
+            for (int32_t l = 0; l < 32; ++l) { G[4 * l + 2] = -1; G[4 * l + 3] = -1; }
+            // The lanes of a shared-memory wavefront (fp64: lanes 0-15 = quarters 0, 1 and lanes 16-31 = quarters 2, 3;
+            // fp32: all 32) should start on distinct bank residues: a quarter boundary may move by up to two nodes and a
+            // lane may start up to 15 steps late (its residue moves with the delay), within the group's step count.
+            const int NBq = w == 8 ? 16 : 32;
+            char used[2][32];
+            std::memset(used, 0, sizeof(used));
+            const int32_t head_m = quads[(size_t)gq * 8].m;
+            const int32_t cap = (head_m - 3 + 3) / 4 + 2;                  // steps of the group: the head's longest quarter + 2
+            int32_t mx = 0;
+            for (int32_t k = 0; k < 8 && (size_t)(gq * 8 + k) < quads.size(); ++k) {
+                const SegTmp& sg = quads[(size_t)gq * 8 + k];
+                int32_t mq[4], aq[4], dq[4] = {0, 0, 0, 0};
+                for (int32_t j = 0; j < 4; ++j) mq[j] = (sg.m - 3) / 4 + (j < (sg.m - 3) % 4 ? 1 : 0);
+                aq[0] = sg.a;
+                for (int32_t j = 0; j < 4; ++j) {
+                    if (j > 0) aq[j] = aq[j - 1] + mq[j - 1] + 1;
+                    char* U = used[w == 8 ? j / 2 : 0];
+                    static const int kShift[5] = {0, 1, -1, 2, -2};
+                    bool done = false;
+                    for (int cost = 0; cost <= 17 && !done; ++cost)
+                        for (int t = 0; t < 5 && !done; ++t) {
+                            const int sh = j > 0 ? kShift[t] : 0, dl = cost - std::abs(sh);
+                            if (dl < 0 || dl > 15 || (j == 0 && t > 0)) continue;
+                            if (j > 0 && (mq[j - 1] + sh < 1 || mq[j] - sh < 1 || mq[j - 1] + sh + dq[j - 1] > cap)) continue;
+                            if (mq[j] - sh + dl > cap) continue;
+                            const int res = ((aq[j] + sh - dl) % NBq + NBq) % NBq;
+                            if (U[res]) continue;
+                            U[res] = 1; done = true;
+                            if (j > 0) { mq[j - 1] += sh; aq[j] += sh; mq[j] -= sh; }
+                            dq[j] = dl;
+                        }
+                }
+                for (int32_t j = 0; j < 4; ++j) {
+                    int32_t* Lq = G + 4 * (k + 8 * j);
+                    Lq[0] = aq[j]; Lq[1] = (int32_t)((uint32_t)mq[j] | ((uint32_t)j << 12) | (3u << 24) | (1u << 26) | ((uint32_t)dq[j] << 27));
+                    Lq[2] = sg.node; Lq[3] = j == 0 ? sg.tnode : -1;
+                    mx = std::max(mx, mq[j] + dq[j]);
+                }
+            }
+            out.padded_steps += 32 * (int64_t)(mx + 3);
+        }
+        for (int32_t gidx = 0; gidx < ngroups2; ++gidx) {
             int32_t mx = 0;
             for (int32_t k = 0; k < 16; ++k) {
                 const int32_t* sgp = &ord[(size_t)(gidx * 16 + k) * 4];
@@ -505,6 +572,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
         }
         pb.nlanes = ngroups * 32;
         for (const SegTmp& sg : segs) if (sg.m >= 0xfff) out.ok = false;
+        for (const SegTmp& sg : quads) if (sg.m >= 0xfff) out.ok = false;
         const int64_t meta = round_up(pb.nlev + 1, 4) + 4 * (int64_t)pb.nnode + 4 * (int64_t)pb.nexp +
                              4 * (int64_t)pb.nghost + 4 * (int64_t)pb.nlanes;
         pb.smem_need = 16 + 512 + 6 * round_up(pb.nnode + 1, E) * w + 4 * meta + narr * (int64_t)pb.L * w;
@@ -705,7 +773,7 @@ static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const It
     P.n_resident_unknowns += ib.n;
 }
 
-struct ItemNeed { int64_t smem; int32_t lanes; int32_t nparts; int32_t kind; int64_t smem_top; int32_t lanes_top; };
+struct ItemNeed { int64_t smem; int32_t lanes; int32_t nparts; int32_t kind; int64_t smem_top; int32_t lanes_top; int32_t quads; };
 
 // P1 + P2: cells -> work items, greedy in input order.  A cell whose lists fit the group budget
 // joins the open group while the group still fits; a cell that fits one block's budget gets its own item; a
@@ -735,7 +803,7 @@ static void pack_items(hines_plan& P, std::vector<ItemNeed>& need, std::vector<c
     ItemBuild cand, alone;
     auto push = [&](const std::vector<int64_t>& cells, const ItemBuild& ib) {
         emit_item(P, cells, ib);
-        need.push_back({ib.smem_need, ib.max_lanes, (int32_t)ib.parts.size(), ib.kind, ib.smem_top, ib.max_lanes_top});
+        need.push_back({ib.smem_need, ib.max_lanes, (int32_t)ib.parts.size(), ib.kind, ib.smem_top, ib.max_lanes_top, ib.has_quads});
     };
     // additive estimate of a cell's shared-memory need as a single part (upper side): arrays + per node the
     // record, two segment lanes and the node descriptor; decides group membership without building the group
@@ -854,7 +922,7 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
     auto slot_of = [&](int64_t smem) { int q = 0; for (int t = 0; t < kNumClassK; ++t) if (smem <= class_cap(t, max_smem)) q = t; return q; };
     std::vector<int> item_q(nitems, 0);
     std::vector<int64_t> need_max(nq, 0), count(nq, 0);
-    std::vector<int32_t> lanes_max(nq, 0);
+    std::vector<int32_t> lanes_max(nq, 0), quads_any(nq, 0);
     for (int64_t i = 0; i < nitems; ++i) {
         int q = slot_of(need[i].smem);
         if (need[i].kind == kItemCluster) q += kNumClassK * need[i].nparts;
@@ -863,11 +931,13 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
             const int qt = qSplitTop + slot_of(need[i].smem_top);
             need_max[qt] = std::max(need_max[qt], need[i].smem_top);
             lanes_max[qt] = std::max(lanes_max[qt], need[i].lanes_top);
+            quads_any[qt] |= need[i].quads;
             count[qt]++;
         }
         item_q[i] = q;
         need_max[q] = std::max(need_max[q], need[i].smem);
         lanes_max[q] = std::max(lanes_max[q], need[i].lanes);
+        quads_any[q] |= need[i].quads;
         count[q]++;
     }
     // launch order of the classes: clusters first (largest first), then single blocks, biggest first; the
@@ -888,6 +958,7 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
         P.class_smem_bytes.push_back((int32_t)smem);
         P.class_cluster.push_back(q >= kNumClassK && q < qSplitSub ? q / kNumClassK : 1);
         P.class_phase.push_back(c.phase);
+        P.class_quads.push_back(quads_any[q]);
         const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
         int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
         tmax = std::max<int64_t>(64, std::min<int64_t>(kMaxThreads, tmax));
@@ -1012,7 +1083,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~2047) ||
+        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~4095) ||
         o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024 || o.split_smem_bytes < 8192) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }
@@ -1030,6 +1101,8 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         P->opt = o;
         P->seg_cluster = o.max_segment;
         P->seg_single = auto_segment ? 40 : o.max_segment;
+        P->quad_min = (o.policy_flags & HINES_POLICY_NO_QUADS) ? 0 : 24;
+        P->quad_max_warps = 22;
         P->cell_offsets.assign(cell_offsets, cell_offsets + ncells + 1);
         hines_status_t st = canonical_tables(*P, parent);
         if (st != HINES_OK) return st;

@@ -87,6 +87,8 @@ struct hines_plan {
     hines_options_t opt{};
     int32_t max_levels = 0;
     int32_t breadth_first = 1;
+    int32_t quad_max_warps = 22;                       // ... where (blocks per SM) x (P1 warps with four lanes) stays within this
+    int32_t quad_min = 24;                             // segments with at least this many interior nodes get four lanes (0: never)
     int32_t seg_single = 64, seg_cluster = 64;         // segment target (max_segment) of single-block / multi-part items
 
     std::vector<int64_t> cell_offsets;
@@ -108,6 +110,7 @@ struct hines_plan {
     std::vector<int32_t> class_cluster;                // per class: blocks per item (cluster size), 1 = no cluster
     std::vector<int32_t> class_threads;                // per class: threads per block
     std::vector<int32_t> class_phase;                  // per class: kPhase*
+    std::vector<int32_t> class_quads;                  // per class: some part has four-lane segment groups
     std::vector<int64_t> class_first, class_count;     // ranges in class_parts (blocks of the class, launch order)
     std::vector<int32_t> class_parts;                  // part ids in launch order, class by class
     int64_t n_xch = 0;                                 // exchange slots (split items)

@@ -251,6 +251,7 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
         // No level is wider than the block: at most one node per thread and level, and only the warps that can ever
         // hold a node take part (named barrier over those; the others wait at the block barrier behind the sweep).
         const int pthreads = (maxwidth + 31) & ~31;
+        tid = nthreads - 1 - tid;                           // the LAST warps of the block sweep: P1 / P3 fill the first ones
         if (tid < pthreads) {
             int lo = ldsi1(lb_sa + 4u * (uint32_t)lfrom), hi = ldsi1(lb_sa + 4u * (uint32_t)(lfrom + 1));
             int lo_n = lfrom > lto ? ldsi1(lb_sa + 4u * (uint32_t)(lfrom - 1)) : 0;
@@ -311,6 +312,7 @@ __device__ __forceinline__ void sweep_forward_top(uint32_t nd_sa, uint32_t lb_sa
     if (ntoplev <= 0) return;
     if (maxwidth <= nthreads) {                             // one node per thread and level at most: see sweep_backward
         const int pthreads = (maxwidth + 31) & ~31;
+        tid = nthreads - 1 - tid;                           // the LAST warps of the block sweep: P1 / P3 fill the first ones
         if (tid < pthreads) {
             int lo = ldsi1(lb_sa), hi = ldsi1(lb_sa + 4u), hi_n = ldsi1(lb_sa + 8u);
             int v = lo + tid;
@@ -439,7 +441,8 @@ __device__ __forceinline__ void solve_cables_pcr(T* nd, const int32_t* cb, int n
 //   kModeRhs     the solve from those factors and b: no reciprocal, one FMA on every dependent chain.
 enum { kModeSolve = 0, kModeFactor = 1, kModeRhs = 2 };
 
-template <typename T, bool CL, int MODE>
+// QUAD: the class has four-lane segment groups (long segments); classes without them run the leaner instantiation.
+template <typename T, bool CL, int MODE, bool QUAD>
 __global__ void __launch_bounds__(384, 2)
 hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __restrict__ meta_g, const int4* __restrict__ runs_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
@@ -525,13 +528,14 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             const int4 sg = seg[base + lane];
             const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
             const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
-            const bool isB = kind == 2;
-            const int m = isB ? mb : (kind == 1 ? mt : 0);
+            const bool isB = kind == 2, quad = QUAD && __any_sync(FULL, kind == 3);
+            const int jq = kind == 3 ? (sg.y >> 12) & 3 : 0;
+            const int m = isB ? mb : (kind != 0 ? mt : 0);
             const int dl = (sg.y >> 27) & 15;
             const int mmax = __reduce_max_sync(FULL, m + dl);
             int i = sg.x;
             T B = T(0), dbt = T(0);
-            if (kind == 1 || (isB && hasq)) B = sb[i];
+            if (kind == 1 || kind == 3 || (isB && hasq)) B = sb[i];
             T g1 = T(0), h1 = T(0), r1 = T(0), b1 = T(0);
             if (m > 0) { g1 = sd[i]; h1 = su[i]; r1 = sr[i]; b1 = sb[i + 1]; }
             for (int s = 0; s < mmax; ++s) {
@@ -546,20 +550,25 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
                     ++i;
                 }
             }
-            const T pB = __shfl_xor_sync(FULL, B, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
-            if (kind == 1) {
-                T* q = nd + 6 * sg.z;
-                int bpos = i;
-                if (hasq) {                                 // i is q now; the separator sits behind B's half
-                    const T Bq = B - pdb;
-                    sb[i] = Bq * sr[i];
-                    dbt = fmad<T>(su[i], Bq, dbt);
-                    q[1] = fnma<T>(sd[i], Bq, pB); q[5] = dbt;
-                    bpos = i + 1 + mb;
-                } else {
-                    q[1] = B; q[5] = T(0);
+            const bool lead = quad ? (kind == 3 && jq == 0) : (kind == 1);
+            const int stride = quad ? 8 : 16, nq = quad ? 3 : 1;
+            T Bc = B;
+            int qi = i;
+            for (int sq = 1; sq <= nq; ++sq) {              // the middle nodes, in turn (see the solve path)
+                const int src = (lane + stride * sq) & 31;
+                const T pB = __shfl_sync(FULL, B, src), pdb = __shfl_sync(FULL, dbt, src);
+                const int pm = __shfl_sync(FULL, m, src);
+                if (lead && hasq) {
+                    const T Bq = Bc - pdb;
+                    sb[qi] = Bq * sr[qi];
+                    dbt = fmad<T>(su[qi], Bq, dbt);
+                    Bc = fnma<T>(sd[qi], Bq, pB);
+                    qi += pm + 1;
                 }
-                q[0] = sd[bpos]; q[2] = su[bpos]; q[3] = sr[bpos]; q[4] = T(0);    // the separator's factors: g = -f, -U, r
+            }
+            if (lead) {                                     // qi is the separator: its factors g = -f, -U, r sit at its place
+                T* q = nd + 6 * sg.z;
+                q[0] = sd[qi]; q[1] = Bc; q[2] = su[qi]; q[3] = sr[qi]; q[4] = T(0); q[5] = hasq ? dbt : T(0);
             }
         }
     } else
@@ -567,14 +576,17 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     for (int base = (tid & ~31); base < nseg_lanes; base += nthreads) {
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
+        // kind 1 / 2: the A / B lane of a two-lane segment (partner = lane ^ 16); kind 3: lane j of a four-lane segment
+        // (its lanes are 8 apart).  Every lane sweeps its piece top-down with fill-in to the node right above the piece.
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
-        const bool isB = kind == 2;
-        const int m = isB ? mb : (kind == 1 ? mt : 0);
+        const bool isB = kind == 2, quad = QUAD && __any_sync(FULL, kind == 3);
+        const int jq = kind == 3 ? (sg.y >> 12) & 3 : 0;
+        const int m = isB ? mb : (kind != 0 ? mt : 0);
         const int dl = (sg.y >> 27) & 15;                   // the lane starts dl steps late (bank residues, plan.cpp)
         const int mmax = __reduce_max_sync(FULL, m + dl);
         int i = sg.x;
         T D = T(1), B = T(0), ee = T(0), ddt = T(0), dbt = T(0), un = T(0), dn = T(0), bn = T(0);
-        if (kind == 1 || (isB && hasq)) { D = sd[i]; if (MODE == kModeSolve) B = sb[i]; if (isB || sg.w >= 0) ee = su[i]; }
+        if (kind == 1 || kind == 3 || (isB && hasq)) { D = sd[i]; if (MODE == kModeSolve) B = sb[i]; if (isB || jq > 0 || sg.w >= 0) ee = su[i]; }
         if (m > 0) { un = su[i + 1]; dn = sd[i + 1]; if (MODE == kModeSolve) bn = sb[i + 1]; }
         {
             // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
@@ -601,20 +613,52 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
 #undef HINES_P1_STEP
             i += m;
         }
-        // B -> A: what is left of b (pD, pB), its coupling to q (pe), B's contribution parked for q (pdd, pdb)
-        const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
-        const T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
-        if (kind == 1) {
-            T* q = nd + 6 * sg.z;
-            if (hasq) {                                     // i is q now
-                const T Dq = D - pdd, Bq = B - pdb;
-                const T r = rcp<T>(Dq);
-                const T gq = pe * r, hq = ee * r;
-                sd[i] = gq; su[i] = hq; sb[i] = MODE == kModeFactor ? r : Bq * r;
-                ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
-                q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = hq * pe; q[4] = ddt; q[5] = dbt;     // slot 2 = -U
-            } else {                                        // a segment of one compartment: the separator as it is
-                q[0] = D; q[1] = B; q[2] = -ee; q[4] = T(0); q[5] = T(0);
+        // The middle nodes, in turn, by the segment's first lane: the lane of the piece below hands over what is left of
+        // the node it arrived at (pD, pB), that node's coupling to the middle node (pe) and the piece's contribution
+        // parked for the middle node (pdd, pdb).  One middle node for a two-lane segment, three for a four-lane one.
+        if (!quad) {
+            // B -> A: what is left of b (pD, pB), its coupling to q (pe), B's contribution parked for q (pdd, pdb)
+            const T pD = __shfl_xor_sync(FULL, D, 16), pB = __shfl_xor_sync(FULL, B, 16), pe = __shfl_xor_sync(FULL, ee, 16);
+            const T pdd = __shfl_xor_sync(FULL, ddt, 16), pdb = __shfl_xor_sync(FULL, dbt, 16);
+            if (kind == 1) {
+                T* q = nd + 6 * sg.z;
+                if (hasq) {                                 // i is q now
+                    const T Dq = D - pdd, Bq = B - pdb;
+                    const T r = rcp<T>(Dq);
+                    const T gq = pe * r, hq = ee * r;
+                    sd[i] = gq; su[i] = hq; sb[i] = MODE == kModeFactor ? r : Bq * r;
+                    ddt = fmad<T>(hq, ee, ddt); dbt = fmad<T>(hq, Bq, dbt);
+                    q[0] = fnma<T>(gq, pe, pD); q[1] = fnma<T>(gq, Bq, pB); q[2] = hq * pe; q[4] = ddt; q[5] = dbt;     // slot 2 = -U
+                    if (MODE == kModeFactor) q[3] = (T)(i + 1 + mb);                                                    // slot 3 = staged index of b
+                } else {                                    // a segment of one compartment: the separator as it is
+                    q[0] = D; q[1] = B; q[2] = -ee; q[4] = T(0); q[5] = T(0);
+                    if (MODE == kModeFactor) q[3] = (T)i;
+                }
+            }
+        } else {
+            const bool lead = kind == 3 && jq == 0;
+            T Dc = D, Bc = B, et = ee;
+            int qi = i;
+#pragma unroll
+            for (int sq = 1; sq <= 3; ++sq) {
+                const int src = (lane + 8 * sq) & 31;
+                const T pD = __shfl_sync(FULL, D, src), pB = __shfl_sync(FULL, B, src), pe = __shfl_sync(FULL, ee, src);
+                const T pdd = __shfl_sync(FULL, ddt, src), pdb = __shfl_sync(FULL, dbt, src);
+                const int pm = __shfl_sync(FULL, m, src);
+                if (lead) {                                 // qi is the middle node
+                    const T Dq = Dc - pdd, Bq = Bc - pdb;
+                    const T r = rcp<T>(Dq);
+                    const T gq = pe * r, hq = et * r;
+                    sd[qi] = gq; su[qi] = hq; sb[qi] = MODE == kModeFactor ? r : Bq * r;
+                    ddt = fmad<T>(hq, et, ddt); dbt = fmad<T>(hq, Bq, dbt);
+                    Dc = fnma<T>(gq, pe, pD); Bc = fnma<T>(gq, Bq, pB); et = -hq * pe;
+                    qi += pm + 1;
+                }
+            }
+            if (lead) {                                     // qi is the separator now; slot 2 = -U, slot 3 = its staged index
+                T* q = nd + 6 * sg.z;
+                q[0] = Dc; q[1] = Bc; q[2] = -et; q[4] = ddt; q[5] = dbt;
+                if (MODE == kModeFactor) q[3] = (T)qi;
             }
         }
     }
@@ -720,18 +764,16 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     const int xs = 2 * (rounds & 1) + 1;                  // record slot that holds x after the forward sweep
     HINES_STAMP(4);
 
-    // ---- P3: expand the interiors: A computes x[q] from x[b] and x[t]; then A walks up from q-1 to a
-    //      (x[i] = c - g x[i+1] - h x[t]) and B walks up from b-1 to q+1 (x[i] = c - g x[i+1] - h x[q]), one FMA
-    //      on the dependent chain per step ----
+    // ---- P3: expand the interiors: the segment's first lane computes x of the middle nodes from x[b] and x[t]; then
+    //      every lane walks its piece upward, x[i] = c - g x[i+1] - h x[top of the piece]: one FMA on the dependent
+    //      chain per step ----
     if (MODE == kModeFactor) {
         // the separators' factors go where their compartments are: g = -f, -U, r = 1 / pivot
         __syncthreads();
-        for (int k = tid; k < nseg_lanes; k += nthreads) {
-            const int4 sg = seg[k];
-            if (((sg.y >> 24) & 3) != 1) continue;
-            const int hasq = (sg.y >> 26) & 1, mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
-            const int bpos = sg.x + (hasq ? mt + 1 + mb : 0);
-            const T* q = nd + 6 * sg.z;
+        for (int v = tid; v < H.nlevnode; v += nthreads) {
+            const T* q = nd + 6 * v;
+            if (reinterpret_cast<const int4*>(meta + H.kp_off)[v].z < 0) continue;       // a ghost child has no compartment here
+            const int bpos = (int)q[3];                                                  // written by the segment's first lane in P1
             sd[bpos] = q[0]; su[bpos] = q[2]; sb[bpos] = q[1];
         }
     } else
@@ -739,25 +781,48 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         const int4 sg = seg[base + lane];
         const int kind = (sg.y >> 24) & 3, hasq = (sg.y >> 26) & 1;
         const int mt = sg.y & 0xfff, mb = (sg.y >> 12) & 0xfff;
-        const bool isB = kind == 2;
-        const int m = isB ? mb : (kind == 1 ? mt : 0);
+        const bool isB = kind == 2, quad = QUAD && __any_sync(FULL, kind == 3);
+        const int jq = kind == 3 ? (sg.y >> 12) & 3 : (isB ? 1 : 0);          // which piece of its segment the lane holds
+        const int m = isB ? mb : (kind != 0 ? mt : 0);
         const int dl = (sg.y >> 27) & 15;
         const int mmax = __reduce_max_sync(FULL, m + dl);
         const int p0 = sg.x;
         T xb = T(0), xt = T(0), xn = T(0);
         if (kind != 0) xb = nd[6 * sg.z + xs];
-        if (kind == 1) {
-            if (sg.w >= 0) xt = nd[6 * sg.w + xs];
-            if (hasq) {
-                const int iq = p0 + mt;
-                xn = fnma<T>(sd[iq], xb, fnma<T>(su[iq], xt, sb[iq]));
-                sb[iq] = xn; sb[iq + 1 + mb] = xb;
-            } else {
-                sb[p0] = xb;
+        if (!quad) {
+            if (kind == 1) {
+                if (sg.w >= 0) xt = nd[6 * sg.w + xs];
+                if (hasq) {
+                    const int iq = p0 + mt;
+                    xn = fnma<T>(sd[iq], xb, fnma<T>(su[iq], xt, sb[iq]));
+                    sb[iq] = xn; sb[iq + 1 + mb] = xb;
+                } else {
+                    sb[p0] = xb;
+                }
             }
+            const T xq = __shfl_xor_sync(FULL, xn, 16);
+            if (isB) { xn = xb; xt = xq; }
+        } else {
+            // the middle nodes, from the separator upward, by the segment's first lane: x[q] = c - g x[below] - h x[t]
+            const bool lead = kind == 3 && jq == 0;
+            const int m1 = __shfl_sync(FULL, m, (lane + 8) & 31), m2 = __shfl_sync(FULL, m, (lane + 16) & 31),
+                      m3 = __shfl_sync(FULL, m, (lane + 24) & 31);
+            T x1 = T(0), x2 = T(0), x3 = T(0);
+            if (lead) {
+                if (sg.w >= 0) xt = nd[6 * sg.w + xs];
+                const int q1 = p0 + m, q2 = q1 + m1 + 1, q3 = q2 + m2 + 1;
+                x3 = fnma<T>(sd[q3], xb, fnma<T>(su[q3], xt, sb[q3]));
+                x2 = fnma<T>(sd[q2], x3, fnma<T>(su[q2], xt, sb[q2]));
+                x1 = fnma<T>(sd[q1], x2, fnma<T>(su[q1], xt, sb[q1]));
+                sb[q3] = x3; sb[q2] = x2; sb[q1] = x1; sb[q3 + m3 + 1] = xb;
+            }
+            // every lane: x of the node above its piece (the top) and of the node below it (where its walk starts)
+            const int ll = (lane - 8 * jq) & 31;                               // the segment's first lane
+            const T s1 = __shfl_sync(FULL, x1, ll), s2 = __shfl_sync(FULL, x2, ll), s3 = __shfl_sync(FULL, x3, ll);
+            const T st = __shfl_sync(FULL, xt, ll);
+            xt = jq == 0 ? st : (jq == 1 ? s1 : (jq == 2 ? s2 : s3));
+            xn = jq == 0 ? s1 : (jq == 1 ? s2 : (jq == 2 ? s3 : xb));
         }
-        const T xq = __shfl_xor_sync(FULL, xn, 16);
-        if (isB) { xn = xb; xt = xq; }
         T g1 = T(0), h1 = T(0), c1 = T(0);
         if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
         for (int jj = mmax - 1; jj >= 0; --jj) {
@@ -888,11 +953,12 @@ static void free_device(DeviceTables* D)
 template <typename T>
 static hines_status_t prepare_kernels(int max_optin)
 {
-#define HINES_PREP(MODE)                                                                                                          \
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, false, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin)); \
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));  \
-    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    HINES_PREP(kModeSolve) HINES_PREP(kModeFactor) HINES_PREP(kModeRhs)
+#define HINES_PREP(MODE, Q)                                                                                                          \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, false, MODE, Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin)); \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE, Q>, cudaFuncAttributeMaxDynamicSharedMemorySize, max_optin));  \
+    CUDA_TRY(cudaFuncSetAttribute(hines_resident_kernel<T, true, MODE, Q>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    HINES_PREP(kModeSolve, false) HINES_PREP(kModeFactor, false) HINES_PREP(kModeRhs, false)
+    HINES_PREP(kModeSolve, true) HINES_PREP(kModeFactor, true) HINES_PREP(kModeRhs, true)
 #undef HINES_PREP
     return HINES_OK;
 }
@@ -911,7 +977,7 @@ static hines_status_t check_clusters(const hines_plan* P)
         attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr; cfg.numAttrs = 1;
         int nclusters = 0;
-        CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, hines_resident_kernel<T, true, kModeSolve>, &cfg));
+        CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, hines_resident_kernel<T, true, kModeSolve, true>, &cfg));
         if (nclusters < 1) {
             set_error("this device cannot co-schedule a cluster of " + std::to_string(cl) + " blocks with " +
                       std::to_string(P->class_smem_bytes[q]) + " bytes of shared memory each: create the plan with a smaller cluster_max");
@@ -1030,33 +1096,27 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         T* xh = static_cast<T*>(D->xch_h); T* xx = static_cast<T*>(D->xch_x);
         const int phase = (int)P->class_phase[q];
         if (mode == kModeFactor && phase == kPhaseC) return HINES_OK;       // the factors of a sub-tree part are complete after phase A
-        if (cl == 1) {
-            const unsigned grid = (unsigned)cnt, thr = (unsigned)P->class_threads[q];
-            const size_t sm = (size_t)P->class_smem_bytes[q];
-            if (mode == kModeSolve)
-                hines_resident_kernel<T, false, kModeSolve><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
-            else if (mode == kModeFactor)
-                hines_resident_kernel<T, false, kModeFactor><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
-            else
-                hines_resident_kernel<T, false, kModeRhs><<<grid, thr, sm, ls>>>(recs, D->meta, D->runs, d, u, b, x, f0, f1, f2, P->n, xh, xx, phase, prof);
-        } else {
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3((unsigned)cnt);
-            cfg.blockDim = dim3((unsigned)P->class_threads[q]);
-            cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
-            cfg.stream = ls;
-            cudaLaunchAttribute attr[1];
-            attr[0].id = cudaLaunchAttributeClusterDimension;
-            attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-            cfg.attrs = attr; cfg.numAttrs = 1;
-            const int32_t* mg_ = D->meta; const int4* rg_ = D->runs; const int64_t n_ = P->n;
-            if (mode == kModeSolve)
-                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeSolve>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
-            else if (mode == kModeFactor)
-                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeFactor>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
-            else
-                CUDA_TRY(cudaLaunchKernelEx(&cfg, hines_resident_kernel<T, true, kModeRhs>, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, 0, prof));
-        }
+        typedef void (*kern_t)(const BlockRecord*, const int32_t*, const int4*, const T*, const T*, const T*, T*, T*, T*, T*,
+                               int64_t, T*, T*, int, unsigned long long*);
+        const bool quads = P->class_quads[q] != 0;
+        kern_t kern;
+#define HINES_PICK(CLV)                                                                                                        \
+        kern = mode == kModeSolve ? (quads ? hines_resident_kernel<T, CLV, kModeSolve, true> : hines_resident_kernel<T, CLV, kModeSolve, false>)     \
+             : mode == kModeFactor ? (quads ? hines_resident_kernel<T, CLV, kModeFactor, true> : hines_resident_kernel<T, CLV, kModeFactor, false>) \
+                                   : (quads ? hines_resident_kernel<T, CLV, kModeRhs, true> : hines_resident_kernel<T, CLV, kModeRhs, false>);
+        if (cl == 1) { HINES_PICK(false) } else { HINES_PICK(true) }
+#undef HINES_PICK
+        const int32_t* mg_ = D->meta; const int4* rg_ = D->runs; const int64_t n_ = P->n;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)cnt);
+        cfg.blockDim = dim3((unsigned)P->class_threads[q]);
+        cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
+        cfg.stream = ls;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr; cfg.numAttrs = cl > 1 ? 1 : 0;
+        CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, cl > 1 ? 0 : phase, prof));
         return HINES_OK;
     };
     // Size classes are independent: the first runs on the caller's stream, the others on side streams forked

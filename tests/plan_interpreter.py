@@ -78,6 +78,34 @@ def pairs(sg):
             yield int(A[0]), mt, mb, hasq, int(A[2]), int(A[3])
 
 
+def segments(sg):
+    """Segments of a part's lane list, two-lane and four-lane groups alike: yields (a, lens, node, tnode) where lens are
+    the steps of the segment's lanes (its halves / quarters; [] for a segment that is its separator alone) and the
+    middle nodes sit between them: the segment covers a .. a + sum(lens) + len(lens) - 1, the last one its separator."""
+    assert len(sg) % 32 == 0
+    for g in range(0, len(sg), 32):
+        kinds = [(int(sg[g + l][1]) >> 24) & 3 for l in range(32)]
+        if 3 in kinds:                                     # a four-lane group: lane k + 8 j = quarter j of segment k
+            assert all(k in (0, 3) for k in kinds)
+            for k in range(8):
+                Ls = [sg[g + k + 8 * j] for j in range(4)]
+                if kinds[k] == 0:
+                    assert all(kinds[k + 8 * j] == 0 and Ls[j][2] == -1 for j in range(4))
+                    continue
+                lens, pos = [], int(Ls[0][0])
+                for j in range(4):
+                    w = int(Ls[j][1])
+                    assert kinds[k + 8 * j] == 3 and (w >> 12) & 3 == j and (w >> 26) & 1 == 1
+                    assert int(Ls[j][0]) == pos and Ls[j][2] == Ls[0][2] and (j == 0 or Ls[j][3] == -1)
+                    lens.append(w & 0xfff)
+                    pos += lens[-1] + 1
+                assert max(lens) - min(lens) <= 5 and min(lens) >= 1
+                yield int(Ls[0][0]), lens, int(Ls[0][2]), int(Ls[0][3])
+        else:
+            for a, mt, mb, hasq, node, tnode in pairs(sg[g:g + 32]):
+                yield a, ([mt, mb] if hasq else []), node, tnode
+
+
 def parts_of(plan):
     hdrs = plan.table("part_header").reshape(-1, 32)
     meta = plan.table("part_meta")
@@ -107,43 +135,41 @@ class _PartState:
         self.w = 16 // E
 
     def condense(self):
-        """P1: two lanes per segment, both top-down."""
+        """P1: the lanes of a segment (two or four), all top-down with fill-in to the lane's top; then the middle nodes
+        in turn, by the segment's first lane."""
         sd, su, sb, rec = self.sd, self.su, self.sb, self.rec
-        for a, mt, mb, hasq, node, tnode in pairs(self.p.seg):
-            i = a
-            D, B = sd[i], sb[i]
-            ee = su[i] if tnode >= 0 else 0.0
-            ddt = dbt = 0.0
-            for _ in range(mt):
-                un, dn, bn = su[i + 1], sd[i + 1], sb[i + 1]
-                r = 1.0 / D
-                g, h, c = un * r, ee * r, B * r
-                sd[i], su[i], sb[i] = g, h, c
-                ddt += h * ee; dbt += h * B
-                D, B, ee = dn - g * un, bn - g * B, -h * un
-                i += 1
-            if hasq:
-                q = a + mt; bp = q + 1 + mb
-                j = q + 1
-                Db, Bb, eb = sd[j], sb[j], su[j]
-                pdd = pdb = 0.0
-                for _ in range(mb):
-                    un, dn, bn = su[j + 1], sd[j + 1], sb[j + 1]
-                    r = 1.0 / Db
-                    g, h, c = un * r, eb * r, Bb * r
-                    sd[j], su[j], sb[j] = g, h, c
-                    pdd += h * eb; pdb += h * Bb
-                    Db, Bb, eb = dn - g * un, bn - g * Bb, -h * un
-                    j += 1
-                assert j == bp
-                Dq, Bq = D - pdd, B - pdb
-                r = 1.0 / Dq
-                gq, hq = eb * r, ee * r
-                sd[q], su[q], sb[q] = gq, hq, Bq * r
-                ddt += hq * ee; dbt += hq * Bq
-                new = (Db - gq * eb, Bb - gq * Bq, hq * eb, ddt, dbt)      # slot 2 holds -U
+        for a, lens, node, tnode in segments(self.p.seg):
+            if not lens:
+                new = (sd[a], sb[a], -(su[a] if tnode >= 0 else 0.0), 0.0, 0.0)
             else:
-                new = (D, B, -ee, 0.0, 0.0)
+                arr, start = [], a
+                for j, mj in enumerate(lens):
+                    i = start
+                    D, B = sd[i], sb[i]
+                    ee = su[i] if (j > 0 or tnode >= 0) else 0.0
+                    ddt = dbt = 0.0
+                    for _ in range(mj):
+                        un, dn, bn = su[i + 1], sd[i + 1], sb[i + 1]
+                        r = 1.0 / D
+                        g, h, c = un * r, ee * r, B * r
+                        sd[i], su[i], sb[i] = g, h, c
+                        ddt += h * ee; dbt += h * B
+                        D, B, ee = dn - g * un, bn - g * B, -h * un
+                        i += 1
+                    arr.append((D, B, ee, ddt, dbt))
+                    start = i + 1
+                Dc, Bc, et, ddt, dbt = arr[0]
+                q = a + lens[0]
+                for s_ in range(1, len(lens)):
+                    pD, pB, pe, pdd, pdb = arr[s_]
+                    Dq, Bq = Dc - pdd, Bc - pdb
+                    r = 1.0 / Dq
+                    gq, hq = pe * r, et * r
+                    sd[q], su[q], sb[q] = gq, hq, Bq * r
+                    ddt += hq * et; dbt += hq * Bq
+                    Dc, Bc, et = pD - gq * pe, pB - gq * Bq, -hq * pe
+                    q += lens[s_] + 1
+                new = (Dc, Bc, -et, ddt, dbt)                   # slot 2 holds -U
             assert 0 <= node < self.p.h["nlevnode"] and np.isnan(rec[node, 0]), "node written twice"
             assert not self.p.ghost[node], "a ghost child has no segment"
             rec[node, 0], rec[node, 1], rec[node, 2], rec[node, 4], rec[node, 5] = new
@@ -233,23 +259,31 @@ class _PartState:
     def expand(self, xnode, x, E):
         """P3 + the store, run by run."""
         sd, su, sb = self.sd, self.su, self.sb
-        for a, mt, mb, hasq, node, tnode in pairs(self.p.seg):
+        for a, lens, node, tnode in segments(self.p.seg):
             xb = xnode[node]
             xt = xnode[tnode] if tnode >= 0 else 0.0
-            if not hasq:
+            if not lens:
                 sb[a] = xb
                 continue
-            q = a + mt; bp = q + 1 + mb
-            xq = (sb[q] - su[q] * xt) - sd[q] * xb
-            sb[q] = xq; sb[bp] = xb
-            xn = xq
-            for j in range(q - 1, a - 1, -1):
-                xn = (sb[j] - su[j] * xt) - sd[j] * xn
-                sb[j] = xn
-            xn = xb
-            for j in range(bp - 1, q, -1):
-                xn = (sb[j] - su[j] * xq) - sd[j] * xn
-                sb[j] = xn
+            qs = [a + lens[0]]
+            for s_ in range(1, len(lens) - 1):
+                qs.append(qs[-1] + lens[s_] + 1)
+            bp = qs[-1] + lens[-1] + 1
+            xq, xnext = {}, xb
+            for s_ in range(len(qs) - 1, -1, -1):              # the middle nodes, from the separator upward
+                q = qs[s_]
+                xq[s_] = (sb[q] - su[q] * xt) - sd[q] * xnext
+                sb[q] = xq[s_]
+                xnext = xq[s_]
+            sb[bp] = xb
+            start = a
+            for j, mj in enumerate(lens):
+                xT = xt if j == 0 else xq[j - 1]
+                xn = xq[j] if j < len(qs) else xb
+                for i in range(start + mj - 1, start - 1, -1):
+                    xn = (sb[i] - su[i] * xT) - sd[i] * xn
+                    sb[i] = xn
+                start += mj + 1
         for g, ln, so, _ in self.p.runs:
             assert np.isnan(x[g:g + ln]).all(), "compartment stored twice"
             x[g:g + ln] = sb[so:so + ln]

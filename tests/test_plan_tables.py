@@ -13,7 +13,7 @@ import morphgen as mg
 import oracle
 import paper_1810_12742_b200 as hb
 from helpers import random_parent
-from plan_interpreter import pairs, parts_of
+from plan_interpreter import parts_of, segments
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -171,8 +171,8 @@ def _check_policy(m, plan, max_segment=0):
         for r, p in enumerate(ps):
             inv = {v: k for k, (pr, v) in where.items() if pr == r}
             seen_nodes = set()
-            for a, mt, mb, hasq, node, tnode in pairs(p.seg):
-                mm = mt + mb + hasq
+            for a, lens, node, tnode in segments(p.seg):
+                mm = sum(lens) + max(0, len(lens) - 1)
                 assert 0 <= node < p.h["nlevnode"] and node not in seen_nodes and not p.ghost[node]
                 seen_nodes.add(node)
                 g0 = inv[a]
