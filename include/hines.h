@@ -69,6 +69,8 @@ enum {
                                         staged arrays (three factors + b) instead of three, and own N x 3 factor values  */
     HINES_POLICY_NO_QUADS     = 1024, /* every segment gets two lanes (default: four lanes for segments with >= 24 interior
                                         compartments: half the dependent steps in P1 / P3)                         */
+    HINES_POLICY_NO_PDL       = 2048, /* split items: the three launches strictly one after the other (default: programmatic
+                                        dependent launch, a phase starts while the one before it still runs)        */
     HINES_POLICY_NO_SPLIT     = 64,  /* no split items: a cell that fits no cluster goes to the streaming path  */
     HINES_POLICY_SPLIT_LEVEL_MEAN = 128 /* f1: cut branches by the paper's own rule first (level by
                                         level from the root, over all cells of the batch, a branch longer than

@@ -1083,7 +1083,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
         o.smem_bytes_per_block < 1024 || o.smem_bytes_per_block > kSmemMaxOptin || o.group_smem_bytes < 0 ||
-        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~4095) ||
+        o.max_segment < 2 || o.max_segment > 1023 || (o.policy_flags & ~8191) ||
         o.cluster_max < 1 || o.cluster_max > 16 || o.chunk_smem_bytes < 1024 || o.split_smem_bytes < 8192) {
         set_error("options: value out of range"); return HINES_ERR_INVALID_ARG;
     }

@@ -189,6 +189,11 @@ template <typename T> __device__ __forceinline__ T fmad(T a, T b, T c);   // c +
 template <> __device__ __forceinline__ double fmad<double>(double a, double b, double c) { return fma(a, b, c); }
 template <> __device__ __forceinline__ float fmad<float>(float a, float b, float c) { return fmaf(a, b, c); }
 
+// programmatic dependent launch (split items): the next launch of the stream may start while this one runs, and waits
+// for this one's completion (and the visibility of its writes) only where it needs its results
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // split-phase cluster barrier (every thread of every block of the cluster arrives and waits, in turn)
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
@@ -469,6 +474,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     if (tid < 32) reinterpret_cast<int4*>(smem + 16)[tid] = reinterpret_cast<const int4*>(recs + blockIdx.x)[tid];
     if (tid == 0) mbar_init(bar, 1);
     __syncthreads();
+    if (!CL && (phase == kPhaseA || phase == kPhaseB)) pdl_launch_dependents();
     const int L = H.L, NN = (H.nnode + 1 + E - 1) / E * E;    // one all-zero record behind the last node
     T* nd = reinterpret_cast<T*>(smem + 16 + sizeof(BlockRecord));
     int32_t* meta = reinterpret_cast<int32_t*>(nd + 6 * NN);
@@ -685,6 +691,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     if (CL) {
         if (rank == 0) { cluster_wait(); cluster_arrive(); cluster_wait(); }   // barrier 1: the other ranks have swept and exported
     } else if (phase == kPhaseB) {
+        pdl_wait();                                         // phase A has completed: the hand-off values are there
         for (int e = tid; e < nghost; e += nthreads) {
             const int4 g = gh[e];
             *reinterpret_cast<V2*>(nd + 6 * g.x + 4) = reinterpret_cast<const V2*>(xch_h)[H.xch_base + g.y];
@@ -724,6 +731,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
         if (MODE != kModeFactor) return;
     } else if (phase == kPhaseC) {
+        pdl_wait();                                         // phase B has completed: the parents' x is there
         for (int e = tid; e < nexp; e += nthreads) {
             const int4 q = ex[e];
             nd[6 * q.w] = T(0); nd[6 * q.w + 1] = xch_x[H.xch_base + q.y];
@@ -1113,9 +1121,18 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
         cfg.dynamicSmemBytes = (size_t)P->class_smem_bytes[q];
         cfg.stream = ls;
         cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeClusterDimension;
-        attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-        cfg.attrs = attr; cfg.numAttrs = cl > 1 ? 1 : 0;
+        cfg.attrs = attr; cfg.numAttrs = 0;
+        if (cl > 1) {
+            attr[0].id = cudaLaunchAttributeClusterDimension;
+            attr[0].val.clusterDim.x = (unsigned)cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+            cfg.numAttrs = 1;
+        } else if ((phase == kPhaseB || phase == kPhaseC) && mode != kModeFactor && !(P->opt.policy_flags & HINES_POLICY_NO_PDL)) {
+            // split items: phases B and C start while the phase before them still runs (load, P1, their own sweeps) and
+            // wait for it only where they import its results
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.numAttrs = 1;
+        }
         CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, cl > 1 ? 0 : phase, prof));
         return HINES_OK;
     };
