@@ -427,9 +427,14 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
                     const int32_t b = nbr[nt.gid];
                     pn = next + pb.nexp;
                     gp_of_branch[b] = pn;
-                    if (kind == kItemCluster) pb.exps.insert(pb.exps.end(), {v, g0_of_branch[b], p0_of_branch[b], pn});
-                    else pb.exps.insert(pb.exps.end(), {v, x_of_branch[b], 0, pn});
-                    if (g0_of_branch[b] < 0) { out.ok = false; return; }
+                    if (g0_of_branch[b] < 0 || pn >= (1 << 20) || p == 0) { out.ok = false; return; }
+                    if (kind == kItemCluster) {
+                        // {node, ghost parent, ghost child in part 0, its parent there}; rank 0 sends the parent's x back
+                        // to the block of this part, behind this entry (its last two ints are dead by then): the ghost
+                        // child's entry names {rank << 20 | export}, turned into a shared-memory word by emit_item
+                        pb.exps.insert(pb.exps.end(), {v, pn, g0_of_branch[b], p0_of_branch[b]});
+                        out.parts[0].ghosts[4 * (size_t)x_of_branch[b] + 3] = (p << 20) | pb.nexp;
+                    } else pb.exps.insert(pb.exps.end(), {v, pn, x_of_branch[b], 0});          // split item: exchange slot
                     ++pb.nexp;
                 }
             }
@@ -734,8 +739,26 @@ static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const It
     P.item_kind.push_back(ib.kind);
     P.item_xch.push_back((int32_t)P.n_xch);
     const int32_t xs0 = 2 * (ib.parts[0].rounds & 1) + 1;
+    // where the blocks of a cluster item receive their parents' x: 4-byte word index, from the start of the block's
+    // shared memory, of int 2 of the export's entry ([mbarriers 16 | block record | node records | lb | kp | exports ..])
+    std::vector<int32_t> land0(ib.parts.size(), 0);
+    const int64_t E = 16 / P.width;
     for (size_t r = 0; r < ib.parts.size(); ++r) {
         const PartBuild& pb = ib.parts[r];
+        const int64_t NN = round_up((int64_t)pb.nnode + 1, E);
+        const int64_t meta_word = (16 + (int64_t)sizeof(hines::BlockRecord) + 6 * P.width * NN) / 4;
+        land0[r] = (int32_t)(meta_word + round_up((int64_t)pb.lb.size(), 4) + round_up((int64_t)pb.kp.size(), 4) + 2);
+    }
+    for (size_t r = 0; r < ib.parts.size(); ++r) {
+        PartBuild pb_patched;
+        if (r == 0 && ib.kind == kItemCluster) {
+            pb_patched = ib.parts[0];
+            for (int32_t g = 0; g < pb_patched.nghost; ++g) {
+                const int32_t w = pb_patched.ghosts[4 * (size_t)g + 3], rr = w >> 20, e = w & 0xfffff;
+                pb_patched.ghosts[4 * (size_t)g + 3] = (rr << 20) | (land0[rr] + 4 * e);
+            }
+        }
+        const PartBuild& pb = (r == 0 && ib.kind == kItemCluster) ? pb_patched : ib.parts[r];
         hines::PartHeader h{};
         h.meta_off = (int64_t)P.part_meta.size();
         std::vector<int32_t>& M = P.part_meta;

@@ -197,6 +197,44 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 // split-phase cluster barrier (every thread of every block of the cluster arrives and waits, in turn)
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+// shared-memory address of the same variable in block `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa_u32(uint32_t addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+// store into another block's shared memory that counts its bytes on THAT block's mbarrier: data and signal in one
+__device__ __forceinline__ void st_async_2(uint32_t raddr, double a, double b, uint32_t rbar)
+{
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];" ::"r"(raddr), "d"(a), "d"(b), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void st_async_2(uint32_t raddr, float a, float b, uint32_t rbar)
+{
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.v2.f32 [%0], {%1, %2}, [%3];" ::"r"(raddr), "f"(a), "f"(b), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void st_async_1(uint32_t raddr, double a, uint32_t rbar)
+{
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(raddr), "d"(a), "r"(rbar) : "memory");
+}
+__device__ __forceinline__ void st_async_1(uint32_t raddr, float a, uint32_t rbar)
+{
+    asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.f32 [%0], %1, [%2];" ::"r"(raddr), "f"(a), "r"(rbar) : "memory");
+}
+// wait for a phase of an mbarrier that blocks of the whole cluster complete
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAITC_LOOP:\n"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAITC_DONE;\n"
+        "bra WAITC_LOOP;\n"
+        "WAITC_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
 
 
 // P2 backward over the levels lfrom .. lto of a part's reduced forest: deepest level first, one
@@ -452,8 +490,9 @@ __global__ void __launch_bounds__(384, 2)
 hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __restrict__ meta_g, const int4* __restrict__ runs_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
                       T* f0, T* f1, T* f2,
-                      int64_t n_total, T* xch_h, T* xch_x, int phase, unsigned long long* prof)
+                      int64_t n_total, T* xch_h, T* xch_x, int ctl, unsigned long long* prof)
 {
+    const int phase = ctl & 3;
     extern __shared__ __align__(128) unsigned char smem[];
     namespace cg = cooperative_groups;
     typedef typename Vec2<T>::type V2;
@@ -465,15 +504,22 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     constexpr uint32_t W = (uint32_t)sizeof(T);
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
     unsigned rank = 0;
-    if (CL) { rank = cg::this_cluster().block_rank(); cluster_arrive(); }     // barrier 0: every block of the cluster is running
+    if (CL) rank = cg::this_cluster().block_rank();
     // One 512-byte record per block, in launch order: the part's header and its first runs side by side, so that a
     // single dependent global load stands between the block's start and its bulk copies.
     uint64_t* bar = reinterpret_cast<uint64_t*>(smem);
     const PartHeader& H = *reinterpret_cast<const PartHeader*>(smem + 16);
     const int4* myruns = reinterpret_cast<const int4*>(smem + 16 + sizeof(PartHeader));
     if (tid < 32) reinterpret_cast<int4*>(smem + 16)[tid] = reinterpret_cast<const int4*>(recs + blockIdx.x)[tid];
-    if (tid == 0) mbar_init(bar, 1);
+    if (tid < 4) {
+        // the record of the block that will take this one's place on the SM (ctl >> 8 blocks later in the launch), into
+        // L2: its one dependent global load then costs an L2 hit instead of a DRAM round trip
+        const unsigned nb = blockIdx.x + (unsigned)(ctl >> 8);
+        if (nb < gridDim.x) asm volatile("prefetch.global.L2 [%0];" ::"l"(reinterpret_cast<const char*>(recs + nb) + 128 * tid));
+    }
+    if (tid == 0) { mbar_init(bar, 1); if (CL) mbar_init(bar + 1, 1); }
     __syncthreads();
+    if (CL) cluster_arrive_relaxed();                       // barrier 0: this block runs and its exchange mbarrier is initialised
     if (!CL && (phase == kPhaseA || phase == kPhaseB)) pdl_launch_dependents();
     const int L = H.L, NN = (H.nnode + 1 + E - 1) / E * E;    // one all-zero record behind the last node
     T* nd = reinterpret_cast<T*>(smem + 16 + sizeof(BlockRecord));
@@ -487,6 +533,8 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     const int nseg_lanes = H.nseg_lanes, nrun = H.nrun;
 
     if (tid == 0) {
+        // what the other blocks of the cluster will send: two values per ghost child (rank 0), one x per exported root
+        if (CL) mbar_expect_tx(bar + 1, rank == 0 ? (uint32_t)H.nghost * 2u * W : (uint32_t)H.nexp * W);
         mbar_expect_tx(bar, (uint32_t)NARR * (uint32_t)H.tx_elems * W + (uint32_t)H.meta_len * 4u);
         tma_load_1d(meta, meta_g + H.meta_off, (uint32_t)H.meta_len * 4u, bar);
     }
@@ -689,7 +737,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // ---- hand-off values of the sub-trees held by other blocks, into the ghost children; then
     //      the top nodes (the ancestors of the ghost children) ----
     if (CL) {
-        if (rank == 0) { cluster_wait(); cluster_arrive(); cluster_wait(); }   // barrier 1: the other ranks have swept and exported
+        if (rank == 0) { cluster_wait(); mbar_wait_cluster(bar + 1, 0); }      // every ghost child has its hand-off
     } else if (phase == kPhaseB) {
         pdl_wait();                                         // phase A has completed: the hand-off values are there
         for (int e = tid; e < nghost; e += nthreads) {
@@ -700,28 +748,26 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     }
     sweep_backward<T, MODE>(nd_sa, lb_sa, kp_sa, H.ntoplev - 1, 0, 1, H.maxwidth, tid, nthreads);
     HINES_STAMP(3);
-    // ---- exchange: exported roots hand their value up and get their parent's x back ----
+    // ---- exchange: an exported root {node, ghost parent, ghost child in part 0 / exchange slot, -} hands its value
+    //      up.  Cluster: a store into rank 0's shared memory that counts its bytes on rank 0's mbarrier (data and
+    //      signal in one message, no cluster-wide barrier, no fence).  The ghost parent becomes the identity
+    //      (g, c) = (1, 0) for the rounds below. ----
+    const bool sub = MODE != kModeFactor && (CL ? rank != 0 : phase == kPhaseC);       // a part that waits for its parents' x
     if (CL) {
         if (rank != 0) {
-            T* nd0 = cg::this_cluster().map_shared_rank(nd, 0);
-            cluster_wait();                                 // barrier 0: rank 0 is running
+            const uint32_t bar0 = mapa_u32(smem_u32(bar + 1), 0), nd0a = mapa_u32(nd_sa, 0);
+            cluster_wait();                                 // barrier 0: rank 0 is running, its mbarrier initialised
             for (int e = tid; e < nexp; e += nthreads) {
                 const int4 q = ex[e];
-                *reinterpret_cast<V2*>(nd0 + 6 * q.y + 4) = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
+                const V2 hv = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
+                st_async_2(nd0a + (6u * (uint32_t)q.z + 4u) * W, hv.x, hv.y, bar0);
+                nd[6 * q.y] = T(1); nd[6 * q.y + 1] = T(0);
             }
-            cluster_arrive(); cluster_wait();               // barrier 1
-            cluster_arrive(); cluster_wait();               // barrier 2: rank 0 has finished its forward sweep
-            for (int e = tid; e < nexp; e += nthreads) {
-                const int4 q = ex[e];
-                nd[6 * q.w] = T(0); nd[6 * q.w + 1] = nd0[6 * q.z + 1];
-            }
-            cluster_arrive();                               // barrier 3: this block no longer reads rank 0's memory
-            __syncthreads();
         }
     } else if (phase == kPhaseA) {
         for (int e = tid; e < nexp; e += nthreads) {
             const int4 q = ex[e];
-            reinterpret_cast<V2*>(xch_h)[H.xch_base + q.y] = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
+            reinterpret_cast<V2*>(xch_h)[H.xch_base + q.z] = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
         }
         if (MODE != kModeFactor && prof && tid == 0) {
             unsigned long long* o = prof + 8 * (size_t)blockIdx.x;
@@ -731,23 +777,28 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
         if (MODE != kModeFactor) return;
     } else if (phase == kPhaseC) {
-        pdl_wait();                                         // phase B has completed: the parents' x is there
-        for (int e = tid; e < nexp; e += nthreads) {
-            const int4 q = ex[e];
-            nd[6 * q.w] = T(0); nd[6 * q.w + 1] = xch_x[H.xch_base + q.y];
-        }
-        __syncthreads();
+        for (int e = tid; e < nexp; e += nthreads) { const int4 q = ex[e]; nd[6 * q.y] = T(1); nd[6 * q.y + 1] = T(0); }
     }
     // ---- P2 forward: first the top nodes, level by level (the other parts of the cell wait
     //      for their x), then everything by pointer jumping over the reduced forest.
-    // x_v = c_v + g_v x_p(v), g = -f, g = 0 at a root, at a finished node and at a ghost parent (c = the imported x).
+    // x_v = c_v + g_v x_p(v), g = -f, g = 0 at a root and at a finished node.
     // One round replaces (g_v, c_v, p(v)) by (g_v g_p, c_v + g_v c_p, p(p(v))): after `rounds` rounds (2^rounds > the
-    // longest path to such a node) every g is 0 and c is x.  All nodes work in every round, with one barrier per
-    // round instead of one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
+    // longest path) every g is 0 and c is x.  All nodes work in every round, with one barrier per round instead of
+    // one per level.  Buffers: record slots {0,1} and {2,3}; parent ids in {4,5}.
+    // A part that waits for its parents' x does its rounds WHILE it waits: its ghost parents are fixed points with the
+    // identity map, so after `rounds` rounds every node holds x_v = c_v + g_v x(its ghost parent); when x has arrived the
+    // ghost parents become (0, x) and one more round finishes.
     if (MODE == kModeFactor) rounds = 0;
     else sweep_forward_top<T>(nd_sa, lb_sa, kp_sa, H.ntoplev, H.maxwidth, tid, nthreads);
     if (CL) {
-        if (rank == 0) { cluster_arrive(); cluster_wait(); cluster_arrive(); }   // barrier 2: x of the top nodes is there (slot 1); barrier 3 below
+        if (rank == 0 && MODE != kModeFactor) {             // x of the top nodes goes to the roots that wait for it
+            const uint32_t bar1 = smem_u32(bar + 1), base = smem_u32(smem);
+            for (int e = tid; e < nghost; e += nthreads) {
+                const int4 g = gh[e];                       // {ghost child, -, parent, rank << 20 | landing word in that block}
+                const uint32_t r = (uint32_t)g.w >> 20, word = (uint32_t)g.w & 0xfffffu;
+                st_async_1(mapa_u32(base + 4u * word, r), nd[6 * g.z + 1], mapa_u32(bar1, r));
+            }
+        }
     } else if (phase == kPhaseB && MODE != kModeFactor) {
         for (int e = tid; e < nghost; e += nthreads) {
             const int4 g = gh[e];
@@ -755,7 +806,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
     }
     const int4* kp = reinterpret_cast<const int4*>(meta + H.kp_off);
-    for (int r = 0; r < rounds; ++r) {
+    auto jump_round = [&](int r) {
         const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
         for (int v = tid; v < nnode; v += nthreads) {
             int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
@@ -768,6 +819,21 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             ip[r & 1] = pp;
         }
         __syncthreads();
+    };
+    if (sub) __syncthreads();                               // the ghost parents' identity records
+    for (int r = 0; r < rounds; ++r) jump_round(r);
+    if (sub) {
+        if (CL) mbar_wait_cluster(bar + 1, 0);              // rank 0 has sent every x this part waits for (behind the export's entry)
+        else pdl_wait();                                    // phase B has completed: the parents' x is in the exchange buffer
+        const int cur = 2 * (rounds & 1);
+        for (int e = tid; e < nexp; e += nthreads) {
+            const int4 q = ex[e];
+            nd[6 * q.y + cur] = T(0);
+            nd[6 * q.y + cur + 1] = CL ? *reinterpret_cast<const T*>(&ex[e].z) : xch_x[H.xch_base + q.z];
+        }
+        __syncthreads();
+        jump_round(rounds);
+        ++rounds;
     }
     const int xs = 2 * (rounds & 1) + 1;                  // record slot that holds x after the forward sweep
     HINES_STAMP(4);
@@ -871,7 +937,6 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         for (int k = 0; k < 7; ++k) o[k] = stamp[k];
         o[7] = ((unsigned long long)smid() << 32) | (unsigned)H.n;
     }
-    if (CL) cluster_wait();                     // barrier 3: rank 0's shared memory stays alive while the others read it
 #undef HINES_STAMP
 }
 
@@ -1133,7 +1198,10 @@ static hines_status_t launch_all(hines_plan* P, const T* d, const T* u, const T*
             attr[0].val.programmaticStreamSerializationAllowed = 1;
             cfg.numAttrs = 1;
         }
-        CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, cl > 1 ? 0 : phase, prof));
+        // ctl = phase | (blocks resident on the device at a time << 8): how far ahead a block prefetches a record
+        const int per_sm = std::max(1, (int)(233472 / (cfg.dynamicSmemBytes + 1024)));
+        const int ctl = (cl > 1 ? 0 : phase) | ((D->num_sms * per_sm) << 8);
+        CUDA_TRY(cudaLaunchKernelEx(&cfg, kern, recs, mg_, rg_, d, u, b, x, f0, f1, f2, n_, xh, xx, ctl, prof));
         return HINES_OK;
     };
     // Size classes are independent: the first runs on the caller's stream, the others on side streams forked

@@ -314,7 +314,7 @@ def solve_with_tables(plan, m, d, u, b):
         for s in ps[1:]:
             s.condense(); s.backward(0); s.backward(1)
             assert not s.p.top.any() and not s.p.chains
-            for v, gx, p0, gp in s.p.exps:
+            for v, gp, gx, p0 in s.p.exps:                      # {node, ghost parent, ghost child / exchange slot, parent in part 0}
                 if kind[it] == 1:
                     ghost = int(gx)
                 else:                                            # split item: through exchange slot gx
@@ -334,12 +334,28 @@ def solve_with_tables(plan, m, d, u, b):
         xtop = ps[0].rec[:, 1].copy()                    # what the other parts read: x of the top nodes
         x0 = ps[0].forward()
         ps[0].expand(x0, x, E)
-        for s in ps[1:]:
-            for v, gx, p0, gp in s.p.exps:
+        landed = [dict() for _ in ps]
+        if kind[it] == 1:
+            # cluster item: rank 0 SENDS the parent's x into the block of the part that waits for it, behind the export's
+            # entry: the ghost child's entry names {rank << 20 | 4-byte word from the start of that block's shared memory}
+            w = 8 if E == 2 else 4
+            for gc, _, p0, dest in ps[0].p.ghosts:
+                r, word = int(dest) >> 20, int(dest) & 0xfffff
+                assert 1 <= r < len(ps)
+                h = ps[r].p.h
+                NN = -(-(h["nnode"] + 1) // E) * E
+                rel = word - (16 + 512 + 6 * w * NN) // 4 - h["exp_off"]
+                assert rel >= 0 and rel % 4 == 2 and rel // 4 < h["nexp"] and rel // 4 not in landed[r]
+                landed[r][rel // 4] = xtop[int(p0)]
+        for r, s in enumerate(ps):
+            if r == 0:
+                continue
+            for e, (v, gp, gx, p0) in enumerate(s.p.exps):
                 if kind[it] != 1:
                     p0 = int([g[2] for g in ps[0].p.ghosts if g[1] == gx][0])
+                    landed[r][e] = xtop[p0]
                 assert gp >= s.p.h["nlevnode"] and s.p.pnode[v] == gp
-                assert xtop[p0] == x0[p0]
-                s.rec[gp, 0], s.rec[gp, 1] = 0.0, xtop[p0]
+                assert xtop[p0] == x0[p0] and landed[r][e] == xtop[p0]
+                s.rec[gp, 0], s.rec[gp, 1] = 0.0, landed[r][e]
             s.expand(s.forward(), x, E)
     return x

@@ -213,10 +213,13 @@ def _check_policy(m, plan, max_segment=0):
                     else:                                      # an exported sub-tree root
                         assert k == 0 and r > 0 and prev[0] == 0
                         e = exports[(r, node)]
-                        assert tnode == e[3] >= p.h["nlevnode"] and p.pnode[node] == e[3]
-                        gl = [g for g in ps[0].ghosts if g[1] == e[1]] if kind[it] == 2 else [g for g in ps[0].ghosts if g[0] == e[1]]
+                        assert tnode == e[1] >= p.h["nlevnode"] and p.pnode[node] == e[1]
+                        gl = [g for g in ps[0].ghosts if g[1] == e[2]] if kind[it] == 2 else [g for g in ps[0].ghosts if g[0] == e[2]]
                         assert len(gl) == 1 and gl[0][2] == prev[1] and ps[0].ghost[gl[0][0]]
                         assert int(gl[0][0]) in ps[0].children(prev[1], w)
+                        # cluster items: the ghost child's entry names where rank 0 sends the parent's x (checked word by
+                        # word in plan_interpreter.solve_with_tables); split items go through the exchange buffer
+                        assert (int(gl[0][3]) >> 20) == (r if kind[it] == 1 else 0) and (kind[it] == 1 or gl[0][3] == 0)
                         n_exp_seen += 1
                     prev = (r, node)
                     pos += plen
