@@ -519,40 +519,63 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
             // The lanes of a shared-memory wavefront (fp64: lanes 0-15 = quarters 0, 1 and lanes 16-31 = quarters 2, 3;
             // fp32: all 32) should start on distinct bank residues: a quarter boundary may move by up to two nodes and a
             // lane may start up to 15 steps late (its residue moves with the delay), within the group's step count.
+            // First fit, lane by lane; a lane that finds no free residue may push the owner of one of its candidate
+            // residues to another free one (a later start of that lane), then take its place.
             const int NBq = w == 8 ? 16 : 32;
-            char used[2][32];
-            std::memset(used, 0, sizeof(used));
+            int owner[2][32];                                              // residue -> lane (k + 8 j) that starts on it, per wavefront
+            for (int h = 0; h < 2; ++h) for (int r = 0; r < 32; ++r) owner[h][r] = -1;
             const int32_t head_m = quads[(size_t)gq * 8].m;
             const int32_t cap = (head_m - 3 + 3) / 4 + 2;                  // steps of the group: the head's longest quarter + 2
-            int32_t mx = 0;
-            for (int32_t k = 0; k < 8 && (size_t)(gq * 8 + k) < quads.size(); ++k) {
+            int32_t mqs[8][4], aqs[8][4], dqs[8][4];
+            int32_t nk = 0;
+            auto half_of = [&](int j) { return w == 8 ? j / 2 : 0; };
+            auto residue = [&](int32_t a, int32_t dl) { return ((a - dl) % NBq + NBq) % NBq; };
+            for (int32_t k = 0; k < 8 && (size_t)(gq * 8 + k) < quads.size(); ++k, ++nk) {
                 const SegTmp& sg = quads[(size_t)gq * 8 + k];
-                int32_t mq[4], aq[4], dq[4] = {0, 0, 0, 0};
-                for (int32_t j = 0; j < 4; ++j) mq[j] = (sg.m - 3) / 4 + (j < (sg.m - 3) % 4 ? 1 : 0);
+                int32_t* mq = mqs[k]; int32_t* aq = aqs[k]; int32_t* dq = dqs[k];
+                for (int32_t j = 0; j < 4; ++j) { mq[j] = (sg.m - 3) / 4 + (j < (sg.m - 3) % 4 ? 1 : 0); dq[j] = 0; }
                 aq[0] = sg.a;
                 for (int32_t j = 0; j < 4; ++j) {
                     if (j > 0) aq[j] = aq[j - 1] + mq[j - 1] + 1;
-                    char* U = used[w == 8 ? j / 2 : 0];
+                    int* O = owner[half_of(j)];
                     static const int kShift[5] = {0, 1, -1, 2, -2};
                     bool done = false;
+                    for (int pass = 0; pass < 2 && !done; ++pass)          // pass 1: with one displacement
                     for (int cost = 0; cost <= 17 && !done; ++cost)
                         for (int t = 0; t < 5 && !done; ++t) {
                             const int sh = j > 0 ? kShift[t] : 0, dl = cost - std::abs(sh);
                             if (dl < 0 || dl > 15 || (j == 0 && t > 0)) continue;
                             if (j > 0 && (mq[j - 1] + sh < 1 || mq[j] - sh < 1 || mq[j - 1] + sh + dq[j - 1] > cap)) continue;
                             if (mq[j] - sh + dl > cap) continue;
-                            const int res = ((aq[j] + sh - dl) % NBq + NBq) % NBq;
-                            if (U[res]) continue;
-                            U[res] = 1; done = true;
+                            const int res = residue(aq[j] + sh, dl);
+                            if (O[res] >= 0) {
+                                if (pass == 0) continue;
+                                // the owner moves to a free residue by starting later, if its steps allow
+                                const int ok_ = O[res] & 7, oj = O[res] >> 3;
+                                int32_t olen = mqs[ok_][oj];
+                                if (ok_ == k && oj == j - 1) olen += sh;   // its length changes with this boundary
+                                bool moved = false;
+                                for (int32_t od = 0; od <= 15 && olen + od <= cap && !moved; ++od) {
+                                    const int r2 = residue(aqs[ok_][oj], od);
+                                    if (O[r2] >= 0 || r2 == res) continue;
+                                    O[r2] = O[res]; dqs[ok_][oj] = od; moved = true;
+                                }
+                                if (!moved) continue;
+                            }
+                            O[res] = k + 8 * j; done = true;
                             if (j > 0) { mq[j - 1] += sh; aq[j] += sh; mq[j] -= sh; }
                             dq[j] = dl;
                         }
                 }
+            }
+            int32_t mx = 0;
+            for (int32_t k = 0; k < nk; ++k) {
+                const SegTmp& sg = quads[(size_t)gq * 8 + k];
                 for (int32_t j = 0; j < 4; ++j) {
                     int32_t* Lq = G + 4 * (k + 8 * j);
-                    Lq[0] = aq[j]; Lq[1] = (int32_t)((uint32_t)mq[j] | ((uint32_t)j << 12) | (3u << 24) | (1u << 26) | ((uint32_t)dq[j] << 27));
+                    Lq[0] = aqs[k][j]; Lq[1] = (int32_t)((uint32_t)mqs[k][j] | ((uint32_t)j << 12) | (3u << 24) | (1u << 26) | ((uint32_t)dqs[k][j] << 27));
                     Lq[2] = sg.node; Lq[3] = j == 0 ? sg.tnode : -1;
-                    mx = std::max(mx, mq[j] + dq[j]);
+                    mx = std::max(mx, mqs[k][j] + dqs[k][j]);
                 }
             }
             out.padded_steps += 32 * (int64_t)(mx + 3);

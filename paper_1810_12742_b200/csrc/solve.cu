@@ -343,70 +343,6 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
     }
 }
 
-// P2 forward over the top nodes only, level by level from the root: x_v = c_v + g_v x_parent.
-// The other parts of the cell wait for exactly these values; everything below the top nodes follows by pointer
-// jumping afterwards.  A finished node holds {g, c} = {0, x}.
-template <typename T>
-__device__ __forceinline__ void sweep_forward_top(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int ntoplev, int maxwidth,
-                                                  int tid, int nthreads)
-{
-    typedef typename Vec2<T>::type V2;
-    constexpr uint32_t W = (uint32_t)sizeof(T), RS = 6u * W;
-    if (ntoplev <= 0) return;
-    if (maxwidth <= nthreads) {                             // one node per thread and level at most: see sweep_backward
-        const int pthreads = (maxwidth + 31) & ~31;
-        tid = nthreads - 1 - tid;                           // the LAST warps of the block sweep: P1 / P3 fill the first ones
-        if (tid < pthreads) {
-            int lo = ldsi1(lb_sa), hi = ldsi1(lb_sa + 4u), hi_n = ldsi1(lb_sa + 8u);
-            int v = lo + tid;
-            uint32_t qa = nd_sa + (uint32_t)v * RS, pa = qa + W;
-            V2 gc; gc.x = T(0); gc.y = T(0);
-            bool have = false;
-            if (v < hi) {
-                const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
-                gc = lds2<T>(qa); pa = nd_sa + (uint32_t)k.w * RS + W;
-                have = k.z >= 0 && ((k.z >> 29) & 1);
-            }
-#pragma unroll 1
-            for (int l = 0; l < ntoplev; ++l) {
-                const int hi_nn = l + 2 < ntoplev ? ldsi1(lb_sa + 4u * (uint32_t)(l + 3)) : 0;
-                if (have) {
-                    const T xp = lds1<T>(pa);               // a root reads its own c: g = 0 there
-                    V2 o; o.x = T(0); o.y = fmad<T>(gc.x, xp, gc.y);
-                    sts2<T>(qa, o);
-                }
-                lo = hi; hi = hi_n; hi_n = hi_nn;
-                v = lo + tid;
-                qa = nd_sa + (uint32_t)v * RS;
-                have = false;
-                if (l + 1 < ntoplev && v < hi) {
-                    const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
-                    gc = lds2<T>(qa); pa = nd_sa + (uint32_t)k.w * RS + W;
-                    have = k.z >= 0 && ((k.z >> 29) & 1);
-                }
-                named_barrier(pthreads);
-            }
-        }
-        __syncthreads();
-        return;
-    }
-#pragma unroll 1
-    for (int l = 0; l < ntoplev; ++l) {
-        const int hi = ldsi1(lb_sa + 4u * (uint32_t)(l + 1));
-        for (int v = ldsi1(lb_sa + 4u * (uint32_t)l) + tid; v < hi; v += nthreads) {
-            const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
-            if (k.z >= 0 && ((k.z >> 29) & 1)) {
-                const uint32_t qa = nd_sa + (uint32_t)v * RS;
-                const V2 gc = lds2<T>(qa);
-                const T xp = lds1<T>(nd_sa + (uint32_t)k.w * RS + W);
-                V2 o; o.x = T(0); o.y = fmad<T>(gc.x, xp, gc.y);
-                sts2<T>(qa, o);
-            }
-        }
-        __syncthreads();
-    }
-}
-
 // Unbranched cables (the degenerate single-branch case): the reduced system of a cable is tridiagonal, one row per
 // segment, and is solved inside ONE warp by parallel cyclic reduction: lane i holds row i = {a, b, c, d} (couplings
 // to rows i-1 and i+1, pivot, right-hand side); a step with stride s eliminates the couplings to i-s and i+s
@@ -789,22 +725,6 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // identity map, so after `rounds` rounds every node holds x_v = c_v + g_v x(its ghost parent); when x has arrived the
     // ghost parents become (0, x) and one more round finishes.
     if (MODE == kModeFactor) rounds = 0;
-    else sweep_forward_top<T>(nd_sa, lb_sa, kp_sa, H.ntoplev, H.maxwidth, tid, nthreads);
-    if (CL) {
-        if (rank == 0 && MODE != kModeFactor) {             // x of the top nodes goes to the roots that wait for it
-            const uint32_t bar1 = smem_u32(bar + 1), base = smem_u32(smem);
-            for (int e = tid; e < nghost; e += nthreads) {
-                const int4 g = gh[e];                       // {ghost child, -, parent, rank << 20 | landing word in that block}
-                const uint32_t r = (uint32_t)g.w >> 20, word = (uint32_t)g.w & 0xfffffu;
-                st_async_1(mapa_u32(base + 4u * word, r), nd[6 * g.z + 1], mapa_u32(bar1, r));
-            }
-        }
-    } else if (phase == kPhaseB && MODE != kModeFactor) {
-        for (int e = tid; e < nghost; e += nthreads) {
-            const int4 g = gh[e];
-            xch_x[H.xch_base + g.y] = nd[6 * g.z + 1];
-        }
-    }
     const int4* kp = reinterpret_cast<const int4*>(meta + H.kp_off);
     auto jump_round = [&](int r) {
         const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
@@ -822,6 +742,22 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     };
     if (sub) __syncthreads();                               // the ghost parents' identity records
     for (int r = 0; r < rounds; ++r) jump_round(r);
+    const int xs_now = 2 * (rounds & 1) + 1;              // record slot that holds x now
+    if (CL) {
+        if (rank == 0 && MODE != kModeFactor) {             // x of the top nodes goes to the roots that wait for it
+            const uint32_t bar1 = smem_u32(bar + 1), base = smem_u32(smem);
+            for (int e = tid; e < nghost; e += nthreads) {
+                const int4 g = gh[e];                       // {ghost child, -, parent, rank << 20 | landing word in that block}
+                const uint32_t r = (uint32_t)g.w >> 20, word = (uint32_t)g.w & 0xfffffu;
+                st_async_1(mapa_u32(base + 4u * word, r), nd[6 * g.z + xs_now], mapa_u32(bar1, r));
+            }
+        }
+    } else if (phase == kPhaseB && MODE != kModeFactor) {
+        for (int e = tid; e < nghost; e += nthreads) {
+            const int4 g = gh[e];
+            xch_x[H.xch_base + g.y] = nd[6 * g.z + xs_now];
+        }
+    }
     if (sub) {
         if (CL) mbar_wait_cluster(bar + 1, 0);              // rank 0 has sent every x this part waits for (behind the export's entry)
         else pdl_wait();                                    // phase B has completed: the parents' x is in the exchange buffer

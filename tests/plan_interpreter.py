@@ -99,7 +99,8 @@ def segments(sg):
                     assert int(Ls[j][0]) == pos and Ls[j][2] == Ls[0][2] and (j == 0 or Ls[j][3] == -1)
                     lens.append(w & 0xfff)
                     pos += lens[-1] + 1
-                assert max(lens) - min(lens) <= 5 and min(lens) >= 1
+                # a quarter boundary moves by at most two nodes: a quarter is within 4 of the balanced length
+                assert max(lens) - min(lens) <= 9 and min(lens) >= 1
                 yield int(Ls[0][0]), lens, int(Ls[0][2]), int(Ls[0][3])
         else:
             for a, mt, mb, hasq, node, tnode in pairs(sg[g:g + 32]):
