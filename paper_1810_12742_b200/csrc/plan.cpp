@@ -54,7 +54,7 @@ static const int kSlotNum[] = {1, 3, 2, 1, 1, 1, 1, 1};
 static const int kSlotDen[] = {1, 4, 3, 2, 3, 4, 6, 8};
 static const int kNumClassK = 8;
 static const int kRegsPerThread = 80;           // the resident kernel is built for __launch_bounds__(384, 2): up to 85
-static const int kMaxThreads = 384;
+static const int kMaxThreads = 768;
 static const int kMaxClusterClass = 16;
 static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descriptor word 1, bits 24-25)
 

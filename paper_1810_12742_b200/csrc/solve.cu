@@ -283,6 +283,31 @@ __device__ __forceinline__ void node_step(uint32_t nd_sa, uint32_t qa, const int
     }
 }
 
+// A level wider than the block (rare: a part with more nodes on one level than the block has threads): every thread loops
+// over the level's nodes.  Out of line: code that hardly ever runs should not sit between the phases of the kernel
+// (its instructions would take room in the instruction cache's lines).
+template <typename T, int MODE>
+__device__ __noinline__ void sweep_backward_wide(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int lfrom, int lto,
+                                                 int topsel, int tid, int nthreads)
+{
+    typedef typename Vec2<T>::type V2;
+    constexpr uint32_t W = (uint32_t)sizeof(T), RS = 6u * W;
+#pragma unroll 1
+    for (int l = lfrom; l >= lto; --l) {
+        const int hi = ldsi1(lb_sa + 4u * (uint32_t)(l + 1));
+        for (int v = ldsi1(lb_sa + 4u * (uint32_t)l) + tid; v < hi; v += nthreads) {
+            const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
+            if (k.z >= 0 && ((k.z >> 29) & 1) == topsel) {
+                const uint32_t qa = nd_sa + (uint32_t)v * RS;
+                const V2 a0 = lds2<T>(qa), a2 = lds2<T>(qa + 4u * W);
+                const T Un = lds1<T>(qa + 2u * W);
+                node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
+            }
+        }
+        __syncthreads();
+    }
+}
+
 template <typename T, int MODE>
 __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, uint32_t kp_sa, int lfrom, int lto,
                                                int topsel, int maxwidth, int tid, int nthreads)
@@ -326,21 +351,7 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
         __syncthreads();
         return;
     }
-    // a level wider than the block: every thread loops over the level's nodes
-#pragma unroll 1
-    for (int l = lfrom; l >= lto; --l) {
-        const int hi = ldsi1(lb_sa + 4u * (uint32_t)(l + 1));
-        for (int v = ldsi1(lb_sa + 4u * (uint32_t)l) + tid; v < hi; v += nthreads) {
-            const int4 k = ldsi4(kp_sa + 16u * (uint32_t)v);
-            if (k.z >= 0 && ((k.z >> 29) & 1) == topsel) {
-                const uint32_t qa = nd_sa + (uint32_t)v * RS;
-                const V2 a0 = lds2<T>(qa), a2 = lds2<T>(qa + 4u * W);
-                const T Un = lds1<T>(qa + 2u * W);
-                node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
-            }
-        }
-        __syncthreads();
-    }
+    sweep_backward_wide<T, MODE>(nd_sa, lb_sa, kp_sa, lfrom, lto, topsel, tid, nthreads);
 }
 
 // Unbranched cables (the degenerate single-branch case): the reduced system of a cable is tridiagonal, one row per
@@ -422,7 +433,7 @@ enum { kModeSolve = 0, kModeFactor = 1, kModeRhs = 2 };
 
 // QUAD: the class has four-lane segment groups (long segments); classes without them run the leaner instantiation.
 template <typename T, bool CL, int MODE, bool QUAD>
-__global__ void __launch_bounds__(384, 2)
+__global__ void __launch_bounds__(768, 1)
 hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __restrict__ meta_g, const int4* __restrict__ runs_g,
                       const T* __restrict__ d, const T* __restrict__ u, const T* __restrict__ b, T* x,
                       T* f0, T* f1, T* f2,
@@ -596,6 +607,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             }                                                                                        \
             ++sl;
             int sl = -dl;
+#pragma unroll 1
             for (int s = 0; s < mmax; s += 2) {
                 HINES_P1_STEP(un, dn, bn, un2, dn2, bn2)
                 HINES_P1_STEP(un2, dn2, bn2, un, dn, bn)
@@ -666,10 +678,9 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         // ---- unbranched cables: the reduced chains by parallel cyclic reduction, one warp per cable ----
         solve_cables_pcr<T>(nd, meta, H.nlev, tid, nthreads);
         __syncthreads();
-    } else {
-        // ---- P2 backward: what does not wait for another part, deepest level first ----
-        sweep_backward<T, MODE>(nd_sa, lb_sa, kp_sa, H.nlev - 1, H.lowlev, 0, H.maxwidth, tid, nthreads);
     }
+    // ---- P2 backward: what does not wait for another part, deepest level first ----
+    if (!cables) sweep_backward<T, MODE>(nd_sa, lb_sa, kp_sa, H.nlev - 1, H.lowlev, 0, H.maxwidth, tid, nthreads);
     // ---- hand-off values of the sub-trees held by other blocks, into the ghost children; then
     //      the top nodes (the ancestors of the ghost children) ----
     if (CL) {
@@ -726,8 +737,24 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // ghost parents become (0, x) and one more round finishes.
     if (MODE == kModeFactor) rounds = 0;
     const int4* kp = reinterpret_cast<const int4*>(meta + H.kp_off);
-    auto jump_round = [&](int r) {
+    if (sub) __syncthreads();                               // the ghost parents' identity records
+    const int nrounds = rounds;
+    if (sub) ++rounds;                                      // the round after x has arrived
+#pragma unroll 1
+    for (int r = 0; r < rounds; ++r) {
+        if (sub && r == nrounds) {
+            if (CL) mbar_wait_cluster(bar + 1, 0);          // rank 0 has sent every x this part waits for (behind the export's entry)
+            else pdl_wait();                                // phase B has completed: the parents' x is in the exchange buffer
+            const int cur = 2 * (r & 1);
+            for (int e = tid; e < nexp; e += nthreads) {
+                const int4 q = ex[e];
+                nd[6 * q.y + cur] = T(0);
+                nd[6 * q.y + cur + 1] = CL ? *reinterpret_cast<const T*>(&ex[e].z) : xch_x[H.xch_base + q.z];
+            }
+            __syncthreads();
+        }
         const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
+#pragma unroll 1
         for (int v = tid; v < nnode; v += nthreads) {
             int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
             const int p = r == 0 ? kp[v].w : ip[(r - 1) & 1];
@@ -739,9 +766,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             ip[r & 1] = pp;
         }
         __syncthreads();
-    };
-    if (sub) __syncthreads();                               // the ghost parents' identity records
-    for (int r = 0; r < rounds; ++r) jump_round(r);
+    }
     const int xs_now = 2 * (rounds & 1) + 1;              // record slot that holds x now
     if (CL) {
         if (rank == 0 && MODE != kModeFactor) {             // x of the top nodes goes to the roots that wait for it
@@ -757,19 +782,6 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             const int4 g = gh[e];
             xch_x[H.xch_base + g.y] = nd[6 * g.z + xs_now];
         }
-    }
-    if (sub) {
-        if (CL) mbar_wait_cluster(bar + 1, 0);              // rank 0 has sent every x this part waits for (behind the export's entry)
-        else pdl_wait();                                    // phase B has completed: the parents' x is in the exchange buffer
-        const int cur = 2 * (rounds & 1);
-        for (int e = tid; e < nexp; e += nthreads) {
-            const int4 q = ex[e];
-            nd[6 * q.y + cur] = T(0);
-            nd[6 * q.y + cur + 1] = CL ? *reinterpret_cast<const T*>(&ex[e].z) : xch_x[H.xch_base + q.z];
-        }
-        __syncthreads();
-        jump_round(rounds);
-        ++rounds;
     }
     const int xs = 2 * (rounds & 1) + 1;                  // record slot that holds x after the forward sweep
     HINES_STAMP(4);
@@ -835,6 +847,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
         T g1 = T(0), h1 = T(0), c1 = T(0);
         if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
+#pragma unroll 2
         for (int jj = mmax - 1; jj >= 0; --jj) {
             const int j = jj - dl;                          // the lane's own step: the same residue shift as in P1
             if ((unsigned)j < (unsigned)m) {
