@@ -445,8 +445,10 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     typedef typename Vec2<T>::type V2;
     // phase clocks (debug hook, prof == nullptr in normal runs): thread 0 stamps %globaltimer
     unsigned long long stamp[7];
-#define HINES_STAMP(k) do { if (prof && threadIdx.x == 0) stamp[k] = globaltimer_ns(); } while (0)
-    HINES_STAMP(0);
+    // A stamp behind a barrier must not be taken before the barrier has completed (BAR.SYNC.DEFER_BLOCKING lets independent
+    // instructions behind it issue while the warp still waits): the timer read is made to depend on a shared-memory load.
+#define HINES_STAMP(k) do { if (prof && threadIdx.x == 0) { if (ldsi1(smem_u32(smem) + 16 + 28) != (int)0x80000001) stamp[k] = globaltimer_ns(); } } while (0)
+    if (prof && threadIdx.x == 0) stamp[0] = globaltimer_ns();
     constexpr int E = 16 / (int)sizeof(T);
     constexpr uint32_t W = (uint32_t)sizeof(T);
     const int tid = threadIdx.x, lane = tid & 31, nthreads = blockDim.x;
