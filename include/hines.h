@@ -273,6 +273,33 @@ hines_status_t hines_solve_rhs(hines_plan_t* plan, const void* b, void* x, hines
 hines_status_t hines_solve_host(hines_plan_t* plan, const void* d, const void* u, const void* b, void* x,
                                 hines_stream_t stream);
 
+/*
+ * The one entry point that allocates NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Every other solve entry needs an uploaded plan, and the upload
+ * allocates.  This one needs no plan: the topology comes as DEVICE arrays, and the kernel's scratch (the working
+ * diagonal of the backward sweep, one value per unknown: what the streaming path keeps in the plan's workspace) is a
+ * file-scope static __device__ array of HINES_STATIC_SCRATCH_BYTES inside the library, held by every GPU that loads the
+ * library until the process exits.  It calls no cudaMalloc / cudaFree / allocating library routine and only enqueues on
+ * `stream`.  The arithmetic is Listing 2 of the paper cell by cell, one thread per cell: a fallback,
+ * several times slower than hines_solve -- not the path bench.py measures.
+ *   parent        DEVICE int32[n], cell-local as for hines_plan_create (parent[first of cell] = -1, 0 <= parent[i] < i).
+ *                 NOT validated (that would need a copy to the host): an entry outside [0, i) is treated as "no parent";
+ *                 nothing is ever read or written outside [0, n).
+ *   cell_offsets  DEVICE int64[ncells + 1], cell_offsets[0] = 0, increasing, cell_offsets[ncells] = n
+ *   d, u, b       DEVICE, n elements of `dtype` (HINES_F64 / HINES_F32), natural order, read only
+ *   x             DEVICE, n elements; may be exactly b, must not overlap it otherwise
+ * Limit: n * sizeof(dtype) <= HINES_STATIC_SCRATCH_BYTES (1,048,576 unknowns in fp64, 2,097,152 in fp32); beyond it
+ * UNSUPPORTED with a message naming the limit.  Other errors: INVALID_ARG (null, bad dtype, sizes, overlap), CUDA.
+ * The scratch array is shared by every call on a device and keeps the last call's contents; nothing in it has to
+ * start at zero (every cell's entries are written before they are read).  Two calls that overlap in time on the same
+ * GPU (different streams, or two host threads) RACE on it: serialise them.  The first call on a device looks the
+ * array's address up (cudaGetSymbolAddress): make that call outside stream capture.
+ */
+#define HINES_STATIC_SCRATCH_BYTES 8388608
+hines_status_t hines_solve_static(const int32_t* parent, const int64_t* cell_offsets, int64_t ncells, int64_t n,
+                                  const void* d, const void* u, const void* b, void* x, int32_t dtype,
+                                  hines_stream_t stream);
+
 hines_status_t hines_plan_destroy(hines_plan_t* plan);
 
 /*

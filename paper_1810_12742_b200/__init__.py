@@ -51,7 +51,7 @@ TABLES = {
 }
 
 # every symbol include/hines.h declares
-ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host",
+ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host", "hines_solve_static",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
                "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
@@ -104,6 +104,7 @@ def load_library(build_if_missing: bool = True):
     lib.hines_partition_cells.argtypes = [vp, i64, i32, vp, vp]
     lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.hines_solve_static.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp]
     lib.hines_factor.argtypes = [vp, vp, vp, vp]
     lib.hines_solve_rhs.argtypes = [vp, vp, vp, vp]
     lib.hines_plan_destroy.argtypes = [vp]
@@ -252,6 +253,22 @@ def partition_cells(cell_offsets, nparts: int):
     cost = np.empty(nparts, np.int64)
     _check(load_library().hines_partition_cells(offs.ctypes.data, len(offs) - 1, int(nparts), part.ctypes.data, cost.ctypes.data))
     return part, cost
+
+
+STATIC_SCRATCH_BYTES = 8388608
+
+
+def solve_static(parent, cell_offsets, d, u, b, x, dtype=F64, stream=None):
+    """hines_solve_static: the entry point that allocates nothing (no plan; scratch in a static __device__ array of
+    STATIC_SCRATCH_BYTES inside the library).  parent (int32, cell-local) and cell_offsets (int64) are DEVICE arrays like
+    d, u, b, x (torch CUDA tensors or raw addresses); ncells and n come from cell_offsets' / d's lengths."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    ncells, n = int(cell_offsets.numel()) - 1, int(d.numel())
+    _check(load_library().hines_solve_static(_ptr(parent), _ptr(cell_offsets), ncells, n, _ptr(d), _ptr(u), _ptr(b), _ptr(x),
+                                             int(dtype), stream))
+    return x
 
 
 def version() -> str:
