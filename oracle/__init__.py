@@ -173,6 +173,30 @@ def level_mean_split(parent, cell_offsets):
     return offs, pl[order].copy(), pv[order].copy(), stat
 
 
+def reroot(parent, cell_offsets):
+    """f2, tree re-rooting (readings R1-R3): per cell the compartment that minimises the depth of the
+    tree becomes the root and the compartments are renumbered branch by branch, breadth first.  Returns a dict:
+    root[ncells] (old cell-local index), depth_before / depth_after[ncells], perm[N] (GLOBAL: new -> old), new_parent[N]
+    (cell-local), usrc[N] (GLOBAL old index whose u holds the coupling of the new compartment's edge to its parent)."""
+    parent, offs, _ = _prep(parent, cell_offsets)
+    nc, n = len(offs) - 1, int(offs[-1])
+    root = np.empty(nc, np.int32); db = np.empty(nc, np.int32); da = np.empty(nc, np.int32)
+    perm = np.empty(n, np.int64); newp = np.empty(n, np.int32); usrc = np.empty(n, np.int64)
+    fn = lib().oracle_reroot_cell
+    fn.restype = C.c_int32
+    for c in range(nc):
+        lo, hi = int(offs[c]), int(offs[c + 1])
+        m = hi - lo
+        pc = np.ascontiguousarray(parent[lo:hi], np.int32)
+        pm = np.empty(m, np.int32); npar = np.empty(m, np.int32); us = np.empty(m, np.int32)
+        r, d0 = C.c_int32(0), C.c_int32(0)
+        dep = fn(C.c_int32(m), _p(pc, C.c_int32), C.byref(r), C.byref(d0), _p(pm, C.c_int32), _p(npar, C.c_int32), _p(us, C.c_int32))
+        assert dep >= 0
+        root[c], db[c], da[c] = r.value, d0.value, dep
+        perm[lo:hi] = pm.astype(np.int64) + lo; newp[lo:hi] = npar; usrc[lo:hi] = us.astype(np.int64) + lo
+    return dict(root=root, depth_before=db, depth_after=da, perm=perm, new_parent=newp, usrc=usrc)
+
+
 def hines_factor(parent, cell_offsets, d, u):
     """f3: the part of Listing 2 that touches only d and u.  Returns (dw, f): pivots and multipliers."""
     parent, offs, nc = _prep(parent, cell_offsets)

@@ -9,7 +9,7 @@ import os
 import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-SOURCES = ["hines_oracle.c", "tables_oracle.c", "split_oracle.c"]
+SOURCES = ["hines_oracle.c", "tables_oracle.c", "split_oracle.c", "reroot_oracle.c"]
 LIB = os.path.join(HERE, "libhines_oracle.so")
 CFLAGS = ["-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off", "-fno-fast-math",
           "-Wall", "-Wextra"]
