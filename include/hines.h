@@ -316,6 +316,39 @@ hines_status_t hines_plan_destroy(hines_plan_t* plan);
 hines_status_t hines_partition_cells(const int64_t* cell_offsets, int64_t ncells, int32_t nparts,
                                      int32_t* cell_part, int64_t* part_cost);
 
+/*
+ * f2, tree re-rooting (section 6): "Balance the dependency tree so that the depth of the tree is
+ * minimized ... find a new root node that minimizes the depth of the tree and permute all unknowns such that they form
+ * a new Hines matrix based on the new root node ... numbering all branches breadth first and then sorting all
+ * compartments by branch index and distance to the root."  Host, setup time, O(N); allocates host memory only.
+ * Per cell: the compartment with the smallest largest distance to any other compartment becomes the root (of two such
+ * compartments the one with the larger index, reading R2); the branches of the re-rooted tree are numbered
+ * breadth first (children of a branch in ascending old index of their first compartment, R3) and the compartments
+ * renumbered by (branch, distance to the root).  Cell sizes do not change: cell_offsets serves the new numbering too.
+ *   parent, cell_offsets   HOST, as for hines_plan_create
+ *   new_parent   HOST int32[N] out, cell-local, new numbering: feed it to hines_plan_create
+ *   perm         HOST int64[N] out, GLOBAL: perm[new] = old compartment
+ *   u_src        HOST int64[N] out, GLOBAL: old compartment whose u holds the coupling of `new` to new_parent[new]
+ *                (edges on the path from the new root to the old one change direction; u_src[root] = perm[root])
+ *   root, depth_before, depth_after   HOST int32[ncells] out, may be NULL: old cell-local index of the new root; the
+ *                largest distance (compartments) from the root before and after
+ * The re-rooted system is d'[k] = d[perm[k]], b'[k] = b[perm[k]], u'[k] = u[u_src[k]] -- a symmetric permutation of the
+ * same matrix -- and its solution is x'[k] = x[perm[k]].  A caller that assembles its matrix in the new numbering pays
+ * nothing per step; one that cannot uses hines_gather / hines_scatter below around the solve.
+ * Errors: INVALID_ARG (null, ncells <= 0), BAD_TOPOLOGY (as hines_plan_create), ALLOC.
+ */
+hines_status_t hines_reroot(const int32_t* parent, const int64_t* cell_offsets, int64_t ncells,
+                            int32_t* new_parent, int64_t* perm, int64_t* u_src, int32_t* root,
+                            int32_t* depth_before, int32_t* depth_after);
+
+/*
+ * The permutation carried through load and store (f2): dst[k] = src[index[k]] (gather) and dst[index[k]] = src[k]
+ * (scatter), k < n, elements of `dtype`; all pointers DEVICE, index int64, dst must not overlap src; only enqueue on
+ * `stream`.  Bytes per element: 2w + 8.  Errors: INVALID_ARG (null, n < 0, bad dtype), CUDA.
+ */
+hines_status_t hines_gather(void* dst, const void* src, const int64_t* index, int64_t n, int32_t dtype, hines_stream_t stream);
+hines_status_t hines_scatter(void* dst, const void* src, const int64_t* index, int64_t n, int32_t dtype, hines_stream_t stream);
+
 /* Introspection: needed for the bit-exact table parity tests and for reporting. */
 hines_status_t hines_plan_get_info(const hines_plan_t* plan, hines_plan_info_t* out);
 

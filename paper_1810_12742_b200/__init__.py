@@ -51,7 +51,7 @@ TABLES = {
 }
 
 # every symbol include/hines.h declares
-ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host", "hines_solve_static",
+ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_reroot", "hines_gather", "hines_scatter", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host", "hines_solve_static",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
                "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
@@ -102,6 +102,9 @@ def load_library(build_if_missing: bool = True):
     lib.hines_plan_create.argtypes = [vp, vp, i64, i32, C.POINTER(Options), C.POINTER(vp)]
     lib.hines_plan_upload.argtypes = [vp]
     lib.hines_partition_cells.argtypes = [vp, i64, i32, vp, vp]
+    lib.hines_reroot.argtypes = [vp, vp, i64, vp, vp, vp, vp, vp, vp]
+    lib.hines_gather.argtypes = [vp, vp, vp, i64, i32, vp]
+    lib.hines_scatter.argtypes = [vp, vp, vp, i64, i32, vp]
     lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_static.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp]
@@ -253,6 +256,39 @@ def partition_cells(cell_offsets, nparts: int):
     cost = np.empty(nparts, np.int64)
     _check(load_library().hines_partition_cells(offs.ctypes.data, len(offs) - 1, int(nparts), part.ctypes.data, cost.ctypes.data))
     return part, cost
+
+
+def reroot(parent, cell_offsets):
+    """hines_reroot (f2): per cell the root that minimises the tree's depth and the breadth-first
+    renumbering.  Returns a dict: new_parent int32[N] (cell-local), perm int64[N] (new -> old, global), u_src int64[N],
+    root / depth_before / depth_after int32[ncells]."""
+    par = np.ascontiguousarray(parent, dtype=np.int32)
+    offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
+    n, nc = len(par), len(offs) - 1
+    out = dict(new_parent=np.empty(n, np.int32), perm=np.empty(n, np.int64), u_src=np.empty(n, np.int64),
+               root=np.empty(nc, np.int32), depth_before=np.empty(nc, np.int32), depth_after=np.empty(nc, np.int32))
+    _check(load_library().hines_reroot(par.ctypes.data, offs.ctypes.data, nc, out["new_parent"].ctypes.data,
+                                       out["perm"].ctypes.data, out["u_src"].ctypes.data, out["root"].ctypes.data,
+                                       out["depth_before"].ctypes.data, out["depth_after"].ctypes.data))
+    return out
+
+
+def gather(dst, src, index, dtype=F64, stream=None):
+    """hines_gather: dst[k] = src[index[k]] on the device (index: int64 CUDA tensor)."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(load_library().hines_gather(_ptr(dst), _ptr(src), _ptr(index), int(index.numel()), int(dtype), stream))
+    return dst
+
+
+def scatter(dst, src, index, dtype=F64, stream=None):
+    """hines_scatter: dst[index[k]] = src[k] on the device."""
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    _check(load_library().hines_scatter(_ptr(dst), _ptr(src), _ptr(index), int(index.numel()), int(dtype), stream))
+    return dst
 
 
 STATIC_SCRATCH_BYTES = 8388608

@@ -60,3 +60,31 @@ def dfs_renumber(p):
     inv = np.empty(n, np.int64); inv[perm] = np.arange(n)
     p_new = np.array([-1] + [inv[p[perm[k]]] for k in range(1, n)], np.int32)
     return perm, p_new
+
+
+def rooted_at(parent, offs, pick):
+    """The same cells (same undirected trees) rooted elsewhere: cell c is re-rooted at its compartment pick(c, n) and
+    renumbered in breadth-first order from there, so that parent[i] < i holds again.  Returns (parent', perm, usrc) with
+    perm[new] = old (global) and usrc[new] = the old compartment holding the coupling of new's edge to its parent --
+    test-side construction of badly rooted inputs for the re-rooting pass (f2); shares nothing with oracle/ or the library."""
+    parent = np.asarray(parent, np.int32); offs = np.asarray(offs, np.int64)
+    newp = np.empty_like(parent); perm = np.empty(len(parent), np.int64); usrc = np.empty(len(parent), np.int64)
+    for c in range(len(offs) - 1):
+        lo, hi = int(offs[c]), int(offs[c + 1])
+        n = hi - lo
+        adj = [[] for _ in range(n)]
+        for i in range(1, n):
+            adj[i].append(int(parent[lo + i])); adj[int(parent[lo + i])].append(i)
+        r = int(pick(c, n))
+        order, par_old, seen = [r], {r: -1}, {r}
+        for v in order:
+            for w in sorted(adj[v]):
+                if w not in seen:
+                    seen.add(w); par_old[w] = v; order.append(w)
+        new_of = {v: k for k, v in enumerate(order)}
+        for k, v in enumerate(order):
+            q = par_old[v]
+            perm[lo + k] = lo + v
+            newp[lo + k] = -1 if q < 0 else new_of[q]
+            usrc[lo + k] = lo + (v if q < 0 or parent[lo + v] == q else q)
+    return newp, perm, usrc

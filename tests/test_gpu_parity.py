@@ -324,3 +324,43 @@ def test_factored_full_size(cfg):
     d, u, _ = mg.system(m)
     err, info = _check_factored(m, d, u, steps=(0, 999) if cfg == 4 else (1,))
     print(f"cfg{cfg} factored: n={m.n} max rel err {err:.3e} split_cells={info.n_split_cells} cluster_cells={info.n_cluster_cells}")
+
+
+# ---- f2, tree re-rooting: badly rooted cells solved as given and after hines_reroot, the permutation
+#      carried through load and store by hines_gather / hines_scatter; both against the oracle on the cells as given ----
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+def test_rerooted_cells_through_gather_and_scatter(dtype):
+    import torch
+    import paper_1810_12742_b200 as hb
+    from helpers import rooted_at
+    hd = hb.F64 if dtype == np.float64 else hb.F32
+    m0 = mg.make_config(2, 0.004)
+    d0, u0, b0 = mg.system(m0)
+    # the same cells rooted at a leaf (their last compartment): the badly balanced input
+    parent, perm0, usrc0 = rooted_at(m0.parent, m0.cell_offsets, lambda c, n: n - 1)
+    d, u, b = d0[perm0], u0[usrc0], b0[perm0]
+    dr, ur, br = (np.ascontiguousarray(a, dtype).astype(np.float64) for a in (d, u, b))
+    xr = oracle.hines_solve(parent, m0.cell_offsets, dr, ur, br)
+    rr = hb.reroot(parent, m0.cell_offsets)
+    assert (rr["depth_after"] < rr["depth_before"]).all()
+    dd, du, db = (torch.from_numpy(np.ascontiguousarray(a, dtype)).cuda() for a in (d, u, b))
+    perm, usrc = torch.from_numpy(rr["perm"]).cuda(), torch.from_numpy(rr["u_src"]).cuda()
+    d2, u2, b2 = torch.full_like(dd, float("nan")), torch.full_like(dd, float("nan")), torch.full_like(dd, float("nan"))
+    hb.gather(d2, dd, perm, hd); hb.gather(u2, du, usrc, hd); hb.gather(b2, db, perm, hd)
+    torch.cuda.synchronize()
+    assert torch.equal(d2, dd[perm]) and torch.equal(u2, du[usrc]) and torch.equal(b2, db[perm])      # bit-exact index work
+    before, after = hb.Plan(parent, m0.cell_offsets, dtype=hd), hb.Plan(rr["new_parent"], m0.cell_offsets, dtype=hd)
+    try:
+        assert after.info.max_levels < before.info.max_levels
+        x_given = torch.full_like(dd, float("nan"))
+        before.solve(dd, du, db, x_given)
+        x2, x = torch.full_like(dd, float("nan")), torch.full_like(dd, float("nan"))
+        after.solve(d2, u2, b2, x2)
+        hb.scatter(x, x2, perm, hd)
+        torch.cuda.synchronize()
+        for xs in (x_given, x):
+            xs = xs.cpu().numpy().astype(np.float64)
+            assert np.isfinite(xs).all()
+            assert oracle.rel_err(m0.cell_offsets, xs, xr).max() <= TOL[dtype]
+    finally:
+        before.close(); after.close()

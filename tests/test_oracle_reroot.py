@@ -1,5 +1,5 @@
-"""Pins of the re-rooting oracle (oracle/reroot_oracle.c; readings R1-R3 of DESIGN.md) and, below,
-the library's hines_reroot against it, bit for bit.  CPU only."""
+"""Pins of the re-rooting oracle (oracle/reroot_oracle.c; readings R1-R3 of DESIGN.md) and, below
+them, the library's hines_reroot against the oracle, bit for bit.  CPU only."""
 import json
 import os
 
@@ -122,3 +122,65 @@ def test_rerooted_system_has_the_permuted_solution():
     x2 = oracle.hines_solve(r["new_parent"], offs, d[r["perm"]], u[r["usrc"]], b[r["perm"]])
     assert np.abs(x2 - x[r["perm"]]).max() <= 1e-12 * np.abs(x).max()
     _check_invariants(parent, offs, r)
+
+
+# ---- the library's hines_reroot (csrc/reroot.cpp: centre of the tree by two breadth-first searches) against the oracle
+#      (every compartment tried as the root), bit for bit --------------------------------------------------------------
+def _lib_vs_oracle(parent, offs):
+    import paper_1810_12742_b200 as hb
+    r, o = hb.reroot(parent, offs), oracle.reroot(parent, offs)
+    for a, b in (("root", "root"), ("depth_before", "depth_before"), ("depth_after", "depth_after"), ("perm", "perm"),
+                 ("new_parent", "new_parent"), ("u_src", "usrc")):
+        assert np.array_equal(r[a], o[b]), a
+    return r
+
+
+def test_library_matches_oracle_on_random_trees():
+    from helpers import rooted_at
+    rng = np.random.default_rng(3)
+    sizes = [1, 2, 3, 5, 8, 31, 32, 33, 100, 257]
+    offs = np.concatenate([[0], np.cumsum(sizes)]).astype(np.int64)
+    for trial in range(6):
+        parent = np.concatenate([random_parent(n, 50 * trial + k, float(rng.uniform(0.1, 0.97))) for k, n in enumerate(sizes)]).astype(np.int32)
+        _lib_vs_oracle(parent, offs)
+        leafy, _, _ = rooted_at(parent, offs, lambda c, n: n - 1)       # the last compartment is always a leaf
+        r = _lib_vs_oracle(leafy, offs)
+        assert (r["depth_after"] <= r["depth_before"]).all()
+        _check_invariants(leafy, offs, dict(r, usrc=r["u_src"]))
+
+
+@pytest.mark.parametrize("cfg,scale", [(0, 1.0), (2, 0.0008), (3, 0.0004), (1, 0.0003)])
+def test_library_matches_oracle_on_configs(cfg, scale):
+    """The synthetic configs as generated (grown from the root: the centre is at or near the root already) and re-rooted
+    at a leaf (the badly balanced case the paper has in mind)."""
+    import morphgen as mg
+    from helpers import rooted_at
+    m = mg.make_config(cfg, scale)
+    _lib_vs_oracle(m.parent, m.cell_offsets)
+    leafy, _, _ = rooted_at(m.parent, m.cell_offsets, lambda c, n: n - 1)
+    r = _lib_vs_oracle(leafy, m.cell_offsets)
+    # a leaf's largest distance lies between the radius and the diameter of its tree
+    assert ((r["depth_after"] <= r["depth_before"]) & (r["depth_before"] <= 2 * r["depth_after"])).all()
+    # the plan built on the re-rooted branching cells has no more levels than the one built on the cells as given
+    import paper_1810_12742_b200 as hb
+    before, after = hb.Plan(leafy, m.cell_offsets), hb.Plan(r["new_parent"], m.cell_offsets)
+    try:
+        if cfg == 1:       # an unbranched cable rooted at its end: the middle as root halves the depth (in compartments)
+            assert (r["depth_after"] == (r["depth_before"] + 1) // 2).all()      # ... and makes two branches of one
+            assert after.info.max_levels == 2 and before.info.max_levels == 1
+        else:
+            assert after.info.max_levels <= before.info.max_levels
+            if cfg == 2:
+                assert after.info.max_levels < before.info.max_levels
+    finally:
+        before.close(); after.close()
+
+
+def test_reroot_rejects_bad_input():
+    import paper_1810_12742_b200 as hb
+    with pytest.raises(hb.HinesError):
+        hb.reroot([-1, 0, 5], [0, 3])
+    with pytest.raises(hb.HinesError):
+        hb.reroot([0, 0, 1], [0, 3])
+    with pytest.raises(hb.HinesError):
+        hb.reroot([-1, 0, 1], [0, 3, 3])
