@@ -11,8 +11,9 @@ solve, forward substitution, store) over one batc
   value      whole-job unknowns/s with inputs resident in HBM: exactly K steps between two CUDA events on the
              launching stream, barrier + synchronize on both sides, max over ranks
   timing     the same in >= 20 intervals of >= 50 ms each: median and best ms per step
-  e2e        the same through hines_solve_host: pinned HOST buffers, H2D of d,u,b and D2H of x inside
-             the timed region every step
+  e2e        the same through hines_host_pipeline_solve: pinned HOST buffers, H2D of d,u,b and D2H of x inside
+             the timed region every step (slices of whole cells, copies and solves overlapped; the figure of the
+             one-call hines_solve_host beside it)
   roofline   HBM: algorithmic bytes (bytes_min = N*4w + 4*branches) / device time of the kernels of one
              step, against MEASURED_PEAKS.json hbm_gbs
   cpu_baseline  the oracle as it stands, timed on this box's host cores (rank 0, N=1 only)
@@ -263,10 +264,10 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     w = np.dtype(np_dtype).itemsize
     m, d, u, b, seed = workload(cfg, args.scale, rank, args.world, args.scaling)
     t0 = time.perf_counter()
-    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32,
-                   threads_per_block=args.threads, policy_flags=args.policy, group_smem_bytes=args.group_smem,
+    plan_kw = dict(threads_per_block=args.threads, policy_flags=args.policy, group_smem_bytes=args.group_smem,
                    smem_bytes_per_block=args.smem, max_segment=args.max_segment, chunk_smem_bytes=args.chunk_smem,
                    cluster_max=args.cluster_max, split_smem_bytes=args.split_smem)
+    plan = hb.Plan(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32, **plan_kw)
     plan.upload()
     plan_s = time.perf_counter() - t0
     info = plan.info
@@ -363,15 +364,31 @@ def measure(cfg, dtype, steps, warmup, rank, args, want_e2e, want_parity, barrie
     if want_e2e:
         hd, hu, hb_, hx = (torch.from_numpy(np.ascontiguousarray(a, np_dtype)).pin_memory() for a in (d, u, b, np.empty_like(b)))
         k_e2e = max(3, min(steps, int(np.ceil(3e9 / max(4 * m.n * w, 1)))))    # ~3 GB of traffic
-        for _ in range(2):
-            plan.solve_host(hd, hu, hb_, hx, stream)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(k_e2e):
-            plan.solve_host(hd, hu, hb_, hx, stream)
-        e2e_s = (time.perf_counter() - t0) / k_e2e
-        barrier()
-        e2e = {"s_per_step": e2e_s, "steps": k_e2e, "h2d": 3 * m.n * w, "d2h": m.n * w}
+
+        def timed(call):
+            for _ in range(2):
+                call()
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(k_e2e):
+                call()
+            dt = (time.perf_counter() - t0) / k_e2e
+            barrier()
+            return dt
+        # one call, the link busy in one direction at a time ...
+        single_s = timed(lambda: plan.solve_host(hd, hu, hb_, hx, stream))
+        x_single = hx.numpy().copy()
+        # ... and the pipelined entry: slices of whole cells, copy-in / solve / copy-out overlapped (the e2e figure)
+        pipe = hb.HostPipeline(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == "f64" else hb.F32, **plan_kw)
+        hx.fill_(float("nan"))
+        e2e_s = timed(lambda: pipe.solve(hd, hu, hb_, hx))
+        x_pipe = hx.numpy()
+        scale_ = np.abs(x_single).max()
+        e2e = {"s_per_step": e2e_s, "steps": k_e2e, "h2d": 3 * m.n * w, "d2h": m.n * w,
+               "entry": f"hines_host_pipeline_solve ({len(pipe.slices) - 1} slices)", "single_call_s_per_step": single_s,
+               "max_abs_diff_vs_single_call_over_max_abs_x": float(np.abs(x_pipe - x_single).max() / scale_)}
+        assert np.isfinite(x_pipe).all() and e2e["max_abs_diff_vs_single_call_over_max_abs_x"] < (1e-10 if w == 8 else 1e-4)
+        pipe.close()
         del hd, hu, hb_, hx
     out = {"m": m, "d": d, "u": u, "b": b, "info": info, "ms": ms, "res_ms": res_ms, "str_ms": str_ms,
            "parity": parity, "e2e": e2e, "plan_s": plan_s, "nsets": nsets, "launches": plan.launches_per_solve,
@@ -606,7 +623,10 @@ def main():
         "gpu_launches": r["launches"] * args.steps,
         "clocks": clocks,
         "e2e": None if e2e is None else {"value": tot_units / e2e_s, "unit": UNIT, "steps": e2e["steps"],
-                                         "h2d_bytes_per_step": e2e["h2d"] * world, "d2h_bytes_per_step": e2e["d2h"] * world},
+                                         "h2d_bytes_per_step": e2e["h2d"] * world, "d2h_bytes_per_step": e2e["d2h"] * world,
+                                         "entry": e2e["entry"],
+                                         "single_call_value_rank0": float(m.n) / e2e["single_call_s_per_step"],
+                                         "max_abs_diff_vs_single_call_over_max_abs_x": e2e["max_abs_diff_vs_single_call_over_max_abs_x"]},
         "roofline": roof,
         "cpu_baseline": cpu,
         "factored": factored,

@@ -274,6 +274,29 @@ hines_status_t hines_solve_host(hines_plan_t* plan, const void* d, const void* u
                                 hines_stream_t stream);
 
 /*
+ * Host buffers with the copies overlapped: the end-to-end entry bench.py times as "e2e".  hines_solve_host keeps the link
+ * busy in one direction at a time; at 32 bytes per unknown the link is the step.  Cells are independent:
+ * the pipeline cuts the batch into `nslices` slices of whole cells with about the same number of unknowns (0 = default
+ * 8; fewer if there are fewer cells), builds one plan per slice, and runs copy-in, solve and copy-out of successive
+ * slices on three streams, so that x of one slice goes back while d, u, b of the next ones come in (PCIe is full
+ * duplex).  Result: bit-identical to hines_solve with the same options on each slice's cells.
+ *   create   HOST parent / cell_offsets / options as for hines_plan_create; host-only work (no device needed)
+ *   solve    HOST d, u, b (read), x (written; may be b), N elements each; pinned memory makes the copies asynchronous,
+ *            pageable memory works (the runtime stages it).  Synchronous: x is complete on return.  The first call
+ *            uploads the plans and allocates 4 device arrays of N elements (+ 32 per slice).
+ *   slices   the slice boundaries: first_compartment[nslices + 1] (may be NULL to query the count)
+ * Errors: as hines_plan_create / hines_solve; INVALID_ARG (null, nslices < 0 or > 1024).
+ */
+typedef struct hines_host_pipeline hines_host_pipeline_t;
+hines_status_t hines_host_pipeline_create(const int32_t* parent, const int64_t* cell_offsets, int64_t ncells,
+                                          hines_dtype_t dtype, const hines_options_t* opt, int32_t nslices,
+                                          hines_host_pipeline_t** out);
+hines_status_t hines_host_pipeline_solve(hines_host_pipeline_t* pipe, const void* d, const void* u, const void* b, void* x);
+hines_status_t hines_host_pipeline_slices(const hines_host_pipeline_t* pipe, int32_t* nslices, int64_t* first_compartment,
+                                          int64_t capacity);
+hines_status_t hines_host_pipeline_destroy(hines_host_pipeline_t* pipe);
+
+/*
  * The one entry point that allocates NOTHING, for callers that cannot call cudaMalloc (code under CUDA graph capture,
  * tight serving loops, harnesses that forbid it).  Every other solve entry needs an uploaded plan, and the upload
  * allocates.  This one needs no plan: the topology comes as DEVICE arrays, and the kernel's scratch (the working

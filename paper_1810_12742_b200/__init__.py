@@ -52,6 +52,7 @@ TABLES = {
 
 # every symbol include/hines.h declares
 ABI_SYMBOLS = ["hines_plan_create", "hines_partition_cells", "hines_reroot", "hines_gather", "hines_scatter", "hines_factor", "hines_solve_rhs", "hines_plan_upload", "hines_solve", "hines_solve_host", "hines_solve_static",
+               "hines_host_pipeline_create", "hines_host_pipeline_solve", "hines_host_pipeline_slices", "hines_host_pipeline_destroy",
                "hines_plan_destroy", "hines_plan_get_info", "hines_plan_get_table",
                "hines_plan_launches_per_solve", "hines_plan_enable_timing", "hines_plan_get_timing",
                "hines_plan_enable_phase_clocks", "hines_plan_get_phase_clocks",
@@ -108,6 +109,10 @@ def load_library(build_if_missing: bool = True):
     lib.hines_solve.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_host.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.hines_solve_static.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, i32, vp]
+    lib.hines_host_pipeline_create.argtypes = [vp, vp, i64, i32, C.POINTER(Options), i32, C.POINTER(vp)]
+    lib.hines_host_pipeline_solve.argtypes = [vp, vp, vp, vp, vp]
+    lib.hines_host_pipeline_slices.argtypes = [vp, C.POINTER(i32), vp, i64]
+    lib.hines_host_pipeline_destroy.argtypes = [vp]
     lib.hines_factor.argtypes = [vp, vp, vp, vp]
     lib.hines_solve_rhs.argtypes = [vp, vp, vp, vp]
     lib.hines_plan_destroy.argtypes = [vp]
@@ -239,6 +244,52 @@ class Plan:
     def close(self):
         if self._h is not None:
             load_library().hines_plan_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class HostPipeline:
+    """hines_host_pipeline_*: host buffers in, host buffers out, the batch cut into slices of whole cells whose copy-in,
+    solve and copy-out overlap (the end-to-end entry; options as for Plan)."""
+
+    def __init__(self, parent, cell_offsets, dtype=F64, nslices=0, **options):
+        lib = load_library()
+        parent = np.ascontiguousarray(parent, dtype=np.int32)
+        offs = np.ascontiguousarray(cell_offsets, dtype=np.int64)
+        o = dict(threads_per_block=0, smem_bytes_per_block=0, policy_flags=0, stream_threads=0, group_smem_bytes=0,
+                 max_segment=0, cluster_max=0, chunk_smem_bytes=0, split_smem_bytes=0)
+        o.update(options)
+        opt = Options(C.sizeof(Options), *[o[k] for k in ("threads_per_block", "smem_bytes_per_block", "policy_flags",
+                                                           "stream_threads", "group_smem_bytes", "max_segment", "cluster_max",
+                                                           "chunk_smem_bytes", "split_smem_bytes")])
+        h = C.c_void_p()
+        self._h = None
+        _check(lib.hines_host_pipeline_create(parent.ctypes.data, offs.ctypes.data, len(offs) - 1, int(dtype), C.byref(opt),
+                                              int(nslices), C.byref(h)))
+        self._h = h
+        self.dtype = int(dtype)
+
+    def solve(self, d, u, b, x):
+        """HOST buffers (numpy arrays or pinned torch CPU tensors); synchronous."""
+        _check(load_library().hines_host_pipeline_solve(self._h, _ptr(d), _ptr(u), _ptr(b), _ptr(x)))
+        return x
+
+    @property
+    def slices(self) -> np.ndarray:
+        n = C.c_int32()
+        _check(load_library().hines_host_pipeline_slices(self._h, C.byref(n), None, 0))
+        out = np.empty(n.value + 1, np.int64)
+        _check(load_library().hines_host_pipeline_slices(self._h, C.byref(n), out.ctypes.data, len(out)))
+        return out
+
+    def close(self):
+        if self._h is not None:
+            load_library().hines_host_pipeline_destroy(self._h)
             self._h = None
 
     def __del__(self):

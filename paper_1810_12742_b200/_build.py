@@ -8,7 +8,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libhines_b200.so")
-SOURCES = ["plan.cpp", "reroot.cpp", "solve.cu", "static_solve.cu", "permute.cu"]
+SOURCES = ["plan.cpp", "reroot.cpp", "solve.cu", "static_solve.cu", "permute.cu", "host_pipeline.cu"]
 HEADERS = [os.path.join(CSRC, "plan_internal.h"), os.path.join(ROOT, "include", "hines.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -107,3 +107,25 @@ def test_reference_arm_prints_the_contract_line(capsys):
     assert line["impl"] == "reference" and line["unit"] == "unknowns/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert line["config"]["workload"].startswith("cfg0") and line["higher_is_better"] is True
+
+
+def test_host_pipeline_slices_tile_the_batch():
+    """hines_host_pipeline_create (host-only work): the slices are runs of whole cells, tile the batch, and are about
+    equal in unknowns when the cells are small against a slice."""
+    import morphgen as mg
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(3, 0.002)
+    for ns in (0, 1, 3, 8, 1000):
+        p = hb.HostPipeline(m.parent, m.cell_offsets, nslices=ns)
+        s = p.slices
+        p.close()
+        assert s[0] == 0 and s[-1] == m.n and (np.diff(s) > 0).all()
+        assert np.isin(s, m.cell_offsets).all()
+        assert len(s) - 1 <= min(ns or 8, m.ncells)
+    p = hb.HostPipeline(m.parent, m.cell_offsets, nslices=4)
+    sizes = np.diff(p.slices)
+    p.close()
+    biggest_cell = int(np.diff(m.cell_offsets).max())
+    assert len(sizes) == 4 and sizes.max() - sizes.min() <= 2 * biggest_cell
+    with pytest.raises(hb.HinesError):
+        hb.HostPipeline(m.parent, m.cell_offsets, nslices=-1)

@@ -364,3 +364,29 @@ def test_rerooted_cells_through_gather_and_scatter(dtype):
             assert oracle.rel_err(m0.cell_offsets, xs, xr).max() <= TOL[dtype]
     finally:
         before.close(); after.close()
+
+
+@pytest.mark.parametrize("dtype", [np.float64, np.float32])
+@pytest.mark.parametrize("pinned", [True, False])
+def test_host_pipeline_matches_oracle(dtype, pinned):
+    """hines_host_pipeline_solve: host buffers in and out, slices overlapped; twice in a row with a fresh right-hand side."""
+    import torch
+    import paper_1810_12742_b200 as hb
+    m = mg.make_config(3, 0.004)
+    d, u, _ = mg.coefficients(m, mg.rng.BASE_SEED)
+    pipe = hb.HostPipeline(m.parent, m.cell_offsets, dtype=hb.F64 if dtype == np.float64 else hb.F32, nslices=5)
+    try:
+        assert len(pipe.slices) == 6
+        for step in range(2):
+            b = mg.rhs(m, mg.rng.BASE_SEED, step)
+            bufs = [np.ascontiguousarray(a, dtype) for a in (d, u, b)] + [np.full(m.n, np.nan, dtype)]
+            if pinned:
+                bufs = [torch.from_numpy(a).pin_memory() for a in bufs]
+            pipe.solve(*bufs)
+            x = (bufs[3].numpy() if pinned else bufs[3]).astype(np.float64)
+            dr, ur, br = (np.ascontiguousarray(a, dtype).astype(np.float64) for a in (d, u, b))
+            xr = oracle.hines_solve(m.parent, m.cell_offsets, dr, ur, br)
+            assert np.isfinite(x).all()
+            assert oracle.rel_err(m.cell_offsets, x, xr).max() <= TOL[dtype]
+    finally:
+        pipe.close()
