@@ -72,12 +72,18 @@ enum {
     HINES_POLICY_NO_PDL       = 2048, /* split items: the three launches strictly one after the other (default: programmatic
                                         dependent launch, a phase starts while the one before it still runs)        */
     HINES_POLICY_NO_SPLIT     = 64,  /* no split items: a cell that fits no cluster goes to the streaming path  */
-    HINES_POLICY_SPLIT_LEVEL_MEAN = 128 /* f1: cut branches by the paper's own rule first (level by
+    HINES_POLICY_SPLIT_LEVEL_MEAN = 128, /* f1: cut branches by the paper's own rule first (level by
                                         level from the root, over all cells of the batch, a branch longer than
                                         c = ceil(mean length on the level) is cut into a head of c compartments and
                                         a rest that moves, with the branch's children, one level down); every piece is
                                         then still bounded by max_segment (set max_segment = 1023 for the paper's rule
                                         alone).  Tables HINES_TABLE_SPLIT_* hold the pieces with or without the flag  */
+    HINES_POLICY_SPLIT_BLOCK_MEAN = 4096 /* f4 ("Some intermediate packing of the matrices in a block can be used to
+                                        compute more local heuristics, like per block averages"): the same cutting rule, but
+                                        the mean of a level is taken over the cells of ONE block (work item) -- the cells
+                                        the packing, done on the uncut branches, has put together -- instead of the whole
+                                        batch.  HINES_TABLE_SPLIT_PIECE_* then hold these pieces (cells of the streaming path:
+                                        uncut), HINES_TABLE_SPLIT_LEVEL_STAT is empty.  Ignored with SPLIT_LEVEL_MEAN        */
 };
 
 typedef struct {

@@ -27,6 +27,7 @@ POLICY_NO_PCR = 256
 POLICY_FACTORED = 512
 POLICY_NO_QUADS = 1024
 POLICY_NO_PDL = 2048
+POLICY_SPLIT_BLOCK_MEAN = 4096
 ITEM_SINGLE, ITEM_CLUSTER, ITEM_SPLIT = 0, 1, 2
 
 STATUS = {0: "HINES_OK", 1: "HINES_ERR_INVALID_ARG", 2: "HINES_ERR_BAD_TOPOLOGY", 3: "HINES_ERR_ALLOC",

@@ -154,6 +154,8 @@ struct Br {
 };
 
 // Tables of one part (policies P3 + P4).
+using hines::SplitPiece;
+
 struct PartBuild {
     std::vector<int32_t> runs;               // 4 per run {item-local first compartment, length, staged index, 0}
     int32_t L = 0, n = 0, tx_elems = 0;
@@ -176,6 +178,7 @@ struct ItemBuild {
     int64_t total_bytes = 0;                 // estimate of the shared memory of the whole item, all parts together
     int32_t max_lanes = 0, max_lanes_top = 0;
     int32_t has_quads = 0;                   // some part has four-lane segment groups
+    std::vector<SplitPiece> split;           // f4 (block means): the pieces of the item's branches under ITS level means
 };
 
 // Pieces of a branch under the fixed-bound rule (P4), top-down: nseg = max(1, floor(len/S + 0.4)) pieces of
@@ -192,6 +195,7 @@ static void fixed_bound_pieces(int32_t len, int32_t smax, std::vector<int32_t>& 
 }
 
 struct NodeTmp { int32_t depth, pkey, gid, ghost; };
+static void split_cells(const hines_plan& P, const std::vector<int64_t>& cells, std::vector<SplitPiece>& out, std::vector<int64_t>* stat);
 
 // kind = single: the given cells (ascending, not necessarily adjacent) in one part.  kind = cluster: ONE cell in K parts, part 0 = top + sub-trees.
 // kind = split: ONE cell, part 0 = top alone, the sub-trees packed into parts of at most `slot` bytes (K is
@@ -201,6 +205,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
     const int32_t w = P.width, E = 16 / w;
     const int32_t smax = kind == kItemSingle ? P.seg_single : P.seg_cluster;
     const bool level_mean = (P.opt.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN) != 0;
+    const bool block_mean = !level_mean && (P.opt.policy_flags & HINES_POLICY_SPLIT_BLOCK_MEAN) != 0;
     const int32_t narr = (P.opt.policy_flags & HINES_POLICY_FACTORED) ? 4 : 3;     // staged arrays: d,u,b, or the three factors + b
     out = ItemBuild();
     out.kind = kind;
@@ -210,6 +215,22 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
     std::vector<Br> br(nb);
     std::vector<int32_t> pieces;
     pieces.reserve(nb + nb / 4);
+    // f4: the level means of THIS block's cells (the intermediate packing has chosen them); pieces by local branch
+    std::vector<int32_t> bm_off, bm_len;
+    if (block_mean) {
+        split_cells(P, cells, out.split, nullptr);
+        std::vector<int64_t> cb0;                                       // first global branch of each cell, and its local index
+        std::vector<int32_t> cl0;
+        int32_t acc = 0;
+        for (int64_t c : cells) { cb0.push_back(P.cell_branch_offsets[c]); cl0.push_back(acc); acc += (int32_t)(P.cell_branch_offsets[c + 1] - P.cell_branch_offsets[c]); }
+        auto local_of = [&](int64_t j) { const size_t k = (size_t)(std::upper_bound(cb0.begin(), cb0.end(), j) - cb0.begin()) - 1; return cl0[k] + (int32_t)(j - cb0[k]); };
+        bm_off.assign((size_t)nb + 1, 0);
+        for (const SplitPiece& sp : out.split) ++bm_off[(size_t)local_of(sp.j) + 1];
+        for (int32_t k = 0; k < nb; ++k) bm_off[(size_t)k + 1] += bm_off[(size_t)k];
+        bm_len.assign(out.split.size(), 0);
+        std::vector<int32_t> fill(bm_off.begin(), bm_off.end() - 1);
+        for (const SplitPiece& sp : out.split) bm_len[(size_t)fill[(size_t)local_of(sp.j)]++] = sp.len;      // top-down within a branch
+    }
     int32_t nn = 0, lb0 = 0;
     for (int64_t c : cells) {
         const int64_t b0 = P.cell_branch_offsets[c], b1 = P.cell_branch_offsets[c + 1];
@@ -226,6 +247,9 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
             if (level_mean) {                           // the paper's pieces first, each then bounded
                 for (int64_t q = P.split_piece_offsets[j]; q < P.split_piece_offsets[j + 1]; ++q)
                     fixed_bound_pieces(P.split_piece_len[q], smax, pieces);
+            } else if (block_mean) {
+                const int32_t lj = lb0 + (int32_t)(j - b0);
+                for (int32_t q = bm_off[(size_t)lj]; q < bm_off[(size_t)lj + 1]; ++q) fixed_bound_pieces(bm_len[(size_t)q], smax, pieces);
             } else {
                 fixed_bound_pieces(e.len, smax, pieces);
             }
@@ -703,52 +727,63 @@ static hines_status_t canonical_tables(hines_plan& P, const int32_t* parent)
 }
 
 // f1: the paper's branch splitting (reading F1).  Level by level from the root, over
-// ALL cells of the batch ("the average length of all dendritic branches on this level"): c = ceil(mean length of
+// ALL cells given ("the average length of all dendritic branches on this level"): c = ceil(mean length of
 // the pieces on the level); a piece longer than c is cut into a head of c compartments, which stays on the level,
 // and the rest, which becomes its only child on the next level ("two shorter branches that are attached to each
 // other") and takes the branch's children along ("causes all child branches to move one level down"); the rest
 // may be cut again there.  Integer arithmetic throughout: c = (sum + count - 1) / count.
-static void level_mean_split(hines_plan& P)
+// The cells are the whole batch (f1, HINES_POLICY_SPLIT_LEVEL_MEAN) or the cells of one block (f4, "more
+// local heuristics, like per block averages", HINES_POLICY_SPLIT_BLOCK_MEAN).
+static void split_cells(const hines_plan& P, const std::vector<int64_t>& cells, std::vector<SplitPiece>& out, std::vector<int64_t>* stat)
 {
-    const int64_t nbr = P.nbranches;
-    std::vector<int64_t> base(nbr);                               // first branch of the branch's cell
-    for (int64_t c = 0; c < P.ncells; ++c)
-        for (int64_t j = P.cell_branch_offsets[c]; j < P.cell_branch_offsets[c + 1]; ++j) base[j] = P.cell_branch_offsets[c];
-    struct It { int64_t j; int32_t rem; };
+    struct It { int64_t j, base; int32_t rem; };
     std::vector<It> cur, nxt;
-    struct Piece { int64_t j; int32_t len, level; };
-    std::vector<Piece> out;
-    out.reserve((size_t)nbr + (size_t)nbr / 2);
-    for (int64_t c = 0; c < P.ncells; ++c) cur.push_back({P.cell_branch_offsets[c], P.branch_len[P.cell_branch_offsets[c]]});
-    P.split_level_stat.clear();
+    out.clear();
+    for (int64_t c : cells) cur.push_back({P.cell_branch_offsets[c], P.cell_branch_offsets[c], P.branch_len[P.cell_branch_offsets[c]]});
+    if (stat) stat->clear();
     for (int32_t level = 0; !cur.empty(); ++level) {
         int64_t sum = 0;
         for (const It& it : cur) sum += it.rem;
         const int64_t cnt = (int64_t)cur.size();
         const int64_t cut = (sum + cnt - 1) / cnt;
-        P.split_level_stat.push_back(sum); P.split_level_stat.push_back(cnt);
+        if (stat) { stat->push_back(sum); stat->push_back(cnt); }
         nxt.clear();
         for (const It& it : cur) {
             if (it.rem > cut) {
                 out.push_back({it.j, (int32_t)cut, level});
-                nxt.push_back({it.j, (int32_t)(it.rem - cut)});
+                nxt.push_back({it.j, it.base, (int32_t)(it.rem - cut)});
             } else {
                 out.push_back({it.j, it.rem, level});
                 for (int64_t k = P.child_offsets[it.j]; k < P.child_offsets[it.j + 1]; ++k) {
-                    const int64_t ch = base[it.j] + P.child_ids[k];
-                    nxt.push_back({ch, P.branch_len[ch]});
+                    const int64_t ch = it.base + P.child_ids[k];
+                    nxt.push_back({ch, it.base, P.branch_len[ch]});
                 }
             }
         }
         cur.swap(nxt);
     }
+}
+
+// pieces (any order, the pieces of a branch top-down) -> the tables by branch
+static void store_split_tables(hines_plan& P, const std::vector<SplitPiece>& out)
+{
+    const int64_t nbr = P.nbranches;
     P.split_piece_offsets.assign(nbr + 1, 0);
-    for (const Piece& p : out) P.split_piece_offsets[p.j + 1]++;
+    for (const SplitPiece& p : out) P.split_piece_offsets[p.j + 1]++;
     for (int64_t j = 0; j < nbr; ++j) P.split_piece_offsets[j + 1] += P.split_piece_offsets[j];
     P.split_piece_len.assign(out.size(), 0);
     P.split_piece_level.assign(out.size(), 0);
     std::vector<int64_t> fill(P.split_piece_offsets.begin(), P.split_piece_offsets.end() - 1);
-    for (const Piece& p : out) { const int64_t q = fill[p.j]++; P.split_piece_len[q] = p.len; P.split_piece_level[q] = p.level; }
+    for (const SplitPiece& p : out) { const int64_t q = fill[p.j]++; P.split_piece_len[q] = p.len; P.split_piece_level[q] = p.level; }
+}
+
+static void level_mean_split(hines_plan& P)
+{
+    std::vector<int64_t> all((size_t)P.ncells);
+    std::iota(all.begin(), all.end(), (int64_t)0);
+    std::vector<SplitPiece> out;
+    split_cells(P, all, out, &P.split_level_stat);
+    store_split_tables(P, out);
 }
 
 static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const ItemBuild& ib)
@@ -758,6 +793,7 @@ static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const It
     P.item_cells.insert(P.item_cells.end(), cells.begin(), cells.end());
     P.item_cell_offsets.push_back((int64_t)P.item_cells.size());
     P.item_unknowns.push_back(ib.n);
+    P.block_split.insert(P.block_split.end(), ib.split.begin(), ib.split.end());
     P.item_class.push_back(0);                     // filled by assign_classes
     P.item_kind.push_back(ib.kind);
     P.item_xch.push_back((int32_t)P.n_xch);
@@ -1156,6 +1192,16 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
         std::vector<ItemNeed> item_need;
         std::vector<char> is_stream;
         pack_items(*P, item_need, is_stream);
+        if ((o.policy_flags & HINES_POLICY_SPLIT_BLOCK_MEAN) && !(o.policy_flags & HINES_POLICY_SPLIT_LEVEL_MEAN)) {
+            // f4: the tables now describe what the blocks were built from; cells of the streaming path are not split
+            for (int64_t c = 0; c < P->ncells; ++c)
+                if (is_stream[c])
+                    for (int64_t j = P->cell_branch_offsets[c]; j < P->cell_branch_offsets[c + 1]; ++j)
+                        P->block_split.push_back({j, P->branch_len[j], P->branch_level[j]});
+            store_split_tables(*P, P->block_split);
+            P->split_level_stat.clear();
+            std::vector<SplitPiece>().swap(P->block_split);
+        }
         assign_classes(*P, item_need);
         build_stream(*P, is_stream);
         *out_plan = holder.release();

@@ -75,6 +75,8 @@ struct StreamDesc {
     int32_t nchild;
 };
 
+struct SplitPiece { int64_t j; int32_t len, level; };       // a piece of global branch j under a splitting pass (f1 / f4)
+
 struct DeviceTables;      // solve.cu
 
 void set_error(const std::string& msg);
@@ -96,10 +98,12 @@ struct hines_plan {
     std::vector<int64_t> cell_branch_offsets, cell_level_offsets, child_offsets;
     std::vector<int32_t> branch_start, branch_len, branch_parent_comp, branch_parent_branch,
         branch_level, cell_nlevels, level_count, level_list, child_ids;
-    // f1: pieces of the level-mean splitting pass, filled when the policy is on
+    // f1: pieces of the level-mean splitting pass over the whole batch; with HINES_POLICY_SPLIT_BLOCK_MEAN (f4,
+    // PAPER.md:189) replaced after packing by the pieces under every block's own level means
     std::vector<int64_t> split_piece_offsets;          // [nbranches+1] into split_piece_len
     std::vector<int32_t> split_piece_len, split_piece_level;
     std::vector<int64_t> split_level_stat;             // per level of the split tree: {sum of the piece lengths, pieces}
+    std::vector<hines::SplitPiece> block_split;        // f4 (HINES_POLICY_SPLIT_BLOCK_MEAN): pieces under every block's own level means, item by item
     // policy tables
     std::vector<int32_t> cell_item, item_class, item_kind, item_launch_order, item_xch;
     std::vector<int64_t> item_cell_offsets, item_cells, item_unknowns, item_part_offsets;

@@ -11,7 +11,7 @@ template <typename T> static std::vector<T> rd(const std::string& f) { FILE* fp 
 int main(int argc, char** argv) {
     int ncase = atoi(argv[1]);
     struct O { int flags, seg, chunk, clmax, smem, split, dtype; };
-    O opts[] = {{0,0,0,0,0,0,0}, {0,0,0,0,0,0,1}, {2,0,0,0,0,0,0}, {128,0,0,0,0,0,0}, {512,0,0,0,0,0,0}, {0,7,30000,16,0,0,0}, {0,9,0,2,64000,12000,0}, {8,0,0,0,60000,0,0}, {1,0,0,0,0,0,0}, {256,3,0,0,0,0,1}, {4,0,0,0,0,0,0}, {64,0,20000,2,48000,20000,0}};
+    O opts[] = {{0,0,0,0,0,0,0}, {0,0,0,0,0,0,1}, {2,0,0,0,0,0,0}, {128,0,0,0,0,0,0}, {512,0,0,0,0,0,0}, {0,7,30000,16,0,0,0}, {0,9,0,2,64000,12000,0}, {8,0,0,0,60000,0,0}, {1,0,0,0,0,0,0}, {256,3,0,0,0,0,1}, {4,0,0,0,0,0,0}, {64,0,20000,2,48000,20000,0}, {4096,0,0,0,0,0,0}, {4096,0,20000,2,48000,20000,0}};
     long plans = 0;
     for (int k = 0; k < ncase; ++k) {
         auto par = rd<int32_t>(std::string(argv[2]) + "/p" + std::to_string(k) + ".bin"); auto offs = rd<int64_t>(std::string(argv[2]) + "/o" + std::to_string(k) + ".bin");

@@ -64,7 +64,8 @@ def test_small_configs_streaming_path(cfg, scale):
 @pytest.mark.parametrize("kw", [dict(policy_flags=2), dict(policy_flags=4), dict(smem_bytes_per_block=48 * 1024, policy_flags=8),
                                 dict(threads_per_block=64), dict(threads_per_block=384, group_smem_bytes=200 * 1024),
                                 dict(group_smem_bytes=8 * 1024, stream_threads=32),
-                                dict(policy_flags=128), dict(policy_flags=128, max_segment=1023), dict(policy_flags=256)])
+                                dict(policy_flags=128), dict(policy_flags=128, max_segment=1023), dict(policy_flags=256),
+                                dict(policy_flags=4096), dict(policy_flags=4096, max_segment=1023)])
 def test_policy_variants_mixed_paths(kw):
     """Several size classes, resident + streaming in one solve, different block sizes."""
     m = mg.make_config(2, 0.006)
@@ -288,7 +289,7 @@ def test_factored_small_configs(cfg, scale, dtype):
 
 @pytest.mark.parametrize("kw", [dict(chunk_smem_bytes=40 * 1024), dict(chunk_smem_bytes=24 * 1024, cluster_max=16, max_segment=9),
                                 dict(smem_bytes_per_block=80000, cluster_max=2, split_smem_bytes=26000),
-                                dict(policy_flags=2), dict(policy_flags=128)])
+                                dict(policy_flags=2), dict(policy_flags=128), dict(policy_flags=4096)])
 def test_factored_clusters_split_items_policies(kw):
     m = mg.make_config(2, 0.006)
     d, u, _ = mg.system(m)

@@ -106,3 +106,57 @@ def test_policy_level_mean_segments_follow_the_pieces():
     _check_interpreted(m, plan)
     plan = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_SPLIT_LEVEL_MEAN)     # pieces bounded by max_segment too
     _check_interpreted(m, plan)
+
+
+# ---- f4 ("more local heuristics, like per block averages"): the same rule with the level means taken over
+#      the cells of one block.  Oracle = oracle_level_mean_split applied to the cells of every work item on their own -----
+def _block_mean_pieces(m, plan):
+    """Per global branch the pieces the ORACLE gives when each item's cells are split as a batch of their own."""
+    t = oracle.tables(m.parent, m.cell_offsets)
+    item_cells, item_offs = plan.table("item_cells"), plan.table("item_cell_offsets")
+    want_len = [None] * len(t.branch_len)
+    want_lev = [None] * len(t.branch_len)
+    seen = np.zeros(m.ncells, bool)
+    for it in range(len(item_offs) - 1):
+        cells = item_cells[item_offs[it]:item_offs[it + 1]]
+        seen[cells] = True
+        par = np.concatenate([m.parent[m.cell_offsets[c]:m.cell_offsets[c + 1]] for c in cells])
+        offs = np.concatenate([[0], np.cumsum([m.cell_offsets[c + 1] - m.cell_offsets[c] for c in cells])]).astype(np.int64)
+        po, ln, lv, _ = oracle.level_mean_split(par, offs)
+        gbr = np.concatenate([np.arange(t.cell_branch_offsets[c], t.cell_branch_offsets[c + 1]) for c in cells])
+        for k, j in enumerate(gbr):
+            want_len[j], want_lev[j] = ln[po[k]:po[k + 1]], lv[po[k]:po[k + 1]]
+    for c in np.nonzero(~seen)[0]:                        # cells of the streaming path: uncut
+        for j in range(t.cell_branch_offsets[c], t.cell_branch_offsets[c + 1]):
+            want_len[j], want_lev[j] = np.array([t.branch_len[j]], np.int32), np.array([t.branch_level[j]], np.int32)
+    return want_len, want_lev
+
+
+@pytest.mark.parametrize("cfg,scale,kw", [(0, 1.0, {}), (3, 0.004, {}), (2, 0.004, {}), (3, 0.004, dict(group_smem_bytes=20000)),
+                                          (2, 0.002, dict(smem_bytes_per_block=48000, cluster_max=2, split_smem_bytes=20000)),
+                                          (1, 0.004, {})])
+def test_policy_block_mean_tables_bit_exact_and_solve(cfg, scale, kw):
+    from test_plan_tables import _check_interpreted
+    m = mg.make_config(cfg, scale)
+    plan = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_SPLIT_BLOCK_MEAN, **kw)
+    want_len, want_lev = _block_mean_pieces(m, plan)
+    po, ln, lv = plan.table("split_piece_offsets"), plan.table("split_piece_len"), plan.table("split_piece_level")
+    assert len(po) == len(want_len) + 1 and len(plan.table("split_level_stat")) == 0
+    for j in range(len(want_len)):
+        assert np.array_equal(ln[po[j]:po[j + 1]], want_len[j]) and np.array_equal(lv[po[j]:po[j + 1]], want_lev[j]), j
+    _check_interpreted(m, plan)                            # the segments follow these pieces and the tables solve the systems
+    # a block's own means differ from the batch's (unless all cells are alike): the heterogeneous config must show it
+    if cfg == 3 and not kw:
+        glob = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_SPLIT_LEVEL_MEAN)
+        assert not np.array_equal(glob.table("split_piece_len"), ln)
+
+
+def test_block_mean_of_one_block_is_the_level_mean():
+    """Closed form: when the whole batch is one block, block means = batch means."""
+    m = mg.make_config(0, 0.25)                            # 16 cells of 75 unknowns: one group
+    a = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_SPLIT_BLOCK_MEAN)
+    b = hb.Plan(m.parent, m.cell_offsets, policy_flags=hb.POLICY_SPLIT_LEVEL_MEAN)
+    assert a.info.n_resident_items == 1 and b.info.n_resident_items == 1
+    for name in ("split_piece_offsets", "split_piece_len", "split_piece_level"):
+        assert np.array_equal(a.table(name), b.table(name))
+    assert np.array_equal(a.table("part_meta"), b.table("part_meta"))

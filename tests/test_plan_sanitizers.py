@@ -1,6 +1,6 @@
 """The setup-time scheduler (csrc/plan.cpp: ~1,100 lines of index arithmetic) under AddressSanitizer,
 UndefinedBehaviorSanitizer and LeakSanitizer: plans for all five configs, a 70-sibling star, odd offsets and a
-20,000-compartment root branch with a fork, under twelve option sets (fp32, no grouping, level-mean splitting,
+20,000-compartment root branch with a fork, under fourteen option sets (fp32, no grouping, level-mean and block-mean splitting,
 factored, small segments / chunks / clusters, split items, streaming, no cable path).  Host only, no GPU needed."""
 import os
 import shutil
@@ -40,4 +40,4 @@ def test_plan_create_under_asan_ubsan(tmp_path):
     out = r.stdout + r.stderr
     assert r.returncode == 0, out[-3000:]
     assert "AddressSanitizer" not in out and "runtime error" not in out and "LeakSanitizer" not in out, out[-3000:]
-    assert f"plans built under ASan/UBSan: {12 * len(cases)}" in out
+    assert f"plans built under ASan/UBSan: {14 * len(cases)}" in out
