@@ -847,18 +847,34 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             xt = jq == 0 ? st : (jq == 1 ? s1 : (jq == 2 ? s2 : s3));
             xn = jq == 0 ? s1 : (jq == 1 ? s2 : (jq == 2 ? s3 : xb));
         }
-        T g1 = T(0), h1 = T(0), c1 = T(0);
-        if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
-#pragma unroll 2
-        for (int jj = mmax - 1; jj >= 0; --jj) {
-            const int j = jj - dl;                          // the lane's own step: the same residue shift as in P1
-            if ((unsigned)j < (unsigned)m) {
-                T g2 = T(0), h2 = T(0), c2 = T(0);
-                if (j > 0) { const int i2 = p0 + j - 1; g2 = sd[i2]; h2 = su[i2]; c2 = sb[i2]; }
-                xn = fnma<T>(g1, xn, fnma<T>(h1, xt, c1));       // one FMA on the dependent chain
-                sb[p0 + j] = xn;
-                g1 = g2; h1 = h2; c1 = c2;
+        // The walk, on 32-bit shared addresses like P1: the lane's step j (its piece's element p0 + j) runs from
+        // m - 1 down to 0 while the warp's counter runs from mmax - 1 down to 0 (j = counter - dl: the same residue
+        // shift as in P1).  Unrolled by two with two register sets that swap roles (no register rotation); the
+        // pointers move once per double step, the half steps use constant offsets.  A step costs what the warp
+        // issues for it (a lone warp: about 5 cycles per instruction), so the loop is kept to the loads of the next
+        // element, two FMAs (one on the dependent chain) and the store.
+        {
+            const uint32_t LW = (uint32_t)L * W;
+            int j = mmax - 1 - dl;
+            // element p0 + j of sd; never dereferenced while j is outside [0, m)
+            uint32_t pg = smem_u32(sd + p0) + (uint32_t)(j * (int)W), ph = pg + LW, pc = pg + 2u * LW;
+            T g1 = T(0), h1 = T(0), c1 = T(0);
+            if (m > 0) { const int i = p0 + m - 1; g1 = sd[i]; h1 = su[i]; c1 = sb[i]; }
+            T g2 = g1, h2 = h1, c2 = c1;                    // a lane's first step may fall on either half of the loop body
+#define HINES_P3_STEP(G1, H1, C1, G2, H2, C2, OFF)                                                                  \
+            if ((unsigned)j < (unsigned)m) {                                                                        \
+                if (j > 0) { G2 = lds1<T>(pg - (OFF + 1u) * W); H2 = lds1<T>(ph - (OFF + 1u) * W); C2 = lds1<T>(pc - (OFF + 1u) * W); } \
+                xn = fnma<T>(G1, xn, fnma<T>(H1, xt, C1));                                                           \
+                sts1<T>(pc - OFF * W, xn);                                                                           \
+            }                                                                                                       \
+            --j;
+#pragma unroll 1
+            for (int s2 = 0; s2 < mmax; s2 += 2) {
+                HINES_P3_STEP(g1, h1, c1, g2, h2, c2, 0u)
+                HINES_P3_STEP(g2, h2, c2, g1, h1, c1, 1u)
+                pg -= 2u * W; ph -= 2u * W; pc -= 2u * W;
             }
+#undef HINES_P3_STEP
         }
     }
 
