@@ -595,24 +595,26 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             // The sweep proper, on 32-bit shared addresses: node i at pa (d), pa + LW (u), pa + 2 LW (b); the
             // loop is unrolled by two with the two register sets swapping roles (no register rotation).
             const uint32_t LW = (uint32_t)L * W;
-            uint32_t pa = smem_u32(sd + i), pu = pa + LW, pb = pa + 2u * LW;
+            // element i + sl of sd (sl = the warp's step - dl); the pointers move once per double step for every lane,
+            // the half steps use constant offsets; nothing is dereferenced while sl is outside [0, m)
+            uint32_t pa = smem_u32(sd + i) - (uint32_t)dl * W, pu = pa + LW, pb = pa + 2u * LW;
             T un2 = un, dn2 = dn, bn2 = bn;                 // a lane's first step may fall on either half of the loop body
-#define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2)                                                     \
+#define HINES_P1_STEP(UN, DN, BN, UN2, DN2, BN2, OFF)                                                \
             if ((unsigned)sl < (unsigned)m) {                                                        \
-                if (sl + 1 < m) { UN2 = lds1<T>(pu + 2u * W); DN2 = lds1<T>(pa + 2u * W); if (MODE == kModeSolve) BN2 = lds1<T>(pb + 2u * W); } \
+                if (sl + 1 < m) { UN2 = lds1<T>(pu + (OFF + 2u) * W); DN2 = lds1<T>(pa + (OFF + 2u) * W); if (MODE == kModeSolve) BN2 = lds1<T>(pb + (OFF + 2u) * W); } \
                 const T r = rcp<T>(D);                                                               \
                 const T g = UN * r, h = ee * r, c = B * r;                                           \
-                sts1<T>(pa, g); sts1<T>(pu, h); sts1<T>(pb, MODE == kModeFactor ? r : c);            \
+                sts1<T>(pa + OFF * W, g); sts1<T>(pu + OFF * W, h); sts1<T>(pb + OFF * W, MODE == kModeFactor ? r : c); \
                 ddt = fmad<T>(h, ee, ddt); dbt = fmad<T>(h, B, dbt);                                 \
                 D = fnma<T>(g, UN, DN); B = fnma<T>(g, B, BN); ee = -h * UN;                         \
-                pa += W; pu += W; pb += W;                                                           \
             }                                                                                        \
             ++sl;
             int sl = -dl;
 #pragma unroll 1
             for (int s = 0; s < mmax; s += 2) {
-                HINES_P1_STEP(un, dn, bn, un2, dn2, bn2)
-                HINES_P1_STEP(un2, dn2, bn2, un, dn, bn)
+                HINES_P1_STEP(un, dn, bn, un2, dn2, bn2, 0u)
+                HINES_P1_STEP(un2, dn2, bn2, un, dn, bn, 1u)
+                pa += 2u * W; pu += 2u * W; pb += 2u * W;
             }
 #undef HINES_P1_STEP
             i += m;
