@@ -53,7 +53,8 @@ static const int64_t kSmemMaxOptin = 232448;    // 227 KiB
 static const int kSlotNum[] = {1, 3, 2, 1, 1, 1, 1, 1};
 static const int kSlotDen[] = {1, 4, 3, 2, 3, 4, 6, 8};
 static const int kNumClassK = 8;
-static const int kRegsPerThread = 80;           // the resident kernel is built for __launch_bounds__(384, 2): up to 85
+static const int kRegsPerThread = 80;           // fp64 instantiations of the resident kernel use 63-76 registers (allocated in eights)
+static const int kRegsPerThreadF32 = 64;        // fp32 instantiations: 54-60
 static const int kMaxThreads = 768;
 static const int kMaxClusterClass = 16;
 static const int32_t kSegA = 1, kSegB = 2;          // segment lane kinds (descriptor word 1, bits 24-25)
@@ -1042,7 +1043,7 @@ static void assign_classes(hines_plan& P, const std::vector<ItemNeed>& need)
         P.class_phase.push_back(c.phase);
         P.class_quads.push_back(quads_any[q]);
         const int64_t per_sm = std::max<int64_t>(1, kSmemPerSM / (smem + 1024));
-        int64_t tmax = 65536 / (kRegsPerThread * per_sm) / 32 * 32;
+        int64_t tmax = 65536 / ((P.width == 4 ? kRegsPerThreadF32 : kRegsPerThread) * per_sm) / 32 * 32;
         tmax = std::max<int64_t>(64, std::min<int64_t>(kMaxThreads, tmax));
         int64_t t = P.opt.threads_per_block ? P.opt.threads_per_block : round_up(std::max(lanes_max[q], 1), 32);
         t = std::max<int64_t>(P.opt.threads_per_block ? 32 : std::min<int64_t>(128, tmax), std::min(t, tmax));

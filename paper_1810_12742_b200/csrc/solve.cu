@@ -514,7 +514,9 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
     }
     if (tid < 2) nd[6 * H.nnode + 4 + tid] = T(0);          // the all-zero record: hand-off slot of a child that is not there
-    mbar_wait(bar, 0);
+    // ONE warp polls the mbarrier, the others wait at the block barrier: a polling warp takes issue slots from the
+    // working warps of the blocks beside it, a warp at a barrier does not
+    if (tid < 32) mbar_wait(bar, 0);
     __syncthreads();
     HINES_STAMP(1);
     const unsigned FULL = 0xffffffffu;
@@ -688,7 +690,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     // ---- hand-off values of the sub-trees held by other blocks, into the ghost children; then
     //      the top nodes (the ancestors of the ghost children) ----
     if (CL) {
-        if (rank == 0) { cluster_wait(); mbar_wait_cluster(bar + 1, 0); }      // every ghost child has its hand-off
+        if (rank == 0) { cluster_wait(); if (tid < 32) mbar_wait_cluster(bar + 1, 0); __syncthreads(); }      // every ghost child has its hand-off (one warp polls)
     } else if (phase == kPhaseB) {
         pdl_wait();                                         // phase A has completed: the hand-off values are there
         for (int e = tid; e < nghost; e += nthreads) {
@@ -747,7 +749,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
 #pragma unroll 1
     for (int r = 0; r < rounds; ++r) {
         if (sub && r == nrounds) {
-            if (CL) mbar_wait_cluster(bar + 1, 0);          // rank 0 has sent every x this part waits for (behind the export's entry)
+            if (CL) { if (tid < 32) mbar_wait_cluster(bar + 1, 0); __syncthreads(); }     // rank 0 has sent every x this part waits for (behind the export's entry); one warp polls
             else pdl_wait();                                // phase B has completed: the parents' x is in the exchange buffer
             const int cur = 2 * (r & 1);
             for (int e = tid; e < nexp; e += nthreads) {
