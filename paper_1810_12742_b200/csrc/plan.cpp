@@ -446,7 +446,7 @@ static void build_item(const hines_plan& P, const std::vector<int64_t>& cells, i
                 if (cnt[v] > 4095) { out.ok = false; return; }
                 pb.kp[4 * v] = cnt[v] > 0 ? first[v] : -1;             // node index for now, byte offset below
                 pb.kp[4 * v + 1] = cnt[v] > 1 ? first[v] + 1 : -1;
-                pb.kp[4 * v + 2] = cnt[v];
+                pb.kp[4 * v + 2] = cnt[v] | (cnt[v] > 2 ? 1 << 28 : 0);    // bit 28: more than two children (the sweep's rare loop)
                 if (nt.pkey >= 0) pn = nt.pkey;
                 else if (nparent[nt.gid] >= 0) {                               // exported sub-tree root: its parent is a ghost
                     const int32_t b = nbr[nt.gid];

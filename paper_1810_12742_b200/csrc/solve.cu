@@ -262,10 +262,10 @@ __device__ __forceinline__ void node_step(uint32_t nd_sa, uint32_t qa, const int
     const V2 h0 = lds2<T>(nd_sa + (uint32_t)k.x), h1 = lds2<T>(nd_sa + (uint32_t)k.y);
     T D = a0.x - h0.x, B = a0.y - h0.y;
     D -= h1.x; B -= h1.y;
-    int nc = k.z & 0xfff;
-    if (nc > 2) {                                           // more than two children: the rest, consecutive records
+    if (k.z & (1 << 28)) {                                  // more than two children (rare): the rest, consecutive records
         uint32_t ca = nd_sa + (uint32_t)k.y + RS;
-        for (nc -= 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
+#pragma unroll 1
+        for (int nc = (k.z & 0xfff) - 2; nc > 0; --nc, ca += RS) { const V2 h = lds2<T>(ca); D -= h.x; B -= h.y; }
     }
     if (MODE == 2) {
         const T r = lds1<T>(qa + 3u * W);
@@ -321,29 +321,29 @@ __device__ __forceinline__ void sweep_backward(uint32_t nd_sa, uint32_t lb_sa, u
         const int pthreads = (maxwidth + 31) & ~31;
         tid = nthreads - 1 - tid;                           // the LAST warps of the block sweep: P1 / P3 fill the first ones
         if (tid < pthreads) {
+            // the thread's node on a level: index lb[l] + tid, if that is below lb[l + 1].  Whether the node takes part in
+            // this sweep is read off its info word (bit 31: a ghost child, bit 29: a top node) when the step comes;
+            // a thread without a node on the level carries the word of a ghost.
+            const int want = topsel << 29;
             int lo = ldsi1(lb_sa + 4u * (uint32_t)lfrom), hi = ldsi1(lb_sa + 4u * (uint32_t)(lfrom + 1));
             int lo_n = lfrom > lto ? ldsi1(lb_sa + 4u * (uint32_t)(lfrom - 1)) : 0;
+            uint32_t lbp = lb_sa + 4u * (uint32_t)(lfrom - 2);        // lb[l - 2] of the level in hand
             int v = lo + tid;
-            int4 k = make_int4(0, 0, -1, 0);
+            int4 k = make_int4(0, 0, (int)0x80000000, 0);
             V2 a0, a2; T Un = T(0);
             a0.x = T(1); a0.y = T(0); a2.x = T(0); a2.y = T(0);
             uint32_t qa = nd_sa + (uint32_t)v * RS;
-            bool have = false;
-            if (v < hi) {
-                k = ldsi4(kp_sa + 16u * (uint32_t)v); a0 = lds2<T>(qa); Un = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
-                have = k.z >= 0 && ((k.z >> 29) & 1) == topsel;
-            }
+            if (v < hi) { k = ldsi4(kp_sa + 16u * (uint32_t)v); a0 = lds2<T>(qa); Un = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W); }
 #pragma unroll 1
-            for (int l = lfrom; l >= lto; --l) {
-                const int lo_nn = l > lto + 1 ? ldsi1(lb_sa + 4u * (uint32_t)(l - 2)) : 0;     // two levels ahead: off the chain
-                if (have) node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
+            for (int n = lfrom - lto; n >= 0; --n, lbp -= 4u) {
+                const int lo_nn = n > 1 ? ldsi1(lbp) : 0;             // two levels ahead: off the chain
+                if (((k.z ^ want) & (int)0xA0000000) == 0) node_step<T, MODE>(nd_sa, qa, k, a0, Un, a2);
                 hi = lo; lo = lo_n; lo_n = lo_nn;
                 v = lo + tid;
                 qa = nd_sa + (uint32_t)v * RS;
-                have = false;
-                if (l > lto && v < hi) {                    // this thread's node on the next level: lands while the barrier is pending
+                k.z = (int)0x80000000;
+                if (n > 0 && v < hi) {                      // this thread's node on the next level: lands while the barrier is pending
                     k = ldsi4(kp_sa + 16u * (uint32_t)v); a0 = lds2<T>(qa); Un = lds1<T>(qa + 2u * W); a2 = lds2<T>(qa + 4u * W);
-                    have = k.z >= 0 && ((k.z >> 29) & 1) == topsel;
                 }
                 named_barrier(pthreads);
             }
