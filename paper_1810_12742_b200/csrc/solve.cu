@@ -495,6 +495,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         // lanes 0-2, so that the copies of a part with many runs are issued by all warps side by side)
         const int64_t gemax = n_total / E * E;
         const int nwarps = nthreads >> 5, warp = tid >> 5;
+#pragma unroll 1
         for (int r = warp; r < nrun; r += nwarps) {
             const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
             const int64_t g = rd.x, gend = g + rd.y;
@@ -693,6 +694,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         if (rank == 0) { cluster_wait(); if (tid < 32) mbar_wait_cluster(bar + 1, 0); __syncthreads(); }      // every ghost child has its hand-off (one warp polls)
     } else if (phase == kPhaseB) {
         pdl_wait();                                         // phase A has completed: the hand-off values are there
+#pragma unroll 1
         for (int e = tid; e < nghost; e += nthreads) {
             const int4 g = gh[e];
             *reinterpret_cast<V2*>(nd + 6 * g.x + 4) = reinterpret_cast<const V2*>(xch_h)[H.xch_base + g.y];
@@ -710,6 +712,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         if (rank != 0) {
             const uint32_t bar0 = mapa_u32(smem_u32(bar + 1), 0), nd0a = mapa_u32(nd_sa, 0);
             cluster_wait();                                 // barrier 0: rank 0 is running, its mbarrier initialised
+#pragma unroll 1
             for (int e = tid; e < nexp; e += nthreads) {
                 const int4 q = ex[e];
                 const V2 hv = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
@@ -718,6 +721,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             }
         }
     } else if (phase == kPhaseA) {
+#pragma unroll 1
         for (int e = tid; e < nexp; e += nthreads) {
             const int4 q = ex[e];
             reinterpret_cast<V2*>(xch_h)[H.xch_base + q.z] = *reinterpret_cast<const V2*>(nd + 6 * q.x + 4);
@@ -730,6 +734,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         }
         if (MODE != kModeFactor) return;
     } else if (phase == kPhaseC) {
+#pragma unroll 1
         for (int e = tid; e < nexp; e += nthreads) { const int4 q = ex[e]; nd[6 * q.y] = T(1); nd[6 * q.y + 1] = T(0); }
     }
     // ---- P2 forward: first the top nodes, level by level (the other parts of the cell wait
@@ -752,6 +757,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             if (CL) { if (tid < 32) mbar_wait_cluster(bar + 1, 0); __syncthreads(); }     // rank 0 has sent every x this part waits for (behind the export's entry); one warp polls
             else pdl_wait();                                // phase B has completed: the parents' x is in the exchange buffer
             const int cur = 2 * (r & 1);
+#pragma unroll 1
             for (int e = tid; e < nexp; e += nthreads) {
                 const int4 q = ex[e];
                 nd[6 * q.y + cur] = T(0);
@@ -777,6 +783,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     if (CL) {
         if (rank == 0 && MODE != kModeFactor) {             // x of the top nodes goes to the roots that wait for it
             const uint32_t bar1 = smem_u32(bar + 1), base = smem_u32(smem);
+#pragma unroll 1
             for (int e = tid; e < nghost; e += nthreads) {
                 const int4 g = gh[e];                       // {ghost child, -, parent, rank << 20 | landing word in that block}
                 const uint32_t r = (uint32_t)g.w >> 20, word = (uint32_t)g.w & 0xfffffu;
@@ -784,6 +791,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             }
         }
     } else if (phase == kPhaseB && MODE != kModeFactor) {
+#pragma unroll 1
         for (int e = tid; e < nghost; e += nthreads) {
             const int4 g = gh[e];
             xch_x[H.xch_base + g.y] = nd[6 * g.z + xs_now];
@@ -798,6 +806,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     if (MODE == kModeFactor) {
         // the separators' factors go where their compartments are: g = -f, -U, r = 1 / pivot
         __syncthreads();
+#pragma unroll 1
         for (int v = tid; v < H.nlevnode; v += nthreads) {
             const T* q = nd + 6 * v;
             if (reinterpret_cast<const int4*>(meta + H.kp_off)[v].z < 0) continue;       // a ghost child has no compartment here
@@ -886,6 +895,7 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     fence_proxy_async();
     __syncthreads();
     HINES_STAMP(5);
+#pragma unroll 1
     for (int r = tid >> 5; r < nrun; r += nthreads >> 5) {
         const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
         const int64_t g = rd.x;
