@@ -836,7 +836,19 @@ static void emit_item(hines_plan& P, const std::vector<int64_t>& cells, const It
         h.run_off = (int32_t)(P.part_runs.size() / 4);
         h.nrun = (int32_t)(pb.runs.size() / 4);
         for (int32_t k = 0; k < h.nrun; ++k)
-            P.part_runs.insert(P.part_runs.end(), {(int32_t)(ib.comp_begin + pb.runs[4 * k]), pb.runs[4 * k + 1], pb.runs[4 * k + 2], 0});
+        {
+            // {global first compartment, length, staged index, w}: w spares the loader and the store their index
+            // arithmetic: bits 0-15 the elements the bulk copy brings (the run widened to 16-byte words, clipped at the
+            // end of the arrays), bits 16-19 the elements in front of the first whole word of the run (stored by hand),
+            // bits 20-23 the elements behind its last whole word, bit 24: elements beyond the arrays' last whole word
+            // (loaded by hand)
+            const int64_t g = ib.comp_begin + pb.runs[4 * k], len = pb.runs[4 * k + 1], E = 16 / P.width;
+            const int64_t ga = g - g % E, ge = std::min<int64_t>(round_up(g + len, E), P.n / E * E);
+            const int64_t cnt = std::max<int64_t>(0, ge - ga);
+            const int64_t head = std::min<int64_t>(len, (E - g % E) % E), tail = std::max<int64_t>(head, (g + len) / E * E - g);
+            const int32_t wd = (int32_t)(cnt | (head << 16) | ((len - tail) << 20) | ((int64_t)(g + len > ge) << 24));
+            P.part_runs.insert(P.part_runs.end(), {(int32_t)g, (int32_t)len, pb.runs[4 * k + 2], wd});
+        }
         h.tx_elems = pb.tx_elems; h.L = pb.L; h.n = pb.n;
         h.nnode = pb.nnode; h.nlevnode = pb.nlevnode; h.nlev = pb.nlev; h.rounds = pb.rounds;
         h.nexp = pb.nexp; h.nghost = pb.nghost; h.nseg_lanes = pb.nlanes;

@@ -106,6 +106,11 @@ __device__ __forceinline__ void tma_load_1d(void* dst_smem, const void* src_gmem
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst_smem)), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
+__device__ __forceinline__ void tma_load_1d_sa(uint32_t dst_sa, const void* src_gmem, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_sa), "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
 // shared -> global bulk copy (bulk async-group completion)
 __device__ __forceinline__ void tma_store_1d(void* dst_gmem, const void* src_smem, uint32_t bytes)
 {
@@ -493,24 +498,25 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         // and are ignored); words beyond the end of the arrays are not touched: that remainder by plain loads
         // (a bulk-copy instruction costs its warp ~70 cycles per active lane: one run per warp, its three arrays by
         // lanes 0-2, so that the copies of a part with many runs are issued by all warps side by side)
-        const int64_t gemax = n_total / E * E;
+        // The lane's array is chosen once (solve: d, b, u; factor: d, u; right-hand side: f0, b, f1, f2); per run the plan
+        // has the index arithmetic done (word 3 of the run: elements the copy brings, a flag for elements beyond the
+        // arrays' last whole 16-byte word): the loop is a handful of instructions in front of each bulk copy.
         const int nwarps = nthreads >> 5, warp = tid >> 5;
+        const T* src = nullptr; T* dst = nullptr;
+        if (MODE == kModeSolve) { src = lane == 0 ? d : (lane == 1 ? b : (lane == 2 ? u : nullptr)); dst = lane == 0 ? sd : (lane == 1 ? sb : su); }
+        if (MODE == kModeFactor) { src = lane == 0 ? d : (lane == 2 ? u : nullptr); dst = lane == 0 ? sd : su; }
+        if (MODE == kModeRhs) { src = lane == 0 ? f0 : (lane == 1 ? b : (lane == 2 ? f1 : (lane == 3 ? f2 : nullptr))); dst = lane == 0 ? sd : (lane == 1 ? sb : (lane == 2 ? su : sr)); }
+        if (src != nullptr) {
+            const uint32_t dst_sa = smem_u32(dst);
 #pragma unroll 1
-        for (int r = warp; r < nrun; r += nwarps) {
-            const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
-            const int64_t g = rd.x, gend = g + rd.y;
-            const int64_t ga = g & ~(int64_t)(E - 1);
-            int64_t ge = (gend + E - 1) / E * E;
-            if (ge > gemax) ge = gemax;
-            const int sdst = rd.z - (int)(g - ga);
-            // lanes 0-3: the arrays this mode stages (solve: d, b, u; factor: d, u; right-hand side: f0, b, f1, f2)
-            const T* src = nullptr; T* dst = nullptr;
-            if (MODE == kModeSolve) { src = lane == 0 ? d : (lane == 1 ? b : (lane == 2 ? u : nullptr)); dst = lane == 0 ? sd : (lane == 1 ? sb : su); }
-            if (MODE == kModeFactor) { src = lane == 0 ? d : (lane == 2 ? u : nullptr); dst = lane == 0 ? sd : su; }
-            if (MODE == kModeRhs) { src = lane == 0 ? f0 : (lane == 1 ? b : (lane == 2 ? f1 : (lane == 3 ? f2 : nullptr))); dst = lane == 0 ? sd : (lane == 1 ? sb : (lane == 2 ? su : sr)); }
-            if (src != nullptr) {
-                if (ge > ga) tma_load_1d(dst + sdst, src + ga, (uint32_t)(ge - ga) * W, bar);
-                for (int64_t i = ge > ga ? ge : ga; i < gend; ++i) dst[sdst + (int)(i - ga)] = src[i];    // words beyond the arrays' end
+            for (int r = warp; r < nrun; r += nwarps) {
+                const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
+                const int ga = rd.x & ~(E - 1);                        // N < 2^31 (hines_plan_create)
+                const int sdst = rd.z - (rd.x - ga);
+                const uint32_t cnt = (uint32_t)rd.w & 0xffffu;
+                if (cnt) tma_load_1d_sa(dst_sa + (uint32_t)sdst * W, src + ga, cnt * W, bar);
+                if (rd.w & (1 << 24))                                  // the elements beyond the arrays' last whole word
+                    for (int i = ga + (int)cnt; i < rd.x + rd.y; ++i) dst[sdst + (i - ga)] = src[i];
             }
         }
     }
@@ -898,10 +904,8 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
 #pragma unroll 1
     for (int r = tid >> 5; r < nrun; r += nthreads >> 5) {
         const int4 rd = r < kInlineRuns ? myruns[r] : runs_g[H.run_off + r];
-        const int64_t g = rd.x;
-        const int len = rd.y, so = rd.z;
-        const int head = min(len, (int)((E - (g & (E - 1))) & (E - 1)));                 // run-local [0, head)
-        const int tail = max(head, (int)(((g + len) & ~(int64_t)(E - 1)) - g));          // run-local [tail, len)
+        const int g = rd.x, len = rd.y, so = rd.z;                                       // N < 2^31 (hines_plan_create)
+        const int head = (rd.w >> 16) & 15, tail = len - ((rd.w >> 20) & 15);            // run-local [0, head) and [tail, len): by hand
 #pragma unroll
         for (int a = 0; a < (MODE == kModeFactor ? 3 : 1); ++a) {                        // x, or the three factor arrays
             T* dstg = MODE == kModeFactor ? (a == 0 ? f0 : (a == 1 ? f1 : f2)) : x;

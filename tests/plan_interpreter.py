@@ -122,12 +122,17 @@ class _PartState:
         self.sd = np.full(L, np.nan); self.su = np.full(L, np.nan); self.sb = np.full(L, np.nan)
         tx = 0
         cursor = 0
-        for g, ln, so, _ in part.runs:
-            g, ln, so = int(g), int(ln), int(so)
+        for g, ln, so, wd in part.runs:
+            g, ln, so, wd = int(g), int(ln), int(so), int(wd)
             assert ln > 0 and so % E == g % E and so >= cursor and so + ln <= L, "run staged at the parity of its global index"
             cursor = so + ln
             ga, ge = g - g % E, min(-(-(g + ln) // E) * E, n_total // E * E)
             tx += max(0, ge - ga)
+            # word 3: what the loader and the store would otherwise compute per run
+            head = min(ln, (E - g % E) % E)
+            tail = max(head, (g + ln) // E * E - g)
+            assert wd & 0xffff == max(0, ge - ga) and (wd >> 16) & 15 == head and (wd >> 20) & 15 == ln - tail
+            assert (wd >> 24) == (1 if g + ln > ge else 0)
             self.sd[so:so + ln] = d[g:g + ln]; self.su[so:so + ln] = u[g:g + ln]; self.sb[so:so + ln] = b[g:g + ln]
         assert tx == h["tx_elems"] and L % E == 0 and sum(int(r[1]) for r in part.runs) == h["n"]
         nn = h["nnode"]
