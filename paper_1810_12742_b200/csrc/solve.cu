@@ -492,7 +492,9 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
         mbar_expect_tx(bar, (uint32_t)NARR * (uint32_t)H.tx_elems * W + (uint32_t)H.meta_len * 4u);
         tma_load_1d(meta, meta_g + H.meta_off, (uint32_t)H.meta_len * 4u, bar);
     }
-    __syncthreads();                                        // the expected byte count is set before any copy can complete
+    // No barrier between the expect-tx and the copies of the other warps: a copy that completes first takes the
+    // barrier's tx-count below zero for a moment, which is allowed; the phase cannot complete before thread 0's
+    // arrive.expect_tx, the only arrival the barrier waits for.
     {
         // a run [g, g+len) is brought as the 16-byte words that cover it (neighbouring compartments come along
         // and are ignored); words beyond the end of the arrays are not touched: that remainder by plain loads
