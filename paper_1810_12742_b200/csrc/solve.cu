@@ -185,6 +185,7 @@ template <> __device__ __forceinline__ void sts1<double>(uint32_t a, double v)
 { asm volatile("st.shared.f64 [%0], %1;" ::"r"(a), "d"(v) : "memory"); }
 template <> __device__ __forceinline__ void sts1<float>(uint32_t a, float v)
 { asm volatile("st.shared.f32 [%0], %1;" ::"r"(a), "f"(v) : "memory"); }
+__device__ __forceinline__ void stsi1(uint32_t a, int v) { asm volatile("st.shared.s32 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 template <typename T> __device__ __forceinline__ void sts2(uint32_t a, typename Vec2<T>::type v);
 template <> __device__ __forceinline__ void sts2<double>(uint32_t a, double2 v)
 { asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(a), "d"(v.x), "d"(v.y) : "memory"); }
@@ -759,6 +760,12 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
     if (sub) __syncthreads();                               // the ghost parents' identity records
     const int nrounds = rounds;
     if (sub) ++rounds;                                      // the round after x has arrived
+    constexpr uint32_t RSB = 6u * W;                        // bytes per node record
+    const bool one_node = nnode <= nthreads;
+    const uint32_t my_qa = nd_sa + (uint32_t)tid * RSB;
+    V2 my_gc; my_gc.x = T(0); my_gc.y = T(0);
+    int my_p = 0;
+    if (one_node && rounds > 0 && tid < nnode) { my_gc = lds2<T>(my_qa); my_p = ldsi1(kp_sa + 16u * (uint32_t)tid + 12u); }
 #pragma unroll 1
     for (int r = 0; r < rounds; ++r) {
         if (sub && r == nrounds) {
@@ -774,6 +781,21 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             __syncthreads();
         }
         const int sbuf = 2 * (r & 1), dbuf = 2 - sbuf;
+        if (one_node) {
+            // one node per thread: its (g, c) and parent stay in registers over the rounds; a round is the parent's
+            // (g, c) and parent from shared memory, two fp operations and the thread's own two stores
+            if (tid < nnode) {
+                const uint32_t pa = nd_sa + (uint32_t)my_p * RSB;
+                const V2 ap = lds2<T>(pa + (uint32_t)sbuf * W);
+                const int pp = r == 0 ? ldsi1(kp_sa + 16u * (uint32_t)my_p + 12u) : ldsi1(pa + 4u * W + 4u * (uint32_t)((r - 1) & 1));
+                V2 o; o.x = my_gc.x * ap.x; o.y = fmad<T>(my_gc.x, ap.y, my_gc.y);
+                sts2<T>(my_qa + (uint32_t)dbuf * W, o);
+                stsi1(my_qa + 4u * W + 4u * (uint32_t)(r & 1), pp);
+                my_gc = o; my_p = pp;
+            }
+            __syncthreads();
+            continue;
+        }
 #pragma unroll 1
         for (int v = tid; v < nnode; v += nthreads) {
             int* ip = reinterpret_cast<int*>(nd + 6 * v + 4);
