@@ -553,17 +553,28 @@ hines_resident_kernel(const BlockRecord* __restrict__ recs, const int32_t* __res
             if (kind == 1 || kind == 3 || (isB && hasq)) B = sb[i];
             T g1 = T(0), h1 = T(0), r1 = T(0), b1 = T(0);
             if (m > 0) { g1 = sd[i]; h1 = su[i]; r1 = sr[i]; b1 = sb[i + 1]; }
-            for (int s = 0; s < mmax; ++s) {
-                const int sl = s - dl;
-                if ((unsigned)sl < (unsigned)m) {
-                    T g2 = T(0), h2 = T(0), r2 = T(0), b2 = T(0);
-                    if (sl + 1 < m) { g2 = sd[i + 1]; h2 = su[i + 1]; r2 = sr[i + 1]; b2 = sb[i + 2]; }
-                    sb[i] = B * r1;
-                    dbt = fmad<T>(h1, B, dbt);
-                    B = fnma<T>(g1, B, b1);
-                    g1 = g2; h1 = h2; r1 = r2; b1 = b2;
-                    ++i;
+            {
+                // the walk on shared addresses, two register sets, pointers moved once per double step (as in the solve path)
+                const uint32_t LW = (uint32_t)L * W;
+                uint32_t pg = smem_u32(sd + i) - (uint32_t)dl * W, ph = pg + LW, pc = pg + 2u * LW, pr = pg + 3u * LW;
+                T g2 = g1, h2 = h1, r2 = r1, b2 = b1;       // a lane's first step may fall on either half of the loop body
+                int sl = -dl;
+#define HINES_P1R_STEP(G1, H1, R1, B1, G2, H2, R2, B2, OFF)                                              \
+                if ((unsigned)sl < (unsigned)m) {                                                        \
+                    if (sl + 1 < m) { G2 = lds1<T>(pg + (OFF + 1u) * W); H2 = lds1<T>(ph + (OFF + 1u) * W); R2 = lds1<T>(pr + (OFF + 1u) * W); B2 = lds1<T>(pc + (OFF + 2u) * W); } \
+                    sts1<T>(pc + OFF * W, B * R1);                                                       \
+                    dbt = fmad<T>(H1, B, dbt);                                                           \
+                    B = fnma<T>(G1, B, B1);                                                              \
+                }                                                                                        \
+                ++sl;
+#pragma unroll 1
+                for (int s = 0; s < mmax; s += 2) {
+                    HINES_P1R_STEP(g1, h1, r1, b1, g2, h2, r2, b2, 0u)
+                    HINES_P1R_STEP(g2, h2, r2, b2, g1, h1, r1, b1, 1u)
+                    pg += 2u * W; ph += 2u * W; pc += 2u * W; pr += 2u * W;
                 }
+#undef HINES_P1R_STEP
+                i += m;
             }
             const bool lead = quad ? (kind == 3 && jq == 0) : (kind == 1);
             const int stride = quad ? 8 : 16, nq = quad ? 3 : 1;
