@@ -105,10 +105,11 @@ typedef struct {
                                        long ("we split branches that are too long")               */
     int32_t cluster_max;            /* 0 = default (8), 1..16: largest thread-block cluster a cell may be spread
                                        over (more than 8 needs the non-portable cluster size)                  */
-    int32_t chunk_smem_bytes;       /* 0 = default (227 KiB: a cell that fits one block's shared memory stays in one
-                                       block; measured optimum of configs 2 and 3): the size above which a cell is
-                                       cut into the parts of a cluster; the parts aim at 1/2, 1/3 or 1/4 of an SM's
-                                       shared memory, whichever they fill best, but never more than this           */
+    int32_t chunk_smem_bytes;       /* 0 = default (117 KiB, half an SM's shared memory: two blocks per SM overlap each
+                                       other's phases; measured optimum of configs 2 and 3, +2 % over 227 KiB): the
+                                       size above which a cell is cut into the parts of a cluster; the parts aim at
+                                       1/2, 1/3 or 1/4 of an SM's shared memory, whichever they fill best, but never
+                                       more than this                                                              */
     int32_t split_smem_bytes;       /* 0 = default (113 KiB): shared memory of one sub-tree part of a split item
                                        (a cell beyond the largest cluster, run as three dependent launches)     */
 } hines_options_t;

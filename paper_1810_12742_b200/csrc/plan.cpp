@@ -1173,7 +1173,7 @@ hines_status_t hines_plan_create(const int32_t* parent, const int64_t* cell_offs
     const bool auto_segment = o.max_segment == 0;     // default: 40 in a block of its own, 64 in the blocks of a cluster
     if (auto_segment) o.max_segment = 64;
     if (o.cluster_max == 0) o.cluster_max = 8;
-    if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = (int32_t)kSmemMaxOptin;
+    if (o.chunk_smem_bytes == 0) o.chunk_smem_bytes = 117 * 1024;       // half an SM: two blocks per SM overlap each other's phases (measured optimum)
     if (o.split_smem_bytes == 0) o.split_smem_bytes = 113 * 1024;
     if (o.threads_per_block < 0 || o.threads_per_block > kMaxThreads || o.threads_per_block % 32 ||
         o.stream_threads < 32 || o.stream_threads > 1024 || o.stream_threads % 32 ||
