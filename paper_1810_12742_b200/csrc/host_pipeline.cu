@@ -64,18 +64,20 @@ hines_status_t setup_device(hines_host_pipeline* P)
         hines::set_error("no CUDA device: this library has no CPU fallback");
         return HINES_ERR_CUDA;
     }
-    PIPE_TRY(cudaGetDevice(&P->device));
+    // every resource is created once: a call that failed half way is picked up where it stopped by the next one, and the
+    // pipeline counts as set up (device >= 0) only when everything is there
+    int dev = -1;
+    PIPE_TRY(cudaGetDevice(&dev));
     int64_t total = 0;
     for (auto& s : P->slices) { s.off = total; total += (s.len + 31) / 32 * 32; }
-    for (void*& p : P->dev) PIPE_TRY(cudaMalloc(&p, (size_t)total * P->width));
-    PIPE_TRY(cudaStreamCreateWithFlags(&P->s_in, cudaStreamNonBlocking));
-    PIPE_TRY(cudaStreamCreateWithFlags(&P->s_solve, cudaStreamNonBlocking));
-    PIPE_TRY(cudaStreamCreateWithFlags(&P->s_out, cudaStreamNonBlocking));
+    for (void*& p : P->dev) if (!p) PIPE_TRY(cudaMalloc(&p, (size_t)total * P->width));
+    for (cudaStream_t* st : {&P->s_in, &P->s_solve, &P->s_out}) if (!*st) PIPE_TRY(cudaStreamCreateWithFlags(st, cudaStreamNonBlocking));
     for (auto& s : P->slices) {
-        PIPE_TRY(cudaEventCreateWithFlags(&s.in, cudaEventDisableTiming));
-        PIPE_TRY(cudaEventCreateWithFlags(&s.out, cudaEventDisableTiming));
+        if (!s.in) PIPE_TRY(cudaEventCreateWithFlags(&s.in, cudaEventDisableTiming));
+        if (!s.out) PIPE_TRY(cudaEventCreateWithFlags(&s.out, cudaEventDisableTiming));
         if (hines_status_t st = hines_plan_upload(s.plan)) return st;
     }
+    P->device = dev;
     return HINES_OK;
 }
 
